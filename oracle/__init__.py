@@ -1,0 +1,25 @@
+"""CPU oracle — TEST INFRASTRUCTURE ONLY (see bs_oracle.c header).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import this
+package.  It imports nothing from paper_2412_04676_b200.
+"""
+from .bs_oracle import (  # noqa: F401
+    ERR_ARG,
+    ERR_CAPACITY,
+    ERR_CORRUPT,
+    ERR_UNSUPPORTED,
+    OK,
+    OracleError,
+    build,
+    deserialize,
+    emit_header,
+    emit_payload_range,
+    header_bytes,
+    plan,
+    pool_bytes,
+    serialize,
+    serialized_size,
+    stream_info,
+    validate_set,
+    validate_stream,
+)
