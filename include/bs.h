@@ -1,0 +1,229 @@
+/*
+ * bs.h — C ABI of libbsstream: serialize / deserialize / offload / prefetch of symmetry-blocked
+ * (U(1) quantum-number-labelled) block-sparse fp64 matrices and rank-3 tensors on one NVIDIA B200.
+ *
+ * The operations are those of arXiv 2412.04676 (Menczer & Legeza), /root/reference/PAPER.md:
+ *   - §III (L85): saving scratch data = (1) serialization, "generating long continuous stripes in
+ *     memory", (2) transfer to a storage medium; loading = transfer + deserialization.
+ *   - §III.B.2 (L104-108): exact size prediction before serialization; every worker gets an exact,
+ *     disjoint interval of one output buffer; independent parallel fill; the single stream
+ *     "deserializes into an object identical to the one used as the original input".
+ *   - §II.B (L63): blocks travel with their meta data (sector indices, quantum numbers, sector dims).
+ *   - §III.A (L89-92), §III.B.4 (L132-138): segment-wise synchronous IO, asynchronous save / load
+ *     overlapped with computation, with a completion point ("checkpoint") before the data is used.
+ * The paper defines no byte format; "wire format v1" below is this project's.
+ *
+ * Conventions
+ *   - Every function returns int: BS_OK (0), BS_PENDING (1) or a negative BS_ERR_*.
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers (h_pinned: page-locked).  Structs
+ *     passed by pointer (bs_set_desc, bs_opts, bs_engine_cfg, bs_stream_info_t) live on the HOST.
+ *   - Ownership: the caller owns every buffer it passes (descriptor arrays, blocks, stream, pool,
+ *     workspace, pinned host memory) and keeps it alive and unmodified until the stream work / ticket
+ *     of the call has completed.  The library owns only what bs_engine_create allocates.
+ *   - Calls enqueue work on the given cudaStream_t and return without synchronising unless stated.
+ *     Errors detected on the device (capacity, corrupt header, bad descriptor) are DEFERRED: they land
+ *     in bs_result.status (device memory) and, for engine calls, in the ticket.  When status != BS_OK
+ *     no stream / block / descriptor output has been written by the data-movement kernels.
+ *   - The path does no floating-point arithmetic: fp64 values move as opaque 8-byte words; results
+ *     are bit-exact (tolerance 0).
+ *   - Thread-safety: functions are re-entrant; one bs_engine must be driven by one host thread.
+ *   - There is no CPU fallback: without a CUDA device every device-touching call fails with BS_ERR_CUDA.
+ *
+ * Wire format v1 (little-endian, no implicit padding):
+ *   stream  := fixed_header(64) | tensor_rec[T](32 each) | block_rec[B](48 each) | zeros to a multiple
+ *              of 128 | payload(P)
+ *   fixed_header: char magic[8]="BSPARSE1"; u32 version=1; u32 endian_tag=0x01020304; u32 dtype=0;
+ *                 u32 n_qn=2; u32 max_rank=3; u32 align=16; u64 n_tensors; u64 n_blocks;
+ *                 u64 header_bytes; u64 payload_bytes
+ *   tensor_rec  : bs_tensor_rec, byte for byte
+ *   block_rec   : i32 qn[3][2]; u32 dim[3]; u32 tensor; u64 offset
+ *   payload     : block i's 8*prod(dim_i) raw bytes at payload+offset_i, then zeros up to the next
+ *                 multiple of 16; offset_i = sum_{j<i} align16(8*prod(dim_j))   (descriptor order)
+ */
+#ifndef BS_H_
+#define BS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__CUDACC__) || defined(CUDART_VERSION) || defined(__DRIVER_TYPES_H__)
+/* cudaStream_t comes from the CUDA headers */
+#else
+typedef struct CUstream_st *cudaStream_t;
+#endif
+
+#define BS_VERSION 0x00010000u /* library 1.0, wire format v1 */
+
+enum {
+    BS_OK = 0,
+    BS_PENDING = 1,          /* bs_ticket_query: work still in flight */
+    BS_ERR_ARG = -1,         /* NULL / misaligned pointer, bad descriptor partition, size overflow */
+    BS_ERR_CAPACITY = -2,    /* stream / pool / workspace / descriptor arrays too small */
+    BS_ERR_CORRUPT = -3,     /* header validation failed; nothing was written */
+    BS_ERR_UNSUPPORTED = -4, /* rank not in {2,3}, dtype != f64, n_qn != 2 */
+    BS_ERR_CUDA = -5         /* a CUDA runtime call failed; see bs_last_cuda_error() */
+};
+
+enum { BS_F64 = 0 };
+
+/* bs_deserialize / bs_prefetch_async destination layout */
+enum {
+    BS_LAYOUT_POOL = 0,     /* out->addr[i] = d_pool + sum_{j<i} align256(nbytes_j); written by the call */
+    BS_SCATTER_TO_ADDR = 1  /* out->addr[i] and out->dim are INPUTS: caller-chosen destinations; extents
+                               must equal the stream's, else BS_ERR_ARG */
+};
+
+/* One tensor of the set; 32 bytes; identical bytes on the wire (PAPER L63 meta data). */
+typedef struct bs_tensor_rec {
+    uint32_t rank;        /* 2 (operator matrix) or 3 (MPS site tensor, PAPER Eq. 2) */
+    uint32_t first_block; /* index of its first block in the per-block arrays */
+    uint32_t n_blocks;    /* tensors partition the block table in order: first_block[t+1] = first_block[t] + n_blocks[t] */
+    int32_t dq[2];        /* conserved charge (dN, d2Sz): sum_k sign[k]*qn[k] == dq for every block */
+    int8_t sign[4];       /* leg arrows +-1; unused legs 0 */
+    uint32_t tag;         /* opaque user id */
+    uint32_t reserved;    /* 0 */
+} bs_tensor_rec;
+
+/* A set of block-sparse tensors.  HOST struct; every pointer is a DEVICE pointer. */
+typedef struct bs_set_desc {
+    uint32_t n_tensors;     /* T.  For bs_deserialize / bs_prefetch_async outputs: CAPACITY of tensors[] */
+    uint32_t n_blocks;      /* B.  For outputs: CAPACITY of qn / dim / addr */
+    uint32_t n_qn;          /* 2: (N, 2Sz) */
+    uint32_t dtype;         /* BS_F64 */
+    bs_tensor_rec *tensors; /* [T]        */
+    int32_t *qn;            /* [B][3][2]  labels per leg; unused legs 0 */
+    uint32_t *dim;          /* [B][3]     extents; unused legs 1 */
+    uint64_t *addr;         /* [B]        device address of each dense, contiguous, row-major (last index
+                                          fastest) block; must be 8-byte aligned, 16-byte aligned for the
+                                          vector fast path */
+} bs_set_desc;
+
+/* Deferred outcome of one call; 64 bytes in DEVICE memory, written by the call's kernels. */
+typedef struct bs_result {
+    uint64_t total_bytes;   /* header_bytes + payload_bytes (required capacity, also on BS_ERR_CAPACITY) */
+    uint64_t header_bytes;
+    uint64_t payload_bytes;
+    uint64_t pool_bytes;    /* deserialize: bytes BS_LAYOUT_POOL needs = sum align256(nbytes_i) */
+    int32_t status;         /* BS_OK or BS_ERR_* */
+    uint32_t n_tensors;
+    uint32_t n_blocks;
+    uint32_t reserved[5];
+} bs_result;
+
+typedef struct bs_stream_info_t {
+    uint64_t n_tensors, n_blocks, header_bytes, payload_bytes, total_bytes;
+} bs_stream_info_t;
+
+/* Launch tuning.  NULL everywhere means defaults.  The stream produced never depends on these
+ * (decomposition independence; tests/test_gpu_parity.py P6). */
+typedef struct bs_opts {
+    uint32_t variant;     /* 0 = default; 1 = BS_VARIANT_LDG (16-byte vector loads/stores);
+                             2 = BS_VARIANT_TMA (cp.async.bulk global<->shared staging) */
+    uint32_t tile_bytes;  /* stream bytes per work tile; 0 = default; multiple of 16384, <= 65536 */
+    uint32_t ctas_per_sm; /* persistent CTAs per SM; 0 = default */
+    uint32_t reserved;
+} bs_opts;
+enum { BS_VARIANT_DEFAULT = 0, BS_VARIANT_LDG = 1, BS_VARIANT_TMA = 2 };
+
+/* ---- host-only helpers ------------------------------------------------------------------------ */
+uint32_t bs_version(void);
+const char *bs_strerror(int code);
+int bs_last_cuda_error(void); /* cudaError_t of the last BS_ERR_CUDA on this thread */
+
+/* align128(64 + 32*T + 48*B): the header size is known from the counts alone. */
+uint64_t bs_header_bytes(uint64_t n_tensors, uint64_t n_blocks);
+
+/* Bytes of device workspace a call needs for a set of up to n_blocks blocks whose stream is at most
+ * stream_capacity bytes: the offset table ("pointer structure") and scan state. */
+uint64_t bs_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint64_t stream_capacity);
+
+/* Parse the 64-byte fixed header (HOST memory).  BS_ERR_CORRUPT if it is not a v1 header. */
+int bs_stream_info(const void *h_first_64_bytes, bs_stream_info_t *out);
+
+/* ---- serialize ------------------------------------------------------------ */
+
+/* Exact size of the stream before any data moves.  Runs the size/offset pass on `stream`
+ * and SYNCHRONISES it.  header_bytes / total_bytes are HOST outputs. */
+int bs_serialized_size(const bs_set_desc *set, void *d_workspace, uint64_t workspace_bytes,
+                       uint64_t *header_bytes, uint64_t *total_bytes, cudaStream_t stream);
+
+/* Write the stream of `set` to d_stream[0 .. total).  d_stream 16-byte aligned, `capacity` bytes.
+ * Asynchronous.  d_result (DEVICE, 64 bytes) receives total/header/payload bytes and the status:
+ * BS_ERR_CAPACITY if total > capacity (total_bytes = required size), BS_ERR_ARG for a descriptor that
+ * does not partition its blocks, a block address not 8-byte aligned or a size overflow,
+ * BS_ERR_UNSUPPORTED for rank not in {2,3}.  Every byte of [0,total) is written, including padding. */
+int bs_serialize(const bs_set_desc *set, void *d_stream, uint64_t capacity, void *d_workspace,
+                 uint64_t workspace_bytes, bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
+
+/* Segment form (Fig 4(b)): write stream bytes [lo, hi) to d_dst[0 .. hi-lo).  lo, hi
+ * multiples of 16 (hi is clipped to the total).  The size/offset pass must have run on the same
+ * workspace (bs_serialized_size, bs_serialize or a previous range call with lo == 0 runs it).
+ * run_scan != 0 runs it first.  concat over a partition of [0,total) == the bs_serialize stream. */
+int bs_serialize_range(const bs_set_desc *set, void *d_dst, uint64_t lo, uint64_t hi, int run_scan,
+                       void *d_workspace, uint64_t workspace_bytes, bs_result *d_result,
+                       const bs_opts *opts, cudaStream_t stream);
+
+/* ---- deserialize ---------------------------------------------------------------- */
+
+/* Validate the header of d_stream[0..nbytes) (every check of DESIGN.md "deserialize"), rebuild the
+ * descriptor into out's device arrays (capacities out->n_tensors / out->n_blocks) and copy every
+ * block out: to d_pool (BS_LAYOUT_POOL) or to out->addr (BS_SCATTER_TO_ADDR).  Asynchronous.
+ * d_result: status BS_ERR_CORRUPT (nothing written), BS_ERR_CAPACITY (arrays / pool / workspace too
+ * small; pool_bytes = required), BS_ERR_ARG (scatter extents differ); n_tensors / n_blocks = counts. */
+int bs_deserialize(const void *d_stream, uint64_t nbytes, bs_set_desc *out, void *d_pool,
+                   uint64_t pool_bytes, uint32_t flags, void *d_workspace, uint64_t workspace_bytes,
+                   bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
+
+/* ---- asynchronous offload / prefetch engine ------------------- */
+
+typedef struct bs_engine bs_engine;
+typedef struct bs_ticket bs_ticket;
+
+typedef struct bs_engine_cfg {
+    uint64_t chunk_bytes;      /* staging chunk ("segment", PAPER Fig 4(b)); 0 = 256 MiB; multiple of 65536 */
+    uint32_t n_staging;        /* staging buffers; 0 = 2 (double buffering) */
+    uint32_t max_tensors;      /* largest T the engine will see */
+    uint32_t max_blocks;       /* largest B the engine will see */
+    uint64_t max_stream_bytes; /* largest stream the engine will see */
+    bs_opts opts;
+} bs_engine_cfg;
+
+typedef struct bs_ticket_stats {
+    uint64_t bytes;    /* stream bytes moved over PCIe */
+    uint32_t n_chunks;
+    int32_t status;
+    float dma_ms;      /* first DMA start -> last DMA end, device-timed */
+    float total_ms;    /* first engine kernel -> completion, device-timed */
+} bs_ticket_stats;
+
+/* Allocates the side streams (highest priority), events, n_staging staging chunks, the workspace and
+ * a header buffer sized for max_blocks.  Device memory use = n_staging*chunk_bytes + O(max_blocks). */
+int bs_engine_create(bs_engine **out, const bs_engine_cfg *cfg);
+int bs_engine_destroy(bs_engine *e); /* waits for in-flight work */
+
+/* Save: after everything already enqueued on `producer`, pack the stream of `set` chunk by chunk into
+ * the staging buffers and DMA each chunk to h_pinned[0..total).  Returns at once; `producer` is not
+ * blocked.  total_bytes = the value bs_serialized_size returned for this set (the paper's size
+ * prediction, L106; it fixes the chunk count on the host and is re-checked on the device);
+ * total_bytes == 0 makes the call compute it, which SYNCHRONISES `producer`.
+ * BS_ERR_CAPACITY at once if total_bytes > h_capacity or exceeds the engine's limits. */
+int bs_offload_async(bs_engine *e, const bs_set_desc *set, uint64_t total_bytes, void *h_pinned,
+                     uint64_t h_capacity, cudaStream_t producer, bs_ticket **ticket);
+
+/* Load: DMA the stream h_pinned[0..nbytes) chunk by chunk to the staging buffers, validate the header,
+ * rebuild `out` and scatter every block (flags as bs_deserialize).  `consumer` is made to wait for
+ * completion (cudaStreamWaitEvent — the "checkpoint" of PAPER L138); the host is not blocked. */
+int bs_prefetch_async(bs_engine *e, const void *h_pinned, uint64_t nbytes, bs_set_desc *out, void *d_pool,
+                      uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket **ticket);
+
+int bs_ticket_wait(bs_ticket *t, bs_ticket_stats *stats /* may be NULL */); /* blocks the host; returns the deferred status */
+int bs_ticket_query(const bs_ticket *t);                                   /* BS_OK | BS_PENDING | BS_ERR_* */
+int bs_ticket_destroy(bs_ticket *t);                                       /* after completion */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BS_H_ */

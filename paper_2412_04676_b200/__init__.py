@@ -1,0 +1,15 @@
+"""paper_2412_04676_b200 — B200-native serialization / offload of U(1) block-sparse DMRG scratch data.
+
+Python face of the C-ABI library ``libbsstream.so`` (include/bs.h): same names, argument marshalling only.
+PyTorch is used for device memory and streams, nothing else; every step of the path (size/offset scan, header
+write, pack, header parse, unpack, chunked offload/prefetch) runs in the library's hand-written CUDA kernels.
+There is no CPU fallback.
+"""
+from ._binding import (  # noqa: F401
+    ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_CUDA, ERR_UNSUPPORTED, F64, LAYOUT_POOL, OK, PENDING, SCATTER_TO_ADDR,
+    VARIANT_DEFAULT, VARIANT_LDG, VARIANT_TMA,
+    BsError, Engine, Opts, Result, SetDesc, Ticket,
+    deserialize, header_bytes, last_cuda_error, lib, make_desc, serialize, serialize_range, serialized_size,
+    stream_info, strerror, version, workspace_bytes,
+)
+from .device import DeviceSet, Workspace, current_stream  # noqa: F401

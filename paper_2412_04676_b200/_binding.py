@@ -1,0 +1,234 @@
+"""ctypes binding of libbsstream.so (include/bs.h).  Argument marshalling only: every step of the
+path runs in the library's CUDA kernels.  There is no CPU fallback — if the shared library cannot be
+loaded this module raises, and every device call fails with BS_ERR_CUDA on a box without a GPU."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+from . import build as _build
+
+OK, PENDING = 0, 1
+ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_UNSUPPORTED, ERR_CUDA = -1, -2, -3, -4, -5
+F64 = 0
+LAYOUT_POOL, SCATTER_TO_ADDR = 0, 1
+VARIANT_DEFAULT, VARIANT_LDG, VARIANT_TMA = 0, 1, 2
+
+
+class BsError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what}: {strerror(code)} ({code})" + (f", cudaError {last_cuda_error()}" if code == ERR_CUDA else ""))
+        self.code = code
+
+
+class TensorRec(C.Structure):
+    _fields_ = [("rank", C.c_uint32), ("first_block", C.c_uint32), ("n_blocks", C.c_uint32), ("dq", C.c_int32 * 2),
+                ("sign", C.c_int8 * 4), ("tag", C.c_uint32), ("reserved", C.c_uint32)]
+
+
+class SetDesc(C.Structure):
+    _fields_ = [("n_tensors", C.c_uint32), ("n_blocks", C.c_uint32), ("n_qn", C.c_uint32), ("dtype", C.c_uint32),
+                ("tensors", C.c_void_p), ("qn", C.c_void_p), ("dim", C.c_void_p), ("addr", C.c_void_p)]
+
+
+class Result(C.Structure):
+    _fields_ = [("total_bytes", C.c_uint64), ("header_bytes", C.c_uint64), ("payload_bytes", C.c_uint64),
+                ("pool_bytes", C.c_uint64), ("status", C.c_int32), ("n_tensors", C.c_uint32), ("n_blocks", C.c_uint32),
+                ("reserved", C.c_uint32 * 5)]
+
+
+class StreamInfo(C.Structure):
+    _fields_ = [("n_tensors", C.c_uint64), ("n_blocks", C.c_uint64), ("header_bytes", C.c_uint64),
+                ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64)]
+
+
+class Opts(C.Structure):
+    _fields_ = [("variant", C.c_uint32), ("tile_bytes", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("reserved", C.c_uint32)]
+
+
+class EngineCfg(C.Structure):
+    _fields_ = [("chunk_bytes", C.c_uint64), ("n_staging", C.c_uint32), ("max_tensors", C.c_uint32),
+                ("max_blocks", C.c_uint32), ("max_stream_bytes", C.c_uint64), ("opts", Opts)]
+
+
+class TicketStats(C.Structure):
+    _fields_ = [("bytes", C.c_uint64), ("n_chunks", C.c_uint32), ("status", C.c_int32), ("dma_ms", C.c_float),
+                ("total_ms", C.c_float)]
+
+
+assert C.sizeof(TensorRec) == 32 and C.sizeof(Result) == 64
+
+_lib = None
+
+
+def lib():
+    """Load libbsstream.so, building it in-tree first if it is missing or stale (nvcc, sm_100a)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    so = _build.SO
+    if _build.is_stale():
+        try:
+            so = _build.build()
+        except Exception as e:  # no nvcc on this box and no prebuilt library: fail loudly
+            if not os.path.exists(so):
+                raise ImportError(f"libbsstream.so is not built and cannot be built here: {e}") from e
+    L = C.CDLL(so)
+    u32, u64, vp, i32 = C.c_uint32, C.c_uint64, C.c_void_p, C.c_int
+    pu64 = C.POINTER(C.c_uint64)
+    L.bs_version.restype = u32
+    L.bs_strerror.restype = C.c_char_p
+    L.bs_strerror.argtypes = [i32]
+    L.bs_last_cuda_error.restype = i32
+    L.bs_header_bytes.restype = u64
+    L.bs_header_bytes.argtypes = [u64, u64]
+    L.bs_workspace_bytes.restype = u64
+    L.bs_workspace_bytes.argtypes = [u32, u32, u64]
+    L.bs_stream_info.argtypes = [vp, C.POINTER(StreamInfo)]
+    L.bs_serialized_size.argtypes = [C.POINTER(SetDesc), vp, u64, pu64, pu64, vp]
+    L.bs_serialize.argtypes = [C.POINTER(SetDesc), vp, u64, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_serialize_range.argtypes = [C.POINTER(SetDesc), vp, u64, u64, i32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_deserialize.argtypes = [vp, u64, C.POINTER(SetDesc), vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_engine_create.argtypes = [C.POINTER(vp), C.POINTER(EngineCfg)]
+    L.bs_engine_destroy.argtypes = [vp]
+    L.bs_offload_async.argtypes = [vp, C.POINTER(SetDesc), u64, vp, u64, vp, C.POINTER(vp)]
+    L.bs_prefetch_async.argtypes = [vp, vp, u64, C.POINTER(SetDesc), vp, u64, u32, vp, C.POINTER(vp)]
+    L.bs_ticket_wait.argtypes = [vp, C.POINTER(TicketStats)]
+    L.bs_ticket_query.argtypes = [vp]
+    L.bs_ticket_destroy.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def _check(rc: int, what: str) -> int:
+    if rc < 0:
+        raise BsError(rc, what)
+    return rc
+
+
+def _opts(opts):
+    if opts is None:
+        return None
+    if isinstance(opts, Opts):
+        return C.byref(opts)
+    return C.byref(Opts(int(opts.get("variant", 0)), int(opts.get("tile_bytes", 0)), int(opts.get("ctas_per_sm", 0)), 0))
+
+
+def version() -> int:
+    return int(lib().bs_version())
+
+
+def strerror(code: int) -> str:
+    return lib().bs_strerror(code).decode()
+
+
+def last_cuda_error() -> int:
+    return int(lib().bs_last_cuda_error())
+
+
+def header_bytes(n_tensors: int, n_blocks: int) -> int:
+    return int(lib().bs_header_bytes(n_tensors, n_blocks))
+
+
+def workspace_bytes(n_tensors: int, n_blocks: int, stream_capacity: int) -> int:
+    return int(lib().bs_workspace_bytes(n_tensors, n_blocks, stream_capacity))
+
+
+def stream_info(first_64_bytes) -> dict:
+    """Parse the fixed header from HOST bytes (bytes / bytearray / numpy uint8)."""
+    buf = (C.c_ubyte * 64).from_buffer_copy(bytes(first_64_bytes[:64]).ljust(64, b"\0"))
+    info = StreamInfo()
+    _check(lib().bs_stream_info(C.addressof(buf), C.byref(info)), "bs_stream_info")
+    return {k: int(getattr(info, k)) for k, _ in StreamInfo._fields_}
+
+
+def make_desc(n_tensors: int, n_blocks: int, tensors_ptr: int, qn_ptr: int, dim_ptr: int, addr_ptr: int) -> SetDesc:
+    return SetDesc(n_tensors, n_blocks, 2, F64, tensors_ptr, qn_ptr, dim_ptr, addr_ptr)
+
+
+def serialized_size(desc: SetDesc, ws_ptr: int, ws_bytes: int, stream: int = 0):
+    hb, tot = C.c_uint64(0), C.c_uint64(0)
+    _check(lib().bs_serialized_size(C.byref(desc), ws_ptr, ws_bytes, C.byref(hb), C.byref(tot), stream), "bs_serialized_size")
+    return int(hb.value), int(tot.value)
+
+
+def serialize(desc: SetDesc, stream_ptr: int, capacity: int, ws_ptr: int, ws_bytes: int, result_ptr: int,
+              opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_serialize(C.byref(desc), stream_ptr, capacity, ws_ptr, ws_bytes, result_ptr, _opts(opts), stream),
+                  "bs_serialize")
+
+
+def serialize_range(desc: SetDesc, dst_ptr: int, lo: int, hi: int, run_scan: bool, ws_ptr: int, ws_bytes: int,
+                    result_ptr: int, opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_serialize_range(C.byref(desc), dst_ptr, lo, hi, int(run_scan), ws_ptr, ws_bytes, result_ptr,
+                                           _opts(opts), stream), "bs_serialize_range")
+
+
+def deserialize(stream_ptr: int, nbytes: int, out: SetDesc, pool_ptr: int, pool_bytes: int, flags: int, ws_ptr: int,
+                ws_bytes: int, result_ptr: int, opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_deserialize(stream_ptr, nbytes, C.byref(out), pool_ptr, pool_bytes, flags, ws_ptr, ws_bytes,
+                                       result_ptr, _opts(opts), stream), "bs_deserialize")
+
+
+class Ticket:
+    def __init__(self, handle: int):
+        self._h = handle
+
+    def query(self) -> int:
+        return int(lib().bs_ticket_query(self._h))
+
+    def wait(self) -> dict:
+        st = TicketStats()
+        rc = lib().bs_ticket_wait(self._h, C.byref(st))
+        out = dict(status=int(rc), bytes=int(st.bytes), n_chunks=int(st.n_chunks), dma_ms=float(st.dma_ms),
+                   total_ms=float(st.total_ms))
+        return out
+
+    def destroy(self):
+        if self._h:
+            lib().bs_ticket_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class Engine:
+    """bs_engine_create / bs_offload_async / bs_prefetch_async."""
+
+    def __init__(self, max_tensors: int, max_blocks: int, max_stream_bytes: int, chunk_bytes: int = 0, n_staging: int = 0,
+                 opts=None):
+        o = Opts()
+        if opts:
+            o = Opts(int(opts.get("variant", 0)), int(opts.get("tile_bytes", 0)), int(opts.get("ctas_per_sm", 0)), 0)
+        cfg = EngineCfg(chunk_bytes, n_staging, max_tensors, max_blocks, max_stream_bytes, o)
+        h = C.c_void_p(0)
+        _check(lib().bs_engine_create(C.byref(h), C.byref(cfg)), "bs_engine_create")
+        self._h = h.value
+
+    def offload_async(self, desc: SetDesc, total_bytes: int, h_pinned_ptr: int, h_capacity: int, producer: int = 0) -> Ticket:
+        t = C.c_void_p(0)
+        _check(lib().bs_offload_async(self._h, C.byref(desc), total_bytes, h_pinned_ptr, h_capacity, producer, C.byref(t)),
+               "bs_offload_async")
+        return Ticket(t.value)
+
+    def prefetch_async(self, h_pinned_ptr: int, nbytes: int, out: SetDesc, pool_ptr: int, pool_bytes: int, flags: int = 0,
+                       consumer: int = 0) -> Ticket:
+        t = C.c_void_p(0)
+        _check(lib().bs_prefetch_async(self._h, h_pinned_ptr, nbytes, C.byref(out), pool_ptr, pool_bytes, flags, consumer,
+                                       C.byref(t)), "bs_prefetch_async")
+        return Ticket(t.value)
+
+    def destroy(self):
+        if self._h:
+            lib().bs_engine_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

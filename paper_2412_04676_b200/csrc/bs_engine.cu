@@ -1,0 +1,305 @@
+// bs_engine.cu — asynchronous offload / prefetch engine: steps S8, S9 of SURVEY §8(a).
+//
+// PAPER L89 (Fig 4(b)): "serialization of data in small segments based on the size of a preallocated buffer
+// and saving each segment ... immediately"; L90/L132: "a single CPU thread takes care of saving the serialized
+// data while the remaining CPU threads ... proceed with subsequent computational tasks"; L134: the load runs
+// "in parallel of the renormalization step"; L138: "checkpoints to make sure that required data ... are already
+// available".  On a B200 the "single thread" is a pair of high-priority side streams and the copy engine:
+//     kernel stream : scan | pack(chunk 0) | pack(chunk 1) | ...          (waits for staging buffer k%S to drain)
+//     copy   stream :        D2H(chunk 0)  | D2H(chunk 1)  | ...          (waits for pack(chunk k))
+// with S = n_staging (2: double buffering) staging buffers of chunk_bytes (256 MiB).  The producer / consumer
+// stream is never blocked on the host; the ticket's event is the checkpoint.  Device memory held by the engine
+// is S*chunk_bytes + O(max_blocks) — the "small additional memory" of L89/L94, not the +30-50 % of L92/L166.
+// Bound: the PCIe link (one direction per call); the pack / unpack kernels are ~50x faster than the DMA.
+#include <new>
+#include <string.h>
+
+#include "bs_internal.cuh"
+
+namespace bs {
+int cuda_fail(cudaError_t e);
+int device_sm_count(int* out);
+int run_serialize_scan(const bs_set_desc* set, const WsLayout& L, uint64_t capacity, uint64_t expect_total,
+                       bs_result* d_result, int sms, cudaStream_t stream);
+int run_pack_range(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint64_t lo, uint64_t hi,
+                   const bs_opts& o, int sms, cudaStream_t stream);
+int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_set_desc* out,
+                         void* d_pool, uint64_t pool_bytes, uint32_t flags, const WsLayout& L, bs_result* d_result,
+                         int sms, cudaStream_t stream);
+int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header,
+                     uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream);
+}  // namespace bs
+
+using namespace bs;
+
+namespace {
+constexpr uint32_t kMaxStaging = 8;
+constexpr uint32_t kFlagCheckPad = 0x100u;
+}
+
+struct bs_engine {
+    bs_engine_cfg cfg;
+    bs_opts opts;
+    int sms;
+    cudaStream_t kstream, cstream;
+    unsigned char* staging[kMaxStaging];
+    cudaEvent_t ev_k[kMaxStaging];  // kernel finished with staging[b]
+    cudaEvent_t ev_c[kMaxStaging];  // DMA finished with staging[b]
+    cudaEvent_t ev_fence_k, ev_fence_c, ev_dep;
+    void* ws;
+    uint64_t ws_bytes;
+    unsigned char* header_buf;
+    uint64_t header_cap;
+    bs_result* d_result;
+};
+
+struct bs_ticket {
+    cudaEvent_t t_begin, dma_begin, dma_end, done;
+    bs_result* h_result;  // pinned
+    uint64_t bytes;
+    uint32_t n_chunks;
+    int immediate;  // status known at submit time (no device work was enqueued)
+    bool is_prefetch;
+};
+
+#define CK(call)                                          \
+    do {                                                  \
+        cudaError_t e__ = (call);                         \
+        if (e__ != cudaSuccess) return cuda_fail(e__);    \
+    } while (0)
+
+static int ticket_create(bs_ticket** out)
+{
+    bs_ticket* t = new (std::nothrow) bs_ticket;
+    if (!t) return BS_ERR_ARG;
+    memset(t, 0, sizeof(*t));
+    cudaError_t e;
+    if ((e = cudaEventCreate(&t->t_begin)) != cudaSuccess || (e = cudaEventCreate(&t->dma_begin)) != cudaSuccess ||
+        (e = cudaEventCreate(&t->dma_end)) != cudaSuccess || (e = cudaEventCreate(&t->done)) != cudaSuccess ||
+        (e = cudaHostAlloc((void**)&t->h_result, sizeof(bs_result), cudaHostAllocDefault)) != cudaSuccess) {
+        delete t;
+        return cuda_fail(e);
+    }
+    memset(t->h_result, 0, sizeof(bs_result));
+    t->h_result->status = BS_PENDING;
+    *out = t;
+    return BS_OK;
+}
+
+// serialise engine calls: everything already enqueued on either side stream precedes the new call on both
+static int engine_fence(bs_engine* e)
+{
+    CK(cudaEventRecord(e->ev_fence_k, e->kstream));
+    CK(cudaEventRecord(e->ev_fence_c, e->cstream));
+    CK(cudaStreamWaitEvent(e->cstream, e->ev_fence_k, 0));
+    CK(cudaStreamWaitEvent(e->kstream, e->ev_fence_c, 0));
+    return BS_OK;
+}
+
+extern "C" {
+
+int bs_engine_create(bs_engine** out, const bs_engine_cfg* cfg)
+{
+    if (out == nullptr || cfg == nullptr) return BS_ERR_ARG;
+    bs_engine* e = new (std::nothrow) bs_engine;
+    if (!e) return BS_ERR_ARG;
+    memset(e, 0, sizeof(*e));
+    e->cfg = *cfg;
+    if (e->cfg.chunk_bytes == 0) e->cfg.chunk_bytes = 256ull << 20;
+    if (e->cfg.n_staging == 0) e->cfg.n_staging = 2;
+    if (e->cfg.chunk_bytes % 65536 != 0 || e->cfg.n_staging > kMaxStaging || e->cfg.n_staging < 1) { delete e; return BS_ERR_ARG; }
+    resolve_opts(&cfg->opts, &e->opts);
+    int rc = device_sm_count(&e->sms);
+    if (rc) { delete e; return rc; }
+    int lo_prio = 0, hi_prio = 0;
+    cudaError_t ce = cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio);
+    if (ce == cudaSuccess) ce = cudaStreamCreateWithPriority(&e->kstream, cudaStreamNonBlocking, hi_prio);
+    if (ce == cudaSuccess) ce = cudaStreamCreateWithPriority(&e->cstream, cudaStreamNonBlocking, hi_prio);
+    for (uint32_t b = 0; ce == cudaSuccess && b < e->cfg.n_staging; ++b) {
+        ce = cudaMalloc((void**)&e->staging[b], e->cfg.chunk_bytes);
+        if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e->ev_k[b], cudaEventDisableTiming);
+        if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e->ev_c[b], cudaEventDisableTiming);
+    }
+    if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e->ev_fence_k, cudaEventDisableTiming);
+    if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e->ev_fence_c, cudaEventDisableTiming);
+    if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e->ev_dep, cudaEventDisableTiming);
+    e->ws_bytes = bs_workspace_bytes(e->cfg.max_tensors, e->cfg.max_blocks, e->cfg.max_stream_bytes);
+    e->header_cap = bs_header_bytes(e->cfg.max_tensors, e->cfg.max_blocks);
+    if (ce == cudaSuccess) ce = cudaMalloc(&e->ws, e->ws_bytes);
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&e->header_buf, e->header_cap);
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&e->d_result, sizeof(bs_result));
+    if (ce != cudaSuccess) {
+        bs_engine_destroy(e);
+        return cuda_fail(ce);
+    }
+    *out = e;
+    return BS_OK;
+}
+
+int bs_engine_destroy(bs_engine* e)
+{
+    if (e == nullptr) return BS_ERR_ARG;
+    if (e->kstream) cudaStreamSynchronize(e->kstream);
+    if (e->cstream) cudaStreamSynchronize(e->cstream);
+    for (uint32_t b = 0; b < kMaxStaging; ++b) {
+        if (e->staging[b]) cudaFree(e->staging[b]);
+        if (e->ev_k[b]) cudaEventDestroy(e->ev_k[b]);
+        if (e->ev_c[b]) cudaEventDestroy(e->ev_c[b]);
+    }
+    if (e->ev_fence_k) cudaEventDestroy(e->ev_fence_k);
+    if (e->ev_fence_c) cudaEventDestroy(e->ev_fence_c);
+    if (e->ev_dep) cudaEventDestroy(e->ev_dep);
+    if (e->ws) cudaFree(e->ws);
+    if (e->header_buf) cudaFree(e->header_buf);
+    if (e->d_result) cudaFree(e->d_result);
+    if (e->kstream) cudaStreamDestroy(e->kstream);
+    if (e->cstream) cudaStreamDestroy(e->cstream);
+    delete e;
+    return BS_OK;
+}
+
+int bs_offload_async(bs_engine* e, const bs_set_desc* set, uint64_t total_bytes, void* h_pinned, uint64_t h_capacity,
+                     cudaStream_t producer, bs_ticket** ticket)
+{
+    if (e == nullptr || set == nullptr || h_pinned == nullptr || ticket == nullptr) return BS_ERR_ARG;
+    if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
+    WsLayout L;
+    if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
+    int rc;
+    if (total_bytes == 0) {  // size prediction on the producer stream (synchronises it)
+        uint64_t hb = 0;
+        if ((rc = bs_serialized_size(set, e->ws, e->ws_bytes, &hb, &total_bytes, producer))) return rc;
+    }
+    if (total_bytes > h_capacity || total_bytes > e->cfg.max_stream_bytes) return BS_ERR_CAPACITY;
+    if (total_bytes & 15) return BS_ERR_ARG;
+    bs_ticket* t = nullptr;
+    if ((rc = ticket_create(&t))) return rc;
+    const uint64_t C = e->cfg.chunk_bytes;
+    const uint32_t S = e->cfg.n_staging;
+    t->bytes = total_bytes;
+    t->n_chunks = (uint32_t)((total_bytes + C - 1) / C);
+
+    if ((rc = engine_fence(e))) return rc;
+    CK(cudaEventRecord(e->ev_dep, producer));          // the data is ready after everything enqueued so far
+    CK(cudaStreamWaitEvent(e->kstream, e->ev_dep, 0));
+    CK(cudaEventRecord(t->t_begin, e->kstream));
+    if ((rc = run_serialize_scan(set, L, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream))) return rc;
+    CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
+    for (uint32_t k = 0; k < t->n_chunks; ++k) {
+        const uint32_t b = k % S;
+        const uint64_t lo = (uint64_t)k * C, hi = (lo + C < total_bytes) ? lo + C : total_bytes;
+        if (k >= S) CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));  // staging[b] drained by DMA k-S
+        if ((rc = run_pack_range(set, L, e->staging[b], lo, hi, e->opts, e->sms, e->kstream))) return rc;
+        CK(cudaEventRecord(e->ev_k[b], e->kstream));
+        CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));
+        if (k == 0) CK(cudaEventRecord(t->dma_begin, e->cstream));
+        CK(cudaMemcpyAsync((unsigned char*)h_pinned + lo, e->staging[b], hi - lo, cudaMemcpyDeviceToHost, e->cstream));
+        CK(cudaEventRecord(e->ev_c[b], e->cstream));
+    }
+    if (t->n_chunks == 0) CK(cudaEventRecord(t->dma_begin, e->cstream));
+    CK(cudaEventRecord(t->dma_end, e->cstream));
+    CK(cudaEventRecord(t->done, e->cstream));  // after the last DMA, which is after every kernel-stream step
+    *ticket = t;
+    return BS_OK;
+}
+
+int bs_prefetch_async(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs_set_desc* out, void* d_pool,
+                      uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket** ticket)
+{
+    if (e == nullptr || h_pinned == nullptr || out == nullptr || ticket == nullptr) return BS_ERR_ARG;
+    if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
+    if (nbytes < kFixedHeader) return BS_ERR_CORRUPT;
+    bs_stream_info_t info;
+    int rc = bs_stream_info(h_pinned, &info);  // the stream is in host RAM: its counts cost nothing to read
+    if (rc) return rc;
+    if (info.total_bytes != nbytes) return BS_ERR_CORRUPT;
+    if (info.n_blocks > e->cfg.max_blocks || info.n_tensors > e->cfg.max_tensors || info.header_bytes > e->header_cap ||
+        nbytes > e->cfg.max_stream_bytes)
+        return BS_ERR_CAPACITY;
+    if (info.n_blocks > out->n_blocks || info.n_tensors > out->n_tensors) return BS_ERR_CAPACITY;
+    WsLayout L;
+    if (!ws_layout(e->ws, e->ws_bytes, out->n_blocks, &L)) return BS_ERR_CAPACITY;
+    bs_ticket* t = nullptr;
+    if ((rc = ticket_create(&t))) return rc;
+    t->is_prefetch = true;
+    const uint64_t C = e->cfg.chunk_bytes;
+    const uint32_t S = e->cfg.n_staging;
+    const uint64_t hb = info.header_bytes;
+    t->bytes = nbytes;
+    t->n_chunks = (uint32_t)((info.payload_bytes + C - 1) / C);
+
+    if ((rc = engine_fence(e))) return rc;
+    CK(cudaEventRecord(e->ev_dep, consumer));  // destinations may still be in use by work already enqueued
+    CK(cudaStreamWaitEvent(e->cstream, e->ev_dep, 0));
+    CK(cudaStreamWaitEvent(e->kstream, e->ev_dep, 0));
+    CK(cudaEventRecord(t->t_begin, e->cstream));
+    CK(cudaEventRecord(t->dma_begin, e->cstream));
+    // header first: validate + offset table + descriptor rebuild, while the payload chunks stream in
+    CK(cudaMemcpyAsync(e->header_buf, h_pinned, hb, cudaMemcpyHostToDevice, e->cstream));
+    CK(cudaEventRecord(e->ev_fence_c, e->cstream));
+    CK(cudaStreamWaitEvent(e->kstream, e->ev_fence_c, 0));
+    if ((rc = run_deserialize_scan(e->header_buf, nullptr, nbytes, out, d_pool, pool_bytes, flags, L, e->d_result,
+                                   e->sms, e->kstream)))
+        return rc;
+    CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
+    if ((rc = run_unpack_range(out, L, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream))) return rc;
+    for (uint32_t k = 0; k < t->n_chunks; ++k) {
+        const uint32_t b = k % S;
+        const uint64_t lo = hb + (uint64_t)k * C, hi = (lo + C < nbytes) ? lo + C : nbytes;
+        if (k >= S) CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));  // staging[b] consumed by unpack k-S
+        CK(cudaMemcpyAsync(e->staging[b], (const unsigned char*)h_pinned + lo, hi - lo, cudaMemcpyHostToDevice, e->cstream));
+        CK(cudaEventRecord(e->ev_c[b], e->cstream));
+        CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));
+        if ((rc = run_unpack_range(out, L, e->staging[b], nullptr, lo, hi, flags | kFlagCheckPad, e->opts, e->sms, e->kstream)))
+            return rc;
+        CK(cudaEventRecord(e->ev_k[b], e->kstream));
+    }
+    CK(cudaEventRecord(t->dma_end, e->cstream));
+    // final status (the pad check of the unpack kernels can still flip it) and the checkpoint event
+    CK(cudaMemcpyAsync(&t->h_result->status, &L.head->status, sizeof(int32_t), cudaMemcpyDeviceToHost, e->kstream));
+    CK(cudaEventRecord(t->done, e->kstream));
+    CK(cudaStreamWaitEvent(consumer, t->done, 0));
+    *ticket = t;
+    return BS_OK;
+}
+
+int bs_ticket_query(const bs_ticket* t)
+{
+    if (t == nullptr) return BS_ERR_ARG;
+    cudaError_t e = cudaEventQuery(t->done);
+    if (e == cudaErrorNotReady) return BS_PENDING;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return t->h_result->status;
+}
+
+int bs_ticket_wait(bs_ticket* t, bs_ticket_stats* stats)
+{
+    if (t == nullptr) return BS_ERR_ARG;
+    CK(cudaEventSynchronize(t->done));
+    if (stats) {
+        stats->bytes = t->bytes;
+        stats->n_chunks = t->n_chunks;
+        stats->status = t->h_result->status;
+        stats->dma_ms = 0.f;
+        stats->total_ms = 0.f;
+        CK(cudaEventSynchronize(t->dma_end));
+        CK(cudaEventElapsedTime(&stats->dma_ms, t->dma_begin, t->dma_end));
+        CK(cudaEventElapsedTime(&stats->total_ms, t->t_begin, t->done));
+    }
+    return t->h_result->status;
+}
+
+int bs_ticket_destroy(bs_ticket* t)
+{
+    if (t == nullptr) return BS_ERR_ARG;
+    cudaEventSynchronize(t->done);
+    cudaEventDestroy(t->t_begin);
+    cudaEventDestroy(t->dma_begin);
+    cudaEventDestroy(t->dma_end);
+    cudaEventDestroy(t->done);
+    cudaFreeHost(t->h_result);
+    delete t;
+    return BS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,122 @@
+// bs_internal.cuh — shared declarations of libbsstream's translation units (not part of the C ABI).
+//
+// Data layout in HBM:
+//   workspace := bs_wshead (256 B) | scan_state[n_scan_tiles+1] u64 | blk[B_cap+1] (16 B each)
+//                | tile_first[n_granules_cap] u32
+//   blk[i]        = { payload offset of block i , device address of block i | odd-flag in bit 0 }
+//                   — the paper's "pointer structure ... grid structure of the serialized data"
+//                   (PAPER L90-92), built before any data moves;  blk[B] = { P, 0 } sentinel.
+//   tile_first[g] = index of the block that holds payload byte g*BS_GRANULE  (work partition, S4)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "bs.h"
+
+namespace bs {
+
+constexpr uint32_t kFixedHeader = 64;
+constexpr uint32_t kTensorRec = 32;
+constexpr uint32_t kBlockRec = 48;
+constexpr uint32_t kHeaderAlign = 128;
+constexpr uint32_t kPoolAlign = 256;
+constexpr uint32_t kGranule = 16384;  // bytes of payload per tile_first entry
+
+constexpr uint32_t kScanThreads = 256;
+constexpr uint32_t kScanItems = 4;
+constexpr uint32_t kScanTile = kScanThreads * kScanItems;
+
+struct __align__(16) Blk {
+    uint64_t off;   // payload offset (exclusive prefix sum of stored sizes)
+    uint64_t addr;  // device address of the dense block; bit 0 set: nbytes = stored - 8 (odd element count)
+};
+
+struct __align__(256) WsHead {
+    uint32_t scan_ticket;    // dynamic tile id of the single-pass scan
+    uint32_t ctas_done;      // last CTA out finalises
+    int32_t status;          // first error wins (atomicCAS)
+    uint32_t n_tensors;
+    uint32_t n_blocks;
+    uint32_t pad0;
+    uint64_t header_bytes;
+    uint64_t payload_bytes;
+    uint64_t pool_bytes;
+    uint64_t n_granules;     // ceil(P / kGranule)
+};
+
+struct WsLayout {
+    WsHead* head;
+    uint64_t* scan_state;
+    Blk* blk;
+    uint32_t* tile_first;
+    uint64_t n_granules_cap;
+    uint64_t zero_bytes;  // head + scan_state: cleared before every scan
+};
+
+__host__ __device__ inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + (a - 1)) / a * a; }
+
+inline uint64_t ws_fixed_bytes(uint32_t n_blocks)
+{
+    uint64_t n_scan_tiles = ((uint64_t)n_blocks + kScanTile) / kScanTile + 1;
+    return sizeof(WsHead) + align_up(n_scan_tiles * 8, 256) + align_up(((uint64_t)n_blocks + 1) * sizeof(Blk), 256);
+}
+
+inline bool ws_layout(void* d_ws, uint64_t ws_bytes, uint32_t n_blocks, WsLayout* L)
+{
+    uint64_t n_scan_tiles = ((uint64_t)n_blocks + kScanTile) / kScanTile + 1;
+    uint64_t fixed = ws_fixed_bytes(n_blocks);
+    if (d_ws == nullptr || ((uintptr_t)d_ws & 255) != 0 || ws_bytes < fixed + 16) return false;
+    unsigned char* p = (unsigned char*)d_ws;
+    L->head = (WsHead*)p;
+    L->scan_state = (uint64_t*)(p + sizeof(WsHead));
+    L->zero_bytes = sizeof(WsHead) + align_up(n_scan_tiles * 8, 256);
+    L->blk = (Blk*)(p + L->zero_bytes);
+    L->tile_first = (uint32_t*)(p + fixed);
+    L->n_granules_cap = (ws_bytes - fixed) / 4;
+    return true;
+}
+
+// ---- scan pass (S1, S2, S4 / S6): sizes -> offsets -> blk table + tile_first; validation -------------
+struct ScanParams {
+    WsLayout ws;
+    bs_result* result;       // device, may be null
+    uint64_t capacity;       // SER: stream capacity; DESER: unused
+    uint64_t expect_total;   // SER: if nonzero, total must equal it (engine re-check of the size prediction)
+    // SER inputs (descriptor, device arrays)
+    const bs_tensor_rec* tensors;
+    const uint32_t* dim;
+    const uint64_t* addr;
+    uint32_t T, B;           // SER: counts; DESER: capacities of the out arrays
+    // DESER inputs
+    const unsigned char* header;  // stream byte 0 .. header_bytes (device)
+    const unsigned char* payload; // stream byte 0 when the payload is resident behind the header (pad-zero check), else null
+    uint64_t nbytes;              // total stream length
+    uint64_t pool_base;           // BS_LAYOUT_POOL: device address of the pool
+    uint64_t pool_bytes;
+    const uint32_t* out_dim;      // BS_SCATTER_TO_ADDR inputs
+    const uint64_t* out_addr;
+    uint32_t flags;
+};
+
+cudaError_t launch_scan(bool deser, const ScanParams& p, int sm_count, cudaStream_t stream);
+
+// ---- data movement (S3, S5 / S7): stream bytes [lo,hi) <-> blocks ------------------------------------------
+struct MoveParams {
+    WsLayout ws;
+    // descriptor arrays: SER inputs, DESER outputs
+    bs_tensor_rec* tensors;
+    int32_t* qn;
+    uint32_t* dim;
+    uint64_t* addr;
+    unsigned char* stream;        // p with p[s - lo] = stream byte s   (pack: destination; unpack: source)
+    const unsigned char* header;  // DESER: stream byte 0.. (whole header region), null = no descriptor rebuild
+    uint64_t lo, hi;
+    uint32_t tile_bytes;
+    uint32_t flags;
+};
+
+cudaError_t launch_move(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream);
+
+void resolve_opts(const bs_opts* in, bs_opts* out);
+
+}  // namespace bs

@@ -1,0 +1,261 @@
+// bs_move.cu — the data-movement kernels: steps S3 + S5 (header write + pack) and S7 (descriptor rebuild +
+// unpack / scatter) of SURVEY §8(a).
+//
+// once the output buffer is mapped, "all threads serialize in parallel and in complete
+// independence. Yet, together they produce a single, continuos stream of bytes".  Here the unit of
+// independence is a TILE of the stream (tile_bytes, a multiple of the 16 KiB granule): tile k of the payload is
+// stream bytes [header_bytes + k*tile_bytes, +tile_bytes), whatever blocks happen to lie in it.  A persistent
+// grid of CTAs walks the tiles; tile_first[] says which block the tile starts in, blk[] gives every block's
+// {payload offset, device address}.  So the work per CTA is uniform no matter how skewed the block sizes are
+// (0.5 KiB .. 1 MiB in the paper-shaped sets), the stream side of every access is perfectly contiguous, and a
+// byte range [lo,hi) of the stream (one 256 MiB offload segment, PAPER Fig 4(b)) is just a range of tiles.
+//
+// Roofline: pure data movement — 1 byte read + 1 byte written per stream byte, HBM-bound.
+//
+// Variant LDG (this file, variant 1): every thread moves 16-byte units with vector loads / stores
+// (ld.global.cs.v4 / st.global.cs.v4), UPT units in flight per thread.
+// Variant TMA (bs_move_tma.cu, variant 2): cp.async.bulk global<->shared staging.
+#include "bs_internal.cuh"
+
+namespace bs {
+
+namespace {
+
+constexpr uint32_t kThreads = 256;
+
+__device__ __forceinline__ uint4 ld_stream16(const void* p) { return __ldcs(reinterpret_cast<const uint4*>(p)); }
+__device__ __forceinline__ uint2 ld_stream8(const void* p) { return __ldcs(reinterpret_cast<const uint2*>(p)); }
+__device__ __forceinline__ void st_stream16(void* p, uint4 v) { __stcs(reinterpret_cast<uint4*>(p), v); }
+__device__ __forceinline__ void st_stream8(void* p, uint2 v) { __stcs(reinterpret_cast<uint2*>(p), v); }
+
+// owner of block r: the last tensor t with first_block[t] <= r (tensors partition the blocks in order)
+__device__ __forceinline__ uint32_t tensor_of_block(const bs_tensor_rec* tensors, uint32_t T, uint32_t r)
+{
+    uint32_t lo = 0, hi = T;  // invariant: first_block[lo] <= r (tensor 0 starts at 0), answer in [lo, hi)
+    while (hi - lo > 1) {
+        uint32_t mid = (lo + hi) >> 1;
+        if (__ldg(&tensors[mid].first_block) <= r) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// ---- S3: one 16-byte unit of the header region (wire format v1) -------------------------------------------
+__device__ __forceinline__ uint4 header_unit(const MoveParams& p, uint64_t u, uint32_t T, uint32_t B, uint64_t hb,
+                                             uint64_t P)
+{
+    uint4 v = make_uint4(0, 0, 0, 0);
+    if (u < 4) {
+        if (u == 0) v = make_uint4(0x41505342u, 0x31455352u, 1u, 0x01020304u);  // "BSPARSE1", version, endian_tag
+        else if (u == 1) v = make_uint4(0u, 2u, 3u, 16u);                        // dtype, n_qn, max_rank, align
+        else if (u == 2) v = make_uint4(T, 0u, B, 0u);                           // u64 n_tensors, u64 n_blocks
+        else v = make_uint4((uint32_t)hb, (uint32_t)(hb >> 32), (uint32_t)P, (uint32_t)(P >> 32));
+        return v;
+    }
+    u -= 4;
+    if (u < 2ull * T) {  // tensor records travel byte for byte
+        return __ldg(reinterpret_cast<const uint4*>(p.tensors) + u);
+    }
+    u -= 2ull * T;
+    if (u < 3ull * B) {
+        const uint32_t r = (uint32_t)(u / 3), part = (uint32_t)(u % 3);
+        const int32_t* q = p.qn + 6ull * r;
+        const uint32_t* d = p.dim + 3ull * r;
+        if (part == 0) {
+            int2 a = __ldg(reinterpret_cast<const int2*>(q)), b = __ldg(reinterpret_cast<const int2*>(q + 2));
+            v = make_uint4((uint32_t)a.x, (uint32_t)a.y, (uint32_t)b.x, (uint32_t)b.y);
+        } else if (part == 1) {
+            int2 a = __ldg(reinterpret_cast<const int2*>(q + 4));
+            v = make_uint4((uint32_t)a.x, (uint32_t)a.y, __ldg(d), __ldg(d + 1));
+        } else {
+            const uint64_t off = p.ws.blk[r].off;
+            v = make_uint4(__ldg(d + 2), tensor_of_block(p.tensors, T, r), (uint32_t)off, (uint32_t)(off >> 32));
+        }
+    }
+    return v;  // slack up to header_bytes: zeros
+}
+
+// ---- S7 (descriptor part): one record of the header -> the out descriptor arrays ------------------------------
+__device__ __forceinline__ void rebuild_record(const MoveParams& p, uint64_t rec, uint32_t T, uint32_t B)
+{
+    if (rec < T) {
+        const uint4* s = reinterpret_cast<const uint4*>(p.header + kFixedHeader + kTensorRec * rec);
+        uint4* d = reinterpret_cast<uint4*>(p.tensors + rec);
+        d[0] = __ldg(s);
+        d[1] = __ldg(s + 1);
+        return;
+    }
+    const uint64_t r = rec - T;
+    if (r >= B) return;
+    const uint4* s = reinterpret_cast<const uint4*>(p.header + kFixedHeader + kTensorRec * (uint64_t)T + kBlockRec * r);
+    const uint4 r0 = __ldg(s), r1 = __ldg(s + 1), r2 = __ldg(s + 2);
+    int2* q = reinterpret_cast<int2*>(p.qn + 6 * r);
+    q[0] = make_int2((int)r0.x, (int)r0.y);
+    q[1] = make_int2((int)r0.z, (int)r0.w);
+    q[2] = make_int2((int)r1.x, (int)r1.y);
+    if ((p.flags & 1u) == BS_LAYOUT_POOL) {  // scatter mode: dim / addr are caller inputs, already checked equal
+        p.dim[3 * r + 0] = r1.z;
+        p.dim[3 * r + 1] = r1.w;
+        p.dim[3 * r + 2] = r2.x;
+        p.addr[r] = p.ws.blk[r].addr & ~7ull;
+    }
+}
+
+// largest j in [jlo, jhi] with blk[j].off <= s   (zero-size blocks share an offset with their successor: the
+// last of such a run is the one that owns byte s)
+__device__ __forceinline__ uint32_t find_block(const Blk* __restrict__ blk, uint32_t jlo, uint32_t jhi, uint64_t s)
+{
+    while (jlo < jhi) {
+        const uint32_t mid = jlo + ((jhi - jlo + 1) >> 1);
+        if (__ldg(reinterpret_cast<const unsigned long long*>(&blk[mid].off)) <= s) jlo = mid; else jhi = mid - 1;
+    }
+    return jlo;
+}
+
+constexpr uint32_t kFlagCheckPad = 0x100u;  // unpack: pad bytes must be zero (engine path; see bs_engine.cu)
+
+template <bool UNPACK, int UPT>
+__global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
+{
+    const WsHead* head = p.ws.head;
+    if (head->status != 0) return;  // deferred error: nothing is written
+    const uint32_t T = head->n_tensors, B = head->n_blocks;
+    const uint64_t hb = head->header_bytes, P = head->payload_bytes, total = hb + P;
+    const uint64_t ng = head->n_granules;
+    const uint64_t lo = p.lo, hi = p.hi < total ? p.hi : total;
+    const uint32_t tid = threadIdx.x;
+    constexpr uint64_t kTileUnits = (uint64_t)kThreads * UPT;
+    constexpr uint64_t kTileBytes = kTileUnits * 16;
+
+    // ---- header tiles ----
+    uint64_t nh = 0;
+    if (UNPACK) {
+        if (p.header != nullptr) nh = ((uint64_t)T + B + kTileUnits - 1) / kTileUnits;
+    } else if (lo < hb && lo < hi) {
+        nh = ((hi < hb ? hi : hb) - lo + kTileBytes - 1) / kTileBytes;
+    }
+    // ---- payload tiles: tile k = payload bytes [k*kTileBytes, (k+1)*kTileBytes) ----
+    uint64_t plo = 0, phi = 0, k0 = 0, np = 0;
+    if (hi > hb && hi > lo) {
+        plo = (lo > hb ? lo : hb) - hb;
+        phi = hi - hb;
+        k0 = plo / kTileBytes;
+        np = (phi + kTileBytes - 1) / kTileBytes - k0;
+    }
+    const Blk* __restrict__ blk = p.ws.blk;
+
+    for (uint64_t w = blockIdx.x; w < nh + np; w += gridDim.x) {
+        if (w >= np) {
+            const uint64_t h = w - np;
+            if (UNPACK) {
+#pragma unroll
+                for (int k = 0; k < UPT; ++k) rebuild_record(p, h * kTileUnits + (uint64_t)k * kThreads + tid, T, B);
+            } else {
+                const uint64_t hend = hi < hb ? hi : hb;
+#pragma unroll
+                for (int k = 0; k < UPT; ++k) {
+                    const uint64_t s = lo + (h * kTileUnits + (uint64_t)k * kThreads + tid) * 16;
+                    if (s < hend) st_stream16(p.stream + (s - lo), header_unit(p, s >> 4, T, B, hb, P));
+                }
+            }
+            continue;
+        }
+        const uint64_t tile = k0 + w;
+        const uint64_t tbase = tile * kTileBytes;
+        const uint64_t g0 = tbase / kGranule;
+        uint64_t g1 = (tbase + kTileBytes) / kGranule;
+        if (g1 > ng) g1 = ng;
+        const uint32_t jlo = __ldg(p.ws.tile_first + g0);
+        uint32_t jhi = __ldg(p.ws.tile_first + g1);  // tile_first[ng] == B
+        if (jhi >= B) jhi = B - 1;
+
+        uint64_t src[UPT];   // pack: block address of the unit; unpack: destination address
+        uint32_t kind[UPT];  // 0 skip, 1 full 16 B aligned, 2 full 16 B as 2x8, 3 tail 8 B (+ 8 B pad)
+        uint64_t soff[UPT];
+#pragma unroll
+        for (int k = 0; k < UPT; ++k) {
+            const uint64_t s = tbase + ((uint64_t)k * kThreads + tid) * 16;  // payload offset of the unit
+            soff[k] = s;
+            kind[k] = 0;
+            src[k] = 0;
+            if (s >= plo && s < phi) {
+                const uint32_t j = find_block(blk, jlo, jhi, s);
+                const Blk e = blk[j];
+                const uint64_t next = __ldg(reinterpret_cast<const unsigned long long*>(&blk[j + 1].off));
+                const uint64_t intra = s - e.off;
+                const uint64_t nbytes = (next - e.off) - ((e.addr & 1ull) ? 8 : 0);
+                const uint64_t a = (e.addr & ~7ull) + intra;
+                src[k] = a;
+                kind[k] = (intra + 16 <= nbytes) ? ((a & 15ull) ? 2u : 1u) : 3u;
+            }
+        }
+        if (!UNPACK) {
+            uint4 v[UPT];
+#pragma unroll
+            for (int k = 0; k < UPT; ++k) {
+                v[k] = make_uint4(0, 0, 0, 0);
+                if (kind[k] == 1) v[k] = ld_stream16(reinterpret_cast<const void*>(src[k]));
+                else if (kind[k] == 2) {
+                    uint2 a = ld_stream8(reinterpret_cast<const void*>(src[k]));
+                    uint2 b = ld_stream8(reinterpret_cast<const void*>(src[k] + 8));
+                    v[k] = make_uint4(a.x, a.y, b.x, b.y);
+                } else if (kind[k] == 3) {
+                    uint2 a = ld_stream8(reinterpret_cast<const void*>(src[k]));
+                    v[k] = make_uint4(a.x, a.y, 0u, 0u);  // 8 data bytes + 8 zero pad bytes (D3)
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < UPT; ++k)
+                if (kind[k]) st_stream16(p.stream + (hb + soff[k] - lo), v[k]);
+        } else {
+            uint4 v[UPT];
+#pragma unroll
+            for (int k = 0; k < UPT; ++k)
+                if (kind[k]) v[k] = ld_stream16(p.stream + (hb + soff[k] - lo));
+#pragma unroll
+            for (int k = 0; k < UPT; ++k) {
+                if (kind[k] == 1) st_stream16(reinterpret_cast<void*>(src[k]), v[k]);
+                else if (kind[k] == 2) {
+                    st_stream8(reinterpret_cast<void*>(src[k]), make_uint2(v[k].x, v[k].y));
+                    st_stream8(reinterpret_cast<void*>(src[k] + 8), make_uint2(v[k].z, v[k].w));
+                } else if (kind[k] == 3) {
+                    st_stream8(reinterpret_cast<void*>(src[k]), make_uint2(v[k].x, v[k].y));
+                    if ((p.flags & kFlagCheckPad) && (v[k].z | v[k].w) != 0)
+                        atomicCAS(const_cast<int*>(&head->status), 0, BS_ERR_CORRUPT);
+                }
+            }
+        }
+    }
+}
+
+template <bool UNPACK>
+cudaError_t launch_ldg(const MoveParams& p, const bs_opts& o, int sm_count, cudaStream_t stream)
+{
+    const unsigned per_sm = o.ctas_per_sm ? o.ctas_per_sm : 4;
+    const unsigned grid = (unsigned)sm_count * per_sm;
+    switch (o.tile_bytes) {
+        case 16384: move_kernel<UNPACK, 4><<<grid, kThreads, 0, stream>>>(p); break;
+        case 32768: move_kernel<UNPACK, 8><<<grid, kThreads, 0, stream>>>(p); break;
+        case 49152: move_kernel<UNPACK, 12><<<grid, kThreads, 0, stream>>>(p); break;
+        case 65536: move_kernel<UNPACK, 16><<<grid, kThreads, 0, stream>>>(p); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+void resolve_opts(const bs_opts* in, bs_opts* out)
+{
+    bs_opts o = {0, 0, 0, 0};
+    if (in) o = *in;
+    if (o.variant == BS_VARIANT_DEFAULT) o.variant = BS_VARIANT_LDG;
+    if (o.tile_bytes == 0) o.tile_bytes = 32768;
+    *out = o;
+}
+
+cudaError_t launch_move(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream)
+{
+    return unpack ? launch_ldg<true>(p, opts, sm_count, stream) : launch_ldg<false>(p, opts, sm_count, stream);
+}
+
+}  // namespace bs

@@ -1,0 +1,77 @@
+"""The C-ABI library loads and exports every symbol include/bs.h declares; host-only entry points work without a GPU."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2412_04676_b200 as bs
+from tests.util import read_hex_fixture
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "bs.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    names = re.findall(r"\b(bs_[a-z0-9_]+)\s*\(", src)
+    return sorted(set(names))
+
+
+def test_every_declared_symbol_is_exported():
+    lib = bs.lib()
+    names = declared_functions()
+    assert {"bs_serialize", "bs_deserialize", "bs_offload_async", "bs_prefetch_async", "bs_serialized_size",
+            "bs_stream_info", "bs_engine_create", "bs_ticket_wait"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/bs.h but not exported"
+
+
+def test_struct_layouts_match_the_header():
+    assert ctypes.sizeof(bs.SetDesc) == 48
+    assert ctypes.sizeof(bs.Result) == 64
+    assert ctypes.sizeof(bs.Opts) == 16
+
+
+def test_host_only_entry_points():
+    assert bs.version() == 0x00010000
+    assert bs.header_bytes(1, 2) == 256 and bs.header_bytes(0, 0) == 128
+    assert bs.header_bytes(2000, 446140) == (64 + 32 * 2000 + 48 * 446140 + 127) // 128 * 128
+    assert bs.workspace_bytes(1, 7, 1 << 20) % 256 == 0
+    assert bs.workspace_bytes(9008, 3299211, 45 << 30) < 200 << 20      # O(B) + 4 B per 16 KiB of stream
+    raw = read_hex_fixture(os.path.join(ROOT, "tests", "golden", "p7_golden_stream.hex"))
+    assert bs.stream_info(raw) == dict(n_tensors=1, n_blocks=2, header_bytes=256, payload_bytes=32, total_bytes=288)
+    for pos in (0, 8, 12, 16, 20, 24, 28, 48):
+        bad = bytearray(raw)
+        bad[pos] ^= 1
+        with pytest.raises(bs.BsError) as e:
+            bs.stream_info(bad)
+        assert e.value.code == bs.ERR_CORRUPT
+    assert "corrupt" in bs.strerror(bs.ERR_CORRUPT) and bs.strerror(0) == "ok"
+
+
+def test_argument_errors_need_no_device():
+    d = bs.make_desc(1, 1, 16, 16, 16, 16)
+    d.n_qn = 3
+    with pytest.raises(bs.BsError) as e:
+        bs.serialize(d, 256, 1024, 256, 1 << 20, 0)
+    assert e.value.code == bs.ERR_UNSUPPORTED
+    d = bs.make_desc(1, 1, 8, 16, 16, 16)          # tensors not 16-byte aligned
+    with pytest.raises(bs.BsError) as e:
+        bs.serialize(d, 256, 1024, 256, 1 << 20, 0)
+    assert e.value.code == bs.ERR_ARG
+    d = bs.make_desc(1, 1, 16, 16, 16, 16)
+    with pytest.raises(bs.BsError) as e:
+        bs.serialize(d, 256, 1024, 256, 64, 0)     # workspace too small
+    assert e.value.code == bs.ERR_CAPACITY
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("box has a GPU")
+    d = bs.make_desc(0, 0, 0, 0, 0, 0)
+    with pytest.raises(bs.BsError) as e:
+        bs.serialize(d, 256, 1024, 256, 1 << 20, 0)
+    assert e.value.code == bs.ERR_CUDA

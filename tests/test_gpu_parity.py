@@ -1,0 +1,317 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle: bit-exact, tolerance 0.
+Every test here needs a GPU.  Inputs: seeded synthetic sets (workloads/), never a value from the CUDA path."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2412_04676_b200 as bs
+import workloads as W
+from tests.gpu_util import DEV, Uploaded, gpu_deserialize, gpu_serialize
+from tests.streamreader import read_stream
+from tests.util import host_addrs, oracle_stream
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = [dict(variant=bs.VARIANT_LDG, tile_bytes=16384), dict(variant=bs.VARIANT_LDG, tile_bytes=32768),
+            dict(variant=bs.VARIANT_LDG, tile_bytes=49152), dict(variant=bs.VARIANT_LDG, tile_bytes=65536, ctas_per_sm=1),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=16384), dict(variant=bs.VARIANT_TMA, tile_bytes=32768),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=65536, ctas_per_sm=1)]
+
+
+def small_sets():
+    return [W.make_config("1"), W.make_config("2"),
+            W.make_set("tiny-ops+site", 11, D=48, S=10, M=2, N0=2, n_ops=20, n_site=2, dims="multinomial"),
+            W.make_set("lognormal", 12, D=300, S=30, M=4, N0=3, n_ops=40, n_site=2, dims="lognormal", sigma=1.0)]
+
+
+def check_stream(bset, up, opts=None, slack=4096):
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    total = len(want)
+    got_t, res = gpu_serialize(up.dset, total + slack, opts)
+    assert res["status"] == bs.OK, res
+    hb, tot = oracle.serialized_size(bset.n_tensors, bset.dim)
+    assert (res["header_bytes"], res["total_bytes"], res["payload_bytes"]) == (hb, tot, tot - hb)
+    got = got_t.cpu().numpy()
+    bad = np.nonzero(got[:total] != want)[0]
+    assert bad.size == 0, f"first mismatch at stream byte {bad[0]} (header_bytes={hb}), opts={opts}"
+    assert (got[total:] == 0xCD).all(), "bytes beyond the stream were written"
+    return got_t, want
+
+
+@pytest.mark.parametrize("bset", small_sets(), ids=lambda s: s.name)
+def test_serialize_matches_oracle_byte_for_byte(bset):
+    up = Uploaded(bset)
+    check_stream(bset, up)
+
+
+@pytest.mark.parametrize("opts", VARIANTS, ids=lambda o: f"v{o['variant']}-t{o['tile_bytes']}-c{o.get('ctas_per_sm', 0)}")
+def test_P6_stream_independent_of_decomposition(opts):
+    for bset in (W.make_config("2"), W.make_set("lognormal", 12, D=300, S=30, M=4, N0=3, n_ops=40, n_site=2,
+                                                dims="lognormal", sigma=1.0)):
+        up = Uploaded(bset)
+        check_stream(bset, up, opts)
+
+
+@pytest.mark.parametrize("bset", small_sets(), ids=lambda s: s.name)
+def test_deserialize_matches_oracle_and_round_trips(bset):
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    ref = oracle.deserialize(want)                       # pool poisoned 0xEE, as on the GPU side
+    stream_t = torch.from_numpy(want.copy()).to(DEV)
+    need = oracle.pool_bytes(want)
+    out, pool, res = gpu_deserialize(stream_t, len(want), bset.n_tensors, bset.n_blocks, need)
+    assert res["status"] == bs.OK, res
+    assert (res["n_tensors"], res["n_blocks"], res["pool_bytes"]) == (bset.n_tensors, bset.n_blocks, need)
+    h = out.to_host()
+    assert h["tensors"].tobytes() == ref["tensors"].tobytes() == bset.tensors.tobytes()
+    assert (h["qn"] == ref["qn"]).all() and (h["dim"] == ref["dim"]).all()
+    # D14 placement: same pool-relative addresses as the oracle, and byte-identical pools (untouched bytes included)
+    assert ((h["addr"] - np.uint64(pool.data_ptr())) == (ref["addr"] - np.uint64(ref["pool"].ctypes.data))).all()
+    gp = pool.cpu().numpy()
+    assert (gp[:need] == ref["pool"][:need]).all()
+    # fixpoint on the device: serialize(deserialize(S)) == S
+    again, res2 = gpu_serialize(out, len(want))
+    assert res2["status"] == bs.OK
+    assert (again.cpu().numpy()[:len(want)] == want).all()
+
+
+@pytest.mark.parametrize("opts", VARIANTS, ids=lambda o: f"v{o['variant']}-t{o['tile_bytes']}-c{o.get('ctas_per_sm', 0)}")
+def test_P6_unpack_independent_of_decomposition(opts):
+    bset = W.make_set("lognormal", 12, D=300, S=30, M=4, N0=3, n_ops=40, n_site=2, dims="lognormal", sigma=1.0)
+    want, _, _ = oracle_stream(bset)
+    ref = oracle.deserialize(want)
+    need = oracle.pool_bytes(want)
+    out, pool, res = gpu_deserialize(torch.from_numpy(want.copy()).to(DEV), len(want), bset.n_tensors, bset.n_blocks,
+                                     need, opts=opts)
+    assert res["status"] == bs.OK
+    assert (pool.cpu().numpy()[:need] == ref["pool"][:need]).all()
+
+
+@pytest.mark.parametrize("chunk", [16, 4096, 65536, 100000 * 16, 1 << 22])
+def test_P6_concat_of_ranges_is_the_stream(chunk):
+    bset = W.make_config("2")
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    total = len(want)
+    if chunk == 16:      # byte-granular ranges only around the header/payload boundary (keeps the test fast)
+        hb = oracle.header_bytes(bset.n_tensors, bset.n_blocks)
+        cuts = [0] + list(range(hb - 64, hb + 64, 16)) + [total]
+    else:
+        cuts = list(range(0, total, chunk)) + [total]
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, total, DEV)
+    out = torch.full((total,), 0xCD, dtype=torch.uint8, device=DEV)
+    first = True
+    for lo, hi in zip(cuts[:-1], cuts[1:]):
+        seg = torch.full((hi - lo + 32,), 0x77, dtype=torch.uint8, device=DEV)
+        bs.serialize_range(up.dset.desc, seg.data_ptr(), lo, hi, first, ws.ptr, ws.nbytes, ws.result_ptr, None,
+                           bs.current_stream())
+        first = False
+        assert (seg[hi - lo:] == 0x77).all(), "range call wrote beyond its segment"
+        out[lo:hi] = seg[:hi - lo]
+    assert ws.read_result()["status"] == bs.OK
+    assert (out.cpu().numpy() == want).all()
+
+
+def test_serialized_size_is_exact_prediction():
+    for bset in small_sets():
+        up = Uploaded(bset)
+        ws = bs.Workspace(bset.n_tensors, bset.n_blocks, 1 << 16, DEV)     # tile index far too small: still exact
+        hb, tot = bs.serialized_size(up.dset.desc, ws.ptr, ws.nbytes, bs.current_stream())
+        assert (hb, tot) == oracle.serialized_size(bset.n_tensors, bset.dim)
+
+
+# ---- edge cases ---------------------------------------------------------------------------------------------
+def _custom(tensor_rows, dim, data, qn=None):
+    tensors = np.zeros(len(tensor_rows), dtype=W.TENSOR_REC_DTYPE)
+    for i, r in enumerate(tensor_rows):
+        tensors[i] = r
+    dim = np.array(dim, np.uint32).reshape(-1, 3)
+    B = len(dim)
+    qn = np.zeros((B, 3, 2), np.int32) if qn is None else qn
+    ne = dim.astype(np.int64).prod(axis=1)
+    offs = np.zeros(B, np.uint64)
+    sz = (ne * 8 + 511) // 512 * 512
+    if B > 1:
+        offs[1:] = np.cumsum(sz[:-1])
+    pool = np.zeros(max(int(sz.sum()) // 8, 1))
+    for i in range(B):
+        pool[int(offs[i]) // 8: int(offs[i]) // 8 + int(ne[i])] = data[i]
+    bset = W.BlockSparseSet("custom", 0, tensors, qn, dim, offs, pool.nbytes)
+    return bset, pool, offs
+
+
+def test_D11_empty_set():
+    bset, pool, offs = _custom([], np.zeros((0, 3)), [])
+    up = Uploaded(bset, pool, offs)
+    got, want = check_stream(bset, up)
+    assert len(want) == 128
+    out, p, res = gpu_deserialize(got, 128, 0, 0, 0)
+    assert res["status"] == bs.OK and res["n_blocks"] == 0
+
+
+def test_D11_zero_extent_blocks_and_empty_tensors():
+    rows = [(2, 0, 2, (0, 0), (-1, 1, 0, 0), 0, 0), (3, 2, 0, (0, 0), (1, 1, -1, 0), 1, 0),
+            (2, 2, 3, (0, 0), (-1, 1, 0, 0), 2, 0)]
+    dim = [[0, 5, 1], [3, 1, 1], [2, 0, 1], [0, 0, 1], [1, 1, 1]]
+    bset, pool, offs = _custom(rows, dim, [[], [1., 2., 3.], [], [], [4.]])
+    up = Uploaded(bset, pool, offs)
+    got, want = check_stream(bset, up)
+    out, p, res = gpu_deserialize(got, len(want), 3, 5, oracle.pool_bytes(want))
+    assert res["status"] == bs.OK
+    ref = oracle.deserialize(want)
+    assert (p.cpu().numpy()[:len(ref["pool"])] == ref["pool"]).all()
+    assert (out.to_host()["dim"] == bset.dim).all()
+
+
+def test_many_tiny_blocks_per_tile():
+    # 1x1 blocks: 16 stored bytes each -> 2048 blocks per 32 KiB tile, every unit is a tail unit
+    B = 9000
+    rng = np.random.default_rng(1)
+    dim = np.ones((B, 3), np.int64)
+    dim[::7, 1] = 2
+    dim[::11, 0] = 3
+    data = [rng.uniform(-1, 1, int(d.prod())) for d in dim]
+    bset, pool, offs = _custom([(2, 0, B, (0, 0), (-1, 1, 0, 0), 0, 0)], dim, data)
+    up = Uploaded(bset, pool, offs)
+    for opts in (None, dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
+        got, want = check_stream(bset, up, opts)
+        out, p, res = gpu_deserialize(got, len(want), 1, B, oracle.pool_bytes(want), opts=opts)
+        assert res["status"] == bs.OK
+        ref = oracle.deserialize(want)
+        assert (p.cpu().numpy()[:len(ref["pool"])] == ref["pool"]).all()
+
+
+def test_one_huge_block_and_neighbours():
+    rng = np.random.default_rng(2)
+    dim = [[3, 3, 1], [1500, 1501, 1], [5, 1, 7]]           # 18 MB block: thousands of tiles, odd element count
+    data = [rng.uniform(-1, 1, int(np.prod(d))) for d in dim]
+    bset, pool, offs = _custom([(2, 0, 2, (0, 0), (-1, 1, 0, 0), 0, 0), (3, 2, 1, (0, 0), (1, 1, -1, 0), 1, 0)], dim, data)
+    up = Uploaded(bset, pool, offs)
+    for opts in (None, dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
+        got, want = check_stream(bset, up, opts)
+        out, p, res = gpu_deserialize(got, len(want), 2, 3, oracle.pool_bytes(want), opts=opts)
+        ref = oracle.deserialize(want)
+        assert res["status"] == bs.OK and (p.cpu().numpy()[:len(ref["pool"])] == ref["pool"]).all()
+
+
+def test_D16_eight_byte_aligned_sources_take_the_slow_path():
+    bset = W.make_set("mis", 13, D=120, S=12, M=2, N0=3, n_ops=13, n_site=1, dims="multinomial")
+    up = Uploaded(bset, misalign=8)
+    assert (up.addr % 16 == 8).all()
+    for opts in (None, dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
+        check_stream(bset, up, opts)
+    # and scatter back to 8-byte-aligned destinations
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    dst = torch.full((up.pool.numel(),), 0xEE, dtype=torch.uint8, device=DEV)
+    daddr = (np.uint64(dst.data_ptr() + 8) + up.host_offs).astype(np.uint64)
+    out = bs.DeviceSet.from_host(np.zeros(bset.n_tensors, W.TENSOR_REC_DTYPE), np.zeros_like(bset.qn), bset.dim, daddr, DEV)
+    for opts in (None, dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
+        dst.fill_(0xEE)
+        ws = bs.Workspace(bset.n_tensors, bset.n_blocks, len(want), DEV)
+        st = torch.from_numpy(want.copy()).to(DEV)
+        bs.deserialize(st.data_ptr(), len(want), out.desc, 0, 0, bs.SCATTER_TO_ADDR, ws.ptr, ws.nbytes, ws.result_ptr, opts,
+                       bs.current_stream())
+        assert ws.read_result()["status"] == bs.OK
+        got = dst.cpu().numpy()
+        src = up.host_pool.view(np.uint8)
+        ne = bset.nelems
+        expect = np.full_like(got, 0xEE)
+        for i in range(bset.n_blocks):
+            o, n = int(up.host_offs[i]), int(ne[i]) * 8
+            expect[8 + o: 8 + o + n] = src[o:o + n]
+        assert (got == expect).all()
+        assert out.to_host()["tensors"].tobytes() == bset.tensors.tobytes()
+
+
+def test_P11_special_bit_patterns():
+    pats = np.array([0x7FF8000000000001, 0xFFF0000000000000, 0x8000000000000000, 0x0000000000000001,
+                     0x7FF0000000000000, 0x7FF4DEADBEEF0001, 0x000FFFFFFFFFFFFF], dtype=np.uint64)
+    bset, pool, offs = _custom([(2, 0, 1, (0, 0), (-1, 1, 0, 0), 0, 0)], [[1, 7, 1]], [pats.view(np.float64)])
+    assert (pool.view(np.uint64)[:7] == pats).all()
+    up = Uploaded(bset, pool, offs)
+    got, want = check_stream(bset, up)
+    out, p, res = gpu_deserialize(got, len(want), 1, 1, 256)
+    assert (p.cpu().numpy()[:56].view(np.uint64) == pats).all()
+
+
+# ---- deferred errors -------------------------------------------------------------------------------------------
+def test_capacity_error_reports_required_size_and_writes_nothing():
+    bset = W.make_config("1")
+    up = Uploaded(bset)
+    hb, tot = oracle.serialized_size(1, bset.dim)
+    out, res = gpu_serialize(up.dset, tot - 16)
+    assert res["status"] == bs.ERR_CAPACITY and res["total_bytes"] == tot
+    assert (out == 0xCD).all()
+
+
+def test_bad_descriptors_are_rejected_on_the_device():
+    bset = W.make_config("1")
+    up = Uploaded(bset)
+    t = bset.tensors.copy()
+    t["n_blocks"][0] -= 1
+    d = bs.DeviceSet.from_host(t, bset.qn, bset.dim, up.addr, DEV)
+    out, res = gpu_serialize(d, 1 << 16)
+    assert res["status"] == bs.ERR_ARG and (out == 0xCD).all()
+    t = bset.tensors.copy()
+    t["rank"][0] = 4
+    d = bs.DeviceSet.from_host(t, bset.qn, bset.dim, up.addr, DEV)
+    out, res = gpu_serialize(d, 1 << 16)
+    assert res["status"] == bs.ERR_UNSUPPORTED and (out == 0xCD).all()
+    a = up.addr.copy()
+    a[3] += 4
+    d = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, a, DEV)
+    out, res = gpu_serialize(d, 1 << 16)
+    assert res["status"] == bs.ERR_ARG and (out == 0xCD).all()
+    # host-side argument errors are immediate
+    with pytest.raises(bs.BsError) as e:
+        bs.serialize(up.dset.desc, 8, 1 << 16, 0, 0, 0, None, 0)
+    assert e.value.code == bs.ERR_ARG
+
+
+def test_P10_corrupt_headers_are_rejected_and_nothing_is_written():
+    from tests.test_oracle_invariants import _mutations
+    bset = W.make_set("fault", 41, D=40, S=9, M=2, N0=3, n_ops=13, n_site=1, dims="multinomial")
+    want, _, _ = oracle_stream(bset)
+    need = oracle.pool_bytes(want)
+    cases = [(name, pos, xor, len(want)) for name, pos, xor in _mutations(want, bset)]
+    for name, pos, xor, n in cases:
+        bad = want.copy()
+        bad[pos] ^= xor
+        assert oracle.validate_stream(bad) == oracle.ERR_CORRUPT
+        out, pool, res = gpu_deserialize(torch.from_numpy(bad).to(DEV), n, bset.n_tensors + 1, bset.n_blocks + 1, need + 4096)
+        assert res["status"] == bs.ERR_CORRUPT, (name, res)
+        assert (pool == 0xEE).all(), f"{name}: pool written despite corrupt header"
+        for arr in (out.tensors, out.qn, out.dim, out.addr):
+            assert (arr == 0xAB).all(), f"{name}: descriptor written despite corrupt header"
+    st = torch.from_numpy(want.copy()).to(DEV)
+    for n in (len(want) - 16, 48):
+        out, pool, res = gpu_deserialize(st, n, bset.n_tensors, bset.n_blocks, need)
+        assert res["status"] == bs.ERR_CORRUPT and (pool == 0xEE).all()
+
+
+def test_deserialize_capacity_errors():
+    bset = W.make_set("cap", 42, D=40, S=9, M=2, N0=3, n_ops=13, n_site=1, dims="multinomial")
+    want, _, _ = oracle_stream(bset)
+    need = oracle.pool_bytes(want)
+    st = torch.from_numpy(want.copy()).to(DEV)
+    out, pool, res = gpu_deserialize(st, len(want), bset.n_tensors, bset.n_blocks, need - 256)
+    assert res["status"] == bs.ERR_CAPACITY and res["pool_bytes"] == need and (pool == 0xEE).all()
+    out, pool, res = gpu_deserialize(st, len(want), bset.n_tensors, bset.n_blocks - 1, need)
+    assert res["status"] == bs.ERR_CAPACITY and res["n_blocks"] == bset.n_blocks and (pool == 0xEE).all()
+
+
+def test_scatter_extent_mismatch_is_an_argument_error():
+    bset = W.make_set("scat", 51, D=30, S=8, M=2, N0=3, n_ops=5, n_site=0, dims="multinomial")
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    wrong = bset.dim.copy()
+    wrong[0, 0] += 1
+    dst = torch.full((up.pool.numel(),), 0xEE, dtype=torch.uint8, device=DEV)
+    daddr = (np.uint64(dst.data_ptr()) + up.host_offs).astype(np.uint64)
+    out = bs.DeviceSet.from_host(np.zeros(bset.n_tensors, W.TENSOR_REC_DTYPE), np.zeros_like(bset.qn), wrong, daddr, DEV)
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, len(want), DEV)
+    st = torch.from_numpy(want.copy()).to(DEV)
+    bs.deserialize(st.data_ptr(), len(want), out.desc, 0, 0, bs.SCATTER_TO_ADDR, ws.ptr, ws.nbytes, ws.result_ptr, None,
+                   bs.current_stream())
+    assert ws.read_result()["status"] == bs.ERR_ARG and (dst == 0xEE).all()
