@@ -221,6 +221,8 @@ int bs_prefetch_async(bs_engine *e, const void *h_pinned, uint64_t nbytes, bs_se
 
 int bs_ticket_wait(bs_ticket *t, bs_ticket_stats *stats /* may be NULL */); /* blocks the host; returns the deferred status */
 int bs_ticket_query(const bs_ticket *t);                                   /* BS_OK | BS_PENDING | BS_ERR_* */
+int bs_ticket_stream_wait(const bs_ticket *t, cudaStream_t stream);        /* make `stream` wait for completion (no host block):
+                                                                               after an offload the blocks may be overwritten */
 int bs_ticket_destroy(bs_ticket *t);                                       /* after completion */
 
 #ifdef __cplusplus

@@ -96,6 +96,7 @@ def lib():
     L.bs_ticket_wait.argtypes = [vp, C.POINTER(TicketStats)]
     L.bs_ticket_query.argtypes = [vp]
     L.bs_ticket_destroy.argtypes = [vp]
+    L.bs_ticket_stream_wait.argtypes = [vp, vp]
     _lib = L
     return L
 
@@ -183,6 +184,9 @@ class Ticket:
         out = dict(status=int(rc), bytes=int(st.bytes), n_chunks=int(st.n_chunks), dma_ms=float(st.dma_ms),
                    total_ms=float(st.total_ms))
         return out
+
+    def stream_wait(self, stream: int) -> None:
+        _check(lib().bs_ticket_stream_wait(self._h, stream), "bs_ticket_stream_wait")
 
     def destroy(self):
         if self._h:

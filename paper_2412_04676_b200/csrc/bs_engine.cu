@@ -289,6 +289,13 @@ int bs_ticket_wait(bs_ticket* t, bs_ticket_stats* stats)
     return t->h_result->status;
 }
 
+int bs_ticket_stream_wait(const bs_ticket* t, cudaStream_t stream)
+{
+    if (t == nullptr) return BS_ERR_ARG;
+    CK(cudaStreamWaitEvent(stream, t->done, 0));
+    return BS_OK;
+}
+
 int bs_ticket_destroy(bs_ticket* t)
 {
     if (t == nullptr) return BS_ERR_ARG;

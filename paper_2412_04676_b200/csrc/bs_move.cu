@@ -227,19 +227,33 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
     }
 }
 
+// persistent grid: exactly one wave of resident CTAs (SM count x occupancy), tiles dealt round-robin
+template <bool UNPACK, int UPT>
+cudaError_t launch_ldg_upt(const MoveParams& p, const bs_opts& o, int sm_count, cudaStream_t stream)
+{
+    static int occ = 0;  // per kernel instantiation
+    if (occ == 0) {
+        int n = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, move_kernel<UNPACK, UPT>, (int)kThreads, 0);
+        if (e != cudaSuccess) return e;
+        occ = n > 0 ? n : 1;
+    }
+    unsigned per_sm = (unsigned)occ;
+    if (o.ctas_per_sm && o.ctas_per_sm < per_sm) per_sm = o.ctas_per_sm;
+    move_kernel<UNPACK, UPT><<<(unsigned)sm_count * per_sm, kThreads, 0, stream>>>(p);
+    return cudaGetLastError();
+}
+
 template <bool UNPACK>
 cudaError_t launch_ldg(const MoveParams& p, const bs_opts& o, int sm_count, cudaStream_t stream)
 {
-    const unsigned per_sm = o.ctas_per_sm ? o.ctas_per_sm : 4;
-    const unsigned grid = (unsigned)sm_count * per_sm;
     switch (o.tile_bytes) {
-        case 16384: move_kernel<UNPACK, 4><<<grid, kThreads, 0, stream>>>(p); break;
-        case 32768: move_kernel<UNPACK, 8><<<grid, kThreads, 0, stream>>>(p); break;
-        case 49152: move_kernel<UNPACK, 12><<<grid, kThreads, 0, stream>>>(p); break;
-        case 65536: move_kernel<UNPACK, 16><<<grid, kThreads, 0, stream>>>(p); break;
+        case 16384: return launch_ldg_upt<UNPACK, 4>(p, o, sm_count, stream);
+        case 32768: return launch_ldg_upt<UNPACK, 8>(p, o, sm_count, stream);
+        case 49152: return launch_ldg_upt<UNPACK, 12>(p, o, sm_count, stream);
+        case 65536: return launch_ldg_upt<UNPACK, 16>(p, o, sm_count, stream);
         default: return cudaErrorInvalidValue;
     }
-    return cudaGetLastError();
 }
 
 }  // namespace
