@@ -57,6 +57,19 @@ def measured_peaks():
     return {"hbm_gbs": FALLBACK_HBM_GBS}, "fallback"
 
 
+def committed_traffic(key: str):
+    """dram__bytes_read + dram__bytes_write per launch from the committed ncu capture (profiles/traffic.csv), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        import csv
+        for row in csv.DictReader(open(p)):
+            if row["key"] == key:
+                return int(row["traffic_bytes"])
+    except Exception:
+        pass
+    return None
+
+
 # ---- rank plumbing (pure host logic; covered by tests/test_bench_dist.py with gloo) ---------------------------
 def dist_env():
     return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
@@ -302,12 +315,7 @@ def run_mine(args):
                 "unit": "GB/s", "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": None,
                 "algorithmic_bytes_per_launch": int(algo_bytes), "kernel_ms": round(pack_ms, 4),
                 "frac_of_nominal_8TBs": round(achieved / 8000.0, 4)}
-    tr = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
-    if os.path.exists(tr):
-        try:
-            roofline["traffic"] = json.load(open(tr)).get(f"pack:{args.workload}")
-        except Exception:
-            pass
+    roofline["traffic"] = committed_traffic(f"pack:{args.workload}")
 
     # ---- e2e leg: host (pinned) buffers through the engine, copies inside the timed region ----
     detail = {"serialize_ms": round(float(np.median(ser_ms)), 4), "deserialize_ms": round(float(np.median(des_ms)), 4),
