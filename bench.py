@@ -223,8 +223,9 @@ def run_mine(args):
         dist.init_process_group("nccl", device_id=torch.device(dev))
         ready = True
     opts = None
-    if args.variant or args.tile_bytes or args.ctas_per_sm:
-        opts = dict(variant=args.variant, tile_bytes=args.tile_bytes, ctas_per_sm=args.ctas_per_sm)
+    if args.variant or args.tile_bytes or args.ctas_per_sm or args.stages or args.warps:
+        opts = dict(variant=args.variant, tile_bytes=args.tile_bytes, ctas_per_sm=args.ctas_per_sm, stages=args.stages,
+                    warps=args.warps)
 
     def ev():
         return torch.cuda.Event(enable_timing=True)
@@ -484,6 +485,8 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--tile-bytes", type=int, default=0)
     ap.add_argument("--ctas-per-sm", type=int, default=0)
+    ap.add_argument("--stages", type=int, default=0)
+    ap.add_argument("--warps", type=int, default=0)
     ap.add_argument("--chunk-mb", type=int, default=256)
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--sample-mb", type=float, default=400.0, help="payload of the oracle's bounded sample")

@@ -43,7 +43,18 @@ class StreamInfo(C.Structure):
 
 
 class Opts(C.Structure):
-    _fields_ = [("variant", C.c_uint32), ("tile_bytes", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("reserved", C.c_uint32)]
+    _fields_ = [("variant", C.c_uint32), ("tile_bytes", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("stages", C.c_uint32),
+                ("warps", C.c_uint32), ("reserved", C.c_uint32 * 3)]
+
+
+def make_opts(opts) -> "Opts":
+    """dict / Opts / None -> Opts (zeros = library defaults)."""
+    if isinstance(opts, Opts):
+        return opts
+    o = Opts()
+    for k in ("variant", "tile_bytes", "ctas_per_sm", "stages", "warps"):
+        setattr(o, k, int((opts or {}).get(k, 0) or 0))
+    return o
 
 
 class EngineCfg(C.Structure):
@@ -110,9 +121,7 @@ def _check(rc: int, what: str) -> int:
 def _opts(opts):
     if opts is None:
         return None
-    if isinstance(opts, Opts):
-        return C.byref(opts)
-    return C.byref(Opts(int(opts.get("variant", 0)), int(opts.get("tile_bytes", 0)), int(opts.get("ctas_per_sm", 0)), 0))
+    return C.byref(make_opts(opts))
 
 
 def version() -> int:
@@ -205,9 +214,7 @@ class Engine:
 
     def __init__(self, max_tensors: int, max_blocks: int, max_stream_bytes: int, chunk_bytes: int = 0, n_staging: int = 0,
                  opts=None):
-        o = Opts()
-        if opts:
-            o = Opts(int(opts.get("variant", 0)), int(opts.get("tile_bytes", 0)), int(opts.get("ctas_per_sm", 0)), 0)
+        o = make_opts(opts)
         cfg = EngineCfg(chunk_bytes, n_staging, max_tensors, max_blocks, max_stream_bytes, o)
         h = C.c_void_p(0)
         _check(lib().bs_engine_create(C.byref(h), C.byref(cfg)), "bs_engine_create")

@@ -49,6 +49,10 @@ static int check_opts(const bs_opts& o)
     if (o.variant != BS_VARIANT_LDG && o.variant != BS_VARIANT_TMA) return BS_ERR_ARG;
     if (o.tile_bytes == 0 || o.tile_bytes % kGranule != 0 || o.tile_bytes > 65536) return BS_ERR_ARG;
     if (o.ctas_per_sm > 32) return BS_ERR_ARG;
+    if (o.variant == BS_VARIANT_TMA &&
+        (o.stages < 3 || o.stages > 8 || o.warps < 1 || o.warps > 16 ||
+         (uint64_t)o.stages * o.warps * o.tile_bytes > 225u * 1024u))
+        return BS_ERR_ARG;
     return BS_OK;
 }
 

@@ -116,6 +116,7 @@ struct MoveParams {
 };
 
 cudaError_t launch_move(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream);
+cudaError_t launch_move_tma(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream);
 
 void resolve_opts(const bs_opts* in, bs_opts* out);
 

@@ -1,0 +1,360 @@
+// bs_move_tma.cu — data movement through the TMA bulk-copy engine: steps S3 + S5 (header write + pack) and
+// S7 (descriptor rebuild + unpack / scatter) of SURVEY §8(a), variant BS_VARIANT_TMA.
+//
+// every worker owns an exact, disjoint interval of the one output buffer and fills it "in complete
+// independence".  Here a worker is one WARP and its interval is a TILE of the stream (tile_bytes of payload,
+// whatever blocks lie in it; see bs_move.cu for why tiles and not blocks are the unit).  A tile never touches the
+// register file:
+//
+//   pack   : for every block segment inside the tile, one lane issues   cp.async.bulk global -> shared
+//            (completion counted in bytes on the stage's mbarrier); the 8 data bytes + 8 zero pad bytes that end
+//            an odd-sized block are one zero-filling 16-byte cp.async; when the stage is full ONE
+//            cp.async.bulk shared -> global writes the whole tile (the stream side is contiguous).
+//   unpack : ONE cp.async.bulk global -> shared brings the tile in; then one cp.async.bulk shared -> global per
+//            block segment; the last 8 bytes of an odd-sized block are a plain 8-byte store (the pad bytes of
+//            the stream must not be written past the end of a destination block).
+//
+// Each warp runs its own ring of `stages` tiles in dynamic shared memory (software pipeline: tile i is loaded while
+// tile i-(stages-2) is stored), `warps` rings per CTA, one persistent CTA per SM; tiles are dealt round-robin over
+// all warps of the grid.  Blocks whose address is only 8-byte aligned take a correct slower path of
+// 8-byte cp.async / 8-byte stores.  The stream produced is byte-identical to the LDG variant's (tests: P6).
+//
+// Roofline: pure data movement — 1 byte read + 1 byte written per stream byte, HBM-bound; ~2 instructions per
+// block segment and per tile instead of ~70 per 512 bytes in the LDG variant.
+#include "bs_move_common.cuh"
+
+namespace bs {
+
+namespace {
+
+constexpr uint32_t kMaxWarps = 16;
+constexpr uint32_t kMaxStages = 8;
+constexpr uint32_t kSmemLimit = 227u * 1024u;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+// the mbarrier also waits for every cp.async this thread has issued so far (pending count +1 now, -1 on completion)
+__device__ __forceinline__ void cp_async_mbar_arrive(uint32_t bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read()
+{
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// 8 data bytes + 8 zero bytes (the tail of an odd-sized block and its pad)
+__device__ __forceinline__ void cp_async_tail16(uint32_t dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16, 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_8(uint32_t dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+
+struct Seg {          // intersection of one block with one tile, payload coordinates
+    uint64_t lo;      // first payload byte
+    uint32_t bulk;    // bytes movable as one 16-byte-granular copy (whole 16-byte units of block data)
+    uint32_t tail;    // 1: the segment ends with the 8 data + 8 pad bytes of an odd-sized block
+    uint64_t addr;    // device address of the block byte that maps to payload byte `lo`
+};
+
+// block entry (e, next = offset of block j+1) clipped to [tlo, thi).  Returns false when the intersection is empty
+// (zero-size blocks, clipped tiles).
+__device__ __forceinline__ bool clip_seg(const Blk& e, uint64_t next, uint64_t tlo, uint64_t thi, Seg* s)
+{
+    const uint64_t lo = e.off > tlo ? e.off : tlo;
+    const uint64_t hi = next < thi ? next : thi;
+    if (hi <= lo) return false;
+    const bool odd = (e.addr & 1ull) != 0;
+    s->lo = lo;
+    s->addr = (e.addr & ~7ull) + (lo - e.off);
+    s->tail = (odd && hi == next) ? 1u : 0u;
+    s->bulk = (uint32_t)(hi - lo) - (s->tail ? 16u : 0u);
+    return true;
+}
+__device__ __forceinline__ bool make_seg(const Blk* __restrict__ blk, uint32_t j, uint64_t tlo, uint64_t thi, Seg* s)
+{
+    const Blk e = blk[j];
+    const uint64_t next = __ldg(reinterpret_cast<const unsigned long long*>(&blk[j + 1].off));
+    return clip_seg(e, next, tlo, thi, s);
+}
+
+struct TileIdx {  // blocks jlo..jhi may intersect the tile (jhi < jlo: none / no such tile)
+    uint32_t jlo, jhi;
+};
+struct LaneBlk {  // table entry of block jlo + lane, fetched one tile ahead
+    Blk e;
+    uint64_t next;
+};
+
+// pack: stage one block segment.  Bulk part: counted in *tx, issued later (after the expect_tx); 8-byte-aligned
+// blocks (D16) and odd tails: cp.async now.  Returns the number of cp.async groups this lane started.
+__device__ __forceinline__ uint32_t pack_seg_async(const Seg& s, uint32_t d, uint32_t* tx)
+{
+    uint32_t n_async = 0;
+    if (s.addr & 15ull) {  // D16 slow path: 8-byte pieces; the pad is a plain shared store
+        const uint32_t nb = s.bulk + (s.tail ? 8u : 0u);
+        for (uint32_t b = 0; b < nb; b += 8) cp_async_8(d + b, reinterpret_cast<const void*>(s.addr + b));
+        n_async += nb ? 1u : 0u;
+        if (s.tail) {
+            asm volatile("st.shared.u64 [%0], %1;" ::"r"(d + s.bulk + 8), "l"(0ull) : "memory");
+            fence_proxy_async();
+        }
+    } else {
+        *tx += s.bulk;
+        if (s.tail) {
+            cp_async_tail16(d + s.bulk, reinterpret_cast<const void*>(s.addr + s.bulk));
+            ++n_async;
+        }
+    }
+    return n_async;
+}
+
+// unpack: scatter one block segment out of the staged tile
+__device__ __forceinline__ void unpack_seg(const Seg& s, uint32_t saddr, const unsigned char* sp, uint32_t flags, int* status)
+{
+    if (s.addr & 15ull) {  // D16 slow path: 8-byte stores
+        for (uint32_t b = 0; b < s.bulk; b += 8)
+            *reinterpret_cast<uint64_t*>(s.addr + b) = *reinterpret_cast<const uint64_t*>(sp + b);
+    } else if (s.bulk) {
+        bulk_s2g(reinterpret_cast<void*>(s.addr), saddr, s.bulk);
+    }
+    if (s.tail) {  // 8 data bytes; the 8 pad bytes stay in the stream
+        const uint2 v = *reinterpret_cast<const uint2*>(sp + s.bulk);
+        const uint2 z = *reinterpret_cast<const uint2*>(sp + s.bulk + 8);
+        *reinterpret_cast<uint2*>(s.addr + s.bulk) = v;
+        if ((flags & kFlagCheckPad) && (z.x | z.y) != 0) atomicCAS(status, 0, BS_ERR_CORRUPT);
+    }
+}
+
+template <bool UNPACK>
+__global__ void __launch_bounds__(kMaxWarps * 32, 1) move_tma_kernel(const MoveParams p, const uint32_t n_stages)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ __align__(8) uint64_t s_bar[kMaxWarps * kMaxStages];
+
+    const WsHead* head = p.ws.head;
+    if (head->status != 0) return;  // deferred error: nothing is written
+    const uint32_t T = head->n_tensors, B = head->n_blocks;
+    const uint64_t hb = head->header_bytes, P = head->payload_bytes, total = hb + P;
+    const uint64_t ng = head->n_granules;
+    const uint64_t lo = p.lo, hi = p.hi < total ? p.hi : total;
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+    const uint32_t tile_bytes = p.tile_bytes;
+    const Blk* __restrict__ blk = p.ws.blk;
+
+    const uint32_t ring = smem_u32(smem) + warp * n_stages * tile_bytes;  // this warp's stages
+    unsigned char* ring_ptr = smem + (size_t)warp * n_stages * tile_bytes;
+    const uint32_t bar0 = smem_u32(&s_bar[warp * kMaxStages]);
+    if (lane == 0) {
+        for (uint32_t s = 0; s < n_stages; ++s) mbar_init(bar0 + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    fence_proxy_async();
+    __syncwarp();
+
+    // ---- payload tiles of [lo, hi): tile k = payload bytes [k*tile_bytes, (k+1)*tile_bytes) ----
+    uint64_t plo = 0, phi = 0, k0 = 0, np = 0;
+    if (hi > hb && hi > lo) {
+        plo = (lo > hb ? lo : hb) - hb;
+        phi = hi - hb;
+        k0 = plo / tile_bytes;
+        np = (phi + tile_bytes - 1) / tile_bytes - k0;
+    }
+    const uint64_t worker = (uint64_t)blockIdx.x * n_warps + warp, n_workers = (uint64_t)gridDim.x * n_warps;
+    const int64_t n_mine = np > worker ? (int64_t)((np - worker + n_workers - 1) / n_workers) : 0;
+    const int64_t lag = n_stages - 2;  // tile i is stored while tiles i+1 .. i+lag are loading
+
+    // The block table is read once per tile and never cached (the data streaming past evicts it), so each lookup
+    // costs a DRAM round trip.  Both levels are fetched ahead: tile_first[] two tiles, blk[] one tile before use.
+    auto tile_base = [&](int64_t i) { return (k0 + worker + (uint64_t)i * n_workers) * tile_bytes; };
+    auto load_tile_idx = [&](int64_t i) {
+        TileIdx t;
+        t.jlo = 1; t.jhi = 0;
+        if (i >= 0 && i < n_mine && B != 0) {
+            const uint64_t tb = tile_base(i);
+            const uint64_t g0 = tb / kGranule;
+            uint64_t g1 = (tb + tile_bytes) / kGranule;
+            if (g1 > ng) g1 = ng;
+            t.jlo = __ldg(p.ws.tile_first + g0);
+            t.jhi = __ldg(p.ws.tile_first + g1);  // tile_first[ng] == B
+            if (t.jhi >= B) t.jhi = B - 1;
+        }
+        return t;
+    };
+    auto load_lane_blk = [&](const TileIdx& t) {
+        LaneBlk b;
+        b.e.off = 0; b.e.addr = 0; b.next = 0;  // clips to nothing
+        const uint32_t j = t.jlo + lane;
+        if (t.jlo <= t.jhi && j <= t.jhi) {
+            b.e = blk[j];
+            b.next = __ldg(reinterpret_cast<const unsigned long long*>(&blk[j + 1].off));
+        }
+        return b;
+    };
+    const int64_t m0 = UNPACK ? -lag : 0;  // index of the tile whose block table the first iteration needs
+    TileIdx ti_cur = load_tile_idx(m0), ti_nxt = load_tile_idx(m0 + 1);
+    LaneBlk lb_cur = load_lane_blk(ti_cur);
+
+    for (int64_t it = 0; it < n_mine + lag; ++it) {
+        const TileIdx ti_nx2 = load_tile_idx(m0 + it + 2);
+        const LaneBlk lb_nxt = load_lane_blk(ti_nxt);
+        // the store that last read stage it % n_stages was committed two iterations ago
+        bulk_wait_read<1>();
+        __syncwarp();
+        if (it < n_mine) {  // ---- produce: load tile `it` of this warp into its stage ----
+            const uint32_t st = (uint32_t)(it % n_stages);
+            const uint64_t tbase = tile_base(it);
+            const uint64_t tlo = tbase > plo ? tbase : plo;
+            const uint64_t thi = tbase + tile_bytes < phi ? tbase + tile_bytes : phi;
+            const uint32_t sbase = ring + st * tile_bytes, bar = bar0 + 8 * st;
+            if (UNPACK) {
+                if (lane == 0) {
+                    mbar_arrive_expect_tx(bar, (uint32_t)(thi - tlo));
+                    bulk_g2s(sbase + (uint32_t)(tlo - tbase), p.stream + (hb + tlo - lo), (uint32_t)(thi - tlo), bar);
+                }
+            } else {
+                const uint32_t jlo = ti_cur.jlo, jhi = ti_cur.jhi;
+                // pass 1: bytes the bulk copies will deliver; tails and 8-byte-aligned blocks go through cp.async
+                uint32_t tx = 0, n_async = 0;
+                Seg s0;  // the lane's first segment (tiles rarely hold > 32 blocks)
+                const bool have0 = clip_seg(lb_cur.e, lb_cur.next, tlo, thi, &s0);
+                if (have0) n_async += pack_seg_async(s0, sbase + (uint32_t)(s0.lo - tbase), &tx);
+                if (jhi >= jlo + 32) {
+                    for (uint32_t j = jlo + lane + 32; j <= jhi; j += 32) {
+                        Seg s;
+                        if (make_seg(blk, j, tlo, thi, &s)) n_async += pack_seg_async(s, sbase + (uint32_t)(s.lo - tbase), &tx);
+                    }
+                }
+                if (n_async) cp_async_mbar_arrive(bar);
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) tx += __shfl_xor_sync(0xffffffffu, tx, d);
+                __syncwarp();  // every lane's cp.async arrival is registered before the phase can complete
+                if (lane == 0) mbar_arrive_expect_tx(bar, tx);
+                __syncwarp();
+                // pass 2: the bulk copies
+                if (have0 && (s0.addr & 15ull) == 0 && s0.bulk)
+                    bulk_g2s(sbase + (uint32_t)(s0.lo - tbase), reinterpret_cast<const void*>(s0.addr), s0.bulk, bar);
+                if (jhi >= jlo + 32) {
+                    for (uint32_t j = jlo + lane + 32; j <= jhi; j += 32) {
+                        Seg s;
+                        if (make_seg(blk, j, tlo, thi, &s) && (s.addr & 15ull) == 0 && s.bulk)
+                            bulk_g2s(sbase + (uint32_t)(s.lo - tbase), reinterpret_cast<const void*>(s.addr), s.bulk, bar);
+                    }
+                }
+            }
+        }
+        if (it >= lag) {  // ---- consume: store tile `it - lag` ----
+            const int64_t ci = it - lag;
+            const uint32_t st = (uint32_t)(ci % n_stages), parity = (uint32_t)((ci / n_stages) & 1);
+            const uint64_t tbase = tile_base(ci);
+            const uint64_t tlo = tbase > plo ? tbase : plo;
+            const uint64_t thi = tbase + tile_bytes < phi ? tbase + tile_bytes : phi;
+            const uint32_t sbase = ring + st * tile_bytes, bar = bar0 + 8 * st;
+            if (!UNPACK) {
+                if (lane == 0) {
+                    mbar_wait(bar, parity);
+                    fence_proxy_async();  // the cp.async tails were written through the generic proxy
+                    bulk_s2g(p.stream + (hb + tlo - lo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo));
+                }
+            } else {
+                const uint32_t jlo = ti_cur.jlo, jhi = ti_cur.jhi;
+                int* status = const_cast<int*>(&head->status);
+                const unsigned char* sp = ring_ptr + (size_t)st * tile_bytes;
+                Seg s0;
+                const bool have0 = clip_seg(lb_cur.e, lb_cur.next, tlo, thi, &s0);
+                mbar_wait(bar, parity);
+                if (have0) unpack_seg(s0, sbase + (uint32_t)(s0.lo - tbase), sp + (s0.lo - tbase), p.flags, status);
+                if (jhi >= jlo + 32) {
+                    for (uint32_t j = jlo + lane + 32; j <= jhi; j += 32) {
+                        Seg s;
+                        if (make_seg(blk, j, tlo, thi, &s))
+                            unpack_seg(s, sbase + (uint32_t)(s.lo - tbase), sp + (s.lo - tbase), p.flags, status);
+                    }
+                }
+            }
+        }
+        bulk_commit();
+        ti_cur = ti_nxt;
+        ti_nxt = ti_nx2;
+        lb_cur = lb_nxt;
+    }
+    bulk_wait_read<0>();
+
+    // ---- header region: generated (pack) / rebuilt into the descriptor arrays (unpack) by plain stores ----
+    constexpr uint64_t kChunk = 512;  // 16-byte units (pack) or records (unpack) per warp work item
+    uint64_t n_units = 0;
+    if (UNPACK) {
+        if (p.header != nullptr) n_units = (uint64_t)T + B;
+    } else if (lo < hb && lo < hi) {
+        n_units = ((hi < hb ? hi : hb) - lo) / 16;
+    }
+    for (uint64_t c = worker; c * kChunk < n_units; c += n_workers) {
+        const uint64_t u1 = (c + 1) * kChunk < n_units ? (c + 1) * kChunk : n_units;
+        for (uint64_t u = c * kChunk + lane; u < u1; u += 32) {
+            if (UNPACK) rebuild_record(p, u, T, B);
+            else __stcs(reinterpret_cast<uint4*>(p.stream + u * 16), header_unit(p, (lo >> 4) + u, T, B, hb, P));
+        }
+    }
+}
+
+template <bool UNPACK>
+cudaError_t launch_tma_t(const MoveParams& p, const bs_opts& o, int sm_count, cudaStream_t stream)
+{
+    const uint32_t stages = o.stages, warps = o.warps;
+    const size_t smem = (size_t)warps * stages * o.tile_bytes;
+    if (stages < 3 || stages > kMaxStages || warps < 1 || warps > kMaxWarps || smem + 2048 > kSmemLimit)
+        return cudaErrorInvalidValue;
+    static size_t configured = 0;  // per kernel instantiation
+    if (smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(move_tma_kernel<UNPACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    move_tma_kernel<UNPACK><<<(unsigned)sm_count, warps * 32, smem, stream>>>(p, stages);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_move_tma(bool unpack, const MoveParams& p, const bs_opts& o, int sm_count, cudaStream_t stream)
+{
+    return unpack ? launch_tma_t<true>(p, o, sm_count, stream) : launch_tma_t<false>(p, o, sm_count, stream);
+}
+
+}  // namespace bs

@@ -16,7 +16,14 @@ pytestmark = pytest.mark.gpu
 VARIANTS = [dict(variant=bs.VARIANT_LDG, tile_bytes=16384), dict(variant=bs.VARIANT_LDG, tile_bytes=32768),
             dict(variant=bs.VARIANT_LDG, tile_bytes=49152), dict(variant=bs.VARIANT_LDG, tile_bytes=65536, ctas_per_sm=1),
             dict(variant=bs.VARIANT_TMA, tile_bytes=16384), dict(variant=bs.VARIANT_TMA, tile_bytes=32768),
-            dict(variant=bs.VARIANT_TMA, tile_bytes=65536, ctas_per_sm=1)]
+            dict(variant=bs.VARIANT_TMA, tile_bytes=65536), dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=1),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=8, warps=1),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=4),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=3, warps=2)]
+
+
+def _vid(o):
+    return f"v{o['variant']}-t{o['tile_bytes']}-c{o.get('ctas_per_sm', 0)}-s{o.get('stages', 0)}-w{o.get('warps', 0)}"
 
 
 def small_sets():
@@ -45,7 +52,7 @@ def test_serialize_matches_oracle_byte_for_byte(bset):
     check_stream(bset, up)
 
 
-@pytest.mark.parametrize("opts", VARIANTS, ids=lambda o: f"v{o['variant']}-t{o['tile_bytes']}-c{o.get('ctas_per_sm', 0)}")
+@pytest.mark.parametrize("opts", VARIANTS, ids=_vid)
 def test_P6_stream_independent_of_decomposition(opts):
     for bset in (W.make_config("2"), W.make_set("lognormal", 12, D=300, S=30, M=4, N0=3, n_ops=40, n_site=2,
                                                 dims="lognormal", sigma=1.0)):
@@ -76,7 +83,7 @@ def test_deserialize_matches_oracle_and_round_trips(bset):
     assert (again.cpu().numpy()[:len(want)] == want).all()
 
 
-@pytest.mark.parametrize("opts", VARIANTS, ids=lambda o: f"v{o['variant']}-t{o['tile_bytes']}-c{o.get('ctas_per_sm', 0)}")
+@pytest.mark.parametrize("opts", VARIANTS, ids=_vid)
 def test_P6_unpack_independent_of_decomposition(opts):
     bset = W.make_set("lognormal", 12, D=300, S=30, M=4, N0=3, n_ops=40, n_site=2, dims="lognormal", sigma=1.0)
     want, _, _ = oracle_stream(bset)
