@@ -54,6 +54,7 @@ def make_opts(opts) -> "Opts":
     o = Opts()
     for k in ("variant", "tile_bytes", "ctas_per_sm", "stages", "warps"):
         setattr(o, k, int((opts or {}).get(k, 0) or 0))
+    o.reserved[0] = int((opts or {}).get("tune", 0) or 0)
     return o
 
 

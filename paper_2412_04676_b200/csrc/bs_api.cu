@@ -47,11 +47,13 @@ static int check_set(const bs_set_desc* s)
 static int check_opts(const bs_opts& o)
 {
     if (o.variant != BS_VARIANT_LDG && o.variant != BS_VARIANT_TMA) return BS_ERR_ARG;
-    if (o.tile_bytes == 0 || o.tile_bytes % kGranule != 0 || o.tile_bytes > 65536) return BS_ERR_ARG;
     if (o.ctas_per_sm > 32) return BS_ERR_ARG;
+    if (o.variant == BS_VARIANT_TMA && o.tile_bytes == 0 && o.stages == 0 && o.warps == 0) return BS_OK;  // presets
+    if (o.tile_bytes == 0 || o.tile_bytes % kGranule != 0 || o.tile_bytes > 65536) return BS_ERR_ARG;
+    if (o.variant == BS_VARIANT_LDG && o.tile_bytes % 16384 != 0) return BS_ERR_ARG;
     if (o.variant == BS_VARIANT_TMA &&
         (o.stages < 3 || o.stages > 8 || o.warps < 1 || o.warps > 16 ||
-         (uint64_t)o.stages * o.warps * o.tile_bytes > 225u * 1024u))
+         (uint64_t)o.warps * ((uint64_t)o.stages * o.tile_bytes + 1120ull) > 224u * 1024u))
         return BS_ERR_ARG;
     return BS_OK;
 }
@@ -92,6 +94,7 @@ int run_pack_range(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint6
     mp.lo = lo;
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
+    mp.tune = o.reserved[0];
     cudaError_t e = launch_move(false, mp, o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
@@ -137,6 +140,7 @@ int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_sr
     mp.lo = lo;
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
+    mp.tune = o.reserved[0];
     mp.flags = flags;
     cudaError_t e = launch_move(true, mp, o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);

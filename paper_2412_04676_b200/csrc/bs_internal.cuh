@@ -20,7 +20,7 @@ constexpr uint32_t kTensorRec = 32;
 constexpr uint32_t kBlockRec = 48;
 constexpr uint32_t kHeaderAlign = 128;
 constexpr uint32_t kPoolAlign = 256;
-constexpr uint32_t kGranule = 16384;  // bytes of payload per tile_first entry
+constexpr uint32_t kGranule = 4096;   // bytes of payload per tile_first entry
 
 constexpr uint32_t kScanThreads = 256;
 constexpr uint32_t kScanItems = 4;
@@ -113,6 +113,7 @@ struct MoveParams {
     uint64_t lo, hi;
     uint32_t tile_bytes;
     uint32_t flags;
+    uint32_t tune;                // bs_opts.reserved[0]: experiment switches of the TMA variant
 };
 
 cudaError_t launch_move(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream);

@@ -79,4 +79,74 @@ __device__ __forceinline__ void rebuild_record(const MoveParams& p, uint64_t rec
     }
 }
 
+// ---- warp-level header workers (TMA variant: a dedicated warp per CTA runs these beside the data warps) -------
+// Header worker `hw` of `n_hw` (one warp each).  Nothing here depends on another worker.
+
+// S3 for stream bytes [lo, hend), hend <= header_bytes: fixed header, tensor records and zero slack unit by unit
+// (few); block records one LANE per record, four records per lane in flight, each worker a contiguous run of
+// records so the owning tensor is found by one binary search and then only ever steps forward.
+__device__ __forceinline__ void write_header_warp(const MoveParams& p, uint32_t T, uint32_t B, uint64_t hb, uint64_t P,
+                                                  uint64_t lo, uint64_t hend, uint64_t hw, uint64_t n_hw, uint32_t lane)
+{
+    if (lo >= hend) return;
+    const uint64_t rec0 = kFixedHeader + kTensorRec * (uint64_t)T;  // stream offset of block record 0
+    const uint64_t rec_end = rec0 + kBlockRec * (uint64_t)B;
+    {   // everything that is not a block record
+        const uint64_t n_head = rec0 / 16, n_slack = (hb - rec_end) / 16;
+        for (uint64_t i = hw * 32 + lane; i < n_head + n_slack; i += n_hw * 32) {
+            const uint64_t u = i < n_head ? i : rec_end / 16 + (i - n_head);
+            const uint64_t s = u * 16;
+            if (s >= lo && s < hend) __stcs(reinterpret_cast<uint4*>(p.stream + (s - lo)), header_unit(p, u, T, B, hb, P));
+        }
+    }
+    if (B == 0 || hend <= rec0 || lo >= rec_end) return;
+    const uint64_t r_lo = lo > rec0 ? (lo - rec0) / kBlockRec : 0;                        // first record touching [lo, hend)
+    const uint64_t r_hi = hend < rec_end ? (hend - rec0 + kBlockRec - 1) / kBlockRec : B;  // one past the last
+    const uint64_t per = (r_hi - r_lo + n_hw - 1) / n_hw;
+    const uint64_t my0 = r_lo + hw * per, my1 = my0 + per < r_hi ? my0 + per : r_hi;
+    if (my0 >= my1) return;
+    uint32_t t = tensor_of_block(p.tensors, T, (uint32_t)my0);  // warp-uniform; each lane then walks forward
+    constexpr int K = 4;
+    for (uint64_t base = my0; base < my1; base += 32 * K) {
+        int2 q0[K], q1[K], q2[K];
+        uint32_t d0[K], d1[K], d2[K];
+        uint64_t off[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const uint64_t r = base + (uint64_t)k * 32 + lane;
+            if (r < my1) {
+                const int2* q = reinterpret_cast<const int2*>(p.qn + 6 * r);
+                q0[k] = __ldg(q); q1[k] = __ldg(q + 1); q2[k] = __ldg(q + 2);
+                d0[k] = __ldg(p.dim + 3 * r); d1[k] = __ldg(p.dim + 3 * r + 1); d2[k] = __ldg(p.dim + 3 * r + 2);
+                off[k] = p.ws.blk[r].off;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const uint64_t r = base + (uint64_t)k * 32 + lane;
+            if (r < my1) {
+                while (t + 1 < T && __ldg(&p.tensors[t + 1].first_block) <= r) ++t;  // tensors partition the blocks in order
+                const uint64_t s = rec0 + kBlockRec * r;
+                const uint4 v0 = make_uint4((uint32_t)q0[k].x, (uint32_t)q0[k].y, (uint32_t)q1[k].x, (uint32_t)q1[k].y);
+                const uint4 v1 = make_uint4((uint32_t)q2[k].x, (uint32_t)q2[k].y, d0[k], d1[k]);
+                const uint4 v2 = make_uint4(d2[k], t, (uint32_t)off[k], (uint32_t)(off[k] >> 32));
+                if (s >= lo && s < hend) __stcs(reinterpret_cast<uint4*>(p.stream + (s - lo)), v0);
+                if (s + 16 >= lo && s + 16 < hend) __stcs(reinterpret_cast<uint4*>(p.stream + (s + 16 - lo)), v1);
+                if (s + 32 >= lo && s + 32 < hend) __stcs(reinterpret_cast<uint4*>(p.stream + (s + 32 - lo)), v2);
+            }
+        }
+    }
+}
+
+// S7 (descriptor part): records [0, T+B) of p.header -> the out descriptor arrays, 128 records per step
+__device__ __forceinline__ void rebuild_header_warp(const MoveParams& p, uint32_t T, uint32_t B, uint64_t hw, uint64_t n_hw,
+                                                    uint32_t lane)
+{
+    const uint64_t n_rec = (uint64_t)T + B;
+    for (uint64_t base = hw * 128; base < n_rec; base += n_hw * 128) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) rebuild_record(p, base + (uint64_t)k * 32 + lane, T, B);
+    }
+}
+
 }  // namespace bs

@@ -27,7 +27,7 @@ namespace bs {
 
 namespace {
 
-constexpr uint32_t kMaxWarps = 16;
+constexpr uint32_t kMaxWarps = 16;   // data warps; one more warp per CTA works on the header
 constexpr uint32_t kMaxStages = 8;
 constexpr uint32_t kSmemLimit = 227u * 1024u;
 
@@ -69,6 +69,36 @@ __device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes
 {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_hint(void* dst, uint32_t src, uint32_t bytes, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dst), "r"(src), "r"(bytes),
+                 "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+struct Hints {  // MoveParams.tune: bit 0 = L2 evict_first on bulk loads, bit 1 = on bulk stores
+    uint64_t pol;
+    bool ld, st;
+};
+__device__ __forceinline__ void bulk_g2s_x(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, const Hints& h)
+{
+    if (h.ld) bulk_g2s_hint(dst, src, bytes, bar, h.pol); else bulk_g2s(dst, src, bytes, bar);
+}
+__device__ __forceinline__ void bulk_s2g_x(void* dst, uint32_t src, uint32_t bytes, const Hints& h)
+{
+    if (h.st) bulk_s2g_hint(dst, src, bytes, h.pol); else bulk_s2g(dst, src, bytes);
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void bulk_wait_read()
@@ -84,6 +114,21 @@ __device__ __forceinline__ void cp_async_tail16(uint32_t dst, const void* src)
 __device__ __forceinline__ void cp_async_8(uint32_t dst, const void* src)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+
+__device__ __forceinline__ void cp_async_4(uint32_t dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait()
+{
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
 struct Seg {          // intersection of one block with one tile, payload coordinates
@@ -114,13 +159,11 @@ __device__ __forceinline__ bool make_seg(const Blk* __restrict__ blk, uint32_t j
     return clip_seg(e, next, tlo, thi, s);
 }
 
-struct TileIdx {  // blocks jlo..jhi may intersect the tile (jhi < jlo: none / no such tile)
-    uint32_t jlo, jhi;
-};
-struct LaneBlk {  // table entry of block jlo + lane, fetched one tile ahead
-    Blk e;
-    uint64_t next;
-};
+// Per-warp metadata in shared memory, filled by cp.async ahead of use (no register is tied up, no warp stalls):
+//   tf[3][2]   tile_first[] pair {jlo, jhi_raw} of tiles m, m+1, m+2 (slot = tile index mod 3)
+//   blk[2][34] block table entries jlo .. jlo+32 of tiles m, m+1     (slot = tile index mod 2)
+constexpr uint32_t kMetaBlk = 34;
+constexpr uint32_t kMetaBytes = 2 * kMetaBlk * 16 + 32;  // 1120 per warp
 
 // pack: stage one block segment.  Bulk part: counted in *tx, issued later (after the expect_tx); 8-byte-aligned
 // blocks (D16) and odd tails: cp.async now.  Returns the number of cp.async groups this lane started.
@@ -146,13 +189,14 @@ __device__ __forceinline__ uint32_t pack_seg_async(const Seg& s, uint32_t d, uin
 }
 
 // unpack: scatter one block segment out of the staged tile
-__device__ __forceinline__ void unpack_seg(const Seg& s, uint32_t saddr, const unsigned char* sp, uint32_t flags, int* status)
+__device__ __forceinline__ void unpack_seg(const Seg& s, uint32_t saddr, const unsigned char* sp, uint32_t flags, int* status,
+                                           const Hints& h)
 {
     if (s.addr & 15ull) {  // D16 slow path: 8-byte stores
         for (uint32_t b = 0; b < s.bulk; b += 8)
             *reinterpret_cast<uint64_t*>(s.addr + b) = *reinterpret_cast<const uint64_t*>(sp + b);
     } else if (s.bulk) {
-        bulk_s2g(reinterpret_cast<void*>(s.addr), saddr, s.bulk);
+        bulk_s2g_x(reinterpret_cast<void*>(s.addr), saddr, s.bulk, h);
     }
     if (s.tail) {  // 8 data bytes; the 8 pad bytes stay in the stream
         const uint2 v = *reinterpret_cast<const uint2*>(sp + s.bulk);
@@ -162,8 +206,26 @@ __device__ __forceinline__ void unpack_seg(const Seg& s, uint32_t saddr, const u
     }
 }
 
+struct Preset {
+    uint32_t tile_bytes, stages, warps;
+};
+constexpr uint64_t kSmallMeanBlock = 8192;  // mean stored block size below which the small-block pack preset is used
+__host__ __device__ inline Preset preset(int which)  // 0 pack, large blocks; 1 pack, small blocks; 2 unpack
+{
+    Preset ps = {16384, 3, 3};
+    if (which == 1) { ps.tile_bytes = 4096; ps.warps = 10; }
+    if (which == 2) ps.warps = 2;
+    return ps;
+}
+__host__ __device__ inline Preset pick_preset(bool unpack, uint64_t payload_bytes, uint64_t n_blocks)
+{
+    if (unpack) return preset(2);
+    return preset(payload_bytes >= kSmallMeanBlock * n_blocks ? 0 : 1);
+}
+
 template <bool UNPACK>
-__global__ void __launch_bounds__(kMaxWarps * 32, 1) move_tma_kernel(const MoveParams p, const uint32_t n_stages)
+__global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const MoveParams p, const uint32_t opt_stages,
+                                                                     const uint32_t opt_warps)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t s_bar[kMaxWarps * kMaxStages];
@@ -174,20 +236,14 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) move_tma_kernel(const MoveP
     const uint64_t hb = head->header_bytes, P = head->payload_bytes, total = hb + P;
     const uint64_t ng = head->n_granules;
     const uint64_t lo = p.lo, hi = p.hi < total ? p.hi : total;
-    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
-    const uint32_t tile_bytes = p.tile_bytes;
-    const Blk* __restrict__ blk = p.ws.blk;
-
-    const uint32_t ring = smem_u32(smem) + warp * n_stages * tile_bytes;  // this warp's stages
-    unsigned char* ring_ptr = smem + (size_t)warp * n_stages * tile_bytes;
-    const uint32_t bar0 = smem_u32(&s_bar[warp * kMaxStages]);
-    if (lane == 0) {
-        for (uint32_t s = 0; s < n_stages; ++s) mbar_init(bar0 + 8 * s, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // launch shape: given (bs_opts), or a preset picked here from the mean block size the scan pass found —
+    // many small segments per tile want more, smaller rings (the per-tile issue work is serial within a warp)
+    uint32_t tile_bytes = p.tile_bytes, n_stages = opt_stages, n_warps = opt_warps;
+    if (tile_bytes == 0) {
+        const Preset ps = pick_preset(UNPACK, P, B);
+        tile_bytes = ps.tile_bytes; n_stages = ps.stages; n_warps = ps.warps;
     }
-    fence_proxy_async();
-    __syncwarp();
-
     // ---- payload tiles of [lo, hi): tile k = payload bytes [k*tile_bytes, (k+1)*tile_bytes) ----
     uint64_t plo = 0, phi = 0, k0 = 0, np = 0;
     if (hi > hb && hi > lo) {
@@ -196,47 +252,106 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) move_tma_kernel(const MoveP
         k0 = plo / tile_bytes;
         np = (phi + tile_bytes - 1) / tile_bytes - k0;
     }
+    // ---- header region: generated (pack) / rebuilt into the descriptor arrays (unpack) with plain loads and stores
+    // by warp `n_warps` of every CTA, beside the data warps; by every warp when the range holds no payload ----
+    if (warp > n_warps) return;
+    if (warp == n_warps || np == 0) {
+        const uint64_t hw = np == 0 ? (uint64_t)blockIdx.x * (n_warps + 1) + warp : blockIdx.x;
+        const uint64_t n_hw = np == 0 ? (uint64_t)gridDim.x * (n_warps + 1) : gridDim.x;
+        if (UNPACK) {
+            if (p.header != nullptr) rebuild_header_warp(p, T, B, hw, n_hw, lane);
+        } else {
+            write_header_warp(p, T, B, hb, P, lo, hi < hb ? hi : hb, hw, n_hw, lane);
+        }
+        return;
+    }
+    const Blk* __restrict__ blk = p.ws.blk;
+
+    const uint32_t ring = smem_u32(smem) + warp * n_stages * tile_bytes;  // this warp's stages
+    unsigned char* ring_ptr = smem + (size_t)warp * n_stages * tile_bytes;
+    unsigned char* meta_ptr = smem + (size_t)n_warps * n_stages * tile_bytes + (size_t)warp * kMetaBytes;
+    const Blk* m_blk = reinterpret_cast<const Blk*>(meta_ptr);                                  // [2][kMetaBlk]
+    const uint32_t* m_tf = reinterpret_cast<const uint32_t*>(meta_ptr + 2 * kMetaBlk * 16);    // [3][2]
+    const uint32_t m_blk_s = smem_u32(meta_ptr), m_tf_s = m_blk_s + 2 * kMetaBlk * 16;
+    const uint32_t bar0 = smem_u32(&s_bar[warp * kMaxStages]);
+    if (lane == 0) {
+        for (uint32_t s = 0; s < n_stages; ++s) mbar_init(bar0 + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    fence_proxy_async();
+    __syncwarp();
+
     const uint64_t worker = (uint64_t)blockIdx.x * n_warps + warp, n_workers = (uint64_t)gridDim.x * n_warps;
-    const int64_t n_mine = np > worker ? (int64_t)((np - worker + n_workers - 1) / n_workers) : 0;
+    const bool blocked = (p.tune & 4u) != 0;  // experiment: contiguous run of tiles per warp instead of round-robin
+    const uint64_t per = (np + n_workers - 1) / n_workers;
+    const int64_t n_mine = blocked ? (np > worker * per ? (int64_t)(np - worker * per < per ? np - worker * per : per) : 0)
+                                   : (np > worker ? (int64_t)((np - worker + n_workers - 1) / n_workers) : 0);
+    Hints hints;
+    hints.pol = policy_evict_first();
+    hints.ld = (p.tune & 1u) != 0;
+    hints.st = (p.tune & 2u) != 0;
     const int64_t lag = n_stages - 2;  // tile i is stored while tiles i+1 .. i+lag are loading
 
-    // The block table is read once per tile and never cached (the data streaming past evicts it), so each lookup
-    // costs a DRAM round trip.  Both levels are fetched ahead: tile_first[] two tiles, blk[] one tile before use.
-    auto tile_base = [&](int64_t i) { return (k0 + worker + (uint64_t)i * n_workers) * tile_bytes; };
-    auto load_tile_idx = [&](int64_t i) {
-        TileIdx t;
-        t.jlo = 1; t.jhi = 0;
-        if (i >= 0 && i < n_mine && B != 0) {
-            const uint64_t tb = tile_base(i);
-            const uint64_t g0 = tb / kGranule;
-            uint64_t g1 = (tb + tile_bytes) / kGranule;
-            if (g1 > ng) g1 = ng;
-            t.jlo = __ldg(p.ws.tile_first + g0);
-            t.jhi = __ldg(p.ws.tile_first + g1);  // tile_first[ng] == B
-            if (t.jhi >= B) t.jhi = B - 1;
-        }
-        return t;
+    // The block table is read once per tile and never cached (the data streaming past evicts it), so each of the
+    // two lookup levels costs a DRAM round trip.  Both are fetched ahead with cp.async into shared memory:
+    // tile_first[] two tiles, blk[] one tile before use.
+    auto tile_base = [&](int64_t i) {
+        return (blocked ? k0 + worker * per + (uint64_t)i : k0 + worker + (uint64_t)i * n_workers) * tile_bytes;
     };
-    auto load_lane_blk = [&](const TileIdx& t) {
-        LaneBlk b;
-        b.e.off = 0; b.e.addr = 0; b.next = 0;  // clips to nothing
-        const uint32_t j = t.jlo + lane;
-        if (t.jlo <= t.jhi && j <= t.jhi) {
-            b.e = blk[j];
-            b.next = __ldg(reinterpret_cast<const unsigned long long*>(&blk[j + 1].off));
+    auto has_tile = [&](int64_t i) { return i >= 0 && i < n_mine && B != 0; };
+    auto fetch_tf = [&](int64_t i) {  // lanes 0, 1: tile_first[g0], tile_first[g1] of tile i
+        if (has_tile(i) && lane < 2) {
+            const uint64_t tb = tile_base(i);
+            uint64_t g = lane == 0 ? tb / kGranule : (tb + tile_bytes) / kGranule;
+            if (g > ng) g = ng;  // tile_first[ng] == B
+            cp_async_4(m_tf_s + (uint32_t)((i + 6) % 3) * 8 + lane * 4, p.ws.tile_first + g);
         }
-        return b;
+    };
+    auto read_tf = [&](int64_t i, uint32_t* jlo, uint32_t* jhi) {
+        *jlo = 1; *jhi = 0;
+        if (has_tile(i)) {
+            const uint32_t s = (uint32_t)((i + 6) % 3) * 2;
+            *jlo = m_tf[s];
+            *jhi = m_tf[s + 1];
+            if (*jhi >= B) *jhi = B - 1;
+        }
+    };
+    auto fetch_blk = [&](int64_t i) {  // entries jlo .. min(jlo+32, jhi+1) of tile i (blk[B] is the sentinel)
+        uint32_t jlo, jhi;
+        read_tf(i, &jlo, &jhi);
+        if (jlo > jhi) return;
+        const uint32_t slot = m_blk_s + (uint32_t)((i + 6) % 2) * kMetaBlk * 16;
+        if (jlo + lane <= jhi + 1) cp_async_16(slot + lane * 16, blk + jlo + lane);
+        if (lane == 0 && jlo + 32 <= jhi + 1) cp_async_16(slot + 32 * 16, blk + jlo + 32);
     };
     const int64_t m0 = UNPACK ? -lag : 0;  // index of the tile whose block table the first iteration needs
-    TileIdx ti_cur = load_tile_idx(m0), ti_nxt = load_tile_idx(m0 + 1);
-    LaneBlk lb_cur = load_lane_blk(ti_cur);
+    fetch_tf(m0);
+    fetch_tf(m0 + 1);
+    cp_async_commit();
+    cp_async_wait<0>();
+    __syncwarp();
+    fetch_blk(m0);
+    cp_async_commit();
 
     for (int64_t it = 0; it < n_mine + lag; ++it) {
-        const TileIdx ti_nx2 = load_tile_idx(m0 + it + 2);
-        const LaneBlk lb_nxt = load_lane_blk(ti_nxt);
+        const int64_t m = m0 + it;
+        fetch_tf(m + 2);
+        cp_async_commit();
+        cp_async_wait<1>();  // everything fetched during the previous iteration has landed
         // the store that last read stage it % n_stages was committed two iterations ago
         bulk_wait_read<1>();
         __syncwarp();
+        fetch_blk(m + 1);
+        cp_async_commit();
+        uint32_t jlo, jhi;
+        read_tf(m, &jlo, &jhi);
+        Blk e0;
+        e0.off = 0; e0.addr = 0;
+        uint64_t next0 = 0;  // clips to nothing
+        if (jlo <= jhi && jlo + lane <= jhi) {
+            e0 = m_blk[(uint32_t)((m + 6) % 2) * kMetaBlk + lane];
+            next0 = m_blk[(uint32_t)((m + 6) % 2) * kMetaBlk + lane + 1].off;
+        }
         if (it < n_mine) {  // ---- produce: load tile `it` of this warp into its stage ----
             const uint32_t st = (uint32_t)(it % n_stages);
             const uint64_t tbase = tile_base(it);
@@ -246,14 +361,13 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) move_tma_kernel(const MoveP
             if (UNPACK) {
                 if (lane == 0) {
                     mbar_arrive_expect_tx(bar, (uint32_t)(thi - tlo));
-                    bulk_g2s(sbase + (uint32_t)(tlo - tbase), p.stream + (hb + tlo - lo), (uint32_t)(thi - tlo), bar);
+                    bulk_g2s_x(sbase + (uint32_t)(tlo - tbase), p.stream + (hb + tlo - lo), (uint32_t)(thi - tlo), bar, hints);
                 }
             } else {
-                const uint32_t jlo = ti_cur.jlo, jhi = ti_cur.jhi;
                 // pass 1: bytes the bulk copies will deliver; tails and 8-byte-aligned blocks go through cp.async
                 uint32_t tx = 0, n_async = 0;
                 Seg s0;  // the lane's first segment (tiles rarely hold > 32 blocks)
-                const bool have0 = clip_seg(lb_cur.e, lb_cur.next, tlo, thi, &s0);
+                const bool have0 = clip_seg(e0, next0, tlo, thi, &s0);
                 if (have0) n_async += pack_seg_async(s0, sbase + (uint32_t)(s0.lo - tbase), &tx);
                 if (jhi >= jlo + 32) {
                     for (uint32_t j = jlo + lane + 32; j <= jhi; j += 32) {
@@ -269,12 +383,12 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) move_tma_kernel(const MoveP
                 __syncwarp();
                 // pass 2: the bulk copies
                 if (have0 && (s0.addr & 15ull) == 0 && s0.bulk)
-                    bulk_g2s(sbase + (uint32_t)(s0.lo - tbase), reinterpret_cast<const void*>(s0.addr), s0.bulk, bar);
+                    bulk_g2s_x(sbase + (uint32_t)(s0.lo - tbase), reinterpret_cast<const void*>(s0.addr), s0.bulk, bar, hints);
                 if (jhi >= jlo + 32) {
                     for (uint32_t j = jlo + lane + 32; j <= jhi; j += 32) {
                         Seg s;
                         if (make_seg(blk, j, tlo, thi, &s) && (s.addr & 15ull) == 0 && s.bulk)
-                            bulk_g2s(sbase + (uint32_t)(s.lo - tbase), reinterpret_cast<const void*>(s.addr), s.bulk, bar);
+                            bulk_g2s_x(sbase + (uint32_t)(s.lo - tbase), reinterpret_cast<const void*>(s.addr), s.bulk, bar, hints);
                     }
                 }
             }
@@ -290,63 +404,57 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) move_tma_kernel(const MoveP
                 if (lane == 0) {
                     mbar_wait(bar, parity);
                     fence_proxy_async();  // the cp.async tails were written through the generic proxy
-                    bulk_s2g(p.stream + (hb + tlo - lo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo));
+                    bulk_s2g_x(p.stream + (hb + tlo - lo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo), hints);
                 }
             } else {
-                const uint32_t jlo = ti_cur.jlo, jhi = ti_cur.jhi;
                 int* status = const_cast<int*>(&head->status);
                 const unsigned char* sp = ring_ptr + (size_t)st * tile_bytes;
                 Seg s0;
-                const bool have0 = clip_seg(lb_cur.e, lb_cur.next, tlo, thi, &s0);
+                const bool have0 = clip_seg(e0, next0, tlo, thi, &s0);
                 mbar_wait(bar, parity);
-                if (have0) unpack_seg(s0, sbase + (uint32_t)(s0.lo - tbase), sp + (s0.lo - tbase), p.flags, status);
+                if (have0) unpack_seg(s0, sbase + (uint32_t)(s0.lo - tbase), sp + (s0.lo - tbase), p.flags, status, hints);
                 if (jhi >= jlo + 32) {
                     for (uint32_t j = jlo + lane + 32; j <= jhi; j += 32) {
                         Seg s;
                         if (make_seg(blk, j, tlo, thi, &s))
-                            unpack_seg(s, sbase + (uint32_t)(s.lo - tbase), sp + (s.lo - tbase), p.flags, status);
+                            unpack_seg(s, sbase + (uint32_t)(s.lo - tbase), sp + (s.lo - tbase), p.flags, status, hints);
                     }
                 }
             }
         }
         bulk_commit();
-        ti_cur = ti_nxt;
-        ti_nxt = ti_nx2;
-        lb_cur = lb_nxt;
     }
+    cp_async_wait<0>();
     bulk_wait_read<0>();
 
-    // ---- header region: generated (pack) / rebuilt into the descriptor arrays (unpack) by plain stores ----
-    constexpr uint64_t kChunk = 512;  // 16-byte units (pack) or records (unpack) per warp work item
-    uint64_t n_units = 0;
-    if (UNPACK) {
-        if (p.header != nullptr) n_units = (uint64_t)T + B;
-    } else if (lo < hb && lo < hi) {
-        n_units = ((hi < hb ? hi : hb) - lo) / 16;
-    }
-    for (uint64_t c = worker; c * kChunk < n_units; c += n_workers) {
-        const uint64_t u1 = (c + 1) * kChunk < n_units ? (c + 1) * kChunk : n_units;
-        for (uint64_t u = c * kChunk + lane; u < u1; u += 32) {
-            if (UNPACK) rebuild_record(p, u, T, B);
-            else __stcs(reinterpret_cast<uint4*>(p.stream + u * 16), header_unit(p, (lo >> 4) + u, T, B, hb, P));
-        }
-    }
 }
 
 template <bool UNPACK>
 cudaError_t launch_tma_t(const MoveParams& p, const bs_opts& o, int sm_count, cudaStream_t stream)
 {
-    const uint32_t stages = o.stages, warps = o.warps;
-    const size_t smem = (size_t)warps * stages * o.tile_bytes;
-    if (stages < 3 || stages > kMaxStages || warps < 1 || warps > kMaxWarps || smem + 2048 > kSmemLimit)
-        return cudaErrorInvalidValue;
+    uint32_t stages = o.stages, warps = o.warps;
+    size_t smem = 0;
+    if (o.tile_bytes == 0) {  // presets: launch the largest shape, the kernel retires the warps it does not use
+        const Preset cands[3] = {preset(0), preset(1), preset(2)};
+        warps = 0;
+        for (int i = UNPACK ? 2 : 0; i < (UNPACK ? 3 : 2); ++i) {
+            const size_t need = (size_t)cands[i].warps * (cands[i].stages * cands[i].tile_bytes + kMetaBytes);
+            smem = need > smem ? need : smem;
+            warps = cands[i].warps > warps ? cands[i].warps : warps;
+        }
+        stages = 0;
+    } else {
+        smem = (size_t)warps * stages * o.tile_bytes + (size_t)warps * kMetaBytes;
+        if (stages < 3 || stages > kMaxStages || warps < 1 || warps > kMaxWarps) return cudaErrorInvalidValue;
+    }
+    if (smem + 1024 > kSmemLimit) return cudaErrorInvalidValue;
     static size_t configured = 0;  // per kernel instantiation
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(move_tma_kernel<UNPACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    move_tma_kernel<UNPACK><<<(unsigned)sm_count, warps * 32, smem, stream>>>(p, stages);
+    move_tma_kernel<UNPACK><<<(unsigned)sm_count, (warps + 1) * 32, smem, stream>>>(p, stages, warps);  // + the header warp
     return cudaGetLastError();
 }
 

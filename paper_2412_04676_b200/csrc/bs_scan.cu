@@ -6,7 +6,7 @@
 // the stored block sizes over all B blocks, which at the same time
 //   - validates the descriptor (serialize) or every header field (deserialize: SURVEY §8(c) list),
 //   - writes the blk[] table {payload offset, block address} = the "pointer structure" of L90-92,
-//   - writes tile_first[] (which block holds the first byte of every 16 KiB payload granule) = the work
+//   - writes tile_first[] (which block holds the first byte of every 4 KiB payload granule) = the work
 //     partition the data-movement kernel uses to give every CTA an exact, disjoint stream interval,
 //   - reports header / payload / total bytes and the deferred status in bs_result.
 // Roofline: HBM-bound, ~12+8 B read and 16 B written per block (serialize) — <1 % of the payload traffic.
@@ -305,9 +305,18 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
             run += val[k];
         }
         __syncthreads();
-        for (uint32_t s = 0; s < s_big_n; ++s) {  // large blocks: the whole CTA fills their boundaries
+        // large blocks: one warp per block fills its boundaries; huge ones (> 2048 granules) take the whole CTA
+        for (uint32_t s = warp; s < s_big_n; s += kScanThreads / 32) {
             const uint64_t g0 = s_big_g0[s];
             const uint32_t cnt = s_big_cnt[s], idx = s_big_idx[s];
+            if (cnt > 2048) continue;
+            for (uint64_t j = lane; j < cnt; j += 32)
+                if (g0 + j < p.ws.n_granules_cap) p.ws.tile_first[g0 + j] = idx;
+        }
+        for (uint32_t s = 0; s < s_big_n; ++s) {
+            const uint64_t g0 = s_big_g0[s];
+            const uint32_t cnt = s_big_cnt[s], idx = s_big_idx[s];
+            if (cnt <= 2048) continue;
             for (uint64_t j = tid; j < cnt; j += kScanThreads)
                 if (g0 + j < p.ws.n_granules_cap) p.ws.tile_first[g0 + j] = idx;
         }

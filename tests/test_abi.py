@@ -31,7 +31,7 @@ def test_every_declared_symbol_is_exported():
 def test_struct_layouts_match_the_header():
     assert ctypes.sizeof(bs.SetDesc) == 48
     assert ctypes.sizeof(bs.Result) == 64
-    assert ctypes.sizeof(bs.Opts) == 16
+    assert ctypes.sizeof(bs.Opts) == 32
 
 
 def test_host_only_entry_points():

@@ -15,6 +15,8 @@ pytestmark = pytest.mark.gpu
 
 VARIANTS = [dict(variant=bs.VARIANT_LDG, tile_bytes=16384), dict(variant=bs.VARIANT_LDG, tile_bytes=32768),
             dict(variant=bs.VARIANT_LDG, tile_bytes=49152), dict(variant=bs.VARIANT_LDG, tile_bytes=65536, ctas_per_sm=1),
+            dict(variant=bs.VARIANT_TMA), dict(variant=bs.VARIANT_TMA, tile_bytes=4096, stages=3, warps=10),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=12288, stages=4, warps=4),
             dict(variant=bs.VARIANT_TMA, tile_bytes=16384), dict(variant=bs.VARIANT_TMA, tile_bytes=32768),
             dict(variant=bs.VARIANT_TMA, tile_bytes=65536), dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=1),
             dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=8, warps=1),
@@ -23,7 +25,7 @@ VARIANTS = [dict(variant=bs.VARIANT_LDG, tile_bytes=16384), dict(variant=bs.VARI
 
 
 def _vid(o):
-    return f"v{o['variant']}-t{o['tile_bytes']}-c{o.get('ctas_per_sm', 0)}-s{o.get('stages', 0)}-w{o.get('warps', 0)}"
+    return f"v{o['variant']}-t{o.get('tile_bytes', 0)}-c{o.get('ctas_per_sm', 0)}-s{o.get('stages', 0)}-w{o.get('warps', 0)}"
 
 
 def small_sets():
@@ -181,7 +183,7 @@ def test_many_tiny_blocks_per_tile():
     data = [rng.uniform(-1, 1, int(d.prod())) for d in dim]
     bset, pool, offs = _custom([(2, 0, B, (0, 0), (-1, 1, 0, 0), 0, 0)], dim, data)
     up = Uploaded(bset, pool, offs)
-    for opts in (None, dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
+    for opts in (None, dict(variant=bs.VARIANT_LDG), dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
         got, want = check_stream(bset, up, opts)
         out, p, res = gpu_deserialize(got, len(want), 1, B, oracle.pool_bytes(want), opts=opts)
         assert res["status"] == bs.OK
@@ -195,7 +197,7 @@ def test_one_huge_block_and_neighbours():
     data = [rng.uniform(-1, 1, int(np.prod(d))) for d in dim]
     bset, pool, offs = _custom([(2, 0, 2, (0, 0), (-1, 1, 0, 0), 0, 0), (3, 2, 1, (0, 0), (1, 1, -1, 0), 1, 0)], dim, data)
     up = Uploaded(bset, pool, offs)
-    for opts in (None, dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
+    for opts in (None, dict(variant=bs.VARIANT_LDG), dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
         got, want = check_stream(bset, up, opts)
         out, p, res = gpu_deserialize(got, len(want), 2, 3, oracle.pool_bytes(want), opts=opts)
         ref = oracle.deserialize(want)
@@ -206,14 +208,14 @@ def test_D16_eight_byte_aligned_sources_take_the_slow_path():
     bset = W.make_set("mis", 13, D=120, S=12, M=2, N0=3, n_ops=13, n_site=1, dims="multinomial")
     up = Uploaded(bset, misalign=8)
     assert (up.addr % 16 == 8).all()
-    for opts in (None, dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
+    for opts in (None, dict(variant=bs.VARIANT_LDG), dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
         check_stream(bset, up, opts)
     # and scatter back to 8-byte-aligned destinations
     want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
     dst = torch.full((up.pool.numel(),), 0xEE, dtype=torch.uint8, device=DEV)
     daddr = (np.uint64(dst.data_ptr() + 8) + up.host_offs).astype(np.uint64)
     out = bs.DeviceSet.from_host(np.zeros(bset.n_tensors, W.TENSOR_REC_DTYPE), np.zeros_like(bset.qn), bset.dim, daddr, DEV)
-    for opts in (None, dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
+    for opts in (None, dict(variant=bs.VARIANT_LDG), dict(variant=bs.VARIANT_TMA, tile_bytes=32768)):
         dst.fill_(0xEE)
         ws = bs.Workspace(bset.n_tensors, bset.n_blocks, len(want), DEV)
         st = torch.from_numpy(want.copy()).to(DEV)
