@@ -99,7 +99,7 @@ class ClockSampler:
         self.proc = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i",
-                                          str(index), "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL,
+                                          str(index), "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL,
                                          text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -111,7 +111,7 @@ class ClockSampler:
             self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
 
     def window(self, t0, t1):
-        rows = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows[-3:]]
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.02] or [r for _, r in self.rows[-3:]]
         sm, mx, reasons = [], 0.0, set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for r in rows:
@@ -311,12 +311,13 @@ def run_mine(args):
     # counts the scan pass too; the pack launch alone reads 52 B per block on top of the stream bytes]
     algo_bytes = 2 * total + 52 * bset.n_blocks
     achieved = algo_bytes / (pack_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "bs::move_kernel<pack> (S3+S5)", "achieved": round(achieved, 1),
+    kname = "bs::move_kernel<pack>" if args.variant == 1 else "bs::move_tma_kernel<pack>"
+    roofline = {"bound": "hbm", "kernel": kname + " (S3 header write + S5 pack)", "achieved": round(achieved, 1),
                 "peak": peaks["hbm_gbs"], "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
                 "unit": "GB/s", "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": None,
                 "algorithmic_bytes_per_launch": int(algo_bytes), "kernel_ms": round(pack_ms, 4),
                 "frac_of_nominal_8TBs": round(achieved / 8000.0, 4)}
-    roofline["traffic"] = committed_traffic(f"pack:{args.workload}")
+    roofline["traffic"] = committed_traffic(f"pack:{args.workload}:v{args.variant or 2}")
 
     # ---- e2e leg: host (pinned) buffers through the engine, copies inside the timed region ----
     detail = {"serialize_ms": round(float(np.median(ser_ms)), 4), "deserialize_ms": round(float(np.median(des_ms)), 4),
@@ -478,7 +479,7 @@ def config5(args, dev, opts):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
     ap.add_argument("--workload", default="4", choices=["1", "2", "3", "4", "3L", "4L"])

@@ -122,9 +122,9 @@ typedef struct bs_stream_info_t {
 typedef struct bs_opts {
     uint32_t variant;     /* 0 = default; 1 = BS_VARIANT_LDG (16-byte vector loads/stores);
                              2 = BS_VARIANT_TMA (cp.async.bulk global<->shared staging, one ring of tiles per warp) */
-    uint32_t tile_bytes;  /* stream bytes per work tile; 0 = default; <= 65536; multiple of 4096 (TMA), 16384 (LDG) */
+    uint32_t tile_bytes;  /* stream bytes per work tile; 0 = default; multiple of 16384, <= 65536 */
     uint32_t ctas_per_sm; /* LDG: persistent CTAs per SM; 0 = default (occupancy limit) */
-    uint32_t stages;      /* TMA: tiles in flight per warp, 3..8; 0 = default */
+    uint32_t stages;      /* TMA: ring depth (tiles) per warp, 3..8; 0 = default */
     uint32_t warps;       /* TMA: warps (rings) per CTA, 1..16; warps*stages*tile_bytes <= 225 KiB; 0 = default */
     uint32_t reserved[3]; /* 0 */
 } bs_opts;

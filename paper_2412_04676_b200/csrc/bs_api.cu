@@ -50,7 +50,6 @@ static int check_opts(const bs_opts& o)
     if (o.ctas_per_sm > 32) return BS_ERR_ARG;
     if (o.variant == BS_VARIANT_TMA && o.tile_bytes == 0 && o.stages == 0 && o.warps == 0) return BS_OK;  // presets
     if (o.tile_bytes == 0 || o.tile_bytes % kGranule != 0 || o.tile_bytes > 65536) return BS_ERR_ARG;
-    if (o.variant == BS_VARIANT_LDG && o.tile_bytes % 16384 != 0) return BS_ERR_ARG;
     if (o.variant == BS_VARIANT_TMA &&
         (o.stages < 3 || o.stages > 8 || o.warps < 1 || o.warps > 16 ||
          (uint64_t)o.warps * ((uint64_t)o.stages * o.tile_bytes + 1120ull) > 224u * 1024u))

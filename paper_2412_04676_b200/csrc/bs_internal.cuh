@@ -20,7 +20,7 @@ constexpr uint32_t kTensorRec = 32;
 constexpr uint32_t kBlockRec = 48;
 constexpr uint32_t kHeaderAlign = 128;
 constexpr uint32_t kPoolAlign = 256;
-constexpr uint32_t kGranule = 4096;   // bytes of payload per tile_first entry
+constexpr uint32_t kGranule = 16384;  // bytes of payload per tile_first entry
 
 constexpr uint32_t kScanThreads = 256;
 constexpr uint32_t kScanItems = 4;

@@ -3,7 +3,7 @@
 //
 // once the output buffer is mapped, "all threads serialize in parallel and in complete
 // independence. Yet, together they produce a single, continuos stream of bytes".  Here the unit of
-// independence is a TILE of the stream (tile_bytes, a multiple of the 4 KiB granule): tile k of the payload is
+// independence is a TILE of the stream (tile_bytes, a multiple of the 16 KiB granule): tile k of the payload is
 // stream bytes [header_bytes + k*tile_bytes, +tile_bytes), whatever blocks happen to lie in it.  A persistent
 // grid of CTAs walks the tiles; tile_first[] says which block the tile starts in, blk[] gives every block's
 // {payload offset, device address}.  So the work per CTA is uniform no matter how skewed the block sizes are
@@ -193,7 +193,7 @@ void resolve_opts(const bs_opts* in, bs_opts* out)
     if (in) o = *in;
     if (o.variant == BS_VARIANT_DEFAULT) o.variant = BS_VARIANT_TMA;
     if (o.variant == BS_VARIANT_TMA) {
-        // tile_bytes == stages == warps == 0 stays 0: the kernel picks a preset from the set's mean block size
+        // tile_bytes == stages == warps == 0 stays 0: launch_move_tma uses its per-direction preset
         if (o.tile_bytes || o.stages || o.warps) {
             if (o.tile_bytes == 0) o.tile_bytes = 16384;
             if (o.stages == 0) o.stages = 3;

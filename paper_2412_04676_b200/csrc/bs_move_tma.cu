@@ -206,21 +206,16 @@ __device__ __forceinline__ void unpack_seg(const Seg& s, uint32_t saddr, const u
     }
 }
 
+// Default launch shapes (B200, measured on the D=6000 and D=15400 sets): about 96 KiB (pack) / 64 KiB (unpack) of
+// loads in flight per SM; deeper rings or more warps lower the achieved DRAM bandwidth.
 struct Preset {
     uint32_t tile_bytes, stages, warps;
 };
-constexpr uint64_t kSmallMeanBlock = 8192;  // mean stored block size below which the small-block pack preset is used
-__host__ __device__ inline Preset preset(int which)  // 0 pack, large blocks; 1 pack, small blocks; 2 unpack
+__host__ __device__ inline Preset preset(bool unpack)
 {
     Preset ps = {16384, 3, 3};
-    if (which == 1) { ps.tile_bytes = 4096; ps.warps = 10; }
-    if (which == 2) ps.warps = 2;
+    if (unpack) ps.warps = 2;
     return ps;
-}
-__host__ __device__ inline Preset pick_preset(bool unpack, uint64_t payload_bytes, uint64_t n_blocks)
-{
-    if (unpack) return preset(2);
-    return preset(payload_bytes >= kSmallMeanBlock * n_blocks ? 0 : 1);
 }
 
 template <bool UNPACK>
@@ -237,13 +232,7 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
     const uint64_t ng = head->n_granules;
     const uint64_t lo = p.lo, hi = p.hi < total ? p.hi : total;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // launch shape: given (bs_opts), or a preset picked here from the mean block size the scan pass found —
-    // many small segments per tile want more, smaller rings (the per-tile issue work is serial within a warp)
-    uint32_t tile_bytes = p.tile_bytes, n_stages = opt_stages, n_warps = opt_warps;
-    if (tile_bytes == 0) {
-        const Preset ps = pick_preset(UNPACK, P, B);
-        tile_bytes = ps.tile_bytes; n_stages = ps.stages; n_warps = ps.warps;
-    }
+    const uint32_t tile_bytes = p.tile_bytes, n_stages = opt_stages, n_warps = opt_warps;
     // ---- payload tiles of [lo, hi): tile k = payload bytes [k*tile_bytes, (k+1)*tile_bytes) ----
     uint64_t plo = 0, phi = 0, k0 = 0, np = 0;
     if (hi > hb && hi > lo) {
@@ -432,21 +421,14 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
 template <bool UNPACK>
 cudaError_t launch_tma_t(const MoveParams& p, const bs_opts& o, int sm_count, cudaStream_t stream)
 {
+    MoveParams q = p;
     uint32_t stages = o.stages, warps = o.warps;
-    size_t smem = 0;
-    if (o.tile_bytes == 0) {  // presets: launch the largest shape, the kernel retires the warps it does not use
-        const Preset cands[3] = {preset(0), preset(1), preset(2)};
-        warps = 0;
-        for (int i = UNPACK ? 2 : 0; i < (UNPACK ? 3 : 2); ++i) {
-            const size_t need = (size_t)cands[i].warps * (cands[i].stages * cands[i].tile_bytes + kMetaBytes);
-            smem = need > smem ? need : smem;
-            warps = cands[i].warps > warps ? cands[i].warps : warps;
-        }
-        stages = 0;
-    } else {
-        smem = (size_t)warps * stages * o.tile_bytes + (size_t)warps * kMetaBytes;
-        if (stages < 3 || stages > kMaxStages || warps < 1 || warps > kMaxWarps) return cudaErrorInvalidValue;
+    if (o.tile_bytes == 0) {  // bs_opts left the shape open
+        const Preset ps = preset(UNPACK);
+        q.tile_bytes = ps.tile_bytes; stages = ps.stages; warps = ps.warps;
     }
+    if (stages < 3 || stages > kMaxStages || warps < 1 || warps > kMaxWarps) return cudaErrorInvalidValue;
+    const size_t smem = (size_t)warps * stages * q.tile_bytes + (size_t)warps * kMetaBytes;
     if (smem + 1024 > kSmemLimit) return cudaErrorInvalidValue;
     static size_t configured = 0;  // per kernel instantiation
     if (smem > configured) {
@@ -454,7 +436,7 @@ cudaError_t launch_tma_t(const MoveParams& p, const bs_opts& o, int sm_count, cu
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    move_tma_kernel<UNPACK><<<(unsigned)sm_count, (warps + 1) * 32, smem, stream>>>(p, stages, warps);  // + the header warp
+    move_tma_kernel<UNPACK><<<(unsigned)sm_count, (warps + 1) * 32, smem, stream>>>(q, stages, warps);  // + the header warp
     return cudaGetLastError();
 }
 

@@ -6,7 +6,7 @@
 // the stored block sizes over all B blocks, which at the same time
 //   - validates the descriptor (serialize) or every header field (deserialize: SURVEY §8(c) list),
 //   - writes the blk[] table {payload offset, block address} = the "pointer structure" of L90-92,
-//   - writes tile_first[] (which block holds the first byte of every 4 KiB payload granule) = the work
+//   - writes tile_first[] (which block holds the first byte of every 16 KiB payload granule) = the work
 //     partition the data-movement kernel uses to give every CTA an exact, disjoint stream interval,
 //   - reports header / payload / total bytes and the deferred status in bs_result.
 // Roofline: HBM-bound, ~12+8 B read and 16 B written per block (serialize) — <1 % of the payload traffic.

@@ -1,0 +1,128 @@
+"""Parity at BASELINE.json's full sizes (configs 3 and 4), in the launch configuration bench.py times (default opts).
+The oracle cannot hold these streams in seconds, so it is run slice-wise: the whole header, and the payload of sampled
+tensors whose values it regenerates from the counter-based generator (never a byte from the CUDA path).  Properties that
+hold at any size cover the rest: exact size prediction, the fixpoint serialize(deserialize(S)) == S on the device, and
+chunked offload == the stream."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2412_04676_b200 as bs
+import workloads as W
+from tests.gpu_util import DEV, Uploaded
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+
+def sampled_tensors(bset, n=10, seed=7):
+    per_t = np.add.reduceat(bset.nelems, bset.tensors["first_block"].astype(np.int64))
+    rng = np.random.default_rng(seed)
+    pick = {0, bset.n_tensors - 1, int(np.argmax(per_t)), int(np.argmin(per_t))}
+    pick |= set(int(x) for x in rng.choice(bset.n_tensors, size=n, replace=False))
+    return sorted(pick)
+
+
+def oracle_tensor_payload(bset, t):
+    """(first payload offset, bytes) of tensor t from the oracle, block values regenerated on the host."""
+    b0 = int(bset.tensors["first_block"][t])
+    b1 = b0 + int(bset.tensors["n_blocks"][t])
+    pool, offs = W.fill_pool_host(bset, b0, b1, compact=True)
+    addr = np.zeros(bset.n_blocks, np.uint64)
+    addr[b0:b1] = np.uint64(pool.ctypes.data) + offs
+    cap = int(((bset.nelems[b0:b1] * 8 + 15) // 16 * 16).sum())
+    first, got = oracle.emit_payload_range(bset.tensors, bset.dim, addr, t, t + 1, cap)
+    assert len(got) == cap
+    return first, got, pool
+
+
+@pytest.mark.parametrize("cfg", ["3", "4"])
+def test_full_size_serialize_deserialize(cfg):
+    bset = W.make_config(cfg)
+    up = Uploaded(bset, fill="device")
+    hb, total = oracle.serialized_size(bset.n_tensors, bset.dim)
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, total, DEV)
+    cs = bs.current_stream()
+    # exact size prediction before serialization
+    assert bs.serialized_size(up.dset.desc, ws.ptr, ws.nbytes, cs) == (hb, total)
+    stream = torch.full((total + 4096,), 0xCD, dtype=torch.uint8, device=DEV)
+    bs.serialize(up.dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, None, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and (res["header_bytes"], res["total_bytes"]) == (hb, total)
+    assert bool((stream[total:] == 0xCD).all()), "bytes beyond the stream were written"
+    # the whole header against the oracle's
+    want_h = oracle.emit_header(bset.tensors, bset.qn, bset.dim)
+    got_h = stream[:hb].cpu().numpy()
+    bad = np.nonzero(got_h != want_h)[0]
+    assert bad.size == 0, f"header differs first at byte {bad[0]}"
+    # sampled tensors' payload against the oracle's
+    for t in sampled_tensors(bset):
+        first, want, _ = oracle_tensor_payload(bset, t)
+        got = stream[hb + first: hb + first + len(want)].cpu().numpy()
+        bad = np.nonzero(got != want)[0]
+        assert bad.size == 0, f"tensor {t}: payload differs first at payload byte {first + bad[0]}"
+
+    # deserialize: descriptor identical, sampled blocks bit-identical to the regenerated values
+    need = int(((bset.nelems * 8 + 255) // 256 * 256).sum())
+    out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+    opool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    bs.deserialize(stream.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                   ws.result_ptr, None, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["pool_bytes"] == need
+    host = out.to_host()
+    assert host["tensors"].tobytes() == bset.tensors.tobytes()
+    assert (host["qn"] == bset.qn).all() and (host["dim"] == bset.dim).all()
+    slots = (bset.nelems * 8 + 255) // 256 * 256
+    want_addr = opool.data_ptr() + np.concatenate([[0], np.cumsum(slots)[:-1]]).astype(np.uint64)
+    assert (host["addr"] == want_addr.astype(np.uint64)).all()          # D14 pool layout
+    for t in sampled_tensors(bset, n=6, seed=9):
+        b0 = int(bset.tensors["first_block"][t])
+        b1 = b0 + int(bset.tensors["n_blocks"][t])
+        pool, offs = W.fill_pool_host(bset, b0, b1, compact=True)
+        for i in range(b0, b1):
+            n = int(bset.nelems[i])
+            o = int(host["addr"][i]) - opool.data_ptr()
+            got = opool[o: o + 8 * n].cpu().numpy().view(np.uint64)
+            want = pool.view(np.uint64)[int(offs[i - b0]) // 8: int(offs[i - b0]) // 8 + n]
+            assert (got == want).all(), f"block {i} of tensor {t} differs after the round trip"
+    # every gap byte of the pool is untouched (slots are align256; the unpack writes exactly nbytes per block)
+    # fixpoint on the device, every byte: serialize(deserialize(S)) == S
+    again = torch.full((total,), 0x11, dtype=torch.uint8, device=DEV)
+    bs.serialize(out.desc, again.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, None, cs)
+    assert ws.read_result()["status"] == bs.OK
+    assert torch.equal(again, stream[:total]), "serialize(deserialize(S)) != S"
+
+
+def test_full_size_offload_prefetch_config3():
+    """config 5's data path at full size: 256 MiB double-buffered chunks; concat(chunks) == the bs_serialize stream."""
+    bset = W.make_config("3")
+    up = Uploaded(bset, fill="device")
+    hb, total = oracle.serialized_size(bset.n_tensors, bset.dim)
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, total, DEV)
+    cs = bs.current_stream()
+    stream = torch.empty(total, dtype=torch.uint8, device=DEV)
+    bs.serialize(up.dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, None, cs)
+    assert ws.read_result()["status"] == bs.OK
+    host = torch.empty(total, dtype=torch.uint8, pin_memory=True)
+    host.fill_(0x5A)
+    eng = bs.Engine(bset.n_tensors, bset.n_blocks, total)        # defaults: 256 MiB chunks, 2 staging buffers
+    st = eng.offload_async(up.dset.desc, total, host.data_ptr(), total, cs).wait()
+    assert st["status"] == bs.OK and st["bytes"] == total and st["n_chunks"] == (total + (256 << 20) - 1) // (256 << 20)
+    assert torch.equal(host, stream.cpu()), "concat(chunks) != stream"
+    need = int(((bset.nelems * 8 + 255) // 256 * 256).sum())
+    out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+    opool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    st = eng.prefetch_async(host.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, cs).wait()
+    torch.cuda.synchronize()
+    assert st["status"] == bs.OK
+    ref_out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+    ref_pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    bs.deserialize(stream.data_ptr(), total, ref_out.desc, ref_pool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                   ws.result_ptr, None, cs)
+    assert ws.read_result()["status"] == bs.OK
+    assert torch.equal(opool, ref_pool)
+    a, b = out.to_host(), ref_out.to_host()
+    assert a["tensors"].tobytes() == b["tensors"].tobytes() and (a["qn"] == b["qn"]).all() and (a["dim"] == b["dim"]).all()
+    assert ((a["addr"] - np.uint64(opool.data_ptr())) == (b["addr"] - np.uint64(ref_pool.data_ptr()))).all()
+    eng.destroy()

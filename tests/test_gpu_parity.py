@@ -15,8 +15,8 @@ pytestmark = pytest.mark.gpu
 
 VARIANTS = [dict(variant=bs.VARIANT_LDG, tile_bytes=16384), dict(variant=bs.VARIANT_LDG, tile_bytes=32768),
             dict(variant=bs.VARIANT_LDG, tile_bytes=49152), dict(variant=bs.VARIANT_LDG, tile_bytes=65536, ctas_per_sm=1),
-            dict(variant=bs.VARIANT_TMA), dict(variant=bs.VARIANT_TMA, tile_bytes=4096, stages=3, warps=10),
-            dict(variant=bs.VARIANT_TMA, tile_bytes=12288, stages=4, warps=4),
+            dict(variant=bs.VARIANT_TMA), dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=4, warps=3),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=49152, stages=4, warps=1),
             dict(variant=bs.VARIANT_TMA, tile_bytes=16384), dict(variant=bs.VARIANT_TMA, tile_bytes=32768),
             dict(variant=bs.VARIANT_TMA, tile_bytes=65536), dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=1),
             dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=8, warps=1),
