@@ -3,6 +3,7 @@
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import this
 package.  It imports nothing from paper_2412_04676_b200.
 """
+from . import bs_oracle_v2 as v2  # noqa: F401  (wire format v2: structure-shared layers)
 from .bs_oracle import (  # noqa: F401
     ERR_ARG,
     ERR_CAPACITY,
@@ -10,7 +11,6 @@ from .bs_oracle import (  # noqa: F401
     ERR_UNSUPPORTED,
     OK,
     OracleError,
-    build,
     deserialize,
     emit_header,
     emit_payload_range,
@@ -23,3 +23,11 @@ from .bs_oracle import (  # noqa: F401
     validate_set,
     validate_stream,
 )
+from .bs_oracle import build as _build_v1
+
+
+def build(force: bool = False) -> str:
+    """Compile every C file of the oracle (v1 and v2 libraries)."""
+    so = _build_v1(force)
+    v2.build(force)
+    return so

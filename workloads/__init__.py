@@ -9,9 +9,12 @@ header fields.  It imports neither ``oracle`` nor ``paper_2412_04676_b200``.
 from .blocksparse import (  # noqa: F401
     BASE_SEED,
     CONFIGS,
+    LAYER_REC_DTYPE,
+    STRUCT_REC_DTYPE,
     TENSOR_REC_DTYPE,
     BlockSparseSet,
     label_grid,
+    layered_view,
     make_config,
     make_set,
     selection_rules,

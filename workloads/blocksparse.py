@@ -213,8 +213,55 @@ def make_set(name: str, seed: int, D: int, S: int, M: int, N0: int, n_ops: int, 
     nelems = d64[:, 0] * d64[:, 1] * d64[:, 2]
     pool_off, pool_bytes = _place(rng, nelems, pool_align, scatter)
     meta = dict(D=D, S=S, M=M, N0=N0, n_ops=n_ops, n_site=n_site, dims=dims, sigma=sigma,
-                pool_align=pool_align, scatter=scatter, bond_dims=bond)
+                pool_align=pool_align, scatter=scatter, bond_dims=bond,
+                # the structure classes the tensors were drawn from (layered_view)
+                cls_of=cls_of, cls_start=cls_start, cls_nb=cls_nb, cls_qn=all_qn, cls_dim=all_dim, n_rules=len(rules),
+                rules=rules)
     return BlockSparseSet(name, seed, tensors, qn, dim, pool_off, pool_bytes, meta)
+
+
+# descriptor records of the structure-shared ("layered") form of a set (include/bs.h bs_struct_rec, bs_layer_rec):
+# the layers of PAPER Fig 4(a) (L75) name a structure; a structure owns one table of labelled sectors
+STRUCT_REC_DTYPE = np.dtype([("rank", "<u4"), ("first_block", "<u4"), ("n_blocks", "<u4"), ("dq", "<i4", (2,)),
+                             ("sign", "i1", (4,)), ("layer_bytes", "<u8")])
+LAYER_REC_DTYPE = np.dtype([("structure", "<u4"), ("tag", "<u4"), ("offset", "<u8")])
+assert STRUCT_REC_DTYPE.itemsize == 32 and LAYER_REC_DTYPE.itemsize == 16
+
+
+def layered_view(bset: BlockSparseSet, keep_unused: bool = False) -> dict:
+    """The same set in structure-shared form: operators drawn from one selection rule are LAYERS of one
+    structure (Fig 4(a), L75); every site tensor is the single layer of its own structure.  Inputs only:
+    ``layer_bytes`` / ``offset`` (the serializer's outputs) are left 0.  Block i of ``bset`` is entry i of the
+    layered form's address list (layer-major, structure order inside a layer), so pools and addresses are shared.
+    keep_unused: keep structures no layer refers to (n_ops < number of rules) instead of dropping them."""
+    m = bset.meta
+    cls_of, cls_start, cls_nb = m["cls_of"], m["cls_start"], m["cls_nb"]
+    n_cls = len(cls_nb)
+    used = np.zeros(n_cls, dtype=bool)
+    used[cls_of] = True
+    keep = np.ones(n_cls, dtype=bool) if keep_unused else used
+    new_id = np.cumsum(keep) - 1
+    ids = np.nonzero(keep)[0]
+    structs = np.zeros(len(ids), dtype=STRUCT_REC_DTYPE)
+    nb = cls_nb[ids]
+    structs["n_blocks"] = nb
+    structs["first_block"] = np.concatenate([[0], np.cumsum(nb)])[:-1] if len(ids) else np.zeros(0)
+    is_op = ids < m["n_rules"]
+    structs["rank"] = np.where(is_op, 2, 3)
+    for k, c in enumerate(ids):
+        if c < m["n_rules"]:
+            structs["dq"][k] = m["rules"][c]
+            structs["sign"][k] = (-1, 1, 0, 0)
+        else:
+            structs["dq"][k] = (0, 0)
+            structs["sign"][k] = (1, 1, -1, 0)
+    src = np.concatenate([np.arange(cls_start[c], cls_start[c] + cls_nb[c]) for c in ids]).astype(np.int64) \
+        if len(ids) else np.zeros(0, np.int64)
+    layers = np.zeros(bset.n_tensors, dtype=LAYER_REC_DTYPE)
+    layers["structure"] = new_id[cls_of]
+    layers["tag"] = bset.tensors["tag"]
+    return dict(structs=structs, layers=layers, qn=np.ascontiguousarray(m["cls_qn"][src]),
+                dim=np.ascontiguousarray(m["cls_dim"][src]))
 
 
 # BASELINE.json configs 1-4 (config 5 = config 3 through the offload engine); "L" = operator count
