@@ -179,6 +179,86 @@ int bs_deserialize(const void *d_stream, uint64_t nbytes, bs_set_desc *out, void
                    uint64_t pool_bytes, uint32_t flags, void *d_workspace, uint64_t workspace_bytes,
                    bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
 
+
+/* ==== wire format v2: structure-shared layers (PAPER Fig 4(a), L75) =============================
+ *
+ * "Layers indicate position dependent operators which have the same block-sparse structure, but the dense sector
+ * matrices take different values for the different layers" (L75).  A layered set is C STRUCTURES (one table of
+ * labelled sectors each: the meta data of L63, stored once) and T LAYERS, each naming its structure and owning one
+ * dense block per sector of it.  The payload is byte-identical to the v1 payload of the same tensors; only the header
+ * differs (48 bytes per structure block + 16 per layer instead of 48 per block of every tensor).
+ *
+ *   stream      := fixed_header(64) | struct_rec[C](32) | layer_rec[T](16) | block_rec[Bs](48) | zeros to a multiple
+ *                  of 128 | payload(P)
+ *   fixed_header: char magic[8]="BSPARSE1"; u32 version=2; u32 endian_tag=0x01020304; u32 dtype=0; u32 n_qn=2;
+ *                 u32 max_rank=3; u32 align=16; u32 n_structs=C; u32 n_struct_blocks=Bs; u64 n_layers=T;
+ *                 u64 header_bytes; u64 payload_bytes
+ *   struct_rec  : bs_struct_rec, byte for byte (layer_bytes = sum over its blocks of align16(8*prod(dim)))
+ *   layer_rec   : bs_layer_rec, byte for byte  (offset = sum over earlier layers of their structure's layer_bytes)
+ *   block_rec   : i32 qn[3][2]; u32 dim[3]; u32 structure; u64 offset   (offset relative to the start of a layer =
+ *                 sum over earlier blocks of the same structure of align16(8*prod(dim)))
+ *   payload     : layer t at payload + offset_t, block j of its structure at + offset_j, zero padded to 16
+ *   header_bytes = align128(64 + 32*C + 16*T + 48*Bs)
+ */
+typedef struct bs_struct_rec {
+    uint32_t rank;        /* 2 or 3 */
+    uint32_t first_block; /* structures partition the structure block table (qn / dim) in order */
+    uint32_t n_blocks;
+    int32_t dq[2];        /* conserved charge: sum_k sign[k]*qn[k] == dq for every block */
+    int8_t sign[4];
+    uint64_t layer_bytes; /* OUTPUT of deserialize (from the wire); ignored by serialize */
+} bs_struct_rec;
+
+typedef struct bs_layer_rec {
+    uint32_t structure;   /* index into structs[] */
+    uint32_t tag;         /* opaque user id (operator index / site) */
+    uint64_t offset;      /* OUTPUT of deserialize (payload offset of the layer, from the wire); ignored by serialize */
+} bs_layer_rec;
+
+/* HOST struct; every pointer is a DEVICE pointer.  addr[] lists the blocks layer by layer (descriptor order), inside
+ * a layer in the order of its structure's block table: B = sum_t structs[layers[t].structure].n_blocks entries. */
+typedef struct bs_layered_desc {
+    uint32_t n_structs;       /* C.   For deserialize / prefetch outputs: CAPACITY of structs[] */
+    uint32_t n_struct_blocks; /* Bs.  For outputs: CAPACITY of qn / dim */
+    uint32_t n_layers;        /* T.   For outputs: CAPACITY of layers[] */
+    uint32_t n_qn;            /* 2 */
+    uint32_t dtype;           /* BS_F64 */
+    uint32_t reserved;        /* 0 */
+    uint64_t n_addr;          /* entries of addr[]: must be >= B (serialize: B is checked on the device) */
+    bs_struct_rec *structs;   /* [C]         */
+    bs_layer_rec *layers;     /* [T]         */
+    int32_t *qn;              /* [Bs][3][2]  */
+    uint32_t *dim;            /* [Bs][3]     */
+    uint64_t *addr;           /* [B]         8-byte aligned block addresses (16 for the fast path) */
+} bs_layered_desc;
+
+typedef struct bs_layered_stream_info_t {
+    uint64_t n_structs, n_struct_blocks, n_layers, header_bytes, payload_bytes, total_bytes;
+} bs_layered_stream_info_t;
+
+/* align128(64 + 32*C + 16*T + 48*Bs) */
+uint64_t bs_layered_header_bytes(uint64_t n_structs, uint64_t n_layers, uint64_t n_struct_blocks);
+/* workspace for a layered set of up to these counts (n_addr = B) whose stream is at most stream_capacity bytes */
+uint64_t bs_layered_workspace_bytes(uint32_t n_structs, uint32_t n_struct_blocks, uint32_t n_layers, uint64_t n_addr,
+                                    uint64_t stream_capacity);
+int bs_layered_stream_info(const void *h_first_64_bytes, bs_layered_stream_info_t *out); /* HOST memory */
+
+/* As bs_serialized_size / bs_serialize / bs_serialize_range / bs_deserialize, for wire format v2.  bs_result:
+ * n_tensors = T, n_blocks = B, reserved[0] = C, reserved[1] = Bs.  Deferred statuses as for v1; additionally
+ * BS_ERR_ARG for a layer naming a structure >= C and BS_ERR_CAPACITY for n_addr < B.  bs_layered_deserialize writes
+ * structs / layers (wire records), qn / dim (BS_LAYOUT_POOL; with BS_SCATTER_TO_ADDR dim [Bs][3] and addr [B] are
+ * INPUTS) and addr. */
+int bs_layered_serialized_size(const bs_layered_desc *set, void *d_workspace, uint64_t workspace_bytes,
+                               uint64_t *header_bytes, uint64_t *total_bytes, cudaStream_t stream);
+int bs_layered_serialize(const bs_layered_desc *set, void *d_stream, uint64_t capacity, void *d_workspace,
+                         uint64_t workspace_bytes, bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
+int bs_layered_serialize_range(const bs_layered_desc *set, void *d_dst, uint64_t lo, uint64_t hi, int run_scan,
+                               void *d_workspace, uint64_t workspace_bytes, bs_result *d_result, const bs_opts *opts,
+                               cudaStream_t stream);
+int bs_layered_deserialize(const void *d_stream, uint64_t nbytes, bs_layered_desc *out, void *d_pool,
+                           uint64_t pool_bytes, uint32_t flags, void *d_workspace, uint64_t workspace_bytes,
+                           bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
+
 /* ---- asynchronous offload / prefetch engine ------------------- */
 
 typedef struct bs_engine bs_engine;
@@ -220,6 +300,14 @@ int bs_offload_async(bs_engine *e, const bs_set_desc *set, uint64_t total_bytes,
  * completion (cudaStreamWaitEvent — the "checkpoint" of PAPER L138); the host is not blocked. */
 int bs_prefetch_async(bs_engine *e, const void *h_pinned, uint64_t nbytes, bs_set_desc *out, void *d_pool,
                       uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket **ticket);
+
+
+/* The same two calls for layered sets (wire format v2).  The engine must have been created with max_tensors >= C and
+ * >= T, max_blocks >= Bs and >= B. */
+int bs_offload_layered_async(bs_engine *e, const bs_layered_desc *set, uint64_t total_bytes, void *h_pinned,
+                             uint64_t h_capacity, cudaStream_t producer, bs_ticket **ticket);
+int bs_prefetch_layered_async(bs_engine *e, const void *h_pinned, uint64_t nbytes, bs_layered_desc *out, void *d_pool,
+                              uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket **ticket);
 
 int bs_ticket_wait(bs_ticket *t, bs_ticket_stats *stats /* may be NULL */); /* blocks the host; returns the deferred status */
 int bs_ticket_query(const bs_ticket *t);                                   /* BS_OK | BS_PENDING | BS_ERR_* */

@@ -31,6 +31,26 @@ class SetDesc(C.Structure):
                 ("tensors", C.c_void_p), ("qn", C.c_void_p), ("dim", C.c_void_p), ("addr", C.c_void_p)]
 
 
+class StructRec(C.Structure):
+    _fields_ = [("rank", C.c_uint32), ("first_block", C.c_uint32), ("n_blocks", C.c_uint32), ("dq", C.c_int32 * 2),
+                ("sign", C.c_int8 * 4), ("layer_bytes", C.c_uint64)]
+
+
+class LayerRec(C.Structure):
+    _fields_ = [("structure", C.c_uint32), ("tag", C.c_uint32), ("offset", C.c_uint64)]
+
+
+class LayeredDesc(C.Structure):
+    _fields_ = [("n_structs", C.c_uint32), ("n_struct_blocks", C.c_uint32), ("n_layers", C.c_uint32), ("n_qn", C.c_uint32),
+                ("dtype", C.c_uint32), ("reserved", C.c_uint32), ("n_addr", C.c_uint64), ("structs", C.c_void_p),
+                ("layers", C.c_void_p), ("qn", C.c_void_p), ("dim", C.c_void_p), ("addr", C.c_void_p)]
+
+
+class LayeredStreamInfo(C.Structure):
+    _fields_ = [("n_structs", C.c_uint64), ("n_struct_blocks", C.c_uint64), ("n_layers", C.c_uint64),
+                ("header_bytes", C.c_uint64), ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64)]
+
+
 class Result(C.Structure):
     _fields_ = [("total_bytes", C.c_uint64), ("header_bytes", C.c_uint64), ("payload_bytes", C.c_uint64),
                 ("pool_bytes", C.c_uint64), ("status", C.c_int32), ("n_tensors", C.c_uint32), ("n_blocks", C.c_uint32),
@@ -68,7 +88,7 @@ class TicketStats(C.Structure):
                 ("total_ms", C.c_float)]
 
 
-assert C.sizeof(TensorRec) == 32 and C.sizeof(Result) == 64
+assert C.sizeof(TensorRec) == 32 and C.sizeof(Result) == 64 and C.sizeof(StructRec) == 32 and C.sizeof(LayerRec) == 16
 
 _lib = None
 
@@ -105,6 +125,18 @@ def lib():
     L.bs_engine_destroy.argtypes = [vp]
     L.bs_offload_async.argtypes = [vp, C.POINTER(SetDesc), u64, vp, u64, vp, C.POINTER(vp)]
     L.bs_prefetch_async.argtypes = [vp, vp, u64, C.POINTER(SetDesc), vp, u64, u32, vp, C.POINTER(vp)]
+    LD = C.POINTER(LayeredDesc)
+    L.bs_layered_header_bytes.restype = u64
+    L.bs_layered_header_bytes.argtypes = [u64, u64, u64]
+    L.bs_layered_workspace_bytes.restype = u64
+    L.bs_layered_workspace_bytes.argtypes = [u32, u32, u32, u64, u64]
+    L.bs_layered_stream_info.argtypes = [vp, C.POINTER(LayeredStreamInfo)]
+    L.bs_layered_serialized_size.argtypes = [LD, vp, u64, pu64, pu64, vp]
+    L.bs_layered_serialize.argtypes = [LD, vp, u64, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_layered_serialize_range.argtypes = [LD, vp, u64, u64, i32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_layered_deserialize.argtypes = [vp, u64, LD, vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_offload_layered_async.argtypes = [vp, LD, u64, vp, u64, vp, C.POINTER(vp)]
+    L.bs_prefetch_layered_async.argtypes = [vp, vp, u64, LD, vp, u64, u32, vp, C.POINTER(vp)]
     L.bs_ticket_wait.argtypes = [vp, C.POINTER(TicketStats)]
     L.bs_ticket_query.argtypes = [vp]
     L.bs_ticket_destroy.argtypes = [vp]
@@ -181,6 +213,53 @@ def deserialize(stream_ptr: int, nbytes: int, out: SetDesc, pool_ptr: int, pool_
                                        result_ptr, _opts(opts), stream), "bs_deserialize")
 
 
+# ---- wire format v2: structure-shared layers ----------------------------------------------------------------------
+def layered_header_bytes(n_structs: int, n_layers: int, n_struct_blocks: int) -> int:
+    return int(lib().bs_layered_header_bytes(n_structs, n_layers, n_struct_blocks))
+
+
+def layered_workspace_bytes(n_structs: int, n_struct_blocks: int, n_layers: int, n_addr: int, stream_capacity: int) -> int:
+    return int(lib().bs_layered_workspace_bytes(n_structs, n_struct_blocks, n_layers, n_addr, stream_capacity))
+
+
+def layered_stream_info(first_64_bytes) -> dict:
+    buf = (C.c_ubyte * 64).from_buffer_copy(bytes(first_64_bytes[:64]).ljust(64, b"\0"))
+    info = LayeredStreamInfo()
+    _check(lib().bs_layered_stream_info(C.addressof(buf), C.byref(info)), "bs_layered_stream_info")
+    return {k: int(getattr(info, k)) for k, _ in LayeredStreamInfo._fields_}
+
+
+def make_layered_desc(n_structs: int, n_struct_blocks: int, n_layers: int, n_addr: int, structs_ptr: int, layers_ptr: int,
+                      qn_ptr: int, dim_ptr: int, addr_ptr: int) -> LayeredDesc:
+    return LayeredDesc(n_structs, n_struct_blocks, n_layers, 2, F64, 0, n_addr, structs_ptr, layers_ptr, qn_ptr, dim_ptr,
+                       addr_ptr)
+
+
+def layered_serialized_size(desc: LayeredDesc, ws_ptr: int, ws_bytes: int, stream: int = 0):
+    hb, tot = C.c_uint64(0), C.c_uint64(0)
+    _check(lib().bs_layered_serialized_size(C.byref(desc), ws_ptr, ws_bytes, C.byref(hb), C.byref(tot), stream),
+           "bs_layered_serialized_size")
+    return int(hb.value), int(tot.value)
+
+
+def layered_serialize(desc: LayeredDesc, stream_ptr: int, capacity: int, ws_ptr: int, ws_bytes: int, result_ptr: int,
+                      opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_layered_serialize(C.byref(desc), stream_ptr, capacity, ws_ptr, ws_bytes, result_ptr, _opts(opts),
+                                             stream), "bs_layered_serialize")
+
+
+def layered_serialize_range(desc: LayeredDesc, dst_ptr: int, lo: int, hi: int, run_scan: bool, ws_ptr: int, ws_bytes: int,
+                            result_ptr: int, opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_layered_serialize_range(C.byref(desc), dst_ptr, lo, hi, int(run_scan), ws_ptr, ws_bytes, result_ptr,
+                                                   _opts(opts), stream), "bs_layered_serialize_range")
+
+
+def layered_deserialize(stream_ptr: int, nbytes: int, out: LayeredDesc, pool_ptr: int, pool_bytes: int, flags: int,
+                        ws_ptr: int, ws_bytes: int, result_ptr: int, opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_layered_deserialize(stream_ptr, nbytes, C.byref(out), pool_ptr, pool_bytes, flags, ws_ptr, ws_bytes,
+                                               result_ptr, _opts(opts), stream), "bs_layered_deserialize")
+
+
 class Ticket:
     def __init__(self, handle: int):
         self._h = handle
@@ -232,6 +311,20 @@ class Engine:
         t = C.c_void_p(0)
         _check(lib().bs_prefetch_async(self._h, h_pinned_ptr, nbytes, C.byref(out), pool_ptr, pool_bytes, flags, consumer,
                                        C.byref(t)), "bs_prefetch_async")
+        return Ticket(t.value)
+
+    def offload_layered_async(self, desc: LayeredDesc, total_bytes: int, h_pinned_ptr: int, h_capacity: int,
+                              producer: int = 0) -> Ticket:
+        t = C.c_void_p(0)
+        _check(lib().bs_offload_layered_async(self._h, C.byref(desc), total_bytes, h_pinned_ptr, h_capacity, producer,
+                                              C.byref(t)), "bs_offload_layered_async")
+        return Ticket(t.value)
+
+    def prefetch_layered_async(self, h_pinned_ptr: int, nbytes: int, out: LayeredDesc, pool_ptr: int, pool_bytes: int,
+                               flags: int = 0, consumer: int = 0) -> Ticket:
+        t = C.c_void_p(0)
+        _check(lib().bs_prefetch_layered_async(self._h, h_pinned_ptr, nbytes, C.byref(out), pool_ptr, pool_bytes, flags,
+                                               consumer, C.byref(t)), "bs_prefetch_layered_async")
         return Ticket(t.value)
 
     def destroy(self):

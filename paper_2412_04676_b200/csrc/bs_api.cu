@@ -44,7 +44,7 @@ static int check_set(const bs_set_desc* s)
     return BS_OK;
 }
 
-static int check_opts(const bs_opts& o)
+int check_opts(const bs_opts& o)
 {
     if (o.variant != BS_VARIANT_LDG && o.variant != BS_VARIANT_TMA) return BS_ERR_ARG;
     if (o.ctas_per_sm > 32) return BS_ERR_ARG;

@@ -28,6 +28,17 @@ int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t n
                          int sms, cudaStream_t stream);
 int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header,
                      uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream);
+// wire format v2 (bs_layered.cu)
+int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t capacity,
+                               uint64_t expect_total, bs_result* d_result, int sms, cudaStream_t stream);
+int run_layered_deserialize_plan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_layered_desc* out,
+                                 void* d_pool, uint64_t pool_bytes, uint32_t flags, void* d_ws, uint64_t ws_bytes,
+                                 bs_result* d_result, int sms, cudaStream_t stream);
+int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, void* d_dst, uint64_t lo, uint64_t hi,
+                           const bs_opts& o, int sms, cudaStream_t stream);
+int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws_bytes, const void* d_src,
+                             const void* d_header, uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms,
+                             cudaStream_t stream);
 }  // namespace bs
 
 using namespace bs;
@@ -125,6 +136,13 @@ int bs_engine_create(bs_engine** out, const bs_engine_cfg* cfg)
     if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e->ev_dep, cudaEventDisableTiming);
     e->ws_bytes = bs_workspace_bytes(e->cfg.max_tensors, e->cfg.max_blocks, e->cfg.max_stream_bytes);
     e->header_cap = bs_header_bytes(e->cfg.max_tensors, e->cfg.max_blocks);
+    {   // layered sets (wire format v2): C, T <= max_tensors; Bs, B <= max_blocks
+        const uint64_t w2 = bs_layered_workspace_bytes(e->cfg.max_tensors, e->cfg.max_blocks, e->cfg.max_tensors,
+                                                       e->cfg.max_blocks, e->cfg.max_stream_bytes);
+        const uint64_t h2 = bs_layered_header_bytes(e->cfg.max_tensors, e->cfg.max_tensors, e->cfg.max_blocks);
+        if (w2 > e->ws_bytes) e->ws_bytes = w2;
+        if (h2 > e->header_cap) e->header_cap = h2;
+    }
     if (ce == cudaSuccess) ce = cudaMalloc(&e->ws, e->ws_bytes);
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&e->header_buf, e->header_cap);
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&e->d_result, sizeof(bs_result));
@@ -158,17 +176,28 @@ int bs_engine_destroy(bs_engine* e)
     return BS_OK;
 }
 
-int bs_offload_async(bs_engine* e, const bs_set_desc* set, uint64_t total_bytes, void* h_pinned, uint64_t h_capacity,
-                     cudaStream_t producer, bs_ticket** ticket)
+}  // extern "C"
+
+// one body for both wire formats: exactly one of set / lset is non-null
+static int offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layered_desc* lset, uint64_t total_bytes,
+                        void* h_pinned, uint64_t h_capacity, cudaStream_t producer, bs_ticket** ticket)
 {
-    if (e == nullptr || set == nullptr || h_pinned == nullptr || ticket == nullptr) return BS_ERR_ARG;
-    if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
+    if (e == nullptr || (set == nullptr && lset == nullptr) || h_pinned == nullptr || ticket == nullptr) return BS_ERR_ARG;
     WsLayout L;
-    if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
     int rc;
+    if (set) {
+        if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
+        if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
+    } else {
+        if (lset->n_structs > e->cfg.max_tensors || lset->n_layers > e->cfg.max_tensors ||
+            lset->n_struct_blocks > e->cfg.max_blocks || lset->n_addr > e->cfg.max_blocks)
+            return BS_ERR_CAPACITY;
+    }
     if (total_bytes == 0) {  // size prediction on the producer stream (synchronises it)
         uint64_t hb = 0;
-        if ((rc = bs_serialized_size(set, e->ws, e->ws_bytes, &hb, &total_bytes, producer))) return rc;
+        rc = set ? bs_serialized_size(set, e->ws, e->ws_bytes, &hb, &total_bytes, producer)
+                 : bs_layered_serialized_size(lset, e->ws, e->ws_bytes, &hb, &total_bytes, producer);
+        if (rc) return rc;
     }
     if (total_bytes > h_capacity || total_bytes > e->cfg.max_stream_bytes) return BS_ERR_CAPACITY;
     if (total_bytes & 15) return BS_ERR_ARG;
@@ -183,13 +212,17 @@ int bs_offload_async(bs_engine* e, const bs_set_desc* set, uint64_t total_bytes,
     CK(cudaEventRecord(e->ev_dep, producer));          // the data is ready after everything enqueued so far
     CK(cudaStreamWaitEvent(e->kstream, e->ev_dep, 0));
     CK(cudaEventRecord(t->t_begin, e->kstream));
-    if ((rc = run_serialize_scan(set, L, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream))) return rc;
+    rc = set ? run_serialize_scan(set, L, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream)
+             : run_layered_serialize_plan(lset, e->ws, e->ws_bytes, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream);
+    if (rc) return rc;
     CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
     for (uint32_t k = 0; k < t->n_chunks; ++k) {
         const uint32_t b = k % S;
         const uint64_t lo = (uint64_t)k * C, hi = (lo + C < total_bytes) ? lo + C : total_bytes;
         if (k >= S) CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));  // staging[b] drained by DMA k-S
-        if ((rc = run_pack_range(set, L, e->staging[b], lo, hi, e->opts, e->sms, e->kstream))) return rc;
+        rc = set ? run_pack_range(set, L, e->staging[b], lo, hi, e->opts, e->sms, e->kstream)
+                 : run_layered_pack_range(lset, e->ws, e->ws_bytes, e->staging[b], lo, hi, e->opts, e->sms, e->kstream);
+        if (rc) return rc;
         CK(cudaEventRecord(e->ev_k[b], e->kstream));
         CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));
         if (k == 0) CK(cudaEventRecord(t->dma_begin, e->cstream));
@@ -203,22 +236,39 @@ int bs_offload_async(bs_engine* e, const bs_set_desc* set, uint64_t total_bytes,
     return BS_OK;
 }
 
-int bs_prefetch_async(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs_set_desc* out, void* d_pool,
-                      uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket** ticket)
+static int prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs_set_desc* out, bs_layered_desc* lout,
+                         void* d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket** ticket)
 {
-    if (e == nullptr || h_pinned == nullptr || out == nullptr || ticket == nullptr) return BS_ERR_ARG;
+    if (e == nullptr || h_pinned == nullptr || (out == nullptr && lout == nullptr) || ticket == nullptr) return BS_ERR_ARG;
     if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
     if (nbytes < kFixedHeader) return BS_ERR_CORRUPT;
     bs_stream_info_t info;
-    int rc = bs_stream_info(h_pinned, &info);  // the stream is in host RAM: its counts cost nothing to read
-    if (rc) return rc;
-    if (info.total_bytes != nbytes) return BS_ERR_CORRUPT;
-    if (info.n_blocks > e->cfg.max_blocks || info.n_tensors > e->cfg.max_tensors || info.header_bytes > e->header_cap ||
-        nbytes > e->cfg.max_stream_bytes)
-        return BS_ERR_CAPACITY;
-    if (info.n_blocks > out->n_blocks || info.n_tensors > out->n_tensors) return BS_ERR_CAPACITY;
     WsLayout L;
-    if (!ws_layout(e->ws, e->ws_bytes, out->n_blocks, &L)) return BS_ERR_CAPACITY;
+    int rc;
+    if (out) {
+        rc = bs_stream_info(h_pinned, &info);  // the stream is in host RAM: its counts cost nothing to read
+        if (rc) return rc;
+        if (info.total_bytes != nbytes) return BS_ERR_CORRUPT;
+        if (info.n_blocks > e->cfg.max_blocks || info.n_tensors > e->cfg.max_tensors || info.header_bytes > e->header_cap ||
+            nbytes > e->cfg.max_stream_bytes)
+            return BS_ERR_CAPACITY;
+        if (info.n_blocks > out->n_blocks || info.n_tensors > out->n_tensors) return BS_ERR_CAPACITY;
+        if (!ws_layout(e->ws, e->ws_bytes, out->n_blocks, &L)) return BS_ERR_CAPACITY;
+    } else {
+        bs_layered_stream_info_t li;
+        rc = bs_layered_stream_info(h_pinned, &li);
+        if (rc) return rc;
+        if (li.total_bytes != nbytes) return BS_ERR_CORRUPT;
+        if (li.n_structs > e->cfg.max_tensors || li.n_layers > e->cfg.max_tensors || li.n_struct_blocks > e->cfg.max_blocks ||
+            lout->n_addr > e->cfg.max_blocks || li.header_bytes > e->header_cap || nbytes > e->cfg.max_stream_bytes)
+            return BS_ERR_CAPACITY;
+        if (li.n_structs > lout->n_structs || li.n_layers > lout->n_layers || li.n_struct_blocks > lout->n_struct_blocks)
+            return BS_ERR_CAPACITY;
+        if (bs_layered_workspace_bytes(lout->n_structs, lout->n_struct_blocks, lout->n_layers, lout->n_addr, nbytes) > e->ws_bytes)
+            return BS_ERR_CAPACITY;
+        info.header_bytes = li.header_bytes;
+        info.payload_bytes = li.payload_bytes;
+    }
     bs_ticket* t = nullptr;
     if ((rc = ticket_create(&t))) return rc;
     t->is_prefetch = true;
@@ -238,11 +288,16 @@ int bs_prefetch_async(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs_se
     CK(cudaMemcpyAsync(e->header_buf, h_pinned, hb, cudaMemcpyHostToDevice, e->cstream));
     CK(cudaEventRecord(e->ev_fence_c, e->cstream));
     CK(cudaStreamWaitEvent(e->kstream, e->ev_fence_c, 0));
-    if ((rc = run_deserialize_scan(e->header_buf, nullptr, nbytes, out, d_pool, pool_bytes, flags, L, e->d_result,
-                                   e->sms, e->kstream)))
-        return rc;
+    rc = out ? run_deserialize_scan(e->header_buf, nullptr, nbytes, out, d_pool, pool_bytes, flags, L, e->d_result, e->sms,
+                                    e->kstream)
+             : run_layered_deserialize_plan(e->header_buf, nullptr, nbytes, lout, d_pool, pool_bytes, flags, e->ws, e->ws_bytes,
+                                            e->d_result, e->sms, e->kstream);
+    if (rc) return rc;
     CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
-    if ((rc = run_unpack_range(out, L, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream))) return rc;
+    rc = out ? run_unpack_range(out, L, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream)
+             : run_layered_unpack_range(lout, e->ws, e->ws_bytes, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms,
+                                        e->kstream);
+    if (rc) return rc;
     for (uint32_t k = 0; k < t->n_chunks; ++k) {
         const uint32_t b = k % S;
         const uint64_t lo = hb + (uint64_t)k * C, hi = (lo + C < nbytes) ? lo + C : nbytes;
@@ -250,17 +305,49 @@ int bs_prefetch_async(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs_se
         CK(cudaMemcpyAsync(e->staging[b], (const unsigned char*)h_pinned + lo, hi - lo, cudaMemcpyHostToDevice, e->cstream));
         CK(cudaEventRecord(e->ev_c[b], e->cstream));
         CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));
-        if ((rc = run_unpack_range(out, L, e->staging[b], nullptr, lo, hi, flags | kFlagCheckPad, e->opts, e->sms, e->kstream)))
-            return rc;
+        rc = out ? run_unpack_range(out, L, e->staging[b], nullptr, lo, hi, flags | kFlagCheckPad, e->opts, e->sms, e->kstream)
+                 : run_layered_unpack_range(lout, e->ws, e->ws_bytes, e->staging[b], nullptr, lo, hi, flags | kFlagCheckPad,
+                                            e->opts, e->sms, e->kstream);
+        if (rc) return rc;
         CK(cudaEventRecord(e->ev_k[b], e->kstream));
     }
     CK(cudaEventRecord(t->dma_end, e->cstream));
     // final status (the pad check of the unpack kernels can still flip it) and the checkpoint event
-    CK(cudaMemcpyAsync(&t->h_result->status, &L.head->status, sizeof(int32_t), cudaMemcpyDeviceToHost, e->kstream));
+    CK(cudaMemcpyAsync(&t->h_result->status, &((WsHead*)e->ws)->status, sizeof(int32_t), cudaMemcpyDeviceToHost, e->kstream));
     CK(cudaEventRecord(t->done, e->kstream));
     CK(cudaStreamWaitEvent(consumer, t->done, 0));
     *ticket = t;
     return BS_OK;
+}
+
+extern "C" {
+
+int bs_offload_async(bs_engine* e, const bs_set_desc* set, uint64_t total_bytes, void* h_pinned, uint64_t h_capacity,
+                     cudaStream_t producer, bs_ticket** ticket)
+{
+    if (set == nullptr) return BS_ERR_ARG;
+    return offload_impl(e, set, nullptr, total_bytes, h_pinned, h_capacity, producer, ticket);
+}
+
+int bs_offload_layered_async(bs_engine* e, const bs_layered_desc* set, uint64_t total_bytes, void* h_pinned,
+                             uint64_t h_capacity, cudaStream_t producer, bs_ticket** ticket)
+{
+    if (set == nullptr) return BS_ERR_ARG;
+    return offload_impl(e, nullptr, set, total_bytes, h_pinned, h_capacity, producer, ticket);
+}
+
+int bs_prefetch_async(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs_set_desc* out, void* d_pool,
+                      uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket** ticket)
+{
+    if (out == nullptr) return BS_ERR_ARG;
+    return prefetch_impl(e, h_pinned, nbytes, out, nullptr, d_pool, pool_bytes, flags, consumer, ticket);
+}
+
+int bs_prefetch_layered_async(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs_layered_desc* out, void* d_pool,
+                              uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket** ticket)
+{
+    if (out == nullptr) return BS_ERR_ARG;
+    return prefetch_impl(e, h_pinned, nbytes, nullptr, out, d_pool, pool_bytes, flags, consumer, ticket);
 }
 
 int bs_ticket_query(const bs_ticket* t)

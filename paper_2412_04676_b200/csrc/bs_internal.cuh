@@ -37,11 +37,16 @@ struct __align__(256) WsHead {
     int32_t status;          // first error wins (atomicCAS)
     uint32_t n_tensors;
     uint32_t n_blocks;
-    uint32_t pad0;
+    uint32_t status_pass1;   // layered sets: status after the first plan pass (read by the second)
     uint64_t header_bytes;
     uint64_t payload_bytes;
     uint64_t pool_bytes;
     uint64_t n_granules;     // ceil(P / kGranule)
+    // layered sets (wire format v2, bs_layered.cu): counts and the tickets of the second plan kernel
+    uint32_t n_structs;
+    uint32_t n_struct_blocks;
+    uint32_t scan_ticket2;
+    uint32_t ctas_done2;
 };
 
 struct WsLayout {
@@ -100,6 +105,20 @@ struct ScanParams {
 
 cudaError_t launch_scan(bool deser, const ScanParams& p, int sm_count, cudaStream_t stream);
 
+// ---- layered sets (wire format v2): what the header generator / parser of the move kernels needs ---------
+struct __align__(16) LayerPos {
+    uint64_t off;         // serialize: payload offset of the layer; deserialize: pool offset of the layer
+    uint64_t first_addr;  // index of the layer's first block in addr[] / blk[]
+};
+struct LayeredView {
+    uint32_t on;                   // 0: wire format v1
+    uint32_t C, Bs;                // serialize: counts (deserialize reads them from WsHead)
+    bs_struct_rec* structs;        // descriptor arrays: serialize inputs, deserialize outputs
+    bs_layer_rec* layers;
+    const uint64_t* gs;            // [Bs+1] exclusive prefix of stored sizes over the structure block table | odd bit
+    const LayerPos* lpos;          // [T+1]
+};
+
 // ---- data movement (S3, S5 / S7): stream bytes [lo,hi) <-> blocks ------------------------------------------
 struct MoveParams {
     WsLayout ws;
@@ -114,6 +133,7 @@ struct MoveParams {
     uint32_t tile_bytes;
     uint32_t flags;
     uint32_t tune;                // bs_opts.reserved[0]: experiment switches of the TMA variant
+    LayeredView lay;              // lay.on != 0: qn / dim are the structure block table, header is wire format v2
 };
 
 cudaError_t launch_move(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream);

@@ -1,0 +1,857 @@
+// bs_layered.cu — wire format v2, structure-shared layers (include/bs.h).
+//
+// PAPER Fig 4(a) (L75): "Layers indicate position dependent operators which have the same block-sparse structure,
+// but the dense sector matrices take different values for the different layers."  The meta data of a structure
+// (L63: sector indices, quantum numbers, sector dimensions) is stored once; every layer adds 16 bytes.  The
+// "pointer structure ... grid structure of the serialized data" (L90-92) is built in three small launches before
+// any data moves:
+//   lplan_blocks_kernel : chained scan over the STRUCTURE block table (Bs entries): stored sizes -> gs[] (serialize);
+//                         header validation, stored sizes + pool slot sizes -> gs[], gp[] (deserialize)
+//   lplan_layers_kernel : chained scan over the LAYERS (T entries): bytes and block count of every layer's structure
+//                         -> lpos[] = {payload (or pool) offset, index of the layer's first block}; totals, checks, result
+//   lexpand_kernel      : one warp per layer writes the flat work table the data-movement kernels already use
+//                         (blk[] = {payload offset, block address}, tile_first[]) — B entries, 16 bytes each
+// after which the payload moves through the SAME pack / unpack kernels as wire format v1 (bs_move_tma.cu, bs_move.cu);
+// only their header generator / parser differs (bs_move_common.cuh, *_v2).
+// Roofline: HBM-bound; the three plan launches touch 8 B (address) + 16 B (table entry) per block plus the structure
+// tables, < 0.5 % of the payload traffic; the header itself shrinks from 48 B per block to 48 B per structure block.
+#include <string.h>
+
+#include "bs_internal.cuh"
+
+namespace bs {
+int cuda_fail(cudaError_t e);
+int device_sm_count(int* out);
+
+namespace {
+
+constexpr uint32_t kV2Struct = 32, kV2Layer = 16;
+constexpr uint64_t kFlagAgg = 1ull << 62;
+constexpr uint64_t kFlagPrefix = 2ull << 62;
+constexpr uint64_t kValMask = (1ull << 62) - 1;
+constexpr uint32_t kLThreads = 256, kLItems = 4, kLTile = kLThreads * kLItems;
+
+struct LwLayout {
+    WsLayout ws;        // head, blk, tile_first: what the move kernels see
+    uint64_t* st1[2];   // chained-scan state of the block pass
+    uint64_t* st2[2];   // chained-scan state of the layer pass
+    uint64_t* gs;       // [Bs+1] exclusive prefix of stored sizes over the structure block table | odd flag (bit 0)
+    uint64_t* gp;       // [Bs+1] exclusive prefix of pool slot sizes (deserialize)
+    LayerPos* lpos;     // [T+1]
+    uint64_t blk_cap;   // B the blk[] table can hold (plus the sentinel)
+};
+
+uint64_t lw_fixed_bytes(uint32_t Bs, uint32_t T, uint64_t B)
+{
+    const uint64_t t1 = ((uint64_t)Bs + kLTile) / kLTile + 1, t2 = ((uint64_t)T + kLTile) / kLTile + 1;
+    return sizeof(WsHead) + 2 * align_up(t1 * 8, 256) + 2 * align_up(t2 * 8, 256) + 2 * align_up(((uint64_t)Bs + 1) * 8, 256) +
+           align_up(((uint64_t)T + 1) * sizeof(LayerPos), 256) + align_up((B + 1) * sizeof(Blk), 256);
+}
+
+bool lw_layout(void* d_ws, uint64_t ws_bytes, uint32_t Bs, uint32_t T, uint64_t B, LwLayout* L)
+{
+    const uint64_t fixed = lw_fixed_bytes(Bs, T, B);
+    if (d_ws == nullptr || ((uintptr_t)d_ws & 255) != 0 || ws_bytes < fixed + 16) return false;
+    const uint64_t t1 = ((uint64_t)Bs + kLTile) / kLTile + 1, t2 = ((uint64_t)T + kLTile) / kLTile + 1;
+    unsigned char* p = (unsigned char*)d_ws;
+    L->ws.head = (WsHead*)p;
+    p += sizeof(WsHead);
+    L->ws.scan_state = (uint64_t*)p;
+    for (int c = 0; c < 2; ++c) { L->st1[c] = (uint64_t*)p; p += align_up(t1 * 8, 256); }
+    for (int c = 0; c < 2; ++c) { L->st2[c] = (uint64_t*)p; p += align_up(t2 * 8, 256); }
+    L->ws.zero_bytes = (uint64_t)(p - (unsigned char*)d_ws);
+    L->gs = (uint64_t*)p; p += align_up(((uint64_t)Bs + 1) * 8, 256);
+    L->gp = (uint64_t*)p; p += align_up(((uint64_t)Bs + 1) * 8, 256);
+    L->lpos = (LayerPos*)p; p += align_up(((uint64_t)T + 1) * sizeof(LayerPos), 256);
+    L->ws.blk = (Blk*)p; p += align_up((B + 1) * sizeof(Blk), 256);
+    L->ws.tile_first = (uint32_t*)p;
+    L->ws.n_granules_cap = (ws_bytes - fixed) / 4;
+    L->blk_cap = B;
+    return true;
+}
+
+struct LPlanParams {
+    LwLayout lw;
+    bs_result* result;        // device, may be null
+    uint64_t capacity;        // serialize: stream capacity
+    uint64_t expect_total;    // serialize: if nonzero the total must equal it (engine re-check of the size prediction)
+    // serialize inputs (descriptor arrays, device)
+    const bs_struct_rec* structs;
+    const bs_layer_rec* layers;
+    const uint32_t* dim;
+    const uint64_t* addr;
+    uint32_t C, Bs, T;        // serialize: counts; deserialize: capacities of the out arrays
+    uint64_t n_addr;          // entries of addr[] (deserialize: capacity of out addr)
+    // deserialize inputs
+    const unsigned char* header;   // stream byte 0 .. header_bytes
+    const unsigned char* payload;  // stream byte 0 when the payload is resident behind the header, else null
+    uint64_t nbytes;
+    uint64_t pool_base, pool_bytes;
+    const uint32_t* out_dim;       // BS_SCATTER_TO_ADDR: caller's extents [Bs][3]
+    uint64_t* out_addr;            // pool layout: written; scatter: read
+    uint32_t flags;
+};
+
+__device__ __forceinline__ uint64_t ld_acquire_u64(const uint64_t* p)
+{
+    uint64_t v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u64(uint64_t* p, uint64_t v)
+{
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void set_err(WsHead* h, bs_result* r, int code)
+{
+    if (code == 0) return;
+    atomicCAS(&h->status, 0, code);
+    if (r != nullptr) atomicCAS(&r->status, 0, code);  // the plan result may already have been written
+}
+__device__ __forceinline__ uint64_t warp_incl_scan(uint64_t v, uint32_t lane)
+{
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        uint64_t o = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= (uint32_t)d) v += o;
+    }
+    return v;
+}
+__device__ __forceinline__ uint64_t warp_sum(uint64_t v)
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    return v;
+}
+
+// ---- single-pass chained (decoupled look-back) exclusive scan of NV u64 components over tiles claimed in order ----
+template <int NV>
+struct ChainSmem {
+    uint64_t warp_sum[NV][kLThreads / 32];
+    uint64_t prefix[NV];
+    uint64_t total[NV];
+};
+
+// tsum: this thread's sum per component; on return excl = exclusive prefix of the thread over the whole sequence.
+// Must be called by all kLThreads threads of the CTA; ends with the CTA synchronised.
+template <int NV>
+__device__ __forceinline__ void chained_scan(const uint64_t (&tsum)[NV], uint64_t (&excl)[NV], uint64_t tile, uint64_t* st0,
+                                             uint64_t* st1, ChainSmem<NV>& sm)
+{
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint64_t incl[NV];
+#pragma unroll
+    for (int c = 0; c < NV; ++c) {
+        incl[c] = warp_incl_scan(tsum[c], lane);
+        if (lane == 31) sm.warp_sum[c][warp] = incl[c];
+    }
+    __syncthreads();
+    if (warp < (uint32_t)NV) {  // warp c looks back for component c
+        const int c = (int)warp;
+        uint64_t* state = c == 0 ? st0 : st1;
+        const uint64_t ws = (lane < kLThreads / 32) ? sm.warp_sum[c][lane] : 0;
+        const uint64_t agg = warp_sum(ws);
+        uint64_t pre = 0;
+        if (tile == 0) {
+            if (lane == 0) st_release_u64(state, kFlagPrefix | (agg & kValMask));
+        } else {
+            if (lane == 0) st_release_u64(state + tile, kFlagAgg | (agg & kValMask));
+            int64_t look = (int64_t)tile - 1;
+            for (;;) {
+                const int64_t idx = look - (int64_t)lane;
+                uint64_t w = (idx >= 0) ? ld_acquire_u64(state + idx) : kFlagPrefix;
+                while (__any_sync(0xffffffffu, (w >> 62) == 0)) {
+                    if ((w >> 62) == 0) w = ld_acquire_u64(state + idx);
+                }
+                const uint32_t is_prefix = __ballot_sync(0xffffffffu, (w >> 62) == 2);
+                const uint32_t first = is_prefix ? (uint32_t)__ffs((int)is_prefix) - 1u : 32u;
+                pre += warp_sum(lane <= first ? (w & kValMask) : 0ull);
+                if (is_prefix) break;
+                look -= 32;
+            }
+            if (lane == 0) st_release_u64(state + tile, kFlagPrefix | ((pre + agg) & kValMask));
+        }
+        if (lane == 0) { sm.prefix[c] = pre; sm.total[c] = agg; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < NV; ++c) {
+        uint64_t run = sm.prefix[c] + (incl[c] - tsum[c]);
+        for (uint32_t w = 0; w < warp; ++w) run += sm.warp_sum[c][w];
+        excl[c] = run;
+    }
+}
+
+struct StructHead {
+    uint32_t rank, first, n;
+    uint64_t layer_bytes;
+};
+__device__ __forceinline__ StructHead load_struct(const void* recs, uint64_t s)
+{
+    const uint4* r = reinterpret_cast<const uint4*>(recs) + 2 * s;
+    const uint4 a = __ldg(r), b = __ldg(r + 1);
+    StructHead h;
+    h.rank = a.x; h.first = a.y; h.n = a.z;
+    h.layer_bytes = (uint64_t)b.z | ((uint64_t)b.w << 32);
+    return h;
+}
+
+// ---- pass 1: the structure block table -------------------------------------------------------------------------
+template <bool DESER>
+__global__ void __launch_bounds__(kLThreads) lplan_blocks_kernel(const LPlanParams p)
+{
+    __shared__ uint32_t s_tile;
+    __shared__ ChainSmem<2> sm;
+    WsHead* head = p.lw.ws.head;
+    const uint32_t tid = threadIdx.x;
+    constexpr int kErrBad = DESER ? BS_ERR_CORRUPT : BS_ERR_ARG;
+    constexpr int kErrRank = DESER ? BS_ERR_CORRUPT : BS_ERR_UNSUPPORTED;
+
+    uint64_t C = p.C, Bs = p.Bs, T = p.T, hb = 0;
+    bool ok = true;
+    if (DESER) {  // the fixed header, field by field in stream order
+        int code = 0;
+        C = Bs = T = 0;
+        if (p.nbytes < kFixedHeader) {
+            code = BS_ERR_CORRUPT;
+        } else {
+            const uint4* f = reinterpret_cast<const uint4*>(p.header);
+            const uint4 w0 = __ldg(f), w1 = __ldg(f + 1), w2 = __ldg(f + 2), w3 = __ldg(f + 3);
+            const uint64_t hC = w2.x, hBs = w2.y, hT = (uint64_t)w2.z | ((uint64_t)w2.w << 32);
+            const uint64_t hH = (uint64_t)w3.x | ((uint64_t)w3.y << 32), hP = (uint64_t)w3.z | ((uint64_t)w3.w << 32);
+            if (w0.x != 0x41505342u || w0.y != 0x31455352u)      code = BS_ERR_CORRUPT;  // "BSPARSE1"
+            else if (w0.z != 2u)                                  code = BS_ERR_CORRUPT;  // version
+            else if (w0.w != 0x01020304u)                         code = BS_ERR_CORRUPT;  // endian_tag
+            else if (w1.x != 0u)                                  code = BS_ERR_CORRUPT;  // dtype f64
+            else if (w1.y != 2u)                                  code = BS_ERR_CORRUPT;  // n_qn
+            else if (w1.z != 3u)                                  code = BS_ERR_CORRUPT;  // max_rank
+            else if (w1.w != 16u)                                 code = BS_ERR_CORRUPT;  // align
+            else if (hT >= (1ull << 32))                          code = BS_ERR_CORRUPT;
+            else if (hH != align_up(kFixedHeader + kV2Struct * hC + kV2Layer * hT + kBlockRec * hBs, kHeaderAlign)) code = BS_ERR_CORRUPT;
+            else if (hH > p.nbytes || hP != p.nbytes - hH)        code = BS_ERR_CORRUPT;
+            else if (hC > p.C || hBs > p.Bs || hT > p.T)          code = BS_ERR_CAPACITY;  // out arrays too small
+            else { C = hC; Bs = hBs; T = hT; hb = hH; }
+            if (blockIdx.x == 0 && tid == 0 && (code == 0 || code == BS_ERR_CAPACITY)) {
+                head->n_structs = (uint32_t)hC; head->n_struct_blocks = (uint32_t)hBs; head->n_tensors = (uint32_t)hT;
+                head->header_bytes = hH; head->payload_bytes = hP;
+            }
+        }
+        if (code != 0) {
+            ok = false;
+            if (blockIdx.x == 0 && tid == 0) set_err(head, nullptr, code);
+        }
+    }
+    const void* srecs = DESER ? (const void*)(p.header + kFixedHeader) : (const void*)p.structs;
+
+    // ---- structure records partition the structure block table in order ----
+    if (ok) {
+        for (uint64_t s = (uint64_t)blockIdx.x * kLThreads + tid; s < C; s += (uint64_t)gridDim.x * kLThreads) {
+            const StructHead h = load_struct(srecs, s);
+            uint64_t prev_end = 0;
+            if (s > 0) {
+                const StructHead q = load_struct(srecs, s - 1);
+                prev_end = (uint64_t)q.first + q.n;
+            }
+            int code = 0;
+            if (h.rank != 2 && h.rank != 3) code = kErrRank;
+            else if (h.first != prev_end) code = kErrBad;
+            else if ((uint64_t)h.first + h.n > Bs) code = kErrBad;
+            else if (s == C - 1 && (uint64_t)h.first + h.n != Bs) code = kErrBad;
+            set_err(head, nullptr, code);
+        }
+        if (C == 0 && Bs != 0 && blockIdx.x == 0 && tid == 0) set_err(head, nullptr, kErrBad);
+        if (DESER && blockIdx.x == 0) {  // header slack must be zero
+            const uint64_t used = kFixedHeader + kV2Struct * C + kV2Layer * T + kBlockRec * Bs;
+            const uint64_t z = used + 16ull * tid;
+            if (z < hb) {
+                const uint4 w = __ldg(reinterpret_cast<const uint4*>(p.header + z));
+                if ((w.x | w.y | w.z | w.w) != 0) set_err(head, nullptr, BS_ERR_CORRUPT);
+            }
+        }
+        if (Bs == 0 && blockIdx.x == 0 && tid == 0) { p.lw.gs[0] = 0; p.lw.gp[0] = 0; }
+    }
+
+    const uint64_t n_tiles = ok ? (Bs + kLTile - 1) / kLTile : 0;
+    const unsigned char* brec = DESER ? p.header + kFixedHeader + kV2Struct * C + kV2Layer * T : nullptr;
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_tile = atomicAdd(&head->scan_ticket, 1u);
+        __syncthreads();
+        const uint64_t tile = s_tile;
+        if (tile >= n_tiles) break;
+
+        uint64_t stored[kLItems], slot[kLItems];
+        uint32_t oddf[kLItems];
+        uint64_t tsum[2] = {0, 0};
+        int err = 0;
+#pragma unroll
+        for (uint32_t k = 0; k < kLItems; ++k) {
+            const uint64_t j = tile * kLTile + (uint64_t)tid * kLItems + k;
+            const bool valid = j < Bs;
+            uint32_t d0 = 1, d1 = 1, d2 = 0, owner = 0;
+            int32_t q4 = 0, q5 = 0;
+            uint64_t offset = 0;
+            if (valid) {
+                if (DESER) {
+                    const uint4* r = reinterpret_cast<const uint4*>(brec + kBlockRec * j);
+                    const uint4 r1 = __ldg(r + 1), r2 = __ldg(r + 2);
+                    q4 = (int32_t)r1.x; q5 = (int32_t)r1.y;
+                    d0 = r1.z; d1 = r1.w; d2 = r2.x; owner = r2.y;
+                    offset = (uint64_t)r2.z | ((uint64_t)r2.w << 32);
+                } else {
+                    d0 = __ldg(p.dim + 3 * j); d1 = __ldg(p.dim + 3 * j + 1); d2 = __ldg(p.dim + 3 * j + 2);
+                }
+            }
+            const uint64_t n01 = (uint64_t)d0 * d1;
+            uint64_t n = n01 * d2;
+            if (valid && (__umul64hi(n01, (uint64_t)d2) != 0 || n >= (1ull << 57))) { err = kErrBad; n = 0; }
+            const uint64_t nbytes = n * 8;
+            const uint64_t st = (nbytes + 15) & ~15ull;
+            stored[k] = valid ? st : 0;
+            slot[k] = (DESER && valid) ? align_up(nbytes, kPoolAlign) : 0;
+            oddf[k] = (uint32_t)(n & 1);
+            if (DESER && valid) {
+                if (owner >= C) err = BS_ERR_CORRUPT;
+                else {
+                    const StructHead h = load_struct(srecs, owner);
+                    const uint64_t end = (uint64_t)h.first + h.n;
+                    if (j < h.first || j >= end) err = BS_ERR_CORRUPT;
+                    else {
+                        if (h.rank == 2 && (d2 != 1 || q4 != 0 || q5 != 0)) err = BS_ERR_CORRUPT;
+                        // relative offsets = exclusive prefix sum inside the structure, checked link by link
+                        uint64_t next = h.layer_bytes;
+                        if (j + 1 < end) next = __ldg(reinterpret_cast<const unsigned long long*>(brec + kBlockRec * (j + 1) + 40));
+                        if (j == h.first && offset != 0) err = BS_ERR_CORRUPT;
+                        if (offset >= (1ull << 62) || offset + st != next) err = BS_ERR_CORRUPT;
+                    }
+                }
+                if (p.flags == BS_SCATTER_TO_ADDR &&
+                    (__ldg(p.out_dim + 3 * j) != d0 || __ldg(p.out_dim + 3 * j + 1) != d1 || __ldg(p.out_dim + 3 * j + 2) != d2)) {
+                    if (!err) err = BS_ERR_ARG;
+                }
+            }
+            tsum[0] += stored[k];
+            tsum[1] += slot[k];
+        }
+        if (err) set_err(head, nullptr, err);
+        uint64_t excl[2];
+        chained_scan<2>(tsum, excl, tile, p.lw.st1[0], p.lw.st1[1], sm);
+        uint64_t r0 = excl[0], r1 = excl[1];
+#pragma unroll
+        for (uint32_t k = 0; k < kLItems; ++k) {
+            const uint64_t j = tile * kLTile + (uint64_t)tid * kLItems + k;
+            if (j < Bs) {
+                p.lw.gs[j] = r0 | oddf[k];
+                p.lw.gp[j] = r1;
+            }
+            r0 += stored[k];
+            r1 += slot[k];
+        }
+        if (tile == n_tiles - 1 && tid == 0) {  // the owner of the last tile knows the totals
+            p.lw.gs[Bs] = sm.prefix[0] + sm.total[0];
+            p.lw.gp[Bs] = sm.prefix[1] + sm.total[1];
+        }
+    }
+    // last CTA out: snapshot of the status for the second pass
+    __shared__ uint32_t s_last;
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        s_last = (atomicAdd(&head->ctas_done, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last && tid == 0) {
+        __threadfence();
+        volatile WsHead* vh = head;
+        vh->status_pass1 = (uint32_t)vh->status;
+        __threadfence();
+    }
+}
+
+// ---- pass 2: the layers --------------------------------------------------------------------------------------------
+template <bool DESER>
+__global__ void __launch_bounds__(kLThreads) lplan_layers_kernel(const LPlanParams p)
+{
+    __shared__ uint32_t s_tile;
+    __shared__ uint32_t s_last;
+    __shared__ ChainSmem<2> sm;
+    WsHead* head = p.lw.ws.head;
+    volatile WsHead* vh = head;
+    const uint32_t tid = threadIdx.x;
+    const bool bad = vh->status_pass1 != 0;  // snapshot taken by the first pass: uniform over the grid (tiles are ticketed)
+    uint64_t C = p.C, Bs = p.Bs, T = p.T, hb, P_hdr = 0;
+    if (DESER) {
+        C = vh->n_structs; Bs = vh->n_struct_blocks; T = vh->n_tensors; hb = vh->header_bytes; P_hdr = vh->payload_bytes;
+    } else {
+        hb = align_up(kFixedHeader + kV2Struct * C + kV2Layer * T + kBlockRec * Bs, kHeaderAlign);
+    }
+    const void* srecs = DESER ? (const void*)(p.header + kFixedHeader) : (const void*)p.structs;
+    const bs_layer_rec* ly = DESER ? reinterpret_cast<const bs_layer_rec*>(p.header + kFixedHeader + kV2Struct * C) : p.layers;
+    constexpr int kErrBad = DESER ? BS_ERR_CORRUPT : BS_ERR_ARG;
+
+    const uint64_t n_tiles = bad ? 0 : (T + kLTile - 1) / kLTile;
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_tile = atomicAdd(&head->scan_ticket2, 1u);
+        __syncthreads();
+        const uint64_t tile = s_tile;
+        if (tile >= n_tiles) break;
+        uint64_t vb[kLItems], vn[kLItems];
+        uint64_t tsum[2] = {0, 0};
+        int err = 0;
+#pragma unroll
+        for (uint32_t k = 0; k < kLItems; ++k) {
+            const uint64_t t = tile * kLTile + (uint64_t)tid * kLItems + k;
+            vb[k] = 0; vn[k] = 0;
+            if (t < T) {
+                const uint4 w = __ldg(reinterpret_cast<const uint4*>(ly + t));  // structure, tag, offset
+                const uint32_t s = w.x;
+                if (s >= C) err = kErrBad;
+                else {
+                    const StructHead h = load_struct(srecs, s);
+                    const uint64_t* g = DESER ? p.lw.gp : p.lw.gs;
+                    vb[k] = (g[(uint64_t)h.first + h.n] & ~15ull) - (g[h.first] & ~15ull);
+                    vn[k] = h.n;
+                    if (DESER) {  // layer offsets = exclusive prefix sum of layer_bytes, checked link by link, inside [0, P]
+                        const uint64_t off = (uint64_t)w.z | ((uint64_t)w.w << 32);
+                        uint64_t next = P_hdr;
+                        if (t + 1 < T) next = __ldg(reinterpret_cast<const unsigned long long*>(&ly[t + 1].offset));
+                        if (t == 0 && off != 0) err = BS_ERR_CORRUPT;
+                        if (off > P_hdr || h.layer_bytes > P_hdr - off || off + h.layer_bytes != next) err = BS_ERR_CORRUPT;
+                    }
+                }
+            }
+            tsum[0] += vb[k];
+            tsum[1] += vn[k];
+        }
+        if (err) set_err(head, nullptr, err);
+        uint64_t excl[2];
+        chained_scan<2>(tsum, excl, tile, p.lw.st2[0], p.lw.st2[1], sm);
+        uint64_t r0 = excl[0], r1 = excl[1];
+#pragma unroll
+        for (uint32_t k = 0; k < kLItems; ++k) {
+            const uint64_t t = tile * kLTile + (uint64_t)tid * kLItems + k;
+            if (t < T) {
+                LayerPos lp; lp.off = r0; lp.first_addr = r1;
+                p.lw.lpos[t] = lp;
+            }
+            r0 += vb[k];
+            r1 += vn[k];
+        }
+        if (tile == n_tiles - 1 && tid == 0) {
+            LayerPos lp; lp.off = sm.prefix[0] + sm.total[0]; lp.first_addr = sm.prefix[1] + sm.total[1];
+            p.lw.lpos[T] = lp;
+        }
+    }
+
+    // ---- last CTA out: totals, capacity checks, sentinel, result ----
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        s_last = (atomicAdd(&head->ctas_done2, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last && tid == 0) {
+        __threadfence();
+        int status = vh->status;
+        uint64_t tot_bytes = 0, tot_blocks = 0;
+        if (!bad && T != 0) {
+            const volatile LayerPos* end = p.lw.lpos + T;
+            tot_bytes = end->off; tot_blocks = end->first_addr;
+        } else if (!bad) {
+            LayerPos lp; lp.off = 0; lp.first_addr = 0;
+            p.lw.lpos[0] = lp;
+        }
+        uint64_t P = DESER ? P_hdr : tot_bytes;
+        uint64_t pool = DESER ? tot_bytes : 0;
+        if (bad) { P = 0; pool = 0; }
+        const uint64_t total = hb + P;
+        const uint64_t ng = (P + kGranule - 1) / kGranule;
+        if (status == 0) {
+            if (DESER && T == 0 && P_hdr != 0) status = BS_ERR_CORRUPT;
+            else if (tot_blocks >= (1ull << 32)) status = BS_ERR_UNSUPPORTED;
+            else if (!DESER && total > p.capacity) status = BS_ERR_CAPACITY;
+            else if (!DESER && p.expect_total != 0 && total != p.expect_total) status = BS_ERR_ARG;
+            else if (ng + 1 > p.lw.ws.n_granules_cap) status = BS_ERR_CAPACITY;
+            else if (tot_blocks > p.lw.blk_cap || tot_blocks > p.n_addr) status = BS_ERR_CAPACITY;
+            else if (DESER && p.flags == BS_LAYOUT_POOL && pool > p.pool_bytes) status = BS_ERR_CAPACITY;
+        }
+        if (!bad && tot_blocks <= p.lw.blk_cap) {
+            Blk e; e.off = P; e.addr = 0;
+            p.lw.ws.blk[tot_blocks] = e;
+            if (ng < p.lw.ws.n_granules_cap) p.lw.ws.tile_first[ng] = (uint32_t)tot_blocks;
+        }
+        vh->n_structs = (uint32_t)C;
+        vh->n_struct_blocks = (uint32_t)Bs;
+        vh->n_tensors = (uint32_t)T;
+        vh->n_blocks = (uint32_t)tot_blocks;
+        vh->header_bytes = hb;
+        vh->payload_bytes = P;
+        vh->pool_bytes = pool;
+        vh->n_granules = ng;
+        vh->status = status;
+        if (p.result != nullptr) {
+            bs_result r;
+            r.total_bytes = total; r.header_bytes = hb; r.payload_bytes = P; r.pool_bytes = pool;
+            r.status = status; r.n_tensors = (uint32_t)T; r.n_blocks = (uint32_t)tot_blocks;
+            r.reserved[0] = (uint32_t)C; r.reserved[1] = (uint32_t)Bs;
+            for (int z = 2; z < 5; ++z) r.reserved[z] = 0;
+            *p.result = r;
+        }
+        __threadfence();
+    }
+}
+
+// ---- pass 3: one warp per layer writes the flat work table blk[] / tile_first[] ------------------------------------------
+template <bool DESER>
+__global__ void __launch_bounds__(kLThreads) lexpand_kernel(const LPlanParams p)
+{
+    __shared__ uint32_t s_big_idx[kLThreads];
+    __shared__ uint32_t s_big_cnt[kLThreads];
+    __shared__ uint64_t s_big_g0[kLThreads];
+    WsHead* head = p.lw.ws.head;
+    if (head->status != 0) return;  // deferred error: no table, and the move kernels will write nothing
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint64_t C = head->n_structs, T = head->n_tensors, hb = head->header_bytes;
+    const void* srecs = DESER ? (const void*)(p.header + kFixedHeader) : (const void*)p.structs;
+    const bs_layer_rec* ly = DESER ? reinterpret_cast<const bs_layer_rec*>(p.header + kFixedHeader + kV2Struct * C) : p.layers;
+    const uint64_t n_warps = (uint64_t)gridDim.x * (kLThreads / 32);
+    uint32_t* big_idx = s_big_idx + warp * 32;
+    uint32_t* big_cnt = s_big_cnt + warp * 32;
+    uint64_t* big_g0 = s_big_g0 + warp * 32;
+
+    for (uint64_t t = (uint64_t)blockIdx.x * (kLThreads / 32) + warp; t < T; t += n_warps) {
+        const uint4 w = __ldg(reinterpret_cast<const uint4*>(ly + t));
+        const StructHead h = load_struct(srecs, w.x);
+        const LayerPos lp = p.lw.lpos[t];
+        const uint64_t base_off = DESER ? ((uint64_t)w.z | ((uint64_t)w.w << 32)) : lp.off;
+        const uint64_t gs_f = p.lw.gs[h.first] & ~15ull;
+        const uint64_t gp_f = DESER ? p.lw.gp[h.first] : 0;
+        for (uint32_t j0 = 0; j0 < h.n; j0 += 32) {
+            const uint32_t j = j0 + lane;
+            bool big = false;
+            uint64_t g0 = 0, cnt = 0;
+            uint64_t i = 0;
+            if (j < h.n) {
+                const uint64_t g = p.lw.gs[(uint64_t)h.first + j], gn = p.lw.gs[(uint64_t)h.first + j + 1];
+                const uint64_t off = base_off + ((g & ~15ull) - gs_f);
+                const uint64_t stored = (gn & ~15ull) - (g & ~15ull);
+                const uint64_t odd = g & 1ull;
+                i = lp.first_addr + j;
+                uint64_t address;
+                if (!DESER) {
+                    address = __ldg(reinterpret_cast<const unsigned long long*>(p.addr + i));
+                    if (address & 7) set_err(head, p.result, BS_ERR_ARG);  // D16
+                } else if (p.flags == BS_SCATTER_TO_ADDR) {
+                    address = __ldg(reinterpret_cast<const unsigned long long*>(p.out_addr + i));
+                    if (address & 7) set_err(head, p.result, BS_ERR_ARG);
+                } else {
+                    address = p.pool_base + lp.off + (p.lw.gp[(uint64_t)h.first + j] - gp_f);
+                    p.out_addr[i] = address;
+                }
+                if (DESER && odd && p.payload != nullptr) {  // pad bytes are zero
+                    const uint64_t pad = __ldg(reinterpret_cast<const unsigned long long*>(p.payload + hb + off + stored - 8));
+                    if (pad != 0) set_err(head, p.result, BS_ERR_CORRUPT);
+                }
+                Blk e;
+                e.off = off;
+                e.addr = (address & ~7ull) | odd;
+                p.lw.ws.blk[i] = e;
+                // granule boundaries g*kGranule inside [off, off + stored)
+                g0 = (off + kGranule - 1) / kGranule;
+                const uint64_t g1 = (off + stored + kGranule - 1) / kGranule;
+                cnt = g1 > g0 ? g1 - g0 : 0;
+                if (cnt <= 4) {
+                    for (uint64_t q = 0; q < cnt; ++q)
+                        if (g0 + q < p.lw.ws.n_granules_cap) p.lw.ws.tile_first[g0 + q] = (uint32_t)i;
+                } else {
+                    big = true;
+                }
+            }
+            // large blocks: the whole warp fills their boundaries
+            const uint32_t bigs = __ballot_sync(0xffffffffu, big);
+            if (bigs) {
+                if (big) {
+                    const uint32_t slot = __popc(bigs & ((1u << lane) - 1u));
+                    big_idx[slot] = (uint32_t)i;
+                    big_g0[slot] = g0;
+                    big_cnt[slot] = cnt > 0xffffffffull ? 0xffffffffu : (uint32_t)cnt;
+                }
+                __syncwarp();
+                const uint32_t nb = __popc(bigs);
+                for (uint32_t s = 0; s < nb; ++s) {
+                    const uint64_t b0 = big_g0[s];
+                    const uint32_t c = big_cnt[s], idx = big_idx[s];
+                    for (uint64_t q = lane; q < c; q += 32)
+                        if (b0 + q < p.lw.ws.n_granules_cap) p.lw.ws.tile_first[b0 + q] = idx;
+                }
+                __syncwarp();
+            }
+        }
+    }
+}
+
+int check_layered(const bs_layered_desc* s)
+{
+    if (s == nullptr) return BS_ERR_ARG;
+    if (s->n_qn != 2 || s->dtype != BS_F64) return BS_ERR_UNSUPPORTED;
+    auto al = [](const void* q, uintptr_t a) { return ((uintptr_t)q & (a - 1)) == 0; };
+    if (s->n_structs && (s->structs == nullptr || !al(s->structs, 16))) return BS_ERR_ARG;
+    if (s->n_layers && (s->layers == nullptr || !al(s->layers, 16))) return BS_ERR_ARG;
+    if (s->n_struct_blocks && (s->qn == nullptr || !al(s->qn, 8))) return BS_ERR_ARG;
+    if (s->n_struct_blocks && (s->dim == nullptr || !al(s->dim, 4))) return BS_ERR_ARG;
+    if (s->n_addr && (s->addr == nullptr || !al(s->addr, 8))) return BS_ERR_ARG;
+    if (s->n_addr >= (1ull << 32)) return BS_ERR_UNSUPPORTED;
+    return BS_OK;
+}
+
+unsigned grid_for(uint64_t items, uint64_t per_cta, int sms, int per_sm)
+{
+    uint64_t want = (items + per_cta - 1) / per_cta;
+    const uint64_t cap = (uint64_t)sms * per_sm;
+    if (want > cap) want = cap;
+    return want == 0 ? 1u : (unsigned)want;
+}
+
+}  // namespace
+
+// ---- entry points used by bs_engine.cu -----------------------------------------------------------------------------------
+bool layered_ws(void* d_ws, uint64_t ws_bytes, uint32_t Bs, uint32_t T, uint64_t B, WsLayout* out)
+{
+    LwLayout L;
+    if (!lw_layout(d_ws, ws_bytes, Bs, T, B, &L)) return false;
+    *out = L.ws;
+    return true;
+}
+
+LayeredView layered_view(const bs_layered_desc* d, void* d_ws, uint64_t ws_bytes)
+{
+    LayeredView v;
+    memset(&v, 0, sizeof(v));
+    LwLayout L;
+    if (!lw_layout(d_ws, ws_bytes, d->n_struct_blocks, d->n_layers, d->n_addr, &L)) return v;
+    v.on = 1;
+    v.C = d->n_structs;
+    v.Bs = d->n_struct_blocks;
+    v.structs = d->structs;
+    v.layers = d->layers;
+    v.gs = L.gs;
+    v.lpos = L.lpos;
+    return v;
+}
+
+// the three plan launches of a layered serialize (S1, S2, S4 for wire format v2)
+int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t capacity,
+                               uint64_t expect_total, bs_result* d_result, int sms, cudaStream_t stream)
+{
+    LPlanParams p;
+    memset(&p, 0, sizeof(p));
+    if (!lw_layout(d_ws, ws_bytes, set->n_struct_blocks, set->n_layers, set->n_addr, &p.lw)) return BS_ERR_CAPACITY;
+    cudaError_t e = cudaMemsetAsync(p.lw.ws.head, 0, p.lw.ws.zero_bytes, stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    p.result = d_result;
+    p.capacity = capacity;
+    p.expect_total = expect_total;
+    p.structs = set->structs;
+    p.layers = set->layers;
+    p.dim = set->dim;
+    p.addr = set->addr;
+    p.C = set->n_structs;
+    p.Bs = set->n_struct_blocks;
+    p.T = set->n_layers;
+    p.n_addr = set->n_addr;
+    const unsigned g1 = grid_for(p.Bs > p.C ? p.Bs : p.C, kLTile, sms, 4);
+    lplan_blocks_kernel<false><<<g1, kLThreads, 0, stream>>>(p);
+    lplan_layers_kernel<false><<<grid_for(p.T, kLTile, sms, 4), kLThreads, 0, stream>>>(p);
+    lexpand_kernel<false><<<grid_for(p.T, kLThreads / 32, sms, 8), kLThreads, 0, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    return BS_OK;
+}
+
+int run_layered_deserialize_plan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_layered_desc* out,
+                                 void* d_pool, uint64_t pool_bytes, uint32_t flags, void* d_ws, uint64_t ws_bytes,
+                                 bs_result* d_result, int sms, cudaStream_t stream)
+{
+    LPlanParams p;
+    memset(&p, 0, sizeof(p));
+    if (!lw_layout(d_ws, ws_bytes, out->n_struct_blocks, out->n_layers, out->n_addr, &p.lw)) return BS_ERR_CAPACITY;
+    cudaError_t e = cudaMemsetAsync(p.lw.ws.head, 0, p.lw.ws.zero_bytes, stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    p.result = d_result;
+    p.C = out->n_structs;
+    p.Bs = out->n_struct_blocks;
+    p.T = out->n_layers;
+    p.n_addr = out->n_addr;
+    p.header = (const unsigned char*)d_header;
+    p.payload = (const unsigned char*)d_payload;
+    p.nbytes = nbytes;
+    p.pool_base = (uint64_t)(uintptr_t)d_pool;
+    p.pool_bytes = pool_bytes;
+    p.out_dim = out->dim;
+    p.out_addr = out->addr;
+    p.flags = flags;
+    const unsigned g1 = grid_for(p.Bs > p.C ? p.Bs : p.C, kLTile, sms, 4);
+    lplan_blocks_kernel<true><<<g1, kLThreads, 0, stream>>>(p);
+    lplan_layers_kernel<true><<<grid_for(p.T, kLTile, sms, 4), kLThreads, 0, stream>>>(p);
+    lexpand_kernel<true><<<grid_for(p.T, kLThreads / 32, sms, 8), kLThreads, 0, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    return BS_OK;
+}
+
+int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, void* d_dst, uint64_t lo, uint64_t hi,
+                           const bs_opts& o, int sms, cudaStream_t stream)
+{
+    MoveParams mp;
+    memset(&mp, 0, sizeof(mp));
+    if (!layered_ws(d_ws, ws_bytes, set->n_struct_blocks, set->n_layers, set->n_addr, &mp.ws)) return BS_ERR_CAPACITY;
+    mp.lay = layered_view(set, d_ws, ws_bytes);
+    mp.qn = set->qn;
+    mp.dim = set->dim;
+    mp.addr = set->addr;
+    mp.stream = (unsigned char*)d_dst;
+    mp.lo = lo;
+    mp.hi = hi;
+    mp.tile_bytes = o.tile_bytes;
+    mp.tune = o.reserved[0];
+    cudaError_t e = launch_move(false, mp, o, sms, stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return BS_OK;
+}
+
+int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws_bytes, const void* d_src,
+                             const void* d_header, uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms,
+                             cudaStream_t stream)
+{
+    MoveParams mp;
+    memset(&mp, 0, sizeof(mp));
+    if (!layered_ws(d_ws, ws_bytes, out->n_struct_blocks, out->n_layers, out->n_addr, &mp.ws)) return BS_ERR_CAPACITY;
+    mp.lay = layered_view(out, d_ws, ws_bytes);
+    mp.qn = out->qn;
+    mp.dim = out->dim;
+    mp.addr = out->addr;
+    mp.stream = (unsigned char*)const_cast<void*>(d_src);
+    mp.header = (const unsigned char*)d_header;
+    mp.lo = lo;
+    mp.hi = hi;
+    mp.tile_bytes = o.tile_bytes;
+    mp.tune = o.reserved[0];
+    mp.flags = flags;
+    cudaError_t e = launch_move(true, mp, o, sms, stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return BS_OK;
+}
+
+int check_opts(const bs_opts& o);
+
+}  // namespace bs
+
+using namespace bs;
+
+extern "C" {
+
+uint64_t bs_layered_header_bytes(uint64_t n_structs, uint64_t n_layers, uint64_t n_struct_blocks)
+{
+    return align_up(kFixedHeader + kV2Struct * n_structs + kV2Layer * n_layers + kBlockRec * n_struct_blocks, kHeaderAlign);
+}
+
+uint64_t bs_layered_workspace_bytes(uint32_t n_structs, uint32_t n_struct_blocks, uint32_t n_layers, uint64_t n_addr,
+                                    uint64_t stream_capacity)
+{
+    (void)n_structs;
+    return lw_fixed_bytes(n_struct_blocks, n_layers, n_addr) + align_up(4 * (stream_capacity / kGranule + 4), 256);
+}
+
+int bs_layered_stream_info(const void* h, bs_layered_stream_info_t* out)
+{
+    if (h == nullptr || out == nullptr) return BS_ERR_ARG;
+    const unsigned char* s = (const unsigned char*)h;
+    uint32_t w[10];
+    uint64_t q[3];
+    memcpy(w, s, 40);
+    memcpy(q, s + 40, 24);
+    if (memcmp(s, "BSPARSE1", 8) != 0) return BS_ERR_CORRUPT;
+    if (w[2] != 2u || w[3] != 0x01020304u || w[4] != 0u || w[5] != 2u || w[6] != 3u || w[7] != 16u) return BS_ERR_CORRUPT;
+    if (q[0] >= (1ull << 32)) return BS_ERR_CORRUPT;
+    if (q[1] != bs_layered_header_bytes(w[8], q[0], w[9])) return BS_ERR_CORRUPT;
+    out->n_structs = w[8];
+    out->n_struct_blocks = w[9];
+    out->n_layers = q[0];
+    out->header_bytes = q[1];
+    out->payload_bytes = q[2];
+    out->total_bytes = q[1] + q[2];
+    return BS_OK;
+}
+
+int bs_layered_serialized_size(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t* header_bytes,
+                               uint64_t* total_bytes, cudaStream_t stream)
+{
+    int rc = check_layered(set);
+    if (rc) return rc;
+    if (header_bytes == nullptr || total_bytes == nullptr) return BS_ERR_ARG;
+    int sms;
+    if ((rc = device_sm_count(&sms))) return rc;
+    if ((rc = run_layered_serialize_plan(set, d_ws, ws_bytes, UINT64_MAX, 0, nullptr, sms, stream))) return rc;
+    WsHead h;
+    cudaError_t e = cudaMemcpyAsync(&h, d_ws, sizeof(h), cudaMemcpyDeviceToHost, stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    *header_bytes = h.header_bytes;
+    *total_bytes = h.header_bytes + h.payload_bytes;
+    if (h.status == BS_ERR_CAPACITY) return BS_OK;  // a workspace too small for the tile index is fine for a size query
+    return h.status;
+}
+
+int bs_layered_serialize_range(const bs_layered_desc* set, void* d_dst, uint64_t lo, uint64_t hi, int run_scan, void* d_ws,
+                               uint64_t ws_bytes, bs_result* d_result, const bs_opts* opts, cudaStream_t stream)
+{
+    int rc = check_layered(set);
+    if (rc) return rc;
+    if (d_dst == nullptr || ((uintptr_t)d_dst & 15) || (lo & 15) || (hi & 15) || lo > hi) return BS_ERR_ARG;
+    bs_opts o;
+    resolve_opts(opts, &o);
+    if ((rc = check_opts(o))) return rc;
+    int sms;
+    if ((rc = device_sm_count(&sms))) return rc;
+    if (run_scan && (rc = run_layered_serialize_plan(set, d_ws, ws_bytes, UINT64_MAX, 0, d_result, sms, stream))) return rc;
+    return run_layered_pack_range(set, d_ws, ws_bytes, d_dst, lo, hi, o, sms, stream);
+}
+
+int bs_layered_serialize(const bs_layered_desc* set, void* d_stream, uint64_t capacity, void* d_ws, uint64_t ws_bytes,
+                         bs_result* d_result, const bs_opts* opts, cudaStream_t stream)
+{
+    int rc = check_layered(set);
+    if (rc) return rc;
+    if (d_stream == nullptr || ((uintptr_t)d_stream & 15)) return BS_ERR_ARG;
+    bs_opts o;
+    resolve_opts(opts, &o);
+    if ((rc = check_opts(o))) return rc;
+    int sms;
+    if ((rc = device_sm_count(&sms))) return rc;
+    if ((rc = run_layered_serialize_plan(set, d_ws, ws_bytes, capacity, 0, d_result, sms, stream))) return rc;
+    return run_layered_pack_range(set, d_ws, ws_bytes, d_stream, 0, capacity & ~15ull, o, sms, stream);
+}
+
+int bs_layered_deserialize(const void* d_stream, uint64_t nbytes, bs_layered_desc* out, void* d_pool, uint64_t pool_bytes,
+                           uint32_t flags, void* d_ws, uint64_t ws_bytes, bs_result* d_result, const bs_opts* opts,
+                           cudaStream_t stream)
+{
+    int rc = check_layered(out);
+    if (rc) return rc;
+    if (d_stream == nullptr || ((uintptr_t)d_stream & 15)) return BS_ERR_ARG;
+    if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
+    if (flags == BS_LAYOUT_POOL && pool_bytes && (d_pool == nullptr || ((uintptr_t)d_pool & 255))) return BS_ERR_ARG;
+    bs_opts o;
+    resolve_opts(opts, &o);
+    if ((rc = check_opts(o))) return rc;
+    int sms;
+    if ((rc = device_sm_count(&sms))) return rc;
+    const unsigned char* s = (const unsigned char*)d_stream;
+    if ((rc = run_layered_deserialize_plan(s, s, nbytes, out, d_pool, pool_bytes, flags, d_ws, ws_bytes, d_result, sms, stream)))
+        return rc;
+    return run_layered_unpack_range(out, d_ws, ws_bytes, s, s, 0, nbytes & ~15ull, flags, o, sms, stream);
+}
+
+}  // extern "C"

@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
     // ---- header tiles ----
     uint64_t nh = 0;
     if (UNPACK) {
-        if (p.header != nullptr) nh = ((uint64_t)T + B + kTileUnits - 1) / kTileUnits;
+        if (p.header != nullptr) nh = (n_rebuild_records(p, head) + kTileUnits - 1) / kTileUnits;
     } else if (lo < hb && lo < hi) {
         nh = ((hi < hb ? hi : hb) - lo + kTileBytes - 1) / kTileBytes;
     }
@@ -76,13 +76,13 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
             const uint64_t h = w - np;
             if (UNPACK) {
 #pragma unroll
-                for (int k = 0; k < UPT; ++k) rebuild_record(p, h * kTileUnits + (uint64_t)k * kThreads + tid, T, B);
+                for (int k = 0; k < UPT; ++k) rebuild_record_any(p, head, h * kTileUnits + (uint64_t)k * kThreads + tid);
             } else {
                 const uint64_t hend = hi < hb ? hi : hb;
 #pragma unroll
                 for (int k = 0; k < UPT; ++k) {
                     const uint64_t s = lo + (h * kTileUnits + (uint64_t)k * kThreads + tid) * 16;
-                    if (s < hend) st_stream16(p.stream + (s - lo), header_unit(p, s >> 4, T, B, hb, P));
+                    if (s < hend) st_stream16(p.stream + (s - lo), header_unit_any(p, s >> 4, T, B, hb, P));
                 }
             }
             continue;

@@ -79,6 +79,116 @@ __device__ __forceinline__ void rebuild_record(const MoveParams& p, uint64_t rec
     }
 }
 
+
+// ==== wire format v2 (structure-shared layers; include/bs.h) ==========================================================
+// owner of structure block j: the last structure s with first_block[s] <= j and a non-empty range holding j
+__device__ __forceinline__ uint32_t struct_of_block(const bs_struct_rec* st, uint32_t C, uint32_t j)
+{
+    uint32_t lo = 0, hi = C;
+    while (hi - lo > 1) {
+        uint32_t mid = (lo + hi) >> 1;
+        if (__ldg(&st[mid].first_block) <= j) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// S3, v2: one 16-byte unit of the header region.  The scan kernels of bs_layered.cu left gs[] (prefix of stored sizes
+// over the structure block table, odd flag in bit 0) and lpos[] (payload offset of every layer).
+__device__ __forceinline__ uint4 header_unit_v2(const MoveParams& p, uint64_t u, uint32_t T, uint64_t hb, uint64_t P)
+{
+    const uint32_t C = p.lay.C, Bs = p.lay.Bs;
+    uint4 v = make_uint4(0, 0, 0, 0);
+    if (u < 4) {
+        if (u == 0) v = make_uint4(0x41505342u, 0x31455352u, 2u, 0x01020304u);  // "BSPARSE1", version 2, endian_tag
+        else if (u == 1) v = make_uint4(0u, 2u, 3u, 16u);                        // dtype, n_qn, max_rank, align
+        else if (u == 2) v = make_uint4(C, Bs, T, 0u);                           // u32 C, u32 Bs, u64 n_layers
+        else v = make_uint4((uint32_t)hb, (uint32_t)(hb >> 32), (uint32_t)P, (uint32_t)(P >> 32));
+        return v;
+    }
+    u -= 4;
+    if (u < 2ull * C) {
+        const uint32_t s = (uint32_t)(u >> 1);
+        const uint4 w = __ldg(reinterpret_cast<const uint4*>(p.lay.structs) + u);
+        if ((u & 1) == 0) return w;  // rank, first_block, n_blocks, dq[0]
+        const uint32_t f = __ldg(&p.lay.structs[s].first_block), n = __ldg(&p.lay.structs[s].n_blocks);
+        const uint64_t lb = (p.lay.gs[f + n] & ~15ull) - (p.lay.gs[f] & ~15ull);
+        return make_uint4(w.x, w.y, (uint32_t)lb, (uint32_t)(lb >> 32));  // dq[1], sign, layer_bytes
+    }
+    u -= 2ull * C;
+    if (u < T) {
+        const uint2 w = __ldg(reinterpret_cast<const uint2*>(p.lay.layers + u));  // structure, tag
+        const uint64_t off = p.lay.lpos[u].off;
+        return make_uint4(w.x, w.y, (uint32_t)off, (uint32_t)(off >> 32));
+    }
+    u -= T;
+    if (u < 3ull * Bs) {
+        const uint32_t r = (uint32_t)(u / 3), part = (uint32_t)(u % 3);
+        const int32_t* q = p.qn + 6ull * r;
+        const uint32_t* d = p.dim + 3ull * r;
+        if (part == 0) {
+            int2 a = __ldg(reinterpret_cast<const int2*>(q)), b = __ldg(reinterpret_cast<const int2*>(q + 2));
+            v = make_uint4((uint32_t)a.x, (uint32_t)a.y, (uint32_t)b.x, (uint32_t)b.y);
+        } else if (part == 1) {
+            int2 a = __ldg(reinterpret_cast<const int2*>(q + 4));
+            v = make_uint4((uint32_t)a.x, (uint32_t)a.y, __ldg(d), __ldg(d + 1));
+        } else {
+            const uint32_t s = struct_of_block(p.lay.structs, C, r);
+            const uint64_t rel = (p.lay.gs[r] & ~15ull) - (p.lay.gs[__ldg(&p.lay.structs[s].first_block)] & ~15ull);
+            v = make_uint4(__ldg(d + 2), s, (uint32_t)rel, (uint32_t)(rel >> 32));
+        }
+    }
+    return v;
+}
+
+// S7, v2 (descriptor part): record `rec` of the header -> structs / layers / qn / dim.  addr[] was written by the
+// expansion kernel of bs_layered.cu.
+__device__ __forceinline__ void rebuild_record_v2(const MoveParams& p, uint64_t rec, uint32_t C, uint32_t T, uint32_t Bs)
+{
+    const unsigned char* h = p.header + kFixedHeader;
+    if (rec < C) {
+        const uint4* s = reinterpret_cast<const uint4*>(h + 32 * rec);
+        uint4* d = reinterpret_cast<uint4*>(p.lay.structs + rec);
+        d[0] = __ldg(s);
+        d[1] = __ldg(s + 1);
+        return;
+    }
+    rec -= C;
+    if (rec < T) {
+        *reinterpret_cast<uint4*>(p.lay.layers + rec) = __ldg(reinterpret_cast<const uint4*>(h + 32ull * C + 16 * rec));
+        return;
+    }
+    rec -= T;
+    if (rec >= Bs) return;
+    const uint4* s = reinterpret_cast<const uint4*>(h + 32ull * C + 16ull * T + kBlockRec * rec);
+    const uint4 r0 = __ldg(s), r1 = __ldg(s + 1), r2 = __ldg(s + 2);
+    int2* q = reinterpret_cast<int2*>(p.qn + 6 * rec);
+    q[0] = make_int2((int)r0.x, (int)r0.y);
+    q[1] = make_int2((int)r0.z, (int)r0.w);
+    q[2] = make_int2((int)r1.x, (int)r1.y);
+    if ((p.flags & 1u) == BS_LAYOUT_POOL) {  // scatter mode: dim is a caller input, already checked equal
+        p.dim[3 * rec + 0] = r1.z;
+        p.dim[3 * rec + 1] = r1.w;
+        p.dim[3 * rec + 2] = r2.x;
+    }
+}
+
+// ---- format dispatch used by both move kernels ---------------------------------------------------------------------------
+__device__ __forceinline__ uint4 header_unit_any(const MoveParams& p, uint64_t u, uint32_t T, uint32_t B, uint64_t hb,
+                                                 uint64_t P)
+{
+    return p.lay.on ? header_unit_v2(p, u, T, hb, P) : header_unit(p, u, T, B, hb, P);
+}
+__device__ __forceinline__ uint64_t n_rebuild_records(const MoveParams& p, const WsHead* head)
+{
+    return p.lay.on ? (uint64_t)head->n_structs + head->n_tensors + head->n_struct_blocks
+                    : (uint64_t)head->n_tensors + head->n_blocks;
+}
+__device__ __forceinline__ void rebuild_record_any(const MoveParams& p, const WsHead* head, uint64_t rec)
+{
+    if (p.lay.on) rebuild_record_v2(p, rec, head->n_structs, head->n_tensors, head->n_struct_blocks);
+    else rebuild_record(p, rec, head->n_tensors, head->n_blocks);
+}
+
 // ---- warp-level header workers (TMA variant: a dedicated warp per CTA runs these beside the data warps) -------
 // Header worker `hw` of `n_hw` (one warp each).  Nothing here depends on another worker.
 
@@ -138,14 +248,26 @@ __device__ __forceinline__ void write_header_warp(const MoveParams& p, uint32_t 
     }
 }
 
+// S3, v2: the header is small when layers share structures (48 bytes per STRUCTURE block); unit by unit
+__device__ __forceinline__ void write_header_warp_v2(const MoveParams& p, uint32_t T, uint64_t hb, uint64_t P, uint64_t lo,
+                                                     uint64_t hend, uint64_t hw, uint64_t n_hw, uint32_t lane)
+{
+    if (lo >= hend) return;
+    const uint64_t u0 = lo / 16, n = (hend - lo) / 16;
+    for (uint64_t i = hw * 32 + lane; i < n; i += n_hw * 32)
+        __stcs(reinterpret_cast<uint4*>(p.stream + i * 16), header_unit_v2(p, u0 + i, T, hb, P));
+}
+
 // S7 (descriptor part): records [0, T+B) of p.header -> the out descriptor arrays, 128 records per step
 __device__ __forceinline__ void rebuild_header_warp(const MoveParams& p, uint32_t T, uint32_t B, uint64_t hw, uint64_t n_hw,
                                                     uint32_t lane)
 {
-    const uint64_t n_rec = (uint64_t)T + B;
+    (void)T; (void)B;
+    const WsHead* head = p.ws.head;
+    const uint64_t n_rec = n_rebuild_records(p, head);
     for (uint64_t base = hw * 128; base < n_rec; base += n_hw * 128) {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) rebuild_record(p, base + (uint64_t)k * 32 + lane, T, B);
+        for (int k = 0; k < 4; ++k) rebuild_record_any(p, head, base + (uint64_t)k * 32 + lane);
     }
 }
 

@@ -250,7 +250,8 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
         if (UNPACK) {
             if (p.header != nullptr) rebuild_header_warp(p, T, B, hw, n_hw, lane);
         } else {
-            write_header_warp(p, T, B, hb, P, lo, hi < hb ? hi : hb, hw, n_hw, lane);
+            if (p.lay.on) write_header_warp_v2(p, T, hb, P, lo, hi < hb ? hi : hb, hw, n_hw, lane);
+            else write_header_warp(p, T, B, hb, P, lo, hi < hb ? hi : hb, hw, n_hw, lane);
         }
         return;
     }

@@ -63,11 +63,61 @@ class DeviceSet:
         )
 
 
+_STRUCT_DTYPE = np.dtype([("rank", "<u4"), ("first_block", "<u4"), ("n_blocks", "<u4"), ("dq", "<i4", (2,)),
+                          ("sign", "i1", (4,)), ("layer_bytes", "<u8")])
+_LAYER_DTYPE = np.dtype([("structure", "<u4"), ("tag", "<u4"), ("offset", "<u8")])
+
+
+class DeviceLayeredSet:
+    """The five device arrays of one bs_layered_desc (wire format v2), as torch uint8 tensors."""
+
+    def __init__(self, structs, layers, qn, dim, addr, n_structs: int, n_struct_blocks: int, n_layers: int, n_addr: int):
+        self.structs, self.layers, self.qn, self.dim, self.addr = structs, layers, qn, dim, addr
+        self.n_structs, self.n_struct_blocks, self.n_layers, self.n_addr = n_structs, n_struct_blocks, n_layers, n_addr
+
+    @classmethod
+    def from_host(cls, structs: np.ndarray, layers: np.ndarray, qn: np.ndarray, dim: np.ndarray, addr: np.ndarray,
+                  device="cuda"):
+        assert structs.dtype.itemsize == 32 and layers.dtype.itemsize == 16
+        return cls(_to_dev(structs, device), _to_dev(layers, device), _to_dev(qn.astype(np.int32, copy=False), device),
+                   _to_dev(dim.astype(np.uint32, copy=False), device), _to_dev(addr.astype(np.uint64, copy=False), device),
+                   len(structs), int(np.asarray(dim).reshape(-1, 3).shape[0]), len(layers), int(np.asarray(addr).size))
+
+    @classmethod
+    def empty(cls, cap_structs: int, cap_struct_blocks: int, cap_layers: int, cap_addr: int, device="cuda",
+              fill: int | None = None):
+        def mk(n):
+            t = torch.empty(max(n, 16), dtype=torch.uint8, device=device)
+            if fill is not None:
+                t.fill_(fill)
+            return t
+        return cls(mk(32 * cap_structs), mk(16 * cap_layers), mk(24 * cap_struct_blocks), mk(12 * cap_struct_blocks),
+                   mk(8 * cap_addr), cap_structs, cap_struct_blocks, cap_layers, cap_addr)
+
+    @property
+    def desc(self) -> B.LayeredDesc:
+        return B.make_layered_desc(self.n_structs, self.n_struct_blocks, self.n_layers, self.n_addr, self.structs.data_ptr(),
+                                   self.layers.data_ptr(), self.qn.data_ptr(), self.dim.data_ptr(), self.addr.data_ptr())
+
+    def to_host(self, n_structs: int, n_struct_blocks: int, n_layers: int, n_addr: int) -> dict:
+        return dict(
+            structs=self.structs[: 32 * n_structs].cpu().numpy().view(_STRUCT_DTYPE).copy(),
+            layers=self.layers[: 16 * n_layers].cpu().numpy().view(_LAYER_DTYPE).copy(),
+            qn=self.qn[: 24 * n_struct_blocks].cpu().numpy().view(np.int32).reshape(n_struct_blocks, 3, 2).copy(),
+            dim=self.dim[: 12 * n_struct_blocks].cpu().numpy().view(np.uint32).reshape(n_struct_blocks, 3).copy(),
+            addr=self.addr[: 8 * n_addr].cpu().numpy().view(np.uint64).copy(),
+        )
+
+
 class Workspace:
     """Device workspace + the 64-byte bs_result word of one call site."""
 
-    def __init__(self, n_tensors: int, n_blocks: int, stream_capacity: int, device="cuda"):
-        self.nbytes = B.workspace_bytes(n_tensors, n_blocks, stream_capacity)
+    def __init__(self, n_tensors: int, n_blocks: int, stream_capacity: int, device="cuda", layered=None):
+        """layered = (n_structs, n_struct_blocks, n_layers, n_addr) sizes the workspace for wire format v2 instead."""
+        if layered is not None:
+            self.nbytes = B.layered_workspace_bytes(*layered, stream_capacity)
+        else:
+            self.nbytes = B.workspace_bytes(n_tensors, n_blocks, stream_capacity)
         self.buf = torch.empty(self.nbytes, dtype=torch.uint8, device=device)
         self.result = torch.zeros(64, dtype=torch.uint8, device=device)
         assert self.buf.data_ptr() % 256 == 0
@@ -85,4 +135,5 @@ class Workspace:
         raw = self.result.cpu().numpy().tobytes()
         r = B.Result.from_buffer_copy(raw)
         return dict(total_bytes=int(r.total_bytes), header_bytes=int(r.header_bytes), payload_bytes=int(r.payload_bytes),
-                    pool_bytes=int(r.pool_bytes), status=int(r.status), n_tensors=int(r.n_tensors), n_blocks=int(r.n_blocks))
+                    pool_bytes=int(r.pool_bytes), status=int(r.status), n_tensors=int(r.n_tensors), n_blocks=int(r.n_blocks),
+                    n_structs=int(r.reserved[0]), n_struct_blocks=int(r.reserved[1]))
