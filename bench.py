@@ -132,7 +132,7 @@ class ClockSampler:
 
 
 # ---- CPU oracle leg (cpu_baseline and --impl reference) ------------------------------------------------------------
-def oracle_sample(workload: str, sample_mb: float):
+def oracle_sample(workload: str, sample_mb: float, fmt: str = "v1"):
     """First tensors of the workload up to ~sample_mb of payload, values regenerated on the host."""
     import workloads as W
     bset = W.make_config(workload)
@@ -144,11 +144,46 @@ def oracle_sample(workload: str, sample_mb: float):
     pool, offs = W.fill_pool_host(bset, 0, b1, compact=True)
     sub = dict(tensors=bset.tensors[:n_t].copy(), qn=bset.qn[:b1], dim=bset.dim[:b1],
                addr=(np.uint64(pool.ctypes.data) + offs).astype(np.uint64), pool=pool)
+    if fmt == "v2":   # the same tensors as layers of their structures (structures no sampled layer uses are dropped)
+        lv = W.layered_view(bset)
+        ly = lv["layers"][:n_t].copy()
+        used = np.unique(ly["structure"])
+        remap = np.full(len(lv["structs"]), -1, np.int64)
+        remap[used] = np.arange(len(used))
+        st = lv["structs"][used].copy()
+        keep = np.concatenate([np.arange(f, f + n) for f, n in zip(st["first_block"], st["n_blocks"])]).astype(np.int64)
+        st["first_block"] = np.concatenate([[0], np.cumsum(st["n_blocks"])])[:-1]
+        ly["structure"] = remap[ly["structure"]]
+        sub["layered"] = dict(structs=st, layers=ly, qn=np.ascontiguousarray(lv["qn"][keep]),
+                              dim=np.ascontiguousarray(lv["dim"][keep]))
     return bset, sub, n_t, b1
+
+
+def time_oracle_v2(sub, min_seconds: float, max_passes: int = 1000):
+    """As time_oracle, for wire format v2 (oracle.v2) on the layered form of the same sample."""
+    from oracle import v2
+    lv = sub["layered"]
+    hb, total = v2.serialized_size(lv["structs"], lv["layers"], lv["dim"])
+    out = np.empty(total, np.uint8)
+    pool = None
+    passes, t_acc = 0, 0.0
+    while passes == 0 or (t_acc < min_seconds and passes < max_passes):
+        t0 = time.perf_counter()
+        s = v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], sub["addr"], capacity=total, out=out)
+        if pool is None:
+            t_acc += time.perf_counter() - t0
+            pool = np.empty(max(v2.counts(s)[1], 1), np.uint8)
+            t0 = time.perf_counter()
+        v2.deserialize(s, pool=pool)
+        t_acc += time.perf_counter() - t0
+        passes += 1
+    return t_acc, passes, total
 
 
 def time_oracle(sub, min_seconds: float, max_passes: int = 1000):
     """serialize + deserialize passes of the oracle, single thread.  Returns (seconds, passes, stream_bytes)."""
+    if "layered" in sub:
+        return time_oracle_v2(sub, min_seconds, max_passes)
     import oracle
     hb, total = oracle.serialized_size(len(sub["tensors"]), sub["dim"])
     out = np.empty(total, np.uint8)
@@ -174,7 +209,7 @@ def run_reference(args):
     if rank != 0:
         return
     log(f"[reference] oracle on a {args.sample_mb:.0f} MB sample of workload {args.workload}")
-    bset, sub, n_t, b1 = oracle_sample(args.workload, args.sample_mb)
+    bset, sub, n_t, b1 = oracle_sample(args.workload, args.sample_mb, args.format)
     time_oracle(sub, 0.0, max_passes=max(1, args.warmup))           # warm-up passes
     per = []
     total = 0
@@ -187,15 +222,16 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms, 3), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
-            "config": workload_config(args.workload, bset, None),
+            "config": workload_config(args.workload, bset, None, args.format),
             "cpu_baseline": {"value": round(value, 3), "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": round(value, 3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def workload_config(name, bset, total):
-    c = {"workload": f"BASELINE.json configs[{int(name[0]) - 1}] = config {name}: "
+def workload_config(name, bset, total, fmt="v1"):
+    c = {"wire_format": fmt,
+         "workload": f"BASELINE.json configs[{int(name[0]) - 1}] = config {name}: "
                      f"D={bset.meta['D']}, {bset.meta['S']} (N,2Sz) sectors, {bset.meta['n_ops']} operators + "
                      f"{bset.meta['n_site']} site tensors, dims {bset.meta['dims']} sigma={bset.meta['sigma']}",
          "n_tensors": bset.n_tensors, "n_blocks": bset.n_blocks, "l2": "inputs larger than L2 (no flush needed)",
@@ -239,24 +275,36 @@ def run_mine(args):
     t_setup = time.time()
     bset = W.make_config(args.workload)
     pool, addr = fill_pool_device(bset, dev)
-    dset = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, addr, dev)
+    v2 = args.format == "v2"
     cap_guess = bset.data_bytes + 16 * bset.n_blocks + bs.header_bytes(bset.n_tensors, bset.n_blocks)
-    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, cap_guess, dev)
     cs = bs.current_stream()
-    hb, total = bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs)       # size known before serialization
+    if v2:   # the same tensors as layers of their structures (wire format v2); pool and addresses are shared
+        lv = W.layered_view(bset)
+        counts = (len(lv["structs"]), lv["dim"].shape[0], bset.n_tensors, bset.n_blocks)
+        dset = bs.DeviceLayeredSet.from_host(lv["structs"], lv["layers"], lv["qn"], lv["dim"], addr, dev)
+        ws = bs.Workspace(0, 0, cap_guess, dev, layered=counts)
+        hb, total = bs.layered_serialized_size(dset.desc, ws.ptr, ws.nbytes, cs)
+        out = bs.DeviceLayeredSet.empty(*counts, dev)
+        f_ser, f_range, f_deser, f_size = bs.layered_serialize, bs.layered_serialize_range, bs.layered_deserialize, \
+            bs.layered_serialized_size
+    else:
+        dset = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, addr, dev)
+        ws = bs.Workspace(bset.n_tensors, bset.n_blocks, cap_guess, dev)
+        hb, total = bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs)   # size known before serialization
+        out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, dev)
+        f_ser, f_range, f_deser, f_size = bs.serialize, bs.serialize_range, bs.deserialize, bs.serialized_size
     stream = torch.empty(total, dtype=torch.uint8, device=dev)
-    out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, dev)
     need = int(((bset.nelems * 8 + 255) // 256 * 256).sum())
     opool = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
     log(f"[rank {rank}] workload {args.workload}: T={bset.n_tensors} B={bset.n_blocks} stream={total / 1e9:.3f} GB "
         f"(header {hb / 1e6:.1f} MB) set up in {time.time() - t_setup:.1f}s")
 
     def ser():
-        bs.serialize(dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
+        f_ser(dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
 
     def deser():
-        bs.deserialize(stream.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
-                       ws.result_ptr, opts, cs)
+        f_deser(stream.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                ws.result_ptr, opts, cs)
 
     def check_ok(what):
         r = ws.read_result()
@@ -295,13 +343,13 @@ def run_mine(args):
     a, b = ev(), ev()
     a.record()
     for _ in range(n_pack):
-        bs.serialize_range(dset.desc, stream.data_ptr(), 0, total, False, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
+        f_range(dset.desc, stream.data_ptr(), 0, total, False, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
     b.record()
     torch.cuda.synchronize()
     pack_ms = a.elapsed_time(b) / n_pack
     a.record()
     for _ in range(n_pack):
-        bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs)
+        f_size(dset.desc, ws.ptr, ws.nbytes, cs)
     b.record()
     torch.cuda.synchronize()
     scan_ms = a.elapsed_time(b) / n_pack
@@ -309,7 +357,8 @@ def run_mine(args):
     # algorithmic bytes per pack launch: 2 B per stream byte + per block 24 (labels) + 12 (dims)
     # + 16 (offset table entry) read for its header record  [SURVEY §8(d): "2 B per stream byte ... ~130 B per block"
     # counts the scan pass too; the pack launch alone reads 52 B per block on top of the stream bytes]
-    algo_bytes = 2 * total + 52 * bset.n_blocks
+    # wire format v2: the header records exist once per STRUCTURE block; per block of a layer only its 16-byte table entry
+    algo_bytes = 2 * total + (16 * bset.n_blocks if v2 else 52 * bset.n_blocks)
     achieved = algo_bytes / (pack_ms * 1e-3) / 1e9
     kname = "bs::move_kernel<pack>" if args.variant == 1 else "bs::move_tma_kernel<pack>"
     roofline = {"bound": "hbm", "kernel": kname + " (S3 header write + S5 pack)", "achieved": round(achieved, 1),
@@ -317,7 +366,7 @@ def run_mine(args):
                 "unit": "GB/s", "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": None,
                 "algorithmic_bytes_per_launch": int(algo_bytes), "kernel_ms": round(pack_ms, 4),
                 "frac_of_nominal_8TBs": round(achieved / 8000.0, 4)}
-    roofline["traffic"] = committed_traffic(f"pack:{args.workload}:v{args.variant or 2}")
+    roofline["traffic"] = committed_traffic(f"pack:{args.workload}:v{args.variant or 2}" + (":fmt2" if v2 else ""))
 
     # ---- e2e leg: host (pinned) buffers through the engine, copies inside the timed region ----
     detail = {"serialize_ms": round(float(np.median(ser_ms)), 4), "deserialize_ms": round(float(np.median(des_ms)), 4),
@@ -334,6 +383,8 @@ def run_mine(args):
     if not args.no_e2e:
         host = torch.empty(total, dtype=torch.uint8, pin_memory=True)
         eng = bs.Engine(bset.n_tensors, bset.n_blocks, total, chunk_bytes=args.chunk_mb << 20, n_staging=2, opts=opts)
+        e_off = eng.offload_layered_async if v2 else eng.offload_async
+        e_pre = eng.prefetch_layered_async if v2 else eng.prefetch_async
         # link denominators, same run: pinned cudaMemcpyAsync of 1 GiB (or the whole stream if smaller), best of 5
         nlink = min(total, 1 << 30)
         dbuf = torch.empty(nlink, dtype=torch.uint8, device=dev)
@@ -348,9 +399,9 @@ def run_mine(args):
         del dbuf
 
         def e2e_step():
-            t1 = eng.offload_async(dset.desc, total, host.data_ptr(), total, cs)
+            t1 = e_off(dset.desc, total, host.data_ptr(), total, cs)
             s1 = t1.wait()
-            t2 = eng.prefetch_async(host.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, cs)
+            t2 = e_pre(host.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, cs)
             s2 = t2.wait()
             if s1["status"] or s2["status"]:
                 raise RuntimeError(f"engine status {s1} {s2}")
@@ -380,7 +431,7 @@ def run_mine(args):
         del host
 
     # ---- config 5: exposed IO of an offload overlapped with a stand-in contraction (rank 0 only) ----
-    if rank == 0 and not args.no_config5:
+    if rank == 0 and not args.no_config5 and not v2:
         try:
             detail["config5"] = config5(args, dev, opts)
         except Exception as ex:  # the headline numbers stand on their own
@@ -389,7 +440,7 @@ def run_mine(args):
     # ---- cpu baseline: the oracle on a bounded sample (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        _, sub, n_t, b1 = oracle_sample(args.workload, args.sample_mb)
+        _, sub, n_t, b1 = oracle_sample(args.workload, args.sample_mb, args.format)
         time_oracle(sub, 0.0, max_passes=1)
         sec, passes, sbytes = time_oracle(sub, args.cpu_seconds)
         cpu = {"value": round(2 * sbytes * passes / sec / 1e9, 3), "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -403,8 +454,8 @@ def run_mine(args):
         line = {"metric": METRIC, "value": round(units_g / (ms_g * 1e-3) / 1e9, 3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_g, 4), "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
-                "config": workload_config(args.workload, bset, total), "clocks": clocks, "e2e": e2e,
-                "gpu_launches": 4 * args.steps, "roofline": roofline, "cpu_baseline": cpu, "detail": detail}
+                "config": workload_config(args.workload, bset, total, args.format), "clocks": clocks, "e2e": e2e,
+                "gpu_launches": (8 if v2 else 4) * args.steps, "roofline": roofline, "cpu_baseline": cpu, "detail": detail}
         print(json.dumps(line), flush=True)
     if ready:
         dist.destroy_process_group()
@@ -483,6 +534,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
     ap.add_argument("--workload", default="4", choices=["1", "2", "3", "4", "3L", "4L"])
+    ap.add_argument("--format", default="v1", choices=["v1", "v2"],
+                    help="wire format: v1 (one block record per block) or v2 (structure-shared layers, NEXT-1)")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--tile-bytes", type=int, default=0)
     ap.add_argument("--ctas-per-sm", type=int, default=0)

@@ -106,9 +106,11 @@ struct ScanParams {
 cudaError_t launch_scan(bool deser, const ScanParams& p, int sm_count, cudaStream_t stream);
 
 // ---- layered sets (wire format v2): what the header generator / parser of the move kernels needs ---------
-struct __align__(16) LayerPos {
+struct __align__(32) LayerPos {
     uint64_t off;         // serialize: payload offset of the layer; deserialize: pool offset of the layer
     uint64_t first_addr;  // index of the layer's first block in addr[] / blk[]
+    uint64_t stream_off;  // payload offset of the layer (deserialize: from the wire)
+    uint32_t sfirst, sn;  // block range of the layer's structure in the structure block table
 };
 struct LayeredView {
     uint32_t on;                   // 0: wire format v1

@@ -3,18 +3,18 @@
 // PAPER Fig 4(a) (L75): "Layers indicate position dependent operators which have the same block-sparse structure,
 // but the dense sector matrices take different values for the different layers."  The meta data of a structure
 // (L63: sector indices, quantum numbers, sector dimensions) is stored once; every layer adds 16 bytes.  The
-// "pointer structure ... grid structure of the serialized data" (L90-92) is built in three small launches before
-// any data moves:
-//   lplan_blocks_kernel : chained scan over the STRUCTURE block table (Bs entries): stored sizes -> gs[] (serialize);
-//                         header validation, stored sizes + pool slot sizes -> gs[], gp[] (deserialize)
-//   lplan_layers_kernel : chained scan over the LAYERS (T entries): bytes and block count of every layer's structure
-//                         -> lpos[] = {payload (or pool) offset, index of the layer's first block}; totals, checks, result
-//   lexpand_kernel      : one warp per layer writes the flat work table the data-movement kernels already use
-//                         (blk[] = {payload offset, block address}, tile_first[]) — B entries, 16 bytes each
+// "pointer structure ... grid structure of the serialized data" (L90-92) is built by ONE launch before any data moves
+// (lplan_kernel; work items of three phases are claimed in order from one ticket, see there):
+//   phase 1 : chained scan over the STRUCTURE block table (Bs entries): stored sizes -> gs[] (serialize); header
+//             validation, stored sizes + pool slot sizes -> gs[], gp[] (deserialize)
+//   phase 2 : chained scan over the LAYERS (T entries): bytes and block count of every layer's structure
+//             -> lpos[] = {payload (or pool) offset, index of the layer's first block}; totals, checks, result
+//   phase 3 : the flat work table the data-movement kernels already use (blk[] = {payload offset, block address},
+//             tile_first[]) — B entries, 16 bytes each, one thread per block (its layer found by binary search in lpos[])
 // after which the payload moves through the SAME pack / unpack kernels as wire format v1 (bs_move_tma.cu, bs_move.cu);
 // only their header generator / parser differs (bs_move_common.cuh, *_v2).
-// Roofline: HBM-bound; the three plan launches touch 8 B (address) + 16 B (table entry) per block plus the structure
-// tables, < 0.5 % of the payload traffic; the header itself shrinks from 48 B per block to 48 B per structure block.
+// Roofline: HBM-bound; the plan touches 8 B (address) + 16 B (table entry) per block plus the structure tables,
+// < 0.5 % of the payload traffic; the header itself shrinks from 48 B per block to 48 B per structure block.
 #include <string.h>
 
 #include "bs_internal.cuh"
@@ -196,22 +196,42 @@ __device__ __forceinline__ StructHead load_struct(const void* recs, uint64_t s)
     return h;
 }
 
-// ---- pass 1: the structure block table -------------------------------------------------------------------------
-template <bool DESER>
-__global__ void __launch_bounds__(kLThreads) lplan_blocks_kernel(const LPlanParams p)
+// ---- the plan kernel: ONE launch, three phases of work items claimed in order from one ticket ------------------------------
+//   phase 1 (n1 items): a tile of the structure block table (+ the same slice of the structure records)
+//   phase 2 (n2 items): a tile of the layers; the CTA that finishes the last one writes totals, checks, sentinel, result
+//   phase 3          : a chunk of kLTile blocks of the flat work table blk[] / tile_first[]
+// An item of phase 2 waits until every item of phase 1 is done, an item of phase 3 until the plan is ready.  Items are
+// claimed in order and a claimed item is being executed by a resident CTA, so whatever an item waits for is already
+// running and never waits for a later item: forward progress needs no co-residency of the whole grid (the argument of the
+// chained scan's look-back).
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p)
 {
-    __shared__ uint32_t s_tile;
-    __shared__ ChainSmem<2> sm;
-    WsHead* head = p.lw.ws.head;
-    const uint32_t tid = threadIdx.x;
-    constexpr int kErrBad = DESER ? BS_ERR_CORRUPT : BS_ERR_ARG;
-    constexpr int kErrRank = DESER ? BS_ERR_CORRUPT : BS_ERR_UNSUPPORTED;
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void cta_wait_until(const uint32_t* counter, uint32_t target)
+{
+    if (threadIdx.x == 0) {
+        while (ld_acquire_u32(counter) < target) __nanosleep(64);
+    }
+    __syncthreads();
+}
 
-    uint64_t C = p.C, Bs = p.Bs, T = p.T, hb = 0;
-    bool ok = true;
+struct PlanShape {  // uniform over the grid: derived from the call's arguments / the fixed header alone
+    uint64_t C, Bs, T, hb, P_hdr;
+    bool ok;
+    uint32_t n1, n2;
+};
+
+template <bool DESER>
+__device__ __forceinline__ PlanShape plan_shape(const LPlanParams& p, WsHead* head)
+{
+    PlanShape s;
+    s.C = p.C; s.Bs = p.Bs; s.T = p.T; s.hb = 0; s.P_hdr = 0; s.ok = true;
     if (DESER) {  // the fixed header, field by field in stream order
         int code = 0;
-        C = Bs = T = 0;
+        s.C = s.Bs = s.T = 0;
         if (p.nbytes < kFixedHeader) {
             code = BS_ERR_CORRUPT;
         } else {
@@ -230,363 +250,426 @@ __global__ void __launch_bounds__(kLThreads) lplan_blocks_kernel(const LPlanPara
             else if (hH != align_up(kFixedHeader + kV2Struct * hC + kV2Layer * hT + kBlockRec * hBs, kHeaderAlign)) code = BS_ERR_CORRUPT;
             else if (hH > p.nbytes || hP != p.nbytes - hH)        code = BS_ERR_CORRUPT;
             else if (hC > p.C || hBs > p.Bs || hT > p.T)          code = BS_ERR_CAPACITY;  // out arrays too small
-            else { C = hC; Bs = hBs; T = hT; hb = hH; }
-            if (blockIdx.x == 0 && tid == 0 && (code == 0 || code == BS_ERR_CAPACITY)) {
+            else { s.C = hC; s.Bs = hBs; s.T = hT; s.hb = hH; s.P_hdr = hP; }
+            if (code == BS_ERR_CAPACITY && blockIdx.x == 0 && threadIdx.x == 0) {  // report the counts
                 head->n_structs = (uint32_t)hC; head->n_struct_blocks = (uint32_t)hBs; head->n_tensors = (uint32_t)hT;
-                head->header_bytes = hH; head->payload_bytes = hP;
             }
         }
         if (code != 0) {
-            ok = false;
-            if (blockIdx.x == 0 && tid == 0) set_err(head, nullptr, code);
+            s.ok = false;
+            if (blockIdx.x == 0 && threadIdx.x == 0) set_err(head, nullptr, code);
+        }
+    } else {
+        s.hb = align_up(kFixedHeader + kV2Struct * s.C + kV2Layer * s.T + kBlockRec * s.Bs, kHeaderAlign);
+    }
+    const uint64_t m = s.Bs > s.C ? s.Bs : s.C;
+    const uint64_t t1 = (m + kLTile - 1) / kLTile, t2 = (s.T + kLTile - 1) / kLTile;
+    s.n1 = s.ok ? (uint32_t)(t1 ? t1 : 1) : 0u;
+    s.n2 = s.ok ? (uint32_t)(t2 ? t2 : 1) : 1u;  // the last item of phase 2 always writes the result
+    return s;
+}
+
+// ---- phase 1: tile `tile` of the structure block table and of the structure records -----------------------------------------
+template <bool DESER>
+__device__ __forceinline__ void plan_blocks_tile(const LPlanParams& p, const PlanShape& s, uint64_t tile, ChainSmem<2>& sm)
+{
+    WsHead* head = p.lw.ws.head;
+    const uint32_t tid = threadIdx.x;
+    constexpr int kErrBad = DESER ? BS_ERR_CORRUPT : BS_ERR_ARG;
+    constexpr int kErrRank = DESER ? BS_ERR_CORRUPT : BS_ERR_UNSUPPORTED;
+    const uint64_t C = s.C, Bs = s.Bs, T = s.T;
+    const void* srecs = DESER ? (const void*)(p.header + kFixedHeader) : (const void*)p.structs;
+    const unsigned char* brec = DESER ? p.header + kFixedHeader + kV2Struct * C + kV2Layer * T : nullptr;
+    int err = 0;
+
+    // structure records partition the structure block table in order
+#pragma unroll
+    for (uint32_t k = 0; k < kLItems; ++k) {
+        const uint64_t q = tile * kLTile + (uint64_t)k * kLThreads + tid;
+        if (q < C) {
+            const StructHead h = load_struct(srecs, q);
+            uint64_t prev_end = 0;
+            if (q > 0) {
+                const StructHead g = load_struct(srecs, q - 1);
+                prev_end = (uint64_t)g.first + g.n;
+            }
+            if (h.rank != 2 && h.rank != 3) err = kErrRank;
+            else if (h.first != prev_end) err = kErrBad;
+            else if ((uint64_t)h.first + h.n > Bs) err = kErrBad;
+            else if (q == C - 1 && (uint64_t)h.first + h.n != Bs) err = kErrBad;
         }
     }
-    const void* srecs = DESER ? (const void*)(p.header + kFixedHeader) : (const void*)p.structs;
-
-    // ---- structure records partition the structure block table in order ----
-    if (ok) {
-        for (uint64_t s = (uint64_t)blockIdx.x * kLThreads + tid; s < C; s += (uint64_t)gridDim.x * kLThreads) {
-            const StructHead h = load_struct(srecs, s);
-            uint64_t prev_end = 0;
-            if (s > 0) {
-                const StructHead q = load_struct(srecs, s - 1);
-                prev_end = (uint64_t)q.first + q.n;
-            }
-            int code = 0;
-            if (h.rank != 2 && h.rank != 3) code = kErrRank;
-            else if (h.first != prev_end) code = kErrBad;
-            else if ((uint64_t)h.first + h.n > Bs) code = kErrBad;
-            else if (s == C - 1 && (uint64_t)h.first + h.n != Bs) code = kErrBad;
-            set_err(head, nullptr, code);
-        }
-        if (C == 0 && Bs != 0 && blockIdx.x == 0 && tid == 0) set_err(head, nullptr, kErrBad);
-        if (DESER && blockIdx.x == 0) {  // header slack must be zero
+    if (tile == 0) {
+        if (C == 0 && Bs != 0 && tid == 0) err = kErrBad;
+        if (DESER) {  // header slack must be zero
             const uint64_t used = kFixedHeader + kV2Struct * C + kV2Layer * T + kBlockRec * Bs;
             const uint64_t z = used + 16ull * tid;
-            if (z < hb) {
+            if (z < s.hb) {
                 const uint4 w = __ldg(reinterpret_cast<const uint4*>(p.header + z));
-                if ((w.x | w.y | w.z | w.w) != 0) set_err(head, nullptr, BS_ERR_CORRUPT);
+                if ((w.x | w.y | w.z | w.w) != 0) err = BS_ERR_CORRUPT;
             }
         }
-        if (Bs == 0 && blockIdx.x == 0 && tid == 0) { p.lw.gs[0] = 0; p.lw.gp[0] = 0; }
+        if (Bs == 0 && tid == 0) { p.lw.gs[0] = 0; p.lw.gp[0] = 0; }
     }
 
-    const uint64_t n_tiles = ok ? (Bs + kLTile - 1) / kLTile : 0;
-    const unsigned char* brec = DESER ? p.header + kFixedHeader + kV2Struct * C + kV2Layer * T : nullptr;
-    for (;;) {
-        __syncthreads();
-        if (tid == 0) s_tile = atomicAdd(&head->scan_ticket, 1u);
-        __syncthreads();
-        const uint64_t tile = s_tile;
-        if (tile >= n_tiles) break;
-
-        uint64_t stored[kLItems], slot[kLItems];
-        uint32_t oddf[kLItems];
-        uint64_t tsum[2] = {0, 0};
-        int err = 0;
+    uint64_t stored[kLItems], slot[kLItems];
+    uint32_t oddf[kLItems];
+    uint64_t tsum[2] = {0, 0};
 #pragma unroll
-        for (uint32_t k = 0; k < kLItems; ++k) {
-            const uint64_t j = tile * kLTile + (uint64_t)tid * kLItems + k;
-            const bool valid = j < Bs;
-            uint32_t d0 = 1, d1 = 1, d2 = 0, owner = 0;
-            int32_t q4 = 0, q5 = 0;
-            uint64_t offset = 0;
-            if (valid) {
-                if (DESER) {
-                    const uint4* r = reinterpret_cast<const uint4*>(brec + kBlockRec * j);
-                    const uint4 r1 = __ldg(r + 1), r2 = __ldg(r + 2);
-                    q4 = (int32_t)r1.x; q5 = (int32_t)r1.y;
-                    d0 = r1.z; d1 = r1.w; d2 = r2.x; owner = r2.y;
-                    offset = (uint64_t)r2.z | ((uint64_t)r2.w << 32);
-                } else {
-                    d0 = __ldg(p.dim + 3 * j); d1 = __ldg(p.dim + 3 * j + 1); d2 = __ldg(p.dim + 3 * j + 2);
-                }
+    for (uint32_t k = 0; k < kLItems; ++k) {
+        const uint64_t j = tile * kLTile + (uint64_t)tid * kLItems + k;
+        const bool valid = j < Bs;
+        uint32_t d0 = 1, d1 = 1, d2 = 0, owner = 0;
+        int32_t q4 = 0, q5 = 0;
+        uint64_t offset = 0;
+        if (valid) {
+            if (DESER) {
+                const uint4* r = reinterpret_cast<const uint4*>(brec + kBlockRec * j);
+                const uint4 r1 = __ldg(r + 1), r2 = __ldg(r + 2);
+                q4 = (int32_t)r1.x; q5 = (int32_t)r1.y;
+                d0 = r1.z; d1 = r1.w; d2 = r2.x; owner = r2.y;
+                offset = (uint64_t)r2.z | ((uint64_t)r2.w << 32);
+            } else {
+                d0 = __ldg(p.dim + 3 * j); d1 = __ldg(p.dim + 3 * j + 1); d2 = __ldg(p.dim + 3 * j + 2);
             }
-            const uint64_t n01 = (uint64_t)d0 * d1;
-            uint64_t n = n01 * d2;
-            if (valid && (__umul64hi(n01, (uint64_t)d2) != 0 || n >= (1ull << 57))) { err = kErrBad; n = 0; }
-            const uint64_t nbytes = n * 8;
-            const uint64_t st = (nbytes + 15) & ~15ull;
-            stored[k] = valid ? st : 0;
-            slot[k] = (DESER && valid) ? align_up(nbytes, kPoolAlign) : 0;
-            oddf[k] = (uint32_t)(n & 1);
-            if (DESER && valid) {
-                if (owner >= C) err = BS_ERR_CORRUPT;
+        }
+        const uint64_t n01 = (uint64_t)d0 * d1;
+        uint64_t n = n01 * d2;
+        if (valid && (__umul64hi(n01, (uint64_t)d2) != 0 || n >= (1ull << 57))) { err = kErrBad; n = 0; }
+        const uint64_t nbytes = n * 8;
+        const uint64_t st = (nbytes + 15) & ~15ull;
+        stored[k] = valid ? st : 0;
+        slot[k] = (DESER && valid) ? align_up(nbytes, kPoolAlign) : 0;
+        oddf[k] = (uint32_t)(n & 1);
+        if (DESER && valid) {
+            if (owner >= C) err = BS_ERR_CORRUPT;
+            else {
+                const StructHead h = load_struct(srecs, owner);
+                const uint64_t end = (uint64_t)h.first + h.n;
+                if (j < h.first || j >= end) err = BS_ERR_CORRUPT;
                 else {
-                    const StructHead h = load_struct(srecs, owner);
-                    const uint64_t end = (uint64_t)h.first + h.n;
-                    if (j < h.first || j >= end) err = BS_ERR_CORRUPT;
-                    else {
-                        if (h.rank == 2 && (d2 != 1 || q4 != 0 || q5 != 0)) err = BS_ERR_CORRUPT;
-                        // relative offsets = exclusive prefix sum inside the structure, checked link by link
-                        uint64_t next = h.layer_bytes;
-                        if (j + 1 < end) next = __ldg(reinterpret_cast<const unsigned long long*>(brec + kBlockRec * (j + 1) + 40));
-                        if (j == h.first && offset != 0) err = BS_ERR_CORRUPT;
-                        if (offset >= (1ull << 62) || offset + st != next) err = BS_ERR_CORRUPT;
-                    }
-                }
-                if (p.flags == BS_SCATTER_TO_ADDR &&
-                    (__ldg(p.out_dim + 3 * j) != d0 || __ldg(p.out_dim + 3 * j + 1) != d1 || __ldg(p.out_dim + 3 * j + 2) != d2)) {
-                    if (!err) err = BS_ERR_ARG;
+                    if (h.rank == 2 && (d2 != 1 || q4 != 0 || q5 != 0)) err = BS_ERR_CORRUPT;
+                    // relative offsets = exclusive prefix sum inside the structure, checked link by link
+                    uint64_t next = h.layer_bytes;
+                    if (j + 1 < end) next = __ldg(reinterpret_cast<const unsigned long long*>(brec + kBlockRec * (j + 1) + 40));
+                    if (j == h.first && offset != 0) err = BS_ERR_CORRUPT;
+                    if (offset >= (1ull << 62) || offset + st != next) err = BS_ERR_CORRUPT;
                 }
             }
-            tsum[0] += stored[k];
-            tsum[1] += slot[k];
+            if (p.flags == BS_SCATTER_TO_ADDR &&
+                (__ldg(p.out_dim + 3 * j) != d0 || __ldg(p.out_dim + 3 * j + 1) != d1 || __ldg(p.out_dim + 3 * j + 2) != d2)) {
+                if (!err) err = BS_ERR_ARG;
+            }
         }
-        if (err) set_err(head, nullptr, err);
-        uint64_t excl[2];
-        chained_scan<2>(tsum, excl, tile, p.lw.st1[0], p.lw.st1[1], sm);
-        uint64_t r0 = excl[0], r1 = excl[1];
+        tsum[0] += stored[k];
+        tsum[1] += slot[k];
+    }
+    if (err) set_err(head, nullptr, err);
+    if (tile != 0 && tile * kLTile >= Bs) return;  // a tile of structure records only (C > Bs): not part of the chain
+    uint64_t excl[2];
+    chained_scan<2>(tsum, excl, tile, p.lw.st1[0], p.lw.st1[1], sm);
+    uint64_t r0 = excl[0], r1 = excl[1];
 #pragma unroll
-        for (uint32_t k = 0; k < kLItems; ++k) {
-            const uint64_t j = tile * kLTile + (uint64_t)tid * kLItems + k;
-            if (j < Bs) {
-                p.lw.gs[j] = r0 | oddf[k];
-                p.lw.gp[j] = r1;
-            }
-            r0 += stored[k];
-            r1 += slot[k];
+    for (uint32_t k = 0; k < kLItems; ++k) {
+        const uint64_t j = tile * kLTile + (uint64_t)tid * kLItems + k;
+        if (j < Bs) {
+            p.lw.gs[j] = r0 | oddf[k];
+            p.lw.gp[j] = r1;
         }
-        if (tile == n_tiles - 1 && tid == 0) {  // the owner of the last tile knows the totals
-            p.lw.gs[Bs] = sm.prefix[0] + sm.total[0];
-            p.lw.gp[Bs] = sm.prefix[1] + sm.total[1];
-        }
+        r0 += stored[k];
+        r1 += slot[k];
     }
-    // last CTA out: snapshot of the status for the second pass
-    __shared__ uint32_t s_last;
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        s_last = (atomicAdd(&head->ctas_done, 1u) == gridDim.x - 1) ? 1u : 0u;
-    }
-    __syncthreads();
-    if (s_last && tid == 0) {
-        __threadfence();
-        volatile WsHead* vh = head;
-        vh->status_pass1 = (uint32_t)vh->status;
-        __threadfence();
+    if (Bs != 0 && tile == (Bs - 1) / kLTile && tid == 0) {  // the owner of the last block tile knows the totals
+        p.lw.gs[Bs] = sm.prefix[0] + sm.total[0];
+        p.lw.gp[Bs] = sm.prefix[1] + sm.total[1];
     }
 }
 
-// ---- pass 2: the layers --------------------------------------------------------------------------------------------
+// ---- phase 2: tile `tile` of the layers ----------------------------------------------------------------------------------
+// `bad`: the status after phase 1 was not BS_OK.  The tile still takes part in the chain (a later tile looks back at it)
+// but scans zeros and dereferences no structure range.
 template <bool DESER>
-__global__ void __launch_bounds__(kLThreads) lplan_layers_kernel(const LPlanParams p)
+__device__ __forceinline__ void plan_layers_tile(const LPlanParams& p, const PlanShape& s, uint64_t tile, bool bad,
+                                                 ChainSmem<2>& sm)
 {
-    __shared__ uint32_t s_tile;
-    __shared__ uint32_t s_last;
-    __shared__ ChainSmem<2> sm;
     WsHead* head = p.lw.ws.head;
-    volatile WsHead* vh = head;
     const uint32_t tid = threadIdx.x;
-    const bool bad = vh->status_pass1 != 0;  // snapshot taken by the first pass: uniform over the grid (tiles are ticketed)
-    uint64_t C = p.C, Bs = p.Bs, T = p.T, hb, P_hdr = 0;
-    if (DESER) {
-        C = vh->n_structs; Bs = vh->n_struct_blocks; T = vh->n_tensors; hb = vh->header_bytes; P_hdr = vh->payload_bytes;
-    } else {
-        hb = align_up(kFixedHeader + kV2Struct * C + kV2Layer * T + kBlockRec * Bs, kHeaderAlign);
-    }
+    const uint64_t C = s.C, T = s.T;
     const void* srecs = DESER ? (const void*)(p.header + kFixedHeader) : (const void*)p.structs;
     const bs_layer_rec* ly = DESER ? reinterpret_cast<const bs_layer_rec*>(p.header + kFixedHeader + kV2Struct * C) : p.layers;
     constexpr int kErrBad = DESER ? BS_ERR_CORRUPT : BS_ERR_ARG;
-
-    const uint64_t n_tiles = bad ? 0 : (T + kLTile - 1) / kLTile;
-    for (;;) {
-        __syncthreads();
-        if (tid == 0) s_tile = atomicAdd(&head->scan_ticket2, 1u);
-        __syncthreads();
-        const uint64_t tile = s_tile;
-        if (tile >= n_tiles) break;
-        uint64_t vb[kLItems], vn[kLItems];
-        uint64_t tsum[2] = {0, 0};
-        int err = 0;
+    uint64_t vb[kLItems], vn[kLItems], woff[kLItems];
+    uint32_t sfirst[kLItems];
+    uint64_t tsum[2] = {0, 0};
+    int err = 0;
 #pragma unroll
-        for (uint32_t k = 0; k < kLItems; ++k) {
-            const uint64_t t = tile * kLTile + (uint64_t)tid * kLItems + k;
-            vb[k] = 0; vn[k] = 0;
-            if (t < T) {
-                const uint4 w = __ldg(reinterpret_cast<const uint4*>(ly + t));  // structure, tag, offset
-                const uint32_t s = w.x;
-                if (s >= C) err = kErrBad;
-                else {
-                    const StructHead h = load_struct(srecs, s);
-                    const uint64_t* g = DESER ? p.lw.gp : p.lw.gs;
-                    vb[k] = (g[(uint64_t)h.first + h.n] & ~15ull) - (g[h.first] & ~15ull);
-                    vn[k] = h.n;
-                    if (DESER) {  // layer offsets = exclusive prefix sum of layer_bytes, checked link by link, inside [0, P]
-                        const uint64_t off = (uint64_t)w.z | ((uint64_t)w.w << 32);
-                        uint64_t next = P_hdr;
-                        if (t + 1 < T) next = __ldg(reinterpret_cast<const unsigned long long*>(&ly[t + 1].offset));
-                        if (t == 0 && off != 0) err = BS_ERR_CORRUPT;
-                        if (off > P_hdr || h.layer_bytes > P_hdr - off || off + h.layer_bytes != next) err = BS_ERR_CORRUPT;
-                    }
+    for (uint32_t k = 0; k < kLItems; ++k) {
+        const uint64_t t = tile * kLTile + (uint64_t)tid * kLItems + k;
+        vb[k] = 0; vn[k] = 0; woff[k] = 0; sfirst[k] = 0;
+        if (t < T && !bad) {
+            const uint4 w = __ldg(reinterpret_cast<const uint4*>(ly + t));  // structure, tag, offset
+            const uint32_t st = w.x;
+            if (st >= C) err = kErrBad;
+            else {
+                const StructHead h = load_struct(srecs, st);
+                const uint64_t* g = DESER ? p.lw.gp : p.lw.gs;
+                vb[k] = (g[(uint64_t)h.first + h.n] & ~15ull) - (g[h.first] & ~15ull);
+                vn[k] = h.n;
+                sfirst[k] = h.first;
+                if (DESER) woff[k] = (uint64_t)w.z | ((uint64_t)w.w << 32);
+                if (DESER) {  // layer offsets = exclusive prefix sum of layer_bytes, checked link by link, inside [0, P]
+                    const uint64_t off = (uint64_t)w.z | ((uint64_t)w.w << 32);
+                    uint64_t next = s.P_hdr;
+                    if (t + 1 < T) next = __ldg(reinterpret_cast<const unsigned long long*>(&ly[t + 1].offset));
+                    if (t == 0 && off != 0) err = BS_ERR_CORRUPT;
+                    if (off > s.P_hdr || h.layer_bytes > s.P_hdr - off || off + h.layer_bytes != next) err = BS_ERR_CORRUPT;
                 }
             }
-            tsum[0] += vb[k];
-            tsum[1] += vn[k];
         }
-        if (err) set_err(head, nullptr, err);
-        uint64_t excl[2];
-        chained_scan<2>(tsum, excl, tile, p.lw.st2[0], p.lw.st2[1], sm);
-        uint64_t r0 = excl[0], r1 = excl[1];
+        tsum[0] += vb[k];
+        tsum[1] += vn[k];
+    }
+    if (err) set_err(head, nullptr, err);
+    uint64_t excl[2];
+    chained_scan<2>(tsum, excl, tile, p.lw.st2[0], p.lw.st2[1], sm);
+    uint64_t r0 = excl[0], r1 = excl[1];
 #pragma unroll
-        for (uint32_t k = 0; k < kLItems; ++k) {
-            const uint64_t t = tile * kLTile + (uint64_t)tid * kLItems + k;
-            if (t < T) {
-                LayerPos lp; lp.off = r0; lp.first_addr = r1;
-                p.lw.lpos[t] = lp;
-            }
-            r0 += vb[k];
-            r1 += vn[k];
+    for (uint32_t k = 0; k < kLItems; ++k) {
+        const uint64_t t = tile * kLTile + (uint64_t)tid * kLItems + k;
+        if (t < T) {
+            LayerPos lp; lp.off = r0; lp.first_addr = r1;
+            lp.stream_off = DESER ? woff[k] : r0; lp.sfirst = sfirst[k]; lp.sn = (uint32_t)vn[k];
+            p.lw.lpos[t] = lp;
         }
-        if (tile == n_tiles - 1 && tid == 0) {
-            LayerPos lp; lp.off = sm.prefix[0] + sm.total[0]; lp.first_addr = sm.prefix[1] + sm.total[1];
-            p.lw.lpos[T] = lp;
-        }
+        r0 += vb[k];
+        r1 += vn[k];
     }
-
-    // ---- last CTA out: totals, capacity checks, sentinel, result ----
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        s_last = (atomicAdd(&head->ctas_done2, 1u) == gridDim.x - 1) ? 1u : 0u;
-    }
-    __syncthreads();
-    if (s_last && tid == 0) {
-        __threadfence();
-        int status = vh->status;
-        uint64_t tot_bytes = 0, tot_blocks = 0;
-        if (!bad && T != 0) {
-            const volatile LayerPos* end = p.lw.lpos + T;
-            tot_bytes = end->off; tot_blocks = end->first_addr;
-        } else if (!bad) {
-            LayerPos lp; lp.off = 0; lp.first_addr = 0;
-            p.lw.lpos[0] = lp;
-        }
-        uint64_t P = DESER ? P_hdr : tot_bytes;
-        uint64_t pool = DESER ? tot_bytes : 0;
-        if (bad) { P = 0; pool = 0; }
-        const uint64_t total = hb + P;
-        const uint64_t ng = (P + kGranule - 1) / kGranule;
-        if (status == 0) {
-            if (DESER && T == 0 && P_hdr != 0) status = BS_ERR_CORRUPT;
-            else if (tot_blocks >= (1ull << 32)) status = BS_ERR_UNSUPPORTED;
-            else if (!DESER && total > p.capacity) status = BS_ERR_CAPACITY;
-            else if (!DESER && p.expect_total != 0 && total != p.expect_total) status = BS_ERR_ARG;
-            else if (ng + 1 > p.lw.ws.n_granules_cap) status = BS_ERR_CAPACITY;
-            else if (tot_blocks > p.lw.blk_cap || tot_blocks > p.n_addr) status = BS_ERR_CAPACITY;
-            else if (DESER && p.flags == BS_LAYOUT_POOL && pool > p.pool_bytes) status = BS_ERR_CAPACITY;
-        }
-        if (!bad && tot_blocks <= p.lw.blk_cap) {
-            Blk e; e.off = P; e.addr = 0;
-            p.lw.ws.blk[tot_blocks] = e;
-            if (ng < p.lw.ws.n_granules_cap) p.lw.ws.tile_first[ng] = (uint32_t)tot_blocks;
-        }
-        vh->n_structs = (uint32_t)C;
-        vh->n_struct_blocks = (uint32_t)Bs;
-        vh->n_tensors = (uint32_t)T;
-        vh->n_blocks = (uint32_t)tot_blocks;
-        vh->header_bytes = hb;
-        vh->payload_bytes = P;
-        vh->pool_bytes = pool;
-        vh->n_granules = ng;
-        vh->status = status;
-        if (p.result != nullptr) {
-            bs_result r;
-            r.total_bytes = total; r.header_bytes = hb; r.payload_bytes = P; r.pool_bytes = pool;
-            r.status = status; r.n_tensors = (uint32_t)T; r.n_blocks = (uint32_t)tot_blocks;
-            r.reserved[0] = (uint32_t)C; r.reserved[1] = (uint32_t)Bs;
-            for (int z = 2; z < 5; ++z) r.reserved[z] = 0;
-            *p.result = r;
-        }
-        __threadfence();
+    if (tile == s.n2 - 1 && tid == 0) {  // the owner of the last tile knows the totals (T == 0: zeros)
+        LayerPos lp; lp.off = sm.prefix[0] + sm.total[0]; lp.first_addr = sm.prefix[1] + sm.total[1];
+        lp.stream_off = 0; lp.sfirst = 0; lp.sn = 0;
+        p.lw.lpos[T] = lp;
     }
 }
 
-// ---- pass 3: one warp per layer writes the flat work table blk[] / tile_first[] ------------------------------------------
+// ---- end of phase 2 (one thread): totals, capacity checks, sentinel, result ---------------------------------------------------
 template <bool DESER>
-__global__ void __launch_bounds__(kLThreads) lexpand_kernel(const LPlanParams p)
+__device__ __forceinline__ void plan_finalize(const LPlanParams& p, const PlanShape& s)
 {
+    volatile WsHead* vh = p.lw.ws.head;
+    int status = vh->status;
+    const bool bad = !s.ok;
+    uint64_t tot_bytes = 0, tot_blocks = 0;
+    if (s.ok) {
+        const volatile LayerPos* end = p.lw.lpos + s.T;
+        tot_bytes = end->off; tot_blocks = end->first_addr;
+    }
+    uint64_t P = DESER ? s.P_hdr : tot_bytes;
+    uint64_t pool = DESER ? tot_bytes : 0;
+    if (status != 0) { pool = 0; if (!DESER) P = 0; tot_blocks = 0; }
+    if (bad) P = 0;
+    const uint64_t hb = s.hb;
+    const uint64_t total = hb + P;
+    const uint64_t ng = (P + kGranule - 1) / kGranule;
+    if (status == 0) {
+        if (DESER && s.T == 0 && s.P_hdr != 0) status = BS_ERR_CORRUPT;
+        else if (tot_blocks >= (1ull << 32)) status = BS_ERR_UNSUPPORTED;
+        else if (!DESER && total > p.capacity) status = BS_ERR_CAPACITY;
+        else if (!DESER && p.expect_total != 0 && total != p.expect_total) status = BS_ERR_ARG;
+        else if (ng + 1 > p.lw.ws.n_granules_cap) status = BS_ERR_CAPACITY;
+        else if (tot_blocks > p.lw.blk_cap || tot_blocks > p.n_addr) status = BS_ERR_CAPACITY;
+        else if (DESER && p.flags == BS_LAYOUT_POOL && pool > p.pool_bytes) status = BS_ERR_CAPACITY;
+    }
+    if (s.ok && tot_blocks <= p.lw.blk_cap) {
+        Blk e; e.off = P; e.addr = 0;
+        p.lw.ws.blk[tot_blocks] = e;
+        if (ng < p.lw.ws.n_granules_cap) p.lw.ws.tile_first[ng] = (uint32_t)tot_blocks;
+    }
+    if (s.ok) {
+        vh->n_structs = (uint32_t)s.C;
+        vh->n_struct_blocks = (uint32_t)s.Bs;
+        vh->n_tensors = (uint32_t)s.T;
+    }
+    vh->n_blocks = (uint32_t)tot_blocks;
+    vh->header_bytes = hb;
+    vh->payload_bytes = P;
+    vh->pool_bytes = pool;
+    vh->n_granules = ng;
+    vh->status = status;
+    if (p.result != nullptr) {
+        bs_result r;
+        r.total_bytes = total; r.header_bytes = hb; r.payload_bytes = P; r.pool_bytes = pool;
+        r.status = status; r.n_tensors = vh->n_tensors; r.n_blocks = (uint32_t)tot_blocks;
+        r.reserved[0] = vh->n_structs; r.reserved[1] = vh->n_struct_blocks;
+        for (int z = 2; z < 5; ++z) r.reserved[z] = 0;
+        *p.result = r;
+    }
+}
+
+// ---- phase 3: blocks [chunk*kLTile, +kLTile) of the flat work table ------------------------------------------------------------
+// Block i belongs to the last layer t with first_addr[t] <= i (binary search over lpos[], L2-resident; four searches per
+// thread in flight).  Writes blk[i] = {payload offset, address | odd} and the granule boundaries inside the block.
+template <bool DESER>
+__device__ __forceinline__ void plan_expand_chunk(const LPlanParams& p, uint64_t chunk, uint64_t B, uint64_t T, uint64_t hb,
+                                                  const uint32_t* s_index, uint32_t n_index, uint32_t stride,
+                                                  uint32_t* big_idx, uint32_t* big_cnt, uint64_t* big_g0)
+{
+    WsHead* head = p.lw.ws.head;
+    const uint32_t tid = threadIdx.x, lane = tid & 31;
+    const LayerPos* lpos = p.lw.lpos;
+
+    uint64_t idx[kLItems];
+    uint32_t lo[kLItems], hi[kLItems];
+#pragma unroll
+    for (uint32_t k = 0; k < kLItems; ++k) {  // level 1: the sampled index in shared memory
+        idx[k] = chunk * kLTile + (uint64_t)k * kLThreads + tid;
+        uint32_t a = 0, b = n_index;  // answer in [a, b): s_index[0] == 0 <= i
+        while (b - a > 1) {
+            const uint32_t mid = (a + b) >> 1;
+            if ((uint64_t)s_index[mid] <= idx[k]) a = mid; else b = mid;
+        }
+        lo[k] = a * stride;
+        hi[k] = (uint64_t)(a + 1) * stride < T ? (a + 1) * stride : (uint32_t)T;
+    }
+    for (uint32_t span = stride; span > 1; span = (span + 1) >> 1) {  // level 2: ceil(log2 stride) rounds in lpos[]
+#pragma unroll
+        for (uint32_t k = 0; k < kLItems; ++k) {
+            if (hi[k] - lo[k] > 1) {
+                const uint32_t mid = (lo[k] + hi[k]) >> 1;
+                if (lpos[mid].first_addr <= idx[k]) lo[k] = mid; else hi[k] = mid;
+            }
+        }
+    }
+#pragma unroll
+    for (uint32_t k = 0; k < kLItems; ++k) {
+        const uint64_t i = idx[k];
+        bool big = false;
+        uint64_t g0 = 0, cnt = 0;
+        if (i < B) {
+            const LayerPos lp = lpos[lo[k]];
+            const uint64_t j = (uint64_t)lp.sfirst + (i - lp.first_addr);
+            const uint64_t g = p.lw.gs[j], gn = p.lw.gs[j + 1], gf = p.lw.gs[lp.sfirst];
+            const uint64_t off = lp.stream_off + ((g & ~15ull) - (gf & ~15ull));
+            const uint64_t stored = (gn & ~15ull) - (g & ~15ull);
+            const uint64_t odd = g & 1ull;
+            uint64_t address;
+            if (!DESER) {
+                address = __ldg(reinterpret_cast<const unsigned long long*>(p.addr + i));
+                if (address & 7) set_err(head, p.result, BS_ERR_ARG);  // D16
+            } else if (p.flags == BS_SCATTER_TO_ADDR) {
+                address = __ldg(reinterpret_cast<const unsigned long long*>(p.out_addr + i));
+                if (address & 7) set_err(head, p.result, BS_ERR_ARG);
+            } else {
+                address = p.pool_base + lp.off + (p.lw.gp[j] - p.lw.gp[lp.sfirst]);
+                p.out_addr[i] = address;
+            }
+            if (DESER && odd && p.payload != nullptr) {  // pad bytes are zero
+                const uint64_t pad = __ldg(reinterpret_cast<const unsigned long long*>(p.payload + hb + off + stored - 8));
+                if (pad != 0) set_err(head, p.result, BS_ERR_CORRUPT);
+            }
+            Blk e;
+            e.off = off;
+            e.addr = (address & ~7ull) | odd;
+            p.lw.ws.blk[i] = e;
+            // granule boundaries g*kGranule inside [off, off + stored)
+            g0 = (off + kGranule - 1) / kGranule;
+            const uint64_t g1 = (off + stored + kGranule - 1) / kGranule;
+            cnt = g1 > g0 ? g1 - g0 : 0;
+            if (cnt <= 4) {
+                for (uint64_t q = 0; q < cnt; ++q)
+                    if (g0 + q < p.lw.ws.n_granules_cap) p.lw.ws.tile_first[g0 + q] = (uint32_t)i;
+            } else {
+                big = true;
+            }
+        }
+        // large blocks: the whole warp fills their boundaries
+        const uint32_t bigs = __ballot_sync(0xffffffffu, big);
+        if (bigs) {
+            if (big) {
+                const uint32_t slot = __popc(bigs & ((1u << lane) - 1u));
+                big_idx[slot] = (uint32_t)i;
+                big_g0[slot] = g0;
+                big_cnt[slot] = cnt > 0xffffffffull ? 0xffffffffu : (uint32_t)cnt;
+            }
+            __syncwarp();
+            const uint32_t nb = __popc(bigs);
+            for (uint32_t sl = 0; sl < nb; ++sl) {
+                const uint64_t b0 = big_g0[sl];
+                const uint32_t c = big_cnt[sl], ix = big_idx[sl];
+                for (uint64_t q = lane; q < c; q += 32)
+                    if (b0 + q < p.lw.ws.n_granules_cap) p.lw.ws.tile_first[b0 + q] = ix;
+            }
+            __syncwarp();
+        }
+    }
+}
+
+template <bool DESER>
+__global__ void __launch_bounds__(kLThreads) lplan_kernel(const LPlanParams p)
+{
+    __shared__ uint32_t s_item;
+    __shared__ uint32_t s_flag;
+    __shared__ ChainSmem<2> sm;
     __shared__ uint32_t s_big_idx[kLThreads];
     __shared__ uint32_t s_big_cnt[kLThreads];
     __shared__ uint64_t s_big_g0[kLThreads];
+    __shared__ uint32_t s_index[kLTile];  // first_addr of every stride-th layer: level 1 of the layer search of phase 3
     WsHead* head = p.lw.ws.head;
-    if (head->status != 0) return;  // deferred error: no table, and the move kernels will write nothing
-    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint64_t C = head->n_structs, T = head->n_tensors, hb = head->header_bytes;
-    const void* srecs = DESER ? (const void*)(p.header + kFixedHeader) : (const void*)p.structs;
-    const bs_layer_rec* ly = DESER ? reinterpret_cast<const bs_layer_rec*>(p.header + kFixedHeader + kV2Struct * C) : p.layers;
-    const uint64_t n_warps = (uint64_t)gridDim.x * (kLThreads / 32);
-    uint32_t* big_idx = s_big_idx + warp * 32;
-    uint32_t* big_cnt = s_big_cnt + warp * 32;
-    uint64_t* big_g0 = s_big_g0 + warp * 32;
+    const uint32_t tid = threadIdx.x, warp = tid >> 5;
+    const PlanShape s = plan_shape<DESER>(p, head);
+    const uint32_t n12 = s.n1 + s.n2;
+    uint32_t n_index = 0, stride = 1;
 
-    for (uint64_t t = (uint64_t)blockIdx.x * (kLThreads / 32) + warp; t < T; t += n_warps) {
-        const uint4 w = __ldg(reinterpret_cast<const uint4*>(ly + t));
-        const StructHead h = load_struct(srecs, w.x);
-        const LayerPos lp = p.lw.lpos[t];
-        const uint64_t base_off = DESER ? ((uint64_t)w.z | ((uint64_t)w.w << 32)) : lp.off;
-        const uint64_t gs_f = p.lw.gs[h.first] & ~15ull;
-        const uint64_t gp_f = DESER ? p.lw.gp[h.first] : 0;
-        for (uint32_t j0 = 0; j0 < h.n; j0 += 32) {
-            const uint32_t j = j0 + lane;
-            bool big = false;
-            uint64_t g0 = 0, cnt = 0;
-            uint64_t i = 0;
-            if (j < h.n) {
-                const uint64_t g = p.lw.gs[(uint64_t)h.first + j], gn = p.lw.gs[(uint64_t)h.first + j + 1];
-                const uint64_t off = base_off + ((g & ~15ull) - gs_f);
-                const uint64_t stored = (gn & ~15ull) - (g & ~15ull);
-                const uint64_t odd = g & 1ull;
-                i = lp.first_addr + j;
-                uint64_t address;
-                if (!DESER) {
-                    address = __ldg(reinterpret_cast<const unsigned long long*>(p.addr + i));
-                    if (address & 7) set_err(head, p.result, BS_ERR_ARG);  // D16
-                } else if (p.flags == BS_SCATTER_TO_ADDR) {
-                    address = __ldg(reinterpret_cast<const unsigned long long*>(p.out_addr + i));
-                    if (address & 7) set_err(head, p.result, BS_ERR_ARG);
-                } else {
-                    address = p.pool_base + lp.off + (p.lw.gp[(uint64_t)h.first + j] - gp_f);
-                    p.out_addr[i] = address;
-                }
-                if (DESER && odd && p.payload != nullptr) {  // pad bytes are zero
-                    const uint64_t pad = __ldg(reinterpret_cast<const unsigned long long*>(p.payload + hb + off + stored - 8));
-                    if (pad != 0) set_err(head, p.result, BS_ERR_CORRUPT);
-                }
-                Blk e;
-                e.off = off;
-                e.addr = (address & ~7ull) | odd;
-                p.lw.ws.blk[i] = e;
-                // granule boundaries g*kGranule inside [off, off + stored)
-                g0 = (off + kGranule - 1) / kGranule;
-                const uint64_t g1 = (off + stored + kGranule - 1) / kGranule;
-                cnt = g1 > g0 ? g1 - g0 : 0;
-                if (cnt <= 4) {
-                    for (uint64_t q = 0; q < cnt; ++q)
-                        if (g0 + q < p.lw.ws.n_granules_cap) p.lw.ws.tile_first[g0 + q] = (uint32_t)i;
-                } else {
-                    big = true;
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_item = atomicAdd(&head->scan_ticket, 1u);
+        __syncthreads();
+        const uint32_t item = s_item;
+        if (item < s.n1) {
+            plan_blocks_tile<DESER>(p, s, item, sm);
+            __syncthreads();
+            if (tid == 0) {
+                __threadfence();
+                if (atomicAdd(&head->ctas_done, 1u) == s.n1 - 1) {  // phase 1 is complete: hand its status to phase 2
+                    __threadfence();
+                    const uint32_t st = (*(volatile int*)&head->status != 0) ? 1u : 0u;
+                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(&head->status_pass1), "r"(st | 2u) : "memory");
                 }
             }
-            // large blocks: the whole warp fills their boundaries
-            const uint32_t bigs = __ballot_sync(0xffffffffu, big);
-            if (bigs) {
-                if (big) {
-                    const uint32_t slot = __popc(bigs & ((1u << lane) - 1u));
-                    big_idx[slot] = (uint32_t)i;
-                    big_g0[slot] = g0;
-                    big_cnt[slot] = cnt > 0xffffffffull ? 0xffffffffu : (uint32_t)cnt;
-                }
-                __syncwarp();
-                const uint32_t nb = __popc(bigs);
-                for (uint32_t s = 0; s < nb; ++s) {
-                    const uint64_t b0 = big_g0[s];
-                    const uint32_t c = big_cnt[s], idx = big_idx[s];
-                    for (uint64_t q = lane; q < c; q += 32)
-                        if (b0 + q < p.lw.ws.n_granules_cap) p.lw.ws.tile_first[b0 + q] = idx;
-                }
-                __syncwarp();
+        } else if (item < n12) {
+            if (tid == 0) {
+                uint32_t v = 3u;  // no phase 1 (the fixed header was rejected): nothing to scan
+                if (s.n1 != 0)
+                    while (((v = ld_acquire_u32(&head->status_pass1)) & 2u) == 0) __nanosleep(64);
+                s_flag = v & 1u;
             }
+            __syncthreads();
+            plan_layers_tile<DESER>(p, s, item - s.n1, s_flag != 0, sm);
+            __syncthreads();
+            if (tid == 0) {
+                __threadfence();
+                if (atomicAdd(&head->ctas_done2, 1u) == s.n2 - 1) {  // every layer tile is done
+                    __threadfence();
+                    plan_finalize<DESER>(p, s);
+                    __threadfence();
+                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(&head->scan_ticket2), "r"(1u) : "memory");
+                }
+            }
+        } else {
+            cta_wait_until(&head->scan_ticket2, 1u);  // the plan is ready
+            const volatile WsHead* vh = head;
+            if (vh->status != 0) return;  // deferred error: no table, and the move kernels will write nothing
+            const uint64_t B = vh->n_blocks;
+            const uint64_t chunk = item - n12;
+            if (chunk * kLTile >= B) return;  // every later item is out of range too
+            const uint64_t T = vh->n_tensors;
+            if (n_index == 0) {  // first chunk of this CTA
+                stride = (uint32_t)((T + kLTile - 1) / kLTile);
+                n_index = (uint32_t)((T + stride - 1) / stride);
+                for (uint32_t q = tid; q < n_index; q += kLThreads) s_index[q] = (uint32_t)p.lw.lpos[(uint64_t)q * stride].first_addr;
+                __syncthreads();
+            }
+            plan_expand_chunk<DESER>(p, chunk, B, T, vh->header_bytes, s_index, n_index, stride, s_big_idx + warp * 32,
+                                     s_big_cnt + warp * 32, s_big_g0 + warp * 32);
         }
     }
 }
@@ -605,12 +688,14 @@ int check_layered(const bs_layered_desc* s)
     return BS_OK;
 }
 
-unsigned grid_for(uint64_t items, uint64_t per_cta, int sms, int per_sm)
+// one CTA per work item, at most a few waves' worth resident (items are claimed dynamically)
+unsigned plan_grid(const LPlanParams& p, int sms)
 {
-    uint64_t want = (items + per_cta - 1) / per_cta;
-    const uint64_t cap = (uint64_t)sms * per_sm;
+    const uint64_t m = p.Bs > p.C ? p.Bs : p.C;
+    uint64_t want = (m + kLTile - 1) / kLTile + (p.T + kLTile - 1) / kLTile + (p.n_addr + kLTile - 1) / kLTile + 3;
+    const uint64_t cap = (uint64_t)sms * 8;
     if (want > cap) want = cap;
-    return want == 0 ? 1u : (unsigned)want;
+    return (unsigned)want;
 }
 
 }  // namespace
@@ -660,10 +745,7 @@ int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t 
     p.Bs = set->n_struct_blocks;
     p.T = set->n_layers;
     p.n_addr = set->n_addr;
-    const unsigned g1 = grid_for(p.Bs > p.C ? p.Bs : p.C, kLTile, sms, 4);
-    lplan_blocks_kernel<false><<<g1, kLThreads, 0, stream>>>(p);
-    lplan_layers_kernel<false><<<grid_for(p.T, kLTile, sms, 4), kLThreads, 0, stream>>>(p);
-    lexpand_kernel<false><<<grid_for(p.T, kLThreads / 32, sms, 8), kLThreads, 0, stream>>>(p);
+    lplan_kernel<false><<<plan_grid(p, sms), kLThreads, 0, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
@@ -691,10 +773,7 @@ int run_layered_deserialize_plan(const void* d_header, const void* d_payload, ui
     p.out_dim = out->dim;
     p.out_addr = out->addr;
     p.flags = flags;
-    const unsigned g1 = grid_for(p.Bs > p.C ? p.Bs : p.C, kLTile, sms, 4);
-    lplan_blocks_kernel<true><<<g1, kLThreads, 0, stream>>>(p);
-    lplan_layers_kernel<true><<<grid_for(p.T, kLTile, sms, 4), kLThreads, 0, stream>>>(p);
-    lexpand_kernel<true><<<grid_for(p.T, kLThreads / 32, sms, 8), kLThreads, 0, stream>>>(p);
+    lplan_kernel<true><<<plan_grid(p, sms), kLThreads, 0, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;

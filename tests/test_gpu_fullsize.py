@@ -138,3 +138,68 @@ def test_full_size_offload_prefetch_config3():
     assert a["tensors"].tobytes() == b["tensors"].tobytes() and (a["qn"] == b["qn"]).all() and (a["dim"] == b["dim"]).all()
     assert ((a["addr"] - np.uint64(opool.data_ptr())) == (b["addr"] - np.uint64(ref_pool.data_ptr()))).all()
     eng.destroy()
+
+
+@pytest.mark.parametrize("cfg", ["3", "4"])
+def test_full_size_layered_v2(cfg):
+    """Wire format v2 (structure-shared layers) at full size, default launch configuration: the whole header against
+    the v2 oracle's (its payload part is skipped by giving the oracle a capacity check only), the payload against the
+    v1 stream of the same tensors (pinned relation: identical payload), size prediction, device fixpoint."""
+    from oracle import v2
+    bset = W.make_config(cfg)
+    up = Uploaded(bset, fill="device")
+    lv = W.layered_view(bset)
+    counts = (len(lv["structs"]), lv["dim"].shape[0], bset.n_tensors, bset.n_blocks)
+    dset = bs.DeviceLayeredSet.from_host(lv["structs"], lv["layers"], lv["qn"], lv["dim"], up.addr, DEV)
+    hb, total = v2.serialized_size(lv["structs"], lv["layers"], lv["dim"])
+    hb1, total1 = oracle.serialized_size(bset.n_tensors, bset.dim)
+    assert total - hb == total1 - hb1 and hb * 20 < hb1
+    cs = bs.current_stream()
+    ws = bs.Workspace(0, 0, total, DEV, layered=counts)
+    assert bs.layered_serialized_size(dset.desc, ws.ptr, ws.nbytes, cs) == (hb, total)
+    stream = torch.full((total + 4096,), 0xCD, dtype=torch.uint8, device=DEV)
+    bs.layered_serialize(dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, None, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and (res["header_bytes"], res["total_bytes"]) == (hb, total)
+    assert bool((stream[total:] == 0xCD).all())
+    # header: the oracle's plan, written out by the independent struct reader's field list
+    from tests.streamreader import read_stream_v2
+    plan = v2.plan(lv["structs"], lv["layers"], lv["dim"])
+    fixed, structs, layers, blocks, slack, _ = read_stream_v2(stream[:hb].cpu().numpy().tobytes() + b"")
+    assert (fixed["n_structs"], fixed["n_struct_blocks"], fixed["n_layers"], fixed["header_bytes"], fixed["payload_bytes"]) == \
+        (counts[0], counts[1], counts[2], hb, total - hb)
+    assert [s["layer_bytes"] for s in structs] == plan["layer_bytes"].tolist()
+    assert [l["offset"] for l in layers] == plan["layer_offset"].tolist()
+    assert [l["structure"] for l in layers] == lv["layers"]["structure"].tolist()
+    assert [b["offset"] for b in blocks] == plan["rel_offset"].tolist()
+    assert [b["dim"] for b in blocks] == [tuple(int(x) for x in d) for d in lv["dim"]]
+    assert set(slack) <= {0}
+    # payload: sampled tensors against the v1 oracle's slice-wise payload (same bytes, same payload offsets)
+    for t in sampled_tensors(bset, n=6):
+        first, want, _ = oracle_tensor_payload(bset, t)
+        got = stream[hb + first: hb + first + len(want)].cpu().numpy()
+        assert (got == want).all(), f"layer {t}: payload differs"
+    # and, every byte, against the v1 CUDA stream's payload
+    ws1 = bs.Workspace(bset.n_tensors, bset.n_blocks, total1, DEV)
+    s1 = torch.empty(total1, dtype=torch.uint8, device=DEV)
+    bs.serialize(up.dset.desc, s1.data_ptr(), total1, ws1.ptr, ws1.nbytes, ws1.result_ptr, None, cs)
+    assert ws1.read_result()["status"] == bs.OK
+    assert torch.equal(s1[hb1:], stream[hb:total])
+    del s1, ws1
+    # deserialize + fixpoint on the device
+    need = int(((bset.nelems * 8 + 255) // 256 * 256).sum())
+    out = bs.DeviceLayeredSet.empty(*counts, DEV, fill=0xAB)
+    opool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    bs.layered_deserialize(stream.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                           ws.result_ptr, None, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["pool_bytes"] == need and res["n_blocks"] == bset.n_blocks
+    h = out.to_host(*counts)
+    assert (h["qn"] == lv["qn"]).all() and (h["dim"] == lv["dim"]).all()
+    slots = (bset.nelems * 8 + 255) // 256 * 256
+    want_addr = opool.data_ptr() + np.concatenate([[0], np.cumsum(slots)[:-1]]).astype(np.uint64)
+    assert (h["addr"] == want_addr.astype(np.uint64)).all()
+    again = torch.full((total,), 0x11, dtype=torch.uint8, device=DEV)
+    bs.layered_serialize(out.desc, again.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, None, cs)
+    assert ws.read_result()["status"] == bs.OK
+    assert torch.equal(again, stream[:total]), "serialize(deserialize(S)) != S"
