@@ -3,6 +3,7 @@
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import this
 package.  It imports nothing from paper_2412_04676_b200.
 """
+from . import bs_oracle_pkg as pkg  # noqa: F401  (self-contained packages)
 from . import bs_oracle_v2 as v2  # noqa: F401  (wire format v2: structure-shared layers)
 from .bs_oracle import (  # noqa: F401
     ERR_ARG,
@@ -27,7 +28,8 @@ from .bs_oracle import build as _build_v1
 
 
 def build(force: bool = False) -> str:
-    """Compile every C file of the oracle (v1 and v2 libraries)."""
+    """Compile every C file of the oracle (v1, v2 and package libraries)."""
     so = _build_v1(force)
     v2.build(force)
+    pkg.build(force)
     return so
