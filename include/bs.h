@@ -309,6 +309,70 @@ int bs_offload_layered_async(bs_engine *e, const bs_layered_desc *set, uint64_t 
 int bs_prefetch_layered_async(bs_engine *e, const void *h_pinned, uint64_t nbytes, bs_layered_desc *out, void *d_pool,
                               uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket **ticket);
 
+/* ==== self-contained packages (PAPER §III.B.3) =========================================
+ *
+ * "Each serialized component is self contained in the sense that the string contains not only the deserializable data,
+ * but also metadata which pinpoints the location of the component within the original, whole object.  As a result,
+ * these packages can be sent, mixed with other packages and received back without the need to keep track of their
+ * order" (L124); they "can be cut down into even smaller packages ... to keep MPI package sizes below an implementation
+ * or self imposed upper limit" (L126).  A package is a 64-byte header followed by a range of a wire-format-v1 stream:
+ *
+ *   package        := package_header(64) | stream bytes [lo, lo + nbytes)
+ *   package_header : char magic[8]="BSPKG001"; u32 version=1; u32 index; u32 count; u32 first_block; u64 stream_id;
+ *                    u64 total_bytes; u64 lo; u64 nbytes; u64 first_block_offset
+ *     first_block        = the block holding the package's first payload byte (the largest i with offset_i <= lo -
+ *                          header_bytes); BS_PKG_NO_BLOCK for a package of the header region
+ *     first_block_offset = lo - header_bytes - offset_{first_block}   (0 for a package of the header region)
+ *   the cut (a function of header_bytes, total_bytes and the size limit `cap`, a multiple of 16): the header region
+ *   [0, header_bytes) is cut into ceil(header_bytes/cap) packages of cap bytes (the last one shorter), then the payload
+ *   likewise; index counts them in stream order.  No package straddles the header / payload boundary, so the packages
+ *   of the header region rebuild the block table and every payload package is then unpacked on its own, in any order.
+ *
+ * Packages live in SLOTS: n_slots buffers of slot_bytes each (slot_bytes a multiple of 16, >= 64 + cap), slot s at
+ * base + s*slot_bytes.  A slot whose magic is not "BSPKG001" or whose stream_id differs is foreign and is skipped
+ * ("mixed with other packages").  Who checks what on the receiving side: the HOST reads the 64-byte package headers to
+ * plan the copies and checks what that plan relies on (version, agreement on count and total_bytes, every index exactly
+ * once, ranges tiling [0,total) in index order, each fitting its slot, none straddling the header boundary) and fails at
+ * once with BS_ERR_CORRUPT; the DEVICE checks each package against the parsed stream (total_bytes, first_block and
+ * first_block_offset against the offset table) and every v1 header check of bs_deserialize, deferred as usual, before
+ * any block is written. */
+enum { BS_PKG_HEADER = 64 };
+#define BS_PKG_NO_BLOCK 0xFFFFFFFFu
+
+/* number of packages of a stream; 0 for an invalid cut (cap == 0, cap % 16 != 0, header_bytes > total_bytes) */
+uint64_t bs_package_count(uint64_t header_bytes, uint64_t total_bytes, uint64_t cap);
+/* stream range [*lo, *hi) of package `index`; BS_ERR_ARG for an invalid cut or index */
+int bs_package_range(uint64_t header_bytes, uint64_t total_bytes, uint64_t cap, uint64_t index, uint64_t *lo, uint64_t *hi);
+/* workspace for bs_package_emit / bs_package_unpack: bs_workspace_bytes + room for the assembled header region */
+uint64_t bs_package_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint64_t stream_capacity);
+
+/* Serialize `set` straight into packages in DEVICE slots: package k -> d_slots + slot(k)*slot_bytes with
+ * slot(k) = h_slot_of[k] (HOST array of `count` entries, each < n_slots, all different) or k when h_slot_of is NULL.
+ * total_bytes = the size prediction (bs_serialized_size; re-checked on the device); 0 computes it, which SYNCHRONISES
+ * `stream`.  Bytes of a slot behind its package are not written.  bs_result: as bs_serialize, reserved[0] = count.
+ * At once: BS_ERR_ARG (cap, slot_bytes, slot map), BS_ERR_CAPACITY (count > n_slots, workspace). */
+int bs_package_emit(const bs_set_desc *set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id, void *d_slots,
+                    uint64_t slot_bytes, uint64_t n_slots, const uint32_t *h_slot_of, void *d_workspace,
+                    uint64_t workspace_bytes, bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
+
+/* Deserialize from packages lying in DEVICE slots in any order, foreign slots skipped.  Copies the n_slots package
+ * headers to the host and SYNCHRONISES `stream` once to plan; then as bs_deserialize (same outputs, flags, deferred
+ * statuses; BS_ERR_CORRUPT also for a package that disagrees with the parsed stream). */
+int bs_package_unpack(const void *d_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id, bs_set_desc *out,
+                      void *d_pool, uint64_t pool_bytes, uint32_t flags, void *d_workspace, uint64_t workspace_bytes,
+                      bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
+
+/* The same through the engine, slots in pinned HOST memory (the receive buffers of L126): package k is packed into a
+ * staging buffer behind its header and DMA'd to h_slots + slot(k)*slot_bytes; cap + 64 <= chunk_bytes.  Prefetch takes
+ * the slots in the order they lie (arrival order): header-region packages first, then every payload package is DMA'd
+ * and unpacked on its own.  Ticket / checkpoint semantics as bs_offload_async / bs_prefetch_async. */
+int bs_offload_packages_async(bs_engine *e, const bs_set_desc *set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id,
+                              void *h_slots, uint64_t slot_bytes, uint64_t n_slots, const uint32_t *h_slot_of,
+                              cudaStream_t producer, bs_ticket **ticket);
+int bs_prefetch_packages_async(bs_engine *e, const void *h_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id,
+                               bs_set_desc *out, void *d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer,
+                               bs_ticket **ticket);
+
 int bs_ticket_wait(bs_ticket *t, bs_ticket_stats *stats /* may be NULL */); /* blocks the host; returns the deferred status */
 int bs_ticket_query(const bs_ticket *t);                                   /* BS_OK | BS_PENDING | BS_ERR_* */
 int bs_ticket_stream_wait(const bs_ticket *t, cudaStream_t stream);        /* make `stream` wait for completion (no host block):

@@ -137,6 +137,16 @@ def lib():
     L.bs_layered_deserialize.argtypes = [vp, u64, LD, vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_offload_layered_async.argtypes = [vp, LD, u64, vp, u64, vp, C.POINTER(vp)]
     L.bs_prefetch_layered_async.argtypes = [vp, vp, u64, LD, vp, u64, u32, vp, C.POINTER(vp)]
+    pu32 = C.POINTER(C.c_uint32)
+    L.bs_package_count.restype = u64
+    L.bs_package_count.argtypes = [u64, u64, u64]
+    L.bs_package_range.argtypes = [u64, u64, u64, u64, pu64, pu64]
+    L.bs_package_workspace_bytes.restype = u64
+    L.bs_package_workspace_bytes.argtypes = [u32, u32, u64]
+    L.bs_package_emit.argtypes = [C.POINTER(SetDesc), u64, u64, u64, vp, u64, u64, pu32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_package_unpack.argtypes = [vp, u64, u64, u64, C.POINTER(SetDesc), vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_offload_packages_async.argtypes = [vp, C.POINTER(SetDesc), u64, u64, u64, vp, u64, u64, pu32, vp, C.POINTER(vp)]
+    L.bs_prefetch_packages_async.argtypes = [vp, vp, u64, u64, u64, C.POINTER(SetDesc), vp, u64, u32, vp, C.POINTER(vp)]
     L.bs_ticket_wait.argtypes = [vp, C.POINTER(TicketStats)]
     L.bs_ticket_query.argtypes = [vp]
     L.bs_ticket_destroy.argtypes = [vp]
@@ -260,6 +270,44 @@ def layered_deserialize(stream_ptr: int, nbytes: int, out: LayeredDesc, pool_ptr
                                                result_ptr, _opts(opts), stream), "bs_layered_deserialize")
 
 
+# ---- self-contained packages ----------------------------------------------------------------------
+PKG_HEADER = 64
+PKG_NO_BLOCK = 0xFFFFFFFF
+
+
+def _slot_map(slot_of):
+    if slot_of is None:
+        return None
+    return (C.c_uint32 * len(slot_of))(*[int(x) for x in slot_of])
+
+
+def package_count(header_bytes: int, total_bytes: int, cap: int) -> int:
+    return int(lib().bs_package_count(header_bytes, total_bytes, cap))
+
+
+def package_range(header_bytes: int, total_bytes: int, cap: int, index: int):
+    lo, hi = C.c_uint64(0), C.c_uint64(0)
+    _check(lib().bs_package_range(header_bytes, total_bytes, cap, index, C.byref(lo), C.byref(hi)), "bs_package_range")
+    return int(lo.value), int(hi.value)
+
+
+def package_workspace_bytes(n_tensors: int, n_blocks: int, stream_capacity: int) -> int:
+    return int(lib().bs_package_workspace_bytes(n_tensors, n_blocks, stream_capacity))
+
+
+def package_emit(desc: SetDesc, total_bytes: int, cap: int, stream_id: int, slots_ptr: int, slot_bytes: int, n_slots: int,
+                 slot_of, ws_ptr: int, ws_bytes: int, result_ptr: int, opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_package_emit(C.byref(desc), total_bytes, cap, stream_id, slots_ptr, slot_bytes, n_slots,
+                                        _slot_map(slot_of), ws_ptr, ws_bytes, result_ptr, _opts(opts), stream),
+                  "bs_package_emit")
+
+
+def package_unpack(slots_ptr: int, slot_bytes: int, n_slots: int, stream_id: int, out: SetDesc, pool_ptr: int,
+                   pool_bytes: int, flags: int, ws_ptr: int, ws_bytes: int, result_ptr: int, opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_package_unpack(slots_ptr, slot_bytes, n_slots, stream_id, C.byref(out), pool_ptr, pool_bytes, flags,
+                                          ws_ptr, ws_bytes, result_ptr, _opts(opts), stream), "bs_package_unpack")
+
+
 class Ticket:
     def __init__(self, handle: int):
         self._h = handle
@@ -311,6 +359,20 @@ class Engine:
         t = C.c_void_p(0)
         _check(lib().bs_prefetch_async(self._h, h_pinned_ptr, nbytes, C.byref(out), pool_ptr, pool_bytes, flags, consumer,
                                        C.byref(t)), "bs_prefetch_async")
+        return Ticket(t.value)
+
+    def offload_packages_async(self, desc: SetDesc, total_bytes: int, cap: int, stream_id: int, h_slots_ptr: int,
+                               slot_bytes: int, n_slots: int, slot_of=None, producer: int = 0) -> Ticket:
+        t = C.c_void_p(0)
+        _check(lib().bs_offload_packages_async(self._h, C.byref(desc), total_bytes, cap, stream_id, h_slots_ptr, slot_bytes,
+                                               n_slots, _slot_map(slot_of), producer, C.byref(t)), "bs_offload_packages_async")
+        return Ticket(t.value)
+
+    def prefetch_packages_async(self, h_slots_ptr: int, slot_bytes: int, n_slots: int, stream_id: int, out: SetDesc,
+                                pool_ptr: int, pool_bytes: int, flags: int = 0, consumer: int = 0) -> Ticket:
+        t = C.c_void_p(0)
+        _check(lib().bs_prefetch_packages_async(self._h, h_slots_ptr, slot_bytes, n_slots, stream_id, C.byref(out), pool_ptr,
+                                                pool_bytes, flags, consumer, C.byref(t)), "bs_prefetch_packages_async")
         return Ticket(t.value)
 
     def offload_layered_async(self, desc: LayeredDesc, total_bytes: int, h_pinned_ptr: int, h_capacity: int,

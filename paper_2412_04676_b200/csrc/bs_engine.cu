@@ -14,7 +14,9 @@
 #include <new>
 #include <string.h>
 
-#include "bs_internal.cuh"
+#include <algorithm>
+
+#include "bs_pkg.cuh"
 
 namespace bs {
 int cuda_fail(cudaError_t e);
@@ -62,6 +64,8 @@ struct bs_engine {
     unsigned char* header_buf;
     uint64_t header_cap;
     bs_result* d_result;
+    unsigned char* pkg_tab;  // device copy of the package headers of a bs_prefetch_packages_async call (grown on demand)
+    uint64_t pkg_tab_slots;
 };
 
 struct bs_ticket {
@@ -169,6 +173,7 @@ int bs_engine_destroy(bs_engine* e)
     if (e->ev_dep) cudaEventDestroy(e->ev_dep);
     if (e->ws) cudaFree(e->ws);
     if (e->header_buf) cudaFree(e->header_buf);
+    if (e->pkg_tab) cudaFree(e->pkg_tab);
     if (e->d_result) cudaFree(e->d_result);
     if (e->kstream) cudaStreamDestroy(e->kstream);
     if (e->cstream) cudaStreamDestroy(e->cstream);
@@ -348,6 +353,141 @@ int bs_prefetch_layered_async(bs_engine* e, const void* h_pinned, uint64_t nbyte
 {
     if (out == nullptr) return BS_ERR_ARG;
     return prefetch_impl(e, h_pinned, nbytes, nullptr, out, d_pool, pool_bytes, flags, consumer, ticket);
+}
+
+// ---- self-contained packages through the engine (bs.h "packages") ------------------------------------
+int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id,
+                              void* h_slots, uint64_t slot_bytes, uint64_t n_slots, const uint32_t* h_slot_of,
+                              cudaStream_t producer, bs_ticket** ticket)
+{
+    if (e == nullptr || set == nullptr || h_slots == nullptr || ticket == nullptr) return BS_ERR_ARG;
+    if (cap == 0 || (cap & 15) || (slot_bytes & 15) || slot_bytes < BS_PKG_HEADER + cap) return BS_ERR_ARG;
+    if (cap + BS_PKG_HEADER > e->cfg.chunk_bytes) return BS_ERR_CAPACITY;
+    if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
+    WsLayout L;
+    if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
+    int rc;
+    uint64_t hb = bs_header_bytes(set->n_tensors, set->n_blocks);
+    if (total_bytes == 0) {
+        if ((rc = bs_serialized_size(set, e->ws, e->ws_bytes, &hb, &total_bytes, producer))) return rc;
+    }
+    if (total_bytes > e->cfg.max_stream_bytes) return BS_ERR_CAPACITY;
+    const uint64_t count = pkg_count(hb, total_bytes, cap);
+    if (count == 0 || count >= (1ull << 32)) return BS_ERR_ARG;
+    if (count > n_slots) return BS_ERR_CAPACITY;
+    if (h_slot_of != nullptr) {
+        std::vector<bool> used((size_t)n_slots, false);
+        for (uint64_t k = 0; k < count; ++k) {
+            if (h_slot_of[k] >= n_slots || used[h_slot_of[k]]) return BS_ERR_ARG;
+            used[h_slot_of[k]] = true;
+        }
+    }
+    bs_ticket* t = nullptr;
+    if ((rc = ticket_create(&t))) return rc;
+    const uint32_t S = e->cfg.n_staging;
+    t->bytes = total_bytes + count * BS_PKG_HEADER;
+    t->n_chunks = (uint32_t)count;
+
+    if ((rc = engine_fence(e))) return rc;
+    CK(cudaEventRecord(e->ev_dep, producer));
+    CK(cudaStreamWaitEvent(e->kstream, e->ev_dep, 0));
+    CK(cudaEventRecord(t->t_begin, e->kstream));
+    if ((rc = run_serialize_scan(set, L, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream))) return rc;
+    for (uint64_t k = 0; k < count; ++k) {
+        const uint32_t b = (uint32_t)(k % S);
+        uint64_t lo = 0, hi = 0;
+        pkg_range(hb, total_bytes, cap, k, &lo, &hi);
+        if (k >= S) CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));  // staging[b] drained by DMA k-S
+        CK(launch_pkg_header(L, cap, stream_id, k, count, e->staging[b], e->d_result, e->kstream));
+        if ((rc = run_pack_range(set, L, e->staging[b] + BS_PKG_HEADER, lo, hi, e->opts, e->sms, e->kstream))) return rc;
+        if (k == 0) CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
+        CK(cudaEventRecord(e->ev_k[b], e->kstream));
+        CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));
+        if (k == 0) CK(cudaEventRecord(t->dma_begin, e->cstream));
+        unsigned char* slot = (unsigned char*)h_slots + (h_slot_of ? (uint64_t)h_slot_of[k] : k) * slot_bytes;
+        CK(cudaMemcpyAsync(slot, e->staging[b], BS_PKG_HEADER + (hi - lo), cudaMemcpyDeviceToHost, e->cstream));
+        CK(cudaEventRecord(e->ev_c[b], e->cstream));
+    }
+    CK(cudaEventRecord(t->dma_end, e->cstream));
+    CK(cudaEventRecord(t->done, e->cstream));
+    *ticket = t;
+    return BS_OK;
+}
+
+int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id,
+                               bs_set_desc* out, void* d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer,
+                               bs_ticket** ticket)
+{
+    if (e == nullptr || h_slots == nullptr || out == nullptr || ticket == nullptr || n_slots == 0) return BS_ERR_ARG;
+    if ((slot_bytes & 15) || slot_bytes < BS_PKG_HEADER + 16) return BS_ERR_ARG;
+    if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
+    const unsigned char* slots = (const unsigned char*)h_slots;
+    PkgPlan plan;  // the packages are in host RAM: their headers cost nothing to read
+    int rc = pkg_plan(slots, slot_bytes, n_slots, slot_bytes, stream_id, &plan);
+    if (rc) return rc;
+    if (plan.hb > e->header_cap || plan.total > e->cfg.max_stream_bytes) return BS_ERR_CAPACITY;
+    if (out->n_blocks > e->cfg.max_blocks || out->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
+    WsLayout L;
+    if (!ws_layout(e->ws, e->ws_bytes, out->n_blocks, &L)) return BS_ERR_CAPACITY;
+    for (const PkgItem& it : plan.items)
+        if (it.nbytes > e->cfg.chunk_bytes) return BS_ERR_CAPACITY;
+    if (n_slots > e->pkg_tab_slots) {  // a call-time allocation, only when a call brings more slots than any before
+        CK(cudaStreamSynchronize(e->kstream));
+        if (e->pkg_tab) cudaFree(e->pkg_tab);
+        e->pkg_tab = nullptr;
+        e->pkg_tab_slots = 0;
+        CK(cudaMalloc((void**)&e->pkg_tab, n_slots * BS_PKG_HEADER));
+        e->pkg_tab_slots = n_slots;
+    }
+    bs_ticket* t = nullptr;
+    if ((rc = ticket_create(&t))) return rc;
+    t->is_prefetch = true;
+    const uint32_t S = e->cfg.n_staging;
+    t->bytes = plan.total + plan.items.size() * BS_PKG_HEADER;
+    t->n_chunks = (uint32_t)plan.items.size();
+
+    if ((rc = engine_fence(e))) return rc;
+    CK(cudaEventRecord(e->ev_dep, consumer));
+    CK(cudaStreamWaitEvent(e->cstream, e->ev_dep, 0));
+    CK(cudaStreamWaitEvent(e->kstream, e->ev_dep, 0));
+    CK(cudaEventRecord(t->t_begin, e->cstream));
+    CK(cudaEventRecord(t->dma_begin, e->cstream));
+    // the package headers and the header region first: validate + offset table + descriptor rebuild
+    CK(cudaMemcpy2DAsync(e->pkg_tab, BS_PKG_HEADER, slots, slot_bytes, BS_PKG_HEADER, n_slots, cudaMemcpyHostToDevice, e->cstream));
+    for (uint32_t k = 0; k < plan.n_header; ++k) {
+        const PkgItem& it = plan.items[k];
+        CK(cudaMemcpyAsync(e->header_buf + it.lo, slots + it.slot * slot_bytes + BS_PKG_HEADER, it.nbytes, cudaMemcpyHostToDevice,
+                           e->cstream));
+    }
+    CK(cudaEventRecord(e->ev_fence_c, e->cstream));
+    CK(cudaStreamWaitEvent(e->kstream, e->ev_fence_c, 0));
+    if ((rc = run_deserialize_scan(e->header_buf, nullptr, plan.total, out, d_pool, pool_bytes, flags, L, e->d_result, e->sms,
+                                   e->kstream)))
+        return rc;
+    CK(launch_pkg_check(L, e->pkg_tab, BS_PKG_HEADER, n_slots, stream_id, e->d_result, e->kstream));
+    CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
+    if ((rc = run_unpack_range(out, L, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream))) return rc;
+    std::vector<PkgItem> by_slot(plan.items.begin() + plan.n_header, plan.items.end());
+    std::sort(by_slot.begin(), by_slot.end(), [](const PkgItem& a, const PkgItem& b) { return a.slot < b.slot; });
+    uint32_t k = 0;
+    for (const PkgItem& it : by_slot) {  // arrival order: each payload package is DMA'd and unpacked on its own
+        const uint32_t b = k % S;
+        if (k >= S) CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));  // staging[b] consumed by unpack k-S
+        CK(cudaMemcpyAsync(e->staging[b], slots + it.slot * slot_bytes + BS_PKG_HEADER, it.nbytes, cudaMemcpyHostToDevice, e->cstream));
+        CK(cudaEventRecord(e->ev_c[b], e->cstream));
+        CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));
+        if ((rc = run_unpack_range(out, L, e->staging[b], nullptr, it.lo, it.lo + it.nbytes, flags | kFlagCheckPad, e->opts, e->sms,
+                                   e->kstream)))
+            return rc;
+        CK(cudaEventRecord(e->ev_k[b], e->kstream));
+        ++k;
+    }
+    CK(cudaEventRecord(t->dma_end, e->cstream));
+    CK(cudaMemcpyAsync(&t->h_result->status, &((WsHead*)e->ws)->status, sizeof(int32_t), cudaMemcpyDeviceToHost, e->kstream));
+    CK(cudaEventRecord(t->done, e->kstream));
+    CK(cudaStreamWaitEvent(consumer, t->done, 0));
+    *ticket = t;
+    return BS_OK;
 }
 
 int bs_ticket_query(const bs_ticket* t)

@@ -112,9 +112,12 @@ class DeviceLayeredSet:
 class Workspace:
     """Device workspace + the 64-byte bs_result word of one call site."""
 
-    def __init__(self, n_tensors: int, n_blocks: int, stream_capacity: int, device="cuda", layered=None):
-        """layered = (n_structs, n_struct_blocks, n_layers, n_addr) sizes the workspace for wire format v2 instead."""
-        if layered is not None:
+    def __init__(self, n_tensors: int, n_blocks: int, stream_capacity: int, device="cuda", layered=None, packages=False):
+        """layered = (n_structs, n_struct_blocks, n_layers, n_addr) sizes the workspace for wire format v2 instead;
+        packages=True adds the room bs_package_unpack needs for the assembled header region."""
+        if packages:
+            self.nbytes = B.package_workspace_bytes(n_tensors, n_blocks, stream_capacity)
+        elif layered is not None:
             self.nbytes = B.layered_workspace_bytes(*layered, stream_capacity)
         else:
             self.nbytes = B.workspace_bytes(n_tensors, n_blocks, stream_capacity)
@@ -136,4 +139,5 @@ class Workspace:
         r = B.Result.from_buffer_copy(raw)
         return dict(total_bytes=int(r.total_bytes), header_bytes=int(r.header_bytes), payload_bytes=int(r.payload_bytes),
                     pool_bytes=int(r.pool_bytes), status=int(r.status), n_tensors=int(r.n_tensors), n_blocks=int(r.n_blocks),
-                    n_structs=int(r.reserved[0]), n_struct_blocks=int(r.reserved[1]))
+                    n_structs=int(r.reserved[0]), n_struct_blocks=int(r.reserved[1]),
+                    n_packages=int(r.reserved[0]))
