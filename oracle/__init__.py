@@ -5,6 +5,7 @@ package.  It imports nothing from paper_2412_04676_b200.
 """
 from . import bs_oracle_pkg as pkg  # noqa: F401  (self-contained packages)
 from . import bs_oracle_v2 as v2  # noqa: F401  (wire format v2: structure-shared layers)
+from .bs_oracle_queue import QueueModel  # noqa: F401  (save / load queue: the sequential definition)
 from .bs_oracle import (  # noqa: F401
     ERR_ARG,
     ERR_CAPACITY,
