@@ -373,6 +373,56 @@ int bs_prefetch_packages_async(bs_engine *e, const void *h_slots, uint64_t slot_
                                bs_set_desc *out, void *d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer,
                                bs_ticket **ticket);
 
+/* ==== save / load queue with checkpoints (PAPER §III.B.4) ============================
+ *
+ * "organizing asynchronous load and save into a kind of queuing system together with checkpoints to make sure that
+ * required data of a given computational task are already available in the memory, could maximize performance rate
+ * regarding IO operations" (L136-138).  A bs_queue is two engines — a SAVE lane and a LOAD lane, each with its own side
+ * streams, staging buffers and workspace — so a save (device -> host) and a load (host -> device) run at the same time,
+ * one in each direction of the PCIe link, and a table of KEYS that orders what must be ordered:
+ *   - what a caller observes is per-key PROGRAM ORDER: a load of `key` returns the object of the last save of `key`
+ *     submitted before it (the load lane waits, on the device, for that save's completion event); a save over a key
+ *     whose load is still running waits for the load (the host buffer is being read); operations on different keys
+ *     are independent and overlap.  Host buffers of different keys must not overlap.
+ *   - checkpoints are events, never host waits: bs_queue_load makes `consumer` wait for the loaded blocks,
+ *     bs_queue_checkpoint makes any stream wait until every operation submitted so far on `key` has completed (after
+ *     it, the saved blocks may be overwritten).
+ * Device memory held = 2 x (n_staging x chunk_bytes + O(max_blocks)), fixed at creation, whatever is in flight — not
+ * the extra serialized + deserialized buffers of the paper's Fig 3(c) (L136).  One queue is driven by one host thread. */
+typedef struct bs_queue bs_queue;
+
+typedef struct bs_queue_stats {
+    uint64_t saves, loads;             /* accepted calls */
+    uint64_t bytes_saved, bytes_loaded; /* stream bytes they move */
+    uint64_t host_bytes_live;          /* sum of the streams the live keys hold in host memory */
+    uint64_t host_bytes_peak;
+    uint64_t keys_live;
+    uint64_t device_bytes;             /* staging + workspace + header buffers of both lanes */
+    uint32_t in_flight;                /* operations submitted and not yet complete (at the time of the call) */
+    uint32_t max_in_flight;
+} bs_queue_stats;
+
+int bs_queue_create(bs_queue **out, const bs_engine_cfg *lane_cfg); /* both lanes get lane_cfg */
+int bs_queue_destroy(bs_queue *q);                                  /* drains first */
+
+/* Save `set` under `key` into h_pinned (as bs_offload_async: total_bytes = the size prediction, 0 computes it and
+ * synchronises `producer`).  A previous stream of `key` is replaced. */
+int bs_queue_save(bs_queue *q, uint64_t key, const bs_set_desc *set, uint64_t total_bytes, void *h_pinned,
+                  uint64_t h_capacity, cudaStream_t producer);
+/* Register a complete stream that is already in pinned host memory (it came from elsewhere) under `key`. */
+int bs_queue_adopt(bs_queue *q, uint64_t key, const void *h_pinned, uint64_t nbytes);
+/* Load the stream of `key` (as bs_prefetch_async).  BS_ERR_ARG for an unknown key. */
+int bs_queue_load(bs_queue *q, uint64_t key, bs_set_desc *out, void *d_pool, uint64_t pool_bytes, uint32_t flags,
+                  cudaStream_t consumer);
+int bs_queue_checkpoint(bs_queue *q, uint64_t key, cudaStream_t stream); /* device-side wait; BS_ERR_ARG: unknown key */
+/* Host-blocking: waits for the last save and the last load of `key`; returns the first deferred status that is not
+ * BS_OK.  Either stats pointer may be NULL; stats of an operation that never happened have n_chunks = 0, bytes = 0. */
+int bs_queue_wait(bs_queue *q, uint64_t key, bs_ticket_stats *save_stats, bs_ticket_stats *load_stats);
+int bs_queue_query(bs_queue *q, uint64_t key);   /* BS_OK | BS_PENDING | BS_ERR_* (BS_ERR_ARG: unknown key) */
+int bs_queue_forget(bs_queue *q, uint64_t key);  /* waits for the key's operations, then drops it: the host buffer is the caller's again */
+int bs_queue_drain(bs_queue *q);                 /* host-blocking: everything submitted so far has completed */
+int bs_queue_get_stats(bs_queue *q, bs_queue_stats *out);
+
 int bs_ticket_wait(bs_ticket *t, bs_ticket_stats *stats /* may be NULL */); /* blocks the host; returns the deferred status */
 int bs_ticket_query(const bs_ticket *t);                                   /* BS_OK | BS_PENDING | BS_ERR_* */
 int bs_ticket_stream_wait(const bs_ticket *t, cudaStream_t stream);        /* make `stream` wait for completion (no host block):

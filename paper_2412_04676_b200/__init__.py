@@ -8,7 +8,7 @@ There is no CPU fallback.
 from ._binding import (  # noqa: F401
     ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_CUDA, ERR_UNSUPPORTED, F64, LAYOUT_POOL, OK, PENDING, SCATTER_TO_ADDR,
     VARIANT_DEFAULT, VARIANT_LDG, VARIANT_TMA,
-    BsError, Engine, LayeredDesc, Opts, Result, SetDesc, Ticket,
+    BsError, Engine, LayeredDesc, Opts, Queue, Result, SetDesc, Ticket,
     layered_deserialize, layered_header_bytes, layered_serialize, layered_serialize_range, layered_serialized_size,
     layered_stream_info, layered_workspace_bytes, make_layered_desc,
     deserialize, header_bytes, last_cuda_error, lib, make_desc, serialize, serialize_range, serialized_size,

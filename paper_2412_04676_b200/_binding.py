@@ -88,6 +88,12 @@ class TicketStats(C.Structure):
                 ("total_ms", C.c_float)]
 
 
+class QueueStats(C.Structure):
+    _fields_ = [("saves", C.c_uint64), ("loads", C.c_uint64), ("bytes_saved", C.c_uint64), ("bytes_loaded", C.c_uint64),
+                ("host_bytes_live", C.c_uint64), ("host_bytes_peak", C.c_uint64), ("keys_live", C.c_uint64),
+                ("device_bytes", C.c_uint64), ("in_flight", C.c_uint32), ("max_in_flight", C.c_uint32)]
+
+
 assert C.sizeof(TensorRec) == 32 and C.sizeof(Result) == 64 and C.sizeof(StructRec) == 32 and C.sizeof(LayerRec) == 16
 
 _lib = None
@@ -147,6 +153,17 @@ def lib():
     L.bs_package_unpack.argtypes = [vp, u64, u64, u64, C.POINTER(SetDesc), vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_offload_packages_async.argtypes = [vp, C.POINTER(SetDesc), u64, u64, u64, vp, u64, u64, pu32, vp, C.POINTER(vp)]
     L.bs_prefetch_packages_async.argtypes = [vp, vp, u64, u64, u64, C.POINTER(SetDesc), vp, u64, u32, vp, C.POINTER(vp)]
+    L.bs_queue_create.argtypes = [C.POINTER(vp), C.POINTER(EngineCfg)]
+    L.bs_queue_destroy.argtypes = [vp]
+    L.bs_queue_save.argtypes = [vp, u64, C.POINTER(SetDesc), u64, vp, u64, vp]
+    L.bs_queue_adopt.argtypes = [vp, u64, vp, u64]
+    L.bs_queue_load.argtypes = [vp, u64, C.POINTER(SetDesc), vp, u64, u32, vp]
+    L.bs_queue_checkpoint.argtypes = [vp, u64, vp]
+    L.bs_queue_wait.argtypes = [vp, u64, C.POINTER(TicketStats), C.POINTER(TicketStats)]
+    L.bs_queue_query.argtypes = [vp, u64]
+    L.bs_queue_forget.argtypes = [vp, u64]
+    L.bs_queue_drain.argtypes = [vp]
+    L.bs_queue_get_stats.argtypes = [vp, C.POINTER(QueueStats)]
     L.bs_ticket_wait.argtypes = [vp, C.POINTER(TicketStats)]
     L.bs_ticket_query.argtypes = [vp]
     L.bs_ticket_destroy.argtypes = [vp]
@@ -392,6 +409,68 @@ class Engine:
     def destroy(self):
         if self._h:
             lib().bs_engine_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class Queue:
+    """bs_queue_*: a save lane and a load lane (one per PCIe direction) + keys ordered by events."""
+
+    def __init__(self, max_tensors: int, max_blocks: int, max_stream_bytes: int, chunk_bytes: int = 0, n_staging: int = 0,
+                 opts=None):
+        cfg = EngineCfg(chunk_bytes, n_staging, max_tensors, max_blocks, max_stream_bytes, make_opts(opts))
+        h = C.c_void_p(0)
+        _check(lib().bs_queue_create(C.byref(h), C.byref(cfg)), "bs_queue_create")
+        self._h = h.value
+        self._keys = set()   # which keys exist (BS_ERR_ARG is also a deferred status, so wait() must tell them apart)
+
+    def save(self, key: int, desc: SetDesc, total_bytes: int, h_pinned_ptr: int, h_capacity: int, producer: int = 0) -> None:
+        _check(lib().bs_queue_save(self._h, key, C.byref(desc), total_bytes, h_pinned_ptr, h_capacity, producer), "bs_queue_save")
+        self._keys.add(key)
+
+    def adopt(self, key: int, h_pinned_ptr: int, nbytes: int) -> None:
+        _check(lib().bs_queue_adopt(self._h, key, h_pinned_ptr, nbytes), "bs_queue_adopt")
+        self._keys.add(key)
+
+    def load(self, key: int, out: SetDesc, pool_ptr: int, pool_bytes: int, flags: int = 0, consumer: int = 0) -> None:
+        _check(lib().bs_queue_load(self._h, key, C.byref(out), pool_ptr, pool_bytes, flags, consumer), "bs_queue_load")
+
+    def checkpoint(self, key: int, stream: int = 0) -> None:
+        _check(lib().bs_queue_checkpoint(self._h, key, stream), "bs_queue_checkpoint")
+
+    def wait(self, key: int) -> dict:
+        """Host-blocking.  Returns the first deferred status and the two operations' stats (no exception for deferred errors)."""
+        s, l = TicketStats(), TicketStats()
+        if key not in self._keys:
+            raise BsError(ERR_ARG, "bs_queue_wait: unknown key")
+        rc = lib().bs_queue_wait(self._h, key, C.byref(s), C.byref(l))
+        f = lambda st: dict(status=int(st.status), bytes=int(st.bytes), n_chunks=int(st.n_chunks), dma_ms=float(st.dma_ms),
+                            total_ms=float(st.total_ms))
+        return dict(status=int(rc), save=f(s), load=f(l))
+
+    def query_raw(self, key: int) -> int:
+        return int(lib().bs_queue_query(self._h, key))
+
+    def forget(self, key: int) -> None:
+        _check(lib().bs_queue_forget(self._h, key), "bs_queue_forget")
+        self._keys.discard(key)
+
+    def drain(self) -> None:
+        _check(lib().bs_queue_drain(self._h), "bs_queue_drain")
+
+    def stats(self) -> dict:
+        st = QueueStats()
+        _check(lib().bs_queue_get_stats(self._h, C.byref(st)), "bs_queue_get_stats")
+        return {k: int(getattr(st, k)) for k, _ in QueueStats._fields_}
+
+    def destroy(self):
+        if self._h:
+            lib().bs_queue_destroy(self._h)
             self._h = None
 
     def __del__(self):

@@ -15,6 +15,8 @@
 #include <string.h>
 
 #include <algorithm>
+#include <unordered_map>
+#include <vector>
 
 #include "bs_pkg.cuh"
 
@@ -200,6 +202,9 @@ static int offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layered_d
     }
     if (total_bytes == 0) {  // size prediction on the producer stream (synchronises it)
         uint64_t hb = 0;
+        // the workspace may still be in use by the kernels of an earlier call: the query runs behind them
+        CK(cudaEventRecord(e->ev_fence_k, e->kstream));
+        CK(cudaStreamWaitEvent(producer, e->ev_fence_k, 0));
         rc = set ? bs_serialized_size(set, e->ws, e->ws_bytes, &hb, &total_bytes, producer)
                  : bs_layered_serialized_size(lset, e->ws, e->ws_bytes, &hb, &total_bytes, producer);
         if (rc) return rc;
@@ -241,8 +246,11 @@ static int offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layered_d
     return BS_OK;
 }
 
+// `known` (v1 only): the counts of a stream that is still on its way to h_pinned (queue: a load submitted behind the save
+// of the same key); otherwise the fixed header is read from host RAM.  Either way the device validates what arrives.
 static int prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs_set_desc* out, bs_layered_desc* lout,
-                         void* d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket** ticket)
+                         void* d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket** ticket,
+                         const bs_stream_info_t* known = nullptr)
 {
     if (e == nullptr || h_pinned == nullptr || (out == nullptr && lout == nullptr) || ticket == nullptr) return BS_ERR_ARG;
     if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
@@ -251,8 +259,8 @@ static int prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs
     WsLayout L;
     int rc;
     if (out) {
-        rc = bs_stream_info(h_pinned, &info);  // the stream is in host RAM: its counts cost nothing to read
-        if (rc) return rc;
+        if (known) info = *known;
+        else if ((rc = bs_stream_info(h_pinned, &info))) return rc;  // the stream is in host RAM: its counts cost nothing to read
         if (info.total_bytes != nbytes) return BS_ERR_CORRUPT;
         if (info.n_blocks > e->cfg.max_blocks || info.n_tensors > e->cfg.max_tensors || info.header_bytes > e->header_cap ||
             nbytes > e->cfg.max_stream_bytes)
@@ -369,6 +377,8 @@ int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t tot
     int rc;
     uint64_t hb = bs_header_bytes(set->n_tensors, set->n_blocks);
     if (total_bytes == 0) {
+        CK(cudaEventRecord(e->ev_fence_k, e->kstream));  // the workspace may still be in use by an earlier call
+        CK(cudaStreamWaitEvent(producer, e->ev_fence_k, 0));
         if ((rc = bs_serialized_size(set, e->ws, e->ws_bytes, &hb, &total_bytes, producer))) return rc;
     }
     if (total_bytes > e->cfg.max_stream_bytes) return BS_ERR_CAPACITY;
@@ -487,6 +497,250 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
     CK(cudaEventRecord(t->done, e->kstream));
     CK(cudaStreamWaitEvent(consumer, t->done, 0));
     *ticket = t;
+    return BS_OK;
+}
+
+// ==== save / load queue with checkpoints (bs.h "queue") ===============================================
+// Two engines (one per PCIe direction) + a key table.  Ordering between the lanes is by CUDA events only.
+struct bs_queue {
+    struct Entry {
+        bs_ticket* save = nullptr;  // last save / last load of the key (each lane is in order, so the last one covers all)
+        bs_ticket* load = nullptr;
+        const void* h = nullptr;
+        uint64_t nbytes = 0;
+        bs_stream_info_t info;
+        bool adopted = false;
+    };
+    bs_engine* lane_save = nullptr;
+    bs_engine* lane_load = nullptr;
+    std::unordered_map<uint64_t, Entry> keys;
+    std::vector<bs_ticket*> retired;  // replaced tickets, destroyed once complete
+    bs_queue_stats st;
+};
+
+static uint64_t engine_device_bytes(const bs_engine* e)
+{
+    return (uint64_t)e->cfg.n_staging * e->cfg.chunk_bytes + e->ws_bytes + e->header_cap + sizeof(bs_result);
+}
+
+static int engine_wait_ticket(bs_engine* e, const bs_ticket* t)  // everything the engine does next waits for t
+{
+    CK(cudaStreamWaitEvent(e->kstream, t->done, 0));
+    CK(cudaStreamWaitEvent(e->cstream, t->done, 0));
+    return BS_OK;
+}
+
+static bool ticket_complete(const bs_ticket* t) { return cudaEventQuery(t->done) != cudaErrorNotReady; }
+
+static void queue_reap(bs_queue* q, bool block)
+{
+    size_t w = 0;
+    for (bs_ticket* t : q->retired) {
+        if (block || ticket_complete(t)) bs_ticket_destroy(t);
+        else q->retired[w++] = t;
+    }
+    q->retired.resize(w);
+}
+
+static void queue_retire(bs_queue* q, bs_ticket*& t)
+{
+    if (t) q->retired.push_back(t);
+    t = nullptr;
+}
+
+static void queue_count_in_flight(bs_queue* q)
+{
+    uint32_t n = 0;
+    for (auto& kv : q->keys) {
+        if (kv.second.save && !ticket_complete(kv.second.save)) ++n;
+        if (kv.second.load && !ticket_complete(kv.second.load)) ++n;
+    }
+    for (bs_ticket* t : q->retired)
+        if (!ticket_complete(t)) ++n;
+    q->st.in_flight = n;
+    if (n > q->st.max_in_flight) q->st.max_in_flight = n;
+}
+
+static void queue_account_host(bs_queue* q)
+{
+    uint64_t live = 0;
+    for (auto& kv : q->keys) live += kv.second.nbytes;
+    q->st.host_bytes_live = live;
+    q->st.keys_live = q->keys.size();
+    if (live > q->st.host_bytes_peak) q->st.host_bytes_peak = live;
+}
+
+int bs_queue_create(bs_queue** out, const bs_engine_cfg* lane_cfg)
+{
+    if (out == nullptr || lane_cfg == nullptr) return BS_ERR_ARG;
+    bs_queue* q = new (std::nothrow) bs_queue;
+    if (!q) return BS_ERR_ARG;
+    memset(&q->st, 0, sizeof(q->st));
+    int rc = bs_engine_create(&q->lane_save, lane_cfg);
+    if (rc == BS_OK) rc = bs_engine_create(&q->lane_load, lane_cfg);
+    if (rc != BS_OK) {
+        if (q->lane_save) bs_engine_destroy(q->lane_save);
+        delete q;
+        return rc;
+    }
+    q->st.device_bytes = engine_device_bytes(q->lane_save) + engine_device_bytes(q->lane_load);
+    *out = q;
+    return BS_OK;
+}
+
+int bs_queue_drain(bs_queue* q)
+{
+    if (q == nullptr) return BS_ERR_ARG;
+    CK(cudaStreamSynchronize(q->lane_save->kstream));
+    CK(cudaStreamSynchronize(q->lane_save->cstream));
+    CK(cudaStreamSynchronize(q->lane_load->kstream));
+    CK(cudaStreamSynchronize(q->lane_load->cstream));
+    queue_reap(q, true);
+    queue_count_in_flight(q);
+    return BS_OK;
+}
+
+int bs_queue_destroy(bs_queue* q)
+{
+    if (q == nullptr) return BS_ERR_ARG;
+    bs_queue_drain(q);
+    for (auto& kv : q->keys) {
+        if (kv.second.save) bs_ticket_destroy(kv.second.save);
+        if (kv.second.load) bs_ticket_destroy(kv.second.load);
+    }
+    bs_engine_destroy(q->lane_save);
+    bs_engine_destroy(q->lane_load);
+    delete q;
+    return BS_OK;
+}
+
+int bs_queue_save(bs_queue* q, uint64_t key, const bs_set_desc* set, uint64_t total_bytes, void* h_pinned, uint64_t h_capacity,
+                  cudaStream_t producer)
+{
+    if (q == nullptr || set == nullptr || h_pinned == nullptr) return BS_ERR_ARG;
+    queue_reap(q, false);
+    int rc;
+    auto it = q->keys.find(key);
+    // the host buffer may still be read by a load of this key (or, for a new buffer under the same key, nothing to wait for)
+    if (it != q->keys.end() && it->second.load && !ticket_complete(it->second.load))
+        if ((rc = engine_wait_ticket(q->lane_save, it->second.load))) return rc;
+    bs_ticket* t = nullptr;
+    if ((rc = bs_offload_async(q->lane_save, set, total_bytes, h_pinned, h_capacity, producer, &t))) return rc;
+    total_bytes = t->bytes;  // the size prediction, if the call made it
+    bs_queue::Entry& en = q->keys[key];
+    queue_retire(q, en.save);
+    en.save = t;
+    en.h = h_pinned;
+    en.nbytes = total_bytes;
+    en.adopted = false;
+    en.info.n_tensors = set->n_tensors;
+    en.info.n_blocks = set->n_blocks;
+    en.info.header_bytes = bs_header_bytes(set->n_tensors, set->n_blocks);
+    en.info.payload_bytes = total_bytes - en.info.header_bytes;
+    en.info.total_bytes = total_bytes;
+    q->st.saves += 1;
+    q->st.bytes_saved += total_bytes;
+    queue_account_host(q);
+    queue_count_in_flight(q);
+    return BS_OK;
+}
+
+int bs_queue_adopt(bs_queue* q, uint64_t key, const void* h_pinned, uint64_t nbytes)
+{
+    if (q == nullptr || h_pinned == nullptr || nbytes < kFixedHeader) return BS_ERR_ARG;
+    queue_reap(q, false);
+    auto it = q->keys.find(key);
+    if (it != q->keys.end()) {  // the old buffer's operations are not ours to order against the new one: finish them
+        int rc = bs_queue_wait(q, key, nullptr, nullptr);
+        (void)rc;
+        queue_retire(q, it->second.save);
+        queue_retire(q, it->second.load);
+    }
+    bs_queue::Entry& en = q->keys[key];
+    en.h = h_pinned;
+    en.nbytes = nbytes;
+    en.adopted = true;
+    queue_account_host(q);
+    return BS_OK;
+}
+
+int bs_queue_load(bs_queue* q, uint64_t key, bs_set_desc* out, void* d_pool, uint64_t pool_bytes, uint32_t flags,
+                  cudaStream_t consumer)
+{
+    if (q == nullptr || out == nullptr) return BS_ERR_ARG;
+    queue_reap(q, false);
+    auto it = q->keys.find(key);
+    if (it == q->keys.end()) return BS_ERR_ARG;
+    bs_queue::Entry& en = it->second;
+    int rc;
+    if (en.save && !ticket_complete(en.save))  // the stream is still on its way to the host buffer
+        if ((rc = engine_wait_ticket(q->lane_load, en.save))) return rc;
+    bs_ticket* t = nullptr;
+    rc = prefetch_impl(q->lane_load, en.h, en.nbytes, out, nullptr, d_pool, pool_bytes, flags, consumer, &t,
+                       en.adopted ? nullptr : &en.info);
+    if (rc) return rc;
+    queue_retire(q, en.load);
+    en.load = t;
+    q->st.loads += 1;
+    q->st.bytes_loaded += en.nbytes;
+    queue_count_in_flight(q);
+    return BS_OK;
+}
+
+int bs_queue_checkpoint(bs_queue* q, uint64_t key, cudaStream_t stream)
+{
+    if (q == nullptr) return BS_ERR_ARG;
+    auto it = q->keys.find(key);
+    if (it == q->keys.end()) return BS_ERR_ARG;
+    if (it->second.save) CK(cudaStreamWaitEvent(stream, it->second.save->done, 0));
+    if (it->second.load) CK(cudaStreamWaitEvent(stream, it->second.load->done, 0));
+    return BS_OK;
+}
+
+int bs_queue_wait(bs_queue* q, uint64_t key, bs_ticket_stats* save_stats, bs_ticket_stats* load_stats)
+{
+    if (q == nullptr) return BS_ERR_ARG;
+    auto it = q->keys.find(key);
+    if (it == q->keys.end()) return BS_ERR_ARG;
+    if (save_stats) memset(save_stats, 0, sizeof(*save_stats));
+    if (load_stats) memset(load_stats, 0, sizeof(*load_stats));
+    int rc_s = it->second.save ? bs_ticket_wait(it->second.save, save_stats) : BS_OK;
+    int rc_l = it->second.load ? bs_ticket_wait(it->second.load, load_stats) : BS_OK;
+    queue_count_in_flight(q);
+    return rc_s != BS_OK ? rc_s : rc_l;
+}
+
+int bs_queue_query(bs_queue* q, uint64_t key)
+{
+    if (q == nullptr) return BS_ERR_ARG;
+    auto it = q->keys.find(key);
+    if (it == q->keys.end()) return BS_ERR_ARG;
+    int rc_s = it->second.save ? bs_ticket_query(it->second.save) : BS_OK;
+    int rc_l = it->second.load ? bs_ticket_query(it->second.load) : BS_OK;
+    if (rc_s < 0) return rc_s;
+    if (rc_l < 0) return rc_l;
+    return (rc_s == BS_PENDING || rc_l == BS_PENDING) ? BS_PENDING : BS_OK;
+}
+
+int bs_queue_forget(bs_queue* q, uint64_t key)
+{
+    if (q == nullptr) return BS_ERR_ARG;
+    auto it = q->keys.find(key);
+    if (it == q->keys.end()) return BS_ERR_ARG;
+    if (it->second.save) bs_ticket_destroy(it->second.save);  // waits for completion
+    if (it->second.load) bs_ticket_destroy(it->second.load);
+    q->keys.erase(it);
+    queue_account_host(q);
+    queue_count_in_flight(q);
+    return BS_OK;
+}
+
+int bs_queue_get_stats(bs_queue* q, bs_queue_stats* out)
+{
+    if (q == nullptr || out == nullptr) return BS_ERR_ARG;
+    queue_reap(q, false);
+    queue_count_in_flight(q);
+    *out = q->st;
     return BS_OK;
 }
 

@@ -1,0 +1,168 @@
+"""NEXT-3 on the GPU: the save / load queue with checkpoints through the C ABI against the sequential
+definition oracle.QueueModel — whatever overlaps in time on the device, a caller sees per-key program order."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2412_04676_b200 as bs
+import workloads as W
+from tests.gpu_util import DEV, Uploaded
+from tests.util import host_addrs, oracle_stream
+
+pytestmark = pytest.mark.gpu
+
+
+def pinned(n, fill=0xCD):
+    t = torch.empty(max(n, 16), dtype=torch.uint8, pin_memory=True)
+    t.fill_(fill)
+    return t
+
+
+class Loaded:
+    def __init__(self, bset, need):
+        self.out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+        self.pool = torch.full((max(need, 256),), 0xEE, dtype=torch.uint8, device=DEV)
+        self.need = need
+
+
+def test_save_two_keys_and_load_them_back_while_saving_a_third():
+    sets = [W.make_config("2", n_ops=26 + 13 * i) for i in range(3)]
+    ups = [Uploaded(b) for b in sets]
+    model = oracle.QueueModel()
+    want = [model.save(k, b.tensors, b.qn, b.dim, host_addrs(u.host_pool, u.host_offs)) for k, (b, u) in enumerate(zip(sets, ups))]
+    cap = max(len(w) for w in want)
+    q = bs.Queue(max(b.n_tensors for b in sets), max(b.n_blocks for b in sets), cap, chunk_bytes=4 * 65536, n_staging=2)
+    hosts = [pinned(len(w) + 256) for w in want]
+    cs = bs.current_stream()
+    q.save(0, ups[0].dset.desc, len(want[0]), hosts[0].data_ptr(), hosts[0].numel(), cs)
+    q.save(1, ups[1].dset.desc, len(want[1]), hosts[1].data_ptr(), hosts[1].numel(), cs)
+    # loads are submitted at once, behind the saves they depend on; the save of key 2 runs in the other lane meanwhile
+    ld = [Loaded(sets[k], oracle.pool_bytes(want[k])) for k in range(2)]
+    q.load(0, ld[0].out.desc, ld[0].pool.data_ptr(), ld[0].need, bs.LAYOUT_POOL, cs)
+    q.save(2, ups[2].dset.desc, 0, hosts[2].data_ptr(), hosts[2].numel(), cs)      # size 0: predicted by the call
+    q.load(1, ld[1].out.desc, ld[1].pool.data_ptr(), ld[1].need, bs.LAYOUT_POOL, cs)
+    snap = [l.pool.clone() for l in ld]     # enqueued on the consumer stream: sees the data (checkpoint, no host wait)
+    for k in range(3):
+        st = q.wait(k)
+        assert st["status"] == bs.OK, st
+        assert st["save"]["bytes"] == len(want[k])
+        assert (hosts[k].numpy()[:len(want[k])] == want[k]).all(), f"stream of key {k} differs from the oracle's"
+        assert (hosts[k].numpy()[len(want[k]):] == 0xCD).all()
+    for k in range(2):
+        ref = model.load(k)
+        assert (snap[k].cpu().numpy()[:ld[k].need] == ref["pool"][:ld[k].need]).all()
+        h = ld[k].out.to_host()
+        assert h["tensors"].tobytes() == sets[k].tensors.tobytes() and (h["qn"] == sets[k].qn).all() and (h["dim"] == sets[k].dim).all()
+    got, ref = q.stats(), model.stats()
+    for f in ("saves", "loads", "bytes_saved", "bytes_loaded", "host_bytes_live", "host_bytes_peak", "keys_live"):
+        assert got[f] == ref[f], (f, got, ref)
+    assert got["in_flight"] == 0 and got["max_in_flight"] >= 2
+    assert got["device_bytes"] < 2 * (2 * 4 * 65536) + (8 << 20)     # 2 lanes x 2 staging chunks + O(B): fixed, small
+    q.destroy()
+
+
+def test_a_seeded_sequence_of_saves_overwrites_loads_and_forgets_matches_the_model():
+    rng = np.random.default_rng(17)
+    model = oracle.QueueModel()
+    q = bs.Queue(64, 4096, 4 << 20, chunk_bytes=65536, n_staging=2)
+    cs = bs.current_stream()
+    hosts = {k: pinned(4 << 20) for k in range(4)}
+    keep = []          # device sets must stay alive until their save completed
+    pending = []       # (Loaded, reference pool, bset)
+    cur = {}           # the set each live key holds
+    for step in range(48):
+        key = int(rng.integers(0, 4))
+        r = rng.random()
+        if r < 0.5 or key not in model.store:
+            bset = W.make_set(f"q{step}", 300 + step, D=int(rng.integers(40, 160)), S=9, M=2, N0=3,
+                              n_ops=int(rng.integers(1, 14)), n_site=int(rng.integers(0, 2)), dims="multinomial")
+            up = Uploaded(bset)
+            keep.append(up)
+            s = model.save(key, bset.tensors, bset.qn, bset.dim, host_addrs(up.host_pool, up.host_offs))
+            q.save(key, up.dset.desc, len(s) if step % 3 else 0, hosts[key].data_ptr(), hosts[key].numel(), cs)
+            cur[key] = bset
+        elif r < 0.9:
+            ref = model.load(key)
+            bset = cur[key]
+            ld = Loaded(bset, oracle.pool_bytes(model.store[key]))
+            q.load(key, ld.out.desc, ld.pool.data_ptr(), ld.need, bs.LAYOUT_POOL, cs)
+            pending.append((ld, ref, bset))
+        else:
+            model.forget(key)
+            q.forget(key)
+            with pytest.raises(bs.BsError) as e:
+                q.load(key, keep[-1].dset.desc, 256, 0, bs.LAYOUT_POOL, cs)
+            assert e.value.code == bs.ERR_ARG
+    q.drain()
+    for ld, ref, bset in pending:     # every load saw the LAST save of its key that preceded it in program order
+        assert (ld.pool.cpu().numpy()[:ld.need] == ref["pool"][:ld.need]).all()
+        h = ld.out.to_host()
+        assert h["tensors"].tobytes() == bset.tensors.tobytes() and (h["dim"] == bset.dim).all()
+    for key, s in model.store.items():
+        assert q.wait(key)["status"] == bs.OK
+        assert (hosts[key].numpy()[:len(s)] == s).all()
+    got, ref = q.stats(), model.stats()
+    for f in ("saves", "loads", "bytes_saved", "bytes_loaded", "host_bytes_live", "host_bytes_peak", "keys_live"):
+        assert got[f] == ref[f], (f, got, ref)
+    q.destroy()
+
+
+def test_checkpoint_lets_the_producer_overwrite_its_blocks_without_a_host_wait():
+    bset = W.make_config("2", n_ops=39)
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    q = bs.Queue(bset.n_tensors, bset.n_blocks, len(want), chunk_bytes=65536, n_staging=2)
+    host = pinned(len(want))
+    cs = bs.current_stream()
+    q.save(5, up.dset.desc, len(want), host.data_ptr(), host.numel(), cs)
+    q.checkpoint(5, cs)
+    up.pool.fill_(0x77)            # on the producer stream, behind the checkpoint: must not leak into the saved stream
+    assert q.wait(5)["status"] == bs.OK
+    assert (host.numpy()[:len(want)] == want).all()
+    with pytest.raises(bs.BsError):
+        q.checkpoint(6, cs)
+    q.destroy()
+
+
+def test_adopted_streams_deferred_errors_and_overwrite_behind_a_running_load():
+    bset = W.make_set("fault", 41, D=40, S=9, M=2, N0=3, n_ops=13, n_site=1, dims="multinomial")
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    model = oracle.QueueModel()
+    q = bs.Queue(bset.n_tensors, bset.n_blocks, len(want) + 64, chunk_bytes=65536)
+    cs = bs.current_stream()
+    good = pinned(len(want))
+    good.numpy()[:] = want
+    model.adopt(1, want)
+    q.adopt(1, good.data_ptr(), len(want))
+    ld = Loaded(bset, oracle.pool_bytes(want))
+    q.load(1, ld.out.desc, ld.pool.data_ptr(), ld.need, bs.LAYOUT_POOL, cs)
+    # overwrite key 1 while its load may still be running: the save waits for the load (the host buffer is being read)
+    bset2 = W.make_set("fault2", 43, D=40, S=9, M=2, N0=3, n_ops=11, n_site=1, dims="multinomial")
+    up2 = Uploaded(bset2)
+    s2 = model.save(1, bset2.tensors, bset2.qn, bset2.dim, host_addrs(up2.host_pool, up2.host_offs))
+    assert len(s2) <= good.numel()
+    first = oracle.deserialize(want)
+    q.save(1, up2.dset.desc, len(s2), good.data_ptr(), good.numel(), cs)
+    assert q.wait(1)["status"] == bs.OK
+    assert (ld.pool.cpu().numpy()[:ld.need] == first["pool"][:ld.need]).all()      # the load saw the FIRST stream
+    assert (good.numpy()[:len(s2)] == s2).all()                                     # the buffer holds the SECOND now
+    # a corrupt adopted stream: deferred BS_ERR_CORRUPT, nothing written
+    bad = pinned(len(want))
+    bad.numpy()[:] = want
+    bad.numpy()[64 + 32 * bset.n_tensors + 48 * 3 + 40] ^= 0x10
+    q.adopt(2, bad.data_ptr(), len(want))
+    ld2 = Loaded(bset, oracle.pool_bytes(want))
+    q.load(2, ld2.out.desc, ld2.pool.data_ptr(), ld2.need, bs.LAYOUT_POOL, cs)
+    assert q.wait(2)["status"] == bs.ERR_CORRUPT
+    assert (ld2.pool.cpu().numpy() == 0xEE).all()
+    # a save whose size prediction is wrong: deferred BS_ERR_ARG; a load behind it is refused on the device
+    h3 = pinned(len(want) + 64)
+    q.save(3, up.dset.desc, len(want) + 16, h3.data_ptr(), h3.numel(), cs)
+    ld3 = Loaded(bset, oracle.pool_bytes(want))
+    q.load(3, ld3.out.desc, ld3.pool.data_ptr(), ld3.need, bs.LAYOUT_POOL, cs)
+    st = q.wait(3)
+    assert st["status"] == bs.ERR_ARG and st["load"]["status"] == bs.ERR_CORRUPT
+    assert (ld3.pool.cpu().numpy() == 0xEE).all()
+    q.destroy()
