@@ -420,7 +420,7 @@ def run_mine(args):
         pre_gbs = float(np.median([s[1]["bytes"] / s[1]["dma_ms"] / 1e6 for s in stats]))
         e2e = {"value": round(units_g / (e2e_ms_g * 1e-3) / 1e9, 3), "unit": UNIT, "h2d_bytes_per_step": int(total),
                "d2h_bytes_per_step": int(total), "ms_per_step": round(e2e_ms_g, 3),
-               "what": "bs_offload_async -> pinned host -> bs_prefetch_async, 256 MiB double-buffered chunks"}
+               "what": "bs_offload_async -> pinned host -> bs_prefetch_async, one after the other, 256 MiB double-buffered chunks"}
         detail.update({"offload_pcie_GBs": round(off_gbs, 2), "prefetch_pcie_GBs": round(pre_gbs, 2),
                        "pinned_d2h_GBs": round(bw["d2h"], 2), "pinned_h2d_GBs": round(bw["h2d"], 2),
                        "offload_frac_of_pinned_d2h": round(off_gbs / bw["d2h"], 4),
@@ -428,7 +428,104 @@ def run_mine(args):
                        "offload_total_ms": round(float(np.median([s[0]["total_ms"] for s in stats])), 3),
                        "prefetch_total_ms": round(float(np.median([s[1]["total_ms"] for s in stats])), 3)})
         eng.destroy()
+        if not v2 and not args.no_queue:
+            # ---- the queue: every step saves the set (device -> pinned host) while the stream saved by
+            # the step before is loaded back (pinned host -> device): both directions of the link at once.  Same bytes
+            # per step as above; this is the e2e headline, the one-after-the-other number stays in detail. ----
+            host2 = torch.empty(total, dtype=torch.uint8, pin_memory=True)
+            hosts = [host, host2]
+            dbuf = torch.empty(2 * nlink, dtype=torch.uint8, device=dev)
+            s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+            best = 1e9
+            for _ in range(5):   # link denominator with both directions busy, same run
+                torch.cuda.synchronize()
+                a.record()
+                s1.wait_stream(torch.cuda.current_stream()); s2.wait_stream(torch.cuda.current_stream())
+                with torch.cuda.stream(s1):
+                    host[:nlink].copy_(dbuf[:nlink], non_blocking=True)
+                with torch.cuda.stream(s2):
+                    dbuf[nlink:].copy_(host2[:nlink], non_blocking=True)
+                torch.cuda.current_stream().wait_stream(s1); torch.cuda.current_stream().wait_stream(s2)
+                b.record(); torch.cuda.synchronize()
+                best = min(best, a.elapsed_time(b))
+            bw["bidir"] = 2 * nlink / best / 1e6
+            del dbuf
+            q = bs.Queue(bset.n_tensors, bset.n_blocks, total, chunk_bytes=args.chunk_mb << 20, n_staging=2, opts=opts)
+            for k in (0, 1):
+                q.save(k, dset.desc, total, hosts[k].data_ptr(), total, cs)
+
+            def q_steps(n, i0):
+                for i in range(i0, i0 + n):
+                    q.save(i % 2, dset.desc, total, hosts[i % 2].data_ptr(), total, cs)
+                    q.load((i + 1) % 2, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, cs)
+                q.checkpoint(0, cs)
+                q.checkpoint(1, cs)
+
+            q_steps(2, 0)
+            barrier()
+            a.record()
+            q_steps(n_e2e, 2)
+            b.record()
+            barrier()
+            for k in (0, 1):
+                st = q.wait(k)
+                if st["status"]:
+                    raise RuntimeError(f"queue status {st}")
+            q_ms = a.elapsed_time(b) / n_e2e
+            q_ms_g, q_units_g = aggregate(q_ms, 2 * total, world, dev, ready)
+            detail["e2e_one_after_the_other"] = dict(e2e)
+            qv = q_units_g / (q_ms_g * 1e-3) / 1e9
+            e2e = {"value": round(qv, 3), "unit": UNIT, "h2d_bytes_per_step": int(total), "d2h_bytes_per_step": int(total),
+                   "ms_per_step": round(q_ms_g, 3),
+                   "what": "bs_queue: every step bs_queue_save of the set (device -> pinned host) overlapped with bs_queue_load "
+                           "of the stream the step before saved (pinned host -> device); 256 MiB double-buffered chunks per lane"}
+            detail["queue"] = {"aggregate_pcie_GBs": round(2 * total / q_ms / 1e6, 2),
+                               "pinned_bidirectional_memcpy_GBs": round(bw["bidir"], 2),
+                               "frac_of_bidirectional_memcpy": round(2 * total / q_ms / 1e6 / bw["bidir"], 4),
+                               "device_bytes_held": q.stats()["device_bytes"], "host_bytes_live": q.stats()["host_bytes_live"]}
+            q.destroy()
+            del host2, hosts
         del host
+
+    # ---- self-contained packages: the same bytes as packages in device slots, emitted and unpacked
+    # package by package; the size limit decides how many launches the bytes are spread over ----
+    if not v2 and not args.no_packages:
+        pk = {}
+        for cap_mb in (256, 4):
+            cap = cap_mb << 20
+            n_pk = bs.package_count(hb, total, cap)
+            slot_bytes = 64 + cap
+            try:
+                slots = torch.empty(n_pk * slot_bytes, dtype=torch.uint8, device=dev)
+            except torch.cuda.OutOfMemoryError:
+                break
+            wsp = bs.Workspace(bset.n_tensors, bset.n_blocks, cap_guess, dev, packages=True)
+
+            def emit():
+                bs.package_emit(dset.desc, total, cap, 7, slots.data_ptr(), slot_bytes, n_pk, None, wsp.ptr, wsp.nbytes,
+                                wsp.result_ptr, opts, cs)
+
+            def unpack():
+                bs.package_unpack(slots.data_ptr(), slot_bytes, n_pk, 7, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL,
+                                  wsp.ptr, wsp.nbytes, wsp.result_ptr, opts, cs)
+
+            emit(); unpack()
+            if wsp.read_result()["status"] != bs.OK:
+                raise RuntimeError(f"packages: {wsp.read_result()}")
+            t = {}
+            for name, fn in (("emit", emit), ("unpack", unpack)):
+                torch.cuda.synchronize()
+                a.record()
+                for _ in range(3):
+                    fn()
+                b.record()
+                torch.cuda.synchronize()
+                t[name] = a.elapsed_time(b) / 3
+            pk[f"cap_{cap_mb}MiB"] = {"packages": int(n_pk), "emit_ms": round(t["emit"], 3), "unpack_ms_incl_plan_sync": round(t["unpack"], 3),
+                                      "emit_hbm_GBs": round(2 * total / t["emit"] / 1e6, 1),
+                                      "unpack_hbm_GBs": round(2 * total / t["unpack"] / 1e6, 1)}
+            del slots, wsp
+        detail["packages"] = pk
 
     # ---- config 5: exposed IO of an offload overlapped with a stand-in contraction (rank 0 only) ----
     if rank == 0 and not args.no_config5 and not v2:
@@ -547,6 +644,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--standin-items", type=int, default=60000)
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-packages", action="store_true")
+    ap.add_argument("--no-queue", action="store_true", help="e2e: offload then prefetch only, no duplex queue leg")
     ap.add_argument("--no-config5", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

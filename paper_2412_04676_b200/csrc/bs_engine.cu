@@ -15,6 +15,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <unordered_map>
 #include <vector>
 
@@ -85,6 +86,67 @@ struct bs_ticket {
         if (e__ != cudaSuccess) return cuda_fail(e__);    \
     } while (0)
 
+// Pinned result words of the tickets come from a process-wide slab: cudaHostAlloc / cudaFreeHost synchronise the
+// device, and a ticket created while another lane's transfer is running must not wait for it.
+namespace {
+constexpr size_t kResultSlab = 1024;
+std::mutex g_slab_mutex;
+bs_result* g_slab = nullptr;
+std::vector<bs_result*> g_slab_free;
+
+cudaError_t result_slot_get(bs_result** out)
+{
+    std::lock_guard<std::mutex> lock(g_slab_mutex);
+    if (g_slab == nullptr) {
+        cudaError_t e = cudaHostAlloc((void**)&g_slab, kResultSlab * sizeof(bs_result), cudaHostAllocDefault);
+        if (e != cudaSuccess) return e;
+        for (size_t i = kResultSlab; i-- > 0;) g_slab_free.push_back(g_slab + i);
+    }
+    if (g_slab_free.empty()) return cudaHostAlloc((void**)out, sizeof(bs_result), cudaHostAllocDefault);  // > 1024 live tickets
+    *out = g_slab_free.back();
+    g_slab_free.pop_back();
+    return cudaSuccess;
+}
+
+void result_slot_put(bs_result* r)
+{
+    std::lock_guard<std::mutex> lock(g_slab_mutex);
+    if (g_slab != nullptr && r >= g_slab && r < g_slab + kResultSlab) g_slab_free.push_back(r);
+    else cudaFreeHost(r);
+}
+}  // namespace
+
+// The deferred outcome reaches the ticket's pinned result word by plain stores of a one-thread kernel (pinned host
+// memory is device-addressable), not by a copy-engine transfer: a 64-byte cudaMemcpyAsync would queue behind the
+// bulk DMA chunks of the OTHER lane that go in the same direction and stall this lane's kernel stream for milliseconds.
+__global__ void post_result_kernel(bs_result* h_dst, const bs_result* d_src)
+{
+    const bs_result r = *d_src;
+    volatile bs_result* o = h_dst;
+    o->total_bytes = r.total_bytes; o->header_bytes = r.header_bytes; o->payload_bytes = r.payload_bytes;
+    o->pool_bytes = r.pool_bytes; o->n_tensors = r.n_tensors; o->n_blocks = r.n_blocks;
+    for (int i = 0; i < 5; ++i) o->reserved[i] = r.reserved[i];
+    __threadfence_system();
+    o->status = r.status;
+    __threadfence_system();
+}
+__global__ void post_status_kernel(bs_result* h_dst, const int32_t* d_status)
+{
+    volatile bs_result* o = h_dst;
+    o->status = *d_status;
+    __threadfence_system();
+}
+static cudaError_t post_result(bs_result* h_dst, const bs_result* d_src, cudaStream_t stream)
+{
+    post_result_kernel<<<1, 1, 0, stream>>>(h_dst, d_src);
+    return cudaGetLastError();
+}
+static cudaError_t post_status(bs_result* h_dst, const int32_t* d_status, cudaStream_t stream)
+{
+    post_status_kernel<<<1, 1, 0, stream>>>(h_dst, d_status);
+    return cudaGetLastError();
+}
+
 static int ticket_create(bs_ticket** out)
 {
     bs_ticket* t = new (std::nothrow) bs_ticket;
@@ -93,7 +155,7 @@ static int ticket_create(bs_ticket** out)
     cudaError_t e;
     if ((e = cudaEventCreate(&t->t_begin)) != cudaSuccess || (e = cudaEventCreate(&t->dma_begin)) != cudaSuccess ||
         (e = cudaEventCreate(&t->dma_end)) != cudaSuccess || (e = cudaEventCreate(&t->done)) != cudaSuccess ||
-        (e = cudaHostAlloc((void**)&t->h_result, sizeof(bs_result), cudaHostAllocDefault)) != cudaSuccess) {
+        (e = result_slot_get(&t->h_result)) != cudaSuccess) {
         delete t;
         return cuda_fail(e);
     }
@@ -225,7 +287,7 @@ static int offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layered_d
     rc = set ? run_serialize_scan(set, L, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream)
              : run_layered_serialize_plan(lset, e->ws, e->ws_bytes, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
+    CK(post_result(t->h_result, e->d_result, e->kstream));
     for (uint32_t k = 0; k < t->n_chunks; ++k) {
         const uint32_t b = k % S;
         const uint64_t lo = (uint64_t)k * C, hi = (lo + C < total_bytes) ? lo + C : total_bytes;
@@ -306,7 +368,7 @@ static int prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs
              : run_layered_deserialize_plan(e->header_buf, nullptr, nbytes, lout, d_pool, pool_bytes, flags, e->ws, e->ws_bytes,
                                             e->d_result, e->sms, e->kstream);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
+    CK(post_result(t->h_result, e->d_result, e->kstream));
     rc = out ? run_unpack_range(out, L, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream)
              : run_layered_unpack_range(lout, e->ws, e->ws_bytes, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms,
                                         e->kstream);
@@ -326,7 +388,7 @@ static int prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs
     }
     CK(cudaEventRecord(t->dma_end, e->cstream));
     // final status (the pad check of the unpack kernels can still flip it) and the checkpoint event
-    CK(cudaMemcpyAsync(&t->h_result->status, &((WsHead*)e->ws)->status, sizeof(int32_t), cudaMemcpyDeviceToHost, e->kstream));
+    CK(post_status(t->h_result, &((WsHead*)e->ws)->status, e->kstream));
     CK(cudaEventRecord(t->done, e->kstream));
     CK(cudaStreamWaitEvent(consumer, t->done, 0));
     *ticket = t;
@@ -410,7 +472,7 @@ int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t tot
         if (k >= S) CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));  // staging[b] drained by DMA k-S
         CK(launch_pkg_header(L, cap, stream_id, k, count, e->staging[b], e->d_result, e->kstream));
         if ((rc = run_pack_range(set, L, e->staging[b] + BS_PKG_HEADER, lo, hi, e->opts, e->sms, e->kstream))) return rc;
-        if (k == 0) CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
+        if (k == 0) CK(post_result(t->h_result, e->d_result, e->kstream));
         CK(cudaEventRecord(e->ev_k[b], e->kstream));
         CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));
         if (k == 0) CK(cudaEventRecord(t->dma_begin, e->cstream));
@@ -475,7 +537,7 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
                                    e->kstream)))
         return rc;
     CK(launch_pkg_check(L, e->pkg_tab, BS_PKG_HEADER, n_slots, stream_id, e->d_result, e->kstream));
-    CK(cudaMemcpyAsync(t->h_result, e->d_result, sizeof(bs_result), cudaMemcpyDeviceToHost, e->kstream));
+    CK(post_result(t->h_result, e->d_result, e->kstream));
     if ((rc = run_unpack_range(out, L, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream))) return rc;
     std::vector<PkgItem> by_slot(plan.items.begin() + plan.n_header, plan.items.end());
     std::sort(by_slot.begin(), by_slot.end(), [](const PkgItem& a, const PkgItem& b) { return a.slot < b.slot; });
@@ -493,7 +555,7 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
         ++k;
     }
     CK(cudaEventRecord(t->dma_end, e->cstream));
-    CK(cudaMemcpyAsync(&t->h_result->status, &((WsHead*)e->ws)->status, sizeof(int32_t), cudaMemcpyDeviceToHost, e->kstream));
+    CK(post_status(t->h_result, &((WsHead*)e->ws)->status, e->kstream));
     CK(cudaEventRecord(t->done, e->kstream));
     CK(cudaStreamWaitEvent(consumer, t->done, 0));
     *ticket = t;
@@ -785,7 +847,7 @@ int bs_ticket_destroy(bs_ticket* t)
     cudaEventDestroy(t->dma_begin);
     cudaEventDestroy(t->dma_end);
     cudaEventDestroy(t->done);
-    cudaFreeHost(t->h_result);
+    result_slot_put(t->h_result);
     delete t;
     return BS_OK;
 }
