@@ -491,7 +491,7 @@ def run_mine(args):
     # package by package; the size limit decides how many launches the bytes are spread over ----
     if not v2 and not args.no_packages:
         pk = {}
-        for cap_mb in (256, 4):
+        for cap_mb in (256, 4, 1):
             cap = cap_mb << 20
             n_pk = bs.package_count(hb, total, cap)
             slot_bytes = 64 + cap

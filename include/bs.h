@@ -343,7 +343,11 @@ enum { BS_PKG_HEADER = 64 };
 uint64_t bs_package_count(uint64_t header_bytes, uint64_t total_bytes, uint64_t cap);
 /* stream range [*lo, *hi) of package `index`; BS_ERR_ARG for an invalid cut or index */
 int bs_package_range(uint64_t header_bytes, uint64_t total_bytes, uint64_t cap, uint64_t index, uint64_t *lo, uint64_t *hi);
-/* workspace for bs_package_emit / bs_package_unpack: bs_workspace_bytes + room for the assembled header region */
+/* workspace for bs_package_emit / bs_package_unpack: bs_workspace_bytes + room for the assembled header region and for
+ * the slot table of the one-launch path.  (bs_package_emit also accepts a plain bs_workspace_bytes workspace, and
+ * bs_package_unpack one with room for the header region only; the slot table is then a stream-ordered allocation.)
+ * Limits that are a multiple of the work tile (bs_opts.tile_bytes, 16 KiB by default) cost a fixed number of launches
+ * whatever the number of packages; any other multiple of 16 is served package by package. */
 uint64_t bs_package_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint64_t stream_capacity);
 
 /* Serialize `set` straight into packages in DEVICE slots: package k -> d_slots + slot(k)*slot_bytes with

@@ -146,6 +146,49 @@ int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_sr
     return BS_OK;
 }
 
+// the whole stream <-> package slots in one launch each (bs.h "packages"; PkgMap in bs_internal.cuh)
+int run_pack_packages(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, const bs_opts& o, int sms, cudaStream_t stream)
+{
+    MoveParams mp;
+    memset(&mp, 0, sizeof(mp));
+    mp.ws = L;
+    mp.tensors = set->tensors;
+    mp.qn = set->qn;
+    mp.dim = set->dim;
+    mp.addr = set->addr;
+    mp.lo = 0;
+    mp.hi = UINT64_MAX;
+    mp.tile_bytes = o.tile_bytes;
+    mp.tune = o.reserved[0];
+    mp.pkg = pm;
+    cudaError_t e = launch_move(false, mp, o, sms, stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return BS_OK;
+}
+
+// payload only: the header region was gathered and parsed before (header = nullptr: no descriptor rebuild here)
+int run_unpack_packages(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t header_bytes, uint32_t flags,
+                        const bs_opts& o, int sms, cudaStream_t stream)
+{
+    MoveParams mp;
+    memset(&mp, 0, sizeof(mp));
+    mp.ws = L;
+    mp.tensors = out->tensors;
+    mp.qn = out->qn;
+    mp.dim = out->dim;
+    mp.addr = out->addr;
+    mp.lo = 0;
+    mp.hi = UINT64_MAX;
+    mp.tile_bytes = o.tile_bytes;
+    mp.tune = o.reserved[0];
+    mp.flags = flags;
+    mp.pkg = pm;
+    (void)header_bytes;
+    cudaError_t e = launch_move(true, mp, o, sms, stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return BS_OK;
+}
+
 }  // namespace bs
 
 using namespace bs;

@@ -121,6 +121,17 @@ struct LayeredView {
     const LayerPos* lpos;          // [T+1]
 };
 
+// ---- self-contained packages (bs.h "packages"): the stream is not one buffer but lies cut into slots -------
+// cap != 0: stream byte s lives at base + slot(k)*slot_bytes + 64 + (s - lo_k), k = its package under the cut of `cap`,
+// slot(k) = slot_of[k] (device table) or k.  The kernels then ignore MoveParams.stream / lo (lo must be 0).  Every
+// work tile lies inside one package because cap is a multiple of the tile size and the payload is cut from its start.
+struct PkgMap {
+    uint64_t cap;
+    uint64_t slot_bytes;
+    unsigned char* base;
+    const uint32_t* slot_of;
+};
+
 // ---- data movement (S3, S5 / S7): stream bytes [lo,hi) <-> blocks ------------------------------------------
 struct MoveParams {
     WsLayout ws;
@@ -136,7 +147,25 @@ struct MoveParams {
     uint32_t flags;
     uint32_t tune;                // bs_opts.reserved[0]: experiment switches of the TMA variant
     LayeredView lay;              // lay.on != 0: qn / dim are the structure block table, header is wire format v2
+    PkgMap pkg;                   // pkg.cap != 0: the stream side is a set of package slots
 };
+
+// where stream byte s lives (valid for a run of bytes that does not leave s's package; hb = header_bytes)
+__device__ __forceinline__ unsigned char* stream_at(const MoveParams& p, uint64_t hb, uint64_t s)
+{
+    if (p.pkg.cap == 0) return p.stream + (s - p.lo);
+    uint64_t k, within;
+    if (s < hb) {
+        k = s / p.pkg.cap;
+        within = s - k * p.pkg.cap;
+    } else {
+        const uint64_t x = s - hb, j = x / p.pkg.cap;
+        k = (hb + p.pkg.cap - 1) / p.pkg.cap + j;
+        within = x - j * p.pkg.cap;
+    }
+    const uint64_t slot = p.pkg.slot_of ? (uint64_t)__ldg(p.pkg.slot_of + k) : k;
+    return p.pkg.base + slot * p.pkg.slot_bytes + 64 + within;
+}
 
 cudaError_t launch_move(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream);
 cudaError_t launch_move_tma(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream);

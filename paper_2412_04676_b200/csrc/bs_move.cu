@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
 #pragma unroll
                 for (int k = 0; k < UPT; ++k) {
                     const uint64_t s = lo + (h * kTileUnits + (uint64_t)k * kThreads + tid) * 16;
-                    if (s < hend) st_stream16(p.stream + (s - lo), header_unit_any(p, s >> 4, T, B, hb, P));
+                    if (s < hend) st_stream16(stream_at(p, hb, s), header_unit_any(p, s >> 4, T, B, hb, P));
                 }
             }
             continue;
@@ -96,6 +96,8 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
         uint32_t jhi = __ldg(p.ws.tile_first + g1);  // tile_first[ng] == B
         if (jhi >= B) jhi = B - 1;
 
+        const uint64_t tfirst = tbase > plo ? tbase : plo;  // first payload byte of the tile inside [lo, hi)
+        unsigned char* const tile_ptr = stream_at(p, hb, hb + tfirst) - (tfirst - tbase);  // where payload byte tbase would lie
         uint64_t src[UPT];   // pack: block address of the unit; unpack: destination address
         uint32_t kind[UPT];  // 0 skip, 1 full 16 B aligned, 2 full 16 B as 2x8, 3 tail 8 B (+ 8 B pad)
         uint64_t soff[UPT];
@@ -133,12 +135,12 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
             }
 #pragma unroll
             for (int k = 0; k < UPT; ++k)
-                if (kind[k]) st_stream16(p.stream + (hb + soff[k] - lo), v[k]);
+                if (kind[k]) st_stream16(tile_ptr + (soff[k] - tbase), v[k]);
         } else {
             uint4 v[UPT];
 #pragma unroll
             for (int k = 0; k < UPT; ++k)
-                if (kind[k]) v[k] = ld_stream16(p.stream + (hb + soff[k] - lo));
+                if (kind[k]) v[k] = ld_stream16(tile_ptr + (soff[k] - tbase));
 #pragma unroll
             for (int k = 0; k < UPT; ++k) {
                 if (kind[k] == 1) st_stream16(reinterpret_cast<void*>(src[k]), v[k]);

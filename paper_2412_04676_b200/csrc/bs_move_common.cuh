@@ -206,7 +206,7 @@ __device__ __forceinline__ void write_header_warp(const MoveParams& p, uint32_t 
         for (uint64_t i = hw * 32 + lane; i < n_head + n_slack; i += n_hw * 32) {
             const uint64_t u = i < n_head ? i : rec_end / 16 + (i - n_head);
             const uint64_t s = u * 16;
-            if (s >= lo && s < hend) __stcs(reinterpret_cast<uint4*>(p.stream + (s - lo)), header_unit(p, u, T, B, hb, P));
+            if (s >= lo && s < hend) __stcs(reinterpret_cast<uint4*>(stream_at(p, hb, s)), header_unit(p, u, T, B, hb, P));
         }
     }
     if (B == 0 || hend <= rec0 || lo >= rec_end) return;
@@ -240,9 +240,9 @@ __device__ __forceinline__ void write_header_warp(const MoveParams& p, uint32_t 
                 const uint4 v0 = make_uint4((uint32_t)q0[k].x, (uint32_t)q0[k].y, (uint32_t)q1[k].x, (uint32_t)q1[k].y);
                 const uint4 v1 = make_uint4((uint32_t)q2[k].x, (uint32_t)q2[k].y, d0[k], d1[k]);
                 const uint4 v2 = make_uint4(d2[k], t, (uint32_t)off[k], (uint32_t)(off[k] >> 32));
-                if (s >= lo && s < hend) __stcs(reinterpret_cast<uint4*>(p.stream + (s - lo)), v0);
-                if (s + 16 >= lo && s + 16 < hend) __stcs(reinterpret_cast<uint4*>(p.stream + (s + 16 - lo)), v1);
-                if (s + 32 >= lo && s + 32 < hend) __stcs(reinterpret_cast<uint4*>(p.stream + (s + 32 - lo)), v2);
+                if (s >= lo && s < hend) __stcs(reinterpret_cast<uint4*>(stream_at(p, hb, s)), v0);
+                if (s + 16 >= lo && s + 16 < hend) __stcs(reinterpret_cast<uint4*>(stream_at(p, hb, s + 16)), v1);
+                if (s + 32 >= lo && s + 32 < hend) __stcs(reinterpret_cast<uint4*>(stream_at(p, hb, s + 32)), v2);
             }
         }
     }
@@ -255,7 +255,7 @@ __device__ __forceinline__ void write_header_warp_v2(const MoveParams& p, uint32
     if (lo >= hend) return;
     const uint64_t u0 = lo / 16, n = (hend - lo) / 16;
     for (uint64_t i = hw * 32 + lane; i < n; i += n_hw * 32)
-        __stcs(reinterpret_cast<uint4*>(p.stream + i * 16), header_unit_v2(p, u0 + i, T, hb, P));
+        __stcs(reinterpret_cast<uint4*>(stream_at(p, hb, lo + i * 16)), header_unit_v2(p, u0 + i, T, hb, P));
 }
 
 // S7 (descriptor part): records [0, T+B) of p.header -> the out descriptor arrays, 128 records per step

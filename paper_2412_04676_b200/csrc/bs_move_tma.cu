@@ -351,7 +351,7 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
             if (UNPACK) {
                 if (lane == 0) {
                     mbar_arrive_expect_tx(bar, (uint32_t)(thi - tlo));
-                    bulk_g2s_x(sbase + (uint32_t)(tlo - tbase), p.stream + (hb + tlo - lo), (uint32_t)(thi - tlo), bar, hints);
+                    bulk_g2s_x(sbase + (uint32_t)(tlo - tbase), stream_at(p, hb, hb + tlo), (uint32_t)(thi - tlo), bar, hints);
                 }
             } else {
                 // pass 1: bytes the bulk copies will deliver; tails and 8-byte-aligned blocks go through cp.async
@@ -394,7 +394,7 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
                 if (lane == 0) {
                     mbar_wait(bar, parity);
                     fence_proxy_async();  // the cp.async tails were written through the generic proxy
-                    bulk_s2g_x(p.stream + (hb + tlo - lo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo), hints);
+                    bulk_s2g_x(stream_at(p, hb, hb + tlo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo), hints);
                 }
             } else {
                 int* status = const_cast<int*>(&head->status);

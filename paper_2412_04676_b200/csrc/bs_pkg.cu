@@ -7,6 +7,11 @@
 //   emit   = scan | per package: pkg_header_kernel (64 bytes: where am I, which block do I start in) + pack [lo,hi)
 //   unpack = gather the header-region packages | parse/validate scan | pkg_check_kernel (every package against the
 //            offset table) | descriptor rebuild | per payload package, in the order the slots lie: unpack [lo,hi)
+// and when the size limit is a multiple of the work tile (16 KiB by default) no tile straddles a package, so the move
+// kernels take a PkgMap (stream byte -> slot address, bs_internal.cuh) and the whole set costs a fixed number of
+// launches however many packages the limit makes:
+//   emit   = scan | pkg_headers_kernel (all headers) | pack (whole stream -> slots)
+//   unpack = pkg_index_kernel | pkg_gather_header_kernel | scan | pkg_check_kernel | rebuild | unpack (slots -> blocks)
 // The host reads package headers only to plan these launches (which slot holds which range); see bs.h for who checks
 // what.
 #include <string.h>
@@ -30,6 +35,9 @@ int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t n
                          int sms, cudaStream_t stream);
 int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header, uint64_t lo,
                      uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream);
+int run_pack_packages(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, const bs_opts& o, int sms, cudaStream_t stream);
+int run_unpack_packages(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t header_bytes, uint32_t flags,
+                        const bs_opts& o, int sms, cudaStream_t stream);
 
 namespace {
 
@@ -52,11 +60,10 @@ __device__ __forceinline__ void pkg_fail(WsHead* head, bs_result* result, int co
     if (result != nullptr) result->status = head->status;
 }
 
-// one thread: the 64-byte header of package k -> dst
-__global__ void pkg_header_kernel(WsLayout ws, uint64_t cap, uint64_t stream_id, uint64_t k, uint64_t expect_count,
-                                  unsigned char* dst, bs_result* result)
+// the 64-byte header of package k -> dst
+__device__ __forceinline__ void pkg_write_header(const WsLayout& ws, uint64_t cap, uint64_t stream_id, uint64_t k,
+                                                 uint64_t expect_count, unsigned char* dst, bs_result* result)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
     WsHead* head = ws.head;
     if (head->status != 0) return;  // deferred error: nothing is written
     const uint64_t hb = head->header_bytes, total = hb + head->payload_bytes;
@@ -80,6 +87,48 @@ __global__ void pkg_header_kernel(WsLayout ws, uint64_t cap, uint64_t stream_id,
     const uint64_t nb = hi - lo;
     o[3] = make_uint4((uint32_t)nb, (uint32_t)(nb >> 32), (uint32_t)intra, (uint32_t)(intra >> 32));
     if (k == 0 && result != nullptr) result->reserved[0] = (uint32_t)count;
+}
+
+// one thread: package k -> dst
+__global__ void pkg_header_kernel(WsLayout ws, uint64_t cap, uint64_t stream_id, uint64_t k, uint64_t expect_count,
+                                  unsigned char* dst, bs_result* result)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    pkg_write_header(ws, cap, stream_id, k, expect_count, dst, result);
+}
+
+// one thread per package: every header of the cut -> its slot (slot_of: device table index -> slot, or identity)
+__global__ void pkg_headers_kernel(WsLayout ws, uint64_t cap, uint64_t stream_id, uint64_t count, unsigned char* base,
+                                   uint64_t slot_bytes, const uint32_t* slot_of, bs_result* result)
+{
+    const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    const uint64_t slot = slot_of ? (uint64_t)slot_of[k] : k;
+    pkg_write_header(ws, cap, stream_id, k, count, base + slot * slot_bytes, result);
+}
+
+// one thread per slot: slot_of[index] = slot for the packages of this stream (the host plan proved the indices unique)
+__global__ void pkg_index_kernel(const unsigned char* base, uint64_t stride, uint64_t n_slots, uint64_t stream_id,
+                                 uint32_t* slot_of, uint64_t count)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n_slots) return;
+    const uint4* h = reinterpret_cast<const uint4*>(base + s * stride);
+    const uint4 a = h[0], b = h[1];
+    if (a.x != 0x4b505342u || a.y != 0x31303047u || (((uint64_t)b.w << 32) | b.z) != stream_id) return;
+    if (a.w < count) slot_of[a.w] = (uint32_t)s;
+}
+
+// the header region [0, hb), stored continuously (L126): 16-byte units out of the header-region packages
+__global__ void pkg_gather_header_kernel(const unsigned char* base, uint64_t slot_bytes, const uint32_t* slot_of,
+                                         uint64_t cap, uint64_t hb, unsigned char* dst)
+{
+    const uint64_t n = hb / 16;
+    for (uint64_t u = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; u < n; u += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t s = u * 16, k = s / cap;
+        const uint4 v = *reinterpret_cast<const uint4*>(base + (uint64_t)slot_of[k] * slot_bytes + BS_PKG_HEADER + (s - k * cap));
+        *reinterpret_cast<uint4*>(dst + s) = v;
+    }
 }
 
 // one thread per slot: the package header at base + s*stride against the parsed stream (after the DESER scan)
@@ -112,6 +161,9 @@ __global__ void pkg_check_kernel(WsLayout ws, const unsigned char* base, uint64_
     }
     if (!ok) pkg_fail(head, result, BS_ERR_CORRUPT);
 }
+
+// bytes per work tile of the move kernels for these options (the TMA presets use 16 KiB tiles)
+uint32_t work_tile_bytes(const bs_opts& o) { return o.tile_bytes ? o.tile_bytes : kGranule; }
 
 uint32_t rd32(const unsigned char* p) { uint32_t v; memcpy(&v, p, 4); return v; }
 uint64_t rd64(const unsigned char* p) { uint64_t v; memcpy(&v, p, 8); return v; }
@@ -181,6 +233,22 @@ int pkg_plan(const unsigned char* h_hdrs, uint64_t stride, uint64_t n_slots, uin
     return BS_OK;
 }
 
+// The size limit `cap` whose cut (bs.h) these packages are, if it is a multiple of `tile`; 0 if they are cut otherwise.
+uint64_t plan_uniform_cap(const PkgPlan& plan, uint32_t tile)
+{
+    const uint64_t n = plan.items.size(), nh = plan.n_header;
+    uint64_t cap;
+    if (nh > 1) cap = plan.items[0].nbytes;
+    else if (n - nh > 1) cap = plan.items[nh].nbytes;
+    else cap = align_up(std::max(plan.hb, plan.total - plan.hb), 65536);  // one package per region: any limit this large
+    if (cap == 0 || cap % tile != 0 || pkg_count(plan.hb, plan.total, cap) != n) return 0;
+    for (uint64_t k = 0; k < n; ++k) {
+        uint64_t lo = 0, hi = 0;
+        if (!pkg_range(plan.hb, plan.total, cap, k, &lo, &hi) || lo != plan.items[k].lo || hi - lo != plan.items[k].nbytes) return 0;
+    }
+    return cap;
+}
+
 }  // namespace bs
 
 using namespace bs;
@@ -208,7 +276,10 @@ int bs_package_range(uint64_t header_bytes, uint64_t total_bytes, uint64_t cap, 
 
 uint64_t bs_package_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint64_t stream_capacity)
 {
-    return bs_workspace_bytes(n_tensors, n_blocks, stream_capacity) + align_up(bs_header_bytes(n_tensors, n_blocks), 256);
+    // v1 workspace | slot table of the one-launch path (limits >= 16 KiB: at most one entry per 16 KiB) | header region
+    const uint64_t hb = bs_header_bytes(n_tensors, n_blocks);
+    return bs_workspace_bytes(n_tensors, n_blocks, stream_capacity) + align_up(4 * (stream_capacity / kGranule + hb / kGranule + 4), 256) +
+           256 + align_up(hb, 256);
 }
 
 int bs_package_emit(const bs_set_desc* set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id, void* d_slots,
@@ -244,7 +315,31 @@ int bs_package_emit(const bs_set_desc* set, uint64_t total_bytes, uint64_t cap, 
         }
     }
     if ((rc = run_serialize_scan(set, L, UINT64_MAX, total_bytes, d_result, sms, stream))) return rc;
-    for (uint64_t k = 0; k < count; ++k) {
+    if (cap % work_tile_bytes(o) == 0) {
+        // every work tile lies inside one package: ONE launch writes all package headers, ONE moves the whole stream
+        // into the slots, however many packages the size limit makes
+        uint32_t* d_tab = nullptr;
+        bool tab_owned = false;
+        if (h_slot_of != nullptr) {  // the slot table: the tail of a bs_package_workspace_bytes workspace, else a stream-ordered allocation
+            const uint64_t tab = align_up(count * sizeof(uint32_t), 256);
+            if (ws_bytes >= bs_workspace_bytes(set->n_tensors, set->n_blocks, total_bytes) + tab) {
+                d_tab = (uint32_t*)((unsigned char*)d_ws + ((ws_bytes - tab) & ~255ull));
+            } else {
+                CK(cudaMallocAsync((void**)&d_tab, count * sizeof(uint32_t), stream));
+                tab_owned = true;
+            }
+            CK(cudaMemcpyAsync(d_tab, h_slot_of, count * sizeof(uint32_t), cudaMemcpyHostToDevice, stream));
+        }
+        pkg_headers_kernel<<<(unsigned)((count + 127) / 128), 128, 0, stream>>>(L, cap, stream_id, count, (unsigned char*)d_slots,
+                                                                                 slot_bytes, d_tab, d_result);
+        CK(cudaGetLastError());
+        PkgMap pm;
+        pm.cap = cap; pm.slot_bytes = slot_bytes; pm.base = (unsigned char*)d_slots; pm.slot_of = d_tab;
+        rc = run_pack_packages(set, L, pm, o, sms, stream);
+        if (tab_owned) CK(cudaFreeAsync(d_tab, stream));
+        return rc;
+    }
+    for (uint64_t k = 0; k < count; ++k) {  // any other limit: package by package
         uint64_t lo = 0, hi = 0;
         pkg_range(hb, total_bytes, cap, k, &lo, &hi);
         unsigned char* slot = (unsigned char*)d_slots + (h_slot_of ? (uint64_t)h_slot_of[k] : k) * slot_bytes;
@@ -287,6 +382,41 @@ int bs_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t n_slots
     if (plan.hb > hdr_cap) return BS_ERR_CAPACITY;
 
     const unsigned char* slots = (const unsigned char*)d_slots;
+    const uint64_t cut = plan_uniform_cap(plan, work_tile_bytes(o));
+    if (cut != 0) {
+        // the packages are the cut of one size limit whose tiles never straddle a package: the slot table is built on
+        // the device, the header region gathered, and ONE launch unpacks every payload package wherever it lies
+        const uint64_t count = plan.items.size();
+        uint32_t* d_tab = nullptr;
+        bool tab_owned = false;
+        const uint64_t tab = align_up(count * sizeof(uint32_t), 256);
+        if (w1 >= bs_workspace_bytes(out->n_tensors, out->n_blocks, plan.total) + tab) {  // bs_package_workspace_bytes has room
+            const uint64_t w2 = (w1 - tab) & ~255ull;  // the v1 part shrinks, the table sits between it and the header scratch
+            if (!ws_layout(d_ws, w2, out->n_blocks, &L)) return BS_ERR_CAPACITY;
+            d_tab = (uint32_t*)((unsigned char*)d_ws + w2);
+        } else {
+            CK(cudaMallocAsync((void**)&d_tab, count * sizeof(uint32_t), stream));
+            tab_owned = true;
+        }
+        pkg_index_kernel<<<(unsigned)((n_slots + 127) / 128), 128, 0, stream>>>(slots, slot_bytes, n_slots, stream_id, d_tab, count);
+        CK(cudaGetLastError());
+        {
+            const uint64_t units = plan.hb / 16;
+            unsigned grid = (unsigned)std::min<uint64_t>((units + 255) / 256, (uint64_t)sms * 8);
+            pkg_gather_header_kernel<<<grid ? grid : 1, 256, 0, stream>>>(slots, slot_bytes, d_tab, cut, plan.hb, d_header);
+            CK(cudaGetLastError());
+        }
+        if ((rc = run_deserialize_scan(d_header, nullptr, plan.total, out, d_pool, pool_bytes, flags, L, d_result, sms, stream))) return rc;
+        CK(launch_pkg_check(L, d_slots, slot_bytes, n_slots, stream_id, d_result, stream));
+        if ((rc = run_unpack_range(out, L, d_header, d_header, 0, 0, flags, o, sms, stream))) return rc;  // descriptor rebuild
+        PkgMap pm;
+        pm.cap = cut; pm.slot_bytes = slot_bytes; pm.base = const_cast<unsigned char*>(slots); pm.slot_of = d_tab;
+        if ((rc = run_unpack_packages(out, L, pm, plan.hb, flags | kFlagCheckPad, o, sms, stream))) return rc;
+        if (d_result != nullptr)
+            CK(cudaMemcpyAsync(&d_result->status, &L.head->status, sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
+        if (tab_owned) CK(cudaFreeAsync(d_tab, stream));
+        return BS_OK;
+    }
     for (uint32_t k = 0; k < plan.n_header; ++k) {  // the header region, stored continuously (L126)
         const PkgItem& it = plan.items[k];
         CK(cudaMemcpyAsync(d_header + it.lo, slots + it.slot * slot_bytes + BS_PKG_HEADER, it.nbytes, cudaMemcpyDeviceToDevice, stream));

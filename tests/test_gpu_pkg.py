@@ -42,9 +42,10 @@ def upload_raw(tensors, qn, dim, pool, offs):
     return d_pool, bs.DeviceSet.from_host(tensors, qn, dim, addr, DEV)
 
 
-def emit_on_gpu(dset, total, cap, slot_bytes, n_slots, slot_of=None, opts=None, total_arg=None):
+def emit_on_gpu(dset, total, cap, slot_bytes, n_slots, slot_of=None, opts=None, total_arg=None, pkg_ws=True):
+    """pkg_ws=False: a plain bs_workspace_bytes workspace (the slot table then comes from a stream-ordered allocation)."""
     slots = torch.full((n_slots * slot_bytes,), POISON, dtype=torch.uint8, device=DEV)
-    ws = bs.Workspace(dset.n_tensors, dset.n_blocks, max(total, 1 << 16), DEV)
+    ws = bs.Workspace(dset.n_tensors, dset.n_blocks, max(total, 1 << 16), DEV, packages=pkg_ws)
     bs.package_emit(dset.desc, total if total_arg is None else total_arg, cap, SID, slots.data_ptr(), slot_bytes, n_slots,
                     slot_of, ws.ptr, ws.nbytes, ws.result_ptr, opts, bs.current_stream())
     return slots, ws.read_result()
@@ -129,13 +130,16 @@ def oracle_slots(want, cap, slot_bytes, seed, extra=2, foreign=True):
     return slots, perm[:n], n
 
 
-def unpack_on_gpu(slots_np, bset, want, flags=bs.LAYOUT_POOL, opts=None, sid=SID):
+def unpack_on_gpu(slots_np, bset, want, flags=bs.LAYOUT_POOL, opts=None, sid=SID, pkg_ws=True):
     need = oracle.pool_bytes(want)
     n_slots, slot_bytes = slots_np.shape
     d_slots = torch.from_numpy(slots_np.copy()).to(DEV)
     out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
     pool = torch.full((max(need, 256),), 0xEE, dtype=torch.uint8, device=DEV)
     ws = bs.Workspace(bset.n_tensors, bset.n_blocks, max(len(want), 1 << 16), DEV, packages=True)
+    if not pkg_ws:   # the smallest workspace the call accepts: v1 workspace + the header region, no room for the slot table
+        ws.nbytes = bs.workspace_bytes(bset.n_tensors, bset.n_blocks, max(len(want), 1 << 16)) + \
+            (bs.header_bytes(bset.n_tensors, bset.n_blocks) + 255) // 256 * 256
     bs.package_unpack(d_slots.data_ptr(), slot_bytes, n_slots, sid, out.desc, pool.data_ptr(), need, flags, ws.ptr, ws.nbytes,
                       ws.result_ptr, opts, bs.current_stream())
     return out, pool, ws.read_result(), need
@@ -154,6 +158,27 @@ def test_unpack_from_shuffled_oracle_packages(cfg, kw, cap, variant):
     assert (pool.cpu().numpy()[:need] == ref["pool"][:need]).all(), "blocks differ from the oracle's"
     h = out.to_host()
     assert h["tensors"].tobytes() == bset.tensors.tobytes() and (h["qn"] == bset.qn).all() and (h["dim"] == bset.dim).all()
+
+
+@pytest.mark.parametrize("tile,cap", [(32768, 65536), (32768, 49152), (65536, 1 << 20), (49152, 49152 * 3)])
+@pytest.mark.parametrize("variant", [bs.VARIANT_TMA, bs.VARIANT_LDG])
+def test_the_stream_does_not_depend_on_how_packages_map_onto_work_tiles(tile, cap, variant):
+    """P6 for packages: limits that are a multiple of the work tile take the one-launch path, the others go package by
+    package; both must give the oracle's bytes."""
+    bset = W.make_config("2", n_ops=39)
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    ref = oracle.deserialize(want)
+    hb = bs.header_bytes(bset.n_tensors, bset.n_blocks)
+    n = pkg.count(hb, len(want), cap)
+    slot_of = np.random.default_rng(1).permutation(n)
+    opts = dict(variant=variant, tile_bytes=tile, stages=3, warps=1)
+    slots, res = emit_on_gpu(up.dset, len(want), cap, 64 + cap, n, slot_of, opts=opts, pkg_ws=variant == bs.VARIANT_TMA)
+    got = slots.cpu().numpy().reshape(n, 64 + cap)
+    assert res["status"] == bs.OK
+    assert (got == pkg.emit_slots(want, cap, SID, 64 + cap, slot_of=slot_of, poison=POISON)).all()
+    out, pool, res2, need = unpack_on_gpu(got, bset, want, opts=opts, pkg_ws=variant == bs.VARIANT_TMA)
+    assert res2["status"] == bs.OK and (pool.cpu().numpy()[:need] == ref["pool"][:need]).all()
 
 
 def test_emit_then_unpack_on_the_device_is_the_identity():
