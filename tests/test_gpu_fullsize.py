@@ -203,3 +203,120 @@ def test_full_size_layered_v2(cfg):
     bs.layered_serialize(out.desc, again.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, None, cs)
     assert ws.read_result()["status"] == bs.OK
     assert torch.equal(again, stream[:total]), "serialize(deserialize(S)) != S"
+
+
+def check_blocks_against_generator(bset, host_desc, opool, tensors):
+    """Sampled tensors' blocks in a BS_LAYOUT_POOL pool against values regenerated on the host (never the CUDA path's)."""
+    for t in tensors:
+        b0 = int(bset.tensors["first_block"][t])
+        b1 = b0 + int(bset.tensors["n_blocks"][t])
+        pool, offs = W.fill_pool_host(bset, b0, b1, compact=True)
+        for i in range(b0, b1):
+            n = int(bset.nelems[i])
+            o = int(host_desc["addr"][i]) - opool.data_ptr()
+            got = opool[o: o + 8 * n].cpu().numpy().view(np.uint64)
+            want = pool.view(np.uint64)[int(offs[i - b0]) // 8: int(offs[i - b0]) // 8 + n]
+            assert (got == want).all(), f"block {i} of tensor {t} differs"
+
+
+def test_full_size_packages_config4():
+    """NEXT-2 at full size in the configuration bench.py times: 4 MiB limit (1719 packages), shuffled slots, one launch."""
+    import struct
+    from oracle import pkg
+    bset = W.make_config("4")
+    up = Uploaded(bset, fill="device")
+    hb, total = oracle.serialized_size(bset.n_tensors, bset.dim)
+    cap, sid = 4 << 20, 0xC0FFEE
+    n = pkg.count(hb, total, cap)
+    slot_bytes = 64 + cap
+    slot_of = np.random.default_rng(4).permutation(n)
+    slots = torch.full((n * slot_bytes,), 0x5A, dtype=torch.uint8, device=DEV)
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, total, DEV, packages=True)
+    cs = bs.current_stream()
+    bs.package_emit(up.dset.desc, total, cap, sid, slots.data_ptr(), slot_bytes, n, slot_of, ws.ptr, ws.nbytes, ws.result_ptr,
+                    None, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["n_packages"] == n and res["total_bytes"] == total
+
+    def stream_range(lo, nbytes):
+        """Stream bytes [lo, lo+nbytes) out of the slots, located with the ORACLE's cut."""
+        parts = []
+        nh = -(-hb // cap)
+        while nbytes:
+            k = lo // cap if lo < hb else nh + (lo - hb) // cap
+            plo, phi = pkg.package_range(hb, total, cap, k)
+            take = min(nbytes, phi - lo)
+            base = int(slot_of[k]) * slot_bytes + 64 + (lo - plo)
+            parts.append(slots[base: base + take].cpu().numpy())
+            lo += take
+            nbytes -= take
+        return np.concatenate(parts)
+
+    want_h = oracle.emit_header(bset.tensors, bset.qn, bset.dim)
+    assert (stream_range(0, hb) == want_h).all(), "header region of the packages differs from the oracle's header"
+    for t in sampled_tensors(bset, n=6):
+        first, want, _ = oracle_tensor_payload(bset, t)
+        assert (stream_range(hb + first, len(want)) == want).all(), f"tensor {t}: payload in the packages differs"
+    # package headers: the oracle's cut; first_block by numpy.searchsorted over the oracle's offsets
+    offs = np.frombuffer(want_h[64 + 32 * bset.n_tensors: 64 + 32 * bset.n_tensors + 48 * bset.n_blocks].tobytes(),
+                         dtype=np.dtype([("x", "V40"), ("off", "<u8")]))["off"]
+    for k in [0, 1, n - 1] + [int(x) for x in np.random.default_rng(5).integers(0, n, 24)]:
+        lo, hi = pkg.package_range(hb, total, cap, k)
+        raw = slots[int(slot_of[k]) * slot_bytes: int(slot_of[k]) * slot_bytes + 64].cpu().numpy().tobytes()
+        magic, ver, idx, cnt, fb, psid, ptot, plo, pnb, intra = struct.unpack("<8sIIIIQQQQQ", raw)
+        assert (magic, ver, idx, cnt, psid, ptot, plo, pnb) == (b"BSPKG001", 1, k, n, sid, total, lo, hi - lo)
+        if lo < hb:
+            assert fb == 0xFFFFFFFF and intra == 0
+        else:
+            i = int(np.searchsorted(offs, lo - hb, side="right")) - 1
+            assert fb == i and intra == lo - hb - int(offs[i])
+    for k in range(0, n, max(1, n // 40)):   # bytes behind a short package stay untouched
+        lo, hi = pkg.package_range(hb, total, cap, k)
+        tail = slots[int(slot_of[k]) * slot_bytes + 64 + (hi - lo): (int(slot_of[k]) + 1) * slot_bytes]
+        assert bool((tail == 0x5A).all())
+    # and back: one-launch unpack from the shuffled slots
+    need = int(((bset.nelems * 8 + 255) // 256 * 256).sum())
+    out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+    opool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    bs.package_unpack(slots.data_ptr(), slot_bytes, n, sid, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                      ws.result_ptr, None, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["pool_bytes"] == need
+    host = out.to_host()
+    assert host["tensors"].tobytes() == bset.tensors.tobytes() and (host["qn"] == bset.qn).all() and (host["dim"] == bset.dim).all()
+    check_blocks_against_generator(bset, host, opool, sampled_tensors(bset, n=5, seed=3))
+
+
+def test_full_size_queue_config3():
+    """NEXT-3 at full size: the bench's e2e pattern — save a set while the stream saved before it is loaded back."""
+    bset = W.make_config("3")
+    up = Uploaded(bset, fill="device")
+    hb, total = oracle.serialized_size(bset.n_tensors, bset.dim)
+    cs = bs.current_stream()
+    q = bs.Queue(bset.n_tensors, bset.n_blocks, total)                 # defaults: 256 MiB chunks, 2 staging buffers per lane
+    hosts = [torch.empty(total, dtype=torch.uint8, pin_memory=True) for _ in range(2)]
+    for h in hosts:
+        h.fill_(0x5A)
+    need = int(((bset.nelems * 8 + 255) // 256 * 256).sum())
+    out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+    opool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    q.save(0, up.dset.desc, total, hosts[0].data_ptr(), total, cs)
+    q.save(1, up.dset.desc, total, hosts[1].data_ptr(), total, cs)    # runs behind save 0 in the save lane ...
+    q.load(0, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, cs)   # ... while the load lane brings key 0 back
+    for k in (0, 1):
+        st = q.wait(k)
+        assert st["status"] == bs.OK and st["save"]["bytes"] == total
+    torch.cuda.synchronize()
+    want_h = oracle.emit_header(bset.tensors, bset.qn, bset.dim)
+    for h in hosts:
+        assert (h[:hb].numpy() == want_h).all()
+        for t in sampled_tensors(bset, n=4):
+            first, want, _ = oracle_tensor_payload(bset, t)
+            assert (h[hb + first: hb + first + len(want)].numpy() == want).all(), f"tensor {t}: saved payload differs"
+    assert torch.equal(hosts[0], hosts[1])
+    host = out.to_host()
+    assert host["tensors"].tobytes() == bset.tensors.tobytes() and (host["dim"] == bset.dim).all()
+    check_blocks_against_generator(bset, host, opool, sampled_tensors(bset, n=5, seed=3))
+    st = q.stats()
+    assert st["host_bytes_live"] == 2 * total and st["device_bytes"] < 2 * (2 * (256 << 20)) + (256 << 20)
+    q.destroy()
