@@ -324,3 +324,44 @@ def test_scatter_extent_mismatch_is_an_argument_error():
     bs.deserialize(st.data_ptr(), len(want), out.desc, 0, 0, bs.SCATTER_TO_ADDR, ws.ptr, ws.nbytes, ws.result_ptr, None,
                    bs.current_stream())
     assert ws.read_result()["status"] == bs.ERR_ARG and (dst == 0xEE).all()
+
+
+def test_calls_are_capturable_in_a_cuda_graph():
+    """The calls only enqueue work (no host synchronisation, no allocation), so a launch-bound loop over small sets can be
+    captured once and replayed: the replay must give the oracle's bytes for whatever the blocks hold at replay time."""
+    bset = W.make_config("2", n_ops=26)
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    total = len(want)
+    need = oracle.pool_bytes(want)
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, total, DEV)
+    stream = torch.full((total,), 0xCD, dtype=torch.uint8, device=DEV)
+    out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+    pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+
+    def step(s):
+        bs.serialize(up.dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, None, s)
+        bs.deserialize(stream.data_ptr(), total, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                       ws.result_ptr, None, s)
+
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step(side.cuda_stream)                       # warm-up outside the capture (one-time kernel attributes)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        step(side.cuda_stream)
+    # new values in the same blocks, then replay: the graph holds launches, not data
+    up.pool.copy_(torch.roll(up.pool, 8))
+    rolled = np.roll(up.host_pool.view(np.uint8), 8)
+    want2 = oracle.serialize(bset.tensors, bset.qn, bset.dim,
+                             (np.uint64(rolled.ctypes.data) + up.host_offs.astype(np.uint64)).astype(np.uint64))
+    stream.fill_(0xCD)
+    pool.fill_(0xEE)
+    g.replay()
+    torch.cuda.synchronize()
+    assert ws.read_result()["status"] == bs.OK
+    assert (stream.cpu().numpy() == want2).all(), "graph replay: stream differs from the oracle's"
+    assert (pool.cpu().numpy()[:need] == oracle.deserialize(want2)["pool"][:need]).all()
