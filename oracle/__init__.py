@@ -3,6 +3,7 @@
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import this
 package.  It imports nothing from paper_2412_04676_b200.
 """
+from . import bs_oracle_dtype as dt  # noqa: F401  (element types other than fp64)
 from . import bs_oracle_pkg as pkg  # noqa: F401  (self-contained packages)
 from . import bs_oracle_v2 as v2  # noqa: F401  (wire format v2: structure-shared layers)
 from .bs_oracle_queue import QueueModel  # noqa: F401  (save / load queue: the sequential definition)
