@@ -32,13 +32,13 @@
  * Wire format v1 (little-endian, no implicit padding):
  *   stream  := fixed_header(64) | tensor_rec[T](32 each) | block_rec[B](48 each) | zeros to a multiple
  *              of 128 | payload(P)
- *   fixed_header: char magic[8]="BSPARSE1"; u32 version=1; u32 endian_tag=0x01020304; u32 dtype=0;
- *                 u32 n_qn=2; u32 max_rank=3; u32 align=16; u64 n_tensors; u64 n_blocks;
+ *   fixed_header: char magic[8]="BSPARSE1"; u32 version=1; u32 endian_tag=0x01020304; u32 dtype (0 f64,
+ *                 1 f32, 2 c64, 3 c128: element size e = 8, 4, 8, 16); u32 n_qn=2; u32 max_rank=3; u32 align=16; u64 n_tensors; u64 n_blocks;
  *                 u64 header_bytes; u64 payload_bytes
  *   tensor_rec  : bs_tensor_rec, byte for byte
  *   block_rec   : i32 qn[3][2]; u32 dim[3]; u32 tensor; u64 offset
- *   payload     : block i's 8*prod(dim_i) raw bytes at payload+offset_i, then zeros up to the next
- *                 multiple of 16; offset_i = sum_{j<i} align16(8*prod(dim_j))   (descriptor order)
+ *   payload     : block i's e*prod(dim_i) raw bytes at payload+offset_i, then zeros up to the next
+ *                 multiple of 16; offset_i = sum_{j<i} align16(e*prod(dim_j))   (descriptor order)
  */
 #ifndef BS_H_
 #define BS_H_
@@ -67,7 +67,10 @@ enum {
     BS_ERR_CUDA = -5         /* a CUDA runtime call failed; see bs_last_cuda_error() */
 };
 
-enum { BS_F64 = 0 };
+/* Element type of every block of a set (bs_set_desc.dtype; the header's dtype word).  The path does no arithmetic on the
+ * values: the type only fixes the element size e, nbytes = e * prod(dim).  Wire format v2 (layered
+ * sets) is BS_F64 only. */
+enum { BS_F64 = 0 /* e = 8 */, BS_F32 = 1 /* e = 4 */, BS_C64 = 2 /* e = 8 */, BS_C128 = 3 /* e = 16 */ };
 
 /* bs_deserialize / bs_prefetch_async destination layout */
 enum {
@@ -92,7 +95,7 @@ typedef struct bs_set_desc {
     uint32_t n_tensors;     /* T.  For bs_deserialize / bs_prefetch_async outputs: CAPACITY of tensors[] */
     uint32_t n_blocks;      /* B.  For outputs: CAPACITY of qn / dim / addr */
     uint32_t n_qn;          /* 2: (N, 2Sz) */
-    uint32_t dtype;         /* BS_F64 */
+    uint32_t dtype;         /* BS_F64, BS_F32, BS_C64 or BS_C128; for outputs: written by the call's caller as 0, see bs_result */
     bs_tensor_rec *tensors; /* [T]        */
     int32_t *qn;            /* [B][3][2]  labels per leg; unused legs 0 */
     uint32_t *dim;          /* [B][3]     extents; unused legs 1 */
@@ -110,11 +113,12 @@ typedef struct bs_result {
     int32_t status;         /* BS_OK or BS_ERR_* */
     uint32_t n_tensors;
     uint32_t n_blocks;
-    uint32_t reserved[5];
+    uint32_t reserved[5];   /* [0], [1]: see bs_layered_* / bs_package_emit; [2] = dtype of the stream (deserialize) */
 } bs_result;
 
 typedef struct bs_stream_info_t {
     uint64_t n_tensors, n_blocks, header_bytes, payload_bytes, total_bytes;
+    uint64_t dtype; /* BS_F64 .. BS_C128 */
 } bs_stream_info_t;
 
 /* Launch tuning.  NULL everywhere means defaults.  The stream produced never depends on these

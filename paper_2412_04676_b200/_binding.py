@@ -10,7 +10,7 @@ from . import build as _build
 
 OK, PENDING = 0, 1
 ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_UNSUPPORTED, ERR_CUDA = -1, -2, -3, -4, -5
-F64 = 0
+F64, F32, C64, C128 = 0, 1, 2, 3
 LAYOUT_POOL, SCATTER_TO_ADDR = 0, 1
 VARIANT_DEFAULT, VARIANT_LDG, VARIANT_TMA = 0, 1, 2
 
@@ -59,7 +59,7 @@ class Result(C.Structure):
 
 class StreamInfo(C.Structure):
     _fields_ = [("n_tensors", C.c_uint64), ("n_blocks", C.c_uint64), ("header_bytes", C.c_uint64),
-                ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64)]
+                ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64), ("dtype", C.c_uint64)]
 
 
 class Opts(C.Structure):
@@ -212,8 +212,9 @@ def stream_info(first_64_bytes) -> dict:
     return {k: int(getattr(info, k)) for k, _ in StreamInfo._fields_}
 
 
-def make_desc(n_tensors: int, n_blocks: int, tensors_ptr: int, qn_ptr: int, dim_ptr: int, addr_ptr: int) -> SetDesc:
-    return SetDesc(n_tensors, n_blocks, 2, F64, tensors_ptr, qn_ptr, dim_ptr, addr_ptr)
+def make_desc(n_tensors: int, n_blocks: int, tensors_ptr: int, qn_ptr: int, dim_ptr: int, addr_ptr: int,
+              dtype: int = F64) -> SetDesc:
+    return SetDesc(n_tensors, n_blocks, 2, dtype, tensors_ptr, qn_ptr, dim_ptr, addr_ptr)
 
 
 def serialized_size(desc: SetDesc, ws_ptr: int, ws_bytes: int, stream: int = 0):

@@ -36,7 +36,7 @@ static bool aligned(const void* p, uintptr_t a) { return ((uintptr_t)p & (a - 1)
 static int check_set(const bs_set_desc* s)
 {
     if (s == nullptr) return BS_ERR_ARG;
-    if (s->n_qn != 2 || s->dtype != BS_F64) return BS_ERR_UNSUPPORTED;
+    if (s->n_qn != 2 || s->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
     if (s->n_tensors && (s->tensors == nullptr || !aligned(s->tensors, 16))) return BS_ERR_ARG;
     if (s->n_blocks && (s->qn == nullptr || !aligned(s->qn, 8))) return BS_ERR_ARG;
     if (s->n_blocks && (s->dim == nullptr || !aligned(s->dim, 4))) return BS_ERR_ARG;
@@ -74,6 +74,7 @@ int run_serialize_scan(const bs_set_desc* set, const WsLayout& L, uint64_t capac
     sp.addr = set->addr;
     sp.T = set->n_tensors;
     sp.B = set->n_blocks;
+    sp.dtype = set->dtype;
     e = launch_scan(false, sp, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
@@ -233,7 +234,7 @@ int bs_stream_info(const void* h, bs_stream_info_t* out)
     memcpy(w, s, 32);
     memcpy(q, s + 32, 32);
     if (memcmp(s, "BSPARSE1", 8) != 0) return BS_ERR_CORRUPT;
-    if (w[2] != 1u || w[3] != 0x01020304u || w[4] != 0u || w[5] != 2u || w[6] != 3u || w[7] != 16u) return BS_ERR_CORRUPT;
+    if (w[2] != 1u || w[3] != 0x01020304u || w[4] > (uint32_t)BS_C128 || w[5] != 2u || w[6] != 3u || w[7] != 16u) return BS_ERR_CORRUPT;
     if (q[0] >= (1ull << 32) || q[1] >= (1ull << 32)) return BS_ERR_CORRUPT;
     if (q[2] != bs_header_bytes(q[0], q[1])) return BS_ERR_CORRUPT;
     out->n_tensors = q[0];
@@ -241,6 +242,7 @@ int bs_stream_info(const void* h, bs_stream_info_t* out)
     out->header_bytes = q[2];
     out->payload_bytes = q[3];
     out->total_bytes = q[2] + q[3];
+    out->dtype = w[4];
     return BS_OK;
 }
 

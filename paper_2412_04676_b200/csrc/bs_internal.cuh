@@ -28,8 +28,11 @@ constexpr uint32_t kScanTile = kScanThreads * kScanItems;
 
 struct __align__(16) Blk {
     uint64_t off;   // payload offset (exclusive prefix sum of stored sizes)
-    uint64_t addr;  // device address of the dense block; bit 0 set: nbytes = stored - 8 (odd element count)
+    uint64_t addr;  // device address of the dense block (8-byte aligned); bits 0-1 = c: nbytes = stored - 4*c (zero pad)
 };
+
+// element size of a dtype (bs.h): f64 8, f32 4, c64 8, c128 16
+__host__ __device__ inline uint32_t elem_bytes(uint32_t dtype) { return dtype == BS_F32 ? 4u : (dtype == BS_C128 ? 16u : 8u); }
 
 struct __align__(256) WsHead {
     uint32_t scan_ticket;    // dynamic tile id of the single-pass scan
@@ -47,6 +50,7 @@ struct __align__(256) WsHead {
     uint32_t n_struct_blocks;
     uint32_t scan_ticket2;
     uint32_t ctas_done2;
+    uint32_t dtype;          // element type of the set the tables describe (bs.h BS_F64 ..)
 };
 
 struct WsLayout {
@@ -92,6 +96,7 @@ struct ScanParams {
     const uint32_t* dim;
     const uint64_t* addr;
     uint32_t T, B;           // SER: counts; DESER: capacities of the out arrays
+    uint32_t dtype;          // SER: element type of the set
     // DESER inputs
     const unsigned char* header;  // stream byte 0 .. header_bytes (device)
     const unsigned char* payload; // stream byte 0 when the payload is resident behind the header (pad-zero check), else null

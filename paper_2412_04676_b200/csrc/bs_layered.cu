@@ -568,7 +568,7 @@ __device__ __forceinline__ void plan_expand_chunk(const LPlanParams& p, uint64_t
             }
             Blk e;
             e.off = off;
-            e.addr = (address & ~7ull) | odd;
+            e.addr = (address & ~7ull) | (odd << 1);  // pad code (Blk): 2 words = the 8 zero bytes of an odd f64 block
             p.lw.ws.blk[i] = e;
             // granule boundaries g*kGranule inside [off, off + stored)
             g0 = (off + kGranule - 1) / kGranule;

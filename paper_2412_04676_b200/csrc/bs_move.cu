@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
         const uint64_t tfirst = tbase > plo ? tbase : plo;  // first payload byte of the tile inside [lo, hi)
         unsigned char* const tile_ptr = stream_at(p, hb, hb + tfirst) - (tfirst - tbase);  // where payload byte tbase would lie
         uint64_t src[UPT];   // pack: block address of the unit; unpack: destination address
-        uint32_t kind[UPT];  // 0 skip, 1 full 16 B aligned, 2 full 16 B as 2x8, 3 tail 8 B (+ 8 B pad)
+        uint32_t kind[UPT];  // 0 skip, 1 full 16 B aligned, 2 full 16 B as 2x8, 4 / 8 / 12: tail unit of that many data bytes (+ zero pad)
         uint64_t soff[UPT];
 #pragma unroll
         for (int k = 0; k < UPT; ++k) {
@@ -112,10 +112,10 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
                 const Blk e = blk[j];
                 const uint64_t next = __ldg(reinterpret_cast<const unsigned long long*>(&blk[j + 1].off));
                 const uint64_t intra = s - e.off;
-                const uint64_t nbytes = (next - e.off) - ((e.addr & 1ull) ? 8 : 0);
+                const uint64_t nbytes = (next - e.off) - (e.addr & 3ull) * 4;
                 const uint64_t a = (e.addr & ~7ull) + intra;
                 src[k] = a;
-                kind[k] = (intra + 16 <= nbytes) ? ((a & 15ull) ? 2u : 1u) : 3u;
+                kind[k] = (intra + 16 <= nbytes) ? ((a & 15ull) ? 2u : 1u) : (uint32_t)(nbytes - intra);
             }
         }
         if (!UNPACK) {
@@ -128,9 +128,13 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
                     uint2 a = ld_stream8(reinterpret_cast<const void*>(src[k]));
                     uint2 b = ld_stream8(reinterpret_cast<const void*>(src[k] + 8));
                     v[k] = make_uint4(a.x, a.y, b.x, b.y);
-                } else if (kind[k] == 3) {
+                } else if (kind[k] == 8) {
                     uint2 a = ld_stream8(reinterpret_cast<const void*>(src[k]));
                     v[k] = make_uint4(a.x, a.y, 0u, 0u);  // 8 data bytes + 8 zero pad bytes (D3)
+                } else if (kind[k] != 0) {                // f32 blocks: 4 or 12 data bytes
+                    const uint32_t* w = reinterpret_cast<const uint32_t*>(src[k]);
+                    v[k].x = __ldcs(w);
+                    if (kind[k] == 12) { v[k].y = __ldcs(w + 1); v[k].z = __ldcs(w + 2); }
                 }
             }
 #pragma unroll
@@ -147,10 +151,16 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
                 else if (kind[k] == 2) {
                     st_stream8(reinterpret_cast<void*>(src[k]), make_uint2(v[k].x, v[k].y));
                     st_stream8(reinterpret_cast<void*>(src[k] + 8), make_uint2(v[k].z, v[k].w));
-                } else if (kind[k] == 3) {
+                } else if (kind[k] == 8) {
                     st_stream8(reinterpret_cast<void*>(src[k]), make_uint2(v[k].x, v[k].y));
                     if ((p.flags & kFlagCheckPad) && (v[k].z | v[k].w) != 0)
                         atomicCAS(const_cast<int*>(&head->status), 0, BS_ERR_CORRUPT);
+                } else if (kind[k] != 0) {                // f32 blocks: 4 or 12 data bytes
+                    uint32_t* w = reinterpret_cast<uint32_t*>(src[k]);
+                    __stcs(w, v[k].x);
+                    if (kind[k] == 12) { __stcs(w + 1, v[k].y); __stcs(w + 2, v[k].z); }
+                    const uint32_t z = kind[k] == 12 ? v[k].w : (v[k].y | v[k].z | v[k].w);
+                    if ((p.flags & kFlagCheckPad) && z != 0) atomicCAS(const_cast<int*>(&head->status), 0, BS_ERR_CORRUPT);
                 }
             }
         }

@@ -106,10 +106,10 @@ __device__ __forceinline__ void bulk_wait_read()
     asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-// 8 data bytes + 8 zero bytes (the tail of an odd-sized block and its pad)
-__device__ __forceinline__ void cp_async_tail16(uint32_t dst, const void* src)
+// `data` bytes (4, 8 or 12) + zeros up to 16: the last unit of a padded block
+__device__ __forceinline__ void cp_async_tail16(uint32_t dst, const void* src, uint32_t data)
 {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16, 8;" ::"r"(dst), "l"(src) : "memory");
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(data) : "memory");
 }
 __device__ __forceinline__ void cp_async_8(uint32_t dst, const void* src)
 {
@@ -134,7 +134,7 @@ __device__ __forceinline__ void cp_async_wait()
 struct Seg {          // intersection of one block with one tile, payload coordinates
     uint64_t lo;      // first payload byte
     uint32_t bulk;    // bytes movable as one 16-byte-granular copy (whole 16-byte units of block data)
-    uint32_t tail;    // 1: the segment ends with the 8 data + 8 pad bytes of an odd-sized block
+    uint32_t tail;    // != 0: the segment ends with the last 16-byte unit of a padded block = `tail` data bytes (4, 8, 12) + zeros
     uint64_t addr;    // device address of the block byte that maps to payload byte `lo`
 };
 
@@ -145,10 +145,10 @@ __device__ __forceinline__ bool clip_seg(const Blk& e, uint64_t next, uint64_t t
     const uint64_t lo = e.off > tlo ? e.off : tlo;
     const uint64_t hi = next < thi ? next : thi;
     if (hi <= lo) return false;
-    const bool odd = (e.addr & 1ull) != 0;
+    const uint32_t pad = (uint32_t)(e.addr & 3ull) * 4u;  // zero pad bytes behind the block's data (D3)
     s->lo = lo;
     s->addr = (e.addr & ~7ull) + (lo - e.off);
-    s->tail = (odd && hi == next) ? 1u : 0u;
+    s->tail = (pad != 0 && hi == next) ? 16u - pad : 0u;
     s->bulk = (uint32_t)(hi - lo) - (s->tail ? 16u : 0u);
     return true;
 }
@@ -170,18 +170,20 @@ constexpr uint32_t kMetaBytes = 2 * kMetaBlk * 16 + 32;  // 1120 per warp
 __device__ __forceinline__ uint32_t pack_seg_async(const Seg& s, uint32_t d, uint32_t* tx)
 {
     uint32_t n_async = 0;
-    if (s.addr & 15ull) {  // D16 slow path: 8-byte pieces; the pad is a plain shared store
-        const uint32_t nb = s.bulk + (s.tail ? 8u : 0u);
-        for (uint32_t b = 0; b < nb; b += 8) cp_async_8(d + b, reinterpret_cast<const void*>(s.addr + b));
+    if (s.addr & 15ull) {  // D16 slow path: 8-byte pieces (a last 4-byte one for f32); the pad is plain shared stores
+        const uint32_t nb = s.bulk + s.tail;
+        for (uint32_t b = 0; b + 8 <= nb; b += 8) cp_async_8(d + b, reinterpret_cast<const void*>(s.addr + b));
+        if (nb & 4u) cp_async_4(d + (nb & ~7u), reinterpret_cast<const void*>(s.addr + (nb & ~7u)));
         n_async += nb ? 1u : 0u;
         if (s.tail) {
-            asm volatile("st.shared.u64 [%0], %1;" ::"r"(d + s.bulk + 8), "l"(0ull) : "memory");
+            for (uint32_t b = s.tail; b < 16u; b += 4)
+                asm volatile("st.shared.u32 [%0], %1;" ::"r"(d + s.bulk + b), "r"(0u) : "memory");
             fence_proxy_async();
         }
     } else {
         *tx += s.bulk;
         if (s.tail) {
-            cp_async_tail16(d + s.bulk, reinterpret_cast<const void*>(s.addr + s.bulk));
+            cp_async_tail16(d + s.bulk, reinterpret_cast<const void*>(s.addr + s.bulk), s.tail);
             ++n_async;
         }
     }
@@ -198,11 +200,18 @@ __device__ __forceinline__ void unpack_seg(const Seg& s, uint32_t saddr, const u
     } else if (s.bulk) {
         bulk_s2g_x(reinterpret_cast<void*>(s.addr), saddr, s.bulk, h);
     }
-    if (s.tail) {  // 8 data bytes; the 8 pad bytes stay in the stream
-        const uint2 v = *reinterpret_cast<const uint2*>(sp + s.bulk);
-        const uint2 z = *reinterpret_cast<const uint2*>(sp + s.bulk + 8);
-        *reinterpret_cast<uint2*>(s.addr + s.bulk) = v;
-        if ((flags & kFlagCheckPad) && (z.x | z.y) != 0) atomicCAS(status, 0, BS_ERR_CORRUPT);
+    if (s.tail) {  // `tail` data bytes; the pad bytes stay in the stream
+        const uint4 v = *reinterpret_cast<const uint4*>(sp + s.bulk);
+        if (s.tail == 8u) {
+            *reinterpret_cast<uint2*>(s.addr + s.bulk) = make_uint2(v.x, v.y);
+            if ((flags & kFlagCheckPad) && (v.z | v.w) != 0) atomicCAS(status, 0, BS_ERR_CORRUPT);
+        } else {  // f32 blocks: 4 or 12 data bytes
+            uint32_t* o = reinterpret_cast<uint32_t*>(s.addr + s.bulk);
+            o[0] = v.x;
+            if (s.tail == 12u) { o[1] = v.y; o[2] = v.z; }
+            const uint32_t z = s.tail == 12u ? v.w : (v.y | v.z | v.w);
+            if ((flags & kFlagCheckPad) && z != 0) atomicCAS(status, 0, BS_ERR_CORRUPT);
+        }
     }
 }
 

@@ -90,6 +90,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
 
     // ---- counts; deserialize: the fixed header (SURVEY §8(c) checks, in order) ------------------------
     uint64_t T = p.T, B = p.B, hb = 0, P_hdr = 0;
+    uint32_t dtype = p.dtype;
     bool ok = true;
     if (DESER) {
         int code = 0;
@@ -104,7 +105,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
             if (w0.x != 0x41505342u || w0.y != 0x31455352u)      code = BS_ERR_CORRUPT;  // "BSPARSE1"
             else if (w0.z != 1u)                                  code = BS_ERR_CORRUPT;  // version
             else if (w0.w != 0x01020304u)                         code = BS_ERR_CORRUPT;  // endian_tag
-            else if (w1.x != 0u)                                  code = BS_ERR_CORRUPT;  // dtype f64
+            else if (w1.x > (uint32_t)BS_C128)                    code = BS_ERR_CORRUPT;  // dtype
             else if (w1.y != 2u)                                  code = BS_ERR_CORRUPT;  // n_qn
             else if (w1.z != 3u)                                  code = BS_ERR_CORRUPT;  // max_rank
             else if (w1.w != 16u)                                 code = BS_ERR_CORRUPT;  // align
@@ -112,7 +113,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
             else if (hH != align_up(kFixedHeader + kTensorRec * hT + kBlockRec * hB, kHeaderAlign)) code = BS_ERR_CORRUPT;
             else if (hH > p.nbytes || hP != p.nbytes - hH)        code = BS_ERR_CORRUPT;
             else if (hT > p.T || hB > p.B)                        code = BS_ERR_CAPACITY;  // out arrays too small
-            else { T = hT; B = hB; hb = hH; P_hdr = hP; }
+            else { T = hT; B = hB; hb = hH; P_hdr = hP; dtype = w1.x; }
             if (code == BS_ERR_CAPACITY) { /* report the counts so the caller can size its arrays */
                 if (blockIdx.x == 0 && tid == 0) { head->n_tensors = (uint32_t)hT; head->n_blocks = (uint32_t)hB; }
             }
@@ -152,6 +153,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
         }
     }
 
+    const uint64_t esize = elem_bytes(dtype);
     // ---- single-pass scan over tiles of kScanTile blocks -----------------------------------------------
     const uint64_t n_tiles = ok ? (B + kScanTile - 1) / kScanTile + (B == 0 ? 1 : 0) : 0;
     const unsigned char* brec = DESER ? p.header + kFixedHeader + kTensorRec * T : nullptr;
@@ -189,14 +191,14 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                     a = __ldg(reinterpret_cast<const unsigned long long*>(p.addr + i));
                 }
             }
-            // S1: nbytes = 8 * prod(dim) in u64 (D13); stored = align16(nbytes) (D3)
+            // S1: nbytes = e * prod(dim) in u64 (D13), e = element size of the dtype; stored = align16(nbytes) (D3)
             uint64_t n01 = (uint64_t)d0 * d1;
             uint64_t n = n01 * d2;
             if (valid && (__umul64hi(n01, (uint64_t)d2) != 0 || n >= (1ull << 57))) { err = kErrBad; n = 0; }
-            const uint64_t nbytes = n * 8;
+            const uint64_t nbytes = n * esize;
             const uint64_t st = (nbytes + 15) & ~15ull;
             stored[k] = st;
-            oddf[k] = (uint32_t)(n & 1);
+            oddf[k] = (uint32_t)(st - nbytes) >> 2;  // pad code: 0..3 words of zero pad
             dsta[k] = 0;
             if (DESER) {
                 aux[k] = offset;
@@ -215,8 +217,13 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                     if (i + 1 < B) next = __ldg(reinterpret_cast<const unsigned long long*>(brec + kBlockRec * (i + 1) + 40));
                     if (i == 0 && offset != 0) err = BS_ERR_CORRUPT;
                     if (offset > P_hdr || st > P_hdr - offset || offset + st != next) err = BS_ERR_CORRUPT;
-                    else if ((n & 1) && p.payload != nullptr) {  // pad bytes are zero
-                        uint64_t pad = __ldg(reinterpret_cast<const unsigned long long*>(p.payload + hb + offset + nbytes));
+                    else if (st != nbytes && p.payload != nullptr) {  // pad bytes are zero: the last 16-byte unit of the block
+                        const uint4 u = __ldg(reinterpret_cast<const uint4*>(p.payload + hb + offset + st - 16));
+                        const uint32_t data_words = 4u - ((uint32_t)(st - nbytes) >> 2);
+                        const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+                        uint32_t pad = 0;
+#pragma unroll
+                        for (uint32_t q = 0; q < 4; ++q) pad |= (q >= data_words) ? w[q] : 0u;
                         if (pad != 0) err = BS_ERR_CORRUPT;
                     }
                     if (p.flags == BS_SCATTER_TO_ADDR) {
@@ -357,6 +364,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
             vh->n_blocks = (uint32_t)B;
         }
         vh->header_bytes = hb;
+        vh->dtype = dtype;
         vh->payload_bytes = P;
         vh->pool_bytes = pool;
         vh->n_granules = ng;
@@ -366,6 +374,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
             r.total_bytes = total; r.header_bytes = hb; r.payload_bytes = P; r.pool_bytes = pool;
             r.status = status; r.n_tensors = vh->n_tensors; r.n_blocks = vh->n_blocks;
             for (int z = 0; z < 5; ++z) r.reserved[z] = 0;
+            r.reserved[2] = dtype;
             *p.result = r;
         }
         __threadfence();

@@ -27,16 +27,17 @@ class DeviceSet:
     """The four device arrays of one bs_set_desc, as torch uint8 tensors."""
 
     def __init__(self, tensors: torch.Tensor, qn: torch.Tensor, dim: torch.Tensor, addr: torch.Tensor, n_tensors: int,
-                 n_blocks: int):
+                 n_blocks: int, dtype: int = B.F64):
         self.tensors, self.qn, self.dim, self.addr = tensors, qn, dim, addr
-        self.n_tensors, self.n_blocks = n_tensors, n_blocks
+        self.n_tensors, self.n_blocks, self.dtype = n_tensors, n_blocks, dtype
 
     @classmethod
-    def from_host(cls, tensors: np.ndarray, qn: np.ndarray, dim: np.ndarray, addr: np.ndarray, device="cuda"):
+    def from_host(cls, tensors: np.ndarray, qn: np.ndarray, dim: np.ndarray, addr: np.ndarray, device="cuda",
+                  dtype: int = B.F64):
         assert tensors.dtype.itemsize == 32
         return cls(_to_dev(tensors, device), _to_dev(qn.astype(np.int32, copy=False), device),
                    _to_dev(dim.astype(np.uint32, copy=False), device), _to_dev(addr.astype(np.uint64, copy=False), device),
-                   len(tensors), int(np.asarray(dim).reshape(-1, 3).shape[0]))
+                   len(tensors), int(np.asarray(dim).reshape(-1, 3).shape[0]), dtype)
 
     @classmethod
     def empty(cls, cap_tensors: int, cap_blocks: int, device="cuda", fill: int | None = None):
@@ -50,7 +51,7 @@ class DeviceSet:
     @property
     def desc(self) -> B.SetDesc:
         return B.make_desc(self.n_tensors, self.n_blocks, self.tensors.data_ptr(), self.qn.data_ptr(), self.dim.data_ptr(),
-                           self.addr.data_ptr())
+                           self.addr.data_ptr(), self.dtype)
 
     def to_host(self, n_tensors: int | None = None, n_blocks: int | None = None) -> dict:
         T = self.n_tensors if n_tensors is None else n_tensors
@@ -139,5 +140,5 @@ class Workspace:
         r = B.Result.from_buffer_copy(raw)
         return dict(total_bytes=int(r.total_bytes), header_bytes=int(r.header_bytes), payload_bytes=int(r.payload_bytes),
                     pool_bytes=int(r.pool_bytes), status=int(r.status), n_tensors=int(r.n_tensors), n_blocks=int(r.n_blocks),
-                    n_structs=int(r.reserved[0]), n_struct_blocks=int(r.reserved[1]),
+                    n_structs=int(r.reserved[0]), n_struct_blocks=int(r.reserved[1]), dtype=int(r.reserved[2]),
                     n_packages=int(r.reserved[0]))
