@@ -43,6 +43,9 @@ UNIT = "GB/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
 
+ELEM = {"f64": (0, 8), "f32": (1, 4), "c64": (2, 8), "c128": (3, 16)}   # bs.h dtype, element bytes
+
+
 def log(*a):
     print(*a, file=sys.stderr, flush=True)
 
@@ -241,6 +244,12 @@ def workload_config(name, bset, total, fmt="v1"):
     return c
 
 
+def with_elem(c, elem):
+    if elem != "f64":
+        c["element_type"] = f"{elem}: every block read as {ELEM[elem][1]}-byte elements (the first e*n bytes of its fp64 storage)"
+    return c
+
+
 # ---- the CUDA arm -------------------------------------------------------------------------------------------------------
 def run_mine(args):
     import torch
@@ -276,7 +285,7 @@ def run_mine(args):
     bset = W.make_config(args.workload)
     pool, addr = fill_pool_device(bset, dev)
     v2 = args.format == "v2"
-    cap_guess = bset.data_bytes + 16 * bset.n_blocks + bs.header_bytes(bset.n_tensors, bset.n_blocks)
+    cap_guess = bset.data_bytes * max(1, ELEM[args.elem][1] // 8) + 16 * bset.n_blocks + bs.header_bytes(bset.n_tensors, bset.n_blocks)
     cs = bs.current_stream()
     if v2:   # the same tensors as layers of their structures (wire format v2); pool and addresses are shared
         lv = W.layered_view(bset)
@@ -288,13 +297,14 @@ def run_mine(args):
         f_ser, f_range, f_deser, f_size = bs.layered_serialize, bs.layered_serialize_range, bs.layered_deserialize, \
             bs.layered_serialized_size
     else:
-        dset = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, addr, dev)
+        # --elem: the same blocks read as elements of another size (the first e*n bytes of each fp64 block)
+        dset = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, addr, dev, dtype=ELEM[args.elem][0])
         ws = bs.Workspace(bset.n_tensors, bset.n_blocks, cap_guess, dev)
         hb, total = bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs)   # size known before serialization
         out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, dev)
         f_ser, f_range, f_deser, f_size = bs.serialize, bs.serialize_range, bs.deserialize, bs.serialized_size
     stream = torch.empty(total, dtype=torch.uint8, device=dev)
-    need = int(((bset.nelems * 8 + 255) // 256 * 256).sum())
+    need = int(((bset.nelems * ELEM[args.elem][1] + 255) // 256 * 256).sum())
     opool = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
     log(f"[rank {rank}] workload {args.workload}: T={bset.n_tensors} B={bset.n_blocks} stream={total / 1e9:.3f} GB "
         f"(header {hb / 1e6:.1f} MB) set up in {time.time() - t_setup:.1f}s")
@@ -551,7 +561,7 @@ def run_mine(args):
         line = {"metric": METRIC, "value": round(units_g / (ms_g * 1e-3) / 1e9, 3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_g, 4), "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
-                "config": workload_config(args.workload, bset, total, args.format), "clocks": clocks, "e2e": e2e,
+                "config": with_elem(workload_config(args.workload, bset, total, args.format), args.elem), "clocks": clocks, "e2e": e2e,
                 "gpu_launches": (8 if v2 else 4) * args.steps, "roofline": roofline, "cpu_baseline": cpu, "detail": detail}
         print(json.dumps(line), flush=True)
     if ready:
@@ -676,6 +686,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
     ap.add_argument("--workload", default="4", choices=["1", "2", "3", "4", "3L", "4L"])
+    ap.add_argument("--elem", default="f64", choices=sorted(ELEM), help="element type of the blocks (wire format v1); "
+                    "other than f64: kernels only (no e2e / config-5 / cpu legs)")
     ap.add_argument("--format", default="v1", choices=["v1", "v2"],
                     help="wire format: v1 (one block record per block) or v2 (structure-shared layers, NEXT-1)")
     ap.add_argument("--variant", type=int, default=0)
@@ -695,6 +707,10 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "mine" else args.warmup
+    if args.elem != "f64":   # the e2e / config-5 / cpu legs and wire format v2 are fp64; other element types time the kernels
+        if args.format != "v1" or args.impl != "mine":
+            ap.error("--elem other than f64 needs --format v1 --impl mine")
+        args.no_e2e = args.no_config5 = args.no_cpu = args.no_packages = True
     if args.impl == "reference":
         run_reference(args)
     else:
