@@ -215,15 +215,20 @@ __device__ __forceinline__ void unpack_seg(const Seg& s, uint32_t saddr, const u
     }
 }
 
-// Default launch shapes (B200, measured on the D=6000 and D=15400 sets): about 96 KiB (pack) / 64 KiB (unpack) of
-// loads in flight per SM; deeper rings or more warps lower the achieved DRAM bandwidth.
+// Default launch shapes (B200, measured on the D=6000 and D=15400 sets): pack 3 rings x 3 stages x 16 KiB, unpack one
+// ring of 4 stages x 32 KiB — about 96 KiB of loads in flight per SM either way; deeper rings or more warps lower the
+// achieved DRAM bandwidth.  (Unpack, whole bs_deserialize: 6440 / 6470 GB/s on the two sets with this shape against
+// 6360 / 6235 with 2 rings x 3 x 16 KiB.)  A package map whose size limit is not a multiple of 32 KiB keeps 16 KiB tiles.
 struct Preset {
     uint32_t tile_bytes, stages, warps;
 };
-__host__ __device__ inline Preset preset(bool unpack)
+__host__ __device__ inline Preset preset(bool unpack, uint64_t pkg_cap)
 {
     Preset ps = {16384, 3, 3};
-    if (unpack) ps.warps = 2;
+    if (unpack) {
+        if (pkg_cap % 32768 == 0) { ps.tile_bytes = 32768; ps.stages = 4; ps.warps = 1; }
+        else ps.warps = 2;
+    }
     return ps;
 }
 
@@ -434,7 +439,7 @@ cudaError_t launch_tma_t(const MoveParams& p, const bs_opts& o, int sm_count, cu
     MoveParams q = p;
     uint32_t stages = o.stages, warps = o.warps;
     if (o.tile_bytes == 0) {  // bs_opts left the shape open
-        const Preset ps = preset(UNPACK);
+        const Preset ps = preset(UNPACK, q.pkg.cap);
         q.tile_bytes = ps.tile_bytes; stages = ps.stages; warps = ps.warps;
     }
     if (stages < 3 || stages > kMaxStages || warps < 1 || warps > kMaxWarps) return cudaErrorInvalidValue;
