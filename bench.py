@@ -676,6 +676,81 @@ def config5(args, dev, opts):
     pre["headline"] = pre["sweep"][0]
     res["prefetch"] = pre
     eng.destroy()
+
+    # ---- a sweep, PAPER Fig 3: every DMRG step loads the environment block of the next step, computes, and saves the
+    # block it renormalized.  Synchronous IO (Fig 3(a): compute halts for every save and load) against the queue
+    # (Fig 3(c): the load of step i+1 and the save of step i-1 run behind the compute of step i, checkpoints = events).
+    # The compute is the stand-in contraction at 1.25 x the duplex IO time of one step. ----
+    try:
+        n_steps, n_keys = 12, 4   # 4 scratch slots: a block is loaded two steps after it was saved, as in a sweep that returns to it
+        hosts = [host] + [torch.empty(total, dtype=torch.uint8, pin_memory=True) for _ in range(n_keys - 1)]
+        q = bs.Queue(bset.n_tensors, bset.n_blocks, total, chunk_bytes=args.chunk_mb << 20, n_staging=2, opts=opts)
+        for k in range(n_keys):
+            q.save(k, dset.desc, total, hosts[k].data_ptr(), total, cs)
+        q.drain()
+
+        def duplex_io():
+            a.record()
+            q.save(0, dset.desc, total, hosts[0].data_ptr(), total, cs)
+            q.load(1, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, cs)
+            q.checkpoint(0, cs)
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b)
+
+        duplex_io()
+        io_step = min(duplex_io() for _ in range(3))
+        reps = max(1, int(round(1.25 * io_step / one)))
+        tc_step = min(t_c(reps) for _ in range(2))
+
+        def sweep_sync():
+            a.record()
+            for i in range(n_steps):
+                q.load((i + 1) % n_keys, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, cs)
+                q.wait((i + 1) % n_keys)                 # compute halts until the environment block is in memory
+                work.run(reps)
+                q.save(i % n_keys, dset.desc, total, hosts[i % n_keys].data_ptr(), total, cs)
+                q.wait(i % n_keys)                       # ... and until the renormalized block is saved
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b)
+
+        def sweep_async():
+            a.record()
+            q.load(1, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, side.cuda_stream)
+            for i in range(n_steps):
+                torch.cuda.current_stream().wait_stream(side)        # checkpoint: the environment block of step i is here
+                if i + 1 < n_steps:                                    # next step's environment block, behind this compute
+                    side.wait_stream(torch.cuda.current_stream())
+                    q.load((i + 2) % n_keys, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, side.cuda_stream)
+                work.run(reps)
+                q.save(i % n_keys, dset.desc, total, hosts[i % n_keys].data_ptr(), total, cs)   # runs behind the next compute
+            for k in range(n_keys):
+                q.checkpoint(k, cs)
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b)
+
+        sweep_sync(); sweep_async()
+        t_sync = min(sweep_sync() for _ in range(2))
+        t_async = min(sweep_async() for _ in range(2))
+        for k in range(n_keys):
+            if q.wait(k)["status"]:
+                raise RuntimeError("queue status")
+        res["sweep_fig3"] = {"steps": n_steps, "bytes_saved_and_loaded_per_step": int(2 * total),
+                             "compute_ms_per_step": round(tc_step, 3), "duplex_io_ms_per_step": round(io_step, 3),
+                             "sync_io_ms": round(t_sync, 3), "queue_ms": round(t_async, 3),
+                             "compute_only_ms": round(n_steps * tc_step, 3),
+                             "speedup_queue_over_sync": round(t_sync / t_async, 3),
+                             "exposed_io_frac_queue": round(max(0.0, t_async - n_steps * tc_step) / t_async, 4),
+                             "io_frac_sync": round(max(0.0, t_sync - n_steps * tc_step) / t_sync, 4),
+                             "ends_ms": round(io_ms + pio_ms, 3),
+                             "exposed_io_frac_queue_without_ends": round(max(0.0, t_async - n_steps * tc_step - io_ms - pio_ms) / t_async, 4),
+                             "note": "the first load and the last save of a sweep have no compute to hide behind (ends_ms = one "
+                                     "save alone + one load alone)"}
+        q.destroy()
+    except Exception as ex:
+        res["sweep_fig3"] = {"error": repr(ex)}
     return res
 
 
