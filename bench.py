@@ -497,6 +497,42 @@ def run_mine(args):
             del host2, hosts
         del host
 
+    # ---- the small configs are launch-latency bound: report microseconds per call, device-timed back to
+    # back, next to a plain copy of the same number of bytes ----
+    if rank == 0 and not v2 and args.elem == "f64" and not args.no_small:
+        small = {}
+        for wl in ("1", "2"):
+            sb = W.make_config(wl)
+            sp_, sa = fill_pool_device(sb, dev)
+            sd = bs.DeviceSet.from_host(sb.tensors, sb.qn, sb.dim, sa, dev)
+            sws = bs.Workspace(sb.n_tensors, sb.n_blocks, sb.data_bytes + 16 * sb.n_blocks + (1 << 20), dev)
+            shb, stot = bs.serialized_size(sd.desc, sws.ptr, sws.nbytes, cs)
+            sst = torch.empty(stot, dtype=torch.uint8, device=dev)
+            ssrc = torch.empty(stot, dtype=torch.uint8, device=dev)
+            sneed = int(((sb.nelems * 8 + 255) // 256 * 256).sum())
+            sout = bs.DeviceSet.empty(sb.n_tensors, sb.n_blocks, dev)
+            spool = torch.empty(max(sneed, 256), dtype=torch.uint8, device=dev)
+            fns = {"serialize_us": lambda: bs.serialize(sd.desc, sst.data_ptr(), stot, sws.ptr, sws.nbytes, sws.result_ptr, opts, cs),
+                   "deserialize_us": lambda: bs.deserialize(sst.data_ptr(), stot, sout.desc, spool.data_ptr(), sneed, bs.LAYOUT_POOL,
+                                                            sws.ptr, sws.nbytes, sws.result_ptr, opts, cs),
+                   "plain_copy_us": lambda: sst.copy_(ssrc)}
+            row = {"stream_bytes": int(stot), "n_blocks": int(sb.n_blocks)}
+            fns["serialize_us"]()
+            for name, fn in fns.items():
+                for _ in range(20):
+                    fn()
+                torch.cuda.synchronize()
+                a.record()
+                for _ in range(200):
+                    fn()
+                b.record()
+                torch.cuda.synchronize()
+                row[name] = round(a.elapsed_time(b) / 200 * 1e3, 1)
+            if sws.read_result()["status"] != bs.OK:
+                raise RuntimeError("small sets: deferred status")
+            small[f"config{wl}"] = row
+        detail["small_sets"] = small
+
     # ---- self-contained packages: the same bytes as packages in device slots, emitted and unpacked
     # package by package; the size limit decides how many launches the bytes are spread over ----
     if not v2 and not args.no_packages:
@@ -777,6 +813,7 @@ def main():
     ap.add_argument("--standin-items", type=int, default=60000)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-packages", action="store_true")
+    ap.add_argument("--no-small", action="store_true", help="skip the latency numbers of configs 1 and 2")
     ap.add_argument("--no-queue", action="store_true", help="e2e: offload then prefetch only, no duplex queue leg")
     ap.add_argument("--no-config5", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
