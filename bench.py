@@ -444,22 +444,21 @@ def run_mine(args):
             # per step as above; this is the e2e headline, the one-after-the-other number stays in detail. ----
             host2 = torch.empty(total, dtype=torch.uint8, pin_memory=True)
             hosts = [host, host2]
-            dbuf = torch.empty(2 * nlink, dtype=torch.uint8, device=dev)
             s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+            nb = int(min(total, stream.numel(), opool.numel()))   # the same bytes per direction as one step moves
             best = 1e9
-            for _ in range(5):   # link denominator with both directions busy, same run
+            for _ in range(3):   # link denominator with both directions busy, same run, same size (sustained, not a burst)
                 torch.cuda.synchronize()
                 a.record()
                 s1.wait_stream(torch.cuda.current_stream()); s2.wait_stream(torch.cuda.current_stream())
                 with torch.cuda.stream(s1):
-                    host[:nlink].copy_(dbuf[:nlink], non_blocking=True)
+                    host[:nb].copy_(stream[:nb], non_blocking=True)
                 with torch.cuda.stream(s2):
-                    dbuf[nlink:].copy_(host2[:nlink], non_blocking=True)
+                    opool[:nb].copy_(host2[:nb], non_blocking=True)
                 torch.cuda.current_stream().wait_stream(s1); torch.cuda.current_stream().wait_stream(s2)
                 b.record(); torch.cuda.synchronize()
                 best = min(best, a.elapsed_time(b))
-            bw["bidir"] = 2 * nlink / best / 1e6
-            del dbuf
+            bw["bidir"] = 2 * nb / best / 1e6
             q = bs.Queue(bset.n_tensors, bset.n_blocks, total, chunk_bytes=args.chunk_mb << 20, n_staging=2, opts=opts)
             for k in (0, 1):
                 q.save(k, dset.desc, total, hosts[k].data_ptr(), total, cs)
