@@ -417,7 +417,13 @@ int bs_queue_destroy(bs_queue *q);                                  /* drains fi
  * synchronises `producer`).  A previous stream of `key` is replaced. */
 int bs_queue_save(bs_queue *q, uint64_t key, const bs_set_desc *set, uint64_t total_bytes, void *h_pinned,
                   uint64_t h_capacity, cudaStream_t producer);
-/* Register a complete stream that is already in pinned host memory (it came from elsewhere) under `key`. */
+/* The same for layered sets (wire format v2); a key holds a stream of ONE format: loading it with the other call is
+ * BS_ERR_ARG.  Element types other than fp64 (v1) travel through bs_queue_save / bs_queue_load unchanged. */
+int bs_queue_save_layered(bs_queue *q, uint64_t key, const bs_layered_desc *set, uint64_t total_bytes, void *h_pinned,
+                          uint64_t h_capacity, cudaStream_t producer);
+int bs_queue_load_layered(bs_queue *q, uint64_t key, bs_layered_desc *out, void *d_pool, uint64_t pool_bytes, uint32_t flags,
+                          cudaStream_t consumer);
+/* Register a complete stream (either wire format) that is already in pinned host memory (it came from elsewhere) under `key`. */
 int bs_queue_adopt(bs_queue *q, uint64_t key, const void *h_pinned, uint64_t nbytes);
 /* Load the stream of `key` (as bs_prefetch_async).  BS_ERR_ARG for an unknown key. */
 int bs_queue_load(bs_queue *q, uint64_t key, bs_set_desc *out, void *d_pool, uint64_t pool_bytes, uint32_t flags,

@@ -12,9 +12,12 @@ in time on the GPU, what a user may observe is fixed by PROGRAM ORDER, and that 
 
   save(key, set, data)  the scratch store holds, under `key`, the wire-format-v1 stream of the set as it is at the
                         moment of the call (oracle.serialize); a later save under the same key replaces it
-  adopt(key, stream)    the store holds `stream` (bytes that came from elsewhere) under `key`
+  save_layered(key, ..) the same for a layered set: the store holds its wire-format-v2 stream (oracle.v2.serialize)
+  adopt(key, stream)    the store holds `stream` (bytes that came from elsewhere, either format) under `key`
   load(key)             the object identical to the one saved last under `key` (oracle.deserialize of the stored
                         stream); an unknown key is an error (ERR_ARG); a corrupt stream is ERR_CORRUPT
+  load_layered(key)     the same for a key that holds a v2 stream; a key holds a stream of ONE format, asking for the
+                        other is ERR_ARG
   forget(key)           the store drops `key`
   accounting            host_bytes_live = sum of the stored streams' lengths; host_bytes_peak = its maximum over the
                         calls so far; saves / loads = number of accepted calls; bytes_saved / bytes_loaded = stream
@@ -30,6 +33,7 @@ from __future__ import annotations
 import numpy as np
 
 from . import bs_oracle as _v1
+from . import bs_oracle_v2 as _v2
 
 
 class QueueModel:
@@ -55,18 +59,38 @@ class QueueModel:
         self._account()
         return self.store[int(key)]
 
+    def save_layered(self, key: int, structs, layers, qn, dim, addr) -> np.ndarray:
+        s = _v2.serialize(structs, layers, qn, dim, addr)
+        self.store[int(key)] = s.copy()
+        self.saves += 1
+        self.bytes_saved += len(s)
+        self._account()
+        return self.store[int(key)]
+
     def adopt(self, key: int, stream) -> None:
         self.store[int(key)] = np.ascontiguousarray(stream, dtype=np.uint8).copy()
         self._account()
 
-    def load(self, key: int) -> dict:
+    @staticmethod
+    def _is_v2(s) -> bool:
+        return len(s) >= 12 and int(np.frombuffer(bytes(s[8:12]), "<u4")[0]) == 2     # the header's version word
+
+    def _load(self, key: int, layered: bool) -> dict:
         if int(key) not in self.store:
             raise _v1.OracleError(_v1.ERR_ARG, "queue load: unknown key")
         s = self.store[int(key)]
-        out = _v1.deserialize(s)          # raises ERR_CORRUPT for a bad stream
+        if self._is_v2(s) != layered:
+            raise _v1.OracleError(_v1.ERR_ARG, "queue load: the key holds a stream of the other wire format")
+        out = _v2.deserialize(s) if layered else _v1.deserialize(s)     # raises ERR_CORRUPT for a bad stream
         self.loads += 1
         self.bytes_loaded += len(s)
         return out
+
+    def load(self, key: int) -> dict:
+        return self._load(key, False)
+
+    def load_layered(self, key: int) -> dict:
+        return self._load(key, True)
 
     def forget(self, key: int) -> None:
         if int(key) not in self.store:

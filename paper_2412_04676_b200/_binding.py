@@ -157,6 +157,8 @@ def lib():
     L.bs_queue_destroy.argtypes = [vp]
     L.bs_queue_save.argtypes = [vp, u64, C.POINTER(SetDesc), u64, vp, u64, vp]
     L.bs_queue_adopt.argtypes = [vp, u64, vp, u64]
+    L.bs_queue_save_layered.argtypes = [vp, u64, C.POINTER(LayeredDesc), u64, vp, u64, vp]
+    L.bs_queue_load_layered.argtypes = [vp, u64, C.POINTER(LayeredDesc), vp, u64, u32, vp]
     L.bs_queue_load.argtypes = [vp, u64, C.POINTER(SetDesc), vp, u64, u32, vp]
     L.bs_queue_checkpoint.argtypes = [vp, u64, vp]
     L.bs_queue_wait.argtypes = [vp, u64, C.POINTER(TicketStats), C.POINTER(TicketStats)]
@@ -433,6 +435,14 @@ class Queue:
     def save(self, key: int, desc: SetDesc, total_bytes: int, h_pinned_ptr: int, h_capacity: int, producer: int = 0) -> None:
         _check(lib().bs_queue_save(self._h, key, C.byref(desc), total_bytes, h_pinned_ptr, h_capacity, producer), "bs_queue_save")
         self._keys.add(key)
+
+    def save_layered(self, key: int, desc: LayeredDesc, total_bytes: int, h_pinned_ptr: int, h_capacity: int, producer: int = 0) -> None:
+        _check(lib().bs_queue_save_layered(self._h, key, C.byref(desc), total_bytes, h_pinned_ptr, h_capacity, producer),
+               "bs_queue_save_layered")
+        self._keys.add(key)
+
+    def load_layered(self, key: int, out: LayeredDesc, pool_ptr: int, pool_bytes: int, flags: int = 0, consumer: int = 0) -> None:
+        _check(lib().bs_queue_load_layered(self._h, key, C.byref(out), pool_ptr, pool_bytes, flags, consumer), "bs_queue_load_layered")
 
     def adopt(self, key: int, h_pinned_ptr: int, nbytes: int) -> None:
         _check(lib().bs_queue_adopt(self._h, key, h_pinned_ptr, nbytes), "bs_queue_adopt")

@@ -312,7 +312,7 @@ static int offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layered_d
 // of the same key); otherwise the fixed header is read from host RAM.  Either way the device validates what arrives.
 static int prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs_set_desc* out, bs_layered_desc* lout,
                          void* d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer, bs_ticket** ticket,
-                         const bs_stream_info_t* known = nullptr)
+                         const bs_stream_info_t* known = nullptr, const bs_layered_stream_info_t* known_l = nullptr)
 {
     if (e == nullptr || h_pinned == nullptr || (out == nullptr && lout == nullptr) || ticket == nullptr) return BS_ERR_ARG;
     if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
@@ -331,8 +331,8 @@ static int prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes, bs
         if (!ws_layout(e->ws, e->ws_bytes, out->n_blocks, &L)) return BS_ERR_CAPACITY;
     } else {
         bs_layered_stream_info_t li;
-        rc = bs_layered_stream_info(h_pinned, &li);
-        if (rc) return rc;
+        if (known_l) li = *known_l;
+        else if ((rc = bs_layered_stream_info(h_pinned, &li))) return rc;
         if (li.total_bytes != nbytes) return BS_ERR_CORRUPT;
         if (li.n_structs > e->cfg.max_tensors || li.n_layers > e->cfg.max_tensors || li.n_struct_blocks > e->cfg.max_blocks ||
             lout->n_addr > e->cfg.max_blocks || li.header_bytes > e->header_cap || nbytes > e->cfg.max_stream_bytes)
@@ -571,7 +571,9 @@ struct bs_queue {
         const void* h = nullptr;
         uint64_t nbytes = 0;
         bs_stream_info_t info;
+        bs_layered_stream_info_t linfo;
         bool adopted = false;
+        bool layered = false;  // the stored stream is wire format v2
     };
     bs_engine* lane_save = nullptr;
     bs_engine* lane_load = nullptr;
@@ -676,10 +678,10 @@ int bs_queue_destroy(bs_queue* q)
     return BS_OK;
 }
 
-int bs_queue_save(bs_queue* q, uint64_t key, const bs_set_desc* set, uint64_t total_bytes, void* h_pinned, uint64_t h_capacity,
-                  cudaStream_t producer)
+static int queue_save_impl(bs_queue* q, uint64_t key, const bs_set_desc* set, const bs_layered_desc* lset, uint64_t total_bytes,
+                           void* h_pinned, uint64_t h_capacity, cudaStream_t producer)
 {
-    if (q == nullptr || set == nullptr || h_pinned == nullptr) return BS_ERR_ARG;
+    if (q == nullptr || (set == nullptr && lset == nullptr) || h_pinned == nullptr) return BS_ERR_ARG;
     queue_reap(q, false);
     int rc;
     auto it = q->keys.find(key);
@@ -687,7 +689,7 @@ int bs_queue_save(bs_queue* q, uint64_t key, const bs_set_desc* set, uint64_t to
     if (it != q->keys.end() && it->second.load && !ticket_complete(it->second.load))
         if ((rc = engine_wait_ticket(q->lane_save, it->second.load))) return rc;
     bs_ticket* t = nullptr;
-    if ((rc = bs_offload_async(q->lane_save, set, total_bytes, h_pinned, h_capacity, producer, &t))) return rc;
+    if ((rc = offload_impl(q->lane_save, set, lset, total_bytes, h_pinned, h_capacity, producer, &t))) return rc;
     total_bytes = t->bytes;  // the size prediction, if the call made it
     bs_queue::Entry& en = q->keys[key];
     queue_retire(q, en.save);
@@ -695,16 +697,41 @@ int bs_queue_save(bs_queue* q, uint64_t key, const bs_set_desc* set, uint64_t to
     en.h = h_pinned;
     en.nbytes = total_bytes;
     en.adopted = false;
-    en.info.n_tensors = set->n_tensors;
-    en.info.n_blocks = set->n_blocks;
-    en.info.header_bytes = bs_header_bytes(set->n_tensors, set->n_blocks);
-    en.info.payload_bytes = total_bytes - en.info.header_bytes;
-    en.info.total_bytes = total_bytes;
+    en.layered = lset != nullptr;
+    if (set) {
+        en.info.n_tensors = set->n_tensors;
+        en.info.n_blocks = set->n_blocks;
+        en.info.header_bytes = bs_header_bytes(set->n_tensors, set->n_blocks);
+        en.info.payload_bytes = total_bytes - en.info.header_bytes;
+        en.info.total_bytes = total_bytes;
+        en.info.dtype = set->dtype;
+    } else {
+        en.linfo.n_structs = lset->n_structs;
+        en.linfo.n_struct_blocks = lset->n_struct_blocks;
+        en.linfo.n_layers = lset->n_layers;
+        en.linfo.header_bytes = bs_layered_header_bytes(lset->n_structs, lset->n_layers, lset->n_struct_blocks);
+        en.linfo.payload_bytes = total_bytes - en.linfo.header_bytes;
+        en.linfo.total_bytes = total_bytes;
+    }
     q->st.saves += 1;
     q->st.bytes_saved += total_bytes;
     queue_account_host(q);
     queue_count_in_flight(q);
     return BS_OK;
+}
+
+int bs_queue_save(bs_queue* q, uint64_t key, const bs_set_desc* set, uint64_t total_bytes, void* h_pinned, uint64_t h_capacity,
+                  cudaStream_t producer)
+{
+    if (set == nullptr) return BS_ERR_ARG;
+    return queue_save_impl(q, key, set, nullptr, total_bytes, h_pinned, h_capacity, producer);
+}
+
+int bs_queue_save_layered(bs_queue* q, uint64_t key, const bs_layered_desc* set, uint64_t total_bytes, void* h_pinned,
+                          uint64_t h_capacity, cudaStream_t producer)
+{
+    if (set == nullptr) return BS_ERR_ARG;
+    return queue_save_impl(q, key, nullptr, set, total_bytes, h_pinned, h_capacity, producer);
 }
 
 int bs_queue_adopt(bs_queue* q, uint64_t key, const void* h_pinned, uint64_t nbytes)
@@ -722,24 +749,28 @@ int bs_queue_adopt(bs_queue* q, uint64_t key, const void* h_pinned, uint64_t nby
     en.h = h_pinned;
     en.nbytes = nbytes;
     en.adopted = true;
+    uint32_t version = 0;
+    memcpy(&version, (const unsigned char*)h_pinned + 8, 4);  // the stream is complete and in host RAM
+    en.layered = version == 2u;
     queue_account_host(q);
     return BS_OK;
 }
 
-int bs_queue_load(bs_queue* q, uint64_t key, bs_set_desc* out, void* d_pool, uint64_t pool_bytes, uint32_t flags,
-                  cudaStream_t consumer)
+static int queue_load_impl(bs_queue* q, uint64_t key, bs_set_desc* out, bs_layered_desc* lout, void* d_pool, uint64_t pool_bytes,
+                           uint32_t flags, cudaStream_t consumer)
 {
-    if (q == nullptr || out == nullptr) return BS_ERR_ARG;
+    if (q == nullptr || (out == nullptr && lout == nullptr)) return BS_ERR_ARG;
     queue_reap(q, false);
     auto it = q->keys.find(key);
     if (it == q->keys.end()) return BS_ERR_ARG;
     bs_queue::Entry& en = it->second;
+    if (en.layered != (lout != nullptr)) return BS_ERR_ARG;  // the key holds a stream of the other wire format
     int rc;
     if (en.save && !ticket_complete(en.save))  // the stream is still on its way to the host buffer
         if ((rc = engine_wait_ticket(q->lane_load, en.save))) return rc;
     bs_ticket* t = nullptr;
-    rc = prefetch_impl(q->lane_load, en.h, en.nbytes, out, nullptr, d_pool, pool_bytes, flags, consumer, &t,
-                       en.adopted ? nullptr : &en.info);
+    rc = prefetch_impl(q->lane_load, en.h, en.nbytes, out, lout, d_pool, pool_bytes, flags, consumer, &t,
+                       (en.adopted || en.layered) ? nullptr : &en.info, (en.adopted || !en.layered) ? nullptr : &en.linfo);
     if (rc) return rc;
     queue_retire(q, en.load);
     en.load = t;
@@ -747,6 +778,20 @@ int bs_queue_load(bs_queue* q, uint64_t key, bs_set_desc* out, void* d_pool, uin
     q->st.bytes_loaded += en.nbytes;
     queue_count_in_flight(q);
     return BS_OK;
+}
+
+int bs_queue_load(bs_queue* q, uint64_t key, bs_set_desc* out, void* d_pool, uint64_t pool_bytes, uint32_t flags,
+                  cudaStream_t consumer)
+{
+    if (out == nullptr) return BS_ERR_ARG;
+    return queue_load_impl(q, key, out, nullptr, d_pool, pool_bytes, flags, consumer);
+}
+
+int bs_queue_load_layered(bs_queue* q, uint64_t key, bs_layered_desc* out, void* d_pool, uint64_t pool_bytes, uint32_t flags,
+                          cudaStream_t consumer)
+{
+    if (out == nullptr) return BS_ERR_ARG;
+    return queue_load_impl(q, key, nullptr, out, d_pool, pool_bytes, flags, consumer);
 }
 
 int bs_queue_checkpoint(bs_queue* q, uint64_t key, cudaStream_t stream)

@@ -166,3 +166,56 @@ def test_adopted_streams_deferred_errors_and_overwrite_behind_a_running_load():
     assert st["status"] == bs.ERR_ARG and st["load"]["status"] == bs.ERR_CORRUPT
     assert (ld3.pool.cpu().numpy() == 0xEE).all()
     q.destroy()
+
+
+def test_layered_sets_and_other_element_types_go_through_the_queue():
+    from oracle import dt, v2
+    from tests.test_gpu_dtype import RawSet
+    from tests.test_gpu_layered import LayeredUp
+    bset = W.make_config("2", n_ops=39)
+    lu = LayeredUp(bset)
+    model = oracle.QueueModel()
+    lv = lu.lv if hasattr(lu, "lv") else W.layered_view(bset)
+    want = model.save_layered(1, lv["structs"], lv["layers"], lv["qn"], lv["dim"], host_addrs(lu.up.host_pool, lu.up.host_offs))
+    assert bytes(want) == bytes(lu.want)
+    c = lu.counts
+    rs = RawSet(W.make_set("dtq", 81, D=120, S=11, M=2, N0=3, n_ops=13, n_site=1, dims="multinomial"), dt.F32, seed=4)
+    q = bs.Queue(max(c[0], c[2], rs.bset.n_tensors), max(c[1], c[3], rs.bset.n_blocks), max(len(want), len(rs.want)),
+                 chunk_bytes=2 * 65536)
+    cs = bs.current_stream()
+    h1, h2 = pinned(len(want)), pinned(len(rs.want))
+    q.save_layered(1, lu.dset.desc, 0, h1.data_ptr(), h1.numel(), cs)             # size predicted by the call
+    q.save(2, rs.dset.desc, len(rs.want), h2.data_ptr(), h2.numel(), cs)
+    na, need = v2.counts(want)
+    out = bs.DeviceLayeredSet.empty(*c, DEV, fill=0xAB)
+    pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    q.load_layered(1, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, cs)        # behind its save: counts remembered by the queue
+    ref32 = dt.deserialize(rs.want)
+    out2 = bs.DeviceSet.empty(rs.bset.n_tensors, rs.bset.n_blocks, DEV, fill=0xAB)
+    pool2 = torch.full((ref32["pool_bytes"],), 0xEE, dtype=torch.uint8, device=DEV)
+    q.load(2, out2.desc, pool2.data_ptr(), ref32["pool_bytes"], bs.LAYOUT_POOL, cs)
+    assert q.wait(1)["status"] == bs.OK and q.wait(2)["status"] == bs.OK
+    torch.cuda.synchronize()
+    assert (h1.numpy() == want).all() and (h2.numpy() == rs.want).all()
+    ref = model.load_layered(1)
+    assert (pool.cpu().numpy() == ref["pool"][:need]).all()
+    h = out.to_host(*c)
+    assert h["structs"].tobytes() == ref["structs"].tobytes() and h["layers"].tobytes() == ref["layers"].tobytes()
+    assert (pool2.cpu().numpy() == ref32["pool"][:ref32["pool_bytes"]]).all()
+    # a key holds a stream of one format
+    with pytest.raises(oracle.OracleError):
+        model.load(1)
+    with pytest.raises(bs.BsError) as e:
+        q.load(1, out2.desc, pool2.data_ptr(), ref32["pool_bytes"], bs.LAYOUT_POOL, cs)
+    assert e.value.code == bs.ERR_ARG
+    with pytest.raises(bs.BsError) as e:
+        q.load_layered(2, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, cs)
+    assert e.value.code == bs.ERR_ARG
+    # an adopted v2 stream is recognised by its version word
+    q.adopt(5, h1.data_ptr(), len(want))
+    pool.fill_(0xEE)
+    q.load_layered(5, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, cs)
+    assert q.wait(5)["status"] == bs.OK
+    torch.cuda.synchronize()
+    assert (pool.cpu().numpy() == ref["pool"][:need]).all()
+    q.destroy()

@@ -88,3 +88,25 @@ def test_a_longer_seeded_sequence_keeps_per_key_program_order():
         live = sum(len(v) for v in last.values())
         peak = max(peak, live)
         assert q.stats()["host_bytes_live"] == live and q.stats()["host_bytes_peak"] == peak
+
+
+def test_layered_streams_share_the_store_but_not_the_load_call():
+    """A key holds a stream of one wire format; the G2 golden v2 stream is what a layered save stores."""
+    from oracle import v2
+    from tests.test_oracle_v2 import GOLD, golden_set as golden_v2
+    gold = read_hex_fixture(GOLD)
+    q = oracle.QueueModel()
+    structs, layers, qn, dim, blocks = golden_v2()
+    addr = np.array([b.ctypes.data for b in blocks], dtype=np.uint64)
+    s = q.save_layered(3, structs, layers, qn, dim, addr)
+    assert bytes(s) == gold and q.stats()["host_bytes_live"] == len(gold) and q.stats()["saves"] == 1
+    got = q.load_layered(3)
+    assert (got["pool"] == v2.deserialize(np.frombuffer(gold, np.uint8))["pool"]).all()
+    with pytest.raises(oracle.OracleError) as e:
+        q.load(3)
+    assert e.value.code == oracle.ERR_ARG
+    t, qn1, dim1, pool, offs = golden_set()
+    q.save(3, t, qn1, dim1, host_addrs(pool.view(np.uint8), offs))      # the key changes format with the save
+    with pytest.raises(oracle.OracleError):
+        q.load_layered(3)
+    assert q.load(3)["pool"].view(np.float64)[0] == 1.0 and q.stats()["loads"] == 2
