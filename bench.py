@@ -496,6 +496,35 @@ def run_mine(args):
             del host2, hosts
         del host
 
+    # ---- library comparator for the pack step (context only): one cudaMemcpyAsync (device to device) per block
+    # over the same block list — the first blocks of the set, up to ~256 MB, into the same stream offsets; no header ----
+    if rank == 0 and not v2 and args.elem == "f64" and not args.no_comparator:
+        try:
+            from workloads.device import memcpy_each
+            sizes = (bset.nelems * 8).astype(np.uint64)
+            stored = (sizes + np.uint64(15)) // np.uint64(16) * np.uint64(16)
+            offs = np.concatenate([[0], np.cumsum(stored)[:-1]]).astype(np.uint64)
+            nb = int(min(bset.n_blocks, max(1, np.searchsorted(np.cumsum(sizes), 256 << 20))))
+            keep = np.nonzero(sizes[:nb])[0]
+            dsts = (np.uint64(stream.data_ptr()) + np.uint64(hb) + offs[:nb])[keep]
+            srcs = addr[:nb][keep]
+            memcpy_each(dsts, srcs, sizes[:nb][keep], cs)
+            torch.cuda.synchronize()
+            t0 = time.time()
+            a.record()
+            memcpy_each(dsts, srcs, sizes[:nb][keep], cs)
+            b.record()
+            torch.cuda.synchronize()
+            wall = time.time() - t0
+            moved = int(sizes[:nb][keep].sum())
+            detail["library_comparator"] = {
+                "what": "one cudaMemcpyAsync (device to device) per block over the first blocks of the set (payload only: no header, "
+                        "no pad zeroing)",
+                "blocks": int(len(keep)), "bytes": moved, "ms": round(wall * 1e3, 3),
+                "hbm_GBs": round(2 * moved / wall / 1e9, 1), "us_per_block": round(wall * 1e6 / len(keep), 2)}
+        except Exception as ex:
+            detail["library_comparator"] = {"error": repr(ex)}
+
     # ---- the small configs are launch-latency bound: report microseconds per call, device-timed back to
     # back, next to a plain copy of the same number of bytes ----
     if rank == 0 and not v2 and args.elem == "f64" and not args.no_small:
@@ -812,6 +841,7 @@ def main():
     ap.add_argument("--standin-items", type=int, default=60000)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-packages", action="store_true")
+    ap.add_argument("--no-comparator", action="store_true", help="skip the one-copy-per-block library comparator of the pack step")
     ap.add_argument("--no-small", action="store_true", help="skip the latency numbers of configs 1 and 2")
     ap.add_argument("--no-queue", action="store_true", help="e2e: offload then prefetch only, no duplex queue leg")
     ap.add_argument("--no-config5", action="store_true")

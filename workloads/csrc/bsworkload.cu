@@ -4,6 +4,7 @@
 // stream busy while the offload engine runs.  Holds none of the serializer's arithmetic.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 namespace {
 
@@ -94,6 +95,17 @@ int wl_contract(const void* d_items, uint32_t n_items, uint32_t grid, cudaStream
     if (grid == 0) grid = 148 * 8;
     contract_kernel<<<grid, 256, 0, stream>>>(reinterpret_cast<const GemmItem*>(d_items), n_items);
     return (int)cudaGetLastError();
+}
+
+// Library comparator for the pack step (context only): one cudaMemcpyAsync (device to device) per block over
+// the same block list; h_dsts / h_srcs / h_sizes are HOST arrays of n entries.  Returns the first cudaError_t.
+int wl_memcpy_each(void** h_dsts, void** h_srcs, size_t* h_sizes, uint64_t n, cudaStream_t stream)
+{
+    for (uint64_t i = 0; i < n; ++i) {
+        cudaError_t e = cudaMemcpyAsync(h_dsts[i], h_srcs[i], h_sizes[i], cudaMemcpyDeviceToDevice, stream);
+        if (e != cudaSuccess) return (int)e;
+    }
+    return 0;
 }
 
 }  // extern "C"

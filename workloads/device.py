@@ -36,6 +36,7 @@ def _L():
         lib = C.CDLL(so)
         lib.wl_fill_blocks.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p]
         lib.wl_contract.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p]
+        lib.wl_memcpy_each.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
         _lib = lib
     return _lib
 
@@ -93,3 +94,12 @@ class StandInContraction:
             rc = _L().wl_contract(self.items.data_ptr(), self.n_items, grid, s)
             if rc:
                 raise RuntimeError(f"wl_contract: cudaError {rc}")
+
+
+def memcpy_each(dsts: np.ndarray, srcs: np.ndarray, sizes: np.ndarray, stream: int) -> None:
+    """One cudaMemcpyAsync (device to device) per entry of the host arrays of device pointers / sizes (uint64): the
+    library comparator of the pack step."""
+    dsts, srcs, sizes = (np.ascontiguousarray(a, dtype=np.uint64) for a in (dsts, srcs, sizes))
+    rc = _L().wl_memcpy_each(dsts.ctypes.data, srcs.ctypes.data, sizes.ctypes.data, len(sizes), stream)
+    if rc:
+        raise RuntimeError(f"cudaMemcpyAsync: cudaError {rc}")
