@@ -64,7 +64,8 @@ enum {
     BS_ERR_CAPACITY = -2,    /* stream / pool / workspace / descriptor arrays too small */
     BS_ERR_CORRUPT = -3,     /* header validation failed; nothing was written */
     BS_ERR_UNSUPPORTED = -4, /* rank not in {2,3}, dtype != f64, n_qn != 2 */
-    BS_ERR_CUDA = -5         /* a CUDA runtime call failed; see bs_last_cuda_error() */
+    BS_ERR_CUDA = -5,        /* a CUDA runtime call failed; see bs_last_cuda_error() */
+    BS_ERR_IO = -6           /* the storage tier of a bs_queue: open / read / write of a file failed (errno is the C library's) */
 };
 
 /* Element type of every block of a set (bs_set_desc.dtype; the header's dtype word).  The path does no arithmetic on the
@@ -408,6 +409,7 @@ typedef struct bs_queue_stats {
     uint64_t device_bytes;             /* staging + workspace + header buffers of both lanes */
     uint32_t in_flight;                /* operations submitted and not yet complete (at the time of the call) */
     uint32_t max_in_flight;
+    uint64_t bytes_spilled, bytes_filled; /* storage tier: stream bytes written to / read from files (completed jobs) */
 } bs_queue_stats;
 
 int bs_queue_create(bs_queue **out, const bs_engine_cfg *lane_cfg); /* both lanes get lane_cfg */
@@ -436,6 +438,25 @@ int bs_queue_query(bs_queue *q, uint64_t key);   /* BS_OK | BS_PENDING | BS_ERR_
 int bs_queue_forget(bs_queue *q, uint64_t key);  /* waits for the key's operations, then drops it: the host buffer is the caller's again */
 int bs_queue_drain(bs_queue *q);                 /* host-blocking: everything submitted so far has completed */
 int bs_queue_get_stats(bs_queue *q, bs_queue_stats *out);
+
+/* ---- the storage tier below pinned host RAM (PAPER §III: saving = serialization, then "writing the serialized data
+ * to a storage media"; L90: "a single CPU thread takes care of saving the serialized data while the remaining CPU
+ * threads ... proceed with subsequent computational tasks"; L144/L202: data spilled to a local disk in the background;
+ * SURVEY §8(f) NEXT-4).  The queue owns ONE host IO thread (started by the first call); jobs run in submission order.
+ *   bs_queue_spill   : once the save of `key` has completed, write its stream to the file `path` (created / truncated).
+ *                      Returns at once.  The key stays loadable from host RAM; after bs_queue_io_wait + bs_queue_forget the
+ *                      host buffer is the caller's again and the file is the only copy.
+ *   bs_queue_fill    : read the file `path` (a stream written by bs_queue_spill, either wire format) into h_pinned and
+ *                      register it under `key` (as bs_queue_adopt).  Returns at once; BS_ERR_CAPACITY if the file is larger
+ *                      than h_capacity, BS_ERR_IO if it cannot be opened.  A bs_queue_load of the key submitted before the
+ *                      read has finished BLOCKS THE HOST until it has (the "fetching" stall of L132) — a DMA cannot wait
+ *                      for a host thread.
+ *   bs_queue_io_wait : host-blocking; the outcome of the key's last storage job (BS_OK | BS_ERR_IO), the bytes it moved and
+ *                      the seconds its reads / writes took.
+ * A save over a key, bs_queue_forget and bs_queue_destroy wait for the key's pending storage job (its buffer is in use). */
+int bs_queue_spill(bs_queue *q, uint64_t key, const char *path);
+int bs_queue_fill(bs_queue *q, uint64_t key, const char *path, void *h_pinned, uint64_t h_capacity);
+int bs_queue_io_wait(bs_queue *q, uint64_t key, uint64_t *bytes, double *seconds);
 
 int bs_ticket_wait(bs_ticket *t, bs_ticket_stats *stats /* may be NULL */); /* blocks the host; returns the deferred status */
 int bs_ticket_query(const bs_ticket *t);                                   /* BS_OK | BS_PENDING | BS_ERR_* */

@@ -19,6 +19,9 @@ in time on the GPU, what a user may observe is fixed by PROGRAM ORDER, and that 
   load_layered(key)     the same for a key that holds a v2 stream; a key holds a stream of ONE format, asking for the
                         other is ERR_ARG
   forget(key)           the store drops `key`
+  spill(key, path)      the file `path` holds exactly the bytes of the stream stored under `key` (saving =
+                        serialization, then "writing the serialized data to a storage media"); the key stays in the store
+  fill(key, path)       the store holds the bytes of the file under `key` (as adopt); a missing file is ERR_IO (-6)
   accounting            host_bytes_live = sum of the stored streams' lengths; host_bytes_peak = its maximum over the
                         calls so far; saves / loads = number of accepted calls; bytes_saved / bytes_loaded = stream
                         bytes moved by them
@@ -42,6 +45,7 @@ class QueueModel:
         self.saves = self.loads = 0
         self.bytes_saved = self.bytes_loaded = 0
         self.host_bytes_peak = 0
+        self.bytes_spilled = self.bytes_filled = 0
 
     @property
     def host_bytes_live(self) -> int:
@@ -96,6 +100,24 @@ class QueueModel:
         if int(key) not in self.store:
             raise _v1.OracleError(_v1.ERR_ARG, "queue forget: unknown key")
         del self.store[int(key)]
+
+    def spill(self, key: int, path: str) -> int:
+        if int(key) not in self.store:
+            raise _v1.OracleError(_v1.ERR_ARG, "queue spill: unknown key")
+        with open(path, "wb") as f:
+            f.write(self.store[int(key)].tobytes())
+        self.bytes_spilled += len(self.store[int(key)])
+        return len(self.store[int(key)])
+
+    def fill(self, key: int, path: str) -> int:
+        try:
+            with open(path, "rb") as f:
+                raw = f.read()
+        except OSError:
+            raise _v1.OracleError(-6, "queue fill: cannot read the file")
+        self.adopt(key, np.frombuffer(raw, np.uint8))
+        self.bytes_filled += len(raw)
+        return len(raw)
 
     def stats(self) -> dict:
         return dict(saves=self.saves, loads=self.loads, bytes_saved=self.bytes_saved, bytes_loaded=self.bytes_loaded,

@@ -9,7 +9,7 @@ import os
 from . import build as _build
 
 OK, PENDING = 0, 1
-ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_UNSUPPORTED, ERR_CUDA = -1, -2, -3, -4, -5
+ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_UNSUPPORTED, ERR_CUDA, ERR_IO = -1, -2, -3, -4, -5, -6
 F64, F32, C64, C128 = 0, 1, 2, 3
 LAYOUT_POOL, SCATTER_TO_ADDR = 0, 1
 VARIANT_DEFAULT, VARIANT_LDG, VARIANT_TMA = 0, 1, 2
@@ -91,7 +91,8 @@ class TicketStats(C.Structure):
 class QueueStats(C.Structure):
     _fields_ = [("saves", C.c_uint64), ("loads", C.c_uint64), ("bytes_saved", C.c_uint64), ("bytes_loaded", C.c_uint64),
                 ("host_bytes_live", C.c_uint64), ("host_bytes_peak", C.c_uint64), ("keys_live", C.c_uint64),
-                ("device_bytes", C.c_uint64), ("in_flight", C.c_uint32), ("max_in_flight", C.c_uint32)]
+                ("device_bytes", C.c_uint64), ("in_flight", C.c_uint32), ("max_in_flight", C.c_uint32),
+                ("bytes_spilled", C.c_uint64), ("bytes_filled", C.c_uint64)]
 
 
 assert C.sizeof(TensorRec) == 32 and C.sizeof(Result) == 64 and C.sizeof(StructRec) == 32 and C.sizeof(LayerRec) == 16
@@ -166,6 +167,9 @@ def lib():
     L.bs_queue_forget.argtypes = [vp, u64]
     L.bs_queue_drain.argtypes = [vp]
     L.bs_queue_get_stats.argtypes = [vp, C.POINTER(QueueStats)]
+    L.bs_queue_spill.argtypes = [vp, u64, C.c_char_p]
+    L.bs_queue_fill.argtypes = [vp, u64, C.c_char_p, vp, u64]
+    L.bs_queue_io_wait.argtypes = [vp, u64, pu64, C.POINTER(C.c_double)]
     L.bs_ticket_wait.argtypes = [vp, C.POINTER(TicketStats)]
     L.bs_ticket_query.argtypes = [vp]
     L.bs_ticket_destroy.argtypes = [vp]
@@ -470,6 +474,19 @@ class Queue:
     def forget(self, key: int) -> None:
         _check(lib().bs_queue_forget(self._h, key), "bs_queue_forget")
         self._keys.discard(key)
+
+    def spill(self, key: int, path: str) -> None:
+        _check(lib().bs_queue_spill(self._h, key, os.fsencode(path)), "bs_queue_spill")
+
+    def fill(self, key: int, path: str, h_pinned_ptr: int, h_capacity: int) -> None:
+        _check(lib().bs_queue_fill(self._h, key, os.fsencode(path), h_pinned_ptr, h_capacity), "bs_queue_fill")
+        self._keys.add(key)
+
+    def io_wait(self, key: int) -> dict:
+        """Host-blocking: outcome of the key's last storage job (no exception for BS_ERR_IO)."""
+        n, sec = C.c_uint64(0), C.c_double(0.0)
+        rc = lib().bs_queue_io_wait(self._h, key, C.byref(n), C.byref(sec))
+        return dict(status=int(rc), bytes=int(n.value), seconds=float(sec.value))
 
     def drain(self) -> None:
         _check(lib().bs_queue_drain(self._h), "bs_queue_drain")

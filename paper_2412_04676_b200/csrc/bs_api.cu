@@ -208,6 +208,7 @@ const char* bs_strerror(int code)
         case BS_ERR_CORRUPT: return "corrupt stream header";
         case BS_ERR_UNSUPPORTED: return "unsupported rank, dtype or label count";
         case BS_ERR_CUDA: return "CUDA runtime error";
+        case BS_ERR_IO: return "file IO error in the storage tier";
         default: return "unknown error";
     }
 }

@@ -14,8 +14,19 @@
 #include <new>
 #include <string.h>
 
+#include <fcntl.h>
+#include <sys/stat.h>
+#include <unistd.h>
+
 #include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <condition_variable>
+#include <deque>
+#include <memory>
 #include <mutex>
+#include <string>
+#include <thread>
 #include <unordered_map>
 #include <vector>
 
@@ -564,8 +575,31 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
 
 // ==== save / load queue with checkpoints (bs.h "queue") ===============================================
 // Two engines (one per PCIe direction) + a key table.  Ordering between the lanes is by CUDA events only.
+// one job of the queue's host IO thread (the storage tier; bs.h)
+struct IoJob {
+    bool spill = true;             // else fill
+    std::string path;
+    unsigned char* h = nullptr;
+    uint64_t nbytes = 0;
+    cudaEvent_t after = nullptr;   // spill: recorded behind the save's last DMA; the thread waits for it
+    int status = BS_OK;
+    uint64_t bytes = 0;
+    double seconds = 0.0;
+    bool done = false;             // under IoThread::m
+    bool counted = false;
+};
+struct IoThread {
+    std::thread th;
+    std::mutex m;
+    std::condition_variable cv, cv_done;
+    std::deque<std::shared_ptr<IoJob>> jobs;
+    bool stop = false;
+    int device = 0;
+};
+
 struct bs_queue {
     struct Entry {
+        std::shared_ptr<IoJob> io;  // last storage job of the key
         bs_ticket* save = nullptr;  // last save / last load of the key (each lane is in order, so the last one covers all)
         bs_ticket* load = nullptr;
         const void* h = nullptr;
@@ -580,7 +614,93 @@ struct bs_queue {
     std::unordered_map<uint64_t, Entry> keys;
     std::vector<bs_ticket*> retired;  // replaced tickets, destroyed once complete
     bs_queue_stats st;
+    IoThread* io = nullptr;
 };
+
+// ---- the host IO thread ------------------------------------------------------------------------------------------
+static void io_run(IoJob& j)
+{
+    constexpr size_t kPiece = 64u << 20;
+    if (j.after) cudaEventSynchronize(j.after);  // the stream has landed in the host buffer
+    const auto t0 = std::chrono::steady_clock::now();
+    const int fd = j.spill ? open(j.path.c_str(), O_WRONLY | O_CREAT | O_TRUNC, 0644) : open(j.path.c_str(), O_RDONLY);
+    if (fd < 0) { j.status = BS_ERR_IO; return; }
+    uint64_t pos = 0;
+    while (pos < j.nbytes) {
+        const size_t want = (size_t)std::min<uint64_t>(kPiece, j.nbytes - pos);
+        const ssize_t got = j.spill ? write(fd, j.h + pos, want) : read(fd, j.h + pos, want);
+        if (got <= 0) { j.status = BS_ERR_IO; break; }
+        pos += (uint64_t)got;
+    }
+    if (close(fd) != 0 && j.spill) j.status = BS_ERR_IO;
+    j.bytes = pos;
+    j.seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+}
+
+static void io_loop(IoThread* t)
+{
+    cudaSetDevice(t->device);
+    for (;;) {
+        std::shared_ptr<IoJob> j;
+        {
+            std::unique_lock<std::mutex> lk(t->m);
+            t->cv.wait(lk, [&] { return t->stop || !t->jobs.empty(); });
+            if (t->jobs.empty()) return;  // stop requested and nothing left
+            j = t->jobs.front();
+            t->jobs.pop_front();
+        }
+        io_run(*j);
+        {
+            std::lock_guard<std::mutex> lk(t->m);
+            j->done = true;
+        }
+        t->cv_done.notify_all();
+    }
+}
+
+static int io_submit(bs_queue* q, const std::shared_ptr<IoJob>& j)
+{
+    if (q->io == nullptr) {
+        IoThread* t = new (std::nothrow) IoThread;
+        if (!t) return BS_ERR_ARG;
+        if (cudaGetDevice(&t->device) != cudaSuccess) { delete t; return BS_ERR_CUDA; }
+        t->th = std::thread(io_loop, t);
+        q->io = t;
+    }
+    {
+        std::lock_guard<std::mutex> lk(q->io->m);
+        q->io->jobs.push_back(j);
+    }
+    q->io->cv.notify_one();
+    return BS_OK;
+}
+
+static void io_wait(bs_queue* q, const std::shared_ptr<IoJob>& j)  // host-blocking; accounts the job once
+{
+    if (!j || q->io == nullptr) return;
+    {
+        std::unique_lock<std::mutex> lk(q->io->m);
+        q->io->cv_done.wait(lk, [&] { return j->done; });
+    }
+    if (!j->counted) {
+        j->counted = true;
+        if (j->after) { cudaEventDestroy(j->after); j->after = nullptr; }
+        if (j->status == BS_OK) (j->spill ? q->st.bytes_spilled : q->st.bytes_filled) += j->bytes;
+    }
+}
+
+static void io_shutdown(bs_queue* q)
+{
+    if (q->io == nullptr) return;
+    {
+        std::lock_guard<std::mutex> lk(q->io->m);
+        q->io->stop = true;
+    }
+    q->io->cv.notify_all();
+    q->io->th.join();
+    delete q->io;
+    q->io = nullptr;
+}
 
 static uint64_t engine_device_bytes(const bs_engine* e)
 {
@@ -668,6 +788,8 @@ int bs_queue_destroy(bs_queue* q)
 {
     if (q == nullptr) return BS_ERR_ARG;
     bs_queue_drain(q);
+    for (auto& kv : q->keys) io_wait(q, kv.second.io);
+    io_shutdown(q);
     for (auto& kv : q->keys) {
         if (kv.second.save) bs_ticket_destroy(kv.second.save);
         if (kv.second.load) bs_ticket_destroy(kv.second.load);
@@ -685,6 +807,7 @@ static int queue_save_impl(bs_queue* q, uint64_t key, const bs_set_desc* set, co
     queue_reap(q, false);
     int rc;
     auto it = q->keys.find(key);
+    if (it != q->keys.end()) io_wait(q, it->second.io);  // a storage job may still be reading / filling the key's buffer
     // the host buffer may still be read by a load of this key (or, for a new buffer under the same key, nothing to wait for)
     if (it != q->keys.end() && it->second.load && !ticket_complete(it->second.load))
         if ((rc = engine_wait_ticket(q->lane_save, it->second.load))) return rc;
@@ -740,6 +863,7 @@ int bs_queue_adopt(bs_queue* q, uint64_t key, const void* h_pinned, uint64_t nby
     queue_reap(q, false);
     auto it = q->keys.find(key);
     if (it != q->keys.end()) {  // the old buffer's operations are not ours to order against the new one: finish them
+        io_wait(q, it->second.io);
         int rc = bs_queue_wait(q, key, nullptr, nullptr);
         (void)rc;
         queue_retire(q, it->second.save);
@@ -764,6 +888,13 @@ static int queue_load_impl(bs_queue* q, uint64_t key, bs_set_desc* out, bs_layer
     auto it = q->keys.find(key);
     if (it == q->keys.end()) return BS_ERR_ARG;
     bs_queue::Entry& en = it->second;
+    if (en.io && !en.io->spill) {  // the stream is still being read from its file: the host waits ("fetching", L132)
+        io_wait(q, en.io);
+        if (en.io->status != BS_OK) return BS_ERR_IO;
+        uint32_t version = 0;
+        memcpy(&version, (const unsigned char*)en.h + 8, 4);
+        en.layered = version == 2u;
+    }
     if (en.layered != (lout != nullptr)) return BS_ERR_ARG;  // the key holds a stream of the other wire format
     int rc;
     if (en.save && !ticket_complete(en.save))  // the stream is still on its way to the host buffer
@@ -834,12 +965,80 @@ int bs_queue_forget(bs_queue* q, uint64_t key)
     if (q == nullptr) return BS_ERR_ARG;
     auto it = q->keys.find(key);
     if (it == q->keys.end()) return BS_ERR_ARG;
+    io_wait(q, it->second.io);
     if (it->second.save) bs_ticket_destroy(it->second.save);  // waits for completion
     if (it->second.load) bs_ticket_destroy(it->second.load);
     q->keys.erase(it);
     queue_account_host(q);
     queue_count_in_flight(q);
     return BS_OK;
+}
+
+int bs_queue_spill(bs_queue* q, uint64_t key, const char* path)
+{
+    if (q == nullptr || path == nullptr) return BS_ERR_ARG;
+    auto it = q->keys.find(key);
+    if (it == q->keys.end()) return BS_ERR_ARG;
+    bs_queue::Entry& en = it->second;
+    io_wait(q, en.io);
+    auto j = std::make_shared<IoJob>();
+    j->spill = true;
+    j->path = path;
+    j->h = (unsigned char*)const_cast<void*>(en.h);
+    j->nbytes = en.nbytes;
+    if (en.save) {  // behind the save's last DMA (the save lane is in order)
+        CK(cudaEventCreateWithFlags(&j->after, cudaEventDisableTiming));
+        CK(cudaEventRecord(j->after, q->lane_save->cstream));
+    }
+    int rc = io_submit(q, j);
+    if (rc) return rc;
+    en.io = j;
+    return BS_OK;
+}
+
+int bs_queue_fill(bs_queue* q, uint64_t key, const char* path, void* h_pinned, uint64_t h_capacity)
+{
+    if (q == nullptr || path == nullptr || h_pinned == nullptr) return BS_ERR_ARG;
+    struct stat sb;
+    if (stat(path, &sb) != 0) return BS_ERR_IO;
+    if ((uint64_t)sb.st_size > h_capacity) return BS_ERR_CAPACITY;
+    if ((uint64_t)sb.st_size < kFixedHeader) return BS_ERR_CORRUPT;
+    auto it = q->keys.find(key);
+    if (it != q->keys.end()) {  // as bs_queue_adopt: finish what still uses the old buffer
+        io_wait(q, it->second.io);
+        bs_queue_wait(q, key, nullptr, nullptr);
+        queue_retire(q, it->second.save);
+        queue_retire(q, it->second.load);
+    }
+    auto j = std::make_shared<IoJob>();
+    j->spill = false;
+    j->path = path;
+    j->h = (unsigned char*)h_pinned;
+    j->nbytes = (uint64_t)sb.st_size;
+    int rc = io_submit(q, j);
+    if (rc) return rc;
+    bs_queue::Entry& en = q->keys[key];
+    en.h = h_pinned;
+    en.nbytes = (uint64_t)sb.st_size;
+    en.adopted = true;
+    en.layered = false;  // settled from the version word once the file is in
+    en.io = j;
+    queue_account_host(q);
+    return BS_OK;
+}
+
+int bs_queue_io_wait(bs_queue* q, uint64_t key, uint64_t* bytes, double* seconds)
+{
+    if (q == nullptr) return BS_ERR_ARG;
+    auto it = q->keys.find(key);
+    if (it == q->keys.end()) return BS_ERR_ARG;
+    if (bytes) *bytes = 0;
+    if (seconds) *seconds = 0.0;
+    if (!it->second.io) return BS_OK;
+    io_wait(q, it->second.io);
+    if (bytes) *bytes = it->second.io->bytes;
+    if (seconds) *seconds = it->second.io->seconds;
+    return it->second.io->status;
 }
 
 int bs_queue_get_stats(bs_queue* q, bs_queue_stats* out)

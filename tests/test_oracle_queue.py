@@ -110,3 +110,23 @@ def test_layered_streams_share_the_store_but_not_the_load_call():
     with pytest.raises(oracle.OracleError):
         q.load_layered(3)
     assert q.load(3)["pool"].view(np.float64)[0] == 1.0 and q.stats()["loads"] == 2
+
+
+def test_spill_and_fill_are_the_stream_bytes_in_a_file(tmp_path):
+    """PAPER L85 step (2): the file holds exactly the serialized bytes; reading it back is an adopted stream."""
+    gold = read_hex_fixture(os.path.join(HERE, "golden", "p7_golden_stream.hex"))
+    q = oracle.QueueModel()
+    t, qn, dim, pool, offs = golden_set()
+    q.save(7, t, qn, dim, host_addrs(pool.view(np.uint8), offs))
+    path = str(tmp_path / "block7.bs")
+    assert q.spill(7, path) == 288 and open(path, "rb").read() == gold
+    q.forget(7)
+    assert q.stats()["host_bytes_live"] == 0
+    assert q.fill(9, path) == 288 and q.stats()["host_bytes_live"] == 288
+    assert list(q.load(9)["pool"].view(np.float64)[32:34]) == [2.0, 3.0]
+    assert (q.bytes_spilled, q.bytes_filled) == (288, 288)
+    with pytest.raises(oracle.OracleError) as e:
+        q.fill(1, str(tmp_path / "missing.bs"))
+    assert e.value.code == -6
+    with pytest.raises(oracle.OracleError):
+        q.spill(1, path)
