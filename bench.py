@@ -812,6 +812,26 @@ def config5(args, dev, opts):
                              "exposed_io_frac_queue_without_ends": round(max(0.0, t_async - n_steps * tc_step - io_ms - pio_ms) / t_async, 4),
                              "note": "the first load and the last save of a sweep have no compute to hide behind (ends_ms = one "
                                      "save alone + one load alone)"}
+        # ---- the storage tier (PAPER L85 step (2): the stream goes on to a file; context for the paper's 2.15 GB/s
+        # synchronous save and 1.12 GB/s per-SSD write, L154 / L168): whatever disk this box has under the temp dir ----
+        try:
+            import tempfile
+            with tempfile.TemporaryDirectory() as td:
+                path = os.path.join(td, "block.bs")
+                q.save(0, dset.desc, total, hosts[0].data_ptr(), total, cs)
+                q.spill(0, path)
+                sp = q.io_wait(0)
+                q.fill(9, path, hosts[1].data_ptr(), total)
+                fl = q.io_wait(9)
+                q.load(9, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, cs)
+                ok = q.wait(9)["status"] == 0 and sp["status"] == 0 and fl["status"] == 0
+                res["storage_tier"] = {"ok": bool(ok), "bytes": int(sp["bytes"]),
+                                       "spill_write_GBs": round(sp["bytes"] / max(sp["seconds"], 1e-9) / 1e9, 2),
+                                       "fill_read_GBs_page_cache_warm": round(fl["bytes"] / max(fl["seconds"], 1e-9) / 1e9, 2),
+                                       "note": "one host IO thread, plain write() / read() in 64 MiB pieces, no fsync; the file "
+                                               "was just written, so the read comes from the page cache"}
+        except Exception as ex:
+            res["storage_tier"] = {"error": repr(ex)}
         q.destroy()
     except Exception as ex:
         res["sweep_fig3"] = {"error": repr(ex)}
