@@ -148,7 +148,17 @@ int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_sr
 }
 
 // the whole stream <-> package slots in one launch each (bs.h "packages"; PkgMap in bs_internal.cuh)
+int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, const bs_opts& o,
+                            int sms, cudaStream_t stream);
+
 int run_pack_packages(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, const bs_opts& o, int sms, cudaStream_t stream)
+{
+    return run_pack_packages_range(set, L, pm, 0, UINT64_MAX, o, sms, stream);
+}
+
+// stream bytes [lo, hi) (whole packages of the cut) -> their slots
+int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, const bs_opts& o,
+                            int sms, cudaStream_t stream)
 {
     MoveParams mp;
     memset(&mp, 0, sizeof(mp));
@@ -157,8 +167,8 @@ int run_pack_packages(const bs_set_desc* set, const WsLayout& L, const PkgMap& p
     mp.qn = set->qn;
     mp.dim = set->dim;
     mp.addr = set->addr;
-    mp.lo = 0;
-    mp.hi = UINT64_MAX;
+    mp.lo = lo;
+    mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
     mp.pkg = pm;

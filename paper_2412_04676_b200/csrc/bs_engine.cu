@@ -33,6 +33,8 @@ int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t n
                          int sms, cudaStream_t stream);
 int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header,
                      uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream);
+int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, const bs_opts& o,
+                            int sms, cudaStream_t stream);
 // wire format v2 (bs_layered.cu)
 int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t capacity,
                                uint64_t expect_total, bs_result* d_result, int sms, cudaStream_t stream);
@@ -432,19 +434,47 @@ int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t tot
     CK(cudaStreamWaitEvent(e->kstream, e->ev_dep, 0));
     CK(cudaEventRecord(t->t_begin, e->kstream));
     if ((rc = run_serialize_scan(set, L, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream))) return rc;
-    for (uint64_t k = 0; k < count; ++k) {
-        const uint32_t b = (uint32_t)(k % S);
-        uint64_t lo = 0, hi = 0;
-        pkg_range(hb, total_bytes, cap, k, &lo, &hi);
-        if (k >= S) CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));  // staging[b] drained by DMA k-S
-        CK(launch_pkg_header(L, cap, stream_id, k, count, e->staging[b], e->d_result, e->kstream));
-        if ((rc = run_pack_range(set, L, e->staging[b] + BS_PKG_HEADER, lo, hi, e->opts, e->sms, e->kstream))) return rc;
-        if (k == 0) CK(post_result(t->h_result, e->d_result, e->kstream));
+    // A staging buffer takes a BATCH of packages laid out as slots, and the batch leaves in ONE DMA, when the slots are
+    // exactly header + limit long and the batch's host slots are consecutive; a short package (the last one of the header
+    // region / of the payload) ends its batch, so no byte behind a short package is written on the host.
+    const bool can_batch = slot_bytes == BS_PKG_HEADER + cap;
+    // no work tile straddles a package when the limit is a multiple of the tile (bs_pkg.cu): then the move kernel takes a
+    // package map and a whole batch costs two launches
+    const bool one_launch = can_batch && cap % (e->opts.tile_bytes ? e->opts.tile_bytes : kGranule) == 0;
+    const uint64_t per_buf = can_batch ? std::max<uint64_t>(1, e->cfg.chunk_bytes / slot_bytes) : 1;
+    auto slot_of = [&](uint64_t k) { return h_slot_of ? (uint64_t)h_slot_of[k] : k; };
+    uint64_t batch = 0;
+    for (uint64_t k = 0; k < count; ++batch) {
+        const uint32_t b = (uint32_t)(batch % S);
+        if (batch >= S) CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));  // staging[b] drained by the DMA of batch - S
+        uint64_t m = 0, last_bytes = 0, lo0 = 0, hi1 = 0;
+        const uint64_t k0 = k;
+        for (; k < count && m < per_buf; ++k, ++m) {
+            if (m > 0 && slot_of(k) != slot_of(k - 1) + 1) break;  // the host slots of a batch are consecutive
+            uint64_t lo = 0, hi = 0;
+            pkg_range(hb, total_bytes, cap, k, &lo, &hi);
+            if (m == 0) lo0 = lo;
+            hi1 = hi;
+            if (!one_launch) {
+                unsigned char* dst = e->staging[b] + m * slot_bytes;
+                CK(launch_pkg_header(L, cap, stream_id, k, count, dst, e->d_result, e->kstream));
+                if ((rc = run_pack_range(set, L, dst + BS_PKG_HEADER, lo, hi, e->opts, e->sms, e->kstream))) return rc;
+            }
+            last_bytes = hi - lo;
+            if (last_bytes != cap) { ++k; ++m; break; }  // a short package ends its batch
+        }
+        if (one_launch) {  // the batch's headers in one launch, its stream range [lo0, hi1) in one more
+            CK(launch_pkg_headers(L, cap, stream_id, k0, m, count, e->staging[b], slot_bytes, nullptr, e->d_result, e->kstream));
+            PkgMap pm;
+            pm.cap = cap; pm.slot_bytes = slot_bytes; pm.base = e->staging[b]; pm.slot_of = nullptr; pm.k_base = k0;
+            if ((rc = run_pack_packages_range(set, L, pm, lo0, hi1, e->opts, e->sms, e->kstream))) return rc;
+        }
+        if (k0 == 0) CK(post_result(t->h_result, e->d_result, e->kstream));
         CK(cudaEventRecord(e->ev_k[b], e->kstream));
         CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));
-        if (k == 0) CK(cudaEventRecord(t->dma_begin, e->cstream));
-        unsigned char* slot = (unsigned char*)h_slots + (h_slot_of ? (uint64_t)h_slot_of[k] : k) * slot_bytes;
-        CK(cudaMemcpyAsync(slot, e->staging[b], BS_PKG_HEADER + (hi - lo), cudaMemcpyDeviceToHost, e->cstream));
+        if (k0 == 0) CK(cudaEventRecord(t->dma_begin, e->cstream));
+        CK(cudaMemcpyAsync((unsigned char*)h_slots + slot_of(k0) * slot_bytes, e->staging[b],
+                           (m - 1) * slot_bytes + BS_PKG_HEADER + last_bytes, cudaMemcpyDeviceToHost, e->cstream));
         CK(cudaEventRecord(e->ev_c[b], e->cstream));
     }
     CK(cudaEventRecord(t->dma_end, e->cstream));
@@ -508,18 +538,29 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
     if ((rc = run_unpack_range(out, L, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream))) return rc;
     std::vector<PkgItem> by_slot(plan.items.begin() + plan.n_header, plan.items.end());
     std::sort(by_slot.begin(), by_slot.end(), [](const PkgItem& a, const PkgItem& b) { return a.slot < b.slot; });
-    uint32_t k = 0;
-    for (const PkgItem& it : by_slot) {  // arrival order: each payload package is DMA'd and unpacked on its own
-        const uint32_t b = k % S;
-        if (k >= S) CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));  // staging[b] consumed by unpack k-S
-        CK(cudaMemcpyAsync(e->staging[b], slots + it.slot * slot_bytes + BS_PKG_HEADER, it.nbytes, cudaMemcpyHostToDevice, e->cstream));
+    // arrival order: each payload package is unpacked on its own; runs of consecutive slots that fit a staging buffer
+    // come over in ONE DMA (what lies behind a short package inside the run is read and ignored)
+    const uint64_t per_buf = std::max<uint64_t>(1, e->cfg.chunk_bytes / slot_bytes);
+    uint64_t batch = 0;
+    for (size_t i = 0; i < by_slot.size(); ++batch) {
+        const uint32_t b = (uint32_t)(batch % S);
+        size_t n = 1;
+        while (i + n < by_slot.size() && n < per_buf && by_slot[i + n].slot == by_slot[i + n - 1].slot + 1) ++n;
+        if (batch >= S) CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));  // staging[b] consumed by the unpacks of batch - S
+        const uint64_t bytes = n == 1 ? by_slot[i].nbytes : (n - 1) * slot_bytes + BS_PKG_HEADER + by_slot[i + n - 1].nbytes;
+        const unsigned char* src = slots + by_slot[i].slot * slot_bytes + (n == 1 ? BS_PKG_HEADER : 0);
+        CK(cudaMemcpyAsync(e->staging[b], src, bytes, cudaMemcpyHostToDevice, e->cstream));
         CK(cudaEventRecord(e->ev_c[b], e->cstream));
         CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));
-        if ((rc = run_unpack_range(out, L, e->staging[b], nullptr, it.lo, it.lo + it.nbytes, flags | kFlagCheckPad, e->opts, e->sms,
-                                   e->kstream)))
-            return rc;
+        for (size_t j = 0; j < n; ++j) {
+            const PkgItem& it = by_slot[i + j];
+            const unsigned char* d = e->staging[b] + (n == 1 ? 0 : j * slot_bytes + BS_PKG_HEADER);
+            if ((rc = run_unpack_range(out, L, d, nullptr, it.lo, it.lo + it.nbytes, flags | kFlagCheckPad, e->opts, e->sms,
+                                       e->kstream)))
+                return rc;
+        }
         CK(cudaEventRecord(e->ev_k[b], e->kstream));
-        ++k;
+        i += n;
     }
     CK(cudaEventRecord(t->dma_end, e->cstream));
     CK(post_status(t->h_result, &((WsHead*)e->ws)->status, e->kstream));

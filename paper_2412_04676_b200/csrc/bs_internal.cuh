@@ -135,6 +135,7 @@ struct PkgMap {
     uint64_t slot_bytes;
     unsigned char* base;
     const uint32_t* slot_of;
+    uint64_t k_base;  // without a slot table: package k lies in slot k - k_base (a batch of packages in a staging buffer)
 };
 
 // ---- data movement (S3, S5 / S7): stream bytes [lo,hi) <-> blocks ------------------------------------------
@@ -168,7 +169,7 @@ __device__ __forceinline__ unsigned char* stream_at(const MoveParams& p, uint64_
         k = (hb + p.pkg.cap - 1) / p.pkg.cap + j;
         within = x - j * p.pkg.cap;
     }
-    const uint64_t slot = p.pkg.slot_of ? (uint64_t)__ldg(p.pkg.slot_of + k) : k;
+    const uint64_t slot = p.pkg.slot_of ? (uint64_t)__ldg(p.pkg.slot_of + k) : k - p.pkg.k_base;
     return p.pkg.base + slot * p.pkg.slot_bytes + 64 + within;
 }
 

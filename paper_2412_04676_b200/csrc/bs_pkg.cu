@@ -98,12 +98,13 @@ __global__ void pkg_header_kernel(WsLayout ws, uint64_t cap, uint64_t stream_id,
 }
 
 // one thread per package: every header of the cut -> its slot (slot_of: device table index -> slot, or identity)
-__global__ void pkg_headers_kernel(WsLayout ws, uint64_t cap, uint64_t stream_id, uint64_t count, unsigned char* base,
-                                   uint64_t slot_bytes, const uint32_t* slot_of, bs_result* result)
+__global__ void pkg_headers_kernel(WsLayout ws, uint64_t cap, uint64_t stream_id, uint64_t first, uint64_t n, uint64_t count,
+                                   unsigned char* base, uint64_t slot_bytes, const uint32_t* slot_of, bs_result* result)
 {
-    const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= count) return;
-    const uint64_t slot = slot_of ? (uint64_t)slot_of[k] : k;
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint64_t k = first + i;  // packages [first, first + n) of the cut; without a table they lie in slots 0 .. n-1
+    const uint64_t slot = slot_of ? (uint64_t)slot_of[k] : i;
     pkg_write_header(ws, cap, stream_id, k, count, base + slot * slot_bytes, result);
 }
 
@@ -174,6 +175,15 @@ cudaError_t launch_pkg_header(const WsLayout& L, uint64_t cap, uint64_t stream_i
                               void* d_dst, bs_result* d_result, cudaStream_t stream)
 {
     pkg_header_kernel<<<1, 32, 0, stream>>>(L, cap, stream_id, k, expect_count, (unsigned char*)d_dst, d_result);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pkg_headers(const WsLayout& L, uint64_t cap, uint64_t stream_id, uint64_t first, uint64_t n, uint64_t count,
+                               void* d_base, uint64_t slot_bytes, const uint32_t* d_slot_of, bs_result* d_result, cudaStream_t stream)
+{
+    if (n == 0) return cudaSuccess;
+    pkg_headers_kernel<<<(unsigned)((n + 127) / 128), 128, 0, stream>>>(L, cap, stream_id, first, n, count, (unsigned char*)d_base,
+                                                                         slot_bytes, d_slot_of, d_result);
     return cudaGetLastError();
 }
 
@@ -330,11 +340,9 @@ int bs_package_emit(const bs_set_desc* set, uint64_t total_bytes, uint64_t cap, 
             }
             CK(cudaMemcpyAsync(d_tab, h_slot_of, count * sizeof(uint32_t), cudaMemcpyHostToDevice, stream));
         }
-        pkg_headers_kernel<<<(unsigned)((count + 127) / 128), 128, 0, stream>>>(L, cap, stream_id, count, (unsigned char*)d_slots,
-                                                                                 slot_bytes, d_tab, d_result);
-        CK(cudaGetLastError());
+        CK(launch_pkg_headers(L, cap, stream_id, 0, count, count, d_slots, slot_bytes, d_tab, d_result, stream));
         PkgMap pm;
-        pm.cap = cap; pm.slot_bytes = slot_bytes; pm.base = (unsigned char*)d_slots; pm.slot_of = d_tab;
+        pm.cap = cap; pm.slot_bytes = slot_bytes; pm.base = (unsigned char*)d_slots; pm.slot_of = d_tab; pm.k_base = 0;
         rc = run_pack_packages(set, L, pm, o, sms, stream);
         if (tab_owned) CK(cudaFreeAsync(d_tab, stream));
         return rc;
@@ -410,7 +418,7 @@ int bs_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t n_slots
         CK(launch_pkg_check(L, d_slots, slot_bytes, n_slots, stream_id, d_result, stream));
         if ((rc = run_unpack_range(out, L, d_header, d_header, 0, 0, flags, o, sms, stream))) return rc;  // descriptor rebuild
         PkgMap pm;
-        pm.cap = cut; pm.slot_bytes = slot_bytes; pm.base = const_cast<unsigned char*>(slots); pm.slot_of = d_tab;
+        pm.cap = cut; pm.slot_bytes = slot_bytes; pm.base = const_cast<unsigned char*>(slots); pm.slot_of = d_tab; pm.k_base = 0;
         if ((rc = run_unpack_packages(out, L, pm, plan.hb, flags | kFlagCheckPad, o, sms, stream))) return rc;
         if (d_result != nullptr)
             CK(cudaMemcpyAsync(&d_result->status, &L.head->status, sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));

@@ -321,3 +321,33 @@ def test_engine_offload_packages_then_prefetch_them_in_any_order(cap, chunk, n_s
                                    bs.current_stream())
     assert e.value.code in (bs.ERR_CAPACITY, bs.ERR_ARG)
     eng.destroy()
+
+
+@pytest.mark.parametrize("cap,chunk,n_staging", [(32768, 5 * 65536, 2), (16384, 65536, 3), (49152, 8 * 65536, 1), (32768 + 16, 4 * 65536, 2)])
+def test_engine_batches_consecutive_slots_per_staging_buffer(cap, chunk, n_staging):
+    """Slots in stream order (no slot map): several packages share a staging buffer, leave in one DMA, and — for limits
+    that are a multiple of the work tile — are packed by one launch.  The bytes are the oracle's either way, and the poison
+    behind the two short packages (end of the header region, end of the payload) and behind the last slot survives."""
+    bset = W.make_config("2", n_ops=39)
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    total = len(want)
+    hb = bs.header_bytes(bset.n_tensors, bset.n_blocks)
+    n = pkg.count(hb, total, cap)
+    slot_bytes = 64 + cap
+    ref_slots = pkg.emit_slots(want, cap, SID, slot_bytes, n_slots=n + 1, poison=POISON)
+    eng = bs.Engine(bset.n_tensors, bset.n_blocks, total + 4096, chunk_bytes=chunk, n_staging=n_staging)
+    host = pinned((n + 1) * slot_bytes, POISON)
+    st = eng.offload_packages_async(up.dset.desc, total, cap, SID, host.data_ptr(), slot_bytes, n + 1, None, bs.current_stream()).wait()
+    assert st["status"] == bs.OK and st["n_chunks"] == n
+    got = host.numpy().reshape(n + 1, slot_bytes)
+    assert (got == ref_slots).all(), "host packages differ from the oracle's"
+    ref = oracle.deserialize(want)
+    need = oracle.pool_bytes(want)
+    out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+    pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    st2 = eng.prefetch_packages_async(host.data_ptr(), slot_bytes, n + 1, SID, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL,
+                                      bs.current_stream()).wait()
+    torch.cuda.synchronize()
+    assert st2["status"] == bs.OK and (pool.cpu().numpy() == ref["pool"][:need]).all()
+    eng.destroy()
