@@ -134,6 +134,21 @@ static int ticket_create(bs_ticket** out)
     return BS_OK;
 }
 
+// A call that fails halfway (a CUDA error while enqueueing) must not leak its ticket, and must not free it under work that
+// is already enqueued and will still write the ticket's result word: drain the engine's streams, then destroy.
+struct TicketGuard {
+    bs_engine* e;
+    bs_ticket* t;
+    ~TicketGuard()
+    {
+        if (t == nullptr) return;
+        cudaStreamSynchronize(e->kstream);
+        cudaStreamSynchronize(e->cstream);
+        bs_ticket_destroy(t);
+    }
+    bs_ticket* release() { bs_ticket* r = t; t = nullptr; return r; }
+};
+
 // serialise engine calls: everything already enqueued on either side stream precedes the new call on both
 static int engine_fence(bs_engine* e)
 {
@@ -244,6 +259,7 @@ int bs_engine_offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layere
     if (total_bytes & 15) return BS_ERR_ARG;
     bs_ticket* t = nullptr;
     if ((rc = ticket_create(&t))) return rc;
+    TicketGuard guard{e, t};
     const uint64_t C = e->cfg.chunk_bytes;
     const uint32_t S = e->cfg.n_staging;
     t->bytes = total_bytes;
@@ -273,7 +289,7 @@ int bs_engine_offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layere
     if (t->n_chunks == 0) CK(cudaEventRecord(t->dma_begin, e->cstream));
     CK(cudaEventRecord(t->dma_end, e->cstream));
     CK(cudaEventRecord(t->done, e->cstream));  // after the last DMA, which is after every kernel-stream step
-    *ticket = t;
+    *ticket = guard.release();
     return BS_OK;
 }
 
@@ -315,6 +331,7 @@ int bs_engine_prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes,
     }
     bs_ticket* t = nullptr;
     if ((rc = ticket_create(&t))) return rc;
+    TicketGuard guard{e, t};
     t->is_prefetch = true;
     const uint64_t C = e->cfg.chunk_bytes;
     const uint32_t S = e->cfg.n_staging;
@@ -360,7 +377,7 @@ int bs_engine_prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes,
     CK(post_status(t->h_result, &((WsHead*)e->ws)->status, e->kstream));
     CK(cudaEventRecord(t->done, e->kstream));
     CK(cudaStreamWaitEvent(consumer, t->done, 0));
-    *ticket = t;
+    *ticket = guard.release();
     return BS_OK;
 }
 
@@ -425,6 +442,7 @@ int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t tot
     }
     bs_ticket* t = nullptr;
     if ((rc = ticket_create(&t))) return rc;
+    TicketGuard guard{e, t};
     const uint32_t S = e->cfg.n_staging;
     t->bytes = total_bytes + count * BS_PKG_HEADER;
     t->n_chunks = (uint32_t)count;
@@ -479,7 +497,7 @@ int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t tot
     }
     CK(cudaEventRecord(t->dma_end, e->cstream));
     CK(cudaEventRecord(t->done, e->cstream));
-    *ticket = t;
+    *ticket = guard.release();
     return BS_OK;
 }
 
@@ -510,6 +528,7 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
     }
     bs_ticket* t = nullptr;
     if ((rc = ticket_create(&t))) return rc;
+    TicketGuard guard{e, t};
     t->is_prefetch = true;
     const uint32_t S = e->cfg.n_staging;
     t->bytes = plan.total + plan.items.size() * BS_PKG_HEADER;
@@ -566,7 +585,7 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
     CK(post_status(t->h_result, &((WsHead*)e->ws)->status, e->kstream));
     CK(cudaEventRecord(t->done, e->kstream));
     CK(cudaStreamWaitEvent(consumer, t->done, 0));
-    *ticket = t;
+    *ticket = guard.release();
     return BS_OK;
 }
 

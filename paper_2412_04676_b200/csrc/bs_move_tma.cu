@@ -451,11 +451,14 @@ cudaError_t launch_tma_t(const MoveParams& p, const bs_opts& o, int sm_count, cu
     if (stages < 3 || stages > kMaxStages || warps < 1 || warps > kMaxWarps) return cudaErrorInvalidValue;
     const size_t smem = (size_t)warps * stages * q.tile_bytes + (size_t)warps * kMetaBytes;
     if (smem + 1024 > kSmemLimit) return cudaErrorInvalidValue;
-    static size_t configured = 0;  // per kernel instantiation
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(move_tma_kernel<UNPACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static size_t configured[64] = {0};  // per kernel instantiation and device (the attribute is per device)
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || smem > configured[dev]) {
+        e = cudaFuncSetAttribute(move_tma_kernel<UNPACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = smem;
+        if (dev >= 0 && dev < 64) configured[dev] = smem;
     }
     move_tma_kernel<UNPACK><<<(unsigned)sm_count, (warps + 1) * 32, smem, stream>>>(q, stages, warps | auto_shape);  // + the header warp
     return cudaGetLastError();
