@@ -242,7 +242,7 @@ int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, c
     for (uint64_t t = 0; t < T; ++t) {
         const orc2_struct *s = &st[ly[t].structure];
         for (uint64_t j = s->first_block; j < (uint64_t)s->first_block + s->n_blocks; ++j, ++a) {
-            uint64_t nb;
+            uint64_t nb = 0;                                  /* (initialised for gcc; block_bytes always sets it here: the plan passed) */
             block_bytes(dim + 3 * j, &nb);
             uint64_t sb = up(nb, V2_BLOCK_ALIGN);
             memcpy(q, (const void *)(uintptr_t)addr[a], (size_t)nb);
