@@ -223,7 +223,7 @@ int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, c
     for (uint64_t s = 0; s < C; ++s) {                       /* block records, offsets relative to the layer */
         uint64_t run = 0;
         for (uint64_t j = st[s].first_block; j < (uint64_t)st[s].first_block + st[s].n_blocks; ++j) {
-            uint64_t nb;
+            uint64_t nb = 0;                                  /* (initialised for gcc, as below) */
             block_bytes(dim + 3 * j, &nb);
             memcpy(p, qn + 6 * j, 24);
             w32(p + 24, dim[3 * j + 0]);
