@@ -125,7 +125,7 @@ int orc2_plan(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, const 
     for (uint64_t s = 0; s < C; ++s) {
         uint64_t run = 0;
         for (uint64_t j = st[s].first_block; j < (uint64_t)st[s].first_block + st[s].n_blocks; ++j) {
-            uint64_t nb;
+            uint64_t nb = 0;
             rc = block_bytes(dim + 3 * j, &nb);
             if (rc) return rc;
             if (rel_offset) rel_offset[j] = run;
@@ -138,7 +138,7 @@ int orc2_plan(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, const 
         const orc2_struct *s = &st[ly[t].structure];
         uint64_t lb = 0;
         for (uint64_t j = s->first_block; j < (uint64_t)s->first_block + s->n_blocks; ++j) {
-            uint64_t nb;
+            uint64_t nb = 0;
             block_bytes(dim + 3 * j, &nb);
             lb += up(nb, V2_BLOCK_ALIGN);
         }
@@ -192,7 +192,7 @@ int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, c
     for (uint64_t s = 0; s < C; ++s) {                       /* struct records, with layer_bytes */
         uint64_t lb = 0;
         for (uint64_t j = st[s].first_block; j < (uint64_t)st[s].first_block + st[s].n_blocks; ++j) {
-            uint64_t nb;
+            uint64_t nb = 0;
             block_bytes(dim + 3 * j, &nb);
             lb += up(nb, V2_BLOCK_ALIGN);
         }
@@ -214,7 +214,7 @@ int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, c
             p += V2_LAYER_REC;
             const orc2_struct *s = &st[ly[t].structure];
             for (uint64_t j = s->first_block; j < (uint64_t)s->first_block + s->n_blocks; ++j) {
-                uint64_t nb;
+                uint64_t nb = 0;
                 block_bytes(dim + 3 * j, &nb);
                 run += up(nb, V2_BLOCK_ALIGN);
             }
