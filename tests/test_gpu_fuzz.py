@@ -1,0 +1,117 @@
+"""Seeded random sets through the C ABI against the oracles: free-form descriptors (empty tensors, zero extents, ranks 2 and
+3, every element type, 8- and 16-byte-aligned sources, sizes from bytes to megabytes) that the paper-shaped generator never
+makes.  Everything is compared bit for bit; the launch shape, the chunking and the package limit are drawn too."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2412_04676_b200 as bs
+import workloads as W
+from oracle import dt, pkg
+from tests.gpu_util import DEV
+
+pytestmark = pytest.mark.gpu
+EXTENTS = [0, 1, 1, 2, 3, 5, 8, 17, 64, 127, 300]
+
+
+def random_set(rng):
+    T = int(rng.integers(0, 7))
+    tensors = np.zeros(T, W.TENSOR_REC_DTYPE)
+    qn, dim = [], []
+    for t in range(T):
+        rank = int(rng.choice([2, 3]))
+        nb = int(rng.integers(0, 9))
+        tensors[t] = (rank, len(dim), nb, tuple(int(x) for x in rng.integers(-2, 3, 2)), (-1, 1, 0 if rank == 2 else -1, 0),
+                      int(rng.integers(0, 1 << 31)), 0)
+        for _ in range(nb):
+            d = [int(rng.choice(EXTENTS)), int(rng.choice(EXTENTS)), int(rng.choice(EXTENTS)) if rank == 3 else 1]
+            if rng.random() < 0.1:
+                d[int(rng.integers(0, 2))] = int(rng.integers(500, 1500))       # now and then a block of megabytes
+            q = rng.integers(-5, 6, (3, 2)).astype(np.int32)
+            if rank == 2:
+                q[2] = 0
+            qn.append(q)
+            dim.append(d)
+    qn = np.array(qn, np.int32).reshape(-1, 3, 2)
+    dim = np.array(dim, np.uint32).reshape(-1, 3)
+    return tensors, qn, dim
+
+
+def upload(rng, tensors, qn, dim, dtype):
+    e = dt.ELEM_BYTES[dtype]
+    sizes = [e * int(d[0]) * int(d[1]) * int(d[2]) for d in dim]
+    blocks = [rng.integers(0, 256, n, dtype=np.uint8).tobytes() for n in sizes]
+    cur = 0
+    order = list(rng.permutation(len(blocks))) if blocks else []
+    offs = np.zeros(len(blocks), np.uint64)
+    for i in order:
+        mis = 8 if rng.random() < 0.3 else 0                                       # D16: 8-byte-aligned sources take the slow path
+        offs[i] = cur + mis
+        cur += (sizes[i] + mis + 255) // 256 * 256 + 256
+    host = np.full(max(cur, 256), 0x33, np.uint8)
+    for b, o in zip(blocks, offs):
+        host[int(o): int(o) + len(b)] = np.frombuffer(b, np.uint8)
+    pool = torch.from_numpy(host).to(DEV)
+    addr = (np.uint64(pool.data_ptr()) + offs).astype(np.uint64)
+    dset = bs.DeviceSet.from_host(tensors, qn, dim, addr, DEV, dtype=dtype)
+    return pool, dset, blocks
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_sets_round_trip_bit_exact(seed):
+    rng = np.random.default_rng(1000 + seed)
+    tensors, qn, dim = random_set(rng)
+    dtype = int(rng.integers(0, 4))
+    pool, dset, blocks = upload(rng, tensors, qn, dim, dtype)
+    want = dt.serialize(tensors, qn, dim, blocks, dtype)
+    if dtype == dt.F64 and len(blocks):        # the C oracle is a second opinion where it applies
+        hp = np.frombuffer(b"".join(b.ljust((len(b) + 15) // 16 * 16 + 16, b"\0") for b in blocks), np.uint8).copy()
+        ho = np.concatenate([[0], np.cumsum([(len(b) + 15) // 16 * 16 + 16 for b in blocks])[:-1]]).astype(np.uint64)
+        assert bytes(oracle.serialize(tensors, qn, dim, (np.uint64(hp.ctypes.data) + ho).astype(np.uint64))) == bytes(want)
+    total = len(want)
+    T, B = len(tensors), len(blocks)
+    variant = int(rng.choice([bs.VARIANT_TMA, bs.VARIANT_LDG]))
+    opts = dict(variant=variant, tile_bytes=int(rng.choice([16384, 32768])), stages=3, warps=int(rng.integers(1, 3)))
+    ws = bs.Workspace(T, B, max(total, 1 << 16), DEV, packages=True)
+    cs = bs.current_stream()
+    assert bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs) == (dt.header_bytes(T, B), total)      # L106
+    out = torch.full((total + 32,), 0xCD, dtype=torch.uint8, device=DEV)
+    bs.serialize(dset.desc, out.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
+    assert ws.read_result()["status"] == bs.OK
+    got = out.cpu().numpy()
+    assert (got[:total] == want).all() and (got[total:] == 0xCD).all(), f"seed {seed}: stream differs"
+    # concat of ranges with a random chunk == the stream (D15)
+    chunk = int(rng.integers(1, 40)) * 16 * int(rng.choice([1, 64, 4096]))
+    rng_out = torch.full((total,), 0xCD, dtype=torch.uint8, device=DEV)
+    for lo in range(0, total, chunk):
+        bs.serialize_range(dset.desc, rng_out.data_ptr() + lo, lo, min(lo + chunk, total), lo == 0, ws.ptr, ws.nbytes, ws.result_ptr,
+                           opts, cs)
+    assert (rng_out.cpu().numpy() == want).all(), f"seed {seed}: concat of ranges differs (chunk {chunk})"
+    # deserialize
+    ref = dt.deserialize(want)
+    need = ref["pool_bytes"]
+    o = bs.DeviceSet.empty(T, B, DEV, fill=0xAB)
+    opool = torch.full((max(need, 256),), 0xEE, dtype=torch.uint8, device=DEV)
+    bs.deserialize(out.data_ptr(), total, o.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["pool_bytes"] == need and res["dtype"] == dtype and (res["n_tensors"], res["n_blocks"]) == (T, B)
+    assert (opool.cpu().numpy()[:need] == ref["pool"][:need]).all(), f"seed {seed}: blocks differ"
+    h = o.to_host()
+    assert h["tensors"].tobytes() == tensors.tobytes() and (h["qn"] == qn).all() and (h["dim"] == dim).all()
+    # packages at a random limit, shuffled slots, and back
+    cap = int(rng.choice([16, 4096, 16384, 32768, 49152 + 16]))
+    if cap == 16 and total > 65536:
+        cap = 4096                              # keep the number of packages (two launches each) bounded
+    n = pkg.count(dt.header_bytes(T, B), total, cap)
+    slot_of = rng.permutation(n + 1)[:n]
+    slots = torch.full(((n + 1) * (64 + cap),), 0x5A, dtype=torch.uint8, device=DEV)
+    bs.package_emit(dset.desc, total, cap, 77, slots.data_ptr(), 64 + cap, n + 1, slot_of, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
+    assert ws.read_result()["status"] == bs.OK
+    ref_slots = pkg.emit_slots(want, cap, 77, 64 + cap, slot_of=slot_of, n_slots=n + 1, poison=0x5A)
+    assert (slots.cpu().numpy().reshape(n + 1, -1) == ref_slots).all(), f"seed {seed}: packages differ (limit {cap})"
+    opool.fill_(0xEE)
+    bs.package_unpack(slots.data_ptr(), 64 + cap, n + 1, 77, o.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                      ws.result_ptr, opts, cs)
+    assert ws.read_result()["status"] == bs.OK
+    assert (opool.cpu().numpy()[:need] == ref["pool"][:need]).all(), f"seed {seed}: blocks differ after the package round trip"
