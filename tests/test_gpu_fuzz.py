@@ -115,3 +115,75 @@ def test_random_sets_round_trip_bit_exact(seed):
                       ws.result_ptr, opts, cs)
     assert ws.read_result()["status"] == bs.OK
     assert (opool.cpu().numpy()[:need] == ref["pool"][:need]).all(), f"seed {seed}: blocks differ after the package round trip"
+
+
+def random_layered(rng):
+    """Free-form layered set: C structures (some empty, some unused), T layers naming them in any order."""
+    C = int(rng.integers(1, 6))
+    structs = np.zeros(C, W.STRUCT_REC_DTYPE)
+    qn, dim = [], []
+    for c in range(C):
+        rank = int(rng.choice([2, 3]))
+        nb = int(rng.integers(0, 7))
+        structs[c] = (rank, len(dim), nb, tuple(int(x) for x in rng.integers(-2, 3, 2)), (-1, 1, 0 if rank == 2 else -1, 0), 0)
+        for _ in range(nb):
+            d = [int(rng.choice(EXTENTS)), int(rng.choice(EXTENTS)), int(rng.choice(EXTENTS[:8])) if rank == 3 else 1]
+            q = rng.integers(-5, 6, (3, 2)).astype(np.int32)
+            if rank == 2:
+                q[2] = 0
+            qn.append(q)
+            dim.append(d)
+    T = int(rng.integers(0, 12))
+    layers = np.zeros(T, W.LAYER_REC_DTYPE)
+    for t in range(T):
+        layers[t] = (int(rng.integers(0, C)), int(rng.integers(0, 1 << 31)), 0)
+    return structs, layers, np.array(qn, np.int32).reshape(-1, 3, 2), np.array(dim, np.uint32).reshape(-1, 3)
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_layered_sets_round_trip_bit_exact(seed):
+    from oracle import v2
+    rng = np.random.default_rng(5000 + seed)
+    structs, layers, qn, dim = random_layered(rng)
+    sizes = []                                   # blocks layer by layer, in the order of the layer's structure
+    for ly in layers:
+        s = structs[int(ly["structure"])]
+        for j in range(int(s["first_block"]), int(s["first_block"]) + int(s["n_blocks"])):
+            sizes.append(8 * int(dim[j, 0]) * int(dim[j, 1]) * int(dim[j, 2]))
+    B = len(sizes)
+    offs = np.zeros(B, np.uint64)
+    cur = 0
+    for i in (rng.permutation(B) if B else []):
+        mis = 8 if rng.random() < 0.3 else 0
+        offs[i] = cur + mis
+        cur += (sizes[i] + mis + 255) // 256 * 256 + 256
+    host = rng.integers(0, 256, max(cur, 256), dtype=np.uint8)
+    want = v2.serialize(structs, layers, qn, dim, (np.uint64(host.ctypes.data) + offs).astype(np.uint64))
+    pool = torch.from_numpy(host).to(DEV)
+    addr = (np.uint64(pool.data_ptr()) + offs).astype(np.uint64)
+    dset = bs.DeviceLayeredSet.from_host(structs, layers, qn, dim, addr, DEV)
+    counts = (len(structs), dim.shape[0], len(layers), B)
+    total = len(want)
+    opts = dict(variant=int(rng.choice([bs.VARIANT_TMA, bs.VARIANT_LDG])), tile_bytes=int(rng.choice([16384, 32768])), stages=3,
+                warps=int(rng.integers(1, 3)))
+    ws = bs.Workspace(0, 0, max(total, 1 << 16), DEV, layered=counts)
+    cs = bs.current_stream()
+    assert bs.layered_serialized_size(dset.desc, ws.ptr, ws.nbytes, cs) == v2.serialized_size(structs, layers, dim)
+    out = torch.full((total + 32,), 0xCD, dtype=torch.uint8, device=DEV)
+    bs.layered_serialize(dset.desc, out.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
+    assert ws.read_result()["status"] == bs.OK
+    got = out.cpu().numpy()
+    assert (got[:total] == want).all() and (got[total:] == 0xCD).all(), f"seed {seed}: v2 stream differs"
+    ref = v2.deserialize(want)
+    na, need = v2.counts(want)
+    assert na == B
+    o = bs.DeviceLayeredSet.empty(*counts, DEV, fill=0xAB)
+    opool = torch.full((max(need, 256),), 0xEE, dtype=torch.uint8, device=DEV)
+    bs.layered_deserialize(out.data_ptr(), total, o.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, ws.result_ptr,
+                           opts, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["pool_bytes"] == need
+    assert (opool.cpu().numpy()[:need] == ref["pool"][:need]).all(), f"seed {seed}: blocks differ"
+    h = o.to_host(*counts)
+    assert h["structs"].tobytes() == ref["structs"].tobytes() and h["layers"].tobytes() == ref["layers"].tobytes()
+    assert (h["qn"] == qn).all() and (h["dim"] == dim).all()
