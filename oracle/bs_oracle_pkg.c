@@ -11,7 +11,8 @@
  *         implementation or self imposed upper limit.  The packages produced by the same serialization call
  *         are kept together ... in the end all packages are stored in a way that the whole, deserializable
  *         byte strings are stored continuously in memory."
- * The paper prints no byte layout; the one below is this project's:
+ * The paper prints no byte layout; the one below is this project's.  A package carries
+ * a range of a wire-format-v1 or -v2 stream; for v2 the blocks are counted in the order of the layered descriptor's addr[]:
  *
  *   package     := package_header(64) | stream bytes [lo, lo + nbytes)
  *   package_header: char magic[8]="BSPKG001"; u32 version=1; u32 index; u32 count; u32 first_block;
@@ -73,13 +74,33 @@ int orcp_range(uint64_t header_bytes, uint64_t total_bytes, uint64_t cap, uint64
     return ORC_OK;
 }
 
-/* ---- emit package `index` of a wire-format-v1 stream into out[0 .. 64 + nbytes) --------------------- */
-/* Reads header_bytes, n_tensors, n_blocks and the block records' offsets from the stream itself. */
+/* ---- first_block of a wire-format-v2 (structure-shared layers) stream -------------------------------- */
+/* The blocks of a layered set are counted layer by layer, inside a layer in the order of its structure's block table
+ * (the order of the descriptor's addr[]); block a of layer t, structure block j, starts at payload offset
+ * layer_rec[t].offset + block_rec[j].offset.  first_block = the largest a whose start is <= plo, as for v1. */
+static void first_block_v2(const unsigned char *s, uint64_t plo, uint32_t *first_block, uint64_t *intra)
+{
+    uint64_t C = g32(s + 32), T = g64(s + 40);
+    const unsigned char *srec = s + 64, *lrec = srec + 32 * C, *brec = lrec + 16 * T;
+    uint64_t a = 0;
+    for (uint64_t t = 0; t < T; ++t) {
+        uint64_t st = g32(lrec + 16 * t), loff = g64(lrec + 16 * t + 8);
+        uint64_t fb = g32(srec + 32 * st + 4), nb = g32(srec + 32 * st + 8);
+        for (uint64_t j = fb; j < fb + nb; ++j, ++a) {
+            uint64_t off = loff + g64(brec + 48 * j + 40);
+            if (off <= plo) { *first_block = (uint32_t)a; *intra = plo - off; }
+        }
+    }
+}
+
+/* ---- emit package `index` of a wire-format-v1 or v2 stream into out[0 .. 64 + nbytes) ---------------- */
+/* Reads header_bytes, the counts and the block records' offsets from the stream itself. */
 int orcp_emit(const unsigned char *s, uint64_t n, uint64_t cap, uint64_t stream_id, uint64_t index,
               unsigned char *out, uint64_t capacity, uint64_t *written)
 {
-    if (n < 64 || memcmp(s, "BSPARSE1", 8) != 0 || g32(s + 8) != 1u) return ORC_ERR_ARG;
-    uint64_t T = g64(s + 32), B = g64(s + 40), hb = g64(s + 48);
+    if (n < 64 || memcmp(s, "BSPARSE1", 8) != 0 || (g32(s + 8) != 1u && g32(s + 8) != 2u)) return ORC_ERR_ARG;
+    const int v2 = g32(s + 8) == 2u;
+    uint64_t T = v2 ? 0 : g64(s + 32), B = v2 ? 0 : g64(s + 40), hb = g64(s + 48);
     if (hb > n) return ORC_ERR_ARG;
     uint64_t lo, hi;
     int rc = orcp_range(hb, n, cap, index, &lo, &hi);
@@ -89,7 +110,9 @@ int orcp_emit(const unsigned char *s, uint64_t n, uint64_t cap, uint64_t stream_
     if (capacity < PKG_HEADER + nbytes) return ORC_ERR_CAPACITY;
     uint32_t first_block = PKG_NO_BLOCK;
     uint64_t intra = 0;
-    if (lo >= hb) {                                   /* largest i with offset_i <= lo - hb */
+    if (lo >= hb && v2) {
+        first_block_v2(s, lo - hb, &first_block, &intra);
+    } else if (lo >= hb) {                            /* largest i with offset_i <= lo - hb */
         const unsigned char *brec = s + 64 + 32 * T;
         uint64_t plo = lo - hb;
         for (uint64_t i = 0; i < B; ++i) {

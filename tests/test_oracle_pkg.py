@@ -137,3 +137,46 @@ def test_assemble_fault_injection():
     with pytest.raises(oracle.OracleError) as e:
         pkg.assemble(slots, SID, capacity=len(stream) - 1)
     assert e.value.code == oracle.ERR_CAPACITY and e.value.required == len(stream)
+
+
+# ---- packages of wire-format-v2 streams (layered sets): blocks counted in the order of the descriptor's addr[] ----------
+def test_golden_package_headers_of_the_v2_golden_stream():
+    gold = read_hex_fixture(os.path.join(HERE, "golden", "g5_package_headers_v2.hex"))
+    assert len(gold) == 192
+    stream = np.frombuffer(read_hex_fixture(os.path.join(HERE, "golden", "g2_golden_stream_v2.hex")), np.uint8)
+    a, b, c = pkg.emit(stream, 128, SID, 2), pkg.emit(stream, 16, SID, 19), pkg.emit(stream, 128, SID, 1)
+    assert bytes(a[:64]) == gold[0:64] and bytes(a[64:]) == bytes(stream[256:320])
+    assert bytes(b[:64]) == gold[64:128] and bytes(b[64:]) == bytes(stream[304:320])
+    assert bytes(c[:64]) == gold[128:192] and bytes(c[64:]) == bytes(stream[128:256])
+    assert read_pkg_header(pkg.emit(stream, 16, SID, 18))["first_block"] == 2
+
+
+@pytest.mark.parametrize("cap", [16, 4096, 65536])
+def test_first_block_of_v2_packages_against_searchsorted_and_reassembly(cap):
+    from oracle import v2
+    from tests.streamreader import read_stream_v2
+    bset = W.make_config("1") if cap == 16 else W.make_config("2", n_ops=26)     # keep the number of packages bounded
+    lv = W.layered_view(bset)
+    pool, offs = W.fill_pool_host(bset)
+    from tests.util import host_addrs
+    s = v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], host_addrs(pool, offs))
+    fixed, structs, layers, blocks, _, _ = read_stream_v2(s.tobytes())          # the independent reader
+    starts = []
+    for ly in layers:
+        sr = structs[ly["structure"]]
+        starts += [ly["offset"] + b["offset"] for b in blocks[sr["first_block"]: sr["first_block"] + sr["n_blocks"]]]
+    starts = np.array(starts, np.uint64)
+    assert (np.diff(starts.astype(np.int64)) >= 0).all() and len(starts) == bset.n_blocks
+    hb = fixed["header_bytes"]
+    n = pkg.count(hb, len(s), cap)
+    for k in sorted(set([0, n - 1] + [int(x) for x in np.random.default_rng(cap).integers(0, n, 40)])):
+        h = read_pkg_header(pkg.emit(s, cap, SID, k))
+        lo, hi = pkg.package_range(hb, len(s), cap, k)
+        assert (h["lo"], h["nbytes"], h["total_bytes"], h["count"]) == (lo, hi - lo, len(s), n)
+        if lo < hb:
+            assert h["first_block"] == pkg.NO_BLOCK and h["first_block_offset"] == 0
+        else:
+            i = int(np.searchsorted(starts, lo - hb, side="right")) - 1
+            assert h["first_block"] == i and h["first_block_offset"] == lo - hb - int(starts[i])
+    slots = pkg.emit_slots(s, cap, SID, 64 + cap, slot_of=np.random.default_rng(3).permutation(n))
+    assert bytes(pkg.assemble(slots, SID)) == bytes(s)
