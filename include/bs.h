@@ -114,7 +114,7 @@ typedef struct bs_result {
     int32_t status;         /* BS_OK or BS_ERR_* */
     uint32_t n_tensors;
     uint32_t n_blocks;
-    uint32_t reserved[5];   /* [0], [1]: see bs_layered_* / bs_package_emit; [2] = dtype of the stream (deserialize) */
+    uint32_t reserved[5];   /* [0], [1]: see bs_layered_*; [2] = dtype of the stream (deserialize); [3]: see bs_package_emit */
 } bs_result;
 
 typedef struct bs_stream_info_t {
@@ -358,7 +358,7 @@ uint64_t bs_package_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint6
 /* Serialize `set` straight into packages in DEVICE slots: package k -> d_slots + slot(k)*slot_bytes with
  * slot(k) = h_slot_of[k] (HOST array of `count` entries, each < n_slots, all different) or k when h_slot_of is NULL.
  * total_bytes = the size prediction (bs_serialized_size; re-checked on the device); 0 computes it, which SYNCHRONISES
- * `stream`.  Bytes of a slot behind its package are not written.  bs_result: as bs_serialize, reserved[0] = count.
+ * `stream`.  Bytes of a slot behind its package are not written.  bs_result: as bs_serialize, reserved[3] = count.
  * At once: BS_ERR_ARG (cap, slot_bytes, slot map), BS_ERR_CAPACITY (count > n_slots, workspace). */
 int bs_package_emit(const bs_set_desc *set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id, void *d_slots,
                     uint64_t slot_bytes, uint64_t n_slots, const uint32_t *h_slot_of, void *d_workspace,
@@ -370,6 +370,18 @@ int bs_package_emit(const bs_set_desc *set, uint64_t total_bytes, uint64_t cap, 
 int bs_package_unpack(const void *d_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id, bs_set_desc *out,
                       void *d_pool, uint64_t pool_bytes, uint32_t flags, void *d_workspace, uint64_t workspace_bytes,
                       bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
+
+/* The same for layered sets: packages of a wire-format-v2 stream (first_block counts the blocks in the order of the
+ * layered descriptor's addr[]: layer by layer, inside a layer in the order of its structure's block table).
+ * bs_layered_package_workspace_bytes = bs_layered_workspace_bytes + room for the assembled header region. */
+uint64_t bs_layered_package_workspace_bytes(uint32_t n_structs, uint32_t n_struct_blocks, uint32_t n_layers, uint64_t n_addr,
+                                            uint64_t stream_capacity);
+int bs_layered_package_emit(const bs_layered_desc *set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id, void *d_slots,
+                            uint64_t slot_bytes, uint64_t n_slots, const uint32_t *h_slot_of, void *d_workspace,
+                            uint64_t workspace_bytes, bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
+int bs_layered_package_unpack(const void *d_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id,
+                              bs_layered_desc *out, void *d_pool, uint64_t pool_bytes, uint32_t flags, void *d_workspace,
+                              uint64_t workspace_bytes, bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
 
 /* The same through the engine, slots in pinned HOST memory (the receive buffers of L126): package k is packed into a
  * staging buffer behind its header and DMA'd to h_slots + slot(k)*slot_bytes; cap + 64 <= chunk_bytes.  Prefetch takes

@@ -13,6 +13,6 @@ from ._binding import (  # noqa: F401
     layered_stream_info, layered_workspace_bytes, make_layered_desc,
     deserialize, header_bytes, last_cuda_error, lib, make_desc, serialize, serialize_range, serialized_size,
     stream_info, strerror, version, workspace_bytes,
-    PKG_HEADER, PKG_NO_BLOCK, package_count, package_emit, package_range, package_unpack, package_workspace_bytes,
+    PKG_HEADER, PKG_NO_BLOCK, layered_package_emit, layered_package_unpack, layered_package_workspace_bytes, package_count, package_emit, package_range, package_unpack, package_workspace_bytes,
 )
 from .device import DeviceLayeredSet, DeviceSet, Workspace, current_stream  # noqa: F401

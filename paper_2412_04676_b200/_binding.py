@@ -152,6 +152,10 @@ def lib():
     L.bs_package_workspace_bytes.argtypes = [u32, u32, u64]
     L.bs_package_emit.argtypes = [C.POINTER(SetDesc), u64, u64, u64, vp, u64, u64, pu32, vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_package_unpack.argtypes = [vp, u64, u64, u64, C.POINTER(SetDesc), vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_layered_package_workspace_bytes.restype = u64
+    L.bs_layered_package_workspace_bytes.argtypes = [u32, u32, u32, u64, u64]
+    L.bs_layered_package_emit.argtypes = [LD, u64, u64, u64, vp, u64, u64, pu32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_layered_package_unpack.argtypes = [vp, u64, u64, u64, LD, vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_offload_packages_async.argtypes = [vp, C.POINTER(SetDesc), u64, u64, u64, vp, u64, u64, pu32, vp, C.POINTER(vp)]
     L.bs_prefetch_packages_async.argtypes = [vp, vp, u64, u64, u64, C.POINTER(SetDesc), vp, u64, u32, vp, C.POINTER(vp)]
     L.bs_queue_create.argtypes = [C.POINTER(vp), C.POINTER(EngineCfg)]
@@ -330,6 +334,25 @@ def package_unpack(slots_ptr: int, slot_bytes: int, n_slots: int, stream_id: int
                    pool_bytes: int, flags: int, ws_ptr: int, ws_bytes: int, result_ptr: int, opts=None, stream: int = 0) -> int:
     return _check(lib().bs_package_unpack(slots_ptr, slot_bytes, n_slots, stream_id, C.byref(out), pool_ptr, pool_bytes, flags,
                                           ws_ptr, ws_bytes, result_ptr, _opts(opts), stream), "bs_package_unpack")
+
+
+def layered_package_workspace_bytes(n_structs: int, n_struct_blocks: int, n_layers: int, n_addr: int, stream_capacity: int) -> int:
+    return int(lib().bs_layered_package_workspace_bytes(n_structs, n_struct_blocks, n_layers, n_addr, stream_capacity))
+
+
+def layered_package_emit(desc: LayeredDesc, total_bytes: int, cap: int, stream_id: int, slots_ptr: int, slot_bytes: int,
+                         n_slots: int, slot_of, ws_ptr: int, ws_bytes: int, result_ptr: int, opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_layered_package_emit(C.byref(desc), total_bytes, cap, stream_id, slots_ptr, slot_bytes, n_slots,
+                                                _slot_map(slot_of), ws_ptr, ws_bytes, result_ptr, _opts(opts), stream),
+                  "bs_layered_package_emit")
+
+
+def layered_package_unpack(slots_ptr: int, slot_bytes: int, n_slots: int, stream_id: int, out: LayeredDesc, pool_ptr: int,
+                           pool_bytes: int, flags: int, ws_ptr: int, ws_bytes: int, result_ptr: int, opts=None,
+                           stream: int = 0) -> int:
+    return _check(lib().bs_layered_package_unpack(slots_ptr, slot_bytes, n_slots, stream_id, C.byref(out), pool_ptr, pool_bytes,
+                                                  flags, ws_ptr, ws_bytes, result_ptr, _opts(opts), stream),
+                  "bs_layered_package_unpack")
 
 
 class Ticket:

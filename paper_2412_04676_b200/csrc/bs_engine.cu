@@ -42,10 +42,10 @@ int run_layered_deserialize_plan(const void* d_header, const void* d_payload, ui
                                  void* d_pool, uint64_t pool_bytes, uint32_t flags, void* d_ws, uint64_t ws_bytes,
                                  bs_result* d_result, int sms, cudaStream_t stream);
 int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, void* d_dst, uint64_t lo, uint64_t hi,
-                           const bs_opts& o, int sms, cudaStream_t stream);
+                           const bs_opts& o, int sms, cudaStream_t stream, const PkgMap* pm = nullptr);
 int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws_bytes, const void* d_src,
                              const void* d_header, uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms,
-                             cudaStream_t stream);
+                             cudaStream_t stream, const PkgMap* pm = nullptr);
 }  // namespace bs
 
 using namespace bs;

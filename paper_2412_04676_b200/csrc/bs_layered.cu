@@ -779,8 +779,9 @@ int run_layered_deserialize_plan(const void* d_header, const void* d_payload, ui
     return BS_OK;
 }
 
+// pm != null: the stream side is a set of package slots (bs_pkg.cu); d_dst is then unused
 int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, void* d_dst, uint64_t lo, uint64_t hi,
-                           const bs_opts& o, int sms, cudaStream_t stream)
+                           const bs_opts& o, int sms, cudaStream_t stream, const PkgMap* pm)
 {
     MoveParams mp;
     memset(&mp, 0, sizeof(mp));
@@ -794,6 +795,7 @@ int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_b
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
+    if (pm) mp.pkg = *pm;
     cudaError_t e = launch_move(false, mp, o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
@@ -801,7 +803,7 @@ int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_b
 
 int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws_bytes, const void* d_src,
                              const void* d_header, uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms,
-                             cudaStream_t stream)
+                             cudaStream_t stream, const PkgMap* pm)
 {
     MoveParams mp;
     memset(&mp, 0, sizeof(mp));
@@ -817,6 +819,7 @@ int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
     mp.flags = flags;
+    if (pm) mp.pkg = *pm;
     cudaError_t e = launch_move(true, mp, o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
@@ -895,7 +898,7 @@ int bs_layered_serialize_range(const bs_layered_desc* set, void* d_dst, uint64_t
     int sms;
     if ((rc = device_sm_count(&sms))) return rc;
     if (run_scan && (rc = run_layered_serialize_plan(set, d_ws, ws_bytes, UINT64_MAX, 0, d_result, sms, stream))) return rc;
-    return run_layered_pack_range(set, d_ws, ws_bytes, d_dst, lo, hi, o, sms, stream);
+    return run_layered_pack_range(set, d_ws, ws_bytes, d_dst, lo, hi, o, sms, stream, nullptr);
 }
 
 int bs_layered_serialize(const bs_layered_desc* set, void* d_stream, uint64_t capacity, void* d_ws, uint64_t ws_bytes,
@@ -910,7 +913,7 @@ int bs_layered_serialize(const bs_layered_desc* set, void* d_stream, uint64_t ca
     int sms;
     if ((rc = device_sm_count(&sms))) return rc;
     if ((rc = run_layered_serialize_plan(set, d_ws, ws_bytes, capacity, 0, d_result, sms, stream))) return rc;
-    return run_layered_pack_range(set, d_ws, ws_bytes, d_stream, 0, capacity & ~15ull, o, sms, stream);
+    return run_layered_pack_range(set, d_ws, ws_bytes, d_stream, 0, capacity & ~15ull, o, sms, stream, nullptr);
 }
 
 int bs_layered_deserialize(const void* d_stream, uint64_t nbytes, bs_layered_desc* out, void* d_pool, uint64_t pool_bytes,
@@ -930,7 +933,7 @@ int bs_layered_deserialize(const void* d_stream, uint64_t nbytes, bs_layered_des
     const unsigned char* s = (const unsigned char*)d_stream;
     if ((rc = run_layered_deserialize_plan(s, s, nbytes, out, d_pool, pool_bytes, flags, d_ws, ws_bytes, d_result, sms, stream)))
         return rc;
-    return run_layered_unpack_range(out, d_ws, ws_bytes, s, s, 0, nbytes & ~15ull, flags, o, sms, stream);
+    return run_layered_unpack_range(out, d_ws, ws_bytes, s, s, 0, nbytes & ~15ull, flags, o, sms, stream, nullptr);
 }
 
 }  // extern "C"

@@ -36,6 +36,18 @@ int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t n
 int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header, uint64_t lo,
                      uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream);
 int run_pack_packages(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, const bs_opts& o, int sms, cudaStream_t stream);
+// wire format v2 (bs_layered.cu)
+bool layered_ws(void* d_ws, uint64_t ws_bytes, uint32_t Bs, uint32_t T, uint64_t B, WsLayout* out);
+int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t capacity, uint64_t expect_total,
+                               bs_result* d_result, int sms, cudaStream_t stream);
+int run_layered_deserialize_plan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_layered_desc* out,
+                                 void* d_pool, uint64_t pool_bytes, uint32_t flags, void* d_ws, uint64_t ws_bytes,
+                                 bs_result* d_result, int sms, cudaStream_t stream);
+int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, void* d_dst, uint64_t lo, uint64_t hi,
+                           const bs_opts& o, int sms, cudaStream_t stream, const PkgMap* pm);
+int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws_bytes, const void* d_src, const void* d_header,
+                             uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream,
+                             const PkgMap* pm);
 int run_unpack_packages(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t header_bytes, uint32_t flags,
                         const bs_opts& o, int sms, cudaStream_t stream);
 
@@ -86,7 +98,7 @@ __device__ __forceinline__ void pkg_write_header(const WsLayout& ws, uint64_t ca
     o[2] = make_uint4((uint32_t)total, (uint32_t)(total >> 32), (uint32_t)lo, (uint32_t)(lo >> 32));
     const uint64_t nb = hi - lo;
     o[3] = make_uint4((uint32_t)nb, (uint32_t)(nb >> 32), (uint32_t)intra, (uint32_t)(intra >> 32));
-    if (k == 0 && result != nullptr) result->reserved[0] = (uint32_t)count;
+    if (k == 0 && result != nullptr) result->reserved[3] = (uint32_t)count;
 }
 
 // one thread: package k -> dst
@@ -440,6 +452,137 @@ int bs_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t n_slots
             return rc;
     }
     if (d_result != nullptr)  // the pad check of the unpack kernels can still flip the status
+        CK(cudaMemcpyAsync(&d_result->status, &L.head->status, sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
+    return BS_OK;
+}
+
+// ---- layered sets: packages of a wire-format-v2 stream ------------------------------------------------------------------
+// The package kernels only look at the flat block table blk[] and the sizes in WsHead, which the layered plan builds exactly
+// as the v1 scan does, so they are shared; only the plan and the header generator / parser behind the move kernels differ.
+uint64_t bs_layered_package_workspace_bytes(uint32_t n_structs, uint32_t n_struct_blocks, uint32_t n_layers, uint64_t n_addr,
+                                            uint64_t stream_capacity)
+{
+    return bs_layered_workspace_bytes(n_structs, n_struct_blocks, n_layers, n_addr, stream_capacity) + 256 +
+           align_up(bs_layered_header_bytes(n_structs, n_layers, n_struct_blocks), 256);
+}
+
+int bs_layered_package_emit(const bs_layered_desc* set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id, void* d_slots,
+                            uint64_t slot_bytes, uint64_t n_slots, const uint32_t* h_slot_of, void* d_ws, uint64_t ws_bytes,
+                            bs_result* d_result, const bs_opts* opts, cudaStream_t stream)
+{
+    if (set == nullptr) return BS_ERR_ARG;
+    if (set->n_qn != 2 || set->dtype != BS_F64) return BS_ERR_UNSUPPORTED;
+    if (d_slots == nullptr || !aligned16(d_slots) || cap == 0 || (cap & 15) || (slot_bytes & 15) ||
+        slot_bytes < BS_PKG_HEADER + cap)
+        return BS_ERR_ARG;
+    bs_opts o;
+    resolve_opts(opts, &o);
+    int rc;
+    if ((rc = check_opts(o))) return rc;
+    if (d_ws == nullptr || ((uintptr_t)d_ws & 255)) return BS_ERR_ARG;
+    WsLayout L;
+    if (!layered_ws(d_ws, ws_bytes, set->n_struct_blocks, set->n_layers, set->n_addr, &L)) return BS_ERR_CAPACITY;
+    int sms;
+    if ((rc = device_sm_count(&sms))) return rc;
+    const uint64_t hb = bs_layered_header_bytes(set->n_structs, set->n_layers, set->n_struct_blocks);
+    if (total_bytes == 0) {
+        uint64_t hb2 = 0;
+        if ((rc = bs_layered_serialized_size(set, d_ws, ws_bytes, &hb2, &total_bytes, stream))) return rc;
+    }
+    const uint64_t count = pkg_count(hb, total_bytes, cap);
+    if (count == 0 || count >= (1ull << 32)) return BS_ERR_ARG;
+    if (count > n_slots) return BS_ERR_CAPACITY;
+    if (h_slot_of != nullptr) {
+        std::vector<bool> used((size_t)n_slots, false);
+        for (uint64_t k = 0; k < count; ++k) {
+            if (h_slot_of[k] >= n_slots || used[h_slot_of[k]]) return BS_ERR_ARG;
+            used[h_slot_of[k]] = true;
+        }
+    }
+    if ((rc = run_layered_serialize_plan(set, d_ws, ws_bytes, UINT64_MAX, total_bytes, d_result, sms, stream))) return rc;
+    if (cap % work_tile_bytes(o) == 0) {  // the fixed-launch-count path, as bs_package_emit
+        uint32_t* d_tab = nullptr;
+        if (h_slot_of != nullptr) {
+            CK(cudaMallocAsync((void**)&d_tab, count * sizeof(uint32_t), stream));
+            CK(cudaMemcpyAsync(d_tab, h_slot_of, count * sizeof(uint32_t), cudaMemcpyHostToDevice, stream));
+        }
+        CK(launch_pkg_headers(L, cap, stream_id, 0, count, count, d_slots, slot_bytes, d_tab, d_result, stream));
+        PkgMap pm;
+        pm.cap = cap; pm.slot_bytes = slot_bytes; pm.base = (unsigned char*)d_slots; pm.slot_of = d_tab; pm.k_base = 0;
+        rc = run_layered_pack_range(set, d_ws, ws_bytes, nullptr, 0, UINT64_MAX, o, sms, stream, &pm);
+        if (d_tab) CK(cudaFreeAsync(d_tab, stream));
+        return rc;
+    }
+    for (uint64_t k = 0; k < count; ++k) {
+        uint64_t lo = 0, hi = 0;
+        pkg_range(hb, total_bytes, cap, k, &lo, &hi);
+        unsigned char* slot = (unsigned char*)d_slots + (h_slot_of ? (uint64_t)h_slot_of[k] : k) * slot_bytes;
+        CK(launch_pkg_header(L, cap, stream_id, k, count, slot, d_result, stream));
+        if ((rc = run_layered_pack_range(set, d_ws, ws_bytes, slot + BS_PKG_HEADER, lo, hi, o, sms, stream, nullptr))) return rc;
+    }
+    return BS_OK;
+}
+
+int bs_layered_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id, bs_layered_desc* out,
+                              void* d_pool, uint64_t pool_bytes, uint32_t flags, void* d_ws, uint64_t ws_bytes, bs_result* d_result,
+                              const bs_opts* opts, cudaStream_t stream)
+{
+    if (out == nullptr) return BS_ERR_ARG;
+    if (out->n_qn != 2 || out->dtype != BS_F64) return BS_ERR_UNSUPPORTED;
+    if (d_slots == nullptr || !aligned16(d_slots) || (slot_bytes & 15) || slot_bytes < BS_PKG_HEADER + 16 || n_slots == 0)
+        return BS_ERR_ARG;
+    if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
+    if (flags == BS_LAYOUT_POOL && pool_bytes && (d_pool == nullptr || ((uintptr_t)d_pool & 255))) return BS_ERR_ARG;
+    bs_opts o;
+    resolve_opts(opts, &o);
+    int rc;
+    if ((rc = check_opts(o))) return rc;
+    // workspace := layered workspace | room for the assembled header region
+    const uint64_t hdr_cap = align_up(bs_layered_header_bytes(out->n_structs, out->n_layers, out->n_struct_blocks), 256);
+    if (d_ws == nullptr || ((uintptr_t)d_ws & 255)) return BS_ERR_ARG;
+    if (ws_bytes < hdr_cap) return BS_ERR_CAPACITY;
+    const uint64_t w1 = (ws_bytes - hdr_cap) & ~255ull;
+    WsLayout L;
+    if (!layered_ws(d_ws, w1, out->n_struct_blocks, out->n_layers, out->n_addr, &L)) return BS_ERR_CAPACITY;
+    unsigned char* d_header = (unsigned char*)d_ws + w1;
+    int sms;
+    if ((rc = device_sm_count(&sms))) return rc;
+    std::vector<unsigned char> hdrs((size_t)n_slots * BS_PKG_HEADER);
+    CK(cudaMemcpy2DAsync(hdrs.data(), BS_PKG_HEADER, d_slots, slot_bytes, BS_PKG_HEADER, n_slots, cudaMemcpyDeviceToHost, stream));
+    CK(cudaStreamSynchronize(stream));
+    PkgPlan plan;
+    if ((rc = pkg_plan(hdrs.data(), BS_PKG_HEADER, n_slots, slot_bytes, stream_id, &plan))) return rc;
+    if (plan.hb > hdr_cap) return BS_ERR_CAPACITY;
+    const unsigned char* slots = (const unsigned char*)d_slots;
+    for (uint32_t k = 0; k < plan.n_header; ++k) {  // the header region, stored continuously (L126)
+        const PkgItem& it = plan.items[k];
+        CK(cudaMemcpyAsync(d_header + it.lo, slots + it.slot * slot_bytes + BS_PKG_HEADER, it.nbytes, cudaMemcpyDeviceToDevice, stream));
+    }
+    if ((rc = run_layered_deserialize_plan(d_header, nullptr, plan.total, out, d_pool, pool_bytes, flags, d_ws, w1, d_result, sms, stream)))
+        return rc;
+    CK(launch_pkg_check(L, d_slots, slot_bytes, n_slots, stream_id, d_result, stream));
+    if ((rc = run_layered_unpack_range(out, d_ws, w1, d_header, d_header, 0, 0, flags, o, sms, stream, nullptr))) return rc;  // rebuild
+    const uint64_t cut = plan_uniform_cap(plan, work_tile_bytes(o));
+    if (cut != 0) {  // one launch for every payload package, wherever it lies
+        const uint64_t count = plan.items.size();
+        uint32_t* d_tab = nullptr;
+        CK(cudaMallocAsync((void**)&d_tab, count * sizeof(uint32_t), stream));
+        pkg_index_kernel<<<(unsigned)((n_slots + 127) / 128), 128, 0, stream>>>(slots, slot_bytes, n_slots, stream_id, d_tab, count);
+        CK(cudaGetLastError());
+        PkgMap pm;
+        pm.cap = cut; pm.slot_bytes = slot_bytes; pm.base = const_cast<unsigned char*>(slots); pm.slot_of = d_tab; pm.k_base = 0;
+        rc = run_layered_unpack_range(out, d_ws, w1, nullptr, nullptr, 0, UINT64_MAX, flags | kFlagCheckPad, o, sms, stream, &pm);
+        CK(cudaFreeAsync(d_tab, stream));
+        if (rc) return rc;
+    } else {
+        std::vector<PkgItem> by_slot(plan.items.begin() + plan.n_header, plan.items.end());
+        std::sort(by_slot.begin(), by_slot.end(), [](const PkgItem& a, const PkgItem& b) { return a.slot < b.slot; });
+        for (const PkgItem& it : by_slot)
+            if ((rc = run_layered_unpack_range(out, d_ws, w1, slots + it.slot * slot_bytes + BS_PKG_HEADER, nullptr, it.lo,
+                                               it.lo + it.nbytes, flags | kFlagCheckPad, o, sms, stream, nullptr)))
+                return rc;
+    }
+    if (d_result != nullptr)
         CK(cudaMemcpyAsync(&d_result->status, &L.head->status, sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
     return BS_OK;
 }

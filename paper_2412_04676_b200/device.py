@@ -116,7 +116,9 @@ class Workspace:
     def __init__(self, n_tensors: int, n_blocks: int, stream_capacity: int, device="cuda", layered=None, packages=False):
         """layered = (n_structs, n_struct_blocks, n_layers, n_addr) sizes the workspace for wire format v2 instead;
         packages=True adds the room bs_package_unpack needs for the assembled header region."""
-        if packages:
+        if packages and layered is not None:
+            self.nbytes = B.layered_package_workspace_bytes(*layered, stream_capacity)
+        elif packages:
             self.nbytes = B.package_workspace_bytes(n_tensors, n_blocks, stream_capacity)
         elif layered is not None:
             self.nbytes = B.layered_workspace_bytes(*layered, stream_capacity)
@@ -141,4 +143,4 @@ class Workspace:
         return dict(total_bytes=int(r.total_bytes), header_bytes=int(r.header_bytes), payload_bytes=int(r.payload_bytes),
                     pool_bytes=int(r.pool_bytes), status=int(r.status), n_tensors=int(r.n_tensors), n_blocks=int(r.n_blocks),
                     n_structs=int(r.reserved[0]), n_struct_blocks=int(r.reserved[1]), dtype=int(r.reserved[2]),
-                    n_packages=int(r.reserved[0]))
+                    n_packages=int(r.reserved[3]))

@@ -351,3 +351,57 @@ def test_engine_batches_consecutive_slots_per_staging_buffer(cap, chunk, n_stagi
     torch.cuda.synchronize()
     assert st2["status"] == bs.OK and (pool.cpu().numpy() == ref["pool"][:need]).all()
     eng.destroy()
+
+
+# ---- packages of layered sets (wire format v2) ------------------------------------------------------------------------------
+@pytest.mark.parametrize("cap", [16384, 65536, 4096 + 16, 1 << 20])
+@pytest.mark.parametrize("variant", [bs.VARIANT_TMA, bs.VARIANT_LDG])
+def test_layered_packages_match_the_oracle_and_unpack_in_any_order(cap, variant):
+    from oracle import v2
+    from tests.test_gpu_layered import LayeredUp
+    bset = W.make_config("2", n_ops=39)
+    lu = LayeredUp(bset)
+    want = lu.want
+    total = len(want)
+    c = lu.counts
+    hb = bs.layered_header_bytes(c[0], c[2], c[1])
+    n = pkg.count(hb, total, cap)
+    slot_bytes = 64 + cap
+    slot_of = np.random.default_rng(8).permutation(n + 2)[:n]
+    ref_slots = pkg.emit_slots(want, cap, SID, slot_bytes, slot_of=slot_of, n_slots=n + 2, poison=POISON)
+    slots = torch.full(((n + 2) * slot_bytes,), POISON, dtype=torch.uint8, device=DEV)
+    ws = bs.Workspace(0, 0, max(total, 1 << 16), DEV, layered=c, packages=True)
+    opts = dict(variant=variant)
+    bs.layered_package_emit(lu.dset.desc, total, cap, SID, slots.data_ptr(), slot_bytes, n + 2, slot_of, ws.ptr, ws.nbytes,
+                            ws.result_ptr, opts, bs.current_stream())
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["total_bytes"] == total and res["n_packages"] == n and res["n_structs"] == c[0]
+    got = slots.cpu().numpy().reshape(n + 2, slot_bytes)
+    assert (got == ref_slots).all(), "layered packages differ from the oracle's"
+    # and back, from the oracle's slots with two foreign packages mixed in
+    other = pkg.emit_slots(want, cap, SID + 1, slot_bytes)
+    spare = [s for s in range(n + 2) if s not in set(slot_of.tolist())]
+    ref_slots[spare[0]] = other[0]
+    ref_slots[spare[1]] = other[-1]
+    ref = v2.deserialize(want)
+    na, need = v2.counts(want)
+    out = bs.DeviceLayeredSet.empty(*c, DEV, fill=0xAB)
+    pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    d_slots = torch.from_numpy(ref_slots.copy()).to(DEV)
+    bs.layered_package_unpack(d_slots.data_ptr(), slot_bytes, n + 2, SID, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr,
+                              ws.nbytes, ws.result_ptr, opts, bs.current_stream())
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["pool_bytes"] == need
+    assert (pool.cpu().numpy() == ref["pool"][:need]).all()
+    h = out.to_host(*c)
+    assert h["structs"].tobytes() == ref["structs"].tobytes() and h["layers"].tobytes() == ref["layers"].tobytes()
+    # a payload package that lies about its first block is refused on the device, nothing written
+    k = n - 1
+    s = int(slot_of[k])
+    (fb,) = struct.unpack_from("<I", ref_slots[s].tobytes(), 20)
+    ref_slots[s, 20:24] = np.frombuffer(struct.pack("<I", fb + 1), np.uint8)
+    pool.fill_(0xEE)
+    d_slots = torch.from_numpy(ref_slots.copy()).to(DEV)
+    bs.layered_package_unpack(d_slots.data_ptr(), slot_bytes, n + 2, SID, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr,
+                              ws.nbytes, ws.result_ptr, opts, bs.current_stream())
+    assert ws.read_result()["status"] == bs.ERR_CORRUPT and (pool.cpu().numpy() == 0xEE).all()
