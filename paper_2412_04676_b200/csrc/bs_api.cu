@@ -178,8 +178,19 @@ int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const Pkg
 }
 
 // payload only: the header region was gathered and parsed before (header = nullptr: no descriptor rebuild here)
+int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, uint32_t flags,
+                              const bs_opts& o, int sms, cudaStream_t stream);
+
 int run_unpack_packages(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t header_bytes, uint32_t flags,
                         const bs_opts& o, int sms, cudaStream_t stream)
+{
+    (void)header_bytes;
+    return run_unpack_packages_range(out, L, pm, 0, UINT64_MAX, flags, o, sms, stream);
+}
+
+// payload bytes of the stream range [lo, hi) (whole packages of the cut) out of their slots
+int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, uint32_t flags,
+                              const bs_opts& o, int sms, cudaStream_t stream)
 {
     MoveParams mp;
     memset(&mp, 0, sizeof(mp));
@@ -188,13 +199,12 @@ int run_unpack_packages(const bs_set_desc* out, const WsLayout& L, const PkgMap&
     mp.qn = out->qn;
     mp.dim = out->dim;
     mp.addr = out->addr;
-    mp.lo = 0;
-    mp.hi = UINT64_MAX;
+    mp.lo = lo;
+    mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
     mp.flags = flags;
     mp.pkg = pm;
-    (void)header_bytes;
     cudaError_t e = launch_move(true, mp, o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;

@@ -35,6 +35,8 @@ int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_sr
                      uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream);
 int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, const bs_opts& o,
                             int sms, cudaStream_t stream);
+int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, uint32_t flags,
+                              const bs_opts& o, int sms, cudaStream_t stream);
 // wire format v2 (bs_layered.cu)
 int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t capacity,
                                uint64_t expect_total, bs_result* d_result, int sms, cudaStream_t stream);
@@ -560,6 +562,7 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
     // arrival order: each payload package is unpacked on its own; runs of consecutive slots that fit a staging buffer
     // come over in ONE DMA (what lies behind a short package inside the run is read and ignored)
     const uint64_t per_buf = std::max<uint64_t>(1, e->cfg.chunk_bytes / slot_bytes);
+    const uint64_t cut = plan_uniform_cap(plan, e->opts.tile_bytes ? e->opts.tile_bytes : 32768u);  // 32 KiB: the unpack preset's tile
     uint64_t batch = 0;
     for (size_t i = 0; i < by_slot.size(); ++batch) {
         const uint32_t b = (uint32_t)(batch % S);
@@ -571,12 +574,22 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
         CK(cudaMemcpyAsync(e->staging[b], src, bytes, cudaMemcpyHostToDevice, e->cstream));
         CK(cudaEventRecord(e->ev_c[b], e->cstream));
         CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));
-        for (size_t j = 0; j < n; ++j) {
-            const PkgItem& it = by_slot[i + j];
-            const unsigned char* d = e->staging[b] + (n == 1 ? 0 : j * slot_bytes + BS_PKG_HEADER);
-            if ((rc = run_unpack_range(out, L, d, nullptr, it.lo, it.lo + it.nbytes, flags | kFlagCheckPad, e->opts, e->sms,
-                                       e->kstream)))
+        bool in_order = cut != 0 && n > 1;  // consecutive packages of the cut in consecutive slots: one launch for the batch
+        for (size_t j = 1; in_order && j < n; ++j) in_order = by_slot[i + j].index == by_slot[i + j - 1].index + 1;
+        if (in_order) {
+            PkgMap pm;
+            pm.cap = cut; pm.slot_bytes = slot_bytes; pm.base = e->staging[b]; pm.slot_of = nullptr; pm.k_base = by_slot[i].index;
+            if ((rc = run_unpack_packages_range(out, L, pm, by_slot[i].lo, by_slot[i + n - 1].lo + by_slot[i + n - 1].nbytes,
+                                                flags | kFlagCheckPad, e->opts, e->sms, e->kstream)))
                 return rc;
+        } else {
+            for (size_t j = 0; j < n; ++j) {
+                const PkgItem& it = by_slot[i + j];
+                const unsigned char* d = e->staging[b] + (n == 1 ? 0 : j * slot_bytes + BS_PKG_HEADER);
+                if ((rc = run_unpack_range(out, L, d, nullptr, it.lo, it.lo + it.nbytes, flags | kFlagCheckPad, e->opts, e->sms,
+                                           e->kstream)))
+                    return rc;
+            }
         }
         CK(cudaEventRecord(e->ev_k[b], e->kstream));
         i += n;
