@@ -1,6 +1,6 @@
 /*
  * bs.h — C ABI of libbsstream: serialize / deserialize / offload / prefetch of symmetry-blocked
- * (U(1) quantum-number-labelled) block-sparse fp64 matrices and rank-3 tensors on one NVIDIA B200.
+ * (U(1) quantum-number-labelled) block-sparse matrices and rank-3 tensors (fp64; also f32 / c64 / c128) on one NVIDIA B200.
  *
  * The operations are those of arXiv 2412.04676 (Menczer & Legeza), /root/reference/PAPER.md:
  *   - §III (L85): saving scratch data = (1) serialization, "generating long continuous stripes in
@@ -24,7 +24,7 @@
  *     Errors detected on the device (capacity, corrupt header, bad descriptor) are DEFERRED: they land
  *     in bs_result.status (device memory) and, for engine calls, in the ticket.  When status != BS_OK
  *     no stream / block / descriptor output has been written by the data-movement kernels.
- *   - The path does no floating-point arithmetic: fp64 values move as opaque 8-byte words; results
+ *   - The path does no floating-point arithmetic: values move as opaque words of their element size; results
  *     are bit-exact (tolerance 0).
  *   - Thread-safety: functions are re-entrant; one bs_engine must be driven by one host thread.
  *   - There is no CPU fallback: without a CUDA device every device-touching call fails with BS_ERR_CUDA.
@@ -63,7 +63,7 @@ enum {
     BS_ERR_ARG = -1,         /* NULL / misaligned pointer, bad descriptor partition, size overflow */
     BS_ERR_CAPACITY = -2,    /* stream / pool / workspace / descriptor arrays too small */
     BS_ERR_CORRUPT = -3,     /* header validation failed; nothing was written */
-    BS_ERR_UNSUPPORTED = -4, /* rank not in {2,3}, dtype != f64, n_qn != 2 */
+    BS_ERR_UNSUPPORTED = -4, /* rank not in {2,3}, unknown dtype (layered sets: dtype != f64), n_qn != 2 */
     BS_ERR_CUDA = -5,        /* a CUDA runtime call failed; see bs_last_cuda_error() */
     BS_ERR_IO = -6           /* the storage tier of a bs_queue: open / read / write of a file failed (errno is the C library's) */
 };
@@ -385,8 +385,11 @@ int bs_layered_package_unpack(const void *d_slots, uint64_t slot_bytes, uint64_t
 
 /* The same through the engine, slots in pinned HOST memory (the receive buffers of L126): package k is packed into a
  * staging buffer behind its header and DMA'd to h_slots + slot(k)*slot_bytes; cap + 64 <= chunk_bytes.  Prefetch takes
- * the slots in the order they lie (arrival order): header-region packages first, then every payload package is DMA'd
- * and unpacked on its own.  Ticket / checkpoint semantics as bs_offload_async / bs_prefetch_async. */
+ * the slots in the order they lie (arrival order): header-region packages first, then every payload package is unpacked
+ * on its own.  A staging buffer takes a batch of packages: with slot_bytes == 64 + cap, packages whose host slots are
+ * consecutive cross the link in one DMA (a short package ends its batch, so nothing behind it is written), and limits that
+ * are a multiple of the work tile cost two launches per batch.  ticket n_chunks = number of packages, bytes = stream bytes
+ * + 64 per package.  Ticket / checkpoint semantics as bs_offload_async / bs_prefetch_async. */
 int bs_offload_packages_async(bs_engine *e, const bs_set_desc *set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id,
                               void *h_slots, uint64_t slot_bytes, uint64_t n_slots, const uint32_t *h_slot_of,
                               cudaStream_t producer, bs_ticket **ticket);
