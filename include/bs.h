@@ -396,6 +396,13 @@ int bs_offload_packages_async(bs_engine *e, const bs_set_desc *set, uint64_t tot
 int bs_prefetch_packages_async(bs_engine *e, const void *h_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id,
                                bs_set_desc *out, void *d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer,
                                bs_ticket **ticket);
+/* and for layered sets (packages of a wire-format-v2 stream) */
+int bs_offload_layered_packages_async(bs_engine *e, const bs_layered_desc *set, uint64_t total_bytes, uint64_t cap,
+                                      uint64_t stream_id, void *h_slots, uint64_t slot_bytes, uint64_t n_slots,
+                                      const uint32_t *h_slot_of, cudaStream_t producer, bs_ticket **ticket);
+int bs_prefetch_layered_packages_async(bs_engine *e, const void *h_slots, uint64_t slot_bytes, uint64_t n_slots,
+                                       uint64_t stream_id, bs_layered_desc *out, void *d_pool, uint64_t pool_bytes,
+                                       uint32_t flags, cudaStream_t consumer, bs_ticket **ticket);
 
 /* ==== save / load queue with checkpoints (PAPER §III.B.4) ============================
  *

@@ -158,6 +158,8 @@ def lib():
     L.bs_layered_package_unpack.argtypes = [vp, u64, u64, u64, LD, vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_offload_packages_async.argtypes = [vp, C.POINTER(SetDesc), u64, u64, u64, vp, u64, u64, pu32, vp, C.POINTER(vp)]
     L.bs_prefetch_packages_async.argtypes = [vp, vp, u64, u64, u64, C.POINTER(SetDesc), vp, u64, u32, vp, C.POINTER(vp)]
+    L.bs_offload_layered_packages_async.argtypes = [vp, LD, u64, u64, u64, vp, u64, u64, pu32, vp, C.POINTER(vp)]
+    L.bs_prefetch_layered_packages_async.argtypes = [vp, vp, u64, u64, u64, LD, vp, u64, u32, vp, C.POINTER(vp)]
     L.bs_queue_create.argtypes = [C.POINTER(vp), C.POINTER(EngineCfg)]
     L.bs_queue_destroy.argtypes = [vp]
     L.bs_queue_save.argtypes = [vp, u64, C.POINTER(SetDesc), u64, vp, u64, vp]
@@ -420,6 +422,21 @@ class Engine:
         t = C.c_void_p(0)
         _check(lib().bs_prefetch_packages_async(self._h, h_slots_ptr, slot_bytes, n_slots, stream_id, C.byref(out), pool_ptr,
                                                 pool_bytes, flags, consumer, C.byref(t)), "bs_prefetch_packages_async")
+        return Ticket(t.value)
+
+    def offload_layered_packages_async(self, desc: LayeredDesc, total_bytes: int, cap: int, stream_id: int, h_slots_ptr: int,
+                                       slot_bytes: int, n_slots: int, slot_of=None, producer: int = 0) -> Ticket:
+        t = C.c_void_p(0)
+        _check(lib().bs_offload_layered_packages_async(self._h, C.byref(desc), total_bytes, cap, stream_id, h_slots_ptr, slot_bytes,
+                                                       n_slots, _slot_map(slot_of), producer, C.byref(t)),
+               "bs_offload_layered_packages_async")
+        return Ticket(t.value)
+
+    def prefetch_layered_packages_async(self, h_slots_ptr: int, slot_bytes: int, n_slots: int, stream_id: int, out: LayeredDesc,
+                                        pool_ptr: int, pool_bytes: int, flags: int = 0, consumer: int = 0) -> Ticket:
+        t = C.c_void_p(0)
+        _check(lib().bs_prefetch_layered_packages_async(self._h, h_slots_ptr, slot_bytes, n_slots, stream_id, C.byref(out), pool_ptr,
+                                                        pool_bytes, flags, consumer, C.byref(t)), "bs_prefetch_layered_packages_async")
         return Ticket(t.value)
 
     def offload_layered_async(self, desc: LayeredDesc, total_bytes: int, h_pinned_ptr: int, h_capacity: int,

@@ -38,6 +38,7 @@ int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const Pkg
 int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, uint32_t flags,
                               const bs_opts& o, int sms, cudaStream_t stream);
 // wire format v2 (bs_layered.cu)
+bool layered_ws(void* d_ws, uint64_t ws_bytes, uint32_t Bs, uint32_t T, uint64_t B, WsLayout* out);
 int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t capacity,
                                uint64_t expect_total, bs_result* d_result, int sms, cudaStream_t stream);
 int run_layered_deserialize_plan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_layered_desc* out,
@@ -414,22 +415,34 @@ int bs_prefetch_layered_async(bs_engine* e, const void* h_pinned, uint64_t nbyte
 }
 
 // ---- self-contained packages through the engine (bs.h "packages") ------------------------------------
-int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id,
-                              void* h_slots, uint64_t slot_bytes, uint64_t n_slots, const uint32_t* h_slot_of,
-                              cudaStream_t producer, bs_ticket** ticket)
+// one body for both wire formats: exactly one of set / lset is non-null
+static int offload_packages_impl(bs_engine* e, const bs_set_desc* set, const bs_layered_desc* lset, uint64_t total_bytes, uint64_t cap,
+                                 uint64_t stream_id, void* h_slots, uint64_t slot_bytes, uint64_t n_slots, const uint32_t* h_slot_of,
+                                 cudaStream_t producer, bs_ticket** ticket)
 {
-    if (e == nullptr || set == nullptr || h_slots == nullptr || ticket == nullptr) return BS_ERR_ARG;
+    if (e == nullptr || (set == nullptr && lset == nullptr) || h_slots == nullptr || ticket == nullptr) return BS_ERR_ARG;
     if (cap == 0 || (cap & 15) || (slot_bytes & 15) || slot_bytes < BS_PKG_HEADER + cap) return BS_ERR_ARG;
     if (cap + BS_PKG_HEADER > e->cfg.chunk_bytes) return BS_ERR_CAPACITY;
-    if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
     WsLayout L;
-    if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
+    uint64_t hb;
+    if (set) {
+        if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
+        if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
+        hb = bs_header_bytes(set->n_tensors, set->n_blocks);
+    } else {
+        if (lset->n_structs > e->cfg.max_tensors || lset->n_layers > e->cfg.max_tensors ||
+            lset->n_struct_blocks > e->cfg.max_blocks || lset->n_addr > e->cfg.max_blocks)
+            return BS_ERR_CAPACITY;
+        if (!layered_ws(e->ws, e->ws_bytes, lset->n_struct_blocks, lset->n_layers, lset->n_addr, &L)) return BS_ERR_CAPACITY;
+        hb = bs_layered_header_bytes(lset->n_structs, lset->n_layers, lset->n_struct_blocks);
+    }
     int rc;
-    uint64_t hb = bs_header_bytes(set->n_tensors, set->n_blocks);
     if (total_bytes == 0) {
         CK(cudaEventRecord(e->ev_fence_k, e->kstream));  // the workspace may still be in use by an earlier call
         CK(cudaStreamWaitEvent(producer, e->ev_fence_k, 0));
-        if ((rc = bs_serialized_size(set, e->ws, e->ws_bytes, &hb, &total_bytes, producer))) return rc;
+        rc = set ? bs_serialized_size(set, e->ws, e->ws_bytes, &hb, &total_bytes, producer)
+                 : bs_layered_serialized_size(lset, e->ws, e->ws_bytes, &hb, &total_bytes, producer);
+        if (rc) return rc;
     }
     if (total_bytes > e->cfg.max_stream_bytes) return BS_ERR_CAPACITY;
     const uint64_t count = pkg_count(hb, total_bytes, cap);
@@ -453,7 +466,9 @@ int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t tot
     CK(cudaEventRecord(e->ev_dep, producer));
     CK(cudaStreamWaitEvent(e->kstream, e->ev_dep, 0));
     CK(cudaEventRecord(t->t_begin, e->kstream));
-    if ((rc = run_serialize_scan(set, L, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream))) return rc;
+    rc = set ? run_serialize_scan(set, L, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream)
+             : run_layered_serialize_plan(lset, e->ws, e->ws_bytes, UINT64_MAX, total_bytes, e->d_result, e->sms, e->kstream);
+    if (rc) return rc;
     // A staging buffer takes a BATCH of packages laid out as slots, and the batch leaves in ONE DMA, when the slots are
     // exactly header + limit long and the batch's host slots are consecutive; a short package (the last one of the header
     // region / of the payload) ends its batch, so no byte behind a short package is written on the host.
@@ -478,7 +493,9 @@ int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t tot
             if (!one_launch) {
                 unsigned char* dst = e->staging[b] + m * slot_bytes;
                 CK(launch_pkg_header(L, cap, stream_id, k, count, dst, e->d_result, e->kstream));
-                if ((rc = run_pack_range(set, L, dst + BS_PKG_HEADER, lo, hi, e->opts, e->sms, e->kstream))) return rc;
+                rc = set ? run_pack_range(set, L, dst + BS_PKG_HEADER, lo, hi, e->opts, e->sms, e->kstream)
+                         : run_layered_pack_range(lset, e->ws, e->ws_bytes, dst + BS_PKG_HEADER, lo, hi, e->opts, e->sms, e->kstream);
+                if (rc) return rc;
             }
             last_bytes = hi - lo;
             if (last_bytes != cap) { ++k; ++m; break; }  // a short package ends its batch
@@ -487,7 +504,9 @@ int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t tot
             CK(launch_pkg_headers(L, cap, stream_id, k0, m, count, e->staging[b], slot_bytes, nullptr, e->d_result, e->kstream));
             PkgMap pm;
             pm.cap = cap; pm.slot_bytes = slot_bytes; pm.base = e->staging[b]; pm.slot_of = nullptr; pm.k_base = k0;
-            if ((rc = run_pack_packages_range(set, L, pm, lo0, hi1, e->opts, e->sms, e->kstream))) return rc;
+            rc = set ? run_pack_packages_range(set, L, pm, lo0, hi1, e->opts, e->sms, e->kstream)
+                     : run_layered_pack_range(lset, e->ws, e->ws_bytes, nullptr, lo0, hi1, e->opts, e->sms, e->kstream, &pm);
+            if (rc) return rc;
         }
         if (k0 == 0) CK(post_result(t->h_result, e->d_result, e->kstream));
         CK(cudaEventRecord(e->ev_k[b], e->kstream));
@@ -503,11 +522,11 @@ int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t tot
     return BS_OK;
 }
 
-int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id,
-                               bs_set_desc* out, void* d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer,
-                               bs_ticket** ticket)
+static int prefetch_packages_impl(bs_engine* e, const void* h_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id,
+                                  bs_set_desc* out, bs_layered_desc* lout, void* d_pool, uint64_t pool_bytes, uint32_t flags,
+                                  cudaStream_t consumer, bs_ticket** ticket)
 {
-    if (e == nullptr || h_slots == nullptr || out == nullptr || ticket == nullptr || n_slots == 0) return BS_ERR_ARG;
+    if (e == nullptr || h_slots == nullptr || (out == nullptr && lout == nullptr) || ticket == nullptr || n_slots == 0) return BS_ERR_ARG;
     if ((slot_bytes & 15) || slot_bytes < BS_PKG_HEADER + 16) return BS_ERR_ARG;
     if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
     const unsigned char* slots = (const unsigned char*)h_slots;
@@ -515,9 +534,16 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
     int rc = pkg_plan(slots, slot_bytes, n_slots, slot_bytes, stream_id, &plan);
     if (rc) return rc;
     if (plan.hb > e->header_cap || plan.total > e->cfg.max_stream_bytes) return BS_ERR_CAPACITY;
-    if (out->n_blocks > e->cfg.max_blocks || out->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
     WsLayout L;
-    if (!ws_layout(e->ws, e->ws_bytes, out->n_blocks, &L)) return BS_ERR_CAPACITY;
+    if (out) {
+        if (out->n_blocks > e->cfg.max_blocks || out->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
+        if (!ws_layout(e->ws, e->ws_bytes, out->n_blocks, &L)) return BS_ERR_CAPACITY;
+    } else {
+        if (lout->n_structs > e->cfg.max_tensors || lout->n_layers > e->cfg.max_tensors ||
+            lout->n_struct_blocks > e->cfg.max_blocks || lout->n_addr > e->cfg.max_blocks)
+            return BS_ERR_CAPACITY;
+        if (!layered_ws(e->ws, e->ws_bytes, lout->n_struct_blocks, lout->n_layers, lout->n_addr, &L)) return BS_ERR_CAPACITY;
+    }
     for (const PkgItem& it : plan.items)
         if (it.nbytes > e->cfg.chunk_bytes) return BS_ERR_CAPACITY;
     if (n_slots > e->pkg_tab_slots) {  // a call-time allocation, only when a call brings more slots than any before
@@ -551,12 +577,15 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
     }
     CK(cudaEventRecord(e->ev_fence_c, e->cstream));
     CK(cudaStreamWaitEvent(e->kstream, e->ev_fence_c, 0));
-    if ((rc = run_deserialize_scan(e->header_buf, nullptr, plan.total, out, d_pool, pool_bytes, flags, L, e->d_result, e->sms,
-                                   e->kstream)))
-        return rc;
+    rc = out ? run_deserialize_scan(e->header_buf, nullptr, plan.total, out, d_pool, pool_bytes, flags, L, e->d_result, e->sms, e->kstream)
+             : run_layered_deserialize_plan(e->header_buf, nullptr, plan.total, lout, d_pool, pool_bytes, flags, e->ws, e->ws_bytes,
+                                            e->d_result, e->sms, e->kstream);
+    if (rc) return rc;
     CK(launch_pkg_check(L, e->pkg_tab, BS_PKG_HEADER, n_slots, stream_id, e->d_result, e->kstream));
     CK(post_result(t->h_result, e->d_result, e->kstream));
-    if ((rc = run_unpack_range(out, L, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream))) return rc;
+    rc = out ? run_unpack_range(out, L, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream)
+             : run_layered_unpack_range(lout, e->ws, e->ws_bytes, e->header_buf, e->header_buf, 0, 0, flags, e->opts, e->sms, e->kstream);
+    if (rc) return rc;
     std::vector<PkgItem> by_slot(plan.items.begin() + plan.n_header, plan.items.end());
     std::sort(by_slot.begin(), by_slot.end(), [](const PkgItem& a, const PkgItem& b) { return a.slot < b.slot; });
     // arrival order: each payload package is unpacked on its own; runs of consecutive slots that fit a staging buffer
@@ -579,16 +608,19 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
         if (in_order) {
             PkgMap pm;
             pm.cap = cut; pm.slot_bytes = slot_bytes; pm.base = e->staging[b]; pm.slot_of = nullptr; pm.k_base = by_slot[i].index;
-            if ((rc = run_unpack_packages_range(out, L, pm, by_slot[i].lo, by_slot[i + n - 1].lo + by_slot[i + n - 1].nbytes,
-                                                flags | kFlagCheckPad, e->opts, e->sms, e->kstream)))
-                return rc;
+            const uint64_t blo = by_slot[i].lo, bhi = by_slot[i + n - 1].lo + by_slot[i + n - 1].nbytes;
+            rc = out ? run_unpack_packages_range(out, L, pm, blo, bhi, flags | kFlagCheckPad, e->opts, e->sms, e->kstream)
+                     : run_layered_unpack_range(lout, e->ws, e->ws_bytes, nullptr, nullptr, blo, bhi, flags | kFlagCheckPad, e->opts,
+                                                e->sms, e->kstream, &pm);
+            if (rc) return rc;
         } else {
             for (size_t j = 0; j < n; ++j) {
                 const PkgItem& it = by_slot[i + j];
                 const unsigned char* d = e->staging[b] + (n == 1 ? 0 : j * slot_bytes + BS_PKG_HEADER);
-                if ((rc = run_unpack_range(out, L, d, nullptr, it.lo, it.lo + it.nbytes, flags | kFlagCheckPad, e->opts, e->sms,
-                                           e->kstream)))
-                    return rc;
+                rc = out ? run_unpack_range(out, L, d, nullptr, it.lo, it.lo + it.nbytes, flags | kFlagCheckPad, e->opts, e->sms, e->kstream)
+                         : run_layered_unpack_range(lout, e->ws, e->ws_bytes, d, nullptr, it.lo, it.lo + it.nbytes, flags | kFlagCheckPad,
+                                                    e->opts, e->sms, e->kstream);
+                if (rc) return rc;
             }
         }
         CK(cudaEventRecord(e->ev_k[b], e->kstream));
@@ -600,6 +632,38 @@ int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_
     CK(cudaStreamWaitEvent(consumer, t->done, 0));
     *ticket = guard.release();
     return BS_OK;
+}
+
+int bs_offload_packages_async(bs_engine* e, const bs_set_desc* set, uint64_t total_bytes, uint64_t cap, uint64_t stream_id,
+                              void* h_slots, uint64_t slot_bytes, uint64_t n_slots, const uint32_t* h_slot_of,
+                              cudaStream_t producer, bs_ticket** ticket)
+{
+    if (set == nullptr) return BS_ERR_ARG;
+    return offload_packages_impl(e, set, nullptr, total_bytes, cap, stream_id, h_slots, slot_bytes, n_slots, h_slot_of, producer, ticket);
+}
+
+int bs_offload_layered_packages_async(bs_engine* e, const bs_layered_desc* set, uint64_t total_bytes, uint64_t cap,
+                                      uint64_t stream_id, void* h_slots, uint64_t slot_bytes, uint64_t n_slots,
+                                      const uint32_t* h_slot_of, cudaStream_t producer, bs_ticket** ticket)
+{
+    if (set == nullptr) return BS_ERR_ARG;
+    return offload_packages_impl(e, nullptr, set, total_bytes, cap, stream_id, h_slots, slot_bytes, n_slots, h_slot_of, producer, ticket);
+}
+
+int bs_prefetch_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id,
+                               bs_set_desc* out, void* d_pool, uint64_t pool_bytes, uint32_t flags, cudaStream_t consumer,
+                               bs_ticket** ticket)
+{
+    if (out == nullptr) return BS_ERR_ARG;
+    return prefetch_packages_impl(e, h_slots, slot_bytes, n_slots, stream_id, out, nullptr, d_pool, pool_bytes, flags, consumer, ticket);
+}
+
+int bs_prefetch_layered_packages_async(bs_engine* e, const void* h_slots, uint64_t slot_bytes, uint64_t n_slots, uint64_t stream_id,
+                                       bs_layered_desc* out, void* d_pool, uint64_t pool_bytes, uint32_t flags,
+                                       cudaStream_t consumer, bs_ticket** ticket)
+{
+    if (out == nullptr) return BS_ERR_ARG;
+    return prefetch_packages_impl(e, h_slots, slot_bytes, n_slots, stream_id, nullptr, out, d_pool, pool_bytes, flags, consumer, ticket);
 }
 
 int bs_ticket_query(const bs_ticket* t)

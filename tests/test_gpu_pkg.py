@@ -405,3 +405,36 @@ def test_layered_packages_match_the_oracle_and_unpack_in_any_order(cap, variant)
     bs.layered_package_unpack(d_slots.data_ptr(), slot_bytes, n + 2, SID, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr,
                               ws.nbytes, ws.result_ptr, opts, bs.current_stream())
     assert ws.read_result()["status"] == bs.ERR_CORRUPT and (pool.cpu().numpy() == 0xEE).all()
+
+
+@pytest.mark.parametrize("cap,chunk,shuffle", [(32768, 5 * 65536, False), (65536, 4 * 65536 + 65536, True), (4096 + 16, 65536, False)])
+def test_engine_layered_packages_round_trip(cap, chunk, shuffle):
+    from oracle import v2
+    from tests.test_gpu_layered import LayeredUp
+    bset = W.make_config("2", n_ops=39)
+    lu = LayeredUp(bset)
+    want = lu.want
+    total = len(want)
+    c = lu.counts
+    hb = bs.layered_header_bytes(c[0], c[2], c[1])
+    n = pkg.count(hb, total, cap)
+    slot_bytes = 64 + cap
+    slot_of = np.random.default_rng(12).permutation(n + 1)[:n] if shuffle else None
+    ref_slots = pkg.emit_slots(want, cap, SID, slot_bytes, slot_of=slot_of, n_slots=n + 1, poison=POISON)
+    eng = bs.Engine(max(c[0], c[2]), max(c[1], c[3]), total + 4096, chunk_bytes=chunk, n_staging=2)
+    host = pinned((n + 1) * slot_bytes, POISON)
+    st = eng.offload_layered_packages_async(lu.dset.desc, total if shuffle else 0, cap, SID, host.data_ptr(), slot_bytes, n + 1,
+                                            slot_of, bs.current_stream()).wait()
+    assert st["status"] == bs.OK and st["n_chunks"] == n
+    assert (host.numpy().reshape(n + 1, slot_bytes) == ref_slots).all(), "host packages differ from the oracle's"
+    ref = v2.deserialize(want)
+    na, need = v2.counts(want)
+    out = bs.DeviceLayeredSet.empty(*c, DEV, fill=0xAB)
+    pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    st2 = eng.prefetch_layered_packages_async(host.data_ptr(), slot_bytes, n + 1, SID, out.desc, pool.data_ptr(), need,
+                                              bs.LAYOUT_POOL, bs.current_stream()).wait()
+    torch.cuda.synchronize()
+    assert st2["status"] == bs.OK and (pool.cpu().numpy() == ref["pool"][:need]).all()
+    h = out.to_host(*c)
+    assert h["structs"].tobytes() == ref["structs"].tobytes() and h["layers"].tobytes() == ref["layers"].tobytes()
+    eng.destroy()
