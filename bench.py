@@ -10,13 +10,17 @@ metric's "% of HBM peak" is meaningful on; inputs are ~7 GB, far larger than the
 
     value     stream bytes serialized + deserialized per second (GB/s), inputs resident in HBM, CUDA events.
               HBM traffic is 2 bytes per stream byte, so HBM GB/s = 2 * value.
-    e2e       the same stream bytes through bs_offload_async + bs_prefetch_async with HOST (pinned) buffers:
-              pack -> D2H and H2D -> unpack in 256 MiB double-buffered chunks; PCIe-bound.
+    e2e       the same stream bytes through HOST (pinned) buffers, copies inside the timed region (bs_queue_save overlapped
+              with bs_queue_load); PCIe-bound.  Carries the north_star's offload bars too: offload / prefetch GB/s as a
+              fraction of the pinned cudaMemcpyAsync bandwidth of the same run, and the exposed-IO fraction of an
+              offload / a prefetch of config 3 hidden behind a stand-in contraction at r = T_c / T_io = 1.25 (config 5).
     roofline  the dominant kernel (pack): algorithmic HBM bytes per launch / its CUDA-event duration, against the
-              measured copy bandwidth in MEASURED_PEAKS.json.
-    cpu_baseline  the CPU oracle (oracle/, single thread, as it stands) on a bounded sample of the same workload.
-    detail    per-direction numbers, PCIe fractions and the config-5 exposed-IO measurement (offload of config 3
-              overlapped with a stand-in contraction).
+              measured copy bandwidth in MEASURED_PEAKS.json; beside it the unpack kernel, the whole-call fractions of the
+              8 TB/s nominal figure, an in-run ceiling (the same mover on ONE contiguous block: a pure cp.async.bulk
+              copy) and ``at_scale``: the same numbers on workload 4L (42.5 GB, the total BASELINE.json states).
+    cpu_baseline  the CPU oracle (oracle/, single thread, as it stands) on a bounded sample of the same workload, plus
+              the paper's own design as context: threads filling disjoint intervals of one buffer (L106-108).
+    detail    (last key, context only) per-direction numbers, packages, small sets, the config-5 sweeps.
 
 --impl reference times the oracle itself on the box's host cores (this tier's reference arm).
 With N > 1 (torchrun) every rank runs an independent replica on its own GPU (the path has no exchange step:
@@ -162,74 +166,128 @@ def oracle_sample(workload: str, sample_mb: float, fmt: str = "v1"):
     return bset, sub, n_t, b1
 
 
-def time_oracle_v2(sub, min_seconds: float, max_passes: int = 1000):
-    """As time_oracle, for wire format v2 (oracle.v2) on the layered form of the same sample."""
-    from oracle import v2
-    lv = sub["layered"]
-    hb, total = v2.serialized_size(lv["structs"], lv["layers"], lv["dim"])
-    out = np.empty(total, np.uint8)
-    pool = None
-    passes, t_acc = 0, 0.0
-    while passes == 0 or (t_acc < min_seconds and passes < max_passes):
+class OracleRunner:
+    """serialize + deserialize passes of the oracle, single thread, on a prepared sample.  The output stream and the pool
+    are allocated and touched ONCE, so the reference arm and the cpu_baseline leg time the same thing (round 1's reference
+    arm re-allocated them every step and paid the first-touch page faults inside its timed region)."""
+
+    def __init__(self, sub):
+        if "layered" in sub:
+            from oracle import v2
+            lv = sub["layered"]
+            self.hb, self.total = v2.serialized_size(lv["structs"], lv["layers"], lv["dim"])
+            self.out = np.zeros(self.total, np.uint8)
+            self._ser = lambda: v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], sub["addr"], capacity=self.total,
+                                             out=self.out)
+            self.pool = np.zeros(max(v2.counts(self._ser())[1], 1), np.uint8)
+            self._des = lambda s: v2.deserialize(s, pool=self.pool)
+        else:
+            import oracle
+            self.hb, self.total = oracle.serialized_size(len(sub["tensors"]), sub["dim"])
+            self.out = np.zeros(self.total, np.uint8)
+            self._ser = lambda: oracle.serialize(sub["tensors"], sub["qn"], sub["dim"], sub["addr"], capacity=self.total, out=self.out)
+            self.pool = np.zeros(max(oracle.pool_bytes(self._ser()), 1), np.uint8)
+            self._des = lambda s: oracle.deserialize(s, pool=self.pool)
+        self.one_pass()   # everything mapped and warm
+
+    def one_pass(self) -> float:
         t0 = time.perf_counter()
-        s = v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], sub["addr"], capacity=total, out=out)
-        if pool is None:
-            t_acc += time.perf_counter() - t0
-            pool = np.empty(max(v2.counts(s)[1], 1), np.uint8)
-            t0 = time.perf_counter()
-        v2.deserialize(s, pool=pool)
-        t_acc += time.perf_counter() - t0
-        passes += 1
-    return t_acc, passes, total
+        self._des(self._ser())
+        return time.perf_counter() - t0
+
+    def run_for(self, min_seconds: float, max_passes: int = 1000):
+        """(seconds, passes): at least one pass, then until min_seconds of CPU work."""
+        passes, acc = 0, 0.0
+        while passes == 0 or (acc < min_seconds and passes < max_passes):
+            acc += self.one_pass()
+            passes += 1
+        return acc, passes
 
 
-def time_oracle(sub, min_seconds: float, max_passes: int = 1000):
-    """serialize + deserialize passes of the oracle, single thread.  Returns (seconds, passes, stream_bytes)."""
-    if "layered" in sub:
-        return time_oracle_v2(sub, min_seconds, max_passes)
+def oracle_threads_sweep(sub, seconds_each: float = 2.0):
+    """Context row (optional): the PAPER'S OWN DESIGN on this box's host cores — the main thread maps the one
+    output buffer from the predicted sizes, then threads fill disjoint intervals in complete independence (L106-108); the
+    paper sees saturation at 32 threads (L158).  The oracle is unchanged: every thread calls its slice-wise
+    emit_payload_range on its own tensor ranges (ctypes drops the GIL).  Serialize only; baseline only."""
     import oracle
-    hb, total = oracle.serialized_size(len(sub["tensors"]), sub["dim"])
-    out = np.empty(total, np.uint8)
-    need = None
-    passes, t_acc = 0, 0.0
-    pool = None
-    while passes == 0 or (t_acc < min_seconds and passes < max_passes):
-        t0 = time.perf_counter()
-        s = oracle.serialize(sub["tensors"], sub["qn"], sub["dim"], sub["addr"], capacity=total, out=out)
-        if need is None:
-            t_acc += time.perf_counter() - t0
-            need = oracle.pool_bytes(s)
-            pool = np.empty(max(need, 1), np.uint8)
-            t0 = time.perf_counter()
-        oracle.deserialize(s, pool=pool)
-        t_acc += time.perf_counter() - t0
-        passes += 1
-    return t_acc, passes, total
+    from concurrent.futures import ThreadPoolExecutor
+    tensors, dim, addr = sub["tensors"], sub["dim"], sub["addr"]
+    T = len(tensors)
+    hb, total = oracle.serialized_size(T, dim)
+    _, stored, off, P = oracle.plan(dim)                     # the main thread's map of the buffer (L106)
+    out = np.zeros(total, np.uint8)
+    payload = out[hb:]
+    fb = tensors["first_block"].astype(np.int64)
+    end_b = fb + tensors["n_blocks"].astype(np.int64)
+    cores = os.cpu_count() or 1
+    rows = []
+    for n_thr in sorted({1, min(32, cores), cores}):
+        # ~4 ranges per thread, cut at tensor boundaries at ~equal bytes
+        n_rng = max(1, min(T, 4 * n_thr))
+        t_end_off = np.array([int(off[e - 1] + stored[e - 1]) if e > 0 else 0 for e in end_b])
+        cuts = [0] + [int(np.searchsorted(t_end_off, P * k / n_rng, side="left")) + 1 for k in range(1, n_rng)] + [T]
+        cuts = sorted(set(min(max(c, 0), T) for c in cuts))
+        jobs = []
+        for t0, t1 in zip(cuts[:-1], cuts[1:]):
+            lo = int(off[fb[t0]]) if fb[t0] < len(off) else P
+            hi = t_end_off[t1 - 1]
+            jobs.append((t0, t1, lo, hi - lo))
+
+        def work(j):
+            t0, t1, lo, n = j
+            first, got = oracle.emit_payload_range(tensors, dim, addr, t0, t1, n, out=payload[lo: lo + n] if n else payload[:1])
+            assert first == lo and len(got) == n
+            return n
+
+        with ThreadPoolExecutor(max_workers=n_thr) as ex:
+            list(ex.map(work, jobs))                         # warm
+            passes, t0 = 0, time.perf_counter()
+            while passes == 0 or time.perf_counter() - t0 < seconds_each:
+                moved = sum(ex.map(work, jobs))
+                passes += 1
+            sec = time.perf_counter() - t0
+        assert moved == P
+        rows.append({"threads": n_thr, "serialize_stream_GBs": round(passes * P / sec / 1e9, 2), "ranges": len(jobs)})
+    return rows
 
 
 def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return
+    import oracle
     log(f"[reference] oracle on a {args.sample_mb:.0f} MB sample of workload {args.workload}")
     bset, sub, n_t, b1 = oracle_sample(args.workload, args.sample_mb, args.format)
-    time_oracle(sub, 0.0, max_passes=max(1, args.warmup))           # warm-up passes
-    per = []
-    total = 0
-    for _ in range(args.steps):
-        sec, passes, total = time_oracle(sub, 0.0, max_passes=1)
-        per.append(sec)
+    runner = OracleRunner(sub)
+    for _ in range(max(0, args.warmup - 1)):
+        runner.one_pass()
+    per = [runner.one_pass() for _ in range(args.steps)]
     ms = 1e3 * float(np.mean(per))
-    value = 2 * total / (ms * 1e-3) / 1e9
-    sample = f"first {n_t} of {bset.n_tensors} tensors ({b1} blocks, {total / 1e6:.0f} MB stream) of workload {args.workload}"
+    sbytes = runner.total
+    value = 2 * sbytes / (ms * 1e-3) / 1e9
+    full_total = full_stream_bytes(bset, args.format)
+    sample = (f"every step = one serialize + deserialize pass of the oracle over the first {n_t} of {bset.n_tensors} tensors "
+              f"({b1} blocks, {sbytes / 1e6:.0f} MB stream = {100 * sbytes / full_total:.1f} % of the workload's {full_total / 1e9:.3f} GB)")
     line = {"impl": "reference", "metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms, 3), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
-            "config": workload_config(args.workload, bset, None, args.format),
-            "cpu_baseline": {"value": round(value, 3), "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "config": workload_config(args.workload, bset, full_total, args.format),
+            "cpu_baseline": {"value": round(value, 3), "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                             "sample_stream_bytes": int(sbytes), "host_cores": os.cpu_count()},
             "e2e": {"value": round(value, 3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def full_stream_bytes(bset, fmt="v1"):
+    """Stream size of the whole workload from the oracle's size prediction (host only)."""
+    import workloads as W
+    if fmt == "v2":
+        from oracle import v2
+        lv = W.layered_view(bset)
+        return int(v2.serialized_size(lv["structs"], lv["layers"], lv["dim"])[1])
+    import oracle
+    return int(oracle.serialized_size(bset.n_tensors, bset.dim)[1])
 
 
 def workload_config(name, bset, total, fmt="v1"):
@@ -346,24 +404,32 @@ def run_mine(args):
     des_ms = [e[2 * k + 1].elapsed_time(e[2 * k + 2]) for k in range(args.steps)]
     clocks = sampler.window(w0, w1)
 
-    # ---- roofline leg: the dominant kernel (pack) alone, same launch configuration, CUDA events on its stream ----
-    n_pack = max(args.steps, 5)
-    ser()
-    torch.cuda.synchronize()
-    a, b = ev(), ev()
-    a.record()
-    for _ in range(n_pack):
-        f_range(dset.desc, stream.data_ptr(), 0, total, False, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
-    b.record()
-    torch.cuda.synchronize()
-    pack_ms = a.elapsed_time(b) / n_pack
-    a.record()
-    for _ in range(n_pack):
-        f_size(dset.desc, ws.ptr, ws.nbytes, cs)
-    b.record()
-    torch.cuda.synchronize()
-    scan_ms = a.elapsed_time(b) / n_pack
+    # ---- roofline leg: the dominant kernel (pack) alone, then its mirror image (unpack), same launch configuration,
+    # CUDA events on their stream.  The size / offset pass has run (ser / deser above leave the tables in the workspace). ----
     peaks, peak_kind = measured_peaks()
+    n_k = max(args.steps, 5)
+
+    def timed(fn, n=n_k):
+        torch.cuda.synchronize()
+        a, b = ev(), ev()
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    ser()
+    pack_ms = timed(lambda: f_range(dset.desc, stream.data_ptr(), 0, total, False, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs))
+    scan_ms = timed(lambda: f_size(dset.desc, ws.ptr, ws.nbytes, cs))
+    ser()
+    deser()                          # leaves the parsed tables in the workspace: the unpack kernel alone re-scatters from them
+    if v2:                           # (no range form for layered sets: whole call minus the plan pass of the same set)
+        unpack_ms = max(timed(deser) - scan_ms, 1e-6)
+    else:
+        unpack_ms = timed(lambda: bs.deserialize_range(stream.data_ptr(), 0, total, stream.data_ptr(), out.desc, bs.LAYOUT_POOL,
+                                                       ws.ptr, ws.nbytes, opts, cs))
+    check_ok("roofline leg")
     # algorithmic bytes per pack launch: 2 B per stream byte + per block 24 (labels) + 12 (dims)
     # + 16 (offset table entry) read for its header record  [SURVEY §8(d): "2 B per stream byte ... ~130 B per block"
     # counts the scan pass too; the pack launch alone reads 52 B per block on top of the stream bytes]
@@ -371,24 +437,39 @@ def run_mine(args):
     algo_bytes = 2 * total + (16 * bset.n_blocks if v2 else 52 * bset.n_blocks)
     achieved = algo_bytes / (pack_ms * 1e-3) / 1e9
     kname = "bs::move_kernel<pack>" if args.variant == 1 else "bs::move_tma_kernel<pack>"
+    med_ser, med_des = float(np.median(ser_ms)), float(np.median(des_ms))
     roofline = {"bound": "hbm", "kernel": kname + " (S3 header write + S5 pack)", "achieved": round(achieved, 1),
                 "peak": peaks["hbm_gbs"], "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
                 "unit": "GB/s", "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": None,
                 "algorithmic_bytes_per_launch": int(algo_bytes), "kernel_ms": round(pack_ms, 4),
                 "frac_of_nominal_8TBs": round(achieved / 8000.0, 4)}
-    roofline["traffic"] = committed_traffic(f"pack:{args.workload}:v{args.variant or 2}" + (":fmt2" if v2 else ""))
+    vname = "ldg" if args.variant == 1 else "tma"
+    roofline["traffic"] = committed_traffic(f"pack:{args.workload}:{vname}:fmt{2 if v2 else 1}")
+    # the mirror image: the unpack kernel alone (bs_deserialize_range over the whole stream, descriptor rebuild included)
+    unpack_algo = 2 * total + (16 * bset.n_blocks if v2 else 64 * bset.n_blocks)   # 48 B record read + 16 B table entry per block
+    roofline.update({
+        "unpack_kernel_ms": round(unpack_ms, 4), "unpack_achieved": round(unpack_algo / (unpack_ms * 1e-3) / 1e9, 1),
+        "unpack_frac": round(unpack_algo / (unpack_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], 4),
+        "unpack_kernel": ("bs::move_kernel<unpack>" if args.variant == 1 else "bs::move_tma_kernel<unpack>") + " (S7 rebuild + unpack)",
+        "serialize_ms": round(med_ser, 4), "deserialize_ms": round(med_des, 4),
+        "serialize_hbm_GBs": round(2 * total / med_ser / 1e6, 1), "deserialize_hbm_GBs": round(2 * total / med_des / 1e6, 1),
+        "serialize_frac_of_8TBs": round(2 * total / med_ser / 1e6 / 8000, 4),
+        "deserialize_frac_of_8TBs": round(2 * total / med_des / 1e6 / 8000, 4),
+        "serialize_frac_of_measured_copy": round(2 * total / med_ser / 1e6 / peaks["hbm_gbs"], 4),
+        "deserialize_frac_of_measured_copy": round(2 * total / med_des / 1e6 / peaks["hbm_gbs"], 4)})
+    # in-run ceiling: the same mover on ONE contiguous block (a pure cp.async.bulk copy, no scatter, no header to speak of)
+    if not v2 and args.elem == "f64" and not args.no_ceiling:
+        try:
+            roofline.update(bulk_copy_ceiling(bs, torch, pool, stream, dev, opts, cs, n_k))
+            roofline["frac_of_bulk_copy"] = round(achieved / roofline["bulk_copy_GBs"], 4)
+            roofline["unpack_frac_of_bulk_copy"] = round(roofline["unpack_achieved"] / roofline["bulk_copy_GBs"], 4)
+        except Exception as ex:   # the headline numbers stand on their own
+            roofline["bulk_copy_error"] = repr(ex)
 
     # ---- e2e leg: host (pinned) buffers through the engine, copies inside the timed region ----
-    detail = {"serialize_ms": round(float(np.median(ser_ms)), 4), "deserialize_ms": round(float(np.median(des_ms)), 4),
-              "serialize_stream_GBs": round(total / np.median(ser_ms) / 1e6, 1),
-              "deserialize_stream_GBs": round(total / np.median(des_ms) / 1e6, 1),
-              "serialize_hbm_GBs": round(2 * total / np.median(ser_ms) / 1e6, 1),
-              "deserialize_hbm_GBs": round(2 * total / np.median(des_ms) / 1e6, 1),
-              "serialize_frac_of_measured_copy": round(2 * total / np.median(ser_ms) / 1e6 / peaks["hbm_gbs"], 4),
-              "deserialize_frac_of_measured_copy": round(2 * total / np.median(des_ms) / 1e6 / peaks["hbm_gbs"], 4),
-              "serialize_frac_of_8TBs": round(2 * total / np.median(ser_ms) / 1e6 / 8000, 4),
-              "deserialize_frac_of_8TBs": round(2 * total / np.median(des_ms) / 1e6 / 8000, 4),
-              "scan_kernel_ms_incl_sync": round(scan_ms, 4)}
+    detail = {"serialize_stream_GBs": round(total / med_ser / 1e6, 1), "deserialize_stream_GBs": round(total / med_des / 1e6, 1),
+              "size_pass_ms_incl_sync": round(scan_ms, 4)}
+    a, b = ev(), ev()
     e2e = None
     if not args.no_e2e:
         host = torch.empty(total, dtype=torch.uint8, pin_memory=True)
@@ -431,11 +512,15 @@ def run_mine(args):
         e2e = {"value": round(units_g / (e2e_ms_g * 1e-3) / 1e9, 3), "unit": UNIT, "h2d_bytes_per_step": int(total),
                "d2h_bytes_per_step": int(total), "ms_per_step": round(e2e_ms_g, 3),
                "what": "bs_offload_async -> pinned host -> bs_prefetch_async, one after the other, 256 MiB double-buffered chunks"}
-        detail.update({"offload_pcie_GBs": round(off_gbs, 2), "prefetch_pcie_GBs": round(pre_gbs, 2),
-                       "pinned_d2h_GBs": round(bw["d2h"], 2), "pinned_h2d_GBs": round(bw["h2d"], 2),
-                       "offload_frac_of_pinned_d2h": round(off_gbs / bw["d2h"], 4),
-                       "prefetch_frac_of_pinned_h2d": round(pre_gbs / bw["h2d"], 4),
-                       "offload_total_ms": round(float(np.median([s[0]["total_ms"] for s in stats])), 3),
+        # the north_star's offload bar (>= 80 % of the measured pinned PCIe bandwidth), both directions, same run
+        pcie = {"offload_pcie_GBs": round(off_gbs, 2), "prefetch_pcie_GBs": round(pre_gbs, 2),
+                "pinned_d2h_GBs": round(bw["d2h"], 2), "pinned_h2d_GBs": round(bw["h2d"], 2),
+                "offload_frac_of_pinned_d2h": round(off_gbs / bw["d2h"], 4),
+                "prefetch_frac_of_pinned_h2d": round(pre_gbs / bw["h2d"], 4),
+                "pcie_how": "stream bytes / (first DMA start -> last DMA end) of bs_offload_async / bs_prefetch_async, device-timed, "
+                            "median over the steps; denominators: pinned cudaMemcpyAsync of 1 GiB, best of 5, same run"}
+        e2e.update(pcie)
+        detail.update({"offload_total_ms": round(float(np.median([s[0]["total_ms"] for s in stats])), 3),
                        "prefetch_total_ms": round(float(np.median([s[1]["total_ms"] for s in stats])), 3)})
         eng.destroy()
         if not v2 and not args.no_queue:
@@ -488,10 +573,12 @@ def run_mine(args):
                    "ms_per_step": round(q_ms_g, 3),
                    "what": "bs_queue: every step bs_queue_save of the set (device -> pinned host) overlapped with bs_queue_load "
                            "of the stream the step before saved (pinned host -> device); 256 MiB double-buffered chunks per lane"}
-            detail["queue"] = {"aggregate_pcie_GBs": round(2 * total / q_ms / 1e6, 2),
-                               "pinned_bidirectional_memcpy_GBs": round(bw["bidir"], 2),
-                               "frac_of_bidirectional_memcpy": round(2 * total / q_ms / 1e6 / bw["bidir"], 4),
-                               "device_bytes_held": q.stats()["device_bytes"], "host_bytes_live": q.stats()["host_bytes_live"]}
+            e2e.update(pcie)
+            e2e.update({"one_after_the_other_GBs": detail["e2e_one_after_the_other"]["value"],
+                        "duplex_pcie_GBs": round(2 * total / q_ms / 1e6, 2),
+                        "pinned_bidirectional_memcpy_GBs": round(bw["bidir"], 2),
+                        "duplex_frac_of_bidirectional_memcpy": round(2 * total / q_ms / 1e6 / bw["bidir"], 4)})
+            detail["queue"] = {"device_bytes_held": q.stats()["device_bytes"], "host_bytes_live": q.stats()["host_bytes_live"]}
             q.destroy()
             del host2, hosts
         del host
@@ -604,7 +691,18 @@ def run_mine(args):
     # ---- config 5: exposed IO of an offload overlapped with a stand-in contraction (rank 0 only) ----
     if rank == 0 and not args.no_config5 and not v2:
         try:
-            detail["config5"] = config5(args, dev, opts)
+            c5 = config5(args, dev, opts)
+            detail["config5"] = c5
+            if e2e is not None:   # the north_star's third bar: exposed (non-hidden) IO time < 10 % (config 5 = config 3 through the engine)
+                hs, hl = c5["headline"], c5["prefetch"]["headline"]
+                e2e.update({"exposed_io_frac_save": hs["exposed_io_frac"], "exposed_io_frac_load": hl["exposed_io_frac"],
+                            "exposed_io_r": hs["r_target"], "exposed_io_r_actual": [hs["r_actual"], hl["r_actual"]],
+                            "sustained_pcie_GBs_save": hs["sustained_pcie_GBs"], "sustained_pcie_GBs_load": hl["sustained_pcie_GBs"],
+                            "exposed_io_workload": f"config 5: config 3 ({c5['stream_bytes'] / 1e9:.2f} GB stream) through bs_offload_async / "
+                                                   "bs_prefetch_async behind a stand-in contraction (batched fp64 block GEMMs) on the compute "
+                                                   "stream; exposed = (T_both - T_c) / T_both at r = T_c / T_io"})
+                if "sweep_fig3" in c5 and "error" not in c5["sweep_fig3"]:
+                    e2e["sweep_speedup_queue_over_sync_io"] = c5["sweep_fig3"]["speedup_queue_over_sync"]
         except Exception as ex:  # the headline numbers stand on their own
             detail["config5"] = {"error": repr(ex)}
 
@@ -612,24 +710,151 @@ def run_mine(args):
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         _, sub, n_t, b1 = oracle_sample(args.workload, args.sample_mb, args.format)
-        time_oracle(sub, 0.0, max_passes=1)
-        sec, passes, sbytes = time_oracle(sub, args.cpu_seconds)
+        runner = OracleRunner(sub)
+        sec, passes = runner.run_for(args.cpu_seconds)
+        sbytes = runner.total
         cpu = {"value": round(2 * sbytes * passes / sec / 1e9, 3), "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"{passes} serialize+deserialize passes over the first {n_t} of {bset.n_tensors} tensors "
                          f"({b1} blocks, {sbytes / 1e6:.0f} MB stream) of workload {args.workload}; {sec:.1f} s of CPU work",
-               "host_cores": os.cpu_count()}
+               "sample_stream_bytes": int(sbytes), "host_cores": os.cpu_count()}
+        if not v2 and not args.no_threads_sweep:
+            try:
+                cpu["threads_sweep"] = oracle_threads_sweep(sub)
+                cpu["threads_sweep_what"] = ("context only: the paper's own design (L106-108: the main thread maps one buffer from the "
+                                             "predicted sizes, threads fill disjoint intervals; saturation at 32 threads, L158) with "
+                                             "the unchanged oracle's slice-wise emit per thread; serialize only")
+            except Exception as ex:
+                cpu["threads_sweep"] = {"error": repr(ex)}
+
+    # ---- at scale: workload 4L (the operator count scaled to the 40-60 GB BASELINE.json states), kernels
+    # and whole calls only.  Runs last, after this workload's buffers are released; skipped if HBM cannot hold it. ----
+    if rank == 0 and not v2 and args.elem == "f64" and not args.no_at_scale and args.workload != "4L":
+        del stream, opool, pool, out, dset, ws
+        torch.cuda.empty_cache()
+        try:
+            roofline["at_scale"] = at_scale(bs, torch, W, fill_pool_device, dev, opts, peaks)
+        except Exception as ex:
+            roofline["at_scale"] = {"error": repr(ex)}
 
     ms_g, units_g = aggregate(step_ms, 2 * total, world, dev, ready)
     sampler.stop()
     if rank == 0:
+        fused = (not v2) and args.variant != 1 and max(-(-bset.n_blocks // 1024), -(-bset.n_tensors // 1024)) <= sm_count(torch, dev)
         line = {"metric": METRIC, "value": round(units_g / (ms_g * 1e-3) / 1e9, 3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_g, 4), "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
-                "config": with_elem(workload_config(args.workload, bset, total, args.format), args.elem), "clocks": clocks, "e2e": e2e,
-                "gpu_launches": (8 if v2 else 4) * args.steps, "roofline": roofline, "cpu_baseline": cpu, "detail": detail}
+                "config": with_elem(workload_config(args.workload, bset, total, args.format), args.elem), "clocks": clocks,
+                "gpu_launches": (2 if fused else (8 if v2 else 4)) * args.steps, "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
+                "detail": detail}
         print(json.dumps(line), flush=True)
     if ready:
         dist.destroy_process_group()
+
+
+def sm_count(torch, dev):
+    return torch.cuda.get_device_properties(dev).multi_processor_count
+
+
+def bulk_copy_ceiling(bs, torch, pool, stream, dev, opts, cs, n):
+    """In-run ceiling of the mover: the pack kernel on ONE contiguous fp64 block as large as the workload's stream — every
+    tile is one cp.async.bulk load and one cp.async.bulk store, no scatter.  Reuses the workload's pool as the block and its
+    stream buffer as the destination (both are re-created by the next serialize)."""
+    import workloads as W
+    nbytes = min(pool.numel(), stream.numel() - 4096) // (1 << 20) * (1 << 20)
+    rows = nbytes // 8 // 32768
+    tensors = np.zeros(1, W.TENSOR_REC_DTYPE)
+    tensors["rank"], tensors["n_blocks"], tensors["sign"] = 2, 1, (-1, 1, 0, 0)
+    one = bs.DeviceSet.from_host(tensors, np.zeros((1, 3, 2), np.int32), np.array([[rows, 32768, 1]], np.uint32),
+                                 np.array([pool.data_ptr()], np.uint64), dev)
+    w1 = bs.Workspace(1, 1, stream.numel(), dev)
+    hb1, tot1 = bs.serialized_size(one.desc, w1.ptr, w1.nbytes, cs)
+    assert tot1 <= stream.numel()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(2):
+        bs.serialize_range(one.desc, stream.data_ptr(), 0, tot1, False, w1.ptr, w1.nbytes, w1.result_ptr, opts, cs)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(n):
+        bs.serialize_range(one.desc, stream.data_ptr(), 0, tot1, False, w1.ptr, w1.nbytes, w1.result_ptr, opts, cs)
+    b.record()
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / n
+    # and the runtime's own device-to-device copy of the same bytes (what MEASURED_PEAKS.json's figure is, on this box, now)
+    dst = stream[:tot1 - hb1]
+    src = pool[:tot1 - hb1]
+    for _ in range(2):
+        dst.copy_(src)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(n):
+        dst.copy_(src)
+    b.record()
+    torch.cuda.synchronize()
+    ms_rt = a.elapsed_time(b) / n
+    return {"bulk_copy_GBs": round(2 * tot1 / ms / 1e6, 1), "bulk_copy_bytes": int(tot1),
+            "bulk_copy_what": "this run: bs::move_tma_kernel<pack> on ONE contiguous block of that many bytes (pure cp.async.bulk copy)",
+            "runtime_d2d_copy_GBs": round(2 * (tot1 - hb1) / ms_rt / 1e6, 1)}
+
+
+def at_scale(bs, torch, W, fill_pool_device, dev, opts, peaks, name="4L", steps=5):
+    """Pack / unpack kernels and whole calls on workload 4L (42.5 GB stream, 3.3 M blocks: BASELINE.json configs[3]'s stated total)."""
+    bset = W.make_config(name)
+    need_dev = int(bset.pool_bytes) + 2 * (bset.data_bytes + 64 * bset.n_blocks + (64 << 20)) + (1 << 30)
+    free_dev, _ = torch.cuda.mem_get_info()
+    if need_dev > free_dev:
+        return {"skipped": f"workload {name} needs {need_dev / 1e9:.0f} GB of HBM, {free_dev / 1e9:.0f} GB are free"}
+    cs = bs.current_stream()
+    pool, addr = fill_pool_device(bset, dev)
+    dset = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, addr, dev)
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, bset.data_bytes + 16 * bset.n_blocks + bs.header_bytes(bset.n_tensors, bset.n_blocks), dev)
+    hb, total = bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs)
+    stream = torch.empty(total, dtype=torch.uint8, device=dev)
+    need = int(((bset.nelems * 8 + 255) // 256 * 256).sum())
+    opool = torch.empty(need, dtype=torch.uint8, device=dev)
+    out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, dev)
+
+    def ser():
+        bs.serialize(dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
+
+    def deser():
+        bs.deserialize(stream.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
+
+    def timed(fn, n=steps):
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    for _ in range(3):
+        ser()
+        deser()
+    if ws.read_result()["status"] != bs.OK:
+        raise RuntimeError(f"at_scale warm-up: {ws.read_result()}")
+    ser_ms, des_ms = timed(ser), timed(deser)
+    ser()
+    pack_ms = timed(lambda: bs.serialize_range(dset.desc, stream.data_ptr(), 0, total, False, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs))
+    deser()
+    unpack_ms = timed(lambda: bs.deserialize_range(stream.data_ptr(), 0, total, stream.data_ptr(), out.desc, bs.LAYOUT_POOL, ws.ptr,
+                                                   ws.nbytes, opts, cs))
+    if ws.read_result()["status"] != bs.OK:
+        raise RuntimeError(f"at_scale: {ws.read_result()}")
+    algo_p, algo_u = 2 * total + 52 * bset.n_blocks, 2 * total + 64 * bset.n_blocks
+    pk, hbm = peaks["hbm_gbs"], lambda ms: 2 * total / ms / 1e6
+    return {"workload": f"config 4L: D={bset.meta['D']}, {bset.meta['S']} sectors, {bset.meta['n_ops']} operators + {bset.meta['n_site']} "
+                        "site tensors (configs[3] with the operator count scaled to the 40-60 GB it states, SURVEY §8(d) R1)",
+            "stream_bytes": int(total), "n_tensors": bset.n_tensors, "n_blocks": bset.n_blocks, "steps": steps,
+            "pack_kernel_ms": round(pack_ms, 3), "achieved": round(algo_p / pack_ms / 1e6, 1), "frac": round(algo_p / pack_ms / 1e6 / pk, 4),
+            "frac_of_nominal_8TBs": round(algo_p / pack_ms / 1e6 / 8000, 4),
+            "unpack_kernel_ms": round(unpack_ms, 3), "unpack_achieved": round(algo_u / unpack_ms / 1e6, 1),
+            "unpack_frac": round(algo_u / unpack_ms / 1e6 / pk, 4),
+            "serialize_ms": round(ser_ms, 3), "deserialize_ms": round(des_ms, 3),
+            "serialize_hbm_GBs": round(hbm(ser_ms), 1), "deserialize_hbm_GBs": round(hbm(des_ms), 1),
+            "serialize_frac_of_8TBs": round(hbm(ser_ms) / 8000, 4), "deserialize_frac_of_8TBs": round(hbm(des_ms) / 8000, 4),
+            "value_GBs": round(2 * total / (ser_ms + des_ms) / 1e6, 1)}
 
 
 def config5(args, dev, opts):
@@ -866,6 +1091,9 @@ def main():
     ap.add_argument("--no-queue", action="store_true", help="e2e: offload then prefetch only, no duplex queue leg")
     ap.add_argument("--no-config5", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-ceiling", action="store_true", help="skip the in-run bulk-copy ceiling of the roofline leg")
+    ap.add_argument("--no-at-scale", action="store_true", help="skip roofline.at_scale (workload 4L, 42.5 GB)")
+    ap.add_argument("--no-threads-sweep", action="store_true", help="skip cpu_baseline.threads_sweep")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "mine" else args.warmup
     if args.elem != "f64":   # the e2e / config-5 / cpu legs and wire format v2 are fp64; other element types time the kernels

@@ -131,7 +131,9 @@ typedef struct bs_opts {
     uint32_t ctas_per_sm; /* LDG: persistent CTAs per SM; 0 = default (occupancy limit) */
     uint32_t stages;      /* TMA: ring depth (tiles) per warp, 3..8; 0 = default */
     uint32_t warps;       /* TMA: warps (rings) per CTA, 1..16; warps*stages*tile_bytes <= 225 KiB; 0 = default */
-    uint32_t reserved[3]; /* 0 */
+    uint32_t reserved[3]; /* 0.  [0]: experiment switches of the TMA variant (bits; see bs_move_tma.cu); [1]: bs_serialize /
+                             bs_deserialize as one fused launch (size / offset pass + movement in one kernel): 0 = by size
+                             (sets of up to ~150 k blocks), 1 = never, 2 = always */
 } bs_opts;
 enum { BS_VARIANT_DEFAULT = 0, BS_VARIANT_LDG = 1, BS_VARIANT_TMA = 2 };
 
@@ -183,6 +185,15 @@ int bs_serialize_range(const bs_set_desc *set, void *d_dst, uint64_t lo, uint64_
 int bs_deserialize(const void *d_stream, uint64_t nbytes, bs_set_desc *out, void *d_pool,
                    uint64_t pool_bytes, uint32_t flags, void *d_workspace, uint64_t workspace_bytes,
                    bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
+
+/* Segment form (Fig 4(b); the mirror image of bs_serialize_range): scatter the payload bytes of stream range
+ * [lo, hi), found at d_src[0 .. hi-lo), to their blocks.  lo, hi multiples of 16 (hi is clipped to the total).  The
+ * parse / validate pass must have run on the same workspace with the same `out` and destination (a bs_deserialize call;
+ * the tables it leaves are what this call uses) and its status is honoured: nothing is written unless it was BS_OK.
+ * d_header: stream byte 0 .. header_bytes to rebuild the descriptor arrays from as well, or NULL (payload only).
+ * The union over a partition of [header_bytes, total) rebuilds every block. */
+int bs_deserialize_range(const void *d_src, uint64_t lo, uint64_t hi, const void *d_header, bs_set_desc *out, uint32_t flags,
+                         void *d_workspace, uint64_t workspace_bytes, const bs_opts *opts, cudaStream_t stream);
 
 
 /* ==== wire format v2: structure-shared layers (PAPER Fig 4(a), L75) =============================

@@ -124,11 +124,14 @@ def emit_header(tensors, qn, dim) -> np.ndarray:
     return out
 
 
-def emit_payload_range(tensors, dim, addr, t0: int, t1: int, capacity: int):
-    """Payload bytes of tensors [t0, t1).  Returns (first_offset, bytes ndarray)."""
+def emit_payload_range(tensors, dim, addr, t0: int, t1: int, capacity: int, out: np.ndarray | None = None):
+    """Payload bytes of tensors [t0, t1).  Returns (first_offset, bytes ndarray).  ``out``: a caller buffer of at least
+    ``capacity`` bytes to write into (e.g. a slice of one large stream buffer) instead of a fresh poisoned one."""
     tensors, dim = _tensors(tensors), _c(dim, np.uint32, (3,))
     addr = _c(addr, np.uint64)
-    out = np.full(max(capacity, 1), 0xCD, dtype=np.uint8)
+    if out is None:
+        out = np.full(max(capacity, 1), 0xCD, dtype=np.uint8)
+    assert out.dtype == np.uint8 and out.flags["C_CONTIGUOUS"] and out.size >= capacity
     first, nb = C.c_uint64(0), C.c_uint64(0)
     rc = _L().orc_emit_payload_range(len(tensors), dim.shape[0], _p(tensors), _p(dim), _p(addr), t0, t1,
                                      _p(out), capacity, C.byref(first), C.byref(nb))

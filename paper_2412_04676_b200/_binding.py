@@ -75,6 +75,7 @@ def make_opts(opts) -> "Opts":
     for k in ("variant", "tile_bytes", "ctas_per_sm", "stages", "warps"):
         setattr(o, k, int((opts or {}).get(k, 0) or 0))
     o.reserved[0] = int((opts or {}).get("tune", 0) or 0)
+    o.reserved[1] = int((opts or {}).get("fuse", 0) or 0)
     return o
 
 
@@ -128,6 +129,7 @@ def lib():
     L.bs_serialize.argtypes = [C.POINTER(SetDesc), vp, u64, vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_serialize_range.argtypes = [C.POINTER(SetDesc), vp, u64, u64, i32, vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_deserialize.argtypes = [vp, u64, C.POINTER(SetDesc), vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_deserialize_range.argtypes = [vp, u64, u64, vp, C.POINTER(SetDesc), u32, vp, u64, C.POINTER(Opts), vp]
     L.bs_engine_create.argtypes = [C.POINTER(vp), C.POINTER(EngineCfg)]
     L.bs_engine_destroy.argtypes = [vp]
     L.bs_offload_async.argtypes = [vp, C.POINTER(SetDesc), u64, vp, u64, vp, C.POINTER(vp)]
@@ -251,6 +253,12 @@ def deserialize(stream_ptr: int, nbytes: int, out: SetDesc, pool_ptr: int, pool_
                 ws_bytes: int, result_ptr: int, opts=None, stream: int = 0) -> int:
     return _check(lib().bs_deserialize(stream_ptr, nbytes, C.byref(out), pool_ptr, pool_bytes, flags, ws_ptr, ws_bytes,
                                        result_ptr, _opts(opts), stream), "bs_deserialize")
+
+
+def deserialize_range(src_ptr: int, lo: int, hi: int, header_ptr: int, out: SetDesc, flags: int, ws_ptr: int, ws_bytes: int,
+                      opts=None, stream: int = 0) -> int:
+    return _check(lib().bs_deserialize_range(src_ptr, lo, hi, header_ptr, C.byref(out), flags, ws_ptr, ws_bytes, _opts(opts),
+                                             stream), "bs_deserialize_range")
 
 
 # ---- wire format v2: structure-shared layers ----------------------------------------------------------------------

@@ -33,7 +33,7 @@ int device_sm_count(int* out)
 
 static bool aligned(const void* p, uintptr_t a) { return ((uintptr_t)p & (a - 1)) == 0; }
 
-static int check_set(const bs_set_desc* s)
+int check_set(const bs_set_desc* s)
 {
     if (s == nullptr) return BS_ERR_ARG;
     if (s->n_qn != 2 || s->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
@@ -57,12 +57,9 @@ int check_opts(const bs_opts& o)
     return BS_OK;
 }
 
-// S1/S2/S4: clear the scan state, run the size / offset pass for `set`
-int run_serialize_scan(const bs_set_desc* set, const WsLayout& L, uint64_t capacity, uint64_t expect_total,
-                       bs_result* d_result, int sms, cudaStream_t stream)
+static ScanParams serialize_scan_params(const bs_set_desc* set, const WsLayout& L, uint64_t capacity, uint64_t expect_total,
+                                        bs_result* d_result)
 {
-    cudaError_t e = cudaMemsetAsync(L.head, 0, L.zero_bytes, stream);
-    if (e != cudaSuccess) return cuda_fail(e);
     ScanParams sp;
     memset(&sp, 0, sizeof(sp));
     sp.ws = L;
@@ -75,13 +72,20 @@ int run_serialize_scan(const bs_set_desc* set, const WsLayout& L, uint64_t capac
     sp.T = set->n_tensors;
     sp.B = set->n_blocks;
     sp.dtype = set->dtype;
-    e = launch_scan(false, sp, sms, stream);
+    return sp;
+}
+
+// S1/S2/S4: run the size / offset pass for `set`
+int run_serialize_scan(const bs_set_desc* set, const WsLayout& L, uint64_t capacity, uint64_t expect_total,
+                       bs_result* d_result, int sms, cudaStream_t stream)
+{
+    const cudaError_t e = launch_scan(false, serialize_scan_params(set, L, capacity, expect_total, d_result), sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
 }
 
-int run_pack_range(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint64_t lo, uint64_t hi,
-                   const bs_opts& o, int sms, cudaStream_t stream)
+static MoveParams pack_params(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint64_t lo, uint64_t hi, const bs_opts& o,
+                              uint32_t flags = 0)
 {
     MoveParams mp;
     memset(&mp, 0, sizeof(mp));
@@ -95,17 +99,32 @@ int run_pack_range(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint6
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
-    cudaError_t e = launch_move(false, mp, o, sms, stream);
+    mp.flags = flags;
+    return mp;
+}
+
+int run_pack_range(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint64_t lo, uint64_t hi,
+                   const bs_opts& o, int sms, cudaStream_t stream, uint32_t flags)
+{
+    const cudaError_t e = launch_move(false, pack_params(set, L, d_dst, lo, hi, o, flags), o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
 }
 
-int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_set_desc* out,
-                         void* d_pool, uint64_t pool_bytes, uint32_t flags, const WsLayout& L, bs_result* d_result,
-                         int sms, cudaStream_t stream)
+// One launch or two?  bs_opts.reserved[1]: 0 = by size, 1 = always separate launches, 2 = always one fused launch.  By size:
+// the fused kernel runs the pass on one CTA per SM, so sets of more work items than that leave the pass to its own,
+// wider launch (whose ~5 us are then < 1 % of the call).
+static bool use_fused(const bs_opts& o, uint64_t T, uint64_t B, int sms)
 {
-    cudaError_t e = cudaMemsetAsync(L.head, 0, L.zero_bytes, stream);
-    if (e != cudaSuccess) return cuda_fail(e);
+    if (o.variant != BS_VARIANT_TMA || o.reserved[1] == 1u) return false;
+    if (o.reserved[1] == 2u) return true;
+    const uint64_t nt = (B + kScanTile - 1) / kScanTile, ntt = (T + kScanTile - 1) / kScanTile;
+    return (nt > ntt ? nt : ntt) <= (uint64_t)sms;
+}
+
+static ScanParams deserialize_scan_params(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_set_desc* out,
+                                          void* d_pool, uint64_t pool_bytes, uint32_t flags, const WsLayout& L, bs_result* d_result)
+{
     ScanParams sp;
     memset(&sp, 0, sizeof(sp));
     sp.ws = L;
@@ -120,13 +139,21 @@ int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t n
     sp.out_dim = out->dim;
     sp.out_addr = out->addr;
     sp.flags = flags;
-    e = launch_scan(true, sp, sms, stream);
+    return sp;
+}
+
+int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_set_desc* out,
+                         void* d_pool, uint64_t pool_bytes, uint32_t flags, const WsLayout& L, bs_result* d_result,
+                         int sms, cudaStream_t stream)
+{
+    const cudaError_t e = launch_scan(true, deserialize_scan_params(d_header, d_payload, nbytes, out, d_pool, pool_bytes, flags, L, d_result),
+                                      sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
 }
 
-int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header,
-                     uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream)
+static MoveParams unpack_params(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header, uint64_t lo,
+                                uint64_t hi, uint32_t flags, const bs_opts& o)
 {
     MoveParams mp;
     memset(&mp, 0, sizeof(mp));
@@ -142,15 +169,18 @@ int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_sr
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
     mp.flags = flags;
-    cudaError_t e = launch_move(true, mp, o, sms, stream);
+    return mp;
+}
+
+int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header,
+                     uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream)
+{
+    const cudaError_t e = launch_move(true, unpack_params(out, L, d_src, d_header, lo, hi, flags, o), o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
 }
 
 // the whole stream <-> package slots in one launch each (bs.h "packages"; PkgMap in bs_internal.cuh)
-int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, const bs_opts& o,
-                            int sms, cudaStream_t stream);
-
 int run_pack_packages(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, const bs_opts& o, int sms, cudaStream_t stream)
 {
     return run_pack_packages_range(set, L, pm, 0, UINT64_MAX, o, sms, stream);
@@ -178,9 +208,6 @@ int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const Pkg
 }
 
 // payload only: the header region was gathered and parsed before (header = nullptr: no descriptor rebuild here)
-int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, uint32_t flags,
-                              const bs_opts& o, int sms, cudaStream_t stream);
-
 int run_unpack_packages(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t header_bytes, uint32_t flags,
                         const bs_opts& o, int sms, cudaStream_t stream)
 {
@@ -320,6 +347,11 @@ int bs_serialize(const bs_set_desc* set, void* d_stream, uint64_t capacity, void
     if (!ws_layout(d_ws, ws_bytes, set->n_blocks, &L)) return d_ws && aligned(d_ws, 256) ? BS_ERR_CAPACITY : BS_ERR_ARG;
     int sms;
     if ((rc = device_sm_count(&sms))) return rc;
+    if (use_fused(o, set->n_tensors, set->n_blocks, sms)) {  // the pass and the pack in ONE launch
+        const cudaError_t e = launch_fused_tma(false, serialize_scan_params(set, L, capacity, 0, d_result),
+                                               pack_params(set, L, d_stream, 0, capacity & ~15ull, o), o, capacity, sms, stream);
+        return e == cudaSuccess ? BS_OK : cuda_fail(e);
+    }
     if ((rc = run_serialize_scan(set, L, capacity, 0, d_result, sms, stream))) return rc;
     return run_pack_range(set, L, d_stream, 0, capacity & ~15ull, o, sms, stream);
 }
@@ -342,8 +374,31 @@ int bs_deserialize(const void* d_stream, uint64_t nbytes, bs_set_desc* out, void
     if ((rc = device_sm_count(&sms))) return rc;
     const unsigned char* s = (const unsigned char*)d_stream;
     // the payload is only dereferenced (pad-zero check) after the fixed header proved header_bytes + P == nbytes
+    if (use_fused(o, out->n_tensors, out->n_blocks, sms)) {  // parse / validate and unpack in ONE launch
+        const cudaError_t e = launch_fused_tma(true, deserialize_scan_params(s, s, nbytes, out, d_pool, pool_bytes, flags, L, d_result),
+                                               unpack_params(out, L, s, s, 0, nbytes & ~15ull, flags, o), o, nbytes, sms, stream);
+        return e == cudaSuccess ? BS_OK : cuda_fail(e);
+    }
     if ((rc = run_deserialize_scan(s, s, nbytes, out, d_pool, pool_bytes, flags, L, d_result, sms, stream))) return rc;
     return run_unpack_range(out, L, s, s, 0, nbytes & ~15ull, flags, o, sms, stream);
+}
+
+int bs_deserialize_range(const void* d_src, uint64_t lo, uint64_t hi, const void* d_header, bs_set_desc* out, uint32_t flags,
+                         void* d_ws, uint64_t ws_bytes, const bs_opts* opts, cudaStream_t stream)
+{
+    int rc = check_set(out);
+    if (rc) return rc;
+    if (d_src == nullptr || !aligned(d_src, 16) || (lo & 15) || (hi & 15) || lo > hi) return BS_ERR_ARG;
+    if (d_header != nullptr && !aligned(d_header, 16)) return BS_ERR_ARG;
+    if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
+    bs_opts o;
+    resolve_opts(opts, &o);
+    if ((rc = check_opts(o))) return rc;
+    WsLayout L;
+    if (!ws_layout(d_ws, ws_bytes, out->n_blocks, &L)) return d_ws && aligned(d_ws, 256) ? BS_ERR_CAPACITY : BS_ERR_ARG;
+    int sms;
+    if ((rc = device_sm_count(&sms))) return rc;
+    return run_unpack_range(out, L, d_src, d_header, lo, hi, flags, o, sms, stream);
 }
 
 }  // extern "C"

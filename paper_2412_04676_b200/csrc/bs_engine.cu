@@ -21,41 +21,7 @@
 
 #include "bs_engine.cuh"
 
-namespace bs {
-int cuda_fail(cudaError_t e);
-int device_sm_count(int* out);
-int run_serialize_scan(const bs_set_desc* set, const WsLayout& L, uint64_t capacity, uint64_t expect_total,
-                       bs_result* d_result, int sms, cudaStream_t stream);
-int run_pack_range(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint64_t lo, uint64_t hi,
-                   const bs_opts& o, int sms, cudaStream_t stream);
-int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_set_desc* out,
-                         void* d_pool, uint64_t pool_bytes, uint32_t flags, const WsLayout& L, bs_result* d_result,
-                         int sms, cudaStream_t stream);
-int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header,
-                     uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream);
-int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, const bs_opts& o,
-                            int sms, cudaStream_t stream);
-int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, uint32_t flags,
-                              const bs_opts& o, int sms, cudaStream_t stream);
-// wire format v2 (bs_layered.cu)
-bool layered_ws(void* d_ws, uint64_t ws_bytes, uint32_t Bs, uint32_t T, uint64_t B, WsLayout* out);
-int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t capacity,
-                               uint64_t expect_total, bs_result* d_result, int sms, cudaStream_t stream);
-int run_layered_deserialize_plan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_layered_desc* out,
-                                 void* d_pool, uint64_t pool_bytes, uint32_t flags, void* d_ws, uint64_t ws_bytes,
-                                 bs_result* d_result, int sms, cudaStream_t stream);
-int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, void* d_dst, uint64_t lo, uint64_t hi,
-                           const bs_opts& o, int sms, cudaStream_t stream, const PkgMap* pm = nullptr);
-int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws_bytes, const void* d_src,
-                             const void* d_header, uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms,
-                             cudaStream_t stream, const PkgMap* pm = nullptr);
-}  // namespace bs
-
 using namespace bs;
-
-namespace {
-constexpr uint32_t kFlagCheckPad = 0x100u;
-}
 
 
 // Pinned result words of the tickets come from a process-wide slab: cudaHostAlloc / cudaFreeHost synchronise the
@@ -175,7 +141,8 @@ int bs_engine_create(bs_engine** out, const bs_engine_cfg* cfg)
     if (e->cfg.n_staging == 0) e->cfg.n_staging = 2;
     if (e->cfg.chunk_bytes % 65536 != 0 || e->cfg.n_staging > kMaxStaging || e->cfg.n_staging < 1) { delete e; return BS_ERR_ARG; }
     resolve_opts(&cfg->opts, &e->opts);
-    int rc = device_sm_count(&e->sms);
+    int rc = check_opts(e->opts);  // a shape the kernels cannot run must not wait for the first call to show
+    if (rc == BS_OK) rc = device_sm_count(&e->sms);
     if (rc) { delete e; return rc; }
     int lo_prio = 0, hi_prio = 0;
     cudaError_t ce = cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio);
@@ -240,7 +207,8 @@ int bs_engine_offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layere
 {
     if (e == nullptr || (set == nullptr && lset == nullptr) || h_pinned == nullptr || ticket == nullptr) return BS_ERR_ARG;
     WsLayout L;
-    int rc;
+    int rc = set ? check_set(set) : check_layered_desc(lset);  // as the direct calls: a descriptor no loader accepts is refused here
+    if (rc) return rc;
     if (set) {
         if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
         if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
@@ -280,8 +248,9 @@ int bs_engine_offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layere
         const uint32_t b = k % S;
         const uint64_t lo = (uint64_t)k * C, hi = (lo + C < total_bytes) ? lo + C : total_bytes;
         if (k >= S) CK(cudaStreamWaitEvent(e->kstream, e->ev_c[b], 0));  // staging[b] drained by DMA k-S
-        rc = set ? run_pack_range(set, L, e->staging[b], lo, hi, e->opts, e->sms, e->kstream)
-                 : run_layered_pack_range(lset, e->ws, e->ws_bytes, e->staging[b], lo, hi, e->opts, e->sms, e->kstream);
+        rc = set ? run_pack_range(set, L, e->staging[b], lo, hi, e->opts, e->sms, e->kstream, kFlagPoisonOnError)
+                 : run_layered_pack_range(lset, e->ws, e->ws_bytes, e->staging[b], lo, hi, e->opts, e->sms, e->kstream, nullptr,
+                                          kFlagPoisonOnError);
         if (rc) return rc;
         CK(cudaEventRecord(e->ev_k[b], e->kstream));
         CK(cudaStreamWaitEvent(e->cstream, e->ev_k[b], 0));
@@ -304,10 +273,12 @@ int bs_engine_prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes,
 {
     if (e == nullptr || h_pinned == nullptr || (out == nullptr && lout == nullptr) || ticket == nullptr) return BS_ERR_ARG;
     if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
+    int rc = out ? check_set(out) : check_layered_desc(lout);
+    if (rc) return rc;
+    if (flags == BS_LAYOUT_POOL && pool_bytes && (d_pool == nullptr || ((uintptr_t)d_pool & 255))) return BS_ERR_ARG;
     if (nbytes < kFixedHeader) return BS_ERR_CORRUPT;
     bs_stream_info_t info;
     WsLayout L;
-    int rc;
     if (out) {
         if (known) info = *known;
         else if ((rc = bs_stream_info(h_pinned, &info))) return rc;  // the stream is in host RAM: its counts cost nothing to read
@@ -425,6 +396,8 @@ static int offload_packages_impl(bs_engine* e, const bs_set_desc* set, const bs_
     if (cap + BS_PKG_HEADER > e->cfg.chunk_bytes) return BS_ERR_CAPACITY;
     WsLayout L;
     uint64_t hb;
+    int rc = set ? check_set(set) : check_layered_desc(lset);
+    if (rc) return rc;
     if (set) {
         if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
         if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
@@ -436,7 +409,6 @@ static int offload_packages_impl(bs_engine* e, const bs_set_desc* set, const bs_
         if (!layered_ws(e->ws, e->ws_bytes, lset->n_struct_blocks, lset->n_layers, lset->n_addr, &L)) return BS_ERR_CAPACITY;
         hb = bs_layered_header_bytes(lset->n_structs, lset->n_layers, lset->n_struct_blocks);
     }
-    int rc;
     if (total_bytes == 0) {
         CK(cudaEventRecord(e->ev_fence_k, e->kstream));  // the workspace may still be in use by an earlier call
         CK(cudaStreamWaitEvent(producer, e->ev_fence_k, 0));
@@ -492,7 +464,7 @@ static int offload_packages_impl(bs_engine* e, const bs_set_desc* set, const bs_
             hi1 = hi;
             if (!one_launch) {
                 unsigned char* dst = e->staging[b] + m * slot_bytes;
-                CK(launch_pkg_header(L, cap, stream_id, k, count, dst, e->d_result, e->kstream));
+                CK(launch_pkg_header(L, cap, stream_id, k, count, dst, e->d_result, e->kstream, true));
                 rc = set ? run_pack_range(set, L, dst + BS_PKG_HEADER, lo, hi, e->opts, e->sms, e->kstream)
                          : run_layered_pack_range(lset, e->ws, e->ws_bytes, dst + BS_PKG_HEADER, lo, hi, e->opts, e->sms, e->kstream);
                 if (rc) return rc;
@@ -501,7 +473,7 @@ static int offload_packages_impl(bs_engine* e, const bs_set_desc* set, const bs_
             if (last_bytes != cap) { ++k; ++m; break; }  // a short package ends its batch
         }
         if (one_launch) {  // the batch's headers in one launch, its stream range [lo0, hi1) in one more
-            CK(launch_pkg_headers(L, cap, stream_id, k0, m, count, e->staging[b], slot_bytes, nullptr, e->d_result, e->kstream));
+            CK(launch_pkg_headers(L, cap, stream_id, k0, m, count, e->staging[b], slot_bytes, nullptr, e->d_result, e->kstream, true));
             PkgMap pm;
             pm.cap = cap; pm.slot_bytes = slot_bytes; pm.base = e->staging[b]; pm.slot_of = nullptr; pm.k_base = k0;
             rc = set ? run_pack_packages_range(set, L, pm, lo0, hi1, e->opts, e->sms, e->kstream)
@@ -529,10 +501,12 @@ static int prefetch_packages_impl(bs_engine* e, const void* h_slots, uint64_t sl
     if (e == nullptr || h_slots == nullptr || (out == nullptr && lout == nullptr) || ticket == nullptr || n_slots == 0) return BS_ERR_ARG;
     if ((slot_bytes & 15) || slot_bytes < BS_PKG_HEADER + 16) return BS_ERR_ARG;
     if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
+    int rc = out ? check_set(out) : check_layered_desc(lout);
+    if (rc) return rc;
+    if (flags == BS_LAYOUT_POOL && pool_bytes && (d_pool == nullptr || ((uintptr_t)d_pool & 255))) return BS_ERR_ARG;
     const unsigned char* slots = (const unsigned char*)h_slots;
     PkgPlan plan;  // the packages are in host RAM: their headers cost nothing to read
-    int rc = pkg_plan(slots, slot_bytes, n_slots, slot_bytes, stream_id, &plan);
-    if (rc) return rc;
+    if ((rc = pkg_plan(slots, slot_bytes, n_slots, slot_bytes, stream_id, &plan))) return rc;
     if (plan.hb > e->header_cap || plan.total > e->cfg.max_stream_bytes) return BS_ERR_CAPACITY;
     WsLayout L;
     if (out) {

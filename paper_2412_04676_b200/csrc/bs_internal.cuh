@@ -1,8 +1,11 @@
 // bs_internal.cuh — shared declarations of libbsstream's translation units (not part of the C ABI).
 //
 // Data layout in HBM:
-//   workspace := bs_wshead (256 B) | scan_state[n_scan_tiles+1] u64 | blk[B_cap+1] (16 B each)
+//   workspace := bs_wshead (256 B) | scan_state[n_scan_tiles+1] {word, tag} (16 B each) | blk[B_cap+1] (16 B each)
 //                | tile_first[n_granules_cap] u32
+//   Nothing in the workspace needs clearing between calls of the v1 scan (bs_scan_phase.cuh): every word the scan
+//   synchronises on carries the call's EPOCH tag, so whatever an earlier call (or nobody) left there reads as "not yet
+//   written".  (The layered plan of bs_layered.cu still clears its own head + state.)
 //   blk[i]        = { payload offset of block i , device address of block i | odd-flag in bit 0 }
 //                   — the paper's "pointer structure ... grid structure of the serialized data"
 //                   (PAPER L90-92), built before any data moves;  blk[B] = { P, 0 } sentinel.
@@ -51,15 +54,28 @@ struct __align__(256) WsHead {
     uint32_t scan_ticket2;
     uint32_t ctas_done2;
     uint32_t dtype;          // element type of the set the tables describe (bs.h BS_F64 ..)
+    uint32_t pad0;
+    // the v1 scan's own synchronisation words, each tagged with the epoch of the call that wrote it (bs_scan_phase.cuh):
+    // [63:24] epoch, [23:0] count / code.  A word of another epoch is stale whatever it holds.
+    uint64_t ep_ticket;      // work items handed out
+    uint64_t ep_done;        // work items completed; the CTA that completes the last one finalises
+    uint64_t ep_err;         // first error of the call ([7:0] = -code)
+    uint64_t ep_ready;       // == tag once the tables and the plain fields above are final (fused kernels wait on it)
+};
+static_assert(sizeof(WsHead) == 256, "WsHead is one 256-byte slot");
+
+struct __align__(16) ScanState {  // one tile of the chained scan: {flag | value, epoch tag}, read and written as ONE 16-byte access
+    uint64_t word;
+    uint64_t tag;
 };
 
 struct WsLayout {
     WsHead* head;
-    uint64_t* scan_state;
+    ScanState* scan_state;
     Blk* blk;
     uint32_t* tile_first;
     uint64_t n_granules_cap;
-    uint64_t zero_bytes;  // head + scan_state: cleared before every scan
+    uint64_t zero_bytes;  // head + scan_state: cleared in front of a scan only while a CUDA graph is being captured
 };
 
 __host__ __device__ inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + (a - 1)) / a * a; }
@@ -67,7 +83,7 @@ __host__ __device__ inline uint64_t align_up(uint64_t x, uint64_t a) { return (x
 inline uint64_t ws_fixed_bytes(uint32_t n_blocks)
 {
     uint64_t n_scan_tiles = ((uint64_t)n_blocks + kScanTile) / kScanTile + 1;
-    return sizeof(WsHead) + align_up(n_scan_tiles * 8, 256) + align_up(((uint64_t)n_blocks + 1) * sizeof(Blk), 256);
+    return sizeof(WsHead) + align_up(n_scan_tiles * sizeof(ScanState), 256) + align_up(((uint64_t)n_blocks + 1) * sizeof(Blk), 256);
 }
 
 inline bool ws_layout(void* d_ws, uint64_t ws_bytes, uint32_t n_blocks, WsLayout* L)
@@ -77,8 +93,8 @@ inline bool ws_layout(void* d_ws, uint64_t ws_bytes, uint32_t n_blocks, WsLayout
     if (d_ws == nullptr || ((uintptr_t)d_ws & 255) != 0 || ws_bytes < fixed + 16) return false;
     unsigned char* p = (unsigned char*)d_ws;
     L->head = (WsHead*)p;
-    L->scan_state = (uint64_t*)(p + sizeof(WsHead));
-    L->zero_bytes = sizeof(WsHead) + align_up(n_scan_tiles * 8, 256);
+    L->scan_state = (ScanState*)(p + sizeof(WsHead));
+    L->zero_bytes = sizeof(WsHead) + align_up(n_scan_tiles * sizeof(ScanState), 256);
     L->blk = (Blk*)(p + L->zero_bytes);
     L->tile_first = (uint32_t*)(p + fixed);
     L->n_granules_cap = (ws_bytes - fixed) / 4;
@@ -106,8 +122,11 @@ struct ScanParams {
     const uint32_t* out_dim;      // BS_SCATTER_TO_ADDR inputs
     const uint64_t* out_addr;
     uint32_t flags;
+    uint64_t tag;                 // the call's epoch tag (bs_scan_phase.cuh); filled in by the launchers
 };
 
+uint64_t next_epoch_tag();
+cudaError_t prepare_scan_state(const WsLayout& L, cudaStream_t stream);
 cudaError_t launch_scan(bool deser, const ScanParams& p, int sm_count, cudaStream_t stream);
 
 // ---- layered sets (wire format v2): what the header generator / parser of the move kernels needs ---------
@@ -175,7 +194,48 @@ __device__ __forceinline__ unsigned char* stream_at(const MoveParams& p, uint64_
 
 cudaError_t launch_move(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream);
 cudaError_t launch_move_tma(bool unpack, const MoveParams& p, const bs_opts& opts, int sm_count, cudaStream_t stream);
+// the size / offset pass and the movement of the whole stream in one launch (TMA variant; bs_move_tma.cu)
+cudaError_t launch_fused_tma(bool unpack, const ScanParams& sp, const MoveParams& p, const bs_opts& opts, uint64_t bytes_bound,
+                             int sm_count, cudaStream_t stream);
 
 void resolve_opts(const bs_opts* in, bs_opts* out);
+
+// ---- host-side runners shared by the translation units (bs_api.cu, bs_layered.cu) -------------------------------------------
+constexpr uint32_t kFlagCheckPad = 0x100u;       // unpack: pad bytes must be zero (engine path; the payload is not resident at parse time)
+constexpr uint32_t kFlagPoisonOnError = 0x200u;  // pack (engine): a deferred error zeroes the first 64 bytes of the range that holds
+                                                 // stream byte 0, so a host buffer never keeps a stale but valid header
+int cuda_fail(cudaError_t e);
+int device_sm_count(int* out);
+int check_set(const bs_set_desc* s);
+int check_layered_desc(const bs_layered_desc* s);
+int check_opts(const bs_opts& o);
+int run_serialize_scan(const bs_set_desc* set, const WsLayout& L, uint64_t capacity, uint64_t expect_total,
+                       bs_result* d_result, int sms, cudaStream_t stream);
+int run_pack_range(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint64_t lo, uint64_t hi, const bs_opts& o,
+                   int sms, cudaStream_t stream, uint32_t flags = 0);
+int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_set_desc* out,
+                         void* d_pool, uint64_t pool_bytes, uint32_t flags, const WsLayout& L, bs_result* d_result,
+                         int sms, cudaStream_t stream);
+int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header, uint64_t lo,
+                     uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream);
+int run_pack_packages(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, const bs_opts& o, int sms, cudaStream_t stream);
+int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, const bs_opts& o,
+                            int sms, cudaStream_t stream);
+int run_unpack_packages(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t header_bytes, uint32_t flags,
+                        const bs_opts& o, int sms, cudaStream_t stream);
+int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t lo, uint64_t hi, uint32_t flags,
+                              const bs_opts& o, int sms, cudaStream_t stream);
+// wire format v2 (bs_layered.cu)
+bool layered_ws(void* d_ws, uint64_t ws_bytes, uint32_t Bs, uint32_t T, uint64_t B, WsLayout* out);
+int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t capacity,
+                               uint64_t expect_total, bs_result* d_result, int sms, cudaStream_t stream);
+int run_layered_deserialize_plan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_layered_desc* out,
+                                 void* d_pool, uint64_t pool_bytes, uint32_t flags, void* d_ws, uint64_t ws_bytes,
+                                 bs_result* d_result, int sms, cudaStream_t stream);
+int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, void* d_dst, uint64_t lo, uint64_t hi,
+                           const bs_opts& o, int sms, cudaStream_t stream, const PkgMap* pm = nullptr, uint32_t flags = 0);
+int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws_bytes, const void* d_src,
+                             const void* d_header, uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms,
+                             cudaStream_t stream, const PkgMap* pm = nullptr);
 
 }  // namespace bs

@@ -20,8 +20,6 @@
 #include "bs_internal.cuh"
 
 namespace bs {
-int cuda_fail(cudaError_t e);
-int device_sm_count(int* out);
 
 namespace {
 
@@ -56,7 +54,7 @@ bool lw_layout(void* d_ws, uint64_t ws_bytes, uint32_t Bs, uint32_t T, uint64_t 
     unsigned char* p = (unsigned char*)d_ws;
     L->ws.head = (WsHead*)p;
     p += sizeof(WsHead);
-    L->ws.scan_state = (uint64_t*)p;
+    L->ws.scan_state = (ScanState*)p;  // unused by the layered plan (st1 / st2 below are its chains)
     for (int c = 0; c < 2; ++c) { L->st1[c] = (uint64_t*)p; p += align_up(t1 * 8, 256); }
     for (int c = 0; c < 2; ++c) { L->st2[c] = (uint64_t*)p; p += align_up(t2 * 8, 256); }
     L->ws.zero_bytes = (uint64_t)(p - (unsigned char*)d_ws);
@@ -701,6 +699,8 @@ unsigned plan_grid(const LPlanParams& p, int sms)
 }  // namespace
 
 // ---- entry points used by bs_engine.cu -----------------------------------------------------------------------------------
+int check_layered_desc(const bs_layered_desc* s) { return check_layered(s); }
+
 bool layered_ws(void* d_ws, uint64_t ws_bytes, uint32_t Bs, uint32_t T, uint64_t B, WsLayout* out)
 {
     LwLayout L;
@@ -781,7 +781,7 @@ int run_layered_deserialize_plan(const void* d_header, const void* d_payload, ui
 
 // pm != null: the stream side is a set of package slots (bs_pkg.cu); d_dst is then unused
 int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, void* d_dst, uint64_t lo, uint64_t hi,
-                           const bs_opts& o, int sms, cudaStream_t stream, const PkgMap* pm)
+                           const bs_opts& o, int sms, cudaStream_t stream, const PkgMap* pm, uint32_t flags)
 {
     MoveParams mp;
     memset(&mp, 0, sizeof(mp));
@@ -795,6 +795,7 @@ int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_b
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
+    mp.flags = flags;
     if (pm) mp.pkg = *pm;
     cudaError_t e = launch_move(false, mp, o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
@@ -824,8 +825,6 @@ int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
 }
-
-int check_opts(const bs_opts& o);
 
 }  // namespace bs
 
@@ -898,7 +897,7 @@ int bs_layered_serialize_range(const bs_layered_desc* set, void* d_dst, uint64_t
     int sms;
     if ((rc = device_sm_count(&sms))) return rc;
     if (run_scan && (rc = run_layered_serialize_plan(set, d_ws, ws_bytes, UINT64_MAX, 0, d_result, sms, stream))) return rc;
-    return run_layered_pack_range(set, d_ws, ws_bytes, d_dst, lo, hi, o, sms, stream, nullptr);
+    return run_layered_pack_range(set, d_ws, ws_bytes, d_dst, lo, hi, o, sms, stream, nullptr, 0);
 }
 
 int bs_layered_serialize(const bs_layered_desc* set, void* d_stream, uint64_t capacity, void* d_ws, uint64_t ws_bytes,
@@ -913,7 +912,7 @@ int bs_layered_serialize(const bs_layered_desc* set, void* d_stream, uint64_t ca
     int sms;
     if ((rc = device_sm_count(&sms))) return rc;
     if ((rc = run_layered_serialize_plan(set, d_ws, ws_bytes, capacity, 0, d_result, sms, stream))) return rc;
-    return run_layered_pack_range(set, d_ws, ws_bytes, d_stream, 0, capacity & ~15ull, o, sms, stream, nullptr);
+    return run_layered_pack_range(set, d_ws, ws_bytes, d_stream, 0, capacity & ~15ull, o, sms, stream, nullptr, 0);
 }
 
 int bs_layered_deserialize(const void* d_stream, uint64_t nbytes, bs_layered_desc* out, void* d_pool, uint64_t pool_bytes,

@@ -45,7 +45,10 @@ template <bool UNPACK, int UPT>
 __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
 {
     const WsHead* head = p.ws.head;
-    if (head->status != 0) return;  // deferred error: nothing is written
+    if (head->status != 0) {  // deferred error: nothing is written (the engine has a stale header blanked, see kFlagPoisonOnError)
+        if (!UNPACK) poison_on_error(p);
+        return;
+    }
     const uint32_t T = head->n_tensors, B = head->n_blocks;
     const uint64_t hb = head->header_bytes, P = head->payload_bytes, total = hb + P;
     const uint64_t ng = head->n_granules;
@@ -63,7 +66,7 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
     }
     // ---- payload tiles: tile k = payload bytes [k*kTileBytes, (k+1)*kTileBytes) ----
     uint64_t plo = 0, phi = 0, k0 = 0, np = 0;
-    if (hi > hb && hi > lo) {
+    if (hi > hb && hi > lo && B != 0) {  // no block, no payload tile (the scan rejects a payload without blocks)
         plo = (lo > hb ? lo : hb) - hb;
         phi = hi - hb;
         k0 = plo / kTileBytes;

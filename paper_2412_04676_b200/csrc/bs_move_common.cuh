@@ -5,7 +5,14 @@
 
 namespace bs {
 
-constexpr uint32_t kFlagCheckPad = 0x100u;  // unpack: pad bytes must be zero (engine path; see bs_engine.cu)
+
+// pack with a deferred error, engine path: the staging buffer goes to the host whatever happened, and it may still hold
+// the stream of an earlier call — blank the 64 bytes where this call's fixed header would be
+__device__ __forceinline__ void poison_on_error(const MoveParams& p)
+{
+    if ((p.flags & kFlagPoisonOnError) && p.lo == 0 && p.pkg.cap == 0 && blockIdx.x == 0 && threadIdx.x < 4)
+        reinterpret_cast<uint4*>(p.stream)[threadIdx.x] = make_uint4(0, 0, 0, 0);
+}
 
 // owner of block r: the last tensor t with first_block[t] <= r (tensors partition the blocks in order)
 __device__ __forceinline__ uint32_t tensor_of_block(const bs_tensor_rec* tensors, uint32_t T, uint32_t r)
@@ -20,12 +27,12 @@ __device__ __forceinline__ uint32_t tensor_of_block(const bs_tensor_rec* tensors
 
 // ---- S3: one 16-byte unit of the header region (wire format v1) -------------------------------------------
 __device__ __forceinline__ uint4 header_unit(const MoveParams& p, uint64_t u, uint32_t T, uint32_t B, uint64_t hb,
-                                             uint64_t P)
+                                             uint64_t P, uint32_t dtype)
 {
     uint4 v = make_uint4(0, 0, 0, 0);
     if (u < 4) {
         if (u == 0) v = make_uint4(0x41505342u, 0x31455352u, 1u, 0x01020304u);  // "BSPARSE1", version, endian_tag
-        else if (u == 1) v = make_uint4(p.ws.head->dtype, 2u, 3u, 16u);          // dtype, n_qn, max_rank, align
+        else if (u == 1) v = make_uint4(dtype, 2u, 3u, 16u);                      // dtype, n_qn, max_rank, align
         else if (u == 2) v = make_uint4(T, 0u, B, 0u);                           // u64 n_tensors, u64 n_blocks
         else v = make_uint4((uint32_t)hb, (uint32_t)(hb >> 32), (uint32_t)P, (uint32_t)(P >> 32));
         return v;
@@ -46,7 +53,7 @@ __device__ __forceinline__ uint4 header_unit(const MoveParams& p, uint64_t u, ui
             int2 a = __ldg(reinterpret_cast<const int2*>(q + 4));
             v = make_uint4((uint32_t)a.x, (uint32_t)a.y, __ldg(d), __ldg(d + 1));
         } else {
-            const uint64_t off = p.ws.blk[r].off;
+            const uint64_t off = __ldcg(reinterpret_cast<const unsigned long long*>(&p.ws.blk[r].off));
             v = make_uint4(__ldg(d + 2), tensor_of_block(p.tensors, T, r), (uint32_t)off, (uint32_t)(off >> 32));
         }
     }
@@ -75,7 +82,7 @@ __device__ __forceinline__ void rebuild_record(const MoveParams& p, uint64_t rec
         p.dim[3 * r + 0] = r1.z;
         p.dim[3 * r + 1] = r1.w;
         p.dim[3 * r + 2] = r2.x;
-        p.addr[r] = p.ws.blk[r].addr & ~7ull;
+        p.addr[r] = __ldcg(reinterpret_cast<const unsigned long long*>(&p.ws.blk[r].addr)) & ~7ull;
     }
 }
 
@@ -176,7 +183,7 @@ __device__ __forceinline__ void rebuild_record_v2(const MoveParams& p, uint64_t 
 __device__ __forceinline__ uint4 header_unit_any(const MoveParams& p, uint64_t u, uint32_t T, uint32_t B, uint64_t hb,
                                                  uint64_t P)
 {
-    return p.lay.on ? header_unit_v2(p, u, T, hb, P) : header_unit(p, u, T, B, hb, P);
+    return p.lay.on ? header_unit_v2(p, u, T, hb, P) : header_unit(p, u, T, B, hb, P, p.ws.head->dtype);
 }
 __device__ __forceinline__ uint64_t n_rebuild_records(const MoveParams& p, const WsHead* head)
 {
@@ -196,7 +203,8 @@ __device__ __forceinline__ void rebuild_record_any(const MoveParams& p, const Ws
 // (few); block records one LANE per record, four records per lane in flight, each worker a contiguous run of
 // records so the owning tensor is found by one binary search and then only ever steps forward.
 __device__ __forceinline__ void write_header_warp(const MoveParams& p, uint32_t T, uint32_t B, uint64_t hb, uint64_t P,
-                                                  uint64_t lo, uint64_t hend, uint64_t hw, uint64_t n_hw, uint32_t lane)
+                                                  uint32_t dtype, uint64_t lo, uint64_t hend, uint64_t hw, uint64_t n_hw,
+                                                  uint32_t lane)
 {
     if (lo >= hend) return;
     const uint64_t rec0 = kFixedHeader + kTensorRec * (uint64_t)T;  // stream offset of block record 0
@@ -206,7 +214,7 @@ __device__ __forceinline__ void write_header_warp(const MoveParams& p, uint32_t 
         for (uint64_t i = hw * 32 + lane; i < n_head + n_slack; i += n_hw * 32) {
             const uint64_t u = i < n_head ? i : rec_end / 16 + (i - n_head);
             const uint64_t s = u * 16;
-            if (s >= lo && s < hend) __stcs(reinterpret_cast<uint4*>(stream_at(p, hb, s)), header_unit(p, u, T, B, hb, P));
+            if (s >= lo && s < hend) __stcs(reinterpret_cast<uint4*>(stream_at(p, hb, s)), header_unit(p, u, T, B, hb, P, dtype));
         }
     }
     if (B == 0 || hend <= rec0 || lo >= rec_end) return;
@@ -228,7 +236,7 @@ __device__ __forceinline__ void write_header_warp(const MoveParams& p, uint32_t 
                 const int2* q = reinterpret_cast<const int2*>(p.qn + 6 * r);
                 q0[k] = __ldg(q); q1[k] = __ldg(q + 1); q2[k] = __ldg(q + 2);
                 d0[k] = __ldg(p.dim + 3 * r); d1[k] = __ldg(p.dim + 3 * r + 1); d2[k] = __ldg(p.dim + 3 * r + 2);
-                off[k] = p.ws.blk[r].off;
+                off[k] = __ldcg(reinterpret_cast<const unsigned long long*>(&p.ws.blk[r].off));  // L2: fused kernels
             }
         }
 #pragma unroll
@@ -268,6 +276,18 @@ __device__ __forceinline__ void rebuild_header_warp(const MoveParams& p, uint32_
     for (uint64_t base = hw * 128; base < n_rec; base += n_hw * 128) {
 #pragma unroll
         for (int k = 0; k < 4; ++k) rebuild_record_any(p, head, base + (uint64_t)k * 32 + lane);
+    }
+}
+
+
+// the same for wire format v1 with the counts in registers (fused kernels: the workspace head may not be written yet)
+__device__ __forceinline__ void rebuild_header_warp_v1(const MoveParams& p, uint32_t T, uint32_t B, uint64_t hw, uint64_t n_hw,
+                                                       uint32_t lane)
+{
+    const uint64_t n_rec = (uint64_t)T + B;
+    for (uint64_t base = hw * 128; base < n_rec; base += n_hw * 128) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) rebuild_record(p, base + (uint64_t)k * 32 + lane, T, B);
     }
 }
 

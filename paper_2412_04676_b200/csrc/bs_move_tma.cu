@@ -21,7 +21,10 @@
 //
 // Roofline: pure data movement — 1 byte read + 1 byte written per stream byte, HBM-bound; ~2 instructions per
 // block segment and per tile instead of ~70 per 512 bytes in the LDG variant.
+#include <atomic>
+
 #include "bs_move_common.cuh"
+#include "bs_scan_phase.cuh"
 
 namespace bs {
 
@@ -30,6 +33,7 @@ namespace {
 constexpr uint32_t kMaxWarps = 16;   // data warps; one more warp per CTA works on the header
 constexpr uint32_t kMaxStages = 8;
 constexpr uint32_t kSmemLimit = 227u * 1024u;
+constexpr uint32_t kStaticSmem = 2048u;  // room for the kernels' static shared memory (mbarriers, the pass's outcome)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -41,18 +45,30 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t byt
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
 {
+    uint32_t ok;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity)
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
         : "memory");
+    return ok != 0;
+}
+// Bounded: a phase that never completes (the byte count announced with expect_tx and the copies issued disagree — the
+// one piece of arithmetic the pack path does per tile) must not hang the GPU.  try_wait itself blocks for a
+// hardware-defined slice, so 2^22 rounds are seconds, far beyond any real wait; then the call fails with BS_ERR_CUDA
+// in the workspace status (what was written so far is unspecified) and the warp stops.
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, int* status)
+{
+    for (uint32_t spin = 0; spin < (1u << 22); ++spin)
+        if (mbar_try_wait(bar, parity)) return true;
+    atomicCAS(status, 0, BS_ERR_CUDA);
+    return false;
 }
 // the mbarrier also waits for every cp.async this thread has issued so far (pending count +1 now, -1 on completion)
 __device__ __forceinline__ void cp_async_mbar_arrive(uint32_t bar)
@@ -154,8 +170,12 @@ __device__ __forceinline__ bool clip_seg(const Blk& e, uint64_t next, uint64_t t
 }
 __device__ __forceinline__ bool make_seg(const Blk* __restrict__ blk, uint32_t j, uint64_t tlo, uint64_t thi, Seg* s)
 {
-    const Blk e = blk[j];
-    const uint64_t next = __ldg(reinterpret_cast<const unsigned long long*>(&blk[j + 1].off));
+    // L2 loads: in a fused kernel other CTAs wrote the table during this launch
+    const uint4 w = __ldcg(reinterpret_cast<const uint4*>(blk + j));
+    Blk e;
+    e.off = (uint64_t)w.x | ((uint64_t)w.y << 32);
+    e.addr = (uint64_t)w.z | ((uint64_t)w.w << 32);
+    const uint64_t next = __ldcg(reinterpret_cast<const unsigned long long*>(&blk[j + 1].off));
     return clip_seg(e, next, tlo, thi, s);
 }
 
@@ -232,18 +252,19 @@ __host__ __device__ inline Preset preset(bool unpack, uint64_t pkg_cap)
     return ps;
 }
 
-template <bool UNPACK>
-__global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const MoveParams p, const uint32_t opt_stages,
-                                                                     const uint32_t opt_warps)
+// FUSED: called behind the size / offset pass inside one kernel (fused_tma_kernel); `hv` is that pass's outcome.
+template <bool UNPACK, bool FUSED>
+__device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::HeadView& hv, const uint32_t opt_stages,
+                                              const uint32_t opt_warps, unsigned char* smem, uint64_t* s_bar)
 {
-    extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ __align__(8) uint64_t s_bar[kMaxWarps * kMaxStages];
-
     const WsHead* head = p.ws.head;
-    if (head->status != 0) return;  // deferred error: nothing is written
-    const uint32_t T = head->n_tensors, B = head->n_blocks;
-    const uint64_t hb = head->header_bytes, P = head->payload_bytes, total = hb + P;
-    const uint64_t ng = head->n_granules;
+    if (hv.status != 0) {  // deferred error: nothing is written (the engine has a stale header blanked, see kFlagPoisonOnError)
+        if (!UNPACK) poison_on_error(p);
+        return;
+    }
+    const uint32_t T = hv.T, B = hv.B;
+    const uint64_t hb = hv.hb, P = hv.P, total = hb + P;
+    const uint64_t ng = hv.ng;
     const uint64_t lo = p.lo, hi = p.hi < total ? p.hi : total;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t tile_bytes = p.tile_bytes, n_warps = opt_warps & 0xffffu;
@@ -267,10 +288,13 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
         const uint64_t hw = np == 0 ? (uint64_t)blockIdx.x * (n_warps + 1) + warp : blockIdx.x;
         const uint64_t n_hw = np == 0 ? (uint64_t)gridDim.x * (n_warps + 1) : gridDim.x;
         if (UNPACK) {
-            if (p.header != nullptr) rebuild_header_warp(p, T, B, hw, n_hw, lane);
+            if (p.header != nullptr) {
+                if (FUSED) rebuild_header_warp_v1(p, T, B, hw, n_hw, lane);
+                else rebuild_header_warp(p, T, B, hw, n_hw, lane);
+            }
         } else {
             if (p.lay.on) write_header_warp_v2(p, T, hb, P, lo, hi < hb ? hi : hb, hw, n_hw, lane);
-            else write_header_warp(p, T, B, hb, P, lo, hi < hb ? hi : hb, hw, n_hw, lane);
+            else write_header_warp(p, T, B, hb, P, hv.dtype, lo, hi < hb ? hi : hb, hw, n_hw, lane);
         }
         return;
     }
@@ -295,6 +319,7 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
     const uint64_t per = (np + n_workers - 1) / n_workers;
     const int64_t n_mine = blocked ? (np > worker * per ? (int64_t)(np - worker * per < per ? np - worker * per : per) : 0)
                                    : (np > worker ? (int64_t)((np - worker + n_workers - 1) / n_workers) : 0);
+    int* const status = const_cast<int*>(&head->status);
     Hints hints;
     hints.pol = policy_evict_first();
     hints.ld = (p.tune & 1u) != 0;
@@ -410,17 +435,18 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
             const uint64_t thi = tbase + tile_bytes < phi ? tbase + tile_bytes : phi;
             const uint32_t sbase = ring + st * tile_bytes, bar = bar0 + 8 * st;
             if (!UNPACK) {
+                uint32_t landed = 1;
+                if (lane == 0) landed = mbar_wait(bar, parity, status) ? 1u : 0u;
+                if (__shfl_sync(0xffffffffu, landed, 0) == 0) break;  // warp-uniform
                 if (lane == 0) {
-                    mbar_wait(bar, parity);
                     fence_proxy_async();  // the cp.async tails were written through the generic proxy
                     bulk_s2g_x(stream_at(p, hb, hb + tlo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo), hints);
                 }
             } else {
-                int* status = const_cast<int*>(&head->status);
                 const unsigned char* sp = ring_ptr + (size_t)st * tile_bytes;
                 Seg s0;
                 const bool have0 = clip_seg(e0, next0, tlo, thi, &s0);
-                mbar_wait(bar, parity);
+                if (!__all_sync(0xffffffffu, mbar_wait(bar, parity, status))) break;  // warp-uniform
                 if (have0) unpack_seg(s0, sbase + (uint32_t)(s0.lo - tbase), sp + (s0.lo - tbase), p.flags, status, hints);
                 if (jhi >= jlo + 32) {
                     for (uint32_t j = jlo + lane + 32; j <= jhi; j += 32) {
@@ -435,32 +461,120 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
     }
     cp_async_wait<0>();
     bulk_wait_read<0>();
+}
 
+template <bool UNPACK>
+__global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const MoveParams p, const uint32_t opt_stages,
+                                                                     const uint32_t opt_warps)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ __align__(8) uint64_t s_bar[kMaxWarps * kMaxStages];
+    const WsHead* head = p.ws.head;
+    scan::HeadView hv;
+    hv.status = head->status; hv.T = head->n_tensors; hv.B = head->n_blocks; hv.dtype = head->dtype;
+    hv.hb = head->header_bytes; hv.P = head->payload_bytes; hv.ng = head->n_granules;
+    move_tma_body<UNPACK, false>(p, hv, opt_stages, opt_warps, smem, s_bar);
+}
+
+// ONE launch per bs_serialize / bs_deserialize call: the size / offset pass (bs_scan_phase.cuh) run by the
+// first kScanThreads threads of every CTA — its shared state lives at the start of the dynamic shared memory the rings use
+// afterwards — then the data movement above.  A set of one work item (<= 1024 blocks and tensors) runs the pass
+// replicated: no CTA waits for another; larger sets claim items from the ticket and wait for WsHead.ep_ready.
+template <bool UNPACK>
+__global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) fused_tma_kernel(const ScanParams sp, const MoveParams p,
+                                                                      const uint32_t opt_stages, const uint32_t opt_warps)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ __align__(8) uint64_t s_bar[kMaxWarps * kMaxStages];
+    __shared__ scan::HeadView s_hv;
+    scan::Shared& sm = *reinterpret_cast<scan::Shared*>(smem);
+    const scan::Shape s = scan::shape_of<UNPACK>(sp);
+    const bool replicated = s.n_items == 1;
+    if (threadIdx.x < kScanThreads) scan::run<UNPACK>(sp, s, sp.tag, sm, replicated);
+    scan::HeadView hv;
+    if (replicated) {
+        __syncthreads();
+        hv = sm.out;
+        __syncthreads();  // the rings reuse the pass's shared memory
+    } else {
+        hv = scan::wait_ready(sp.ws.head, sp.tag, &s_hv);
+    }
+    move_tma_body<UNPACK, true>(p, hv, opt_stages, opt_warps, smem, s_bar);
+}
+
+// The kernels may use the whole 227 KiB of dynamic shared memory: opt in once per kernel and device.  The flags are atomic
+// (bs.h: calls are re-entrant); two threads racing here both set the same value.
+template <typename K>
+cudaError_t allow_max_smem(K kernel, std::atomic<uint64_t>* done)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool tracked = dev >= 0 && dev < 64;
+    if (tracked && (done->load(std::memory_order_acquire) >> dev) & 1ull) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmemLimit - kStaticSmem));
+    if (e != cudaSuccess) return e;
+    if (tracked) done->fetch_or(1ull << dev, std::memory_order_release);
+    return cudaSuccess;
+}
+
+struct Shape3 {
+    uint32_t tile_bytes, stages, warps, auto_shape;
+    size_t smem;
+};
+template <bool UNPACK>
+cudaError_t resolve_shape(const MoveParams& p, const bs_opts& o, Shape3* out)
+{
+    Shape3 sh = {p.tile_bytes, o.stages, o.warps, 0u, 0};
+    if (o.tile_bytes == 0) {  // bs_opts left the shape open
+        const Preset ps = preset(UNPACK, p.pkg.cap);
+        sh.tile_bytes = ps.tile_bytes; sh.stages = ps.stages; sh.warps = ps.warps;
+        if (!UNPACK) sh.auto_shape = 0x80000000u;
+    }
+    if (sh.stages < 3 || sh.stages > kMaxStages || sh.warps < 1 || sh.warps > kMaxWarps) return cudaErrorInvalidValue;
+    sh.smem = (size_t)sh.warps * sh.stages * sh.tile_bytes + (size_t)sh.warps * kMetaBytes;
+    if (sh.smem + kStaticSmem > kSmemLimit) return cudaErrorInvalidValue;
+    *out = sh;
+    return cudaSuccess;
 }
 
 template <bool UNPACK>
 cudaError_t launch_tma_t(const MoveParams& p, const bs_opts& o, int sm_count, cudaStream_t stream)
 {
     MoveParams q = p;
-    uint32_t stages = o.stages, warps = o.warps, auto_shape = 0;
-    if (o.tile_bytes == 0) {  // bs_opts left the shape open
-        const Preset ps = preset(UNPACK, q.pkg.cap);
-        q.tile_bytes = ps.tile_bytes; stages = ps.stages; warps = ps.warps;
-        if (!UNPACK) auto_shape = 0x80000000u;
-    }
-    if (stages < 3 || stages > kMaxStages || warps < 1 || warps > kMaxWarps) return cudaErrorInvalidValue;
-    const size_t smem = (size_t)warps * stages * q.tile_bytes + (size_t)warps * kMetaBytes;
-    if (smem + 1024 > kSmemLimit) return cudaErrorInvalidValue;
-    static size_t configured[64] = {0};  // per kernel instantiation and device (the attribute is per device)
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
+    Shape3 sh;
+    cudaError_t e = resolve_shape<UNPACK>(p, o, &sh);
     if (e != cudaSuccess) return e;
-    if (dev < 0 || dev >= 64 || smem > configured[dev]) {
-        e = cudaFuncSetAttribute(move_tma_kernel<UNPACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        if (dev >= 0 && dev < 64) configured[dev] = smem;
-    }
-    move_tma_kernel<UNPACK><<<(unsigned)sm_count, (warps + 1) * 32, smem, stream>>>(q, stages, warps | auto_shape);  // + the header warp
+    q.tile_bytes = sh.tile_bytes;
+    static std::atomic<uint64_t> allowed{0};
+    if ((e = allow_max_smem(move_tma_kernel<UNPACK>, &allowed)) != cudaSuccess) return e;
+    move_tma_kernel<UNPACK><<<(unsigned)sm_count, (sh.warps + 1) * 32, sh.smem, stream>>>(q, sh.stages, sh.warps | sh.auto_shape);  // + the header warp
+    return cudaGetLastError();
+}
+
+// the pass and the movement of the whole stream in ONE launch.  `bytes_bound`: an upper bound of the stream's size
+// (serialize: the capacity; deserialize: nbytes) — CTAs beyond the tiles it can hold would find no work.
+template <bool UNPACK>
+cudaError_t launch_fused_t(const ScanParams& sp, const MoveParams& p, const bs_opts& o, uint64_t bytes_bound, int sm_count,
+                           cudaStream_t stream)
+{
+    MoveParams q = p;
+    Shape3 sh;
+    cudaError_t e = resolve_shape<UNPACK>(p, o, &sh);
+    if (e != cudaSuccess) return e;
+    q.tile_bytes = sh.tile_bytes;
+    if (sh.smem < sizeof(scan::Shared)) return cudaErrorInvalidValue;  // cannot happen: a ring is >= 3 x 16 KiB
+    static std::atomic<uint64_t> allowed{0};
+    if ((e = allow_max_smem(fused_tma_kernel<UNPACK>, &allowed)) != cudaSuccess) return e;
+    if ((e = prepare_scan_state(sp.ws, stream)) != cudaSuccess) return e;
+    ScanParams s2 = sp;
+    s2.tag = next_epoch_tag();
+    const uint64_t items = scan::host_items(sp.T, sp.B);
+    const uint64_t tiles = bytes_bound / kGranule + 2;  // data warps take tiles of >= 16 KiB; + the header's share
+    uint64_t grid = items > tiles ? items : tiles;
+    if (grid > (uint64_t)sm_count) grid = (uint64_t)sm_count;
+    const uint32_t threads = (sh.warps + 1) * 32 > kScanThreads ? (sh.warps + 1) * 32 : kScanThreads;
+    fused_tma_kernel<UNPACK><<<(unsigned)grid, threads, sh.smem, stream>>>(s2, q, sh.stages, sh.warps | sh.auto_shape);
     return cudaGetLastError();
 }
 
@@ -469,6 +583,13 @@ cudaError_t launch_tma_t(const MoveParams& p, const bs_opts& o, int sm_count, cu
 cudaError_t launch_move_tma(bool unpack, const MoveParams& p, const bs_opts& o, int sm_count, cudaStream_t stream)
 {
     return unpack ? launch_tma_t<true>(p, o, sm_count, stream) : launch_tma_t<false>(p, o, sm_count, stream);
+}
+
+cudaError_t launch_fused_tma(bool unpack, const ScanParams& sp, const MoveParams& p, const bs_opts& o, uint64_t bytes_bound,
+                             int sm_count, cudaStream_t stream)
+{
+    return unpack ? launch_fused_t<true>(sp, p, o, bytes_bound, sm_count, stream)
+                  : launch_fused_t<false>(sp, p, o, bytes_bound, sm_count, stream);
 }
 
 }  // namespace bs

@@ -23,37 +23,7 @@
 
 namespace bs {
 
-int cuda_fail(cudaError_t e);
-int device_sm_count(int* out);
-int check_opts(const bs_opts& o);
-int run_serialize_scan(const bs_set_desc* set, const WsLayout& L, uint64_t capacity, uint64_t expect_total,
-                       bs_result* d_result, int sms, cudaStream_t stream);
-int run_pack_range(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint64_t lo, uint64_t hi, const bs_opts& o,
-                   int sms, cudaStream_t stream);
-int run_deserialize_scan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_set_desc* out,
-                         void* d_pool, uint64_t pool_bytes, uint32_t flags, const WsLayout& L, bs_result* d_result,
-                         int sms, cudaStream_t stream);
-int run_unpack_range(const bs_set_desc* out, const WsLayout& L, const void* d_src, const void* d_header, uint64_t lo,
-                     uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream);
-int run_pack_packages(const bs_set_desc* set, const WsLayout& L, const PkgMap& pm, const bs_opts& o, int sms, cudaStream_t stream);
-// wire format v2 (bs_layered.cu)
-bool layered_ws(void* d_ws, uint64_t ws_bytes, uint32_t Bs, uint32_t T, uint64_t B, WsLayout* out);
-int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, uint64_t capacity, uint64_t expect_total,
-                               bs_result* d_result, int sms, cudaStream_t stream);
-int run_layered_deserialize_plan(const void* d_header, const void* d_payload, uint64_t nbytes, const bs_layered_desc* out,
-                                 void* d_pool, uint64_t pool_bytes, uint32_t flags, void* d_ws, uint64_t ws_bytes,
-                                 bs_result* d_result, int sms, cudaStream_t stream);
-int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_bytes, void* d_dst, uint64_t lo, uint64_t hi,
-                           const bs_opts& o, int sms, cudaStream_t stream, const PkgMap* pm);
-int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws_bytes, const void* d_src, const void* d_header,
-                             uint64_t lo, uint64_t hi, uint32_t flags, const bs_opts& o, int sms, cudaStream_t stream,
-                             const PkgMap* pm);
-int run_unpack_packages(const bs_set_desc* out, const WsLayout& L, const PkgMap& pm, uint64_t header_bytes, uint32_t flags,
-                        const bs_opts& o, int sms, cudaStream_t stream);
-
 namespace {
-
-constexpr uint32_t kFlagCheckPad = 0x100u;
 
 // the block holding payload byte x (x < P): the largest i in [0,B) with off_i <= x
 __device__ __forceinline__ uint32_t block_of_byte(const Blk* __restrict__ blk, uint32_t B, uint64_t x)
@@ -73,11 +43,16 @@ __device__ __forceinline__ void pkg_fail(WsHead* head, bs_result* result, int co
 }
 
 // the 64-byte header of package k -> dst
+// poison (engine path): on a deferred error the slot's header is blanked, so a stale package never reaches the host as valid
 __device__ __forceinline__ void pkg_write_header(const WsLayout& ws, uint64_t cap, uint64_t stream_id, uint64_t k,
-                                                 uint64_t expect_count, unsigned char* dst, bs_result* result)
+                                                 uint64_t expect_count, unsigned char* dst, bs_result* result, bool poison)
 {
     WsHead* head = ws.head;
-    if (head->status != 0) return;  // deferred error: nothing is written
+    if (head->status != 0) {  // deferred error: nothing is written
+        if (poison)
+            for (int z = 0; z < 4; ++z) reinterpret_cast<uint4*>(dst)[z] = make_uint4(0, 0, 0, 0);
+        return;
+    }
     const uint64_t hb = head->header_bytes, total = hb + head->payload_bytes;
     const uint32_t B = head->n_blocks;
     const uint64_t count = pkg_count(hb, total, cap);
@@ -103,21 +78,21 @@ __device__ __forceinline__ void pkg_write_header(const WsLayout& ws, uint64_t ca
 
 // one thread: package k -> dst
 __global__ void pkg_header_kernel(WsLayout ws, uint64_t cap, uint64_t stream_id, uint64_t k, uint64_t expect_count,
-                                  unsigned char* dst, bs_result* result)
+                                  unsigned char* dst, bs_result* result, bool poison)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    pkg_write_header(ws, cap, stream_id, k, expect_count, dst, result);
+    pkg_write_header(ws, cap, stream_id, k, expect_count, dst, result, poison);
 }
 
 // one thread per package: every header of the cut -> its slot (slot_of: device table index -> slot, or identity)
 __global__ void pkg_headers_kernel(WsLayout ws, uint64_t cap, uint64_t stream_id, uint64_t first, uint64_t n, uint64_t count,
-                                   unsigned char* base, uint64_t slot_bytes, const uint32_t* slot_of, bs_result* result)
+                                   unsigned char* base, uint64_t slot_bytes, const uint32_t* slot_of, bs_result* result, bool poison)
 {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const uint64_t k = first + i;  // packages [first, first + n) of the cut; without a table they lie in slots 0 .. n-1
     const uint64_t slot = slot_of ? (uint64_t)slot_of[k] : i;
-    pkg_write_header(ws, cap, stream_id, k, count, base + slot * slot_bytes, result);
+    pkg_write_header(ws, cap, stream_id, k, count, base + slot * slot_bytes, result, poison);
 }
 
 // one thread per slot: slot_of[index] = slot for the packages of this stream (the host plan proved the indices unique)
@@ -184,18 +159,19 @@ uint64_t rd64(const unsigned char* p) { uint64_t v; memcpy(&v, p, 8); return v; 
 }  // namespace
 
 cudaError_t launch_pkg_header(const WsLayout& L, uint64_t cap, uint64_t stream_id, uint64_t k, uint64_t expect_count,
-                              void* d_dst, bs_result* d_result, cudaStream_t stream)
+                              void* d_dst, bs_result* d_result, cudaStream_t stream, bool poison)
 {
-    pkg_header_kernel<<<1, 32, 0, stream>>>(L, cap, stream_id, k, expect_count, (unsigned char*)d_dst, d_result);
+    pkg_header_kernel<<<1, 32, 0, stream>>>(L, cap, stream_id, k, expect_count, (unsigned char*)d_dst, d_result, poison);
     return cudaGetLastError();
 }
 
 cudaError_t launch_pkg_headers(const WsLayout& L, uint64_t cap, uint64_t stream_id, uint64_t first, uint64_t n, uint64_t count,
-                               void* d_base, uint64_t slot_bytes, const uint32_t* d_slot_of, bs_result* d_result, cudaStream_t stream)
+                               void* d_base, uint64_t slot_bytes, const uint32_t* d_slot_of, bs_result* d_result, cudaStream_t stream,
+                               bool poison)
 {
     if (n == 0) return cudaSuccess;
     pkg_headers_kernel<<<(unsigned)((n + 127) / 128), 128, 0, stream>>>(L, cap, stream_id, first, n, count, (unsigned char*)d_base,
-                                                                         slot_bytes, d_slot_of, d_result);
+                                                                         slot_bytes, d_slot_of, d_result, poison);
     return cudaGetLastError();
 }
 

@@ -39,9 +39,10 @@ int pkg_plan(const unsigned char* h_hdrs, uint64_t stride, uint64_t n_slots, uin
 // the size limit whose cut (bs.h) the planned packages are, if it is a multiple of `tile`; 0 if they are cut otherwise
 uint64_t plan_uniform_cap(const PkgPlan& plan, uint32_t tile);
 cudaError_t launch_pkg_header(const WsLayout& L, uint64_t cap, uint64_t stream_id, uint64_t k, uint64_t expect_count,
-                              void* d_dst, bs_result* d_result, cudaStream_t stream);
+                              void* d_dst, bs_result* d_result, cudaStream_t stream, bool poison_on_error = false);
 cudaError_t launch_pkg_headers(const WsLayout& L, uint64_t cap, uint64_t stream_id, uint64_t first, uint64_t n, uint64_t count,
-                               void* d_base, uint64_t slot_bytes, const uint32_t* d_slot_of, bs_result* d_result, cudaStream_t stream);
+                               void* d_base, uint64_t slot_bytes, const uint32_t* d_slot_of, bs_result* d_result, cudaStream_t stream,
+                               bool poison_on_error = false);
 cudaError_t launch_pkg_check(const WsLayout& L, const void* d_hdrs, uint64_t stride, uint64_t n_slots, uint64_t stream_id,
                              bs_result* d_result, cudaStream_t stream);
 

@@ -33,6 +33,8 @@ struct IoJob {
     unsigned char* h = nullptr;
     uint64_t nbytes = 0;
     cudaEvent_t after = nullptr;   // spill: recorded behind the save's last DMA; the thread waits for it
+    const bs_ticket* save = nullptr;  // spill: the save whose stream is written out (alive while the job is pending: whatever
+                                      // retires a key's save ticket waits for the key's storage job first)
     int status = BS_OK;
     uint64_t bytes = 0;
     double seconds = 0.0;
@@ -59,6 +61,7 @@ struct bs_queue {
         bs_layered_stream_info_t linfo;
         bool adopted = false;
         bool layered = false;  // the stored stream is wire format v2
+        bool fill_pending = false;  // `io` is a fill whose outcome (and wire format) no load has looked at yet
     };
     bs_engine* lane_save = nullptr;
     bs_engine* lane_load = nullptr;
@@ -73,6 +76,10 @@ static void io_run(IoJob& j)
 {
     constexpr size_t kPiece = 64u << 20;
     if (j.after) cudaEventSynchronize(j.after);  // the stream has landed in the host buffer
+    if (j.spill && j.save != nullptr && j.save->h_result->status != BS_OK) {  // the save failed: the buffer holds no stream
+        j.status = j.save->h_result->status;
+        return;
+    }
     const auto t0 = std::chrono::steady_clock::now();
     const int fd = j.spill ? open(j.path.c_str(), O_WRONLY | O_CREAT | O_TRUNC, 0644) : open(j.path.c_str(), O_RDONLY);
     if (fd < 0) { j.status = BS_ERR_IO; return; }
@@ -266,6 +273,8 @@ static int queue_save_impl(bs_queue* q, uint64_t key, const bs_set_desc* set, co
     if ((rc = bs_engine_offload_impl(q->lane_save, set, lset, total_bytes, h_pinned, h_capacity, producer, &t))) return rc;
     total_bytes = t->bytes;  // the size prediction, if the call made it
     bs_queue::Entry& en = q->keys[key];
+    en.io.reset();  // the key's storage job (waited for above) described the stream this save replaces
+    en.fill_pending = false;
     queue_retire(q, en.save);
     en.save = t;
     en.h = h_pinned;
@@ -321,6 +330,8 @@ int bs_queue_adopt(bs_queue* q, uint64_t key, const void* h_pinned, uint64_t nby
         queue_retire(q, it->second.load);
     }
     bs_queue::Entry& en = q->keys[key];
+    en.io.reset();
+    en.fill_pending = false;
     en.h = h_pinned;
     en.nbytes = nbytes;
     en.adopted = true;
@@ -339,12 +350,13 @@ static int queue_load_impl(bs_queue* q, uint64_t key, bs_set_desc* out, bs_layer
     auto it = q->keys.find(key);
     if (it == q->keys.end()) return BS_ERR_ARG;
     bs_queue::Entry& en = it->second;
-    if (en.io && !en.io->spill) {  // the stream is still being read from its file: the host waits ("fetching", L132)
+    if (en.fill_pending) {  // the stream is still being read from its file: the host waits ("fetching", L132)
         io_wait(q, en.io);
-        if (en.io->status != BS_OK) return BS_ERR_IO;
+        if (en.io->status != BS_OK) return BS_ERR_IO;  // stays pending: every load fails until a save / adopt / fill replaces it
         uint32_t version = 0;
         memcpy(&version, (const unsigned char*)en.h + 8, 4);
-        en.layered = version == 2u;
+        en.layered = version == 2u;  // settled once, from the complete file
+        en.fill_pending = false;
     }
     if (en.layered != (lout != nullptr)) return BS_ERR_ARG;  // the key holds a stream of the other wire format
     int rc;
@@ -432,6 +444,13 @@ int bs_queue_spill(bs_queue* q, uint64_t key, const char* path)
     if (it == q->keys.end()) return BS_ERR_ARG;
     bs_queue::Entry& en = it->second;
     io_wait(q, en.io);
+    if (en.fill_pending) {  // a stream that never arrived from its file cannot be written out again
+        if (en.io->status != BS_OK) return BS_ERR_IO;
+        uint32_t version = 0;
+        memcpy(&version, (const unsigned char*)en.h + 8, 4);
+        en.layered = version == 2u;
+        en.fill_pending = false;
+    }
     auto j = std::make_shared<IoJob>();
     j->spill = true;
     j->path = path;
@@ -440,6 +459,7 @@ int bs_queue_spill(bs_queue* q, uint64_t key, const char* path)
     if (en.save) {  // behind the save's last DMA (the save lane is in order)
         CK(cudaEventCreateWithFlags(&j->after, cudaEventDisableTiming));
         CK(cudaEventRecord(j->after, q->lane_save->cstream));
+        j->save = en.save;
     }
     int rc = io_submit(q, j);
     if (rc) return rc;
@@ -474,6 +494,7 @@ int bs_queue_fill(bs_queue* q, uint64_t key, const char* path, void* h_pinned, u
     en.adopted = true;
     en.layered = false;  // settled from the version word once the file is in
     en.io = j;
+    en.fill_pending = true;
     queue_account_host(q);
     return BS_OK;
 }

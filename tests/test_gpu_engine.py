@@ -103,6 +103,93 @@ def test_prefetch_rejects_corrupt_streams():
     eng.destroy()
 
 
+def test_prefetch_rejects_a_payload_without_blocks():
+    """T = 0, B = 0, payload_bytes != 0 through the engine (the LDG variant used to index the block table at B - 1)."""
+    import struct
+    P = 65536 + 32
+    bad = np.zeros(128 + P, np.uint8)
+    bad[:64] = np.frombuffer(b"BSPARSE1" + struct.pack("<IIIIIIQQQQ", 1, 0x01020304, 0, 2, 3, 16, 0, 0, 128, P), np.uint8)
+    assert oracle.validate_stream(bad) == oracle.ERR_CORRUPT
+    host = pinned(len(bad), 0)
+    host.numpy()[:] = bad
+    for opts in (None, dict(variant=bs.VARIANT_LDG)):
+        eng = bs.Engine(4, 64, len(bad), chunk_bytes=65536, opts=opts)
+        pool = torch.full((4096,), 0xEE, dtype=torch.uint8, device=DEV)
+        out = bs.DeviceSet.empty(4, 64, DEV, fill=0xAB)
+        t = eng.prefetch_async(host.data_ptr(), len(bad), out.desc, pool.data_ptr(), 4096)
+        assert t.wait()["status"] == bs.ERR_CORRUPT
+        torch.cuda.synchronize()
+        assert (pool == 0xEE).all() and (out.qn == 0xAB).all()
+        eng.destroy()
+
+
+def test_engine_checks_what_the_direct_calls_check():
+    """A descriptor or a launch shape bs_serialize would refuse is refused by the engine too, at once — not saved as a
+    stream no loader accepts, not a device fault."""
+    bset = W.make_config("1")
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    host = pinned(1 << 20, 0xCD)
+    with pytest.raises(bs.BsError) as e:      # tile_bytes not a multiple of 16 KiB
+        bs.Engine(4, 64, 1 << 20, chunk_bytes=65536, opts=dict(variant=bs.VARIANT_TMA, tile_bytes=8192, stages=3, warps=1))
+    assert e.value.code == bs.ERR_ARG
+    eng = bs.Engine(4, 64, 1 << 20, chunk_bytes=65536)
+    cs = bs.current_stream()
+    d = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, up.addr, DEV, dtype=7)            # unknown element type
+    with pytest.raises(bs.BsError) as e:
+        eng.offload_async(d.desc, 0, host.data_ptr(), host.numel(), cs)
+    assert e.value.code == bs.ERR_UNSUPPORTED
+    with pytest.raises(bs.BsError) as e:
+        eng.offload_packages_async(d.desc, 0, 16384, 1, host.data_ptr(), 64 + 16384, 8, None, cs)
+    assert e.value.code == bs.ERR_UNSUPPORTED
+    nul = bs.make_desc(bset.n_tensors, bset.n_blocks, up.dset.tensors.data_ptr(), 0, up.dset.dim.data_ptr(),
+                       up.dset.addr.data_ptr())                                               # NULL label array
+    with pytest.raises(bs.BsError) as e:
+        eng.offload_async(nul, len(want), host.data_ptr(), host.numel(), cs)
+    assert e.value.code == bs.ERR_ARG
+    host.numpy()[:len(want)] = want
+    out = bs.DeviceSet.empty(4, 64, DEV, fill=0xAB)
+    bad_out = bs.make_desc(4, 64, out.tensors.data_ptr(), out.qn.data_ptr(), 0, out.addr.data_ptr())
+    with pytest.raises(bs.BsError) as e:
+        eng.prefetch_async(host.data_ptr(), len(want), bad_out, 0, 0)
+    assert e.value.code == bs.ERR_ARG
+    assert (host.numpy()[len(want):] == 0xCD).all()
+    eng.destroy()
+
+
+def test_a_failed_offload_leaves_no_valid_header_on_the_host():
+    """On a deferred error the pack kernels write nothing but the DMA of every chunk still runs: the staging buffers hold
+    the stream of the call before.  The engine has the 64 bytes of the fixed header blanked, so the host never sees a
+    stale stream as valid (chunks and packages)."""
+    bset = W.make_config("1")
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    total = len(want)
+    eng = bs.Engine(4, 64, 1 << 20, chunk_bytes=65536)
+    cs = bs.current_stream()
+    host = pinned(1 << 20, 0xCD)
+    assert eng.offload_async(up.dset.desc, total, host.data_ptr(), host.numel(), cs).wait()["status"] == bs.OK
+    assert bs.stream_info(host.numpy()[:64].tobytes())["total_bytes"] == total
+    host.fill_(0xCD)
+    t = eng.offload_async(up.dset.desc, total + 16, host.data_ptr(), host.numel(), cs)      # wrong size prediction
+    assert t.wait()["status"] == bs.ERR_ARG
+    with pytest.raises(bs.BsError):
+        bs.stream_info(host.numpy()[:64].tobytes())
+    assert (host.numpy()[:64] == 0).all()
+    # packages: every slot header of the failed call is blank
+    cap = 16384
+    n = bs.package_count(bs.header_bytes(bset.n_tensors, bset.n_blocks), total, cap)
+    slots = pinned((n + 1) * (64 + cap), 0xCD)      # one spare slot: the wrong size below may cut one package more
+    assert eng.offload_packages_async(up.dset.desc, total, cap, 5, slots.data_ptr(), 64 + cap, n, None, cs).wait()["status"] == bs.OK
+    assert bytes(slots.numpy()[:8]) == b"BSPKG001"
+    slots.fill_(0xCD)
+    t = eng.offload_packages_async(up.dset.desc, total + 16, cap, 5, slots.data_ptr(), 64 + cap, n + 1, None, cs)
+    assert t.wait()["status"] == bs.ERR_ARG
+    sl = slots.numpy().reshape(n + 1, 64 + cap)
+    assert not any(bytes(sl[k, :8]) == b"BSPKG001" for k in range(n + 1))
+    eng.destroy()
+
+
 def test_offload_overlaps_a_busy_compute_stream():
     """The producer stream is not blocked and the result is the same stream while a stand-in contraction runs."""
     from workloads.device import StandInContraction

@@ -21,11 +21,18 @@ VARIANTS = [dict(variant=bs.VARIANT_LDG, tile_bytes=16384), dict(variant=bs.VARI
             dict(variant=bs.VARIANT_TMA, tile_bytes=65536), dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=1),
             dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=8, warps=1),
             dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=4),
-            dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=3, warps=2)]
+            dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=3, warps=2),
+            # the shape the pack preset switches to on sets of half a GB and more (one ring of 3 x 48 KiB)
+            dict(variant=bs.VARIANT_TMA, tile_bytes=49152, stages=3, warps=1),
+            # one fused launch (size / offset pass + movement) against separate launches; default shape and a wide one
+            dict(variant=bs.VARIANT_TMA, fuse=1), dict(variant=bs.VARIANT_TMA, fuse=2),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=4, fuse=2),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=4, warps=1, fuse=2)]
 
 
 def _vid(o):
-    return f"v{o['variant']}-t{o.get('tile_bytes', 0)}-c{o.get('ctas_per_sm', 0)}-s{o.get('stages', 0)}-w{o.get('warps', 0)}"
+    return (f"v{o['variant']}-t{o.get('tile_bytes', 0)}-c{o.get('ctas_per_sm', 0)}-s{o.get('stages', 0)}-w{o.get('warps', 0)}"
+            f"-f{o.get('fuse', 0)}")
 
 
 def small_sets():
@@ -297,6 +304,93 @@ def test_P10_corrupt_headers_are_rejected_and_nothing_is_written():
     for n in (len(want) - 16, 48):
         out, pool, res = gpu_deserialize(st, n, bset.n_tensors, bset.n_blocks, need)
         assert res["status"] == bs.ERR_CORRUPT and (pool == 0xEE).all()
+
+
+def test_a_payload_without_blocks_is_corrupt():
+    """T = 0, B = 0, payload_bytes != 0: no block record carries the offset link check, so the totals must catch it
+    ("final sum == payload_bytes").  Oracle first, then every kernel variant and both launch forms."""
+    import struct
+    for P in (16, 65536 + 32):
+        bad = np.zeros(128 + P, np.uint8)
+        bad[:64] = np.frombuffer(b"BSPARSE1" + struct.pack("<IIIIIIQQQQ", 1, 0x01020304, 0, 2, 3, 16, 0, 0, 128, P), np.uint8)
+        assert oracle.validate_stream(bad) == oracle.ERR_CORRUPT
+        for opts in (None, dict(variant=bs.VARIANT_TMA, fuse=1), dict(variant=bs.VARIANT_TMA, fuse=2),
+                     dict(variant=bs.VARIANT_LDG), dict(variant=bs.VARIANT_LDG, tile_bytes=65536)):
+            out, pool, res = gpu_deserialize(torch.from_numpy(bad).to(DEV), len(bad), 4, 64, 4096, opts=opts)
+            assert res["status"] == bs.ERR_CORRUPT, (P, opts, res)
+            assert (pool == 0xEE).all()
+            for arr in (out.tensors, out.qn, out.dim, out.addr):
+                assert (arr == 0xAB).all()
+
+
+@pytest.mark.parametrize("junk", ["ones", "random", "previous-call"])
+def test_the_workspace_needs_no_clearing(junk):
+    """The size / offset pass synchronises on epoch-tagged words only (bs_scan_phase.cuh): whatever the workspace holds —
+    all ones, noise, the state of an earlier call on a larger set — the stream is the oracle's.  Both launch forms, sets of
+    one work item (replicated pass), of a few, and deserialize."""
+    sets = [W.make_config("1"), W.make_config("2"),
+            W.make_set("tiny-ops+site", 11, D=48, S=10, M=2, N0=2, n_ops=20, n_site=2, dims="multinomial")]
+    ups = [Uploaded(b) for b in sets]
+    wants = [oracle_stream(b, u.host_pool, u.host_offs)[0] for b, u in zip(sets, ups)]
+    cap_t, cap_b = max(b.n_tensors for b in sets), max(b.n_blocks for b in sets)
+    cap = max(len(w) for w in wants) + 4096
+    ws = bs.Workspace(cap_t, cap_b, cap, DEV)
+    rng = torch.Generator(device=DEV).manual_seed(5)
+    cs = bs.current_stream()
+    for rnd in range(3):
+        for fuse in (2, 1, 0):
+            for bset, up, want in zip(sets, ups, wants):
+                if junk == "ones":
+                    ws.buf.fill_(0xFF)
+                elif junk == "random":
+                    ws.buf.copy_(torch.randint(0, 256, (ws.nbytes,), dtype=torch.uint8, device=DEV, generator=rng))
+                total = len(want)
+                out = torch.full((cap,), 0xCD, dtype=torch.uint8, device=DEV)
+                opts = dict(variant=bs.VARIANT_TMA, fuse=fuse)
+                bs.serialize(up.dset.desc, out.data_ptr(), cap, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
+                res = ws.read_result()
+                assert res["status"] == bs.OK and res["total_bytes"] == total, (junk, fuse, bset.name, res)
+                got = out.cpu().numpy()
+                assert (got[:total] == want).all() and (got[total:] == 0xCD).all(), (junk, fuse, bset.name)
+                need = oracle.pool_bytes(want)
+                dst = bs.DeviceSet.empty(cap_t, cap_b, DEV, fill=0xAB)
+                pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+                bs.deserialize(out.data_ptr(), total, dst.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                               ws.result_ptr, opts, cs)
+                res = ws.read_result()
+                assert res["status"] == bs.OK and res["n_blocks"] == bset.n_blocks, (junk, fuse, bset.name, res)
+                assert (pool.cpu().numpy() == oracle.deserialize(want)["pool"][:need]).all()
+
+
+def test_fused_calls_on_two_streams_at_once():
+    """bs.h: calls are re-entrant.  Two streams each run fused serialize + deserialize calls back to back on their own
+    workspaces; the kernels are persistent (one CTA per SM each) and may be co-resident only in part — items are claimed
+    from a ticket, so a resident CTA never waits for one that is not (bs_scan_phase.cuh).  Results: the oracle's."""
+    bset = W.make_config("2")
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    total, need = len(want), oracle.pool_bytes(want)
+    ref_pool = oracle.deserialize(want)["pool"][:need]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    lanes = []
+    for s in streams:
+        lanes.append(dict(ws=bs.Workspace(bset.n_tensors, bset.n_blocks, total, DEV),
+                          out=torch.full((total,), 0xCD, dtype=torch.uint8, device=DEV),
+                          dst=bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB),
+                          pool=torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)))
+    torch.cuda.synchronize()
+    opts = dict(variant=bs.VARIANT_TMA, fuse=2)
+    for it in range(20):
+        for s, ln in zip(streams, lanes):
+            bs.serialize(up.dset.desc, ln["out"].data_ptr(), total, ln["ws"].ptr, ln["ws"].nbytes, ln["ws"].result_ptr, opts,
+                         s.cuda_stream)
+            bs.deserialize(ln["out"].data_ptr(), total, ln["dst"].desc, ln["pool"].data_ptr(), need, bs.LAYOUT_POOL, ln["ws"].ptr,
+                           ln["ws"].nbytes, ln["ws"].result_ptr, opts, s.cuda_stream)
+    torch.cuda.synchronize()
+    for ln in lanes:
+        assert ln["ws"].read_result()["status"] == bs.OK
+        assert (ln["out"].cpu().numpy() == want).all()
+        assert (ln["pool"].cpu().numpy() == ref_pool).all()
 
 
 def test_deserialize_capacity_errors():

@@ -273,3 +273,63 @@ def test_storage_tier_spill_forget_fill_load(tmp_path):
     q.spill(9, str(tmp_path / "no_such_dir" / "x.bs"))
     assert q.io_wait(9)["status"] == bs.ERR_IO
     q.destroy()
+
+
+def test_a_save_over_a_filled_key_forgets_the_fill(tmp_path):
+    """Per-key program order across the storage tier: fill -> save -> load returns the SAVED object, also when the fill
+    failed or held the other wire format; and a spill behind a failed save fails instead of writing stale bytes."""
+    bset = W.make_config("2", n_ops=26)
+    up = Uploaded(bset)
+    model = oracle.QueueModel()
+    want = model.save(1, bset.tensors, bset.qn, bset.dim, host_addrs(up.host_pool, up.host_offs))
+    total = len(want)
+    q = bs.Queue(bset.n_tensors, bset.n_blocks, total + 4096, chunk_bytes=4 * 65536)
+    cs = bs.current_stream()
+    ref = model.load(1)
+    need = oracle.pool_bytes(want)
+    # (1) a fill that fails (truncated to less than a header's worth of payload ... the read itself fails: a directory)
+    h = pinned(total + 4096)
+    bad_path = str(tmp_path / "short.bs")
+    open(bad_path, "wb").write(want.tobytes()[:4096])
+    q.fill(7, bad_path, h.data_ptr(), h.numel())
+    ld = Loaded(bset, need)
+    with pytest.raises(bs.BsError):                       # 4096 bytes of a longer stream: refused
+        q.load(7, ld.out.desc, ld.pool.data_ptr(), ld.need, bs.LAYOUT_POOL, cs)
+    q.save(7, up.dset.desc, total, h.data_ptr(), h.numel(), cs)    # the key is saved over: the fill no longer counts
+    q.load(7, ld.out.desc, ld.pool.data_ptr(), ld.need, bs.LAYOUT_POOL, cs)
+    assert q.wait(7)["status"] == bs.OK
+    torch.cuda.synchronize()
+    assert (h.numpy()[:total] == want).all()
+    assert (ld.pool.cpu().numpy()[:need] == ref["pool"][:need]).all()
+    # (2) fill (v1 file) -> save_layered -> load_layered: the key holds the layered stream now
+    from oracle import v2
+    lv = W.layered_view(bset)
+    counts = (len(lv["structs"]), lv["dim"].shape[0], bset.n_tensors, bset.n_blocks)
+    lset = bs.DeviceLayeredSet.from_host(lv["structs"], lv["layers"], lv["qn"], lv["dim"], up.addr, DEV)
+    want2 = v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], host_addrs(up.host_pool, up.host_offs))
+    ql = bs.Queue(max(bset.n_tensors, counts[0]), bset.n_blocks, total + 4096, chunk_bytes=4 * 65536)
+    good_path = str(tmp_path / "v1.bs")
+    open(good_path, "wb").write(want.tobytes())
+    h2 = pinned(total + 4096)
+    ql.fill(3, good_path, h2.data_ptr(), h2.numel())
+    ql.save_layered(3, lset.desc, len(want2), h2.data_ptr(), h2.numel(), cs)
+    lout = bs.DeviceLayeredSet.empty(*counts, DEV, fill=0xAB)
+    lpool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    ql.load_layered(3, lout.desc, lpool.data_ptr(), need, bs.LAYOUT_POOL, cs)
+    assert ql.wait(3)["status"] == bs.OK
+    torch.cuda.synchronize()
+    assert (h2.numpy()[:len(want2)] == want2).all()
+    assert (lpool.cpu().numpy()[:need] == ref["pool"][:need]).all()
+    ql.destroy()
+    # (3) a save that fails on the device (wrong size prediction): its spill must fail too, and write no file contents
+    h3 = pinned(total + 4096)
+    q.save(8, up.dset.desc, total, h3.data_ptr(), h3.numel(), cs)          # a good stream first, so the staging buffers hold one
+    assert q.wait(8)["status"] == bs.OK
+    q.save(8, up.dset.desc, total + 16, h3.data_ptr(), h3.numel(), cs)
+    out_path = str(tmp_path / "failed.bs")
+    q.spill(8, out_path)
+    assert q.io_wait(8)["status"] == bs.ERR_ARG
+    assert q.wait(8)["status"] == bs.ERR_ARG
+    import os
+    assert not os.path.exists(out_path) or os.path.getsize(out_path) == 0
+    q.destroy()
