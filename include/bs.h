@@ -63,14 +63,14 @@ enum {
     BS_ERR_ARG = -1,         /* NULL / misaligned pointer, bad descriptor partition, size overflow */
     BS_ERR_CAPACITY = -2,    /* stream / pool / workspace / descriptor arrays too small */
     BS_ERR_CORRUPT = -3,     /* header validation failed; nothing was written */
-    BS_ERR_UNSUPPORTED = -4, /* rank not in {2,3}, unknown dtype (layered sets: dtype != f64), n_qn != 2 */
+    BS_ERR_UNSUPPORTED = -4, /* rank not in {2,3}, unknown dtype, n_qn != 2 */
     BS_ERR_CUDA = -5,        /* a CUDA runtime call failed; see bs_last_cuda_error() */
     BS_ERR_IO = -6           /* the storage tier of a bs_queue: open / read / write of a file failed (errno is the C library's) */
 };
 
 /* Element type of every block of a set (bs_set_desc.dtype; the header's dtype word).  The path does no arithmetic on the
- * values: the type only fixes the element size e, nbytes = e * prod(dim).  Wire format v2 (layered
- * sets) is BS_F64 only. */
+ * values: the type only fixes the element size e, nbytes = e * prod(dim).  Both wire formats carry
+ * every type (a stream holds blocks of ONE type). */
 enum { BS_F64 = 0 /* e = 8 */, BS_F32 = 1 /* e = 4 */, BS_C64 = 2 /* e = 8 */, BS_C128 = 3 /* e = 16 */ };
 
 /* bs_deserialize / bs_prefetch_async destination layout */
@@ -206,13 +206,13 @@ int bs_deserialize_range(const void *d_src, uint64_t lo, uint64_t hi, const void
  *
  *   stream      := fixed_header(64) | struct_rec[C](32) | layer_rec[T](16) | block_rec[Bs](48) | zeros to a multiple
  *                  of 128 | payload(P)
- *   fixed_header: char magic[8]="BSPARSE1"; u32 version=2; u32 endian_tag=0x01020304; u32 dtype=0; u32 n_qn=2;
- *                 u32 max_rank=3; u32 align=16; u32 n_structs=C; u32 n_struct_blocks=Bs; u64 n_layers=T;
+ *   fixed_header: char magic[8]="BSPARSE1"; u32 version=2; u32 endian_tag=0x01020304; u32 dtype (as v1: element size e);
+ *                 u32 n_qn=2; u32 max_rank=3; u32 align=16; u32 n_structs=C; u32 n_struct_blocks=Bs; u64 n_layers=T;
  *                 u64 header_bytes; u64 payload_bytes
- *   struct_rec  : bs_struct_rec, byte for byte (layer_bytes = sum over its blocks of align16(8*prod(dim)))
+ *   struct_rec  : bs_struct_rec, byte for byte (layer_bytes = sum over its blocks of align16(e*prod(dim)))
  *   layer_rec   : bs_layer_rec, byte for byte  (offset = sum over earlier layers of their structure's layer_bytes)
  *   block_rec   : i32 qn[3][2]; u32 dim[3]; u32 structure; u64 offset   (offset relative to the start of a layer =
- *                 sum over earlier blocks of the same structure of align16(8*prod(dim)))
+ *                 sum over earlier blocks of the same structure of align16(e*prod(dim)))
  *   payload     : layer t at payload + offset_t, block j of its structure at + offset_j, zero padded to 16
  *   header_bytes = align128(64 + 32*C + 16*T + 48*Bs)
  */
@@ -238,7 +238,7 @@ typedef struct bs_layered_desc {
     uint32_t n_struct_blocks; /* Bs.  For outputs: CAPACITY of qn / dim */
     uint32_t n_layers;        /* T.   For outputs: CAPACITY of layers[] */
     uint32_t n_qn;            /* 2 */
-    uint32_t dtype;           /* BS_F64 */
+    uint32_t dtype;           /* BS_F64, BS_F32, BS_C64 or BS_C128 (for outputs: 0; the stream's type comes back in bs_result) */
     uint32_t reserved;        /* 0 */
     uint64_t n_addr;          /* entries of addr[]: must be >= B (serialize: B is checked on the device) */
     bs_struct_rec *structs;   /* [C]         */
@@ -250,6 +250,7 @@ typedef struct bs_layered_desc {
 
 typedef struct bs_layered_stream_info_t {
     uint64_t n_structs, n_struct_blocks, n_layers, header_bytes, payload_bytes, total_bytes;
+    uint64_t dtype; /* BS_F64 .. BS_C128 */
 } bs_layered_stream_info_t;
 
 /* align128(64 + 32*C + 16*T + 48*Bs) */
@@ -260,7 +261,7 @@ uint64_t bs_layered_workspace_bytes(uint32_t n_structs, uint32_t n_struct_blocks
 int bs_layered_stream_info(const void *h_first_64_bytes, bs_layered_stream_info_t *out); /* HOST memory */
 
 /* As bs_serialized_size / bs_serialize / bs_serialize_range / bs_deserialize, for wire format v2.  bs_result:
- * n_tensors = T, n_blocks = B, reserved[0] = C, reserved[1] = Bs.  Deferred statuses as for v1; additionally
+ * n_tensors = T, n_blocks = B, reserved[0] = C, reserved[1] = Bs, reserved[2] = dtype.  Deferred statuses as for v1; additionally
  * BS_ERR_ARG for a layer naming a structure >= C and BS_ERR_CAPACITY for n_addr < B.  bs_layered_deserialize writes
  * structs / layers (wire records), qn / dim (BS_LAYOUT_POOL; with BS_SCATTER_TO_ADDR dim [Bs][3] and addr [B] are
  * INPUTS) and addr. */

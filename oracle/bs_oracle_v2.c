@@ -15,20 +15,30 @@
  * Wire format v2 (little-endian, no implicit padding):
  *   stream     := fixed_header(64) | struct_rec[C](32) | layer_rec[T](16) | block_rec[Bs](48)
  *                 | zeros to a multiple of 128 | payload(P)
- *   fixed_header: char magic[8]="BSPARSE1"; u32 version=2; u32 endian_tag=0x01020304; u32 dtype=0;
+ *   fixed_header: char magic[8]="BSPARSE1"; u32 version=2; u32 endian_tag=0x01020304; u32 dtype (0 f64,
+ *                 1 f32, 2 c64, 3 c128: element size e = 8, 4, 8, 16 — reading E-2 below);
  *                 u32 n_qn=2; u32 max_rank=3; u32 align=16; u32 n_structs=C; u32 n_struct_blocks=Bs;
  *                 u64 n_layers=T; u64 header_bytes; u64 payload_bytes
  *   struct_rec  : u32 rank; u32 first_block; u32 n_blocks; i32 dq[2]; i8 sign[4]; u64 layer_bytes
  *   layer_rec   : u32 structure; u32 tag; u64 offset
  *   block_rec   : i32 qn[3][2]; u32 dim[3]; u32 structure; u64 offset     (offset relative to the layer)
  *   payload     : layer t at payload + offset_t; inside it block j of its structure at + offset_j: the
- *                 8*prod(dim_j) raw bytes of that layer's block, then zeros to the next multiple of 16
- *     offset_j      = sum over earlier blocks j' of the SAME structure of align16(8*prod(dim_j'))
- *     layer_bytes_s = sum over the blocks of structure s of align16(8*prod(dim))
+ *                 e*prod(dim_j) raw bytes of that layer's block, then zeros to the next multiple of 16
+ *     offset_j      = sum over earlier blocks j' of the SAME structure of align16(e*prod(dim_j'))
+ *     layer_bytes_s = sum over the blocks of structure s of align16(e*prod(dim))
  *     offset_t      = sum_{t' < t} layer_bytes[structure[t']]                 (descriptor order)
  *     header_bytes  = align128(64 + 32*C + 16*T + 48*Bs)
  * Block addresses: addr[] lists the blocks layer by layer (descriptor order), inside a layer in the
  * order of its structure's block table; it has B = sum_t n_blocks[structure[t]] entries.
+ *
+ * Reading E-2 (round 2; SURVEY §8(f) NEXT-4 "complex128 / fp32 dtypes", applied to layered sets; the paper's Fig 4(a)
+ * layers (L75) are value layers of one structure whatever the element type): exactly as reading E-1 did for wire
+ * format v1, the header's dtype word selects the element size e and nothing else changes —
+ * nbytes = e*prod(dim), stored = align16(nbytes) (an f32 block carries 0, 4, 8 or 12 zero pad bytes), pool slots stay
+ * align256(nbytes).  Every function below that computed 8*prod(dim) computes e*prod(dim); dtype = 0 gives the bytes
+ * round 1 gave.  Pins of the element types (tests/test_oracle_v2.py): G6 hand-typed f32 golden stream; payload ==
+ * the payload of the independently written numpy oracle bs_oracle_dtype.py (v1) on the expanded set for every type;
+ * the c64 stream == the f64 stream but for the dtype word; offsets against numpy.cumsum of e-sized blocks.
  *
  * Relation to v1 (a pin, tests/test_oracle_v2.py): expanding every layer into a v1 tensor with its
  * structure's records gives a v1 set whose PAYLOAD is byte-identical to the v2 payload.
@@ -104,12 +114,15 @@ static int check_desc(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st
     return ORC_OK;
 }
 
-static int block_bytes(const uint32_t *dim3, uint64_t *nbytes)
+/* element size of a dtype word (reading E-2): f64 8, f32 4, c64 8, c128 16 */
+static uint64_t elem_size(uint32_t dtype) { return dtype == 1u ? 4u : (dtype == 3u ? 16u : 8u); }
+
+static int block_bytes(const uint32_t *dim3, uint32_t dtype, uint64_t *nbytes)
 {
     uint64_t d0 = dim3[0], d1 = dim3[1], d2 = dim3[2];
     uint64_t n01 = d0 * d1;
-    if (d2 != 0 && n01 > (UINT64_MAX / 8u) / d2) return ORC_ERR_ARG;
-    *nbytes = 8u * n01 * d2;
+    if (d2 != 0 && n01 > (UINT64_MAX / 16u) / d2) return ORC_ERR_ARG;
+    *nbytes = elem_size(dtype) * n01 * d2;
     return ORC_OK;
 }
 
@@ -117,16 +130,17 @@ static int block_bytes(const uint32_t *dim3, uint64_t *nbytes)
  * rel_offset[j] (j over the structure block table), layer_bytes[s], layer_offset[t], n_addr = B, P.
  * Any output pointer may be NULL. */
 int orc2_plan(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, const orc2_layer *ly,
-              const uint32_t *dim /*[Bs][3]*/, uint64_t *rel_offset, uint64_t *layer_bytes,
+              const uint32_t *dim /*[Bs][3]*/, uint32_t dtype, uint64_t *rel_offset, uint64_t *layer_bytes,
               uint64_t *layer_offset, uint64_t *n_addr, uint64_t *payload_bytes)
 {
     int rc = check_desc(C, Bs, T, st, ly);
     if (rc) return rc;
+    if (dtype > 3u) return ORC_ERR_UNSUPPORTED;
     for (uint64_t s = 0; s < C; ++s) {
         uint64_t run = 0;
         for (uint64_t j = st[s].first_block; j < (uint64_t)st[s].first_block + st[s].n_blocks; ++j) {
             uint64_t nb = 0;
-            rc = block_bytes(dim + 3 * j, &nb);
+            rc = block_bytes(dim + 3 * j, dtype, &nb);
             if (rc) return rc;
             if (rel_offset) rel_offset[j] = run;
             run += up(nb, V2_BLOCK_ALIGN);
@@ -139,7 +153,7 @@ int orc2_plan(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, const 
         uint64_t lb = 0;
         for (uint64_t j = s->first_block; j < (uint64_t)s->first_block + s->n_blocks; ++j) {
             uint64_t nb = 0;
-            block_bytes(dim + 3 * j, &nb);
+            block_bytes(dim + 3 * j, dtype, &nb);
             lb += up(nb, V2_BLOCK_ALIGN);
         }
         if (layer_offset) layer_offset[t] = run;
@@ -152,10 +166,10 @@ int orc2_plan(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, const 
 }
 
 int orc2_serialized_size(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, const orc2_layer *ly,
-                         const uint32_t *dim, uint64_t *header_bytes, uint64_t *total_bytes)
+                         const uint32_t *dim, uint32_t dtype, uint64_t *header_bytes, uint64_t *total_bytes)
 {
     uint64_t P;
-    int rc = orc2_plan(C, Bs, T, st, ly, dim, NULL, NULL, NULL, NULL, &P);
+    int rc = orc2_plan(C, Bs, T, st, ly, dim, dtype, NULL, NULL, NULL, NULL, &P);
     if (rc) return rc;
     *header_bytes = orc2_header_bytes(C, T, Bs);
     *total_bytes = *header_bytes + P;
@@ -165,11 +179,11 @@ int orc2_serialized_size(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct 
 /* ---- serialize: header, then layer by layer, block by block ---------------------------------------- */
 int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, const orc2_layer *ly,
                    const int32_t *qn /*[Bs][3][2]*/, const uint32_t *dim /*[Bs][3]*/,
-                   const uint64_t *addr /*[B] host addresses, layer-major*/, unsigned char *out,
+                   const uint64_t *addr /*[B] host addresses, layer-major*/, uint32_t dtype, unsigned char *out,
                    uint64_t capacity, uint64_t *written)
 {
     uint64_t hb, total;
-    int rc = orc2_serialized_size(C, Bs, T, st, ly, dim, &hb, &total);
+    int rc = orc2_serialized_size(C, Bs, T, st, ly, dim, dtype, &hb, &total);
     if (rc) return rc;
     *written = total;
     if (capacity < total) return ORC_ERR_CAPACITY;
@@ -178,7 +192,7 @@ int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, c
     memcpy(p, "BSPARSE1", 8);
     w32(p + 8, 2u);               /* version */
     w32(p + 12, 0x01020304u);     /* endian_tag */
-    w32(p + 16, 0u);              /* dtype f64 */
+    w32(p + 16, dtype);           /* dtype (reading E-2) */
     w32(p + 20, 2u);              /* n_qn */
     w32(p + 24, 3u);              /* max_rank */
     w32(p + 28, 16u);             /* align */
@@ -193,7 +207,7 @@ int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, c
         uint64_t lb = 0;
         for (uint64_t j = st[s].first_block; j < (uint64_t)st[s].first_block + st[s].n_blocks; ++j) {
             uint64_t nb = 0;
-            block_bytes(dim + 3 * j, &nb);
+            block_bytes(dim + 3 * j, dtype, &nb);
             lb += up(nb, V2_BLOCK_ALIGN);
         }
         w32(p + 0, st[s].rank);
@@ -215,7 +229,7 @@ int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, c
             const orc2_struct *s = &st[ly[t].structure];
             for (uint64_t j = s->first_block; j < (uint64_t)s->first_block + s->n_blocks; ++j) {
                 uint64_t nb = 0;
-                block_bytes(dim + 3 * j, &nb);
+                block_bytes(dim + 3 * j, dtype, &nb);
                 run += up(nb, V2_BLOCK_ALIGN);
             }
         }
@@ -224,7 +238,7 @@ int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, c
         uint64_t run = 0;
         for (uint64_t j = st[s].first_block; j < (uint64_t)st[s].first_block + st[s].n_blocks; ++j) {
             uint64_t nb = 0;                                  /* (initialised for gcc, as below) */
-            block_bytes(dim + 3 * j, &nb);
+            block_bytes(dim + 3 * j, dtype, &nb);
             memcpy(p, qn + 6 * j, 24);
             w32(p + 24, dim[3 * j + 0]);
             w32(p + 28, dim[3 * j + 1]);
@@ -243,7 +257,7 @@ int orc2_serialize(uint64_t C, uint64_t Bs, uint64_t T, const orc2_struct *st, c
         const orc2_struct *s = &st[ly[t].structure];
         for (uint64_t j = s->first_block; j < (uint64_t)s->first_block + s->n_blocks; ++j, ++a) {
             uint64_t nb = 0;                                  /* (initialised for gcc; block_bytes always sets it here: the plan passed) */
-            block_bytes(dim + 3 * j, &nb);
+            block_bytes(dim + 3 * j, dtype, &nb);
             uint64_t sb = up(nb, V2_BLOCK_ALIGN);
             memcpy(q, (const void *)(uintptr_t)addr[a], (size_t)nb);
             memset(q + nb, 0, (size_t)(sb - nb));
@@ -262,7 +276,7 @@ int orc2_stream_info(const unsigned char *s, uint64_t n, uint64_t *C, uint64_t *
     if (memcmp(s, "BSPARSE1", 8) != 0) return ORC_ERR_CORRUPT;
     if (r32(s + 8) != 2u) return ORC_ERR_CORRUPT;
     if (r32(s + 12) != 0x01020304u) return ORC_ERR_CORRUPT;
-    if (r32(s + 16) != 0u) return ORC_ERR_CORRUPT;
+    if (r32(s + 16) > 3u) return ORC_ERR_CORRUPT;               /* dtype: one of the four element types */
     if (r32(s + 20) != 2u) return ORC_ERR_CORRUPT;
     if (r32(s + 24) != 3u) return ORC_ERR_CORRUPT;
     if (r32(s + 28) != 16u) return ORC_ERR_CORRUPT;
@@ -273,6 +287,16 @@ int orc2_stream_info(const unsigned char *s, uint64_t n, uint64_t *C, uint64_t *
     *payload_bytes = r64(s + 56);
     if (*T >= (1ull << 32)) return ORC_ERR_CORRUPT;
     if (*header_bytes != orc2_header_bytes(*C, *T, *Bs)) return ORC_ERR_CORRUPT;
+    return ORC_OK;
+}
+
+/* the element type of a stream whose fixed header orc2_stream_info accepts */
+int orc2_stream_dtype(const unsigned char *s, uint64_t n, uint32_t *dtype)
+{
+    uint64_t C, Bs, T, hb, P;
+    int rc = orc2_stream_info(s, n, &C, &Bs, &T, &hb, &P);
+    if (rc) return rc;
+    *dtype = r32(s + 16);
     return ORC_OK;
 }
 
@@ -287,6 +311,7 @@ int orc2_validate_stream(const unsigned char *s, uint64_t n)
     int rc = orc2_stream_info(s, n, &C, &Bs, &T, &hb, &P);
     if (rc) return rc;
     if (hb > n || hb + P != n) return ORC_ERR_CORRUPT;
+    const uint32_t dtype = r32(s + 16);
     const unsigned char *srec = s + V2_FIXED_HEADER;
     const unsigned char *lrec = srec + V2_STRUCT_REC * C;
     const unsigned char *brec = lrec + V2_LAYER_REC * T;
@@ -307,7 +332,7 @@ int orc2_validate_stream(const unsigned char *s, uint64_t n)
             }
             uint32_t d3[3] = { r32(b + 24), r32(b + 28), r32(b + 32) };
             uint64_t nbytes;
-            if (block_bytes(d3, &nbytes)) return ORC_ERR_CORRUPT;
+            if (block_bytes(d3, dtype, &nbytes)) return ORC_ERR_CORRUPT;
             if (r64(b + 40) != run) return ORC_ERR_CORRUPT;
             uint64_t sb = up(nbytes, V2_BLOCK_ALIGN);
             if (sb < nbytes || run + sb < run) return ORC_ERR_CORRUPT;   /* a structure no layer uses may exceed P */
@@ -336,7 +361,7 @@ int orc2_validate_stream(const unsigned char *s, uint64_t n)
         uint64_t base = hb + r64(r + 8);
         for (uint64_t j = r32(sr + 4); j < (uint64_t)r32(sr + 4) + r32(sr + 8); ++j) {
             const unsigned char *b = brec + V2_BLOCK_REC * j;
-            uint64_t nbytes = 8ull * r32(b + 24) * r32(b + 28) * r32(b + 32);
+            uint64_t nbytes = elem_size(dtype) * r32(b + 24) * r32(b + 28) * r32(b + 32);
             for (uint64_t z = nbytes; z < up(nbytes, V2_BLOCK_ALIGN); ++z)
                 if (s[base + r64(b + 40) + z] != 0) return ORC_ERR_CORRUPT;
         }
@@ -364,7 +389,7 @@ int orc2_counts(const unsigned char *s, uint64_t n, uint64_t *n_addr, uint64_t *
         if (first + nb > Bs) return ORC_ERR_CORRUPT;
         for (uint64_t j = first; j < first + nb; ++j) {
             const unsigned char *b = brec + V2_BLOCK_REC * j;
-            pool += up(8ull * r32(b + 24) * r32(b + 28) * r32(b + 32), V2_POOL_ALIGN);
+            pool += up(elem_size(r32(s + 16)) * r32(b + 24) * r32(b + 28) * r32(b + 32), V2_POOL_ALIGN);
         }
         na += nb;
     }
@@ -413,7 +438,7 @@ int orc2_deserialize(const unsigned char *s, uint64_t n, orc2_struct *structs_ou
         uint64_t base = hb + layers_out[t].offset;
         for (uint64_t j = r32(sr + 4); j < (uint64_t)r32(sr + 4) + r32(sr + 8); ++j, ++a) {
             const unsigned char *b = brec + V2_BLOCK_REC * j;
-            uint64_t nbytes = 8ull * r32(b + 24) * r32(b + 28) * r32(b + 32);
+            uint64_t nbytes = elem_size(r32(s + 16)) * r32(b + 24) * r32(b + 28) * r32(b + 32);
             unsigned char *dst;
             if (flags == 0) {
                 dst = pool + cursor;

@@ -45,10 +45,11 @@ def _L():
         pu64 = C.POINTER(C.c_uint64)
         lib.orc2_header_bytes.restype = u64
         lib.orc2_header_bytes.argtypes = [u64, u64, u64]
-        lib.orc2_plan.argtypes = [u64, u64, u64, vp, vp, vp, vp, vp, vp, pu64, pu64]
-        lib.orc2_serialized_size.argtypes = [u64, u64, u64, vp, vp, vp, pu64, pu64]
-        lib.orc2_serialize.argtypes = [u64, u64, u64, vp, vp, vp, vp, vp, vp, u64, pu64]
+        lib.orc2_plan.argtypes = [u64, u64, u64, vp, vp, vp, u32, vp, vp, vp, pu64, pu64]
+        lib.orc2_serialized_size.argtypes = [u64, u64, u64, vp, vp, vp, u32, pu64, pu64]
+        lib.orc2_serialize.argtypes = [u64, u64, u64, vp, vp, vp, vp, vp, u32, vp, u64, pu64]
         lib.orc2_stream_info.argtypes = [vp, u64, pu64, pu64, pu64, pu64, pu64]
+        lib.orc2_stream_dtype.argtypes = [vp, u64, C.POINTER(u32)]
         lib.orc2_validate_stream.argtypes = [vp, u64]
         lib.orc2_counts.argtypes = [vp, u64, pu64, pu64]
         lib.orc2_deserialize.argtypes = [vp, u64, vp, vp, vp, vp, vp, vp, u64, u32]
@@ -72,42 +73,43 @@ def header_bytes(n_structs: int, n_layers: int, n_struct_blocks: int) -> int:
     return int(_L().orc2_header_bytes(n_structs, n_layers, n_struct_blocks))
 
 
-def plan(structs, layers, dim):
-    """dict(rel_offset[Bs], layer_bytes[C], layer_offset[T], n_addr, payload_bytes)."""
+def plan(structs, layers, dim, dtype: int = 0):
+    """dict(rel_offset[Bs], layer_bytes[C], layer_offset[T], n_addr, payload_bytes).  dtype: 0 f64, 1 f32, 2 c64, 3 c128."""
     structs, layers, dim = _args(structs, layers, dim)
     Cn, Bs, T = len(structs), dim.shape[0], len(layers)
     rel = np.zeros(Bs, np.uint64)
     lb = np.zeros(Cn, np.uint64)
     lo = np.zeros(T, np.uint64)
     na, P = C.c_uint64(0), C.c_uint64(0)
-    rc = _L().orc2_plan(Cn, Bs, T, _p(structs), _p(layers), _p(dim), _p(rel), _p(lb), _p(lo), C.byref(na), C.byref(P))
+    rc = _L().orc2_plan(Cn, Bs, T, _p(structs), _p(layers), _p(dim), dtype, _p(rel), _p(lb), _p(lo), C.byref(na), C.byref(P))
     if rc:
         raise OracleError(rc, "v2 plan")
     return dict(rel_offset=rel, layer_bytes=lb, layer_offset=lo, n_addr=int(na.value), payload_bytes=int(P.value))
 
 
-def serialized_size(structs, layers, dim):
+def serialized_size(structs, layers, dim, dtype: int = 0):
     structs, layers, dim = _args(structs, layers, dim)
     hb, tot = C.c_uint64(0), C.c_uint64(0)
-    rc = _L().orc2_serialized_size(len(structs), dim.shape[0], len(layers), _p(structs), _p(layers), _p(dim),
+    rc = _L().orc2_serialized_size(len(structs), dim.shape[0], len(layers), _p(structs), _p(layers), _p(dim), dtype,
                                    C.byref(hb), C.byref(tot))
     if rc:
         raise OracleError(rc, "v2 serialized_size")
     return int(hb.value), int(tot.value)
 
 
-def serialize(structs, layers, qn, dim, addr, capacity: int | None = None, out: np.ndarray | None = None) -> np.ndarray:
-    """The whole v2 stream.  ``addr``: HOST addresses of the blocks, layer-major."""
+def serialize(structs, layers, qn, dim, addr, capacity: int | None = None, out: np.ndarray | None = None,
+              dtype: int = 0) -> np.ndarray:
+    """The whole v2 stream.  ``addr``: HOST addresses of the blocks, layer-major.  dtype: the element type (reading E-2)."""
     structs, layers, dim = _args(structs, layers, dim)
     qn = np.ascontiguousarray(qn, dtype=np.int32).reshape(-1, 3, 2)
     addr = np.ascontiguousarray(addr, dtype=np.uint64)
     if capacity is None:
-        capacity = serialized_size(structs, layers, dim)[1]
+        capacity = serialized_size(structs, layers, dim, dtype)[1]
     if out is None:
         out = np.full(max(capacity, 1), 0xCD, dtype=np.uint8)
     written = C.c_uint64(0)
     rc = _L().orc2_serialize(len(structs), dim.shape[0], len(layers), _p(structs), _p(layers), _p(qn), _p(dim), _p(addr),
-                             _p(out), capacity, C.byref(written))
+                             dtype, _p(out), capacity, C.byref(written))
     if rc:
         e = OracleError(rc, "v2 serialize")
         e.required = int(written.value)
@@ -121,8 +123,10 @@ def stream_info(stream: np.ndarray):
     rc = _L().orc2_stream_info(_p(s), s.size, *[C.byref(x) for x in v])
     if rc:
         raise OracleError(rc, "v2 stream_info")
+    dt = C.c_uint32(0)
+    _L().orc2_stream_dtype(_p(s), s.size, C.byref(dt))
     return dict(n_structs=int(v[0].value), n_struct_blocks=int(v[1].value), n_layers=int(v[2].value),
-                header_bytes=int(v[3].value), payload_bytes=int(v[4].value))
+                header_bytes=int(v[3].value), payload_bytes=int(v[4].value), dtype=int(dt.value))
 
 
 def validate_stream(stream: np.ndarray) -> int:

@@ -48,7 +48,8 @@ class LayeredDesc(C.Structure):
 
 class LayeredStreamInfo(C.Structure):
     _fields_ = [("n_structs", C.c_uint64), ("n_struct_blocks", C.c_uint64), ("n_layers", C.c_uint64),
-                ("header_bytes", C.c_uint64), ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64)]
+                ("header_bytes", C.c_uint64), ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64),
+                ("dtype", C.c_uint64)]
 
 
 class Result(C.Structure):
@@ -278,8 +279,8 @@ def layered_stream_info(first_64_bytes) -> dict:
 
 
 def make_layered_desc(n_structs: int, n_struct_blocks: int, n_layers: int, n_addr: int, structs_ptr: int, layers_ptr: int,
-                      qn_ptr: int, dim_ptr: int, addr_ptr: int) -> LayeredDesc:
-    return LayeredDesc(n_structs, n_struct_blocks, n_layers, 2, F64, 0, n_addr, structs_ptr, layers_ptr, qn_ptr, dim_ptr,
+                      qn_ptr: int, dim_ptr: int, addr_ptr: int, dtype: int = F64) -> LayeredDesc:
+    return LayeredDesc(n_structs, n_struct_blocks, n_layers, 2, dtype, 0, n_addr, structs_ptr, layers_ptr, qn_ptr, dim_ptr,
                        addr_ptr)
 
 

@@ -11,6 +11,7 @@ static thread_local int g_last_cuda_error = 0;
 int cuda_fail(cudaError_t e)
 {
     g_last_cuda_error = (int)e;
+    cudaGetLastError();  // a non-sticky error must not resurface in the cudaGetLastError() behind a later, unrelated launch
     return BS_ERR_CUDA;
 }
 
@@ -52,7 +53,7 @@ int check_opts(const bs_opts& o)
     if (o.tile_bytes == 0 || o.tile_bytes % kGranule != 0 || o.tile_bytes > 65536) return BS_ERR_ARG;
     if (o.variant == BS_VARIANT_TMA &&
         (o.stages < 3 || o.stages > 8 || o.warps < 1 || o.warps > 16 ||
-         (uint64_t)o.warps * ((uint64_t)o.stages * o.tile_bytes + 1120ull) > 224u * 1024u))
+         (uint64_t)o.warps * ((uint64_t)o.stages * o.tile_bytes + kMetaBytesPerWarp) > 224u * 1024u))
         return BS_ERR_ARG;
     return BS_OK;
 }

@@ -565,7 +565,7 @@ static int prefetch_packages_impl(bs_engine* e, const void* h_slots, uint64_t sl
     // arrival order: each payload package is unpacked on its own; runs of consecutive slots that fit a staging buffer
     // come over in ONE DMA (what lies behind a short package inside the run is read and ignored)
     const uint64_t per_buf = std::max<uint64_t>(1, e->cfg.chunk_bytes / slot_bytes);
-    const uint64_t cut = plan_uniform_cap(plan, e->opts.tile_bytes ? e->opts.tile_bytes : 32768u);  // 32 KiB: the unpack preset's tile
+    const uint64_t cut = plan_uniform_cap(plan, e->opts.tile_bytes ? e->opts.tile_bytes : kGranule);  // the presets work on 16 KiB granules
     uint64_t batch = 0;
     for (size_t i = 0; i < by_slot.size(); ++batch) {
         const uint32_t b = (uint32_t)(batch % S);

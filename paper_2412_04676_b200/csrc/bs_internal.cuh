@@ -24,6 +24,7 @@ constexpr uint32_t kBlockRec = 48;
 constexpr uint32_t kHeaderAlign = 128;
 constexpr uint32_t kPoolAlign = 256;
 constexpr uint32_t kGranule = 16384;  // bytes of payload per tile_first entry
+constexpr uint32_t kMetaBytesPerWarp = 2048;  // TMA variant: shared memory per data warp beside its ring (prefetched block table)
 
 constexpr uint32_t kScanThreads = 256;
 constexpr uint32_t kScanItems = 4;
@@ -37,10 +38,16 @@ struct __align__(16) Blk {
 // element size of a dtype (bs.h): f64 8, f32 4, c64 8, c128 16
 __host__ __device__ inline uint32_t elem_bytes(uint32_t dtype) { return dtype == BS_F32 ? 4u : (dtype == BS_C128 ? 16u : 8u); }
 
+struct __align__(16) ScanState {  // one tile of the chained scan: {flag | value, epoch tag}, read and written as ONE 16-byte access
+    uint64_t word;
+    uint64_t tag;
+};
+
 struct __align__(256) WsHead {
-    uint32_t scan_ticket;    // dynamic tile id of the single-pass scan
-    uint32_t ctas_done;      // last CTA out finalises
-    int32_t status;          // first error wins (atomicCAS)
+    // ---- line 0: what the pass leaves for the data-movement kernels (plain fields, final once the pass is complete) ----
+    uint32_t scan_ticket;    // layered plan (bs_layered.cu): dynamic item id
+    uint32_t ctas_done;      // layered plan: items of phase 1 done
+    int32_t status;          // BS_OK or the first error (the unpack kernels may still flip it: pad check)
     uint32_t n_tensors;
     uint32_t n_blocks;
     uint32_t status_pass1;   // layered sets: status after the first plan pass (read by the second)
@@ -54,20 +61,19 @@ struct __align__(256) WsHead {
     uint32_t scan_ticket2;
     uint32_t ctas_done2;
     uint32_t dtype;          // element type of the set the tables describe (bs.h BS_F64 ..)
-    uint32_t pad0;
-    // the v1 scan's own synchronisation words, each tagged with the epoch of the call that wrote it (bs_scan_phase.cuh):
-    // [63:24] epoch, [23:0] count / code.  A word of another epoch is stale whatever it holds.
-    uint64_t ep_ticket;      // work items handed out
-    uint64_t ep_done;        // work items completed; the CTA that completes the last one finalises
-    uint64_t ep_err;         // first error of the call ([7:0] = -code)
-    uint64_t ep_ready;       // == tag once the tables and the plain fields above are final (fused kernels wait on it)
+    uint32_t pad0[13];
+    // ---- the v1 pass's own synchronisation words (bs_scan_phase.cuh), one 128-byte line each: the CTAs of a fused kernel
+    // that poll `ready` must not slow the atomics of those still working down ----
+    ScanState ready;         // line 1: {payload_bytes << 8 | (status & 0xff), epoch tag} once tables and fields are final
+    uint64_t pad1[14];
+    uint64_t ep_ticket;      // line 2: work items handed out.  [63:24] a fixed "idle" tag, [23:0] count: the last CTA out of
+    uint64_t pad2[15];       //         a launch puts the three counters back to {tag, 0}, so the next launch pays ONE atomic
+    uint64_t ep_done;        // line 3: work items completed; the CTA that completes the last one finalises
+    uint64_t ep_exit;        //         CTAs that have left the item loop; the last one resets the counters
+    uint64_t ep_err;         //         first error of the call: [63:24] epoch tag, [7:0] = -code
+    uint64_t pad3[13];
 };
-static_assert(sizeof(WsHead) == 256, "WsHead is one 256-byte slot");
-
-struct __align__(16) ScanState {  // one tile of the chained scan: {flag | value, epoch tag}, read and written as ONE 16-byte access
-    uint64_t word;
-    uint64_t tag;
-};
+static_assert(sizeof(WsHead) == 512, "WsHead is four 128-byte lines");
 
 struct WsLayout {
     WsHead* head;

@@ -33,7 +33,7 @@ struct LwLayout {
     WsLayout ws;        // head, blk, tile_first: what the move kernels see
     uint64_t* st1[2];   // chained-scan state of the block pass
     uint64_t* st2[2];   // chained-scan state of the layer pass
-    uint64_t* gs;       // [Bs+1] exclusive prefix of stored sizes over the structure block table | odd flag (bit 0)
+    uint64_t* gs;       // [Bs+1] exclusive prefix of stored sizes over the structure block table | pad code (bits 0-1)
     uint64_t* gp;       // [Bs+1] exclusive prefix of pool slot sizes (deserialize)
     LayerPos* lpos;     // [T+1]
     uint64_t blk_cap;   // B the blk[] table can hold (plus the sentinel)
@@ -79,6 +79,7 @@ struct LPlanParams {
     const uint32_t* dim;
     const uint64_t* addr;
     uint32_t C, Bs, T;        // serialize: counts; deserialize: capacities of the out arrays
+    uint32_t dtype;           // serialize: element type of the set (deserialize reads it from the header)
     uint64_t n_addr;          // entries of addr[] (deserialize: capacity of out addr)
     // deserialize inputs
     const unsigned char* header;   // stream byte 0 .. header_bytes
@@ -218,6 +219,7 @@ __device__ __forceinline__ void cta_wait_until(const uint32_t* counter, uint32_t
 
 struct PlanShape {  // uniform over the grid: derived from the call's arguments / the fixed header alone
     uint64_t C, Bs, T, hb, P_hdr;
+    uint32_t dtype;     // element type (bs.h): the element size is all it decides (reading E-2)
     bool ok;
     uint32_t n1, n2;
 };
@@ -226,7 +228,7 @@ template <bool DESER>
 __device__ __forceinline__ PlanShape plan_shape(const LPlanParams& p, WsHead* head)
 {
     PlanShape s;
-    s.C = p.C; s.Bs = p.Bs; s.T = p.T; s.hb = 0; s.P_hdr = 0; s.ok = true;
+    s.C = p.C; s.Bs = p.Bs; s.T = p.T; s.hb = 0; s.P_hdr = 0; s.ok = true; s.dtype = p.dtype;
     if (DESER) {  // the fixed header, field by field in stream order
         int code = 0;
         s.C = s.Bs = s.T = 0;
@@ -240,7 +242,7 @@ __device__ __forceinline__ PlanShape plan_shape(const LPlanParams& p, WsHead* he
             if (w0.x != 0x41505342u || w0.y != 0x31455352u)      code = BS_ERR_CORRUPT;  // "BSPARSE1"
             else if (w0.z != 2u)                                  code = BS_ERR_CORRUPT;  // version
             else if (w0.w != 0x01020304u)                         code = BS_ERR_CORRUPT;  // endian_tag
-            else if (w1.x != 0u)                                  code = BS_ERR_CORRUPT;  // dtype f64
+            else if (w1.x > (uint32_t)BS_C128)                    code = BS_ERR_CORRUPT;  // dtype
             else if (w1.y != 2u)                                  code = BS_ERR_CORRUPT;  // n_qn
             else if (w1.z != 3u)                                  code = BS_ERR_CORRUPT;  // max_rank
             else if (w1.w != 16u)                                 code = BS_ERR_CORRUPT;  // align
@@ -248,7 +250,7 @@ __device__ __forceinline__ PlanShape plan_shape(const LPlanParams& p, WsHead* he
             else if (hH != align_up(kFixedHeader + kV2Struct * hC + kV2Layer * hT + kBlockRec * hBs, kHeaderAlign)) code = BS_ERR_CORRUPT;
             else if (hH > p.nbytes || hP != p.nbytes - hH)        code = BS_ERR_CORRUPT;
             else if (hC > p.C || hBs > p.Bs || hT > p.T)          code = BS_ERR_CAPACITY;  // out arrays too small
-            else { s.C = hC; s.Bs = hBs; s.T = hT; s.hb = hH; s.P_hdr = hP; }
+            else { s.C = hC; s.Bs = hBs; s.T = hT; s.hb = hH; s.P_hdr = hP; s.dtype = w1.x; }
             if (code == BS_ERR_CAPACITY && blockIdx.x == 0 && threadIdx.x == 0) {  // report the counts
                 head->n_structs = (uint32_t)hC; head->n_struct_blocks = (uint32_t)hBs; head->n_tensors = (uint32_t)hT;
             }
@@ -334,11 +336,11 @@ __device__ __forceinline__ void plan_blocks_tile(const LPlanParams& p, const Pla
         const uint64_t n01 = (uint64_t)d0 * d1;
         uint64_t n = n01 * d2;
         if (valid && (__umul64hi(n01, (uint64_t)d2) != 0 || n >= (1ull << 57))) { err = kErrBad; n = 0; }
-        const uint64_t nbytes = n * 8;
+        const uint64_t nbytes = n * elem_bytes(s.dtype);
         const uint64_t st = (nbytes + 15) & ~15ull;
         stored[k] = valid ? st : 0;
         slot[k] = (DESER && valid) ? align_up(nbytes, kPoolAlign) : 0;
-        oddf[k] = (uint32_t)(n & 1);
+        oddf[k] = (uint32_t)(st - nbytes) >> 2;  // pad code: 0..3 words of zero pad (Blk)
         if (DESER && valid) {
             if (owner >= C) err = BS_ERR_CORRUPT;
             else {
@@ -488,6 +490,7 @@ __device__ __forceinline__ void plan_finalize(const LPlanParams& p, const PlanSh
         vh->n_tensors = (uint32_t)s.T;
     }
     vh->n_blocks = (uint32_t)tot_blocks;
+    vh->dtype = s.dtype;
     vh->header_bytes = hb;
     vh->payload_bytes = P;
     vh->pool_bytes = pool;
@@ -499,6 +502,7 @@ __device__ __forceinline__ void plan_finalize(const LPlanParams& p, const PlanSh
         r.status = status; r.n_tensors = vh->n_tensors; r.n_blocks = (uint32_t)tot_blocks;
         r.reserved[0] = vh->n_structs; r.reserved[1] = vh->n_struct_blocks;
         for (int z = 2; z < 5; ++z) r.reserved[z] = 0;
+        r.reserved[2] = s.dtype;
         *p.result = r;
     }
 }
@@ -548,7 +552,7 @@ __device__ __forceinline__ void plan_expand_chunk(const LPlanParams& p, uint64_t
             const uint64_t g = p.lw.gs[j], gn = p.lw.gs[j + 1], gf = p.lw.gs[lp.sfirst];
             const uint64_t off = lp.stream_off + ((g & ~15ull) - (gf & ~15ull));
             const uint64_t stored = (gn & ~15ull) - (g & ~15ull);
-            const uint64_t odd = g & 1ull;
+            const uint64_t padc = g & 3ull;  // words of zero pad behind the block's data
             uint64_t address;
             if (!DESER) {
                 address = __ldg(reinterpret_cast<const unsigned long long*>(p.addr + i));
@@ -560,13 +564,17 @@ __device__ __forceinline__ void plan_expand_chunk(const LPlanParams& p, uint64_t
                 address = p.pool_base + lp.off + (p.lw.gp[j] - p.lw.gp[lp.sfirst]);
                 p.out_addr[i] = address;
             }
-            if (DESER && odd && p.payload != nullptr) {  // pad bytes are zero
-                const uint64_t pad = __ldg(reinterpret_cast<const unsigned long long*>(p.payload + hb + off + stored - 8));
+            if (DESER && padc && p.payload != nullptr) {  // pad bytes are zero: the last 16-byte unit of the block
+                const uint4 u = __ldg(reinterpret_cast<const uint4*>(p.payload + hb + off + stored - 16));
+                const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+                uint32_t pad = 0;
+#pragma unroll
+                for (uint32_t q = 0; q < 4; ++q) pad |= (q >= 4u - (uint32_t)padc) ? w[q] : 0u;
                 if (pad != 0) set_err(head, p.result, BS_ERR_CORRUPT);
             }
             Blk e;
             e.off = off;
-            e.addr = (address & ~7ull) | (odd << 1);  // pad code (Blk): 2 words = the 8 zero bytes of an odd f64 block
+            e.addr = (address & ~7ull) | padc;  // pad code (Blk): e.g. 2 words = the 8 zero bytes of an odd f64 block
             p.lw.ws.blk[i] = e;
             // granule boundaries g*kGranule inside [off, off + stored)
             g0 = (off + kGranule - 1) / kGranule;
@@ -675,7 +683,7 @@ __global__ void __launch_bounds__(kLThreads) lplan_kernel(const LPlanParams p)
 int check_layered(const bs_layered_desc* s)
 {
     if (s == nullptr) return BS_ERR_ARG;
-    if (s->n_qn != 2 || s->dtype != BS_F64) return BS_ERR_UNSUPPORTED;
+    if (s->n_qn != 2 || s->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
     auto al = [](const void* q, uintptr_t a) { return ((uintptr_t)q & (a - 1)) == 0; };
     if (s->n_structs && (s->structs == nullptr || !al(s->structs, 16))) return BS_ERR_ARG;
     if (s->n_layers && (s->layers == nullptr || !al(s->layers, 16))) return BS_ERR_ARG;
@@ -744,6 +752,7 @@ int run_layered_serialize_plan(const bs_layered_desc* set, void* d_ws, uint64_t 
     p.C = set->n_structs;
     p.Bs = set->n_struct_blocks;
     p.T = set->n_layers;
+    p.dtype = set->dtype;
     p.n_addr = set->n_addr;
     lplan_kernel<false><<<plan_grid(p, sms), kLThreads, 0, stream>>>(p);
     e = cudaGetLastError();
@@ -853,9 +862,10 @@ int bs_layered_stream_info(const void* h, bs_layered_stream_info_t* out)
     memcpy(w, s, 40);
     memcpy(q, s + 40, 24);
     if (memcmp(s, "BSPARSE1", 8) != 0) return BS_ERR_CORRUPT;
-    if (w[2] != 2u || w[3] != 0x01020304u || w[4] != 0u || w[5] != 2u || w[6] != 3u || w[7] != 16u) return BS_ERR_CORRUPT;
+    if (w[2] != 2u || w[3] != 0x01020304u || w[4] > (uint32_t)BS_C128 || w[5] != 2u || w[6] != 3u || w[7] != 16u) return BS_ERR_CORRUPT;
     if (q[0] >= (1ull << 32)) return BS_ERR_CORRUPT;
     if (q[1] != bs_layered_header_bytes(w[8], q[0], w[9])) return BS_ERR_CORRUPT;
+    out->dtype = w[4];
     out->n_structs = w[8];
     out->n_struct_blocks = w[9];
     out->n_layers = q[0];

@@ -214,7 +214,7 @@ void resolve_opts(const bs_opts* in, bs_opts* out)
             if (o.stages == 0) o.stages = 3;
             if (o.warps == 0) {  // ~96 KiB of loads in flight per SM
                 o.warps = (96u * 1024u) / ((o.stages - 1) * o.tile_bytes);
-                while (o.warps > 1 && (uint64_t)o.warps * o.stages * (o.tile_bytes + 1120ull) > 216u * 1024u) --o.warps;
+                while (o.warps > 1 && (uint64_t)o.warps * ((uint64_t)o.stages * o.tile_bytes + kMetaBytesPerWarp) > 216u * 1024u) --o.warps;
                 o.warps = o.warps < 1 ? 1 : (o.warps > 16 ? 16 : o.warps);
             }
         }

@@ -99,15 +99,15 @@ __device__ __forceinline__ uint32_t struct_of_block(const bs_struct_rec* st, uin
     return lo;
 }
 
-// S3, v2: one 16-byte unit of the header region.  The scan kernels of bs_layered.cu left gs[] (prefix of stored sizes
-// over the structure block table, odd flag in bit 0) and lpos[] (payload offset of every layer).
+// S3, v2: one 16-byte unit of the header region.  The plan kernel of bs_layered.cu left gs[] (prefix of stored sizes
+// over the structure block table, pad code in bits 0-1), lpos[] (payload offset of every layer) and the set's dtype.
 __device__ __forceinline__ uint4 header_unit_v2(const MoveParams& p, uint64_t u, uint32_t T, uint64_t hb, uint64_t P)
 {
     const uint32_t C = p.lay.C, Bs = p.lay.Bs;
     uint4 v = make_uint4(0, 0, 0, 0);
     if (u < 4) {
         if (u == 0) v = make_uint4(0x41505342u, 0x31455352u, 2u, 0x01020304u);  // "BSPARSE1", version 2, endian_tag
-        else if (u == 1) v = make_uint4(0u, 2u, 3u, 16u);                        // dtype, n_qn, max_rank, align
+        else if (u == 1) v = make_uint4(p.ws.head->dtype, 2u, 3u, 16u);          // dtype, n_qn, max_rank, align
         else if (u == 2) v = make_uint4(C, Bs, T, 0u);                           // u32 C, u32 Bs, u64 n_layers
         else v = make_uint4((uint32_t)hb, (uint32_t)(hb >> 32), (uint32_t)P, (uint32_t)(P >> 32));
         return v;

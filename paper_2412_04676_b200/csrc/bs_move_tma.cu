@@ -179,11 +179,22 @@ __device__ __forceinline__ bool make_seg(const Blk* __restrict__ blk, uint32_t j
     return clip_seg(e, next, tlo, thi, s);
 }
 
-// Per-warp metadata in shared memory, filled by cp.async ahead of use (no register is tied up, no warp stalls):
-//   tf[3][2]   tile_first[] pair {jlo, jhi_raw} of tiles m, m+1, m+2 (slot = tile index mod 3)
-//   blk[2][34] block table entries jlo .. jlo+32 of tiles m, m+1     (slot = tile index mod 2)
+// Per-warp metadata in shared memory, filled by cp.async ahead of use (no register is tied up, no warp stalls).  The
+// block table is read once per tile and never cached (the data streaming past evicts it), so each of the two lookup
+// levels costs a DRAM round trip — about as long as a whole loop iteration of a warp.  kBlkAhead iterations lie between
+// the fetch of a tile's table entries and their use, and as many again between the fetch of its tile_first[] pair and
+// that:
+//   tf[2*kBlkAhead+1][2]  tile_first[] pair {jlo, jhi_raw} of tiles m .. m+2*kBlkAhead (slot = tile index mod the count)
+//   blk[kBlkAhead+1][34]  block table entries jlo .. jlo+32 of tiles m .. m+kBlkAhead
+// Measured (profiles/r02_summary.md): kBlkAhead = 2 takes the wait for the table out of the loop, and the achieved DRAM
+// bandwidth DROPS (unpack 6.9 -> 6.1 TB/s, pack 6.6 -> 5.8 TB/s in its best shape): a warp that never waits runs ahead until
+// every stage of its ring is in flight, and this memory system moves fewer bytes per second the more requests it holds
+// (the same finding as for deeper rings).  With kBlkAhead = 1 the one exposed round trip per iteration paces the warp.
+constexpr uint32_t kBlkAhead = 1;
+constexpr uint32_t kBlkSlots = kBlkAhead + 1, kTfSlots = 2 * kBlkAhead + 1;
 constexpr uint32_t kMetaBlk = 34;
-constexpr uint32_t kMetaBytes = 2 * kMetaBlk * 16 + 32;  // 1120 per warp
+constexpr uint32_t kMetaBytes = (kBlkSlots * kMetaBlk * 16 + kTfSlots * 8 + 15) / 16 * 16;
+static_assert(kMetaBytes <= kMetaBytesPerWarp, "check_opts (bs_api.cu) budgets kMetaBytesPerWarp of shared memory per warp");
 
 // pack: stage one block segment.  Bulk part: counted in *tx, issued later (after the expect_tx); 8-byte-aligned
 // blocks (D16) and odd tails: cp.async now.  Returns the number of cp.async groups this lane started.
@@ -235,22 +246,17 @@ __device__ __forceinline__ void unpack_seg(const Seg& s, uint32_t saddr, const u
     }
 }
 
-// Default launch shapes (B200, measured on the D=6000 and D=15400 sets): pack 3 rings x 3 stages x 16 KiB, unpack one
-// ring of 4 stages x 32 KiB — about 96 KiB of loads in flight per SM either way; deeper rings or more warps lower the
-// achieved DRAM bandwidth.  (Unpack, whole bs_deserialize: 6440 / 6470 GB/s on the two sets with this shape against
-// 6360 / 6235 with 2 rings x 3 x 16 KiB.)  A package map whose size limit is not a multiple of 32 KiB keeps 16 KiB tiles.
+// Default launch shapes (B200, measured; profiles/r02_summary.md).  The launch always has the small-set shape — three rings
+// of 3 stages x 16 KiB per SM, what sets of tens of MB run fastest with in both directions — and the kernel, which knows the
+// payload size, switches sets of half a GB and more to ONE ring in the same shared memory: pack 3 x 48 KiB, unpack 4 x 32 KiB
+// (about 96 KiB of loads in flight per SM either way; deeper rings or more warps lower the achieved DRAM bandwidth).  A
+// package map keeps the small shape unless its size limit is a multiple of the large tile.
 struct Preset {
     uint32_t tile_bytes, stages, warps;
 };
-__host__ __device__ inline Preset preset(bool unpack, uint64_t pkg_cap)
-{
-    Preset ps = {16384, 3, 3};
-    if (unpack) {
-        if (pkg_cap % 32768 == 0) { ps.tile_bytes = 32768; ps.stages = 4; ps.warps = 1; }
-        else ps.warps = 2;
-    }
-    return ps;
-}
+__host__ __device__ inline Preset preset_small() { return Preset{16384, 3, 3}; }
+__host__ __device__ inline Preset preset_large(bool unpack) { return unpack ? Preset{32768, 4, 1} : Preset{49152, 3, 1}; }
+constexpr uint64_t kLargePayload = 512ull << 20;
 
 // FUSED: called behind the size / offset pass inside one kernel (fused_tma_kernel); `hv` is that pass's outcome.
 template <bool UNPACK, bool FUSED>
@@ -267,12 +273,12 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     const uint64_t ng = hv.ng;
     const uint64_t lo = p.lo, hi = p.hi < total ? p.hi : total;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t tile_bytes = p.tile_bytes, n_warps = opt_warps & 0xffffu;
-    const uint32_t n_stages = opt_stages;
-    // The pack preset (bit 31 of opt_warps) is settled here, where the payload size is known: sets of half a GB and more
-    // run ONE ring of 3 x 48 KiB per SM instead of three of 3 x 16 KiB (the same shared memory; bs_serialize +0.6 % on the
-    // D=15400 set, +1.3 % on the D=6000 set), smaller sets keep the three rings (the 77 MB set loses 3.5 % with one).
-    if (!UNPACK && (opt_warps >> 31) && P >= (512ull << 20) && p.pkg.cap % 49152u == 0) { tile_bytes = 49152u; n_warps = 1; }
+    uint32_t tile_bytes = p.tile_bytes, n_warps = opt_warps & 0xffffu, n_stages = opt_stages;
+    // The preset (bit 31 of opt_warps: bs_opts left the shape open) is settled here, where the payload size is known
+    if ((opt_warps >> 31) && P >= kLargePayload && p.pkg.cap % preset_large(UNPACK).tile_bytes == 0) {
+        const Preset ps = preset_large(UNPACK);
+        tile_bytes = ps.tile_bytes; n_stages = ps.stages; n_warps = ps.warps;
+    }
     // ---- payload tiles of [lo, hi): tile k = payload bytes [k*tile_bytes, (k+1)*tile_bytes) ----
     uint64_t plo = 0, phi = 0, k0 = 0, np = 0;
     if (hi > hb && hi > lo) {
@@ -303,9 +309,9 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     const uint32_t ring = smem_u32(smem) + warp * n_stages * tile_bytes;  // this warp's stages
     unsigned char* ring_ptr = smem + (size_t)warp * n_stages * tile_bytes;
     unsigned char* meta_ptr = smem + (size_t)n_warps * n_stages * tile_bytes + (size_t)warp * kMetaBytes;
-    const Blk* m_blk = reinterpret_cast<const Blk*>(meta_ptr);                                  // [2][kMetaBlk]
-    const uint32_t* m_tf = reinterpret_cast<const uint32_t*>(meta_ptr + 2 * kMetaBlk * 16);    // [3][2]
-    const uint32_t m_blk_s = smem_u32(meta_ptr), m_tf_s = m_blk_s + 2 * kMetaBlk * 16;
+    const Blk* m_blk = reinterpret_cast<const Blk*>(meta_ptr);                                          // [kBlkSlots][kMetaBlk]
+    const uint32_t* m_tf = reinterpret_cast<const uint32_t*>(meta_ptr + kBlkSlots * kMetaBlk * 16);    // [kTfSlots][2]
+    const uint32_t m_blk_s = smem_u32(meta_ptr), m_tf_s = m_blk_s + kBlkSlots * kMetaBlk * 16;
     const uint32_t bar0 = smem_u32(&s_bar[warp * kMaxStages]);
     if (lane == 0) {
         for (uint32_t s = 0; s < n_stages; ++s) mbar_init(bar0 + 8 * s, 1);
@@ -326,25 +332,25 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     hints.st = (p.tune & 2u) != 0;
     const int64_t lag = n_stages - 2;  // tile i is stored while tiles i+1 .. i+lag are loading
 
-    // The block table is read once per tile and never cached (the data streaming past evicts it), so each of the
-    // two lookup levels costs a DRAM round trip.  Both are fetched ahead with cp.async into shared memory:
-    // tile_first[] two tiles, blk[] one tile before use.
+    // the block table is fetched ahead into shared memory (see kBlkAhead)
     auto tile_base = [&](int64_t i) {
         return (blocked ? k0 + worker * per + (uint64_t)i : k0 + worker + (uint64_t)i * n_workers) * tile_bytes;
     };
     auto has_tile = [&](int64_t i) { return i >= 0 && i < n_mine && B != 0; };
+    auto tf_slot = [](int64_t i) { return (uint32_t)((i + 8 * (int64_t)kTfSlots) % (int64_t)kTfSlots); };     // i >= -kMaxStages
+    auto blk_slot = [](int64_t i) { return (uint32_t)((i + 8 * (int64_t)kBlkSlots) % (int64_t)kBlkSlots); };
     auto fetch_tf = [&](int64_t i) {  // lanes 0, 1: tile_first[g0], tile_first[g1] of tile i
         if (has_tile(i) && lane < 2) {
             const uint64_t tb = tile_base(i);
             uint64_t g = lane == 0 ? tb / kGranule : (tb + tile_bytes) / kGranule;
             if (g > ng) g = ng;  // tile_first[ng] == B
-            cp_async_4(m_tf_s + (uint32_t)((i + 6) % 3) * 8 + lane * 4, p.ws.tile_first + g);
+            cp_async_4(m_tf_s + tf_slot(i) * 8 + lane * 4, p.ws.tile_first + g);
         }
     };
     auto read_tf = [&](int64_t i, uint32_t* jlo, uint32_t* jhi) {
         *jlo = 1; *jhi = 0;
         if (has_tile(i)) {
-            const uint32_t s = (uint32_t)((i + 6) % 3) * 2;
+            const uint32_t s = tf_slot(i) * 2;
             *jlo = m_tf[s];
             *jhi = m_tf[s + 1];
             if (*jhi >= B) *jhi = B - 1;
@@ -354,28 +360,29 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
         uint32_t jlo, jhi;
         read_tf(i, &jlo, &jhi);
         if (jlo > jhi) return;
-        const uint32_t slot = m_blk_s + (uint32_t)((i + 6) % 2) * kMetaBlk * 16;
+        const uint32_t slot = m_blk_s + blk_slot(i) * kMetaBlk * 16;
         if (jlo + lane <= jhi + 1) cp_async_16(slot + lane * 16, blk + jlo + lane);
         if (lane == 0 && jlo + 32 <= jhi + 1) cp_async_16(slot + 32 * 16, blk + jlo + 32);
     };
     const int64_t m0 = UNPACK ? -lag : 0;  // index of the tile whose block table the first iteration needs
-    fetch_tf(m0);
-    fetch_tf(m0 + 1);
+    for (int64_t i = m0; i < m0 + 2 * (int64_t)kBlkAhead; ++i) fetch_tf(i);
     cp_async_commit();
     cp_async_wait<0>();
     __syncwarp();
-    fetch_blk(m0);
+    for (int64_t i = m0; i < m0 + (int64_t)kBlkAhead; ++i) fetch_blk(i);
     cp_async_commit();
+    for (uint32_t g = 1; g < kBlkAhead; ++g) cp_async_commit();  // (empty groups: the loop counts kBlkAhead groups back)
 
     for (int64_t it = 0; it < n_mine + lag; ++it) {
         const int64_t m = m0 + it;
-        fetch_tf(m + 2);
-        cp_async_commit();
-        cp_async_wait<1>();  // everything fetched during the previous iteration has landed
+        // one cp.async group per iteration; the groups of the last kBlkAhead - 1 iterations may still be in flight: the
+        // table entries of tile m and the tile_first pair of tile m + kBlkAhead, fetched kBlkAhead iterations ago, have landed
+        cp_async_wait<kBlkAhead - 1>();
         // the store that last read stage it % n_stages was committed two iterations ago
         bulk_wait_read<1>();
         __syncwarp();
-        fetch_blk(m + 1);
+        fetch_tf(m + 2 * (int64_t)kBlkAhead);
+        fetch_blk(m + (int64_t)kBlkAhead);
         cp_async_commit();
         uint32_t jlo, jhi;
         read_tf(m, &jlo, &jhi);
@@ -383,8 +390,8 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
         e0.off = 0; e0.addr = 0;
         uint64_t next0 = 0;  // clips to nothing
         if (jlo <= jhi && jlo + lane <= jhi) {
-            e0 = m_blk[(uint32_t)((m + 6) % 2) * kMetaBlk + lane];
-            next0 = m_blk[(uint32_t)((m + 6) % 2) * kMetaBlk + lane + 1].off;
+            e0 = m_blk[blk_slot(m) * kMetaBlk + lane];
+            next0 = m_blk[blk_slot(m) * kMetaBlk + lane + 1].off;
         }
         if (it < n_mine) {  // ---- produce: load tile `it` of this warp into its stage ----
             const uint32_t st = (uint32_t)(it % n_stages);
@@ -497,7 +504,7 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) fused_tma_kernel(cons
         hv = sm.out;
         __syncthreads();  // the rings reuse the pass's shared memory
     } else {
-        hv = scan::wait_ready(sp.ws.head, sp.tag, &s_hv);
+        hv = scan::wait_ready<UNPACK>(sp.ws.head, s, sp.tag, &s_hv);
     }
     move_tma_body<UNPACK, true>(p, hv, opt_stages, opt_warps, smem, s_bar);
 }
@@ -526,10 +533,12 @@ template <bool UNPACK>
 cudaError_t resolve_shape(const MoveParams& p, const bs_opts& o, Shape3* out)
 {
     Shape3 sh = {p.tile_bytes, o.stages, o.warps, 0u, 0};
-    if (o.tile_bytes == 0) {  // bs_opts left the shape open
-        const Preset ps = preset(UNPACK, p.pkg.cap);
+    if (o.tile_bytes == 0) {  // bs_opts left the shape open: launch the small shape, the kernel may switch to the large one
+        const Preset ps = preset_small(), pl = preset_large(UNPACK);
+        if ((size_t)pl.warps * pl.stages * pl.tile_bytes > (size_t)ps.warps * ps.stages * ps.tile_bytes || pl.warps > ps.warps)
+            return cudaErrorInvalidValue;  // the large shape must fit the launch of the small one
         sh.tile_bytes = ps.tile_bytes; sh.stages = ps.stages; sh.warps = ps.warps;
-        if (!UNPACK) sh.auto_shape = 0x80000000u;
+        sh.auto_shape = 0x80000000u;
     }
     if (sh.stages < 3 || sh.stages > kMaxStages || sh.warps < 1 || sh.warps > kMaxWarps) return cudaErrorInvalidValue;
     sh.smem = (size_t)sh.warps * sh.stages * sh.tile_bytes + (size_t)sh.warps * kMetaBytes;

@@ -447,7 +447,7 @@ int bs_layered_package_emit(const bs_layered_desc* set, uint64_t total_bytes, ui
                             bs_result* d_result, const bs_opts* opts, cudaStream_t stream)
 {
     if (set == nullptr) return BS_ERR_ARG;
-    if (set->n_qn != 2 || set->dtype != BS_F64) return BS_ERR_UNSUPPORTED;
+    if (set->n_qn != 2 || set->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
     if (d_slots == nullptr || !aligned16(d_slots) || cap == 0 || (cap & 15) || (slot_bytes & 15) ||
         slot_bytes < BS_PKG_HEADER + cap)
         return BS_ERR_ARG;
@@ -504,7 +504,7 @@ int bs_layered_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t
                               const bs_opts* opts, cudaStream_t stream)
 {
     if (out == nullptr) return BS_ERR_ARG;
-    if (out->n_qn != 2 || out->dtype != BS_F64) return BS_ERR_UNSUPPORTED;
+    if (out->n_qn != 2 || out->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
     if (d_slots == nullptr || !aligned16(d_slots) || (slot_bytes & 15) || slot_bytes < BS_PKG_HEADER + 16 || n_slots == 0)
         return BS_ERR_ARG;
     if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;

@@ -17,11 +17,14 @@
 // publishes WsHead.ep_ready.  An item only ever waits (look-back) for items claimed before it, which are being executed
 // by resident CTAs: forward progress needs no co-residency of the grid.
 //
-// No word the pass synchronises on needs clearing beforehand: tickets, the completion count, the first-error word and
-// every scan-state entry carry the call's 40-bit EPOCH tag (a process-wide counter handed out on the host), and a word
-// with another tag is "not written yet" whatever it holds — the workspace may be uninitialised memory.  (While a CUDA
-// graph is being captured the host cannot hand out a fresh epoch per replay; the call then clears head + state in front
-// of the kernel, as round 1 always did.)
+// No word the pass synchronises on needs clearing beforehand — the workspace may be uninitialised memory:
+//   - every scan-state entry, the first-error word and the `ready` word carry the call's 40-bit EPOCH tag (a process-wide
+//     counter handed out on the host); a word with another tag is "not written yet" whatever it holds;
+//   - the three counters (items handed out, items completed, CTAs out of the item loop) carry a fixed IDLE tag and are
+//     put back to {tag, 0} by the last CTA out of every launch, so a launch normally pays one atomic per count; a counter
+//     that does not carry the tag (first use of the workspace) is re-based by whoever touches it first.
+// (While a CUDA graph is being captured the host cannot hand out a fresh epoch per replay; the call then clears head +
+// state in front of the kernel, as round 1 always did.)
 //
 // A set of at most 1024 blocks and 1024 tensors is ONE item: a fused kernel then runs it REPLICATED — every CTA computes
 // the whole (tiny) table itself, identical values, and nobody waits for anybody; only CTA 0 writes head and result.
@@ -36,7 +39,8 @@ constexpr uint64_t kFlagAgg = 1ull << 62;
 constexpr uint64_t kFlagPrefix = 2ull << 62;
 constexpr uint64_t kValMask = (1ull << 62) - 1;
 constexpr uint32_t kInlineBoundaries = 4;
-constexpr uint64_t kCountMask = (1ull << 24) - 1;  // epoch-tagged words: [63:24] epoch, [23:0] count
+constexpr uint64_t kCountMask = (1ull << 24) - 1;  // tagged words: [63:24] tag, [23:0] count / code
+constexpr uint64_t kIdleTag = 0xB5C0DE5EEDull << 24;  // the counters' tag between launches
 
 // what the data-movement code needs to know about the set once the pass is complete
 struct HeadView {
@@ -502,7 +506,7 @@ __device__ __forceinline__ void run(const ScanParams& p, const Shape& s, uint64_
     }
     for (;;) {
         bar();
-        if (tid == 0) sm.item = tagged_inc(&head->ep_ticket, tag);
+        if (tid == 0) sm.item = tagged_inc(&head->ep_ticket, kIdleTag);
         bar();
         const uint32_t item = sm.item;
         if (item >= s.n_items) break;
@@ -515,29 +519,46 @@ __device__ __forceinline__ void run(const ScanParams& p, const Shape& s, uint64_
             const int code = s.code ? s.code : sm.err;
             if (code) post_err(head, tag, code);
             __threadfence();  // this item's table entries and its error are visible before it counts as done
-            if (tagged_inc(&head->ep_done, tag) == s.n_items - 1) {  // every item is complete: finalise
+            if (tagged_inc(&head->ep_done, kIdleTag) == s.n_items - 1) {  // every item is complete: finalise
                 __threadfence();
                 finalize<DESER, false>(p, s, read_err(head, tag), sm, true);
                 __threadfence();
-                st_release_u64(&head->ep_ready, tag);
+                st_state(&head->ready, (sm.out.P << 8) | (uint64_t)(uint8_t)(int8_t)sm.out.status, tag);
             }
         }
     }
+    // every CTA has its last (out of range) ticket by the time the last one is here: put the counters back for the next launch
+    if (tid == 0 && tagged_inc(&head->ep_exit, kIdleTag) == gridDim.x - 1) {
+        volatile uint64_t* c = &head->ep_ticket;
+        *c = kIdleTag;
+        c = &head->ep_done;
+        *c = kIdleTag;
+        c = &head->ep_exit;
+        *c = kIdleTag;
+        __threadfence();
+    }
 }
 
-// fused kernels, after run(): wait until the pass is complete and fetch its outcome (one thread per CTA polls)
-__device__ __forceinline__ HeadView wait_ready(const WsHead* head, uint64_t tag, HeadView* s_out)
+// fused kernels, after run(): wait until the pass is complete (one thread per CTA polls).  Everything the data movement
+// needs comes out of the ONE polled word and the shape every CTA derived for itself: no second round trip to the head.
+template <bool DESER>
+__device__ __forceinline__ HeadView wait_ready(const WsHead* head, const Shape& s, uint64_t tag, HeadView* s_out)
 {
     if (threadIdx.x == 0) {
-        uint32_t ns = 20;
-        while (ld_acquire_u64(&head->ep_ready) != tag) {
+        uint64_t w = 0, wt = 0;
+        uint32_t ns = 32;
+        for (;;) {
+            ld_state(&head->ready, &w, &wt);
+            if (wt == tag) break;
             __nanosleep(ns);
-            if (ns < 320) ns *= 2;
+            if (ns < 256) ns *= 2;
         }
-        const volatile WsHead* vh = head;
         HeadView hv;
-        hv.status = vh->status; hv.T = vh->n_tensors; hv.B = vh->n_blocks; hv.dtype = vh->dtype;
-        hv.hb = vh->header_bytes; hv.P = vh->payload_bytes; hv.ng = vh->n_granules;
+        hv.status = (int32_t)(int8_t)(uint8_t)(w & 0xffu);
+        hv.T = (uint32_t)s.T; hv.B = (uint32_t)s.B; hv.dtype = s.dtype; hv.hb = s.hb;
+        hv.P = DESER ? s.P_hdr : (w >> 8);
+        if (s.code != 0) hv.P = 0;
+        hv.ng = (hv.P + kGranule - 1) / kGranule;
         *s_out = hv;
     }
     __syncthreads();

@@ -72,17 +72,19 @@ _LAYER_DTYPE = np.dtype([("structure", "<u4"), ("tag", "<u4"), ("offset", "<u8")
 class DeviceLayeredSet:
     """The five device arrays of one bs_layered_desc (wire format v2), as torch uint8 tensors."""
 
-    def __init__(self, structs, layers, qn, dim, addr, n_structs: int, n_struct_blocks: int, n_layers: int, n_addr: int):
+    def __init__(self, structs, layers, qn, dim, addr, n_structs: int, n_struct_blocks: int, n_layers: int, n_addr: int,
+                 dtype: int = B.F64):
         self.structs, self.layers, self.qn, self.dim, self.addr = structs, layers, qn, dim, addr
         self.n_structs, self.n_struct_blocks, self.n_layers, self.n_addr = n_structs, n_struct_blocks, n_layers, n_addr
+        self.dtype = dtype
 
     @classmethod
     def from_host(cls, structs: np.ndarray, layers: np.ndarray, qn: np.ndarray, dim: np.ndarray, addr: np.ndarray,
-                  device="cuda"):
+                  device="cuda", dtype: int = B.F64):
         assert structs.dtype.itemsize == 32 and layers.dtype.itemsize == 16
         return cls(_to_dev(structs, device), _to_dev(layers, device), _to_dev(qn.astype(np.int32, copy=False), device),
                    _to_dev(dim.astype(np.uint32, copy=False), device), _to_dev(addr.astype(np.uint64, copy=False), device),
-                   len(structs), int(np.asarray(dim).reshape(-1, 3).shape[0]), len(layers), int(np.asarray(addr).size))
+                   len(structs), int(np.asarray(dim).reshape(-1, 3).shape[0]), len(layers), int(np.asarray(addr).size), dtype)
 
     @classmethod
     def empty(cls, cap_structs: int, cap_struct_blocks: int, cap_layers: int, cap_addr: int, device="cuda",
@@ -98,7 +100,7 @@ class DeviceLayeredSet:
     @property
     def desc(self) -> B.LayeredDesc:
         return B.make_layered_desc(self.n_structs, self.n_struct_blocks, self.n_layers, self.n_addr, self.structs.data_ptr(),
-                                   self.layers.data_ptr(), self.qn.data_ptr(), self.dim.data_ptr(), self.addr.data_ptr())
+                                   self.layers.data_ptr(), self.qn.data_ptr(), self.dim.data_ptr(), self.addr.data_ptr(), self.dtype)
 
     def to_host(self, n_structs: int, n_struct_blocks: int, n_layers: int, n_addr: int) -> dict:
         return dict(

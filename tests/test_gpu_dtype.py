@@ -195,11 +195,11 @@ def test_bad_element_types_and_nonzero_pad_are_rejected():
         o, pool, res = deserialize_on_gpu(st, total, rs.bset, ref["pool_bytes"])
         assert res["status"] == bs.ERR_CORRUPT, (pos, res)
         assert (pool.cpu().numpy() == 0xEE).all() and (o.tensors.cpu().numpy() == 0xAB).all()
-    # layered sets (wire format v2) stay fp64
+    # layered sets (wire format v2) carry the same four types (tests/test_gpu_layered.py); anything else is refused at once
     lv = W.layered_view(rs.bset)
     ls = bs.DeviceLayeredSet.from_host(lv["structs"], lv["layers"], lv["qn"], lv["dim"], np.zeros(rs.bset.n_blocks, np.uint64), DEV)
     ld = ls.desc
-    ld.dtype = bs.F32
+    ld.dtype = 4
     with pytest.raises(bs.BsError) as e:
         bs.layered_serialize(ld, 256, 1 << 20, 256, 1 << 24, 0)
     assert e.value.code == bs.ERR_UNSUPPORTED

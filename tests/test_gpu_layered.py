@@ -371,3 +371,186 @@ def test_engine_offload_prefetch_round_trip(chunk, n_staging):
     t = eng.prefetch_layered_async(host.data_ptr(), total, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, bs.current_stream())
     assert t.wait()["status"] == bs.ERR_CORRUPT
     eng.destroy()
+
+
+# ---- element types of layered sets (reading E-2) ------------------------------------------
+ELEM = {bs.F64: 8, bs.F32: 4, bs.C64: 8, bs.C128: 16}
+
+
+class TypedLayeredUp:
+    """The blocks of a set read as e-byte elements (the first e*n bytes of each block's storage; for 16-byte elements the
+    pool is laid out with twice the room).  The oracle and the CUDA path see the same host / device bytes."""
+
+    def __init__(self, bset, dtype, misalign=0):
+        e = ELEM[dtype]
+        pool, offs = W.fill_pool_host(bset)
+        if e == 16:
+            big = np.zeros(2 * pool.size + 2, np.float64)
+            offs = offs * 2
+            for o, n in zip(offs, bset.nelems):
+                src = pool[int(o) // 16: int(o) // 16 + int(n)]
+                big[int(o) // 8: int(o) // 8 + 2 * int(n)] = np.repeat(src, 2) * np.tile([1.0, -0.5], int(n))
+            pool = big
+        self.bset, self.dtype, self.e = bset, dtype, e
+        self.up = Uploaded(bset, pool, offs, misalign=misalign)
+        self.lv = lv = W.layered_view(bset)
+        self.dset = bs.DeviceLayeredSet.from_host(lv["structs"], lv["layers"], lv["qn"], lv["dim"], self.up.addr, DEV, dtype=dtype)
+        self.want = v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], host_addrs(pool, offs), dtype=dtype)
+        self.counts = (len(lv["structs"]), lv["dim"].shape[0], len(lv["layers"]), bset.n_blocks)
+
+    def workspace(self, cap):
+        return bs.Workspace(0, 0, max(cap, 1 << 16), DEV, layered=self.counts)
+
+
+def test_golden_v2_f32_stream_from_the_gpu():
+    """The hand-typed G6 bytes (tests/golden/g6_golden_stream_v2_f32.hex) out of the CUDA path, and back."""
+    import os
+    from tests.test_oracle_v2 import GOLD_F32, golden_set_f32
+    from tests.util import read_hex_fixture
+    structs, layers, qn, dim, blocks = golden_set_f32()
+    raw = np.zeros(4 * 64, np.uint8)
+    for k, b in enumerate(blocks):
+        raw[64 * k: 64 * k + b.nbytes] = b.view(np.uint8)
+    d_pool = torch.from_numpy(raw).to(DEV)
+    addr = (np.uint64(d_pool.data_ptr()) + np.arange(4, dtype=np.uint64) * np.uint64(64)).astype(np.uint64)
+    dset = bs.DeviceLayeredSet.from_host(structs, layers, qn, dim, addr, DEV, dtype=bs.F32)
+    ws = bs.Workspace(0, 0, 1 << 16, DEV, layered=(1, 2, 2, 4))
+    out = torch.full((1024,), 0xCD, dtype=torch.uint8, device=DEV)
+    bs.layered_serialize(dset.desc, out.data_ptr(), 1024, ws.ptr, ws.nbytes, ws.result_ptr, None, bs.current_stream())
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["total_bytes"] == 320 and res["dtype"] == bs.F32
+    gold = read_hex_fixture(GOLD_F32)
+    assert out.cpu().numpy()[:320].tobytes() == gold and (out.cpu().numpy()[320:] == 0xCD).all()
+    assert bs.layered_stream_info(gold)["dtype"] == bs.F32
+    o, pool, res = gpu_ldeserialize(out, 320, (1, 2, 2, 4), 1024)
+    ref = v2.deserialize(np.frombuffer(gold, np.uint8))
+    assert res["status"] == bs.OK and res["dtype"] == bs.F32 and (pool.cpu().numpy()[:1024] == ref["pool"][:1024]).all()
+
+
+@pytest.mark.parametrize("opts", [None, dict(variant=bs.VARIANT_LDG, tile_bytes=16384), dict(variant=bs.VARIANT_TMA, tile_bytes=32768)],
+                         ids=["default", "ldg", "tma32k"])
+@pytest.mark.parametrize("dtype", [bs.F32, bs.C64, bs.C128, bs.F64], ids=["f32", "c64", "c128", "f64"])
+def test_typed_layered_sets_match_the_oracle_and_round_trip(dtype, opts):
+    for bset in (W.make_set("tiny-ops+site", 11, D=48, S=10, M=2, N0=2, n_ops=20, n_site=2, dims="multinomial"),
+                 W.make_set("lognormal", 12, D=300, S=30, M=4, N0=3, n_ops=40, n_site=2, dims="lognormal", sigma=1.0)):
+        lu = TypedLayeredUp(bset, dtype)
+        total = len(lu.want)
+        got_t, res = gpu_lserialize(lu, total + 4096, opts)
+        assert res["status"] == bs.OK and res["total_bytes"] == total and res["dtype"] == dtype, res
+        got = got_t.cpu().numpy()
+        bad = np.nonzero(got[:total] != lu.want)[0]
+        assert bad.size == 0, f"first mismatch at stream byte {bad[0]}"
+        assert (got[total:] == 0xCD).all()
+        ws = lu.workspace(total)
+        assert bs.layered_serialized_size(lu.dset.desc, ws.ptr, ws.nbytes, bs.current_stream()) == \
+            v2.serialized_size(lu.lv["structs"], lu.lv["layers"], lu.lv["dim"], dtype)
+        ref = v2.deserialize(lu.want)
+        na, need = v2.counts(lu.want)
+        out, pool, res = gpu_ldeserialize(got_t, total, lu.counts, need, opts=opts)
+        assert res["status"] == bs.OK and res["pool_bytes"] == need and res["dtype"] == dtype, res
+        assert (pool.cpu().numpy()[:need] == ref["pool"][:need]).all()
+        h = out.to_host(*lu.counts)
+        assert (h["dim"] == lu.lv["dim"]).all() and (h["qn"] == lu.lv["qn"]).all()
+        assert (h["structs"]["layer_bytes"] == ref["structs"]["layer_bytes"]).all() and (h["layers"]["offset"] == ref["layers"]["offset"]).all()
+        out.dtype = dtype                     # fixpoint: serialize(deserialize(S)) == S
+        again = torch.full((total,), 0x11, dtype=torch.uint8, device=DEV)
+        bs.layered_serialize(out.desc, again.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, bs.current_stream())
+        assert ws.read_result()["status"] == bs.OK and (again.cpu().numpy() == lu.want).all()
+
+
+def test_typed_layered_sets_eight_byte_sources_ranges_engine_queue_and_packages():
+    bset = W.make_set("lognormal", 12, D=300, S=30, M=4, N0=3, n_ops=40, n_site=2, dims="lognormal", sigma=1.0)
+    cs = bs.current_stream()
+    for dtype in (bs.F32, bs.C128):
+        lu = TypedLayeredUp(bset, dtype, misalign=8)          # 8-byte-aligned sources take the slow path (D16)
+        total = len(lu.want)
+        got_t, res = gpu_lserialize(lu, total)
+        assert res["status"] == bs.OK and (got_t.cpu().numpy()[:total] == lu.want).all()
+        lu = TypedLayeredUp(bset, dtype)
+        ws = lu.workspace(total)
+        # concat(ranges) == the stream
+        out = torch.full((total,), 0xCD, dtype=torch.uint8, device=DEV)
+        cuts = list(range(0, total, 100000 * 16)) + [total]
+        for k, (lo, hi) in enumerate(zip(cuts[:-1], cuts[1:])):
+            bs.layered_serialize_range(lu.dset.desc, out[lo:].data_ptr(), lo, hi, k == 0, ws.ptr, ws.nbytes, ws.result_ptr, None, cs)
+        assert ws.read_result()["status"] == bs.OK and (out.cpu().numpy() == lu.want).all()
+        # engine + queue: the stream crosses PCIe with its element type; packages of it reassemble
+        c = lu.counts
+        eng = bs.Engine(max(c[0], c[2]), c[3], total, chunk_bytes=4 * 65536)
+        host = torch.empty(total, dtype=torch.uint8, pin_memory=True)
+        host.fill_(0x5A)
+        assert eng.offload_layered_async(lu.dset.desc, total, host.data_ptr(), total, cs).wait()["status"] == bs.OK
+        assert (host.numpy() == lu.want).all()
+        ref = v2.deserialize(lu.want)
+        na, need = v2.counts(lu.want)
+        lout = bs.DeviceLayeredSet.empty(*c, DEV, fill=0xAB)
+        pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+        st = eng.prefetch_layered_async(host.data_ptr(), total, lout.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, cs).wait()
+        torch.cuda.synchronize()
+        assert st["status"] == bs.OK and (pool.cpu().numpy()[:need] == ref["pool"][:need]).all()
+        eng.destroy()
+        q = bs.Queue(max(c[0], c[2]), c[3], total, chunk_bytes=4 * 65536)
+        host.fill_(0x5A)
+        pool.fill_(0xEE)
+        q.save_layered(5, lu.dset.desc, total, host.data_ptr(), total, cs)
+        q.load_layered(5, lout.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, cs)
+        assert q.wait(5)["status"] == bs.OK
+        torch.cuda.synchronize()
+        assert (host.numpy() == lu.want).all() and (pool.cpu().numpy()[:need] == ref["pool"][:need]).all()
+        q.destroy()
+        from oracle import pkg
+        cap = 32768
+        hb = v2.stream_info(lu.want)["header_bytes"]
+        n = pkg.count(hb, total, cap)
+        slots = torch.full((n * (64 + cap),), 0x5A, dtype=torch.uint8, device=DEV)
+        wsp = bs.Workspace(0, 0, total, DEV, layered=c, packages=True)
+        bs.layered_package_emit(lu.dset.desc, total, cap, 11, slots.data_ptr(), 64 + cap, n, None, wsp.ptr, wsp.nbytes,
+                                wsp.result_ptr, None, cs)
+        assert wsp.read_result()["status"] == bs.OK
+        assert (slots.cpu().numpy().reshape(n, -1) == pkg.emit_slots(lu.want, cap, 11, 64 + cap, poison=0x5A)).all()
+        pool.fill_(0xEE)
+        bs.layered_package_unpack(slots.data_ptr(), 64 + cap, n, 11, lout.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, wsp.ptr,
+                                  wsp.nbytes, wsp.result_ptr, None, cs)
+        assert wsp.read_result()["status"] == bs.OK and (pool.cpu().numpy()[:need] == ref["pool"][:need]).all()
+
+
+def test_typed_layered_sets_bad_types_and_nonzero_pads_are_rejected():
+    bset = W.make_set("few-ops", 13, D=64, S=12, M=2, N0=2, n_ops=5, n_site=1, dims="multinomial")
+    lu = TypedLayeredUp(bset, bs.F32)
+    d = bs.DeviceLayeredSet.from_host(lu.lv["structs"], lu.lv["layers"], lu.lv["qn"], lu.lv["dim"], lu.up.addr, DEV, dtype=4)
+    ws = lu.workspace(1 << 20)
+    with pytest.raises(bs.BsError) as e:
+        bs.layered_serialize(d.desc, 256, 1 << 20, ws.ptr, ws.nbytes, ws.result_ptr, None, bs.current_stream())
+    assert e.value.code == bs.ERR_UNSUPPORTED
+    na, need = v2.counts(lu.want)
+    bad = lu.want.copy()
+    bad[16] = 4                                   # dtype word
+    assert v2.validate_stream(bad) == oracle.ERR_CORRUPT
+    o, pool, res = gpu_ldeserialize(torch.from_numpy(bad).to(DEV), len(bad), lu.counts, need)
+    assert res["status"] == bs.ERR_CORRUPT and (pool == 0xEE).all()
+    # a non-zero pad byte of every pad length (4, 8, 12) — direct call and through the engine (checked while unpacking)
+    info = v2.stream_info(lu.want)
+    plan = v2.plan(lu.lv["structs"], lu.lv["layers"], lu.lv["dim"], bs.F32)
+    seen = set()
+    for k, srec in enumerate(lu.lv["structs"]):
+        layer0 = int(np.nonzero(lu.lv["layers"]["structure"] == k)[0][0])
+        for j in range(int(srec["first_block"]), int(srec["first_block"]) + int(srec["n_blocks"])):
+            nb = 4 * int(np.prod(lu.lv["dim"][j].astype(np.int64)))
+            pad = -nb % 16
+            if pad and pad not in seen:
+                seen.add(pad)
+                bad = lu.want.copy()
+                bad[info["header_bytes"] + int(plan["layer_offset"][layer0]) + int(plan["rel_offset"][j]) + nb + pad - 1] = 0x80
+                assert v2.validate_stream(bad) == oracle.ERR_CORRUPT
+                o, pool, res = gpu_ldeserialize(torch.from_numpy(bad).to(DEV), len(bad), lu.counts, need)
+                assert res["status"] == bs.ERR_CORRUPT and (pool == 0xEE).all(), (pad, res)
+                c = lu.counts
+                eng = bs.Engine(max(c[0], c[2]), c[3], len(bad), chunk_bytes=65536)
+                host = torch.empty(len(bad), dtype=torch.uint8, pin_memory=True)
+                host.numpy()[:] = bad
+                lout = bs.DeviceLayeredSet.empty(*c, DEV, fill=0xAB)
+                pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+                st = eng.prefetch_layered_async(host.data_ptr(), len(bad), lout.desc, pool.data_ptr(), need).wait()
+                assert st["status"] == bs.ERR_CORRUPT
+                eng.destroy()
+    assert seen == {4, 8, 12}

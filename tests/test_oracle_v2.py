@@ -362,3 +362,131 @@ def test_special_bit_patterns_survive():
     got = np.concatenate([out["pool"][int(a) - base:int(a) - base + 8 * b.size].view(np.uint64)
                           for a, b in zip(out["addr"], blocks)])
     assert (got == pats).all()
+
+
+# ---- element types of layered sets (reading E-2) ------------------------------------------
+GOLD_F32 = os.path.join(os.path.dirname(__file__), "golden", "g6_golden_stream_v2_f32.hex")
+GOLD_F32_SHA = "0b65fe5af21ebb09c2cd433fcad8b1c8621473af4220079b9e0789b1cb581921"
+ELEM = {0: 8, 1: 4, 2: 8, 3: 16}
+
+
+def golden_set_f32():
+    structs = np.zeros(1, dtype=W.STRUCT_REC_DTYPE)
+    structs[0] = (2, 0, 2, (0, 0), (-1, 1, 0, 0), 0)
+    layers = np.zeros(2, dtype=W.LAYER_REC_DTYPE)
+    layers[0] = (0, 9, 0)
+    layers[1] = (0, 11, 0)
+    qn = np.array([[[0, 0], [0, 0], [0, 0]], [[1, 1], [1, 1], [0, 0]]], dtype=np.int32)
+    dim = np.array([[1, 3, 1], [1, 1, 1]], dtype=np.uint32)
+    blocks = [np.array([1, 2, 3], np.float32), np.array([-1], np.float32), np.array([4, 5, 6], np.float32),
+              np.array([-2], np.float32)]
+    return structs, layers, qn, dim, blocks
+
+
+def test_G6_f32_fixture_and_oracle_reproduces_it():
+    raw = read_hex_fixture(GOLD_F32)
+    assert len(raw) == 320 and sha256(raw) == GOLD_F32_SHA
+    structs, layers, qn, dim, blocks = golden_set_f32()
+    addr = np.array([b.ctypes.data for b in blocks], dtype=np.uint64)
+    s = v2.serialize(structs, layers, qn, dim, addr, dtype=1)
+    assert bytes(s) == raw
+    assert v2.serialized_size(structs, layers, dim, dtype=1) == (256, 320)
+    # the independent struct reader sees the stated fields
+    fixed, st, ly, bl, slack, payload = read_stream_v2(raw)
+    assert fixed["dtype"] == 1 and fixed["payload_bytes"] == 64
+    assert st[0]["layer_bytes"] == 32 and [l["offset"] for l in ly] == [0, 32] and [b["offset"] for b in bl] == [0, 16]
+    assert np.frombuffer(payload, np.float32).tolist() == [1, 2, 3, 0, -1, 0, 0, 0, 4, 5, 6, 0, -2, 0, 0, 0]
+    # and back: pool slots are align256(nbytes), the bytes behind a block keep their poison
+    arr = np.frombuffer(raw, np.uint8)
+    assert v2.validate_stream(arr) == oracle.OK and v2.stream_info(arr)["dtype"] == 1
+    out = v2.deserialize(arr)
+    base = out["pool"].ctypes.data
+    assert [int(a) - base for a in out["addr"]] == [0, 256, 512, 768] and v2.counts(arr) == (4, 1024)
+    assert out["pool"][0:12].view(np.float32).tolist() == [1, 2, 3] and out["pool"][768:772].view(np.float32)[0] == -2
+    assert (out["pool"][12:256] == 0xEE).all() and (out["pool"][772:1024] == 0xEE).all()
+
+
+def _typed_blocks(bset, pool, offs, e):
+    """Block i read as e-byte elements: the first e*n bytes of its fp64 storage (c128: the set's storage is too short, so the
+    values are taken from a pool of twice the size built by the caller)."""
+    raw = pool.view(np.uint8)
+    return [raw[int(o): int(o) + e * int(n)] for o, n in zip(offs, bset.nelems)]
+
+
+@pytest.mark.parametrize("dtype", [0, 1, 2, 3])
+@pytest.mark.parametrize("bset", list(small_sets()), ids=lambda s: s.name)
+def test_typed_payload_equals_the_independent_v1_dtype_oracle(bset, dtype):
+    """The v2 payload of a typed layered set == the payload of the (independently written, separately pinned) numpy oracle
+    of wire format v1 for the same element type on the expanded set; offsets against numpy.cumsum of e-sized blocks."""
+    from oracle import dt
+    e = ELEM[dtype]
+    pool, offs = W.fill_pool_host(bset)
+    if e == 16:    # room for 16-byte elements: every block twice as long, same seeded values twice
+        big = np.zeros(2 * pool.size + 2, np.float64)
+        offs = offs * 2
+        for o, n in zip(offs, bset.nelems):
+            src = pool[int(o) // 16: int(o) // 16 + int(n)]
+            big[int(o) // 8: int(o) // 8 + 2 * int(n)] = np.repeat(src, 2)
+        pool = big
+    lv = W.layered_view(bset)
+    s2 = v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], host_addrs(pool, offs), dtype=dtype)
+    s1 = dt.serialize(bset.tensors, bset.qn, bset.dim, _typed_blocks(bset, pool, offs, e), dtype)
+    i2 = v2.stream_info(s2)
+    hb1 = dt.header_bytes(bset.n_tensors, bset.n_blocks)
+    assert i2["dtype"] == dtype and i2["payload_bytes"] == len(s1) - hb1
+    assert (s2[i2["header_bytes"]:] == s1[hb1:]).all()
+    # offsets: numpy.cumsum over align16(e * n), per structure and per layer
+    plan = v2.plan(lv["structs"], lv["layers"], lv["dim"], dtype)
+    d = lv["dim"].astype(np.uint64)
+    st = (np.uint64(e) * d[:, 0] * d[:, 1] * d[:, 2] + np.uint64(15)) // np.uint64(16) * np.uint64(16)
+    for k, srec in enumerate(lv["structs"]):
+        f, n = int(srec["first_block"]), int(srec["n_blocks"])
+        want = np.concatenate([[0], np.cumsum(st[f:f + n])])
+        assert plan["rel_offset"][f:f + n].tolist() == want[:-1].tolist() and int(plan["layer_bytes"][k]) == int(want[-1])
+    lb = plan["layer_bytes"][lv["layers"]["structure"]]
+    assert plan["layer_offset"].tolist() == np.concatenate([[0], np.cumsum(lb)])[:-1].tolist()
+    assert v2.serialized_size(lv["structs"], lv["layers"], lv["dim"], dtype)[1] == len(s2)
+    # round trip, fixpoint, pool layout (slots of align256(e * n), untouched bytes keep their poison)
+    out = v2.deserialize(s2)
+    base = out["pool"].ctypes.data
+    slots = (np.uint64(e) * bset.nelems + np.uint64(255)) // np.uint64(256) * np.uint64(256)
+    assert (out["addr"] - np.uint64(base)).tolist() == np.concatenate([[0], np.cumsum(slots)])[:-1].tolist()
+    for a, blk, sl in zip(out["addr"], _typed_blocks(bset, pool, offs, e), slots):
+        o = int(a) - base
+        assert (out["pool"][o: o + len(blk)] == blk).all() and (out["pool"][o + len(blk): o + int(sl)] == 0xEE).all()
+    again = v2.serialize(out["structs"], out["layers"], out["qn"], out["dim"], out["addr"], dtype=dtype)
+    assert (again == s2).all()
+
+
+def test_c64_stream_is_the_f64_stream_but_for_the_dtype_word_and_bad_types_are_refused():
+    bset = W.make_set("few-ops", 13, D=64, S=12, M=2, N0=2, n_ops=5, n_site=1, dims="multinomial")
+    pool, offs = W.fill_pool_host(bset)
+    lv = W.layered_view(bset)
+    a = v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], host_addrs(pool, offs), dtype=0)
+    b = v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], host_addrs(pool, offs), dtype=2)
+    assert a[16] == 0 and b[16] == 2
+    b2 = b.copy()
+    b2[16] = 0
+    assert (a == b2).all()
+    with pytest.raises(oracle.OracleError) as e:
+        v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], host_addrs(pool, offs), dtype=4)
+    assert e.value.code == oracle.ERR_UNSUPPORTED
+    bad = a.copy()
+    bad[16] = 4
+    assert v2.validate_stream(bad) == oracle.ERR_CORRUPT
+    # an f32 stream: every pad length occurs and a non-zero pad byte of each is refused
+    f = v2.serialize(lv["structs"], lv["layers"], lv["qn"], lv["dim"], host_addrs(pool, offs), dtype=1)
+    info = v2.stream_info(f)
+    plan = v2.plan(lv["structs"], lv["layers"], lv["dim"], 1)
+    seen = set()
+    for k, srec in enumerate(lv["structs"]):
+        layer0 = int(np.nonzero(lv["layers"]["structure"] == k)[0][0])
+        for j in range(int(srec["first_block"]), int(srec["first_block"]) + int(srec["n_blocks"])):
+            nb = 4 * int(np.prod(lv["dim"][j].astype(np.int64)))
+            pad = -nb % 16
+            if pad and pad not in seen:
+                seen.add(pad)
+                bad = f.copy()
+                bad[info["header_bytes"] + int(plan["layer_offset"][layer0]) + int(plan["rel_offset"][j]) + nb] = 1
+                assert v2.validate_stream(bad) == oracle.ERR_CORRUPT
+    assert seen == {4, 8, 12}
