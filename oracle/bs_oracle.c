@@ -32,6 +32,17 @@
  * Unpinned: nothing in this file.  (The paper's GB/s figures are "parity unpinned": no number in
  * the paper is tied to a byte format.)
  *
+ * Reading D19 (round 2; SURVEY §8(c) D3 kept `align` as a header field "so a future align=8 (no pad, literal unpadded
+ * reading) is representable"; SURVEY §8(f) NEXT-4 "align = 8 unpadded streams"; BASELINE.json north_star: "offsets equal to
+ * the exclusive prefix sum of the block byte sizes"): the header's align word is 16 or 8 and is the ONLY thing that
+ * changes — stored_i = align_up(nbytes_i, align), offset_i = the exclusive prefix sum of stored_i, payload_bytes = their sum.
+ * With align = 8 an fp64 block is stored without any pad byte, offsets are the literal prefix sum of the block byte sizes,
+ * and the stream's total is a multiple of 8 (not of 16).  Every function that took no alignment keeps its round-1 meaning
+ * (16) and has an `_al` twin that takes it; the readers take it from the header.  Pins (tests/test_oracle_align8.py): G7
+ * hand-typed 280-byte golden stream (the P7 example unpadded: offsets 0, 8); offsets vs numpy.cumsum of the unpadded sizes;
+ * byte equality with the independently written numpy oracle (bs_oracle_dtype.py) at align 8; payload == the plain
+ * concatenation of the blocks; round trip, fixpoint, fault injection.
+ *
  * All integers little-endian; the host is assumed little-endian (checked in orc_selftest_endian).
  */
 #include <stdint.h>
@@ -81,17 +92,19 @@ uint64_t orc_header_bytes(uint64_t T, uint64_t B)
 }
 
 /* ---- serialize, step 2: the "pointer structure" (L90-92): sizes, stored sizes, offsets ------ */
-/* nbytes[i] = 8*prod(dim[i]);  stored[i] = align16(nbytes[i]);  offset[i] = sum_{j<i} stored[j] */
-int orc_plan(uint64_t B, const uint32_t *dim /*[B][3]*/, uint64_t *nbytes, uint64_t *stored,
-             uint64_t *offset, uint64_t *payload_bytes)
+/* nbytes[i] = 8*prod(dim[i]);  stored[i] = align_up(nbytes[i], align);  offset[i] = sum_{j<i} stored[j];
+ * align = 16 (wire format v1 as round 1 defined it) or 8 (reading D19: unpadded for fp64) */
+int orc_plan_al(uint64_t B, const uint32_t *dim /*[B][3]*/, uint32_t align, uint64_t *nbytes, uint64_t *stored,
+                uint64_t *offset, uint64_t *payload_bytes)
 {
     uint64_t run = 0;
+    if (align != 16u && align != 8u) return ORC_ERR_UNSUPPORTED;
     for (uint64_t i = 0; i < B; ++i) {
         uint64_t d0 = dim[3 * i + 0], d1 = dim[3 * i + 1], d2 = dim[3 * i + 2];
         uint64_t n01 = d0 * d1;                         /* < 2^64 always (u32*u32) */
         if (d2 != 0 && n01 > (UINT64_MAX / 8u) / d2) return ORC_ERR_ARG;
         uint64_t nb = 8u * n01 * d2;
-        uint64_t st = align_up(nb, ORC_BLOCK_ALIGN);
+        uint64_t st = align_up(nb, align);
         if (nbytes) nbytes[i] = nb;
         if (stored) stored[i] = st;
         if (offset) offset[i] = run;
@@ -101,15 +114,27 @@ int orc_plan(uint64_t B, const uint32_t *dim /*[B][3]*/, uint64_t *nbytes, uint6
     return ORC_OK;
 }
 
-int orc_serialized_size(uint64_t T, uint64_t B, const uint32_t *dim, uint64_t *header_bytes,
-                        uint64_t *total_bytes)
+int orc_plan(uint64_t B, const uint32_t *dim /*[B][3]*/, uint64_t *nbytes, uint64_t *stored,
+             uint64_t *offset, uint64_t *payload_bytes)
+{
+    return orc_plan_al(B, dim, ORC_BLOCK_ALIGN, nbytes, stored, offset, payload_bytes);
+}
+
+int orc_serialized_size_al(uint64_t T, uint64_t B, const uint32_t *dim, uint32_t align, uint64_t *header_bytes,
+                           uint64_t *total_bytes)
 {
     uint64_t P;
-    int rc = orc_plan(B, dim, NULL, NULL, NULL, &P);
+    int rc = orc_plan_al(B, dim, align, NULL, NULL, NULL, &P);
     if (rc) return rc;
     *header_bytes = orc_header_bytes(T, B);
     *total_bytes = *header_bytes + P;
     return ORC_OK;
+}
+
+int orc_serialized_size(uint64_t T, uint64_t B, const uint32_t *dim, uint64_t *header_bytes,
+                        uint64_t *total_bytes)
+{
+    return orc_serialized_size_al(T, B, dim, ORC_BLOCK_ALIGN, header_bytes, total_bytes);
 }
 
 /* the descriptor must partition the block table into tensors in order (D5, D8) */
@@ -127,14 +152,14 @@ static int check_descriptor(uint64_t T, uint64_t B, const orc_tensor *t)
 }
 
 /* ---- serialize, step 3: fixed header, tensor records, block records, zero slack ------------- */
-int orc_emit_header(uint64_t T, uint64_t B, const orc_tensor *tensors, const int32_t *qn /*[B][3][2]*/,
-                    const uint32_t *dim /*[B][3]*/, unsigned char *out, uint64_t capacity)
+int orc_emit_header_al(uint64_t T, uint64_t B, const orc_tensor *tensors, const int32_t *qn /*[B][3][2]*/,
+                       const uint32_t *dim /*[B][3]*/, uint32_t align, unsigned char *out, uint64_t capacity)
 {
     int rc = check_descriptor(T, B, tensors);
     if (rc) return rc;
     uint64_t hb = orc_header_bytes(T, B), P;
     if (capacity < hb) return ORC_ERR_CAPACITY;
-    rc = orc_plan(B, dim, NULL, NULL, NULL, &P);
+    rc = orc_plan_al(B, dim, align, NULL, NULL, NULL, &P);
     if (rc) return rc;
 
     unsigned char *p = out;
@@ -144,7 +169,7 @@ int orc_emit_header(uint64_t T, uint64_t B, const orc_tensor *tensors, const int
     put_u32(p + 16, 0u);             /* dtype f64 */
     put_u32(p + 20, 2u);             /* n_qn */
     put_u32(p + 24, 3u);             /* max_rank */
-    put_u32(p + 28, 16u);            /* align */
+    put_u32(p + 28, align);          /* align: 16, or 8 (reading D19) */
     put_u64(p + 32, T);
     put_u64(p + 40, B);
     put_u64(p + 48, hb);
@@ -172,7 +197,7 @@ int orc_emit_header(uint64_t T, uint64_t B, const orc_tensor *tensors, const int
             put_u32(p + 32, dim[3 * i + 2]);
             put_u32(p + 36, (uint32_t)k);               /* owning tensor (L124) */
             put_u64(p + 40, run);                       /* offset inside the payload */
-            run += align_up(8ull * dim[3 * i + 0] * dim[3 * i + 1] * dim[3 * i + 2], ORC_BLOCK_ALIGN);
+            run += align_up(8ull * dim[3 * i + 0] * dim[3 * i + 1] * dim[3 * i + 2], align);
             p += ORC_BLOCK_REC;
         }
     }
@@ -180,22 +205,29 @@ int orc_emit_header(uint64_t T, uint64_t B, const orc_tensor *tensors, const int
     return ORC_OK;
 }
 
+int orc_emit_header(uint64_t T, uint64_t B, const orc_tensor *tensors, const int32_t *qn /*[B][3][2]*/,
+                    const uint32_t *dim /*[B][3]*/, unsigned char *out, uint64_t capacity)
+{
+    return orc_emit_header_al(T, B, tensors, qn, dim, ORC_BLOCK_ALIGN, out, capacity);
+}
+
 /* ---- serialize, step 4 for blocks of tensors [t0,t1): copy, then pad with zeros ------------- */
 /* Writes payload bytes [offset(first block of t0), offset(end of t1-1)) to out[0..).  addr[i] is
  * the host address of block i for i in that range (other entries are not read). */
-int orc_emit_payload_range(uint64_t T, uint64_t B, const orc_tensor *tensors, const uint32_t *dim,
-                           const uint64_t *addr, uint64_t t0, uint64_t t1, unsigned char *out,
-                           uint64_t capacity, uint64_t *first_offset, uint64_t *range_bytes)
+int orc_emit_payload_range_al(uint64_t T, uint64_t B, const orc_tensor *tensors, const uint32_t *dim,
+                              const uint64_t *addr, uint32_t align, uint64_t t0, uint64_t t1, unsigned char *out,
+                              uint64_t capacity, uint64_t *first_offset, uint64_t *range_bytes)
 {
     int rc = check_descriptor(T, B, tensors);
     if (rc) return rc;
+    if (align != 16u && align != 8u) return ORC_ERR_UNSUPPORTED;
     if (t0 > t1 || t1 > T) return ORC_ERR_ARG;
     uint64_t b0 = (t0 < T) ? tensors[t0].first_block : B;
     uint64_t b1 = (t1 < T) ? tensors[t1].first_block : B;
     uint64_t run = 0, start = 0;
     for (uint64_t i = 0; i < b1; ++i) {
         uint64_t nb = 8ull * dim[3 * i + 0] * dim[3 * i + 1] * dim[3 * i + 2];
-        uint64_t st = align_up(nb, ORC_BLOCK_ALIGN);
+        uint64_t st = align_up(nb, align);
         if (i == b0) start = run;
         if (i >= b0) {
             if (run - start + st > capacity) return ORC_ERR_CAPACITY;
@@ -210,24 +242,38 @@ int orc_emit_payload_range(uint64_t T, uint64_t B, const orc_tensor *tensors, co
     return ORC_OK;
 }
 
+int orc_emit_payload_range(uint64_t T, uint64_t B, const orc_tensor *tensors, const uint32_t *dim,
+                           const uint64_t *addr, uint64_t t0, uint64_t t1, unsigned char *out,
+                           uint64_t capacity, uint64_t *first_offset, uint64_t *range_bytes)
+{
+    return orc_emit_payload_range_al(T, B, tensors, dim, addr, ORC_BLOCK_ALIGN, t0, t1, out, capacity, first_offset, range_bytes);
+}
+
 /* ---- serialize, steps 1-5 --------------------------------------------------------------------- */
-int orc_serialize(uint64_t T, uint64_t B, const orc_tensor *tensors, const int32_t *qn,
-                  const uint32_t *dim, const uint64_t *addr, unsigned char *out, uint64_t capacity,
-                  uint64_t *written)
+int orc_serialize_al(uint64_t T, uint64_t B, const orc_tensor *tensors, const int32_t *qn,
+                     const uint32_t *dim, const uint64_t *addr, uint32_t align, unsigned char *out, uint64_t capacity,
+                     uint64_t *written)
 {
     uint64_t hb, total, first, pb;
     int rc = check_descriptor(T, B, tensors);
     if (rc) return rc;
-    rc = orc_serialized_size(T, B, dim, &hb, &total);           /* steps 1-2 */
+    rc = orc_serialized_size_al(T, B, dim, align, &hb, &total);          /* steps 1-2 */
     if (rc) return rc;
-    *written = total;                                            /* required size, also on failure */
+    *written = total;                                                     /* required size, also on failure */
     if (capacity < total) return ORC_ERR_CAPACITY;
-    rc = orc_emit_header(T, B, tensors, qn, dim, out, capacity); /* step 3 */
+    rc = orc_emit_header_al(T, B, tensors, qn, dim, align, out, capacity); /* step 3 */
     if (rc) return rc;
-    rc = orc_emit_payload_range(T, B, tensors, dim, addr, 0, T, out + hb, capacity - hb, &first, &pb);  /* step 4 */
+    rc = orc_emit_payload_range_al(T, B, tensors, dim, addr, align, 0, T, out + hb, capacity - hb, &first, &pb);  /* step 4 */
     if (rc) return rc;
-    if (first != 0 || hb + pb != total) return ORC_ERR_ARG;      /* step 5: prediction == written */
+    if (first != 0 || hb + pb != total) return ORC_ERR_ARG;               /* step 5: prediction == written */
     return ORC_OK;
+}
+
+int orc_serialize(uint64_t T, uint64_t B, const orc_tensor *tensors, const int32_t *qn,
+                  const uint32_t *dim, const uint64_t *addr, unsigned char *out, uint64_t capacity,
+                  uint64_t *written)
+{
+    return orc_serialize_al(T, B, tensors, qn, dim, addr, ORC_BLOCK_ALIGN, out, capacity, written);
 }
 
 /* ---- stream_info: the fixed header alone ----------------------------------------------------- */
@@ -241,13 +287,23 @@ int orc_stream_info(const unsigned char *s, uint64_t n, uint64_t *T, uint64_t *B
     if (get_u32(s + 16) != 0u) return ORC_ERR_CORRUPT;
     if (get_u32(s + 20) != 2u) return ORC_ERR_CORRUPT;
     if (get_u32(s + 24) != 3u) return ORC_ERR_CORRUPT;
-    if (get_u32(s + 28) != 16u) return ORC_ERR_CORRUPT;
+    if (get_u32(s + 28) != 16u && get_u32(s + 28) != 8u) return ORC_ERR_CORRUPT;   /* align (reading D19) */
     *T = get_u64(s + 32);
     *B = get_u64(s + 40);
     *header_bytes = get_u64(s + 48);
     *payload_bytes = get_u64(s + 56);
     if (*T >= (1ull << 32) || *B >= (1ull << 32)) return ORC_ERR_CORRUPT;
     if (*header_bytes != orc_header_bytes(*T, *B)) return ORC_ERR_CORRUPT;
+    return ORC_OK;
+}
+
+/* the align word of a stream whose fixed header orc_stream_info accepts */
+int orc_stream_align(const unsigned char *s, uint64_t n, uint32_t *align)
+{
+    uint64_t T, B, hb, P;
+    int rc = orc_stream_info(s, n, &T, &B, &hb, &P);
+    if (rc) return rc;
+    *align = get_u32(s + 28);
     return ORC_OK;
 }
 
@@ -258,6 +314,7 @@ int orc_validate_stream(const unsigned char *s, uint64_t n)
     int rc = orc_stream_info(s, n, &T, &B, &hb, &P);
     if (rc) return rc;
     if (hb > n || hb + P != n) return ORC_ERR_CORRUPT;
+    const uint32_t align = get_u32(s + 28);
     const unsigned char *trec = s + ORC_FIXED_HEADER;
     const unsigned char *brec = trec + ORC_TENSOR_REC * T;
     uint64_t next = 0, run = 0;
@@ -280,7 +337,7 @@ int orc_validate_stream(const unsigned char *s, uint64_t n)
             if (d2 != 0 && n01 > (UINT64_MAX / 8u) / d2) return ORC_ERR_CORRUPT;
             uint64_t nbytes = 8u * n01 * d2;
             if (get_u64(b + 40) != run) return ORC_ERR_CORRUPT;           /* offsets = exclusive sum */
-            uint64_t st = align_up(nbytes, ORC_BLOCK_ALIGN);
+            uint64_t st = align_up(nbytes, align);
             if (st < nbytes || run + st < run || run + st > P) return ORC_ERR_CORRUPT;
             for (uint64_t z = nbytes; z < st; ++z)                         /* pad bytes are zero */
                 if (s[hb + run + z] != 0) return ORC_ERR_CORRUPT;

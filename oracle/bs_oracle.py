@@ -55,11 +55,12 @@ def _L():
         pu64 = C.POINTER(C.c_uint64)
         lib.orc_header_bytes.restype = u64
         lib.orc_header_bytes.argtypes = [u64, u64]
-        lib.orc_plan.argtypes = [u64, vp, vp, vp, vp, pu64]
-        lib.orc_serialized_size.argtypes = [u64, u64, vp, pu64, pu64]
-        lib.orc_emit_header.argtypes = [u64, u64, vp, vp, vp, vp, u64]
-        lib.orc_emit_payload_range.argtypes = [u64, u64, vp, vp, vp, u64, u64, vp, u64, pu64, pu64]
-        lib.orc_serialize.argtypes = [u64, u64, vp, vp, vp, vp, vp, u64, pu64]
+        lib.orc_plan_al.argtypes = [u64, vp, u32, vp, vp, vp, pu64]
+        lib.orc_serialized_size_al.argtypes = [u64, u64, vp, u32, pu64, pu64]
+        lib.orc_emit_header_al.argtypes = [u64, u64, vp, vp, vp, u32, vp, u64]
+        lib.orc_emit_payload_range_al.argtypes = [u64, u64, vp, vp, vp, u32, u64, u64, vp, u64, pu64, pu64]
+        lib.orc_serialize_al.argtypes = [u64, u64, vp, vp, vp, vp, u32, vp, u64, pu64]
+        lib.orc_stream_align.argtypes = [vp, u64, C.POINTER(u32)]
         lib.orc_stream_info.argtypes = [vp, u64, pu64, pu64, pu64, pu64]
         lib.orc_validate_stream.argtypes = [vp, u64]
         lib.orc_pool_bytes.argtypes = [vp, u64, pu64]
@@ -91,40 +92,40 @@ def header_bytes(T: int, B: int) -> int:
     return int(_L().orc_header_bytes(T, B))
 
 
-def plan(dim):
-    """(nbytes, stored, offset, payload_bytes) of SURVEY §8(c) serialize step 2."""
+def plan(dim, align: int = 16):
+    """(nbytes, stored, offset, payload_bytes) of SURVEY §8(c) serialize step 2.  align: 16, or 8 (reading D19: unpadded)."""
     dim = _c(dim, np.uint32, (3,))
     B = dim.shape[0]
     nbytes = np.zeros(B, np.uint64)
     stored = np.zeros(B, np.uint64)
     offset = np.zeros(B, np.uint64)
     P = C.c_uint64(0)
-    rc = _L().orc_plan(B, _p(dim), _p(nbytes), _p(stored), _p(offset), C.byref(P))
+    rc = _L().orc_plan_al(B, _p(dim), align, _p(nbytes), _p(stored), _p(offset), C.byref(P))
     if rc:
         raise OracleError(rc, "plan")
     return nbytes, stored, offset, int(P.value)
 
 
-def serialized_size(n_tensors: int, dim):
+def serialized_size(n_tensors: int, dim, align: int = 16):
     dim = _c(dim, np.uint32, (3,))
     hb, tot = C.c_uint64(0), C.c_uint64(0)
-    rc = _L().orc_serialized_size(n_tensors, dim.shape[0], _p(dim), C.byref(hb), C.byref(tot))
+    rc = _L().orc_serialized_size_al(n_tensors, dim.shape[0], _p(dim), align, C.byref(hb), C.byref(tot))
     if rc:
         raise OracleError(rc, "serialized_size")
     return int(hb.value), int(tot.value)
 
 
-def emit_header(tensors, qn, dim) -> np.ndarray:
+def emit_header(tensors, qn, dim, align: int = 16) -> np.ndarray:
     tensors, qn, dim = _tensors(tensors), _c(qn, np.int32, (3, 2)), _c(dim, np.uint32, (3,))
     T, B = len(tensors), dim.shape[0]
     out = np.full(header_bytes(T, B), 0xCD, dtype=np.uint8)   # poisoned: every byte must be written
-    rc = _L().orc_emit_header(T, B, _p(tensors), _p(qn), _p(dim), _p(out), out.size)
+    rc = _L().orc_emit_header_al(T, B, _p(tensors), _p(qn), _p(dim), align, _p(out), out.size)
     if rc:
         raise OracleError(rc, "emit_header")
     return out
 
 
-def emit_payload_range(tensors, dim, addr, t0: int, t1: int, capacity: int, out: np.ndarray | None = None):
+def emit_payload_range(tensors, dim, addr, t0: int, t1: int, capacity: int, out: np.ndarray | None = None, align: int = 16):
     """Payload bytes of tensors [t0, t1).  Returns (first_offset, bytes ndarray).  ``out``: a caller buffer of at least
     ``capacity`` bytes to write into (e.g. a slice of one large stream buffer) instead of a fresh poisoned one."""
     tensors, dim = _tensors(tensors), _c(dim, np.uint32, (3,))
@@ -133,24 +134,24 @@ def emit_payload_range(tensors, dim, addr, t0: int, t1: int, capacity: int, out:
         out = np.full(max(capacity, 1), 0xCD, dtype=np.uint8)
     assert out.dtype == np.uint8 and out.flags["C_CONTIGUOUS"] and out.size >= capacity
     first, nb = C.c_uint64(0), C.c_uint64(0)
-    rc = _L().orc_emit_payload_range(len(tensors), dim.shape[0], _p(tensors), _p(dim), _p(addr), t0, t1,
-                                     _p(out), capacity, C.byref(first), C.byref(nb))
+    rc = _L().orc_emit_payload_range_al(len(tensors), dim.shape[0], _p(tensors), _p(dim), _p(addr), align, t0, t1,
+                                        _p(out), capacity, C.byref(first), C.byref(nb))
     if rc:
         raise OracleError(rc, "emit_payload_range")
     return int(first.value), out[: int(nb.value)]
 
 
-def serialize(tensors, qn, dim, addr, capacity: int | None = None, out: np.ndarray | None = None) -> np.ndarray:
-    """The whole stream.  ``addr`` holds HOST addresses (uint64) of the dense row-major blocks."""
+def serialize(tensors, qn, dim, addr, capacity: int | None = None, out: np.ndarray | None = None, align: int = 16) -> np.ndarray:
+    """The whole stream.  ``addr`` holds HOST addresses (uint64) of the dense row-major blocks.  align: 16 or 8 (D19)."""
     tensors, qn, dim = _tensors(tensors), _c(qn, np.int32, (3, 2)), _c(dim, np.uint32, (3,))
     addr = _c(addr, np.uint64)
     T, B = len(tensors), dim.shape[0]
     if capacity is None:
-        capacity = serialized_size(T, dim)[1]
+        capacity = serialized_size(T, dim, align)[1]
     if out is None:
         out = np.full(max(capacity, 1), 0xCD, dtype=np.uint8)
     written = C.c_uint64(0)
-    rc = _L().orc_serialize(T, B, _p(tensors), _p(qn), _p(dim), _p(addr), _p(out), capacity, C.byref(written))
+    rc = _L().orc_serialize_al(T, B, _p(tensors), _p(qn), _p(dim), _p(addr), align, _p(out), capacity, C.byref(written))
     if rc:
         e = OracleError(rc, "serialize")
         e.required = int(written.value)
@@ -164,8 +165,10 @@ def stream_info(stream: np.ndarray):
     rc = _L().orc_stream_info(_p(s), s.size, C.byref(T), C.byref(B), C.byref(hb), C.byref(P))
     if rc:
         raise OracleError(rc, "stream_info")
+    al = C.c_uint32(0)
+    _L().orc_stream_align(_p(s), s.size, C.byref(al))
     return dict(n_tensors=int(T.value), n_blocks=int(B.value), header_bytes=int(hb.value),
-                payload_bytes=int(P.value))
+                payload_bytes=int(P.value), align=int(al.value))
 
 
 def validate_stream(stream: np.ndarray) -> int:

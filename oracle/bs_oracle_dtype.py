@@ -15,6 +15,11 @@ for dtype 0 the two are a cross-check of each other.  Pins (tests/test_oracle_dt
 (separately pinned) C oracle for f64; a hand-typed golden f32 stream; c128 payload == the C oracle's f64 payload of the
 set with its last extent doubled; c64 stream == the f64 stream but for the dtype word; round trip; fault injection.
 Unpinned: nothing.
+
+Round 2, reading D19 (see bs_oracle.c): ``align`` is 16 or 8 — stored_i = align_up(nbytes_i, align) and nothing else
+changes.  With align = 8 an f32 block carries 0 or 4 zero pad bytes and every other type none; the payload is then the
+plain concatenation of the stored blocks and the stream's total a multiple of 8.  Pins (tests/test_oracle_align8.py):
+G7 hand-typed golden stream, byte equality with the C oracle for f64, offsets against numpy.cumsum, round trip.
 """
 from __future__ import annotations
 
@@ -36,16 +41,18 @@ def header_bytes(T: int, B: int) -> int:
     return _align(64 + 32 * T + 48 * B, 128)
 
 
-def plan(dim, dtype: int):
+def plan(dim, dtype: int, align: int = 16):
     """nbytes, stored, offset per block and the payload size (the "pointer structure", L90-92)."""
     if dtype not in ELEM_BYTES:
         raise OracleError(ERR_UNSUPPORTED, "dtype")
+    if align not in (8, 16):
+        raise OracleError(ERR_UNSUPPORTED, "align")
     e = ELEM_BYTES[dtype]
     nbytes, stored, offset = [], [], []
     run = 0
     for d in np.asarray(dim, dtype=np.uint64).reshape(-1, 3):
         nb = e * int(d[0]) * int(d[1]) * int(d[2])
-        st = _align(nb, 16)
+        st = _align(nb, align)
         nbytes.append(nb)
         stored.append(st)
         offset.append(run)
@@ -53,12 +60,12 @@ def plan(dim, dtype: int):
     return nbytes, stored, offset, run
 
 
-def serialize(tensors, qn, dim, blocks, dtype: int) -> np.ndarray:
+def serialize(tensors, qn, dim, blocks, dtype: int, align: int = 16) -> np.ndarray:
     """blocks[i] = the raw bytes of block i (any object with the buffer protocol, exactly nbytes_i long)."""
     T, B = len(tensors), len(blocks)
     dim = np.asarray(dim, dtype=np.uint32).reshape(-1, 3)
     qn = np.asarray(qn, dtype=np.int32).reshape(-1, 3, 2)
-    nbytes, stored, offset, P = plan(dim, dtype)
+    nbytes, stored, offset, P = plan(dim, dtype, align)
     first = 0
     for t in tensors:                                    # tensors partition the block table in order
         if int(t["rank"]) not in (2, 3):
@@ -70,7 +77,7 @@ def serialize(tensors, qn, dim, blocks, dtype: int) -> np.ndarray:
         raise OracleError(ERR_ARG, "partition")
     hb = header_bytes(T, B)
     out = bytearray(hb + P)
-    struct.pack_into("<8sIIIIII QQQQ", out, 0, b"BSPARSE1", 1, 0x01020304, dtype, 2, 3, 16, T, B, hb, P)
+    struct.pack_into("<8sIIIIII QQQQ", out, 0, b"BSPARSE1", 1, 0x01020304, dtype, 2, 3, align, T, B, hb, P)
     pos = 64
     for t in tensors:
         out[pos:pos + 32] = np.asarray(t).tobytes()      # tensor records travel byte for byte
@@ -96,7 +103,7 @@ def deserialize(stream) -> dict:
         raise OracleError(ERR_CORRUPT, "short")
     magic, ver, endian, dtype, n_qn, max_rank, align, T, B, hb, P = struct.unpack_from("<8sIIIIII QQQQ", s, 0)
     if magic != b"BSPARSE1" or ver != 1 or endian != 0x01020304 or dtype not in ELEM_BYTES or n_qn != 2 or max_rank != 3 \
-            or align != 16 or T >= 1 << 32 or B >= 1 << 32 or hb != header_bytes(T, B) or hb > n or hb + P != n:
+            or align not in (8, 16) or T >= 1 << 32 or B >= 1 << 32 or hb != header_bytes(T, B) or hb > n or hb + P != n:
         raise OracleError(ERR_CORRUPT, "fixed header")
     e = ELEM_BYTES[dtype]
     recs = []
@@ -121,7 +128,7 @@ def deserialize(stream) -> dict:
             nbytes = e * d[0] * d[1] * d[2]
             if owner != k or off != run or (rank == 2 and (d[2] != 1 or q[4] != 0 or q[5] != 0)):
                 raise OracleError(ERR_CORRUPT, "block record")
-            st = _align(nbytes, 16)
+            st = _align(nbytes, align)
             if run + st > P or any(s[hb + run + nbytes: hb + run + st]):
                 raise OracleError(ERR_CORRUPT, "pad / range")
             qn[i] = np.array(q, np.int32).reshape(3, 2)
@@ -135,5 +142,5 @@ def deserialize(stream) -> dict:
     pool = np.full(max(cursor, 1), 0xEE, np.uint8)
     for b, o in zip(blocks, pool_off):
         pool[o:o + len(b)] = np.frombuffer(b, np.uint8)
-    return dict(tensors=s[64:64 + 32 * T], qn=qn, dim=dim, dtype=dtype, blocks=blocks, pool=pool,
+    return dict(tensors=s[64:64 + 32 * T], qn=qn, dim=dim, dtype=dtype, align=align, blocks=blocks, pool=pool,
                 pool_off=np.array(pool_off, np.uint64), pool_bytes=cursor)

@@ -486,7 +486,7 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
 // ONE launch per bs_serialize / bs_deserialize call: the size / offset pass (bs_scan_phase.cuh) run by the
 // first kScanThreads threads of every CTA — its shared state lives at the start of the dynamic shared memory the rings use
 // afterwards — then the data movement above.  A set of one work item (<= 1024 blocks and tensors) runs the pass
-// replicated: no CTA waits for another; larger sets claim items from the ticket and wait for WsHead.ep_ready.
+// replicated: no CTA waits for another; larger sets claim items from the ticket and wait for WsHead.ready.
 template <bool UNPACK>
 __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) fused_tma_kernel(const ScanParams sp, const MoveParams p,
                                                                       const uint32_t opt_stages, const uint32_t opt_warps)

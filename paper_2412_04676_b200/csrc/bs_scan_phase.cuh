@@ -14,7 +14,7 @@
 //
 // Work is cut into ITEMS (item i = scan tile i of 1024 blocks + slice i of 1024 tensor records) that CTAs claim in
 // order from one ticket; the CTA that completes the last item finalises (totals, capacity checks, sentinel, result) and
-// publishes WsHead.ep_ready.  An item only ever waits (look-back) for items claimed before it, which are being executed
+// publishes WsHead.ready.  An item only ever waits (look-back) for items claimed before it, which are being executed
 // by resident CTAs: forward progress needs no co-residency of the grid.
 //
 // No word the pass synchronises on needs clearing beforehand — the workspace may be uninitialised memory:
@@ -510,9 +510,9 @@ __device__ __forceinline__ void run(const ScanParams& p, const Shape& s, uint64_
         bar();
         const uint32_t item = sm.item;
         if (item >= s.n_items) break;
-        if (s.code == 0) {
-            if ((uint64_t)item * kScanTile < s.T || item == 0) tensor_slice<DESER>(p, s, item, sm);
+        if (s.code == 0) {  // the block tile first: later tiles look back at its aggregate
             if (item < s.n_tiles) block_tile<DESER, false>(p, s, item, tag, sm);
+            if ((uint64_t)item * kScanTile < s.T || item == 0) tensor_slice<DESER>(p, s, item, sm);
         }
         bar();
         if (tid == 0) {

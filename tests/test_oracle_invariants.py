@@ -355,7 +355,7 @@ def test_D11_empty_set_is_128_bytes():
     s = oracle.serialize(tensors, np.zeros((0, 3, 2), np.int32), np.zeros((0, 3), np.uint32), np.zeros(0, np.uint64))
     assert len(s) == 128 and (s[64:] == 0).all()
     info = oracle.stream_info(s)
-    assert info == dict(n_tensors=0, n_blocks=0, header_bytes=128, payload_bytes=0)
+    assert info == dict(n_tensors=0, n_blocks=0, header_bytes=128, payload_bytes=0, align=16)
     out = oracle.deserialize(s)
     assert len(out["tensors"]) == 0 and out["dim"].shape == (0, 3)
 
