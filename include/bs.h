@@ -33,7 +33,8 @@
  *   stream  := fixed_header(64) | tensor_rec[T](32 each) | block_rec[B](48 each) | zeros to a multiple
  *              of 128 | payload(P)
  *   fixed_header: char magic[8]="BSPARSE1"; u32 version=1; u32 endian_tag=0x01020304; u32 dtype (0 f64,
- *                 1 f32, 2 c64, 3 c128: element size e = 8, 4, 8, 16); u32 n_qn=2; u32 max_rank=3; u32 align=16; u64 n_tensors; u64 n_blocks;
+ *                 1 f32, 2 c64, 3 c128: element size e = 8, 4, 8, 16); u32 n_qn=2; u32 max_rank=3; u32 align=16 (8: BS_ALIGN8
+ *                 below, then read align8 for align16 in the payload rule); u64 n_tensors; u64 n_blocks;
  *                 u64 header_bytes; u64 payload_bytes
  *   tensor_rec  : bs_tensor_rec, byte for byte
  *   block_rec   : i32 qn[3][2]; u32 dim[3]; u32 tensor; u64 offset
@@ -73,6 +74,17 @@ enum {
  * every type (a stream holds blocks of ONE type). */
 enum { BS_F64 = 0 /* e = 8 */, BS_F32 = 1 /* e = 4 */, BS_C64 = 2 /* e = 8 */, BS_C128 = 3 /* e = 16 */ };
 
+/* Stream alignment (DESIGN.md §18 reading D19).  OR-ed into bs_set_desc.dtype of a set that
+ * is SERIALIZED: the stream is written with the header's align word = 8 instead of 16, i.e. stored_i = align8(nbytes_i) — no
+ * pad byte at all for f64 / c64 / c128 blocks (f32: 0 or 4) — so block offsets are the literal exclusive prefix sum of the
+ * block byte sizes and the stream's total is a multiple of 8, not of 16.  Deserialize / prefetch take the alignment from the
+ * stream; bs_result.reserved[2] and bs_stream_info_t report it.  Wire format v1 and the TMA variant only (BS_ERR_UNSUPPORTED
+ * for layered sets and for BS_VARIANT_LDG).  Blocks whose stream offset and address differ by 8 modulo 16 cannot go through
+ * the bulk-copy engine and move as 8-byte words: expect roughly half the bandwidth of the padded format on sets with many
+ * odd-sized blocks (DESIGN.md §18 has the numbers). */
+#define BS_ALIGN8 0x100u
+#define BS_DTYPE_MASK 0xffu
+
 /* bs_deserialize / bs_prefetch_async destination layout */
 enum {
     BS_LAYOUT_POOL = 0,     /* out->addr[i] = d_pool + sum_{j<i} align256(nbytes_j); written by the call */
@@ -96,7 +108,7 @@ typedef struct bs_set_desc {
     uint32_t n_tensors;     /* T.  For bs_deserialize / bs_prefetch_async outputs: CAPACITY of tensors[] */
     uint32_t n_blocks;      /* B.  For outputs: CAPACITY of qn / dim / addr */
     uint32_t n_qn;          /* 2: (N, 2Sz) */
-    uint32_t dtype;         /* BS_F64, BS_F32, BS_C64 or BS_C128; for outputs: written by the call's caller as 0, see bs_result */
+    uint32_t dtype;         /* BS_F64, BS_F32, BS_C64 or BS_C128, optionally | BS_ALIGN8; for outputs: 0, see bs_result */
     bs_tensor_rec *tensors; /* [T]        */
     int32_t *qn;            /* [B][3][2]  labels per leg; unused legs 0 */
     uint32_t *dim;          /* [B][3]     extents; unused legs 1 */
@@ -114,12 +126,14 @@ typedef struct bs_result {
     int32_t status;         /* BS_OK or BS_ERR_* */
     uint32_t n_tensors;
     uint32_t n_blocks;
-    uint32_t reserved[5];   /* [0], [1]: see bs_layered_*; [2] = dtype of the stream (deserialize); [3]: see bs_package_emit */
+    uint32_t reserved[5];   /* [0], [1]: see bs_layered_*; [2] = dtype of the stream (| BS_ALIGN8 for an align-8 stream);
+                               [3]: see bs_package_emit */
 } bs_result;
 
 typedef struct bs_stream_info_t {
     uint64_t n_tensors, n_blocks, header_bytes, payload_bytes, total_bytes;
     uint64_t dtype; /* BS_F64 .. BS_C128 */
+    uint64_t align; /* 16 or 8 (BS_ALIGN8) */
 } bs_stream_info_t;
 
 /* Launch tuning.  NULL everywhere means defaults.  The stream produced never depends on these

@@ -6,7 +6,7 @@ write, pack, header parse, unpack, chunked offload/prefetch) runs in the library
 There is no CPU fallback.
 """
 from ._binding import (  # noqa: F401
-    C64, C128, ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_CUDA, ERR_IO, ERR_UNSUPPORTED, F32, F64, LAYOUT_POOL, OK, PENDING, SCATTER_TO_ADDR,
+    ALIGN8, C64, C128, ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_CUDA, ERR_IO, ERR_UNSUPPORTED, F32, F64, LAYOUT_POOL, OK, PENDING, SCATTER_TO_ADDR,
     VARIANT_DEFAULT, VARIANT_LDG, VARIANT_TMA,
     BsError, Engine, LayeredDesc, Opts, Queue, Result, SetDesc, Ticket,
     layered_deserialize, layered_header_bytes, layered_serialize, layered_serialize_range, layered_serialized_size,

@@ -11,6 +11,7 @@ from . import build as _build
 OK, PENDING = 0, 1
 ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_UNSUPPORTED, ERR_CUDA, ERR_IO = -1, -2, -3, -4, -5, -6
 F64, F32, C64, C128 = 0, 1, 2, 3
+ALIGN8 = 0x100   # OR-ed into a set's dtype: serialize an unpadded stream (bs.h BS_ALIGN8)
 LAYOUT_POOL, SCATTER_TO_ADDR = 0, 1
 VARIANT_DEFAULT, VARIANT_LDG, VARIANT_TMA = 0, 1, 2
 
@@ -60,7 +61,7 @@ class Result(C.Structure):
 
 class StreamInfo(C.Structure):
     _fields_ = [("n_tensors", C.c_uint64), ("n_blocks", C.c_uint64), ("header_bytes", C.c_uint64),
-                ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64), ("dtype", C.c_uint64)]
+                ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64), ("dtype", C.c_uint64), ("align", C.c_uint64)]
 
 
 class Opts(C.Structure):

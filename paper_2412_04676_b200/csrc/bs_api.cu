@@ -37,7 +37,8 @@ static bool aligned(const void* p, uintptr_t a) { return ((uintptr_t)p & (a - 1)
 int check_set(const bs_set_desc* s)
 {
     if (s == nullptr) return BS_ERR_ARG;
-    if (s->n_qn != 2 || s->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
+    if (s->n_qn != 2 || (s->dtype & BS_DTYPE_MASK) > (uint32_t)BS_C128 || (s->dtype & ~(BS_DTYPE_MASK | BS_ALIGN8)) != 0)
+        return BS_ERR_UNSUPPORTED;
     if (s->n_tensors && (s->tensors == nullptr || !aligned(s->tensors, 16))) return BS_ERR_ARG;
     if (s->n_blocks && (s->qn == nullptr || !aligned(s->qn, 8))) return BS_ERR_ARG;
     if (s->n_blocks && (s->dim == nullptr || !aligned(s->dim, 4))) return BS_ERR_ARG;
@@ -283,7 +284,8 @@ int bs_stream_info(const void* h, bs_stream_info_t* out)
     memcpy(w, s, 32);
     memcpy(q, s + 32, 32);
     if (memcmp(s, "BSPARSE1", 8) != 0) return BS_ERR_CORRUPT;
-    if (w[2] != 1u || w[3] != 0x01020304u || w[4] > (uint32_t)BS_C128 || w[5] != 2u || w[6] != 3u || w[7] != 16u) return BS_ERR_CORRUPT;
+    if (w[2] != 1u || w[3] != 0x01020304u || w[4] > (uint32_t)BS_C128 || w[5] != 2u || w[6] != 3u || (w[7] != 16u && w[7] != 8u))
+        return BS_ERR_CORRUPT;
     if (q[0] >= (1ull << 32) || q[1] >= (1ull << 32)) return BS_ERR_CORRUPT;
     if (q[2] != bs_header_bytes(q[0], q[1])) return BS_ERR_CORRUPT;
     out->n_tensors = q[0];
@@ -292,6 +294,7 @@ int bs_stream_info(const void* h, bs_stream_info_t* out)
     out->payload_bytes = q[3];
     out->total_bytes = q[2] + q[3];
     out->dtype = w[4];
+    out->align = w[7];
     return BS_OK;
 }
 
@@ -327,6 +330,7 @@ int bs_serialize_range(const bs_set_desc* set, void* d_dst, uint64_t lo, uint64_
     bs_opts o;
     resolve_opts(opts, &o);
     if ((rc = check_opts(o))) return rc;
+    if ((set->dtype & BS_ALIGN8) && o.variant != BS_VARIANT_TMA) return BS_ERR_UNSUPPORTED;  // the LDG variant moves 16-byte units
     WsLayout L;
     if (!ws_layout(d_ws, ws_bytes, set->n_blocks, &L)) return d_ws && aligned(d_ws, 256) ? BS_ERR_CAPACITY : BS_ERR_ARG;
     int sms;
@@ -344,17 +348,20 @@ int bs_serialize(const bs_set_desc* set, void* d_stream, uint64_t capacity, void
     bs_opts o;
     resolve_opts(opts, &o);
     if ((rc = check_opts(o))) return rc;
+    if ((set->dtype & BS_ALIGN8) && o.variant != BS_VARIANT_TMA) return BS_ERR_UNSUPPORTED;  // the LDG variant moves 16-byte units
     WsLayout L;
     if (!ws_layout(d_ws, ws_bytes, set->n_blocks, &L)) return d_ws && aligned(d_ws, 256) ? BS_ERR_CAPACITY : BS_ERR_ARG;
     int sms;
     if ((rc = device_sm_count(&sms))) return rc;
+    // the range is the whole stream: the pass refuses a total beyond `capacity`, the movement clips to the total
+    constexpr uint64_t kAll = ~15ull;
     if (use_fused(o, set->n_tensors, set->n_blocks, sms)) {  // the pass and the pack in ONE launch
         const cudaError_t e = launch_fused_tma(false, serialize_scan_params(set, L, capacity, 0, d_result),
-                                               pack_params(set, L, d_stream, 0, capacity & ~15ull, o), o, capacity, sms, stream);
+                                               pack_params(set, L, d_stream, 0, kAll, o), o, capacity, sms, stream);
         return e == cudaSuccess ? BS_OK : cuda_fail(e);
     }
     if ((rc = run_serialize_scan(set, L, capacity, 0, d_result, sms, stream))) return rc;
-    return run_pack_range(set, L, d_stream, 0, capacity & ~15ull, o, sms, stream);
+    return run_pack_range(set, L, d_stream, 0, kAll, o, sms, stream);
 }
 
 int bs_deserialize(const void* d_stream, uint64_t nbytes, bs_set_desc* out, void* d_pool, uint64_t pool_bytes,
@@ -374,14 +381,17 @@ int bs_deserialize(const void* d_stream, uint64_t nbytes, bs_set_desc* out, void
     int sms;
     if ((rc = device_sm_count(&sms))) return rc;
     const unsigned char* s = (const unsigned char*)d_stream;
+    // an align-8 stream cannot go through the LDG variant (16-byte units): its parse pass then refuses it
+    const uint32_t pflags = flags | (o.variant != BS_VARIANT_TMA ? kFlagNoAlign8 : 0u);
+    constexpr uint64_t kAll = ~15ull;  // the parse pass proves header_bytes + payload_bytes == nbytes; the movement clips to it
     // the payload is only dereferenced (pad-zero check) after the fixed header proved header_bytes + P == nbytes
     if (use_fused(o, out->n_tensors, out->n_blocks, sms)) {  // parse / validate and unpack in ONE launch
-        const cudaError_t e = launch_fused_tma(true, deserialize_scan_params(s, s, nbytes, out, d_pool, pool_bytes, flags, L, d_result),
-                                               unpack_params(out, L, s, s, 0, nbytes & ~15ull, flags, o), o, nbytes, sms, stream);
+        const cudaError_t e = launch_fused_tma(true, deserialize_scan_params(s, s, nbytes, out, d_pool, pool_bytes, pflags, L, d_result),
+                                               unpack_params(out, L, s, s, 0, kAll, flags, o), o, nbytes, sms, stream);
         return e == cudaSuccess ? BS_OK : cuda_fail(e);
     }
-    if ((rc = run_deserialize_scan(s, s, nbytes, out, d_pool, pool_bytes, flags, L, d_result, sms, stream))) return rc;
-    return run_unpack_range(out, L, s, s, 0, nbytes & ~15ull, flags, o, sms, stream);
+    if ((rc = run_deserialize_scan(s, s, nbytes, out, d_pool, pool_bytes, pflags, L, d_result, sms, stream))) return rc;
+    return run_unpack_range(out, L, s, s, 0, kAll, flags, o, sms, stream);
 }
 
 int bs_deserialize_range(const void* d_src, uint64_t lo, uint64_t hi, const void* d_header, bs_set_desc* out, uint32_t flags,

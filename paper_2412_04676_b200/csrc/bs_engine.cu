@@ -209,6 +209,7 @@ int bs_engine_offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layere
     WsLayout L;
     int rc = set ? check_set(set) : check_layered_desc(lset);  // as the direct calls: a descriptor no loader accepts is refused here
     if (rc) return rc;
+    if (set && (set->dtype & BS_ALIGN8) && e->opts.variant != BS_VARIANT_TMA) return BS_ERR_UNSUPPORTED;
     if (set) {
         if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
         if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
@@ -227,7 +228,7 @@ int bs_engine_offload_impl(bs_engine* e, const bs_set_desc* set, const bs_layere
         if (rc) return rc;
     }
     if (total_bytes > h_capacity || total_bytes > e->cfg.max_stream_bytes) return BS_ERR_CAPACITY;
-    if (total_bytes & 15) return BS_ERR_ARG;
+    if (total_bytes & 7) return BS_ERR_ARG;  // (a multiple of 16, or of 8 for an align-8 stream)
     bs_ticket* t = nullptr;
     if ((rc = ticket_create(&t))) return rc;
     TicketGuard guard{e, t};
@@ -323,8 +324,8 @@ int bs_engine_prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes,
     CK(cudaMemcpyAsync(e->header_buf, h_pinned, hb, cudaMemcpyHostToDevice, e->cstream));
     CK(cudaEventRecord(e->ev_fence_c, e->cstream));
     CK(cudaStreamWaitEvent(e->kstream, e->ev_fence_c, 0));
-    rc = out ? run_deserialize_scan(e->header_buf, nullptr, nbytes, out, d_pool, pool_bytes, flags, L, e->d_result, e->sms,
-                                    e->kstream)
+    rc = out ? run_deserialize_scan(e->header_buf, nullptr, nbytes, out, d_pool, pool_bytes,
+                                    flags | (e->opts.variant != BS_VARIANT_TMA ? kFlagNoAlign8 : 0u), L, e->d_result, e->sms, e->kstream)
              : run_layered_deserialize_plan(e->header_buf, nullptr, nbytes, lout, d_pool, pool_bytes, flags, e->ws, e->ws_bytes,
                                             e->d_result, e->sms, e->kstream);
     if (rc) return rc;
@@ -398,6 +399,7 @@ static int offload_packages_impl(bs_engine* e, const bs_set_desc* set, const bs_
     uint64_t hb;
     int rc = set ? check_set(set) : check_layered_desc(lset);
     if (rc) return rc;
+    if (set && (set->dtype & BS_ALIGN8) && e->opts.variant != BS_VARIANT_TMA) return BS_ERR_UNSUPPORTED;
     if (set) {
         if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
         if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
@@ -551,7 +553,8 @@ static int prefetch_packages_impl(bs_engine* e, const void* h_slots, uint64_t sl
     }
     CK(cudaEventRecord(e->ev_fence_c, e->cstream));
     CK(cudaStreamWaitEvent(e->kstream, e->ev_fence_c, 0));
-    rc = out ? run_deserialize_scan(e->header_buf, nullptr, plan.total, out, d_pool, pool_bytes, flags, L, e->d_result, e->sms, e->kstream)
+    rc = out ? run_deserialize_scan(e->header_buf, nullptr, plan.total, out, d_pool, pool_bytes,
+                                    flags | (e->opts.variant != BS_VARIANT_TMA ? kFlagNoAlign8 : 0u), L, e->d_result, e->sms, e->kstream)
              : run_layered_deserialize_plan(e->header_buf, nullptr, plan.total, lout, d_pool, pool_bytes, flags, e->ws, e->ws_bytes,
                                             e->d_result, e->sms, e->kstream);
     if (rc) return rc;

@@ -118,7 +118,7 @@ struct ScanParams {
     const uint32_t* dim;
     const uint64_t* addr;
     uint32_t T, B;           // SER: counts; DESER: capacities of the out arrays
-    uint32_t dtype;          // SER: element type of the set
+    uint32_t dtype;          // SER: element type of the set | BS_ALIGN8
     // DESER inputs
     const unsigned char* header;  // stream byte 0 .. header_bytes (device)
     const unsigned char* payload; // stream byte 0 when the payload is resident behind the header (pad-zero check), else null
@@ -208,6 +208,7 @@ void resolve_opts(const bs_opts* in, bs_opts* out);
 
 // ---- host-side runners shared by the translation units (bs_api.cu, bs_layered.cu) -------------------------------------------
 constexpr uint32_t kFlagCheckPad = 0x100u;       // unpack: pad bytes must be zero (engine path; the payload is not resident at parse time)
+constexpr uint32_t kFlagNoAlign8 = 0x400u;       // parse pass: the movement that follows cannot take an align-8 stream (LDG variant)
 constexpr uint32_t kFlagPoisonOnError = 0x200u;  // pack (engine): a deferred error zeroes the first 64 bytes of the range that holds
                                                  // stream byte 0, so a host buffer never keeps a stale but valid header
 int cuda_fail(cudaError_t e);

@@ -32,7 +32,7 @@ __device__ __forceinline__ uint4 header_unit(const MoveParams& p, uint64_t u, ui
     uint4 v = make_uint4(0, 0, 0, 0);
     if (u < 4) {
         if (u == 0) v = make_uint4(0x41505342u, 0x31455352u, 1u, 0x01020304u);  // "BSPARSE1", version, endian_tag
-        else if (u == 1) v = make_uint4(dtype, 2u, 3u, 16u);                      // dtype, n_qn, max_rank, align
+        else if (u == 1) v = make_uint4(dtype & BS_DTYPE_MASK, 2u, 3u, (dtype & BS_ALIGN8) ? 8u : 16u);  // dtype, n_qn, max_rank, align
         else if (u == 2) v = make_uint4(T, 0u, B, 0u);                           // u64 n_tensors, u64 n_blocks
         else v = make_uint4((uint32_t)hb, (uint32_t)(hb >> 32), (uint32_t)P, (uint32_t)(P >> 32));
         return v;

@@ -246,6 +246,220 @@ __device__ __forceinline__ void unpack_seg(const Seg& s, uint32_t saddr, const u
     }
 }
 
+// ==== align = 8 streams (bs.h BS_ALIGN8; DESIGN.md §18 reading D19) ===========================================================
+// Stored sizes are rounded to 8 bytes only, so a block may start 8 bytes off the 16-byte grid of the stream.  The bulk-copy
+// engine needs source, destination and size on that grid: a segment whose two sides agree modulo 16 moves an 8-byte head
+// (if it starts off the grid), its 16-byte-aligned body as ONE bulk copy and a short rest; a segment whose sides DISAGREE
+// moves as 8-byte words, spread over the whole warp.  Kept out of line: the align-16 path above is unchanged.
+struct Seg8 {
+    uint64_t lo;    // first payload byte
+    uint32_t n;     // data bytes (a multiple of 4)
+    uint32_t pad;   // zero bytes behind them (f32 only: 4), when the segment ends its block
+    uint64_t addr;  // device address of the block byte that maps to payload byte `lo`
+};
+__device__ __forceinline__ bool clip_seg8(const Blk& e, uint64_t next, uint64_t tlo, uint64_t thi, Seg8* s)
+{
+    const uint64_t lo = e.off > tlo ? e.off : tlo;
+    const uint64_t hi = next < thi ? next : thi;
+    if (hi <= lo) return false;
+    const uint32_t pad = (hi == next) ? (uint32_t)(e.addr & 3ull) * 4u : 0u;
+    s->lo = lo;
+    s->addr = (e.addr & ~7ull) + (lo - e.off);
+    s->n = (uint32_t)(hi - lo) - pad;
+    s->pad = pad;
+    return true;
+}
+__device__ __forceinline__ Blk load_blk(const Blk* __restrict__ blk, uint32_t j, uint64_t* next)
+{
+    const uint4 w = __ldcg(reinterpret_cast<const uint4*>(blk + j));
+    Blk e;
+    e.off = (uint64_t)w.x | ((uint64_t)w.y << 32);
+    e.addr = (uint64_t)w.z | ((uint64_t)w.w << 32);
+    *next = __ldcg(reinterpret_cast<const unsigned long long*>(&blk[j + 1].off));
+    return e;
+}
+struct TileCtx {
+    uint64_t tbase, tlo, thi;  // the tile and its part inside the call's range, payload coordinates
+    uint32_t sbase, bar;       // shared address of the stage, its mbarrier
+    uint32_t jlo, jhi, lane;   // blocks jlo .. jhi touch the tile
+    const Blk* blk;
+    Blk e0;                    // the lane's own block (jlo + lane), prefetched
+    uint64_t next0;
+};
+__device__ __forceinline__ uint64_t shfl_u64(uint64_t v, uint32_t src)
+{
+    const uint32_t lo = __shfl_sync(0xffffffffu, (uint32_t)v, src), hi = __shfl_sync(0xffffffffu, (uint32_t)(v >> 32), src);
+    return ((uint64_t)hi << 32) | lo;
+}
+// split of a co-aligned segment that lands at shared / global offset d: head (0 or 8 bytes up to the grid), body (bulk)
+__device__ __forceinline__ void split8(uint32_t d, uint32_t n, uint32_t* head, uint32_t* body)
+{
+    *head = ((d & 8u) && n >= 8u) ? 8u : 0u;
+    *body = (n - *head) & ~15u;
+}
+
+// pack, align 8: stage every segment of the tile; returns with the bulk copies issued
+__device__ __noinline__ void pack_tile_a8(const TileCtx c)
+{
+    const uint32_t lane = c.lane;
+    uint32_t tx = 0, n_async = 0;
+    Seg8 s0;
+    s0.lo = 0; s0.n = 0; s0.pad = 0; s0.addr = 0;
+    const bool have0 = clip_seg8(c.e0, c.next0, c.tlo, c.thi, &s0);
+    const uint32_t d0 = c.sbase + (uint32_t)(s0.lo - c.tbase);
+    const bool co0 = have0 && (((uint32_t)s0.addr ^ d0) & 15u) == 0;
+    uint32_t head0 = 0, body0 = 0;
+    auto small_parts = [&](const Seg8& s, uint32_t d, uint32_t head, uint32_t body) {  // everything of a co-aligned segment but its body
+        if (head) { cp_async_8(d, reinterpret_cast<const void*>(s.addr)); ++n_async; }
+        uint32_t off = head + body;
+        const uint32_t rest = s.n - off;
+        if (rest & 8u) { cp_async_8(d + off, reinterpret_cast<const void*>(s.addr + off)); off += 8; ++n_async; }
+        if (rest & 4u) { cp_async_4(d + off, reinterpret_cast<const void*>(s.addr + off)); ++n_async; }
+    };
+    auto zero_pad = [&](const Seg8& s, uint32_t d) {
+        if (s.pad) {
+            for (uint32_t b = 0; b < s.pad; b += 4) asm volatile("st.shared.u32 [%0], %1;" ::"r"(d + s.n + b), "r"(0u) : "memory");
+            fence_proxy_async();
+        }
+    };
+    if (co0) {
+        split8(d0, s0.n, &head0, &body0);
+        tx += body0;
+        small_parts(s0, d0, head0, body0);
+    }
+    if (have0) zero_pad(s0, d0);
+    // segments whose two sides disagree modulo 16: 8-byte words, the whole warp on each
+    uint32_t mis = __ballot_sync(0xffffffffu, have0 && !co0);
+    while (mis) {
+        const uint32_t l = (uint32_t)__ffs((int)mis) - 1u;
+        mis &= mis - 1u;
+        const uint64_t a = shfl_u64(s0.addr, l);
+        const uint32_t d = __shfl_sync(0xffffffffu, d0, l), n = __shfl_sync(0xffffffffu, s0.n, l);
+        for (uint32_t b = lane * 8u; b + 8u <= n; b += 256u) cp_async_8(d + b, reinterpret_cast<const void*>(a + b));
+        if ((n & 4u) && lane == 0) cp_async_4(d + (n & ~7u), reinterpret_cast<const void*>(a + (n & ~7u)));
+        ++n_async;
+    }
+    if (c.jhi >= c.jlo + 32) {  // more than 32 blocks in the tile: small blocks, each lane on its own
+        for (uint32_t j = c.jlo + lane + 32; j <= c.jhi; j += 32) {
+            uint64_t next;
+            const Blk e = load_blk(c.blk, j, &next);
+            Seg8 s;
+            if (!clip_seg8(e, next, c.tlo, c.thi, &s)) continue;
+            const uint32_t d = c.sbase + (uint32_t)(s.lo - c.tbase);
+            if ((((uint32_t)s.addr ^ d) & 15u) == 0) {
+                uint32_t head, body;
+                split8(d, s.n, &head, &body);
+                tx += body;
+                small_parts(s, d, head, body);
+            } else {
+                for (uint32_t b = 0; b + 8u <= s.n; b += 8u) cp_async_8(d + b, reinterpret_cast<const void*>(s.addr + b));
+                if (s.n & 4u) cp_async_4(d + (s.n & ~7u), reinterpret_cast<const void*>(s.addr + (s.n & ~7u)));
+                ++n_async;
+            }
+            zero_pad(s, d);
+        }
+    }
+    if (n_async) cp_async_mbar_arrive(c.bar);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) tx += __shfl_xor_sync(0xffffffffu, tx, d);
+    __syncwarp();  // every lane's cp.async arrival is registered before the phase can complete
+    if (lane == 0) mbar_arrive_expect_tx(c.bar, tx);
+    __syncwarp();
+    if (co0 && body0) bulk_g2s(d0 + head0, reinterpret_cast<const void*>(s0.addr + head0), body0, c.bar);
+    if (c.jhi >= c.jlo + 32) {
+        for (uint32_t j = c.jlo + lane + 32; j <= c.jhi; j += 32) {
+            uint64_t next;
+            const Blk e = load_blk(c.blk, j, &next);
+            Seg8 s;
+            if (!clip_seg8(e, next, c.tlo, c.thi, &s)) continue;
+            const uint32_t d = c.sbase + (uint32_t)(s.lo - c.tbase);
+            uint32_t head, body;
+            split8(d, s.n, &head, &body);
+            if ((((uint32_t)s.addr ^ d) & 15u) == 0 && body) bulk_g2s(d + head, reinterpret_cast<const void*>(s.addr + head), body, c.bar);
+        }
+    }
+}
+
+// a tile <-> the stream, align 8: only the last tile of a stream can be 8 bytes off a multiple of 16
+__device__ __forceinline__ void store_tile_a8(unsigned char* dst, uint32_t src, uint32_t n)  // one lane
+{
+    const uint32_t nb = n & ~15u;
+    if (nb) bulk_s2g(dst, src, nb);
+    if (n & 8u) {
+        uint64_t v;
+        asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(src + nb) : "memory");
+        *reinterpret_cast<uint64_t*>(dst + nb) = v;
+    }
+}
+__device__ __forceinline__ void load_tile_a8(uint32_t dst, const unsigned char* src, uint32_t n, uint32_t bar)  // one lane
+{
+    const uint32_t nb = n & ~15u;
+    if (n & 8u) {
+        cp_async_8(dst + nb, src + nb);
+        cp_async_mbar_arrive(bar);
+    }
+    mbar_arrive_expect_tx(bar, nb);
+    if (nb) bulk_g2s(dst, src, nb, bar);
+}
+
+// unpack, align 8: scatter every segment of the staged tile (sp: generic pointer to the stage)
+__device__ __noinline__ void unpack_tile_a8(const TileCtx c, const unsigned char* sp, uint32_t flags, int* status)
+{
+    const uint32_t lane = c.lane;
+    auto check_pad = [&](const Seg8& s, const unsigned char* q) {
+        if (s.pad && (flags & kFlagCheckPad)) {
+            uint32_t z = 0;
+            for (uint32_t b = 0; b < s.pad; b += 4) z |= *reinterpret_cast<const uint32_t*>(q + s.n + b);
+            if (z != 0) atomicCAS(status, 0, BS_ERR_CORRUPT);
+        }
+    };
+    auto co_parts = [&](const Seg8& s, uint32_t d, const unsigned char* q) {  // a co-aligned segment
+        uint32_t head, body;
+        split8(d, s.n, &head, &body);
+        if (head) *reinterpret_cast<uint64_t*>(s.addr) = *reinterpret_cast<const uint64_t*>(q);
+        if (body) bulk_s2g(reinterpret_cast<void*>(s.addr + head), d + head, body);
+        uint32_t off = head + body;
+        const uint32_t rest = s.n - off;
+        if (rest & 8u) { *reinterpret_cast<uint64_t*>(s.addr + off) = *reinterpret_cast<const uint64_t*>(q + off); off += 8; }
+        if (rest & 4u) *reinterpret_cast<uint32_t*>(s.addr + off) = *reinterpret_cast<const uint32_t*>(q + off);
+    };
+    Seg8 s0;
+    s0.lo = 0; s0.n = 0; s0.pad = 0; s0.addr = 0;
+    const bool have0 = clip_seg8(c.e0, c.next0, c.tlo, c.thi, &s0);
+    const uint32_t off0 = (uint32_t)(s0.lo - c.tbase);
+    const uint32_t d0 = c.sbase + off0;
+    const bool co0 = have0 && (((uint32_t)s0.addr ^ d0) & 15u) == 0;
+    if (co0) co_parts(s0, d0, sp + off0);
+    if (have0) check_pad(s0, sp + off0);
+    uint32_t mis = __ballot_sync(0xffffffffu, have0 && !co0);
+    while (mis) {
+        const uint32_t l = (uint32_t)__ffs((int)mis) - 1u;
+        mis &= mis - 1u;
+        const uint64_t a = shfl_u64(s0.addr, l);
+        const uint32_t o = __shfl_sync(0xffffffffu, off0, l), n = __shfl_sync(0xffffffffu, s0.n, l);
+        for (uint32_t b = lane * 8u; b + 8u <= n; b += 256u)
+            *reinterpret_cast<uint64_t*>(a + b) = *reinterpret_cast<const uint64_t*>(sp + o + b);
+        if ((n & 4u) && lane == 0) *reinterpret_cast<uint32_t*>(a + (n & ~7u)) = *reinterpret_cast<const uint32_t*>(sp + o + (n & ~7u));
+    }
+    if (c.jhi >= c.jlo + 32) {
+        for (uint32_t j = c.jlo + lane + 32; j <= c.jhi; j += 32) {
+            uint64_t next;
+            const Blk e = load_blk(c.blk, j, &next);
+            Seg8 s;
+            if (!clip_seg8(e, next, c.tlo, c.thi, &s)) continue;
+            const uint32_t o = (uint32_t)(s.lo - c.tbase), d = c.sbase + o;
+            if ((((uint32_t)s.addr ^ d) & 15u) == 0) {
+                co_parts(s, d, sp + o);
+            } else {
+                for (uint32_t b = 0; b + 8u <= s.n; b += 8u)
+                    *reinterpret_cast<uint64_t*>(s.addr + b) = *reinterpret_cast<const uint64_t*>(sp + o + b);
+                if (s.n & 4u) *reinterpret_cast<uint32_t*>(s.addr + (s.n & ~7u)) = *reinterpret_cast<const uint32_t*>(sp + o + (s.n & ~7u));
+            }
+            check_pad(s, sp + o);
+        }
+    }
+}
+
 // Default launch shapes (B200, measured; profiles/r02_summary.md).  The launch always has the small-set shape — three rings
 // of 3 stages x 16 KiB per SM, what sets of tens of MB run fastest with in both directions — and the kernel, which knows the
 // payload size, switches sets of half a GB and more to ONE ring in the same shared memory: pack 3 x 48 KiB, unpack 4 x 32 KiB
@@ -273,6 +487,7 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     const uint64_t ng = hv.ng;
     const uint64_t lo = p.lo, hi = p.hi < total ? p.hi : total;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool a8 = (hv.dtype & BS_ALIGN8) != 0;  // an unpadded stream: segments may sit 8 bytes off the 16-byte grid
     uint32_t tile_bytes = p.tile_bytes, n_warps = opt_warps & 0xffffu, n_stages = opt_stages;
     // The preset (bit 31 of opt_warps: bs_opts left the shape open) is settled here, where the payload size is known
     if ((opt_warps >> 31) && P >= kLargePayload && p.pkg.cap % preset_large(UNPACK).tile_bytes == 0) {
@@ -401,9 +616,18 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
             const uint32_t sbase = ring + st * tile_bytes, bar = bar0 + 8 * st;
             if (UNPACK) {
                 if (lane == 0) {
-                    mbar_arrive_expect_tx(bar, (uint32_t)(thi - tlo));
-                    bulk_g2s_x(sbase + (uint32_t)(tlo - tbase), stream_at(p, hb, hb + tlo), (uint32_t)(thi - tlo), bar, hints);
+                    if (a8) {
+                        load_tile_a8(sbase + (uint32_t)(tlo - tbase), stream_at(p, hb, hb + tlo), (uint32_t)(thi - tlo), bar);
+                    } else {
+                        mbar_arrive_expect_tx(bar, (uint32_t)(thi - tlo));
+                        bulk_g2s_x(sbase + (uint32_t)(tlo - tbase), stream_at(p, hb, hb + tlo), (uint32_t)(thi - tlo), bar, hints);
+                    }
                 }
+            } else if (a8) {
+                TileCtx c;
+                c.tbase = tbase; c.tlo = tlo; c.thi = thi; c.sbase = sbase; c.bar = bar; c.jlo = jlo; c.jhi = jhi; c.lane = lane;
+                c.blk = blk; c.e0 = e0; c.next0 = next0;
+                pack_tile_a8(c);
             } else {
                 // pass 1: bytes the bulk copies will deliver; tails and 8-byte-aligned blocks go through cp.async
                 uint32_t tx = 0, n_async = 0;
@@ -447,8 +671,15 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
                 if (__shfl_sync(0xffffffffu, landed, 0) == 0) break;  // warp-uniform
                 if (lane == 0) {
                     fence_proxy_async();  // the cp.async tails were written through the generic proxy
-                    bulk_s2g_x(stream_at(p, hb, hb + tlo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo), hints);
+                    if (a8) store_tile_a8(stream_at(p, hb, hb + tlo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo));
+                    else bulk_s2g_x(stream_at(p, hb, hb + tlo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo), hints);
                 }
+            } else if (a8) {
+                if (!__all_sync(0xffffffffu, mbar_wait(bar, parity, status))) break;  // warp-uniform
+                TileCtx c;
+                c.tbase = tbase; c.tlo = tlo; c.thi = thi; c.sbase = sbase; c.bar = bar; c.jlo = jlo; c.jhi = jhi; c.lane = lane;
+                c.blk = blk; c.e0 = e0; c.next0 = next0;
+                unpack_tile_a8(c, ring_ptr + (size_t)st * tile_bytes, p.flags, status);
             } else {
                 const unsigned char* sp = ring_ptr + (size_t)st * tile_bytes;
                 Seg s0;

@@ -219,7 +219,7 @@ int pkg_plan(const unsigned char* h_hdrs, uint64_t stride, uint64_t n_slots, uin
     for (uint64_t k = 0; k < count; ++k) {
         const PkgItem& it = plan->items[k];
         if (it.index != k) return BS_ERR_CORRUPT;  // a duplicate or a hole
-        if (it.lo != next || it.nbytes == 0 || it.nbytes > plan->total - it.lo || ((it.lo | it.nbytes) & 15)) return BS_ERR_CORRUPT;
+        if (it.lo != next || it.nbytes == 0 || it.nbytes > plan->total - it.lo || (it.lo & 15) || (it.nbytes & 7)) return BS_ERR_CORRUPT;  // (the last package of an align-8 stream ends 8 off the grid)
         if (it.nbytes > slot_bytes - BS_PKG_HEADER) return BS_ERR_CORRUPT;
         const bool hdr = it.first_block == BS_PKG_NO_BLOCK;
         if (hdr && !in_header) return BS_ERR_CORRUPT;  // header-region packages are a prefix in index order
@@ -285,7 +285,7 @@ int bs_package_emit(const bs_set_desc* set, uint64_t total_bytes, uint64_t cap, 
                     bs_result* d_result, const bs_opts* opts, cudaStream_t stream)
 {
     if (set == nullptr) return BS_ERR_ARG;
-    if (set->n_qn != 2 || set->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
+    { const int rc0 = check_set(set); if (rc0) return rc0; }
     if (d_slots == nullptr || !aligned16(d_slots) || cap == 0 || (cap & 15) || (slot_bytes & 15) ||
         slot_bytes < BS_PKG_HEADER + cap)
         return BS_ERR_ARG;
@@ -293,6 +293,7 @@ int bs_package_emit(const bs_set_desc* set, uint64_t total_bytes, uint64_t cap, 
     resolve_opts(opts, &o);
     int rc;
     if ((rc = check_opts(o))) return rc;
+    if ((set->dtype & BS_ALIGN8) && o.variant != BS_VARIANT_TMA) return BS_ERR_UNSUPPORTED;  // the LDG variant moves 16-byte units
     WsLayout L;
     if (!ws_layout(d_ws, ws_bytes, set->n_blocks, &L)) return d_ws && ((uintptr_t)d_ws & 255) == 0 ? BS_ERR_CAPACITY : BS_ERR_ARG;
     int sms;
@@ -350,7 +351,7 @@ int bs_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t n_slots
                       const bs_opts* opts, cudaStream_t stream)
 {
     if (out == nullptr) return BS_ERR_ARG;
-    if (out->n_qn != 2 || out->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
+    { const int rc0 = check_set(out); if (rc0) return rc0; }
     if (d_slots == nullptr || !aligned16(d_slots) || (slot_bytes & 15) || slot_bytes < BS_PKG_HEADER + 16 || n_slots == 0)
         return BS_ERR_ARG;
     if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;
@@ -402,7 +403,8 @@ int bs_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t n_slots
             pkg_gather_header_kernel<<<grid ? grid : 1, 256, 0, stream>>>(slots, slot_bytes, d_tab, cut, plan.hb, d_header);
             CK(cudaGetLastError());
         }
-        if ((rc = run_deserialize_scan(d_header, nullptr, plan.total, out, d_pool, pool_bytes, flags, L, d_result, sms, stream))) return rc;
+        if ((rc = run_deserialize_scan(d_header, nullptr, plan.total, out, d_pool, pool_bytes,
+                                       flags | (o.variant != BS_VARIANT_TMA ? kFlagNoAlign8 : 0u), L, d_result, sms, stream))) return rc;
         CK(launch_pkg_check(L, d_slots, slot_bytes, n_slots, stream_id, d_result, stream));
         if ((rc = run_unpack_range(out, L, d_header, d_header, 0, 0, flags, o, sms, stream))) return rc;  // descriptor rebuild
         PkgMap pm;
@@ -417,7 +419,8 @@ int bs_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t n_slots
         const PkgItem& it = plan.items[k];
         CK(cudaMemcpyAsync(d_header + it.lo, slots + it.slot * slot_bytes + BS_PKG_HEADER, it.nbytes, cudaMemcpyDeviceToDevice, stream));
     }
-    if ((rc = run_deserialize_scan(d_header, nullptr, plan.total, out, d_pool, pool_bytes, flags, L, d_result, sms, stream))) return rc;
+    if ((rc = run_deserialize_scan(d_header, nullptr, plan.total, out, d_pool, pool_bytes,
+                                       flags | (o.variant != BS_VARIANT_TMA ? kFlagNoAlign8 : 0u), L, d_result, sms, stream))) return rc;
     CK(launch_pkg_check(L, d_slots, slot_bytes, n_slots, stream_id, d_result, stream));
     if ((rc = run_unpack_range(out, L, d_header, d_header, 0, 0, flags, o, sms, stream))) return rc;  // descriptor rebuild
     std::vector<PkgItem> by_slot(plan.items.begin() + plan.n_header, plan.items.end());
@@ -447,7 +450,7 @@ int bs_layered_package_emit(const bs_layered_desc* set, uint64_t total_bytes, ui
                             bs_result* d_result, const bs_opts* opts, cudaStream_t stream)
 {
     if (set == nullptr) return BS_ERR_ARG;
-    if (set->n_qn != 2 || set->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
+    { const int rc0 = check_layered_desc(set); if (rc0) return rc0; }
     if (d_slots == nullptr || !aligned16(d_slots) || cap == 0 || (cap & 15) || (slot_bytes & 15) ||
         slot_bytes < BS_PKG_HEADER + cap)
         return BS_ERR_ARG;
@@ -504,7 +507,7 @@ int bs_layered_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t
                               const bs_opts* opts, cudaStream_t stream)
 {
     if (out == nullptr) return BS_ERR_ARG;
-    if (out->n_qn != 2 || out->dtype > (uint32_t)BS_C128) return BS_ERR_UNSUPPORTED;
+    { const int rc0 = check_layered_desc(out); if (rc0) return rc0; }
     if (d_slots == nullptr || !aligned16(d_slots) || (slot_bytes & 15) || slot_bytes < BS_PKG_HEADER + 16 || n_slots == 0)
         return BS_ERR_ARG;
     if (flags != BS_LAYOUT_POOL && flags != BS_SCATTER_TO_ADDR) return BS_ERR_ARG;

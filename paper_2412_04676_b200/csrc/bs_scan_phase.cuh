@@ -45,7 +45,7 @@ constexpr uint64_t kIdleTag = 0xB5C0DE5EEDull << 24;  // the counters' tag betwe
 // what the data-movement code needs to know about the set once the pass is complete
 struct HeadView {
     int32_t status;
-    uint32_t T, B, dtype;
+    uint32_t T, B, dtype;  // dtype: element type | BS_ALIGN8
     uint64_t hb, P, ng;
 };
 
@@ -160,7 +160,8 @@ __device__ __forceinline__ TensorHead load_tensor(const ScanParams& p, uint64_t 
 struct Shape {
     uint64_t T, B, hb, P_hdr;
     uint64_t rep_T, rep_B;  // deserialize, out arrays too small: the stream's counts, reported so the caller can size them
-    uint32_t dtype;
+    uint32_t dtype;         // element type (bs.h BS_F64 ..), without flags
+    uint32_t align;         // 16, or 8 (BS_ALIGN8: stored sizes are rounded to 8 only, DESIGN.md §18 reading D19)
     int code;               // != 0: the fixed header was rejected
     uint32_t n_tiles, n_items;
 };
@@ -169,7 +170,9 @@ template <bool DESER>
 __device__ __forceinline__ Shape shape_of(const ScanParams& p)
 {
     Shape s;
-    s.T = p.T; s.B = p.B; s.hb = 0; s.P_hdr = 0; s.rep_T = 0; s.rep_B = 0; s.dtype = p.dtype; s.code = 0;
+    s.T = p.T; s.B = p.B; s.hb = 0; s.P_hdr = 0; s.rep_T = 0; s.rep_B = 0; s.code = 0;
+    s.dtype = p.dtype & BS_DTYPE_MASK;
+    s.align = (p.dtype & BS_ALIGN8) ? 8u : 16u;
     if (DESER) {  // the fixed header (SURVEY §8(c) checks, in order)
         s.T = s.B = 0;
         if (p.nbytes < kFixedHeader) {
@@ -185,12 +188,13 @@ __device__ __forceinline__ Shape shape_of(const ScanParams& p)
             else if (w1.x > (uint32_t)BS_C128)                    s.code = BS_ERR_CORRUPT;  // dtype
             else if (w1.y != 2u)                                  s.code = BS_ERR_CORRUPT;  // n_qn
             else if (w1.z != 3u)                                  s.code = BS_ERR_CORRUPT;  // max_rank
-            else if (w1.w != 16u)                                 s.code = BS_ERR_CORRUPT;  // align
+            else if (w1.w != 16u && w1.w != 8u)                   s.code = BS_ERR_CORRUPT;  // align
+            else if (w1.w == 8u && (p.flags & kFlagNoAlign8))     s.code = BS_ERR_UNSUPPORTED;  // the LDG variant moves 16-byte units
             else if (hT >= (1ull << 32) || hB >= (1ull << 32))   s.code = BS_ERR_CORRUPT;
             else if (hH != align_up(kFixedHeader + kTensorRec * hT + kBlockRec * hB, kHeaderAlign)) s.code = BS_ERR_CORRUPT;
             else if (hH > p.nbytes || hP != p.nbytes - hH)        s.code = BS_ERR_CORRUPT;
             else if (hT > p.T || hB > p.B) { s.code = BS_ERR_CAPACITY; s.rep_T = hT; s.rep_B = hB; }  // out arrays too small
-            else { s.T = hT; s.B = hB; s.hb = hH; s.P_hdr = hP; s.dtype = w1.x; }
+            else { s.T = hT; s.B = hB; s.hb = hH; s.P_hdr = hP; s.dtype = w1.x; s.align = w1.w; }
         }
     } else {
         s.hb = align_up(kFixedHeader + kTensorRec * s.T + kBlockRec * s.B, kHeaderAlign);
@@ -255,6 +259,7 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
     constexpr int kErrBad = DESER ? BS_ERR_CORRUPT : BS_ERR_ARG;
     const uint64_t T = s.T, B = s.B, hb = s.hb, P_hdr = s.P_hdr;
     const uint64_t esize = elem_bytes(s.dtype);
+    const uint64_t amask = s.align - 1;  // S1: stored = align_up(nbytes, align), align = 16 (D3) or 8 (D19)
     const unsigned char* brec = DESER ? p.header + kFixedHeader + kTensorRec * T : nullptr;
 
     uint64_t val[kScanItems];      // what is scanned: stored size (SER) / pool slot size (DESER)
@@ -289,7 +294,7 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
         uint64_t n = n01 * d2;
         if (valid && (__umul64hi(n01, (uint64_t)d2) != 0 || n >= (1ull << 57))) { err = kErrBad; n = 0; }
         const uint64_t nbytes = n * esize;
-        const uint64_t st = (nbytes + 15) & ~15ull;
+        const uint64_t st = (nbytes + amask) & ~amask;
         stored[k] = st;
         oddf[k] = (uint32_t)(st - nbytes) >> 2;  // pad code: 0..3 words of zero pad
         dsta[k] = 0;
@@ -309,16 +314,13 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
                 if (i + 1 < B) next = __ldg(reinterpret_cast<const unsigned long long*>(brec + kBlockRec * (i + 1) + 40));
                 if (i == 0 && offset != 0) err = BS_ERR_CORRUPT;
                 if (offset > P_hdr || st > P_hdr - offset || offset + st != next) err = BS_ERR_CORRUPT;
-                else if (st != nbytes && p.payload != nullptr) {  // pad bytes are zero: the last 16-byte unit of the block
-                    const uint4 u = __ldg(reinterpret_cast<const uint4*>(p.payload + hb + offset + st - 16));
-                    const uint32_t data_words = 4u - ((uint32_t)(st - nbytes) >> 2);
-                    const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+                else if (st != nbytes && p.payload != nullptr) {  // pad bytes are zero: the 1..3 words behind the block's data
+                    const uint32_t* w = reinterpret_cast<const uint32_t*>(p.payload + hb + offset + nbytes);
                     uint32_t pad = 0;
-#pragma unroll
-                    for (uint32_t q = 0; q < 4; ++q) pad |= (q >= data_words) ? w[q] : 0u;
+                    for (uint32_t q = 0; q < (uint32_t)(st - nbytes) >> 2; ++q) pad |= __ldg(w + q);
                     if (pad != 0) err = BS_ERR_CORRUPT;
                 }
-                if (p.flags == BS_SCATTER_TO_ADDR) {
+                if ((p.flags & 1u) == BS_SCATTER_TO_ADDR) {
                     if (__ldg(p.out_dim + 3 * i) != d0 || __ldg(p.out_dim + 3 * i + 1) != d1 ||
                         __ldg(p.out_dim + 3 * i + 2) != d2) { if (!err) err = BS_ERR_ARG; }
                     const uint64_t da = __ldg(reinterpret_cast<const unsigned long long*>(p.out_addr + i));
@@ -380,7 +382,7 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
             uint64_t off, address;
             if (DESER) {
                 off = aux[k];
-                address = (p.flags == BS_SCATTER_TO_ADDR) ? dsta[k] : p.pool_base + run;
+                address = ((p.flags & 1u) == BS_SCATTER_TO_ADDR) ? dsta[k] : p.pool_base + run;
             } else {
                 off = run;
                 address = aux[k];
@@ -454,7 +456,7 @@ __device__ __forceinline__ void finalize(const ScanParams& p, const Shape& s, in
         else if (!DESER && total > p.capacity) status = BS_ERR_CAPACITY;
         else if (!DESER && p.expect_total != 0 && total != p.expect_total) status = BS_ERR_ARG;
         else if (ng + 1 > p.ws.n_granules_cap) status = BS_ERR_CAPACITY;
-        else if (DESER && p.flags == BS_LAYOUT_POOL && pool > p.pool_bytes) status = BS_ERR_CAPACITY;
+        else if (DESER && (p.flags & 1u) == BS_LAYOUT_POOL && pool > p.pool_bytes) status = BS_ERR_CAPACITY;
     }
     if (ok) {
         Blk e; e.off = P; e.addr = 0;
@@ -462,14 +464,15 @@ __device__ __forceinline__ void finalize(const ScanParams& p, const Shape& s, in
         if (ng < p.ws.n_granules_cap) p.ws.tile_first[ng] = (uint32_t)B;
     }
     HeadView hv;
-    hv.status = status; hv.T = (uint32_t)(ok ? s.T : s.rep_T); hv.B = (uint32_t)(ok ? B : s.rep_B); hv.dtype = s.dtype;
+    hv.status = status; hv.T = (uint32_t)(ok ? s.T : s.rep_T); hv.B = (uint32_t)(ok ? B : s.rep_B);
+    hv.dtype = s.dtype | (s.align == 8u ? BS_ALIGN8 : 0u);
     hv.hb = hb; hv.P = P; hv.ng = ng;
     sm.out = hv;
     if (!write_head) return;
     vh->n_tensors = hv.T;
     vh->n_blocks = hv.B;
     vh->header_bytes = hb;
-    vh->dtype = s.dtype;
+    vh->dtype = hv.dtype;
     vh->payload_bytes = P;
     vh->pool_bytes = pool;
     vh->n_granules = ng;
@@ -479,7 +482,7 @@ __device__ __forceinline__ void finalize(const ScanParams& p, const Shape& s, in
         r.total_bytes = total; r.header_bytes = hb; r.payload_bytes = P; r.pool_bytes = pool;
         r.status = status; r.n_tensors = hv.T; r.n_blocks = hv.B;
         for (int z = 0; z < 5; ++z) r.reserved[z] = 0;
-        r.reserved[2] = s.dtype;
+        r.reserved[2] = hv.dtype;
         *p.result = r;
     }
 }
@@ -555,7 +558,7 @@ __device__ __forceinline__ HeadView wait_ready(const WsHead* head, const Shape& 
         }
         HeadView hv;
         hv.status = (int32_t)(int8_t)(uint8_t)(w & 0xffu);
-        hv.T = (uint32_t)s.T; hv.B = (uint32_t)s.B; hv.dtype = s.dtype; hv.hb = s.hb;
+        hv.T = (uint32_t)s.T; hv.B = (uint32_t)s.B; hv.dtype = s.dtype | (s.align == 8u ? BS_ALIGN8 : 0u); hv.hb = s.hb;
         hv.P = DESER ? s.P_hdr : (w >> 8);
         if (s.code != 0) hv.P = 0;
         hv.ng = (hv.P + kGranule - 1) / kGranule;

@@ -41,12 +41,14 @@ def test_host_only_entry_points():
     assert bs.workspace_bytes(1, 7, 1 << 20) % 256 == 0
     assert bs.workspace_bytes(9008, 3299211, 45 << 30) < 200 << 20      # O(B) + 4 B per 16 KiB of stream
     raw = read_hex_fixture(os.path.join(ROOT, "tests", "golden", "p7_golden_stream.hex"))
-    assert bs.stream_info(raw) == dict(n_tensors=1, n_blocks=2, header_bytes=256, payload_bytes=32, total_bytes=288, dtype=0)
+    assert bs.stream_info(raw) == dict(n_tensors=1, n_blocks=2, header_bytes=256, payload_bytes=32, total_bytes=288, dtype=0, align=16)
+    g7 = read_hex_fixture(os.path.join(ROOT, "tests", "golden", "g7_golden_stream_align8.hex"))
+    assert bs.stream_info(g7) == dict(n_tensors=1, n_blocks=2, header_bytes=256, payload_bytes=24, total_bytes=280, dtype=0, align=8)
     f32 = read_hex_fixture(os.path.join(ROOT, "tests", "golden", "g4_golden_stream_f32.hex"))
     assert bs.stream_info(f32)["dtype"] == bs.F32
     for pos in (0, 8, 12, 16, 20, 24, 28, 48):
         bad = bytearray(raw)
-        bad[pos] ^= 4 if pos == 16 else 1      # dtype words 0..3 are element types
+        bad[pos] ^= 4 if pos in (16, 28) else 1      # align words 16 and 8 are both formats (16 ^ 4 = 20 is none)      # dtype words 0..3 are element types
         with pytest.raises(bs.BsError) as e:
             bs.stream_info(bad)
         assert e.value.code == bs.ERR_CORRUPT
