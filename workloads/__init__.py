@@ -17,6 +17,7 @@ from .blocksparse import (  # noqa: F401
     layered_view,
     make_config,
     make_set,
+    make_tree_set,
     selection_rules,
 )
 from .values import block_values, fill_pool_host, splitmix64_at  # noqa: F401

@@ -136,9 +136,17 @@ class BlockSparseSet:
         return int(self.dim.shape[0])
 
     @property
+    def legs(self) -> int:
+        """Legs per block record: 3 (matrices and MPS site tensors), 4 for sets that hold order-4 tensors."""
+        return int(self.dim.shape[1])
+
+    @property
     def nelems(self) -> np.ndarray:
         d = self.dim.astype(np.uint64)
-        return d[:, 0] * d[:, 1] * d[:, 2]
+        n = d[:, 0].copy()
+        for k in range(1, d.shape[1]):
+            n = n * d[:, k]
+        return n
 
     @property
     def data_bytes(self) -> int:
@@ -262,6 +270,64 @@ def layered_view(bset: BlockSparseSet, keep_unused: bool = False) -> dict:
     layers["tag"] = bset.tensors["tag"]
     return dict(structs=structs, layers=layers, qn=np.ascontiguousarray(m["cls_qn"][src]),
                 dim=np.ascontiguousarray(m["cls_dim"][src]))
+
+
+def make_tree_set(name: str, seed: int, D: int = 24, S: int = 6, M: int = 2, n_nodes: int = 3, n_ops: int = 4,
+                  pool_align: int = 512, scatter: bool = True) -> BlockSparseSet:
+    """Order-4 tensors: the nodes of a tree tensor network state (PAPER.md L41 "tree-like tensor network state methods";
+    SURVEY §8(f) NEXT-4 "rank-4 tensors") — two child legs, a physical leg and a parent leg, U(1)-blocked like the order-3 MPS
+    tensors of Eq. 2 (L47): block (a, b, sigma, c) kept iff label_a + label_b + q_sigma = label_c, shape (d_a, d_b, 1, d_c),
+    sign (+1,+1,+1,-1), dq = 0.  Child-leg labels come from the grid G(S, M, 0), the parent leg from a grid wide enough to
+    hold their sums; sector dims are multinomial draws summing to D per leg.  n_ops rank-2 operators on the child bond follow
+    (selection rules as in make_set), so one set mixes ranks: their legs 3 and 4 are unused (dim 1, labels 0).
+    Arrays have FOUR legs per block: qn [B][4][2], dim [B][4].  Inputs only (no stream arithmetic)."""
+    rng = np.random.default_rng(seed)
+    child = label_grid(S, M, 0)
+    parent = label_grid(4 * S + 8, 2 * M + 2, 0)
+    pidx = _label_index(parent)
+    rules = selection_rules()
+    qn_list, dim_list, recs = [], [], []
+    first = 0
+    for node in range(n_nodes):
+        da, db = dims_multinomial(rng, D, S), dims_multinomial(rng, D, S)
+        dc = dims_multinomial(rng, 2 * D, len(parent))
+        rows = []
+        for a, (na, ma) in enumerate(child):
+            for b, (nb, mb) in enumerate(child):
+                for sg, (ns, ms) in enumerate(LOCAL_LABELS):
+                    c = pidx.get((int(na) + int(nb) + int(ns), int(ma) + int(mb) + int(ms)))
+                    if c is not None:
+                        rows.append((a, b, sg, c))
+        rows = np.array(rows, dtype=np.int64).reshape(-1, 4)
+        q = np.zeros((len(rows), 4, 2), np.int32)
+        d = np.ones((len(rows), 4), np.uint32)
+        if len(rows):
+            q[:, 0], q[:, 1], q[:, 2], q[:, 3] = child[rows[:, 0]], child[rows[:, 1]], LOCAL_LABELS[rows[:, 2]], parent[rows[:, 3]]
+            d[:, 0], d[:, 1], d[:, 3] = da[rows[:, 0]], db[rows[:, 1]], dc[rows[:, 3]]
+        qn_list.append(q)
+        dim_list.append(d)
+        recs.append((4, first, len(rows), (0, 0), (1, 1, 1, -1), node, 0))
+        first += len(rows)
+    bond = dims_multinomial(rng, D, S)
+    for k in range(n_ops):
+        q3, d3 = _operator_class(child, bond, rules[k % len(rules)])
+        q = np.zeros((len(q3), 4, 2), np.int32)
+        d = np.ones((len(q3), 4), np.uint32)
+        q[:, :3], d[:, :3] = q3, d3
+        qn_list.append(q)
+        dim_list.append(d)
+        recs.append((2, first, len(q3), tuple(int(x) for x in rules[k % len(rules)]), (-1, 1, 0, 0), n_nodes + k, 0))
+        first += len(q3)
+    tensors = np.zeros(len(recs), dtype=TENSOR_REC_DTYPE)
+    for i, r in enumerate(recs):
+        tensors[i] = r
+    qn = np.ascontiguousarray(np.concatenate(qn_list)) if qn_list else np.zeros((0, 4, 2), np.int32)
+    dim = np.ascontiguousarray(np.concatenate(dim_list)) if dim_list else np.ones((0, 4), np.uint32)
+    d64 = dim.astype(np.uint64)
+    nelems = d64[:, 0] * d64[:, 1] * d64[:, 2] * d64[:, 3]
+    pool_off, pool_bytes = _place(rng, nelems, pool_align, scatter)
+    meta = dict(D=D, S=S, M=M, n_nodes=n_nodes, n_ops=n_ops, dims="multinomial", sigma=0.0, pool_align=pool_align, scatter=scatter)
+    return BlockSparseSet(name, seed, tensors, qn, dim, pool_off, pool_bytes, meta)
 
 
 # BASELINE.json configs 1-4 (config 5 = config 3 through the offload engine); "L" = operator count
