@@ -83,6 +83,16 @@ enum { BS_F64 = 0 /* e = 8 */, BS_F32 = 1 /* e = 4 */, BS_C64 = 2 /* e = 8 */, B
  * the bulk-copy engine and move as 8-byte words: expect roughly half the bandwidth of the padded format on sets with many
  * odd-sized blocks (DESIGN.md §18 has the numbers). */
 #define BS_ALIGN8 0x100u
+/* Tensors of rank up to 4 ("tree-like tensor network state methods": the nodes of a tree
+ * tensor network state are order-4; DESIGN.md §19 reading D20).  OR-ed into bs_set_desc.dtype it says that the per-block
+ * arrays have FOUR legs — qn [B][4][2], dim [B][4] — and that tensors may have rank 2, 3 or 4 (unused legs: dim 1, labels 0).
+ * The stream is then WIRE FORMAT v3 = v1 with a fourth leg:
+ *   fixed_header: as v1 with version = 3 and max_rank = 4;  tensor_rec: as v1;
+ *   block_rec   : i32 qn[4][2]; u32 dim[4]; u32 tensor; u32 reserved = 0; u64 offset      (64 bytes)
+ *   header_bytes = align128(64 + 32*T + 64*B) = bs_header_bytes_rank4(T, B);  payload and pool layout as v1.
+ * For deserialize / prefetch outputs the flag says how the caller shaped `out`'s arrays: a v3 stream needs it, a v1 stream must
+ * not have it (BS_ERR_ARG otherwise).  Not combined with BS_ALIGN8 or layered sets (BS_ERR_UNSUPPORTED). */
+#define BS_RANK4 0x200u
 #define BS_DTYPE_MASK 0xffu
 
 /* bs_deserialize / bs_prefetch_async destination layout */
@@ -94,7 +104,7 @@ enum {
 
 /* One tensor of the set; 32 bytes; identical bytes on the wire (PAPER L63 meta data). */
 typedef struct bs_tensor_rec {
-    uint32_t rank;        /* 2 (operator matrix) or 3 (MPS site tensor, PAPER Eq. 2) */
+    uint32_t rank;        /* 2 (operator matrix) or 3 (MPS site tensor, PAPER Eq. 2); 4 in a BS_RANK4 set (tree node) */
     uint32_t first_block; /* index of its first block in the per-block arrays */
     uint32_t n_blocks;    /* tensors partition the block table in order: first_block[t+1] = first_block[t] + n_blocks[t] */
     int32_t dq[2];        /* conserved charge (dN, d2Sz): sum_k sign[k]*qn[k] == dq for every block */
@@ -108,10 +118,11 @@ typedef struct bs_set_desc {
     uint32_t n_tensors;     /* T.  For bs_deserialize / bs_prefetch_async outputs: CAPACITY of tensors[] */
     uint32_t n_blocks;      /* B.  For outputs: CAPACITY of qn / dim / addr */
     uint32_t n_qn;          /* 2: (N, 2Sz) */
-    uint32_t dtype;         /* BS_F64, BS_F32, BS_C64 or BS_C128, optionally | BS_ALIGN8; for outputs: 0, see bs_result */
+    uint32_t dtype;         /* BS_F64, BS_F32, BS_C64 or BS_C128, optionally | BS_ALIGN8 or | BS_RANK4; for outputs: 0 or
+                               BS_RANK4 (the shape of qn / dim), the stream's type comes back in bs_result */
     bs_tensor_rec *tensors; /* [T]        */
-    int32_t *qn;            /* [B][3][2]  labels per leg; unused legs 0 */
-    uint32_t *dim;          /* [B][3]     extents; unused legs 1 */
+    int32_t *qn;            /* [B][3][2]  labels per leg; unused legs 0            (BS_RANK4: [B][4][2]) */
+    uint32_t *dim;          /* [B][3]     extents; unused legs 1                   (BS_RANK4: [B][4])    */
     uint64_t *addr;         /* [B]        device address of each dense, contiguous, row-major (last index
                                           fastest) block; must be 8-byte aligned, 16-byte aligned for the
                                           vector fast path */
@@ -126,7 +137,7 @@ typedef struct bs_result {
     int32_t status;         /* BS_OK or BS_ERR_* */
     uint32_t n_tensors;
     uint32_t n_blocks;
-    uint32_t reserved[5];   /* [0], [1]: see bs_layered_*; [2] = dtype of the stream (| BS_ALIGN8 for an align-8 stream);
+    uint32_t reserved[5];   /* [0], [1]: see bs_layered_*; [2] = dtype of the stream (| BS_ALIGN8 / BS_RANK4 as the stream is);
                                [3]: see bs_package_emit */
 } bs_result;
 
@@ -134,6 +145,7 @@ typedef struct bs_stream_info_t {
     uint64_t n_tensors, n_blocks, header_bytes, payload_bytes, total_bytes;
     uint64_t dtype; /* BS_F64 .. BS_C128 */
     uint64_t align; /* 16 or 8 (BS_ALIGN8) */
+    uint64_t max_rank; /* 3 (wire format v1) or 4 (wire format v3, BS_RANK4) */
 } bs_stream_info_t;
 
 /* Launch tuning.  NULL everywhere means defaults.  The stream produced never depends on these
@@ -158,12 +170,14 @@ int bs_last_cuda_error(void); /* cudaError_t of the last BS_ERR_CUDA on this thr
 
 /* align128(64 + 32*T + 48*B): the header size is known from the counts alone. */
 uint64_t bs_header_bytes(uint64_t n_tensors, uint64_t n_blocks);
+/* align128(64 + 32*T + 64*B): the same for a BS_RANK4 set (wire format v3). */
+uint64_t bs_header_bytes_rank4(uint64_t n_tensors, uint64_t n_blocks);
 
 /* Bytes of device workspace a call needs for a set of up to n_blocks blocks whose stream is at most
  * stream_capacity bytes: the offset table ("pointer structure") and scan state. */
 uint64_t bs_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint64_t stream_capacity);
 
-/* Parse the 64-byte fixed header (HOST memory).  BS_ERR_CORRUPT if it is not a v1 header. */
+/* Parse the 64-byte fixed header (HOST memory).  BS_ERR_CORRUPT if it is not a v1 or v3 header. */
 int bs_stream_info(const void *h_first_64_bytes, bs_stream_info_t *out);
 
 /* ---- serialize ------------------------------------------------------------ */

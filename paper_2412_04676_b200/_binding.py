@@ -12,6 +12,7 @@ OK, PENDING = 0, 1
 ERR_ARG, ERR_CAPACITY, ERR_CORRUPT, ERR_UNSUPPORTED, ERR_CUDA, ERR_IO = -1, -2, -3, -4, -5, -6
 F64, F32, C64, C128 = 0, 1, 2, 3
 ALIGN8 = 0x100   # OR-ed into a set's dtype: serialize an unpadded stream (bs.h BS_ALIGN8)
+RANK4 = 0x200    # OR-ed into a set's dtype: qn / dim have four legs per block, wire format v3 (bs.h BS_RANK4)
 LAYOUT_POOL, SCATTER_TO_ADDR = 0, 1
 VARIANT_DEFAULT, VARIANT_LDG, VARIANT_TMA = 0, 1, 2
 
@@ -61,7 +62,8 @@ class Result(C.Structure):
 
 class StreamInfo(C.Structure):
     _fields_ = [("n_tensors", C.c_uint64), ("n_blocks", C.c_uint64), ("header_bytes", C.c_uint64),
-                ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64), ("dtype", C.c_uint64), ("align", C.c_uint64)]
+                ("payload_bytes", C.c_uint64), ("total_bytes", C.c_uint64), ("dtype", C.c_uint64), ("align", C.c_uint64),
+                ("max_rank", C.c_uint64)]
 
 
 class Opts(C.Structure):
@@ -124,6 +126,8 @@ def lib():
     L.bs_last_cuda_error.restype = i32
     L.bs_header_bytes.restype = u64
     L.bs_header_bytes.argtypes = [u64, u64]
+    L.bs_header_bytes_rank4.restype = u64
+    L.bs_header_bytes_rank4.argtypes = [u64, u64]
     L.bs_workspace_bytes.restype = u64
     L.bs_workspace_bytes.argtypes = [u32, u32, u64]
     L.bs_stream_info.argtypes = [vp, C.POINTER(StreamInfo)]
@@ -214,6 +218,10 @@ def last_cuda_error() -> int:
 
 def header_bytes(n_tensors: int, n_blocks: int) -> int:
     return int(lib().bs_header_bytes(n_tensors, n_blocks))
+
+
+def header_bytes_rank4(n_tensors: int, n_blocks: int) -> int:
+    return int(lib().bs_header_bytes_rank4(n_tensors, n_blocks))
 
 
 def workspace_bytes(n_tensors: int, n_blocks: int, stream_capacity: int) -> int:

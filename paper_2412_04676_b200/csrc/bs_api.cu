@@ -37,7 +37,8 @@ static bool aligned(const void* p, uintptr_t a) { return ((uintptr_t)p & (a - 1)
 int check_set(const bs_set_desc* s)
 {
     if (s == nullptr) return BS_ERR_ARG;
-    if (s->n_qn != 2 || (s->dtype & BS_DTYPE_MASK) > (uint32_t)BS_C128 || (s->dtype & ~(BS_DTYPE_MASK | BS_ALIGN8)) != 0)
+    if (s->n_qn != 2 || (s->dtype & BS_DTYPE_MASK) > (uint32_t)BS_C128 || (s->dtype & ~(BS_DTYPE_MASK | BS_ALIGN8 | BS_RANK4)) != 0 ||
+        (s->dtype & (BS_ALIGN8 | BS_RANK4)) == (BS_ALIGN8 | BS_RANK4))
         return BS_ERR_UNSUPPORTED;
     if (s->n_tensors && (s->tensors == nullptr || !aligned(s->tensors, 16))) return BS_ERR_ARG;
     if (s->n_blocks && (s->qn == nullptr || !aligned(s->qn, 8))) return BS_ERR_ARG;
@@ -102,6 +103,7 @@ static MoveParams pack_params(const bs_set_desc* set, const WsLayout& L, void* d
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
     mp.flags = flags;
+    mp.rank4 = set->dtype & BS_RANK4;
     return mp;
 }
 
@@ -141,6 +143,7 @@ static ScanParams deserialize_scan_params(const void* d_header, const void* d_pa
     sp.out_dim = out->dim;
     sp.out_addr = out->addr;
     sp.flags = flags;
+    sp.dtype = out->dtype & BS_RANK4;  // the shape of the out arrays (three or four legs per block)
     return sp;
 }
 
@@ -171,6 +174,7 @@ static MoveParams unpack_params(const bs_set_desc* out, const WsLayout& L, const
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
     mp.flags = flags;
+    mp.rank4 = out->dtype & BS_RANK4;
     return mp;
 }
 
@@ -204,6 +208,7 @@ int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const Pkg
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
     mp.pkg = pm;
+    mp.rank4 = set->dtype & BS_RANK4;
     cudaError_t e = launch_move(false, mp, o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
@@ -234,6 +239,7 @@ int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const P
     mp.tune = o.reserved[0];
     mp.flags = flags;
     mp.pkg = pm;
+    mp.rank4 = out->dtype & BS_RANK4;
     cudaError_t e = launch_move(true, mp, o, sms, stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return BS_OK;
@@ -269,6 +275,8 @@ uint64_t bs_header_bytes(uint64_t n_tensors, uint64_t n_blocks)
     return align_up(kFixedHeader + kTensorRec * n_tensors + kBlockRec * n_blocks, kHeaderAlign);
 }
 
+uint64_t bs_header_bytes_rank4(uint64_t n_tensors, uint64_t n_blocks) { return header_bytes_of(n_tensors, n_blocks, BS_RANK4); }
+
 uint64_t bs_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint64_t stream_capacity)
 {
     (void)n_tensors;
@@ -284,10 +292,13 @@ int bs_stream_info(const void* h, bs_stream_info_t* out)
     memcpy(w, s, 32);
     memcpy(q, s + 32, 32);
     if (memcmp(s, "BSPARSE1", 8) != 0) return BS_ERR_CORRUPT;
-    if (w[2] != 1u || w[3] != 0x01020304u || w[4] > (uint32_t)BS_C128 || w[5] != 2u || w[6] != 3u || (w[7] != 16u && w[7] != 8u))
+    const bool v3 = w[2] == 3u;  // wire format v3: four legs per block record
+    if ((w[2] != 1u && !v3) || w[3] != 0x01020304u || w[4] > (uint32_t)BS_C128 || w[5] != 2u || w[6] != (v3 ? 4u : 3u) ||
+        (w[7] != 16u && !(w[7] == 8u && !v3)))
         return BS_ERR_CORRUPT;
     if (q[0] >= (1ull << 32) || q[1] >= (1ull << 32)) return BS_ERR_CORRUPT;
-    if (q[2] != bs_header_bytes(q[0], q[1])) return BS_ERR_CORRUPT;
+    if (q[2] != header_bytes_of(q[0], q[1], v3 ? BS_RANK4 : 0u)) return BS_ERR_CORRUPT;
+    out->max_rank = w[6];
     out->n_tensors = q[0];
     out->n_blocks = q[1];
     out->header_bytes = q[2];

@@ -157,7 +157,7 @@ int bs_engine_create(bs_engine** out, const bs_engine_cfg* cfg)
     if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e->ev_fence_c, cudaEventDisableTiming);
     if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e->ev_dep, cudaEventDisableTiming);
     e->ws_bytes = bs_workspace_bytes(e->cfg.max_tensors, e->cfg.max_blocks, e->cfg.max_stream_bytes);
-    e->header_cap = bs_header_bytes(e->cfg.max_tensors, e->cfg.max_blocks);
+    e->header_cap = header_bytes_of(e->cfg.max_tensors, e->cfg.max_blocks, BS_RANK4);  // room for 64-byte block records (wire format v3)
     {   // layered sets (wire format v2): C, T <= max_tensors; Bs, B <= max_blocks
         const uint64_t w2 = bs_layered_workspace_bytes(e->cfg.max_tensors, e->cfg.max_blocks, e->cfg.max_tensors,
                                                        e->cfg.max_blocks, e->cfg.max_stream_bytes);
@@ -284,6 +284,7 @@ int bs_engine_prefetch_impl(bs_engine* e, const void* h_pinned, uint64_t nbytes,
         if (known) info = *known;
         else if ((rc = bs_stream_info(h_pinned, &info))) return rc;  // the stream is in host RAM: its counts cost nothing to read
         if (info.total_bytes != nbytes) return BS_ERR_CORRUPT;
+        if ((info.max_rank == 4) != ((out->dtype & BS_RANK4) != 0)) return BS_ERR_ARG;  // the out arrays have the other shape
         if (info.n_blocks > e->cfg.max_blocks || info.n_tensors > e->cfg.max_tensors || info.header_bytes > e->header_cap ||
             nbytes > e->cfg.max_stream_bytes)
             return BS_ERR_CAPACITY;
@@ -403,7 +404,7 @@ static int offload_packages_impl(bs_engine* e, const bs_set_desc* set, const bs_
     if (set) {
         if (set->n_blocks > e->cfg.max_blocks || set->n_tensors > e->cfg.max_tensors) return BS_ERR_CAPACITY;
         if (!ws_layout(e->ws, e->ws_bytes, set->n_blocks, &L)) return BS_ERR_CAPACITY;
-        hb = bs_header_bytes(set->n_tensors, set->n_blocks);
+        hb = header_bytes_of(set->n_tensors, set->n_blocks, set->dtype);
     } else {
         if (lset->n_structs > e->cfg.max_tensors || lset->n_layers > e->cfg.max_tensors ||
             lset->n_struct_blocks > e->cfg.max_blocks || lset->n_addr > e->cfg.max_blocks)

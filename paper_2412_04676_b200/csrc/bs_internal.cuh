@@ -21,6 +21,7 @@ namespace bs {
 constexpr uint32_t kFixedHeader = 64;
 constexpr uint32_t kTensorRec = 32;
 constexpr uint32_t kBlockRec = 48;
+constexpr uint32_t kBlockRec4 = 64;  // wire format v3 (BS_RANK4): four legs per block record
 constexpr uint32_t kHeaderAlign = 128;
 constexpr uint32_t kPoolAlign = 256;
 constexpr uint32_t kGranule = 16384;  // bytes of payload per tile_first entry
@@ -37,6 +38,13 @@ struct __align__(16) Blk {
 
 // element size of a dtype (bs.h): f64 8, f32 4, c64 8, c128 16
 __host__ __device__ inline uint32_t elem_bytes(uint32_t dtype) { return dtype == BS_F32 ? 4u : (dtype == BS_C128 ? 16u : 8u); }
+// legs per block and bytes per block record of a set / stream, from the flags of its dtype word (bs.h BS_RANK4)
+__host__ __device__ inline uint32_t legs_of(uint32_t dtype_word) { return (dtype_word & BS_RANK4) ? 4u : 3u; }
+__host__ __device__ inline uint32_t block_rec_bytes(uint32_t dtype_word) { return (dtype_word & BS_RANK4) ? kBlockRec4 : kBlockRec; }
+__host__ __device__ inline uint64_t header_bytes_of(uint64_t T, uint64_t B, uint32_t dtype_word)
+{
+    return (kFixedHeader + kTensorRec * T + (uint64_t)block_rec_bytes(dtype_word) * B + (kHeaderAlign - 1)) / kHeaderAlign * kHeaderAlign;
+}
 
 struct __align__(16) ScanState {  // one tile of the chained scan: {flag | value, epoch tag}, read and written as ONE 16-byte access
     uint64_t word;
@@ -118,7 +126,7 @@ struct ScanParams {
     const uint32_t* dim;
     const uint64_t* addr;
     uint32_t T, B;           // SER: counts; DESER: capacities of the out arrays
-    uint32_t dtype;          // SER: element type of the set | BS_ALIGN8
+    uint32_t dtype;          // SER: element type of the set | BS_ALIGN8 | BS_RANK4; DESER: BS_RANK4 = the shape of the out arrays
     // DESER inputs
     const unsigned char* header;  // stream byte 0 .. header_bytes (device)
     const unsigned char* payload; // stream byte 0 when the payload is resident behind the header (pad-zero check), else null
@@ -177,6 +185,7 @@ struct MoveParams {
     uint32_t tile_bytes;
     uint32_t flags;
     uint32_t tune;                // bs_opts.reserved[0]: experiment switches of the TMA variant
+    uint32_t rank4;               // != 0: qn / dim have four legs per block (BS_RANK4; wire format v3)
     LayeredView lay;              // lay.on != 0: qn / dim are the structure block table, header is wire format v2
     PkgMap pkg;                   // pkg.cap != 0: the stream side is a set of package slots
 };

@@ -30,9 +30,10 @@ __device__ __forceinline__ uint4 header_unit(const MoveParams& p, uint64_t u, ui
                                              uint64_t P, uint32_t dtype)
 {
     uint4 v = make_uint4(0, 0, 0, 0);
+    const bool r4 = (dtype & BS_RANK4) != 0;  // wire format v3: four legs, 64-byte block records
     if (u < 4) {
-        if (u == 0) v = make_uint4(0x41505342u, 0x31455352u, 1u, 0x01020304u);  // "BSPARSE1", version, endian_tag
-        else if (u == 1) v = make_uint4(dtype & BS_DTYPE_MASK, 2u, 3u, (dtype & BS_ALIGN8) ? 8u : 16u);  // dtype, n_qn, max_rank, align
+        if (u == 0) v = make_uint4(0x41505342u, 0x31455352u, r4 ? 3u : 1u, 0x01020304u);  // "BSPARSE1", version, endian_tag
+        else if (u == 1) v = make_uint4(dtype & BS_DTYPE_MASK, 2u, r4 ? 4u : 3u, (dtype & BS_ALIGN8) ? 8u : 16u);  // dtype, n_qn, max_rank, align
         else if (u == 2) v = make_uint4(T, 0u, B, 0u);                           // u64 n_tensors, u64 n_blocks
         else v = make_uint4((uint32_t)hb, (uint32_t)(hb >> 32), (uint32_t)P, (uint32_t)(P >> 32));
         return v;
@@ -42,6 +43,20 @@ __device__ __forceinline__ uint4 header_unit(const MoveParams& p, uint64_t u, ui
         return __ldg(reinterpret_cast<const uint4*>(p.tensors) + u);
     }
     u -= 2ull * T;
+    if (r4) {  // i32 qn[4][2] (two units); u32 dim[4]; u32 tensor, u32 reserved, u64 offset
+        if (u < 4ull * B) {
+            const uint32_t r = (uint32_t)(u >> 2), part = (uint32_t)(u & 3);
+            if (part < 2) {
+                v = __ldg(reinterpret_cast<const uint4*>(p.qn + 8ull * r) + part);
+            } else if (part == 2) {
+                v = __ldg(reinterpret_cast<const uint4*>(p.dim + 4ull * r));
+            } else {
+                const uint64_t off = __ldcg(reinterpret_cast<const unsigned long long*>(&p.ws.blk[r].off));
+                v = make_uint4(tensor_of_block(p.tensors, T, r), 0u, (uint32_t)off, (uint32_t)(off >> 32));
+            }
+        }
+        return v;
+    }
     if (u < 3ull * B) {
         const uint32_t r = (uint32_t)(u / 3), part = (uint32_t)(u % 3);
         const int32_t* q = p.qn + 6ull * r;
@@ -72,6 +87,17 @@ __device__ __forceinline__ void rebuild_record(const MoveParams& p, uint64_t rec
     }
     const uint64_t r = rec - T;
     if (r >= B) return;
+    if (p.rank4) {  // wire format v3: 64-byte records, out arrays with four legs
+        const uint4* s = reinterpret_cast<const uint4*>(p.header + kFixedHeader + kTensorRec * (uint64_t)T + kBlockRec4 * r);
+        uint4* q = reinterpret_cast<uint4*>(p.qn + 8 * r);
+        q[0] = __ldg(s);
+        q[1] = __ldg(s + 1);
+        if ((p.flags & 1u) == BS_LAYOUT_POOL) {
+            *reinterpret_cast<uint4*>(p.dim + 4 * r) = __ldg(s + 2);
+            p.addr[r] = __ldcg(reinterpret_cast<const unsigned long long*>(&p.ws.blk[r].addr)) & ~7ull;
+        }
+        return;
+    }
     const uint4* s = reinterpret_cast<const uint4*>(p.header + kFixedHeader + kTensorRec * (uint64_t)T + kBlockRec * r);
     const uint4 r0 = __ldg(s), r1 = __ldg(s + 1), r2 = __ldg(s + 2);
     int2* q = reinterpret_cast<int2*>(p.qn + 6 * r);
@@ -207,6 +233,12 @@ __device__ __forceinline__ void write_header_warp(const MoveParams& p, uint32_t 
                                                   uint32_t lane)
 {
     if (lo >= hend) return;
+    if (dtype & BS_RANK4) {  // wire format v3: unit by unit (sets of order-4 tensors are small beside the operator sets)
+        const uint64_t u0 = lo / 16, n = (hend - lo) / 16;
+        for (uint64_t i = hw * 32 + lane; i < n; i += n_hw * 32)
+            __stcs(reinterpret_cast<uint4*>(stream_at(p, hb, lo + i * 16)), header_unit(p, u0 + i, T, B, hb, P, dtype));
+        return;
+    }
     const uint64_t rec0 = kFixedHeader + kTensorRec * (uint64_t)T;  // stream offset of block record 0
     const uint64_t rec_end = rec0 + kBlockRec * (uint64_t)B;
     {   // everything that is not a block record

@@ -275,7 +275,7 @@ int bs_package_range(uint64_t header_bytes, uint64_t total_bytes, uint64_t cap, 
 uint64_t bs_package_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint64_t stream_capacity)
 {
     // v1 workspace | slot table of the one-launch path (limits >= 16 KiB: at most one entry per 16 KiB) | header region
-    const uint64_t hb = bs_header_bytes(n_tensors, n_blocks);
+    const uint64_t hb = header_bytes_of(n_tensors, n_blocks, BS_RANK4);  // room for 64-byte block records (wire format v3)
     return bs_workspace_bytes(n_tensors, n_blocks, stream_capacity) + align_up(4 * (stream_capacity / kGranule + hb / kGranule + 4), 256) +
            256 + align_up(hb, 256);
 }
@@ -298,7 +298,7 @@ int bs_package_emit(const bs_set_desc* set, uint64_t total_bytes, uint64_t cap, 
     if (!ws_layout(d_ws, ws_bytes, set->n_blocks, &L)) return d_ws && ((uintptr_t)d_ws & 255) == 0 ? BS_ERR_CAPACITY : BS_ERR_ARG;
     int sms;
     if ((rc = device_sm_count(&sms))) return rc;
-    const uint64_t hb = bs_header_bytes(set->n_tensors, set->n_blocks);
+    const uint64_t hb = header_bytes_of(set->n_tensors, set->n_blocks, set->dtype);
     if (total_bytes == 0) {
         uint64_t hb2 = 0;
         if ((rc = bs_serialized_size(set, d_ws, ws_bytes, &hb2, &total_bytes, stream))) return rc;
@@ -361,7 +361,7 @@ int bs_package_unpack(const void* d_slots, uint64_t slot_bytes, uint64_t n_slots
     int rc;
     if ((rc = check_opts(o))) return rc;
     // workspace := v1 workspace | room for the assembled header region
-    const uint64_t hdr_cap = align_up(bs_header_bytes(out->n_tensors, out->n_blocks), 256);
+    const uint64_t hdr_cap = align_up(header_bytes_of(out->n_tensors, out->n_blocks, out->dtype), 256);
     if (d_ws == nullptr || ((uintptr_t)d_ws & 255)) return BS_ERR_ARG;
     if (ws_bytes < hdr_cap) return BS_ERR_CAPACITY;
     const uint64_t w1 = (ws_bytes - hdr_cap) & ~255ull;

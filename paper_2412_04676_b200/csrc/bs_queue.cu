@@ -284,10 +284,12 @@ static int queue_save_impl(bs_queue* q, uint64_t key, const bs_set_desc* set, co
     if (set) {
         en.info.n_tensors = set->n_tensors;
         en.info.n_blocks = set->n_blocks;
-        en.info.header_bytes = bs_header_bytes(set->n_tensors, set->n_blocks);
+        en.info.header_bytes = header_bytes_of(set->n_tensors, set->n_blocks, set->dtype);
+        en.info.max_rank = legs_of(set->dtype);
+        en.info.align = (set->dtype & BS_ALIGN8) ? 8 : 16;
         en.info.payload_bytes = total_bytes - en.info.header_bytes;
         en.info.total_bytes = total_bytes;
-        en.info.dtype = set->dtype;
+        en.info.dtype = set->dtype & BS_DTYPE_MASK;
     } else {
         en.linfo.n_structs = lset->n_structs;
         en.linfo.n_struct_blocks = lset->n_struct_blocks;

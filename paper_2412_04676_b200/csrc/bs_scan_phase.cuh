@@ -162,6 +162,7 @@ struct Shape {
     uint64_t rep_T, rep_B;  // deserialize, out arrays too small: the stream's counts, reported so the caller can size them
     uint32_t dtype;         // element type (bs.h BS_F64 ..), without flags
     uint32_t align;         // 16, or 8 (BS_ALIGN8: stored sizes are rounded to 8 only, DESIGN.md §18 reading D19)
+    uint32_t legs, rec;     // legs per block and bytes per block record: 3 / 48 (wire format v1), 4 / 64 (v3, BS_RANK4; D20)
     int code;               // != 0: the fixed header was rejected
     uint32_t n_tiles, n_items;
 };
@@ -173,6 +174,8 @@ __device__ __forceinline__ Shape shape_of(const ScanParams& p)
     s.T = p.T; s.B = p.B; s.hb = 0; s.P_hdr = 0; s.rep_T = 0; s.rep_B = 0; s.code = 0;
     s.dtype = p.dtype & BS_DTYPE_MASK;
     s.align = (p.dtype & BS_ALIGN8) ? 8u : 16u;
+    s.legs = legs_of(p.dtype);
+    s.rec = block_rec_bytes(p.dtype);
     if (DESER) {  // the fixed header (SURVEY §8(c) checks, in order)
         s.T = s.B = 0;
         if (p.nbytes < kFixedHeader) {
@@ -183,21 +186,22 @@ __device__ __forceinline__ Shape shape_of(const ScanParams& p)
             const uint64_t hT = (uint64_t)w2.x | ((uint64_t)w2.y << 32), hB = (uint64_t)w2.z | ((uint64_t)w2.w << 32);
             const uint64_t hH = (uint64_t)w3.x | ((uint64_t)w3.y << 32), hP = (uint64_t)w3.z | ((uint64_t)w3.w << 32);
             if (w0.x != 0x41505342u || w0.y != 0x31455352u)      s.code = BS_ERR_CORRUPT;  // "BSPARSE1"
-            else if (w0.z != 1u)                                  s.code = BS_ERR_CORRUPT;  // version
+            else if (w0.z != 1u && w0.z != 3u)                    s.code = BS_ERR_CORRUPT;  // version: 1, or 3 (four legs)
             else if (w0.w != 0x01020304u)                         s.code = BS_ERR_CORRUPT;  // endian_tag
             else if (w1.x > (uint32_t)BS_C128)                    s.code = BS_ERR_CORRUPT;  // dtype
             else if (w1.y != 2u)                                  s.code = BS_ERR_CORRUPT;  // n_qn
-            else if (w1.z != 3u)                                  s.code = BS_ERR_CORRUPT;  // max_rank
-            else if (w1.w != 16u && w1.w != 8u)                   s.code = BS_ERR_CORRUPT;  // align
+            else if (w1.z != (w0.z == 3u ? 4u : 3u))              s.code = BS_ERR_CORRUPT;  // max_rank
+            else if (w1.w != 16u && !(w1.w == 8u && w0.z == 1u))  s.code = BS_ERR_CORRUPT;  // align (8: wire format v1 only)
+            else if ((w0.z == 3u) != (s.legs == 4u))              s.code = BS_ERR_ARG;      // the out arrays have the other shape
             else if (w1.w == 8u && (p.flags & kFlagNoAlign8))     s.code = BS_ERR_UNSUPPORTED;  // the LDG variant moves 16-byte units
             else if (hT >= (1ull << 32) || hB >= (1ull << 32))   s.code = BS_ERR_CORRUPT;
-            else if (hH != align_up(kFixedHeader + kTensorRec * hT + kBlockRec * hB, kHeaderAlign)) s.code = BS_ERR_CORRUPT;
+            else if (hH != align_up(kFixedHeader + kTensorRec * hT + (uint64_t)s.rec * hB, kHeaderAlign)) s.code = BS_ERR_CORRUPT;
             else if (hH > p.nbytes || hP != p.nbytes - hH)        s.code = BS_ERR_CORRUPT;
             else if (hT > p.T || hB > p.B) { s.code = BS_ERR_CAPACITY; s.rep_T = hT; s.rep_B = hB; }  // out arrays too small
             else { s.T = hT; s.B = hB; s.hb = hH; s.P_hdr = hP; s.dtype = w1.x; s.align = w1.w; }
         }
     } else {
-        s.hb = align_up(kFixedHeader + kTensorRec * s.T + kBlockRec * s.B, kHeaderAlign);
+        s.hb = align_up(kFixedHeader + kTensorRec * s.T + (uint64_t)s.rec * s.B, kHeaderAlign);
     }
     const uint64_t nt = (s.B + kScanTile - 1) / kScanTile, ntt = (s.T + kScanTile - 1) / kScanTile;
     s.n_tiles = s.code ? 0u : (uint32_t)(nt ? nt : 1);
@@ -231,7 +235,7 @@ __device__ __forceinline__ void tensor_slice(const ScanParams& p, const Shape& s
                 const TensorHead q = load_tensor<DESER>(p, t - 1);
                 prev_end = (uint64_t)q.first + q.n;
             }
-            if (h.rank != 2 && h.rank != 3) code = kErrRank;
+            if (h.rank < 2 || h.rank > s.legs) code = kErrRank;
             else if (h.first != prev_end) code = kErrBad;
             else if (t == s.T - 1 && (uint64_t)h.first + h.n != s.B) code = kErrBad;
             else if (DESER && h.reserved != 0) code = kErrBad;
@@ -240,7 +244,7 @@ __device__ __forceinline__ void tensor_slice(const ScanParams& p, const Shape& s
     if (item == 0) {
         if (s.T == 0 && s.B != 0 && tid == 0) code = kErrBad;
         if (DESER) {  // header slack must be zero
-            const uint64_t used = kFixedHeader + kTensorRec * s.T + kBlockRec * s.B;
+            const uint64_t used = kFixedHeader + kTensorRec * s.T + (uint64_t)s.rec * s.B;
             const uint64_t z = used + 16ull * tid;
             if (z < s.hb) {
                 const uint4 w = __ldg(reinterpret_cast<const uint4*>(p.header + z));
@@ -273,26 +277,37 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
     for (uint32_t k = 0; k < kScanItems; ++k) {
         const uint64_t i = tile * kScanTile + (uint64_t)tid * kScanItems + k;
         const bool valid = i < B;
-        uint32_t d0 = 1, d1 = 1, d2 = 0;
+        uint32_t d0 = 1, d1 = 1, d2 = 0, d3 = 1;
         uint64_t a = 0, offset = 0;
         uint32_t owner = 0;
-        int32_t q4 = 0, q5 = 0;
+        uint32_t unused3 = 0, unused4 = 0;  // DESER: what must be {dim 1, labels 0} on leg 3 / leg 4 if the tensor does not use it
         if (valid) {
             if (DESER) {
-                const uint4* r = reinterpret_cast<const uint4*>(brec + kBlockRec * i);
-                const uint4 r1 = __ldg(r + 1), r2 = __ldg(r + 2);
-                q4 = (int32_t)r1.x; q5 = (int32_t)r1.y;
-                d0 = r1.z; d1 = r1.w; d2 = r2.x; owner = r2.y;
-                offset = (uint64_t)r2.z | ((uint64_t)r2.w << 32);
+                const uint4* r = reinterpret_cast<const uint4*>(brec + (uint64_t)s.rec * i);
+                if (s.legs == 3) {  // i32 qn[3][2]; u32 dim[3]; u32 tensor; u64 offset
+                    const uint4 r1 = __ldg(r + 1), r2 = __ldg(r + 2);
+                    d0 = r1.z; d1 = r1.w; d2 = r2.x; owner = r2.y;
+                    offset = (uint64_t)r2.z | ((uint64_t)r2.w << 32);
+                    unused3 = (d2 ^ 1u) | r1.x | r1.y;
+                } else {            // i32 qn[4][2]; u32 dim[4]; u32 tensor; u32 reserved; u64 offset
+                    const uint4 r1 = __ldg(r + 1), r2 = __ldg(r + 2), r3 = __ldg(r + 3);
+                    d0 = r2.x; d1 = r2.y; d2 = r2.z; d3 = r2.w; owner = r3.x;
+                    offset = (uint64_t)r3.z | ((uint64_t)r3.w << 32);
+                    unused3 = (d2 ^ 1u) | r1.x | r1.y;
+                    unused4 = (d3 ^ 1u) | r1.z | r1.w;
+                    if (r3.y != 0) err = BS_ERR_CORRUPT;  // reserved
+                }
             } else {
-                d0 = __ldg(p.dim + 3 * i); d1 = __ldg(p.dim + 3 * i + 1); d2 = __ldg(p.dim + 3 * i + 2);
+                const uint32_t* d = p.dim + (uint64_t)s.legs * i;
+                d0 = __ldg(d); d1 = __ldg(d + 1); d2 = __ldg(d + 2);
+                if (s.legs == 4) d3 = __ldg(d + 3);
                 a = __ldg(reinterpret_cast<const unsigned long long*>(p.addr + i));
             }
         }
-        // S1: nbytes = e * prod(dim) in u64 (D13), e = element size of the dtype; stored = align16(nbytes) (D3)
-        const uint64_t n01 = (uint64_t)d0 * d1;
-        uint64_t n = n01 * d2;
-        if (valid && (__umul64hi(n01, (uint64_t)d2) != 0 || n >= (1ull << 57))) { err = kErrBad; n = 0; }
+        // S1: nbytes = e * prod(dim) in u64 (D13), e = element size of the dtype; stored = align_up(nbytes, align) (D3, D19)
+        const uint64_t n01 = (uint64_t)d0 * d1, n23 = (uint64_t)d2 * d3;
+        uint64_t n = n01 * n23;
+        if (valid && (__umul64hi(n01, n23) != 0 || n >= (1ull << 57))) { err = kErrBad; n = 0; }
         const uint64_t nbytes = n * esize;
         const uint64_t st = (nbytes + amask) & ~amask;
         stored[k] = st;
@@ -307,11 +322,11 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
                 else {
                     const TensorHead h = load_tensor<true>(p, owner);
                     if (i < h.first || i >= (uint64_t)h.first + h.n) err = BS_ERR_CORRUPT;
-                    if (h.rank == 2 && (d2 != 1 || q4 != 0 || q5 != 0)) err = BS_ERR_CORRUPT;
+                    if ((h.rank < 3 && unused3 != 0) || (h.rank < 4 && unused4 != 0)) err = BS_ERR_CORRUPT;
                 }
                 // offsets = exclusive prefix sum of stored sizes, checked link by link, inside [0, P]
                 uint64_t next = P_hdr;
-                if (i + 1 < B) next = __ldg(reinterpret_cast<const unsigned long long*>(brec + kBlockRec * (i + 1) + 40));
+                if (i + 1 < B) next = __ldg(reinterpret_cast<const unsigned long long*>(brec + (uint64_t)s.rec * (i + 2) - 8));
                 if (i == 0 && offset != 0) err = BS_ERR_CORRUPT;
                 if (offset > P_hdr || st > P_hdr - offset || offset + st != next) err = BS_ERR_CORRUPT;
                 else if (st != nbytes && p.payload != nullptr) {  // pad bytes are zero: the 1..3 words behind the block's data
@@ -321,8 +336,10 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
                     if (pad != 0) err = BS_ERR_CORRUPT;
                 }
                 if ((p.flags & 1u) == BS_SCATTER_TO_ADDR) {
-                    if (__ldg(p.out_dim + 3 * i) != d0 || __ldg(p.out_dim + 3 * i + 1) != d1 ||
-                        __ldg(p.out_dim + 3 * i + 2) != d2) { if (!err) err = BS_ERR_ARG; }
+                    const uint32_t* od = p.out_dim + (uint64_t)s.legs * i;
+                    if (__ldg(od) != d0 || __ldg(od + 1) != d1 || __ldg(od + 2) != d2 || (s.legs == 4 && __ldg(od + 3) != d3)) {
+                        if (!err) err = BS_ERR_ARG;
+                    }
                     const uint64_t da = __ldg(reinterpret_cast<const unsigned long long*>(p.out_addr + i));
                     if (da & 7) { if (!err) err = BS_ERR_ARG; }
                     dsta[k] = da;
@@ -465,7 +482,7 @@ __device__ __forceinline__ void finalize(const ScanParams& p, const Shape& s, in
     }
     HeadView hv;
     hv.status = status; hv.T = (uint32_t)(ok ? s.T : s.rep_T); hv.B = (uint32_t)(ok ? B : s.rep_B);
-    hv.dtype = s.dtype | (s.align == 8u ? BS_ALIGN8 : 0u);
+    hv.dtype = s.dtype | (s.align == 8u ? BS_ALIGN8 : 0u) | (s.legs == 4u ? BS_RANK4 : 0u);
     hv.hb = hb; hv.P = P; hv.ng = ng;
     sm.out = hv;
     if (!write_head) return;
@@ -558,7 +575,7 @@ __device__ __forceinline__ HeadView wait_ready(const WsHead* head, const Shape& 
         }
         HeadView hv;
         hv.status = (int32_t)(int8_t)(uint8_t)(w & 0xffu);
-        hv.T = (uint32_t)s.T; hv.B = (uint32_t)s.B; hv.dtype = s.dtype | (s.align == 8u ? BS_ALIGN8 : 0u); hv.hb = s.hb;
+        hv.T = (uint32_t)s.T; hv.B = (uint32_t)s.B; hv.dtype = s.dtype | (s.align == 8u ? BS_ALIGN8 : 0u) | (s.legs == 4u ? BS_RANK4 : 0u); hv.hb = s.hb;
         hv.P = DESER ? s.P_hdr : (w >> 8);
         if (s.code != 0) hv.P = 0;
         hv.ng = (hv.P + kGranule - 1) / kGranule;

@@ -31,22 +31,30 @@ class DeviceSet:
         self.tensors, self.qn, self.dim, self.addr = tensors, qn, dim, addr
         self.n_tensors, self.n_blocks, self.dtype = n_tensors, n_blocks, dtype
 
+    @property
+    def legs(self) -> int:
+        """Legs per block of the qn / dim arrays: 4 for a BS_RANK4 set (wire format v3), else 3."""
+        return 4 if self.dtype & B.RANK4 else 3
+
     @classmethod
     def from_host(cls, tensors: np.ndarray, qn: np.ndarray, dim: np.ndarray, addr: np.ndarray, device="cuda",
                   dtype: int = B.F64):
         assert tensors.dtype.itemsize == 32
+        legs = 4 if dtype & B.RANK4 else 3
         return cls(_to_dev(tensors, device), _to_dev(qn.astype(np.int32, copy=False), device),
                    _to_dev(dim.astype(np.uint32, copy=False), device), _to_dev(addr.astype(np.uint64, copy=False), device),
-                   len(tensors), int(np.asarray(dim).reshape(-1, 3).shape[0]), dtype)
+                   len(tensors), int(np.asarray(dim).reshape(-1, legs).shape[0]), dtype)
 
     @classmethod
-    def empty(cls, cap_tensors: int, cap_blocks: int, device="cuda", fill: int | None = None):
+    def empty(cls, cap_tensors: int, cap_blocks: int, device="cuda", fill: int | None = None, rank4: bool = False):
         def mk(n):
             t = torch.empty(max(n, 16), dtype=torch.uint8, device=device)
             if fill is not None:
                 t.fill_(fill)
             return t
-        return cls(mk(32 * cap_tensors), mk(24 * cap_blocks), mk(12 * cap_blocks), mk(8 * cap_blocks), cap_tensors, cap_blocks)
+        legs = 4 if rank4 else 3
+        return cls(mk(32 * cap_tensors), mk(8 * legs * cap_blocks), mk(4 * legs * cap_blocks), mk(8 * cap_blocks), cap_tensors,
+                   cap_blocks, B.RANK4 if rank4 else B.F64)
 
     @property
     def desc(self) -> B.SetDesc:
@@ -58,8 +66,8 @@ class DeviceSet:
         Bn = self.n_blocks if n_blocks is None else n_blocks
         return dict(
             tensors=self.tensors[: 32 * T].cpu().numpy().view(_TENSOR_DTYPE).copy(),
-            qn=self.qn[: 24 * Bn].cpu().numpy().view(np.int32).reshape(Bn, 3, 2).copy(),
-            dim=self.dim[: 12 * Bn].cpu().numpy().view(np.uint32).reshape(Bn, 3).copy(),
+            qn=self.qn[: 8 * self.legs * Bn].cpu().numpy().view(np.int32).reshape(Bn, self.legs, 2).copy(),
+            dim=self.dim[: 4 * self.legs * Bn].cpu().numpy().view(np.uint32).reshape(Bn, self.legs).copy(),
             addr=self.addr[: 8 * Bn].cpu().numpy().view(np.uint64).copy(),
         )
 

@@ -41,9 +41,12 @@ def test_host_only_entry_points():
     assert bs.workspace_bytes(1, 7, 1 << 20) % 256 == 0
     assert bs.workspace_bytes(9008, 3299211, 45 << 30) < 200 << 20      # O(B) + 4 B per 16 KiB of stream
     raw = read_hex_fixture(os.path.join(ROOT, "tests", "golden", "p7_golden_stream.hex"))
-    assert bs.stream_info(raw) == dict(n_tensors=1, n_blocks=2, header_bytes=256, payload_bytes=32, total_bytes=288, dtype=0, align=16)
+    assert bs.stream_info(raw) == dict(n_tensors=1, n_blocks=2, header_bytes=256, payload_bytes=32, total_bytes=288, dtype=0, align=16, max_rank=3)
     g7 = read_hex_fixture(os.path.join(ROOT, "tests", "golden", "g7_golden_stream_align8.hex"))
-    assert bs.stream_info(g7) == dict(n_tensors=1, n_blocks=2, header_bytes=256, payload_bytes=24, total_bytes=280, dtype=0, align=8)
+    assert bs.stream_info(g7) == dict(n_tensors=1, n_blocks=2, header_bytes=256, payload_bytes=24, total_bytes=280, dtype=0, align=8, max_rank=3)
+    g8 = read_hex_fixture(os.path.join(ROOT, "tests", "golden", "g8_golden_stream_v3.hex"))
+    assert bs.stream_info(g8) == dict(n_tensors=2, n_blocks=3, header_bytes=384, payload_bytes=64, total_bytes=448, dtype=0, align=16, max_rank=4)
+    assert bs.header_bytes_rank4(2, 3) == 384
     f32 = read_hex_fixture(os.path.join(ROOT, "tests", "golden", "g4_golden_stream_f32.hex"))
     assert bs.stream_info(f32)["dtype"] == bs.F32
     for pos in (0, 8, 12, 16, 20, 24, 28, 48):
