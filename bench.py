@@ -326,9 +326,9 @@ def run_mine(args):
         dist.init_process_group("nccl", device_id=torch.device(dev))
         ready = True
     opts = None
-    if args.variant or args.tile_bytes or args.ctas_per_sm or args.stages or args.warps:
+    if args.variant or args.tile_bytes or args.ctas_per_sm or args.stages or args.warps or args.tune or args.fuse:
         opts = dict(variant=args.variant, tile_bytes=args.tile_bytes, ctas_per_sm=args.ctas_per_sm, stages=args.stages,
-                    warps=args.warps)
+                    warps=args.warps, tune=args.tune, fuse=args.fuse)
 
     def ev():
         return torch.cuda.Event(enable_timing=True)
@@ -1079,6 +1079,8 @@ def main():
     ap.add_argument("--ctas-per-sm", type=int, default=0)
     ap.add_argument("--stages", type=int, default=0)
     ap.add_argument("--warps", type=int, default=0)
+    ap.add_argument("--tune", type=int, default=0, help="TMA variant experiment bits: 1 = L2 evict_first on bulk loads, 2 = on bulk stores")
+    ap.add_argument("--fuse", type=int, default=0, help="0 = by size, 1 = size pass and movement as separate launches, 2 = one fused launch")
     ap.add_argument("--chunk-mb", type=int, default=256)
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--sample-mb", type=float, default=400.0, help="payload of the oracle's bounded sample")
