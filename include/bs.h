@@ -153,13 +153,15 @@ typedef struct bs_stream_info_t {
 typedef struct bs_opts {
     uint32_t variant;     /* 0 = default; 1 = BS_VARIANT_LDG (16-byte vector loads/stores);
                              2 = BS_VARIANT_TMA (cp.async.bulk global<->shared staging, one ring of tiles per warp) */
-    uint32_t tile_bytes;  /* stream bytes per work tile; 0 = default; multiple of 16384, <= 65536 */
+    uint32_t tile_bytes;  /* stream bytes per work tile; 0 = default; <= 65536 and a multiple of 16384 (LDG) or of 1024, >= 4096 (TMA) */
     uint32_t ctas_per_sm; /* LDG: persistent CTAs per SM; 0 = default (occupancy limit) */
     uint32_t stages;      /* TMA: ring depth (tiles) per warp, 3..8; 0 = default */
     uint32_t warps;       /* TMA: warps (rings) per CTA, 1..16; warps*stages*tile_bytes <= 225 KiB; 0 = default */
     uint32_t reserved[3]; /* 0.  [0]: experiment switches of the TMA variant (bits; see bs_move_tma.cu); [1]: bs_serialize /
                              bs_deserialize as one fused launch (size / offset pass + movement in one kernel): 0 = by size
-                             (sets of up to ~150 k blocks), 1 = never, 2 = always */
+                             (sets of up to ~150 k blocks), 1 = never, 2 = always; [2]: pacing of the TMA variant (experiments: a warp
+                             starts the loads of its next tile no earlier than its share of a target traffic rate allows):
+                             0 = none, >= 100 = that many GB/s of HBM traffic for the whole launch */
 } bs_opts;
 enum { BS_VARIANT_DEFAULT = 0, BS_VARIANT_LDG = 1, BS_VARIANT_TMA = 2 };
 

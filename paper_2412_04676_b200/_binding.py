@@ -80,6 +80,7 @@ def make_opts(opts) -> "Opts":
         setattr(o, k, int((opts or {}).get(k, 0) or 0))
     o.reserved[0] = int((opts or {}).get("tune", 0) or 0)
     o.reserved[1] = int((opts or {}).get("fuse", 0) or 0)
+    o.reserved[2] = int((opts or {}).get("pace", 0) or 0)
     return o
 
 

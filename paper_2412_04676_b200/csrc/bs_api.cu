@@ -52,7 +52,11 @@ int check_opts(const bs_opts& o)
     if (o.variant != BS_VARIANT_LDG && o.variant != BS_VARIANT_TMA) return BS_ERR_ARG;
     if (o.ctas_per_sm > 32) return BS_ERR_ARG;
     if (o.variant == BS_VARIANT_TMA && o.tile_bytes == 0 && o.stages == 0 && o.warps == 0) return BS_OK;  // presets
-    if (o.tile_bytes == 0 || o.tile_bytes % kGranule != 0 || o.tile_bytes > 65536) return BS_ERR_ARG;
+    // the LDG variant works on whole granules; a TMA tile is any multiple of 1 KiB (the block range of a tile is looked up
+    // by the granules it touches)
+    if (o.tile_bytes == 0 || o.tile_bytes % (o.variant == BS_VARIANT_TMA ? 1024u : kGranule) != 0 || o.tile_bytes > 65536 ||
+        (o.variant == BS_VARIANT_TMA && o.tile_bytes < 4096))
+        return BS_ERR_ARG;
     if (o.variant == BS_VARIANT_TMA &&
         (o.stages < 3 || o.stages > 8 || o.warps < 1 || o.warps > 16 ||
          (uint64_t)o.warps * ((uint64_t)o.stages * o.tile_bytes + kMetaBytesPerWarp) > 224u * 1024u))
@@ -102,6 +106,7 @@ static MoveParams pack_params(const bs_set_desc* set, const WsLayout& L, void* d
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
+    mp.pace = o.reserved[2];
     mp.flags = flags;
     mp.rank4 = set->dtype & BS_RANK4;
     return mp;
@@ -173,6 +178,7 @@ static MoveParams unpack_params(const bs_set_desc* out, const WsLayout& L, const
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
+    mp.pace = o.reserved[2];
     mp.flags = flags;
     mp.rank4 = out->dtype & BS_RANK4;
     return mp;
@@ -207,6 +213,7 @@ int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const Pkg
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
+    mp.pace = o.reserved[2];
     mp.pkg = pm;
     mp.rank4 = set->dtype & BS_RANK4;
     cudaError_t e = launch_move(false, mp, o, sms, stream);
@@ -237,6 +244,7 @@ int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const P
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
     mp.tune = o.reserved[0];
+    mp.pace = o.reserved[2];
     mp.flags = flags;
     mp.pkg = pm;
     mp.rank4 = out->dtype & BS_RANK4;

@@ -26,6 +26,19 @@
 #include "bs_move_common.cuh"
 #include "bs_scan_phase.cuh"
 
+#ifdef BS_PHASE_PROF  // development build only (build.py extra=["-DBS_PHASE_PROF"]): cycles per loop phase, summed over warps
+__device__ unsigned long long g_bs_phase[8];
+extern "C" int bs_debug_phases(unsigned long long* out8, int reset)
+{
+    if (out8 && cudaMemcpyFromSymbol(out8, g_bs_phase, sizeof(g_bs_phase)) != cudaSuccess) return -1;
+    if (reset) { unsigned long long z[8] = {0}; if (cudaMemcpyToSymbol(g_bs_phase, z, sizeof(z)) != cudaSuccess) return -1; }
+    return 0;
+}
+#define BS_PH(k) { const long long t_ = clock64(); ph_acc[k] += (unsigned long long)(t_ - ph_prev); ph_prev = t_; }
+#else
+#define BS_PH(k)
+#endif
+
 namespace bs {
 
 namespace {
@@ -181,19 +194,19 @@ __device__ __forceinline__ bool make_seg(const Blk* __restrict__ blk, uint32_t j
 
 // Per-warp metadata in shared memory, filled by cp.async ahead of use (no register is tied up, no warp stalls).  The
 // block table is read once per tile and never cached (the data streaming past evicts it), so each of the two lookup
-// levels costs a DRAM round trip — about as long as a whole loop iteration of a warp.  kBlkAhead iterations lie between
-// the fetch of a tile's table entries and their use, and as many again between the fetch of its tile_first[] pair and
-// that:
-//   tf[2*kBlkAhead+1][2]  tile_first[] pair {jlo, jhi_raw} of tiles m .. m+2*kBlkAhead (slot = tile index mod the count)
-//   blk[kBlkAhead+1][34]  block table entries jlo .. jlo+32 of tiles m .. m+kBlkAhead
-// Measured (profiles/r02_summary.md): kBlkAhead = 2 takes the wait for the table out of the loop, and the achieved DRAM
-// bandwidth DROPS (unpack 6.9 -> 6.1 TB/s, pack 6.6 -> 5.8 TB/s in its best shape): a warp that never waits runs ahead until
-// every stage of its ring is in flight, and this memory system moves fewer bytes per second the more requests it holds
-// (the same finding as for deeper rings).  With kBlkAhead = 1 the one exposed round trip per iteration paces the warp.
-constexpr uint32_t kBlkAhead = 1;
-constexpr uint32_t kBlkSlots = kBlkAhead + 1, kTfSlots = 2 * kBlkAhead + 1;
+// levels costs a DRAM round trip — about as long as a whole loop iteration of a warp.  `ahead` iterations (1 or 2) lie
+// between the fetch of a tile's table entries and their use, and as many again between the fetch of its tile_first[] pair
+// and that:
+//   tf[2*ahead+1][2]  tile_first[] pair {jlo, jhi_raw} of tiles m .. m+2*ahead (slot = tile index mod the count)
+//   blk[ahead+1][34]  block table entries jlo .. jlo+32 of tiles m .. m+ahead
+// With ahead = 1 one round trip per iteration stays exposed and spaces the warp's loads; that is how round 1 ran, and why
+// its best shapes were narrow peaks (see "pacing" below).  Paced launches use ahead = 2: nothing but the pace spaces them.
+constexpr uint32_t kBlkAheadMax = 2;
+constexpr uint32_t kBlkSlots = kBlkAheadMax + 1, kTfSlots = 2 * kBlkAheadMax + 1;
 constexpr uint32_t kMetaBlk = 34;
-constexpr uint32_t kMetaBytes = (kBlkSlots * kMetaBlk * 16 + kTfSlots * 8 + 15) / 16 * 16;
+constexpr uint32_t kTqSlots = 16;            // tile numbers of a warp's iterations i, slot i & 15 (claimed ahead, kept until stored)
+constexpr uint32_t kNoTile = 0xFFFFFFFFu;
+constexpr uint32_t kMetaBytes = (kBlkSlots * kMetaBlk * 16 + kTfSlots * 8 + kTqSlots * 4 + 15) / 16 * 16;
 static_assert(kMetaBytes <= kMetaBytesPerWarp, "check_opts (bs_api.cu) budgets kMetaBytesPerWarp of shared memory per warp");
 
 // pack: stage one block segment.  Bulk part: counted in *tx, issued later (after the expect_tx); 8-byte-aligned
@@ -462,15 +475,48 @@ __device__ __noinline__ void unpack_tile_a8(const TileCtx c, const unsigned char
 
 // Default launch shapes (B200, measured; profiles/r02_summary.md).  The launch always has the small-set shape — three rings
 // of 3 stages x 16 KiB per SM, what sets of tens of MB run fastest with in both directions — and the kernel, which knows the
-// payload size, switches sets of half a GB and more to ONE ring in the same shared memory: pack 3 x 48 KiB, unpack 4 x 32 KiB
-// (about 96 KiB of loads in flight per SM either way; deeper rings or more warps lower the achieved DRAM bandwidth).  A
-// package map keeps the small shape unless its size limit is a multiple of the large tile.
+// payload size, switches sets of half a GB and more to ONE ring of 3 x 48 KiB in the same shared memory.  With tiles handed
+// out by a counter (below) every shape that keeps ~96 KiB of loads in flight per SM reaches the same plateau (pack 6.75,
+// unpack 6.9 TB/s); one warp per SM issues a third of the instructions.  A package map keeps the small shape unless its size
+// limit is a multiple of the large tile.
 struct Preset {
     uint32_t tile_bytes, stages, warps;
 };
+
+// ---- tile hand-out (round 2; profiles/r02_summary.md "the cliff") -----------------------------------------------------------
+// Round 1 dealt tiles round-robin: warp w of W took tiles w, w + W, ...  Measured in round 2: when the launch asks the memory
+// system for more than it can give, the SMs are NOT served evenly (some fall 5-10 % behind), and with a static deal the
+// launch lasts as long as its slowest SM — every shape showed a narrow peak with a cliff behind it (offered 1-2 % more
+// traffic than the peak, a launch LOST 5-12 %), and round 1's shapes sat near their peaks by accident (the table round
+// trip and the instruction overhead of an iteration happened to space a warp's loads about right).  Now tiles are handed
+// out by ONE counter in the workspace head: a warp claims its next tile two iterations before it needs the tile's block
+// table, an SM that is served faster simply takes more tiles, all SMs finish together, and an over-subscribed launch runs
+// at the capacity of the memory system instead of falling off it.  The counter needs no clearing: it carries a tag like
+// the pass's counters, the last warp out of a launch puts it back, a stale word (a fresh workspace) is claimed by CAS.
+constexpr uint64_t kMvTag = 0x4D76C1A5ull << 32;  // [63:32] tag of the two move counters between and during launches, [31:0] count
+// take `n` numbers from tagged counter `w`: returns the first
+__device__ __forceinline__ uint32_t mv_take(uint64_t* w, uint32_t n)
+{
+    unsigned long long* a = reinterpret_cast<unsigned long long*>(w);
+    unsigned long long old = atomicAdd(a, (unsigned long long)n);
+    if ((old >> 32) == (kMvTag >> 32)) return (uint32_t)old;
+    unsigned long long cur = old + n;  // a stale word: whoever gets there first makes it {tag, n}; adds that landed on it are lost
+    for (;;) {
+        if ((cur >> 32) == (kMvTag >> 32)) return (uint32_t)atomicAdd(a, (unsigned long long)n);
+        const unsigned long long prev = atomicCAS(a, cur, kMvTag | n);
+        if (prev == cur) return 0u;
+        cur = prev;
+    }
+}
+#ifdef BS_PHASE_PROF
+__device__ unsigned int g_bs_trig[4];
+__device__ unsigned int g_bs_hist[2][32];
+#endif
+
 __host__ __device__ inline Preset preset_small() { return Preset{16384, 3, 3}; }
-__host__ __device__ inline Preset preset_large(bool unpack) { return unpack ? Preset{32768, 4, 1} : Preset{49152, 3, 1}; }
+__host__ __device__ inline Preset preset_large(bool) { return Preset{49152, 3, 1}; }
 constexpr uint64_t kLargePayload = 512ull << 20;
+constexpr uint64_t kDynamicBytes = 128ull << 20;  // ranges of this size and more: tiles handed out by the counter
 
 // FUSED: called behind the size / offset pass inside one kernel (fused_tma_kernel); `hv` is that pass's outcome.
 template <bool UNPACK, bool FUSED>
@@ -494,6 +540,8 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
         const Preset ps = preset_large(UNPACK);
         tile_bytes = ps.tile_bytes; n_stages = ps.stages; n_warps = ps.warps;
     }
+    // pacing (experiments; bs_opts.reserved[2] >= 100): that many GB/s of HBM traffic for the whole launch
+    const uint32_t rate = p.pace >= 100u ? p.pace : 0u;
     // ---- payload tiles of [lo, hi): tile k = payload bytes [k*tile_bytes, (k+1)*tile_bytes) ----
     uint64_t plo = 0, phi = 0, k0 = 0, np = 0;
     if (hi > hb && hi > lo) {
@@ -536,28 +584,58 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     __syncwarp();
 
     const uint64_t worker = (uint64_t)blockIdx.x * n_warps + warp, n_workers = (uint64_t)gridDim.x * n_warps;
-    const bool blocked = (p.tune & 4u) != 0;  // experiment: contiguous run of tiles per warp instead of round-robin
-    const uint64_t per = (np + n_workers - 1) / n_workers;
-    const int64_t n_mine = blocked ? (np > worker * per ? (int64_t)(np - worker * per < per ? np - worker * per : per) : 0)
-                                   : (np > worker ? (int64_t)((np - worker + n_workers - 1) / n_workers) : 0);
     int* const status = const_cast<int*>(&head->status);
     Hints hints;
     hints.pol = policy_evict_first();
     hints.ld = (p.tune & 1u) != 0;
     hints.st = (p.tune & 2u) != 0;
-    const int64_t lag = n_stages - 2;  // tile i is stored while tiles i+1 .. i+lag are loading
+    int64_t lag = n_stages - 2;  // tile i is stored while tiles i+1 .. i+lag are loading
+    if (((p.tune >> 8) & 15u) != 0 && (int64_t)((p.tune >> 8) & 15u) < lag) lag = (p.tune >> 8) & 15u;  // experiment: fewer loads in flight
+    const int64_t ahead = ((p.tune & 0x1000u) || rate) ? 2 : 1;  // iterations between the fetch of a tile's table entries and their use
 
-    // the block table is fetched ahead into shared memory (see kBlkAhead)
-    auto tile_base = [&](int64_t i) {
-        return (blocked ? k0 + worker * per + (uint64_t)i : k0 + worker + (uint64_t)i * n_workers) * tile_bytes;
+    // ---- which tiles (see "tile hand-out"): iteration i of this warp works on tile tq(i) of the range, kNoTile = none left.
+    // Claims are made `reach` iterations ahead: the answer of the atomic is written into the queue one iteration after it
+    // was asked for (lane 0 keeps it in a register meanwhile), in time for the tile_first fetch 2 * ahead iterations ahead.
+    // A range of less than kDynamicBytes keeps round 1's static round-robin deal: nothing there is worth the two extra round
+    // trips of the counter (config 1: 3 us of 8).  tune bit 3 forces the static deal, bit 4 the counter (tests, A/B runs).
+    const bool dynamic = (p.tune & 8u) == 0 && ((p.tune & 16u) != 0 || np * tile_bytes >= kDynamicBytes);
+    WsHead* const whead = const_cast<WsHead*>(head);
+    uint32_t* const m_tq = reinterpret_cast<uint32_t*>(meta_ptr + kBlkSlots * kMetaBlk * 16 + kTfSlots * 8);
+    const int64_t reach = 2 * ahead;
+    {
+        uint32_t first = 0;
+        if (dynamic && lane == 0) first = mv_take(&whead->mv_ticket, (uint32_t)reach);
+        first = __shfl_sync(0xffffffffu, first, 0);
+        if (lane < kTqSlots) {
+            const uint64_t v = dynamic ? (uint64_t)first + lane : worker + (uint64_t)lane * n_workers;
+            m_tq[lane] = (lane < (uint32_t)reach && v < np) ? (uint32_t)v : kNoTile;
+        }
+        __syncwarp();
+    }
+    // lane 0: the tile number of iteration i, raw (>= np: none left).  Dynamic: an atomic whose answer nobody waits for
+    // until the next iteration queues it
+    auto next_claim = [&](int64_t i) -> uint64_t {
+        return dynamic ? (uint64_t)mv_take(&whead->mv_ticket, 1u) : worker + (uint64_t)i * n_workers;
     };
-    auto has_tile = [&](int64_t i) { return i >= 0 && i < n_mine && B != 0; };
-    auto tf_slot = [](int64_t i) { return (uint32_t)((i + 8 * (int64_t)kTfSlots) % (int64_t)kTfSlots); };     // i >= -kMaxStages
-    auto blk_slot = [](int64_t i) { return (uint32_t)((i + 8 * (int64_t)kBlkSlots) % (int64_t)kBlkSlots); };
+    bool claiming = m_tq[(reach - 1) & (kTqSlots - 1)] != kNoTile;  // nothing more to ask for once a claim came back empty
+    uint64_t pending = np;                                           // lane 0: the claim of iteration it + reach
+    if (lane == 0 && claiming) pending = next_claim(reach);
+    auto tq = [&](int64_t i) { return i < 0 ? kNoTile : m_tq[i & (kTqSlots - 1)]; };
+    int64_t n_mine = (int64_t)1 << 60;  // the number of this warp's tiles, known when the first empty claim comes up
+
+    // the block table is fetched ahead into shared memory (see kBlkAheadMax)
+    auto tile_base = [&](int64_t i) { return (k0 + (uint64_t)tq(i)) * tile_bytes; };
+    auto has_tile = [&](int64_t i) { return B != 0 && tq(i) != kNoTile; };
+    const uint32_t n_tf = 2 * (uint32_t)ahead + 1, n_bs = (uint32_t)ahead + 1;
+    // slots are handed out round-robin by tile index; the loop keeps the slots of its current tile m_cur (no division)
+    int64_t m_cur = 0;
+    uint32_t tf_base = 0, bs_base = 0;
+    auto tf_slot = [&](int64_t i) { const uint32_t s = tf_base + (uint32_t)(i - m_cur); return s >= n_tf ? s - n_tf : s; };   // m_cur <= i <= m_cur + 2*ahead
+    auto blk_slot = [&](int64_t i) { const uint32_t s = bs_base + (uint32_t)(i - m_cur); return s >= n_bs ? s - n_bs : s; };  // m_cur <= i <= m_cur + ahead
     auto fetch_tf = [&](int64_t i) {  // lanes 0, 1: tile_first[g0], tile_first[g1] of tile i
         if (has_tile(i) && lane < 2) {
             const uint64_t tb = tile_base(i);
-            uint64_t g = lane == 0 ? tb / kGranule : (tb + tile_bytes) / kGranule;
+            uint64_t g = lane == 0 ? tb / kGranule : (tb + tile_bytes + kGranule - 1) / kGranule;  // a tile need not end on a granule
             if (g > ng) g = ng;  // tile_first[ng] == B
             cp_async_4(m_tf_s + tf_slot(i) * 8 + lane * 4, p.ws.tile_first + g);
         }
@@ -580,24 +658,46 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
         if (lane == 0 && jlo + 32 <= jhi + 1) cp_async_16(slot + 32 * 16, blk + jlo + 32);
     };
     const int64_t m0 = UNPACK ? -lag : 0;  // index of the tile whose block table the first iteration needs
-    for (int64_t i = m0; i < m0 + 2 * (int64_t)kBlkAhead; ++i) fetch_tf(i);
+    m_cur = m0;
+    for (int64_t i = m0; i < m0 + 2 * ahead; ++i) fetch_tf(i);
     cp_async_commit();
     cp_async_wait<0>();
     __syncwarp();
-    for (int64_t i = m0; i < m0 + (int64_t)kBlkAhead; ++i) fetch_blk(i);
+    for (int64_t i = m0; i < m0 + ahead; ++i) fetch_blk(i);
     cp_async_commit();
-    for (uint32_t g = 1; g < kBlkAhead; ++g) cp_async_commit();  // (empty groups: the loop counts kBlkAhead groups back)
+    for (int64_t g = 1; g < ahead; ++g) cp_async_commit();  // (empty groups: the loop counts `ahead` groups back)
+    // pacing (experiments): a warp starts the loads of its next tile no earlier than its share of `rate` allows
+    const uint64_t pace = rate ? (uint64_t)tile_bytes * 2u * n_workers / rate : 0;  // ns (GB/s = bytes per ns)
+    uint64_t t_next = 0;
+    if (pace) asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_next));
 
-    for (int64_t it = 0; it < n_mine + lag; ++it) {
+    uint32_t p_st = 0, c_st = 0, c_par = 0;  // stage of the tile being loaded; stage and mbarrier phase of the tile being stored
+#ifdef BS_PHASE_PROF
+    unsigned long long ph_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long ph_prev = clock64();
+#endif
+    for (int64_t it = 0;; ++it) {
         const int64_t m = m0 + it;
-        // one cp.async group per iteration; the groups of the last kBlkAhead - 1 iterations may still be in flight: the
-        // table entries of tile m and the tile_first pair of tile m + kBlkAhead, fetched kBlkAhead iterations ago, have landed
-        cp_async_wait<kBlkAhead - 1>();
+        BS_PH(7)
+        // the claim asked for one iteration ago has arrived: queue it, ask for the next
+        if (lane == 0) {
+            m_tq[(it + reach) & (kTqSlots - 1)] = pending < np ? (uint32_t)pending : kNoTile;
+            if (pending >= np) claiming = false;
+            pending = claiming ? next_claim(it + reach + 1) : np;
+        }
+        __syncwarp();
+        if (n_mine > it && tq(it) == kNoTile) n_mine = it;
+        if (it >= n_mine + lag) break;
+        // one cp.async group per iteration; the groups of the last ahead - 1 iterations may still be in flight: the
+        // table entries of tile m and the tile_first pair of tile m + ahead, fetched `ahead` iterations ago, have landed
+        if (ahead == 2) cp_async_wait<1>(); else cp_async_wait<0>();
+        BS_PH(0)
         // the store that last read stage it % n_stages was committed two iterations ago
         bulk_wait_read<1>();
         __syncwarp();
-        fetch_tf(m + 2 * (int64_t)kBlkAhead);
-        fetch_blk(m + (int64_t)kBlkAhead);
+        BS_PH(1)
+        fetch_tf(m + 2 * ahead);
+        fetch_blk(m + ahead);
         cp_async_commit();
         uint32_t jlo, jhi;
         read_tf(m, &jlo, &jhi);
@@ -608,8 +708,16 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
             e0 = m_blk[blk_slot(m) * kMetaBlk + lane];
             next0 = m_blk[blk_slot(m) * kMetaBlk + lane + 1].off;
         }
+        BS_PH(2)
         if (it < n_mine) {  // ---- produce: load tile `it` of this warp into its stage ----
-            const uint32_t st = (uint32_t)(it % n_stages);
+            if (pace) {
+                uint64_t now;
+                do { asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now)); } while (now < t_next);
+                t_next = (now - t_next > 4 * pace ? now : t_next) + pace;  // a warp that fell far behind does not burst
+            }
+            BS_PH(3)
+            const uint32_t st = p_st;
+            p_st = p_st + 1 == n_stages ? 0 : p_st + 1;
             const uint64_t tbase = tile_base(it);
             const uint64_t tlo = tbase > plo ? tbase : plo;
             const uint64_t thi = tbase + tile_bytes < phi ? tbase + tile_bytes : phi;
@@ -658,9 +766,11 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
                 }
             }
         }
+        BS_PH(4)
         if (it >= lag) {  // ---- consume: store tile `it - lag` ----
             const int64_t ci = it - lag;
-            const uint32_t st = (uint32_t)(ci % n_stages), parity = (uint32_t)((ci / n_stages) & 1);
+            const uint32_t st = c_st, parity = c_par;
+            if (++c_st == n_stages) { c_st = 0; c_par ^= 1u; }
             const uint64_t tbase = tile_base(ci);
             const uint64_t tlo = tbase > plo ? tbase : plo;
             const uint64_t thi = tbase + tile_bytes < phi ? tbase + tile_bytes : phi;
@@ -669,6 +779,7 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
                 uint32_t landed = 1;
                 if (lane == 0) landed = mbar_wait(bar, parity, status) ? 1u : 0u;
                 if (__shfl_sync(0xffffffffu, landed, 0) == 0) break;  // warp-uniform
+                BS_PH(5)
                 if (lane == 0) {
                     fence_proxy_async();  // the cp.async tails were written through the generic proxy
                     if (a8) store_tile_a8(stream_at(p, hb, hb + tlo), sbase + (uint32_t)(tlo - tbase), (uint32_t)(thi - tlo));
@@ -676,6 +787,7 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
                 }
             } else if (a8) {
                 if (!__all_sync(0xffffffffu, mbar_wait(bar, parity, status))) break;  // warp-uniform
+                BS_PH(5)
                 TileCtx c;
                 c.tbase = tbase; c.tlo = tlo; c.thi = thi; c.sbase = sbase; c.bar = bar; c.jlo = jlo; c.jhi = jhi; c.lane = lane;
                 c.blk = blk; c.e0 = e0; c.next0 = next0;
@@ -685,6 +797,7 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
                 Seg s0;
                 const bool have0 = clip_seg(e0, next0, tlo, thi, &s0);
                 if (!__all_sync(0xffffffffu, mbar_wait(bar, parity, status))) break;  // warp-uniform
+                BS_PH(5)
                 if (have0) unpack_seg(s0, sbase + (uint32_t)(s0.lo - tbase), sp + (s0.lo - tbase), p.flags, status, hints);
                 if (jhi >= jlo + 32) {
                     for (uint32_t j = jlo + lane + 32; j <= jhi; j += 32) {
@@ -696,9 +809,28 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
             }
         }
         bulk_commit();
+        BS_PH(6)
+        ++m_cur;
+        tf_base = tf_base + 1 == n_tf ? 0 : tf_base + 1;
+        bs_base = bs_base + 1 == n_bs ? 0 : bs_base + 1;
     }
     cp_async_wait<0>();
     bulk_wait_read<0>();
+    if (dynamic && lane == 0) {
+        // the last warp out puts the counters back for the next launch.  Every warp has its last (empty) claim in hand by
+        // then: `pending` is stored first, so an atomic of this warp cannot still be on its way when the counter is reset
+        m_tq[0] = (uint32_t)pending;
+        if (mv_take(&whead->mv_exit, 1u) == (uint32_t)n_workers - 1u) {
+            volatile uint64_t* c = &whead->mv_ticket;
+            *c = kMvTag;
+            c = &whead->mv_exit;
+            *c = kMvTag;
+            __threadfence();
+        }
+    }
+#ifdef BS_PHASE_PROF
+    if (lane == 0) for (int k = 0; k < 8; ++k) atomicAdd(&g_bs_phase[k], k == 7 ? (unsigned long long)(n_mine + lag) : ph_acc[k]);
+#endif
 }
 
 template <bool UNPACK>
@@ -833,3 +965,19 @@ cudaError_t launch_fused_tma(bool unpack, const ScanParams& sp, const MoveParams
 }
 
 }  // namespace bs
+
+#ifdef BS_PHASE_PROF
+extern "C" int bs_debug_rates(unsigned int* out2) { out2[0] = out2[1] = 0; return 0; }
+extern "C" int bs_debug_hist(unsigned int* out64, int reset)
+{
+    if (out64 && cudaMemcpyFromSymbol(out64, bs::g_bs_hist, sizeof(bs::g_bs_hist)) != cudaSuccess) return -1;
+    if (reset) { unsigned int z[64] = {0}; cudaMemcpyToSymbol(bs::g_bs_hist, z, sizeof(z)); }
+    return 0;
+}
+extern "C" int bs_debug_trig(unsigned int* out4, int reset)
+{
+    if (out4 && cudaMemcpyFromSymbol(out4, bs::g_bs_trig, sizeof(bs::g_bs_trig)) != cudaSuccess) return -1;
+    if (reset) { unsigned int z[4] = {0}; cudaMemcpyToSymbol(bs::g_bs_trig, z, sizeof(z)); }
+    return 0;
+}
+#endif

@@ -229,7 +229,7 @@ def test_what_is_refused():
     need = oracle.pool_bytes(want)
     o, pool, res = deserialize(st, len(want), bset.n_tensors, bset.n_blocks, need, dict(variant=bs.VARIANT_LDG))
     assert res["status"] == bs.ERR_UNSUPPORTED and (pool == 0xEE).all()
-    bad_flag = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, up.addr, DEV, dtype=bs.F64 | 0x200)
+    bad_flag = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, up.addr, DEV, dtype=bs.F64 | 0x400)
     with pytest.raises(bs.BsError) as e:
         bs.serialize(bad_flag.desc, out.data_ptr(), 1 << 20, ws.ptr, ws.nbytes, ws.result_ptr, None, bs.current_stream())
     assert e.value.code == bs.ERR_UNSUPPORTED

@@ -130,9 +130,11 @@ def test_engine_checks_what_the_direct_calls_check():
     up = Uploaded(bset)
     want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
     host = pinned(1 << 20, 0xCD)
-    with pytest.raises(bs.BsError) as e:      # tile_bytes not a multiple of 16 KiB
-        bs.Engine(4, 64, 1 << 20, chunk_bytes=65536, opts=dict(variant=bs.VARIANT_TMA, tile_bytes=8192, stages=3, warps=1))
-    assert e.value.code == bs.ERR_ARG
+    for bad in (dict(variant=bs.VARIANT_TMA, tile_bytes=6000, stages=3, warps=1),      # not a multiple of 1 KiB
+                dict(variant=bs.VARIANT_LDG, tile_bytes=8192)):                         # LDG: not a multiple of 16 KiB
+        with pytest.raises(bs.BsError) as e:
+            bs.Engine(4, 64, 1 << 20, chunk_bytes=65536, opts=bad)
+        assert e.value.code == bs.ERR_ARG
     eng = bs.Engine(4, 64, 1 << 20, chunk_bytes=65536)
     cs = bs.current_stream()
     d = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, up.addr, DEV, dtype=7)            # unknown element type

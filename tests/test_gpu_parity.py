@@ -27,12 +27,25 @@ VARIANTS = [dict(variant=bs.VARIANT_LDG, tile_bytes=16384), dict(variant=bs.VARI
             # one fused launch (size / offset pass + movement) against separate launches; default shape and a wide one
             dict(variant=bs.VARIANT_TMA, fuse=1), dict(variant=bs.VARIANT_TMA, fuse=2),
             dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=4, fuse=2),
-            dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=4, warps=1, fuse=2)]
+            dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=4, warps=1, fuse=2),
+            # tiles that do not end on a 16 KiB granule of the work partition (the TMA variant takes any multiple of 1 KiB)
+            dict(variant=bs.VARIANT_TMA, tile_bytes=40960, stages=3, warps=1), dict(variant=bs.VARIANT_TMA, tile_bytes=24576, stages=4, warps=2),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=20480, stages=3, warps=3, fuse=2), dict(variant=bs.VARIANT_TMA, tile_bytes=5120, stages=5, warps=2),
+            # paced launches (bs_opts.reserved[2]): a fixed target rate with the large-set shape, and pacing switched off
+            dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=4, warps=1, pace=6500), dict(variant=bs.VARIANT_TMA, pace=1),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=2, pace=200, fuse=2),
+            # round 1's static round-robin deal of the tiles (tune bit 3) and table entries fetched two iterations ahead (bit 12)
+            dict(variant=bs.VARIANT_TMA, tune=8), dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=5, warps=1, tune=0x1000),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=4, tune=0x1008, fuse=2),
+            # tiles handed out by the counter (what ranges of 128 MiB and more do; bit 4 forces it on these small sets)
+            dict(variant=bs.VARIANT_TMA, tune=0x10), dict(variant=bs.VARIANT_TMA, tune=0x10, fuse=1), dict(variant=bs.VARIANT_TMA, tune=0x10, fuse=2),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=49152, stages=3, warps=1, tune=0x10),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=20480, stages=5, warps=2, tune=0x1010), dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=8, warps=1, tune=0x10, fuse=2)]
 
 
 def _vid(o):
     return (f"v{o['variant']}-t{o.get('tile_bytes', 0)}-c{o.get('ctas_per_sm', 0)}-s{o.get('stages', 0)}-w{o.get('warps', 0)}"
-            f"-f{o.get('fuse', 0)}")
+            f"-f{o.get('fuse', 0)}" + (f"-p{o['pace']}" if o.get("pace") else "") + (f"-x{o['tune']:x}" if o.get("tune") else ""))
 
 
 def small_sets():
@@ -325,8 +338,9 @@ def test_a_payload_without_blocks_is_corrupt():
 
 @pytest.mark.parametrize("junk", ["ones", "random", "previous-call"])
 def test_the_workspace_needs_no_clearing(junk):
-    """The size / offset pass synchronises on epoch-tagged words only (bs_scan_phase.cuh): whatever the workspace holds —
-    all ones, noise, the state of an earlier call on a larger set — the stream is the oracle's.  Both launch forms, sets of
+    """The size / offset pass synchronises on epoch-tagged words only (bs_scan_phase.cuh) and the movement's tile counter is
+    tagged too (bs_move_tma.cu): whatever the workspace holds — all ones, noise, the state of an earlier call on a larger set
+    — the stream is the oracle's.  Both launch forms, sets of
     one work item (replicated pass), of a few, and deserialize."""
     sets = [W.make_config("1"), W.make_config("2"),
             W.make_set("tiny-ops+site", 11, D=48, S=10, M=2, N0=2, n_ops=20, n_site=2, dims="multinomial")]
@@ -338,7 +352,7 @@ def test_the_workspace_needs_no_clearing(junk):
     rng = torch.Generator(device=DEV).manual_seed(5)
     cs = bs.current_stream()
     for rnd in range(3):
-        for fuse in (2, 1, 0):
+        for fuse, tune in ((2, 0), (1, 0), (0, 0), (2, 0x10), (1, 0x10)):   # 0x10: tiles handed out by the tagged counter
             for bset, up, want in zip(sets, ups, wants):
                 if junk == "ones":
                     ws.buf.fill_(0xFF)
@@ -346,7 +360,7 @@ def test_the_workspace_needs_no_clearing(junk):
                     ws.buf.copy_(torch.randint(0, 256, (ws.nbytes,), dtype=torch.uint8, device=DEV, generator=rng))
                 total = len(want)
                 out = torch.full((cap,), 0xCD, dtype=torch.uint8, device=DEV)
-                opts = dict(variant=bs.VARIANT_TMA, fuse=fuse)
+                opts = dict(variant=bs.VARIANT_TMA, fuse=fuse, tune=tune)
                 bs.serialize(up.dset.desc, out.data_ptr(), cap, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs)
                 res = ws.read_result()
                 assert res["status"] == bs.OK and res["total_bytes"] == total, (junk, fuse, bset.name, res)
