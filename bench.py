@@ -326,9 +326,9 @@ def run_mine(args):
         dist.init_process_group("nccl", device_id=torch.device(dev))
         ready = True
     opts = None
-    if args.variant or args.tile_bytes or args.ctas_per_sm or args.stages or args.warps or args.tune or args.fuse:
+    if args.variant or args.tile_bytes or args.ctas_per_sm or args.stages or args.warps or args.tune or args.fuse or args.pace:
         opts = dict(variant=args.variant, tile_bytes=args.tile_bytes, ctas_per_sm=args.ctas_per_sm, stages=args.stages,
-                    warps=args.warps, tune=args.tune, fuse=args.fuse)
+                    warps=args.warps, tune=args.tune, fuse=args.fuse, pace=args.pace)
 
     def ev():
         return torch.cuda.Event(enable_timing=True)
@@ -466,9 +466,32 @@ def run_mine(args):
         except Exception as ex:   # the headline numbers stand on their own
             roofline["bulk_copy_error"] = repr(ex)
 
+    ab = None
+    if args.ab and not v2:
+        def t_pack(o):
+            return timed(lambda: f_range(dset.desc, stream.data_ptr(), 0, total, False, ws.ptr, ws.nbytes, ws.result_ptr, o, cs), 5)
+
+        def t_unpack(o):
+            return timed(lambda: bs.deserialize_range(stream.data_ptr(), 0, total, stream.data_ptr(), out.desc, bs.LAYOUT_POOL,
+                                                      ws.ptr, ws.nbytes, o, cs), 5)
+        ser()
+        ab_p = {}
+        # pack needs the serialize tables in the workspace, unpack the parsed ones: two passes over the list
+        rows_p = ab_table(bs, torch, t_pack, lambda o: 1.0, total, args.ab)
+        ser()
+        deser()
+        rows_u = ab_table(bs, torch, lambda o: 1.0, t_unpack, total, args.ab)
+        check_ok("A/B leg")
+        ab = [{"setting": rp["setting"], "opts": rp["opts"], "pack_GBs": rp["pack_GBs"], "unpack_GBs": ru["unpack_GBs"]}
+              for rp, ru in zip(rows_p, rows_u)]
+        ser()
+        deser()
+
     # ---- e2e leg: host (pinned) buffers through the engine, copies inside the timed region ----
     detail = {"serialize_stream_GBs": round(total / med_ser / 1e6, 1), "deserialize_stream_GBs": round(total / med_des / 1e6, 1),
               "size_pass_ms_incl_sync": round(scan_ms, 4)}
+    if ab is not None:
+        detail["ab"] = ab
     a, b = ev(), ev()
     e2e = None
     if not args.no_e2e:
@@ -753,6 +776,48 @@ def run_mine(args):
 
 def sm_count(torch, dev):
     return torch.cuda.get_device_properties(dev).multi_processor_count
+
+
+AB_SETTINGS = [
+    # name, opts.  `tune` bits: 8 = round 1's static round-robin deal of the tiles, 0x1000 = block table two iterations ahead,
+    # 1 / 2 = L2 evict_first on the bulk loads / stores; `pace` = target HBM traffic of the launch in GB/s
+    ("default", None),
+    ("counter 48K x3 x1", dict(tile_bytes=49152, stages=3, warps=1)),
+    ("static  48K x3 x1 (round 1 pack)", dict(tile_bytes=49152, stages=3, warps=1, tune=8)),
+    ("counter 32K x4 x1", dict(tile_bytes=32768, stages=4, warps=1)),
+    ("static  32K x4 x1 (round 1 unpack)", dict(tile_bytes=32768, stages=4, warps=1, tune=8)),
+    ("counter 40K x3 x1", dict(tile_bytes=40960, stages=3, warps=1)),
+    ("static  40K x3 x1", dict(tile_bytes=40960, stages=3, warps=1, tune=8)),
+    ("counter 64K x3 x1", dict(tile_bytes=65536, stages=3, warps=1)),
+    ("static  64K x3 x1", dict(tile_bytes=65536, stages=3, warps=1, tune=8)),
+    ("counter 48K x4 x1", dict(tile_bytes=49152, stages=4, warps=1)),
+    ("static  48K x4 x1", dict(tile_bytes=49152, stages=4, warps=1, tune=8)),
+    ("counter 16K x3 x3 (small-set shape)", dict(tile_bytes=16384, stages=3, warps=3)),
+    ("static  16K x3 x3", dict(tile_bytes=16384, stages=3, warps=3, tune=8)),
+    ("counter 24K x4 x2", dict(tile_bytes=24576, stages=4, warps=2)),
+    ("static  24K x4 x2", dict(tile_bytes=24576, stages=4, warps=2, tune=8)),
+    ("counter 16K x4 x2", dict(tile_bytes=16384, stages=4, warps=2)),
+    ("static  16K x4 x2", dict(tile_bytes=16384, stages=4, warps=2, tune=8)),
+    ("counter 48K x3 x1, table 2 ahead", dict(tile_bytes=49152, stages=3, warps=1, tune=0x1000)),
+    ("counter 48K x3 x1, evict_first loads", dict(tile_bytes=49152, stages=3, warps=1, tune=1)),
+    ("counter 48K x3 x1, evict_first stores", dict(tile_bytes=49152, stages=3, warps=1, tune=2)),
+    ("counter 48K x3 x1, evict_first both", dict(tile_bytes=49152, stages=3, warps=1, tune=3)),
+] + [(f"static  32K x4 x1, table 2 ahead, paced {r}", dict(tile_bytes=32768, stages=4, warps=1, tune=0x1008, pace=r))
+     for r in (6300, 6500, 6600, 6700, 6800, 6900, 7000, 7100)] \
+  + [(f"counter 32K x4 x1, table 2 ahead, paced {r}", dict(tile_bytes=32768, stages=4, warps=1, tune=0x1000, pace=r))
+     for r in (6500, 6700, 6900, 7100)]
+
+
+def ab_table(bs, torch, time_pack, time_unpack, total, rounds=3):
+    """A/B table of the pack and unpack kernels alone on the resident workload (profiles/r02_summary.md): every setting of
+    AB_SETTINGS, `rounds` interleaved passes, HBM GB/s = 2 * stream bytes / time per launch."""
+    rows = {name: {"pack": [], "unpack": []} for name, _ in AB_SETTINGS}
+    for _ in range(rounds):
+        for name, o in AB_SETTINGS:
+            o2 = None if o is None else dict(variant=bs.VARIANT_TMA, **o)
+            rows[name]["pack"].append(round(2 * total / time_pack(o2) / 1e6, 1))
+            rows[name]["unpack"].append(round(2 * total / time_unpack(o2) / 1e6, 1))
+    return [{"setting": name, "opts": o, "pack_GBs": rows[name]["pack"], "unpack_GBs": rows[name]["unpack"]} for name, o in AB_SETTINGS]
 
 
 def bulk_copy_ceiling(bs, torch, pool, stream, dev, opts, cs, n):
@@ -1079,7 +1144,14 @@ def main():
     ap.add_argument("--ctas-per-sm", type=int, default=0)
     ap.add_argument("--stages", type=int, default=0)
     ap.add_argument("--warps", type=int, default=0)
-    ap.add_argument("--tune", type=int, default=0, help="TMA variant experiment bits: 1 = L2 evict_first on bulk loads, 2 = on bulk stores")
+    ap.add_argument("--tune", type=lambda v: int(v, 0), default=0,
+                    help="TMA variant experiment bits: 1 = L2 evict_first on bulk loads, 2 = on bulk stores, 8 = round 1's static "
+                         "round-robin deal of the tiles, 0x10 = tiles from the counter whatever the size, 0x100..0xf00 = at most that "
+                         "many tiles loading beside the one being stored, 0x1000 = block table fetched two iterations ahead")
+    ap.add_argument("--ab", type=int, default=0, metavar="ROUNDS",
+                    help="also time the pack / unpack kernels alone under the settings of AB_SETTINGS, ROUNDS interleaved passes "
+                         "(detail.ab; the A/B tables of profiles/)")
+    ap.add_argument("--pace", type=int, default=0, help="TMA variant: pace the launches at this many GB/s of HBM traffic (experiments)")
     ap.add_argument("--fuse", type=int, default=0, help="0 = by size, 1 = size pass and movement as separate launches, 2 = one fused launch")
     ap.add_argument("--chunk-mb", type=int, default=256)
     ap.add_argument("--e2e-steps", type=int, default=5)

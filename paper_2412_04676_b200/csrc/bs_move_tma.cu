@@ -473,7 +473,7 @@ __device__ __noinline__ void unpack_tile_a8(const TileCtx c, const unsigned char
     }
 }
 
-// Default launch shapes (B200, measured; profiles/r02_summary.md).  The launch always has the small-set shape — three rings
+// Default launch shapes (B200, measured; profiles/r02b_summary.md).  The launch always has the small-set shape — three rings
 // of 3 stages x 16 KiB per SM, what sets of tens of MB run fastest with in both directions — and the kernel, which knows the
 // payload size, switches sets of half a GB and more to ONE ring of 3 x 48 KiB in the same shared memory.  With tiles handed
 // out by a counter (below) every shape that keeps ~96 KiB of loads in flight per SM reaches the same plateau (pack 6.75,
@@ -483,7 +483,7 @@ struct Preset {
     uint32_t tile_bytes, stages, warps;
 };
 
-// ---- tile hand-out (round 2; profiles/r02_summary.md "the cliff") -----------------------------------------------------------
+// ---- tile hand-out (round 2; profiles/r02b_summary.md "the cliff") -----------------------------------------------------------
 // Round 1 dealt tiles round-robin: warp w of W took tiles w, w + W, ...  Measured in round 2: when the launch asks the memory
 // system for more than it can give, the SMs are NOT served evenly (some fall 5-10 % behind), and with a static deal the
 // launch lasts as long as its slowest SM — every shape showed a narrow peak with a cliff behind it (offered 1-2 % more
