@@ -511,6 +511,10 @@ __device__ __forceinline__ uint32_t mv_take(uint64_t* w, uint32_t n)
 #ifdef BS_PHASE_PROF
 __device__ unsigned int g_bs_trig[4];
 __device__ unsigned int g_bs_hist[2][32];
+__device__ unsigned long long g_bs_tl[160][8];
+#define BS_TL(k) if (threadIdx.x == 0 && blockIdx.x < 160) { unsigned long long t_; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); g_bs_tl[blockIdx.x][k] = t_; }
+#else
+#define BS_TL(k)
 #endif
 
 __host__ __device__ inline Preset preset_small() { return Preset{16384, 3, 3}; }
@@ -709,6 +713,7 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
             next0 = m_blk[blk_slot(m) * kMetaBlk + lane + 1].off;
         }
         BS_PH(2)
+        if (it == 0) { BS_TL(4) }
         if (it < n_mine) {  // ---- produce: load tile `it` of this warp into its stage ----
             if (pace) {
                 uint64_t now;
@@ -767,6 +772,7 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
             }
         }
         BS_PH(4)
+        if (it == lag) { BS_TL(5) }
         if (it >= lag) {  // ---- consume: store tile `it - lag` ----
             const int64_t ci = it - lag;
             const uint32_t st = c_st, parity = c_par;
@@ -814,8 +820,10 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
         tf_base = tf_base + 1 == n_tf ? 0 : tf_base + 1;
         bs_base = bs_base + 1 == n_bs ? 0 : bs_base + 1;
     }
+    BS_TL(6)
     cp_async_wait<0>();
     bulk_wait_read<0>();
+    BS_TL(7)
     if (dynamic && lane == 0) {
         // the last warp out puts the counters back for the next launch.  Every warp has its last (empty) claim in hand by
         // then: `pending` is stored first, so an atomic of this warp cannot still be on its way when the counter is reset
@@ -857,10 +865,12 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) fused_tma_kernel(cons
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t s_bar[kMaxWarps * kMaxStages];
     __shared__ scan::HeadView s_hv;
+    BS_TL(0)
     scan::Shared& sm = *reinterpret_cast<scan::Shared*>(smem);
     const scan::Shape s = scan::shape_of<UNPACK>(sp);
     const bool replicated = s.n_items == 1;
     if (threadIdx.x < kScanThreads) scan::run<UNPACK>(sp, s, sp.tag, sm, replicated);
+    BS_TL(1)
     scan::HeadView hv;
     if (replicated) {
         __syncthreads();
@@ -869,7 +879,9 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) fused_tma_kernel(cons
     } else {
         hv = scan::wait_ready<UNPACK>(sp.ws.head, s, sp.tag, &s_hv);
     }
+    BS_TL(2)
     move_tma_body<UNPACK, true>(p, hv, opt_stages, opt_warps, smem, s_bar);
+    BS_TL(3)
 }
 
 // The kernels may use the whole 227 KiB of dynamic shared memory: opt in once per kernel and device.  The flags are atomic
@@ -974,6 +986,7 @@ extern "C" int bs_debug_hist(unsigned int* out64, int reset)
     if (reset) { unsigned int z[64] = {0}; cudaMemcpyToSymbol(bs::g_bs_hist, z, sizeof(z)); }
     return 0;
 }
+extern "C" int bs_debug_timeline(unsigned long long* out) { return cudaMemcpyFromSymbol(out, bs::g_bs_tl, sizeof(bs::g_bs_tl)) == cudaSuccess ? 0 : -1; }
 extern "C" int bs_debug_trig(unsigned int* out4, int reset)
 {
     if (out4 && cudaMemcpyFromSymbol(out4, bs::g_bs_trig, sizeof(bs::g_bs_trig)) != cudaSuccess) return -1;

@@ -18,13 +18,15 @@ def pinned(n, fill):
     return t
 
 
-@pytest.mark.parametrize("chunk,n_staging", [(65536, 2), (65536 * 5, 1), (65536 * 16, 3), (1 << 28, 2)])
-def test_offload_then_prefetch_round_trip(chunk, n_staging):
+@pytest.mark.parametrize("chunk,n_staging,opts", [(65536, 2, None), (65536 * 5, 1, None), (65536 * 16, 3, None), (1 << 28, 2, None),
+                                                  # every chunk's tiles handed out by the counter (what chunks of 128 MiB and more do)
+                                                  (65536 * 5, 2, dict(variant=2, tune=0x10)), (65536 * 16, 3, dict(variant=2, tune=0x10))])
+def test_offload_then_prefetch_round_trip(chunk, n_staging, opts):
     bset = W.make_config("2")
     up = Uploaded(bset)
     want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
     total = len(want)
-    eng = bs.Engine(bset.n_tensors, bset.n_blocks, total + 4096, chunk_bytes=chunk, n_staging=n_staging)
+    eng = bs.Engine(bset.n_tensors, bset.n_blocks, total + 4096, chunk_bytes=chunk, n_staging=n_staging, opts=opts)
     host = pinned(total + 4096, 0xCD)
     ws = bs.Workspace(bset.n_tensors, bset.n_blocks, total, DEV)
     hb, tot = bs.serialized_size(up.dset.desc, ws.ptr, ws.nbytes, bs.current_stream())

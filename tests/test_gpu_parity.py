@@ -434,9 +434,12 @@ def test_scatter_extent_mismatch_is_an_argument_error():
     assert ws.read_result()["status"] == bs.ERR_ARG and (dst == 0xEE).all()
 
 
-def test_calls_are_capturable_in_a_cuda_graph():
+@pytest.mark.parametrize("opts", [None, dict(variant=bs.VARIANT_TMA, tune=0x10), dict(variant=bs.VARIANT_TMA, tune=0x10, fuse=1)],
+                         ids=["default", "counter", "counter-two-launches"])
+def test_calls_are_capturable_in_a_cuda_graph(opts):
     """The calls only enqueue work (no host synchronisation, no allocation), so a launch-bound loop over small sets can be
-    captured once and replayed: the replay must give the oracle's bytes for whatever the blocks hold at replay time."""
+    captured once and replayed: the replay must give the oracle's bytes for whatever the blocks hold at replay time.  With
+    tiles handed out by the counter (tune 0x10; what large sets do) every replay finds the counter put back by the last one."""
     bset = W.make_config("2", n_ops=26)
     up = Uploaded(bset)
     want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
@@ -448,9 +451,9 @@ def test_calls_are_capturable_in_a_cuda_graph():
     pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
 
     def step(s):
-        bs.serialize(up.dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, None, s)
+        bs.serialize(up.dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, s)
         bs.deserialize(stream.data_ptr(), total, out.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
-                       ws.result_ptr, None, s)
+                       ws.result_ptr, opts, s)
 
     side = torch.cuda.Stream()
     side.wait_stream(torch.cuda.current_stream())
@@ -468,8 +471,11 @@ def test_calls_are_capturable_in_a_cuda_graph():
                              (np.uint64(rolled.ctypes.data) + up.host_offs.astype(np.uint64)).astype(np.uint64))
     stream.fill_(0xCD)
     pool.fill_(0xEE)
-    g.replay()
-    torch.cuda.synchronize()
-    assert ws.read_result()["status"] == bs.OK
-    assert (stream.cpu().numpy() == want2).all(), "graph replay: stream differs from the oracle's"
-    assert (pool.cpu().numpy()[:need] == oracle.deserialize(want2)["pool"][:need]).all()
+    for _ in range(3):   # several replays: each must leave the workspace as the next one expects it
+        stream.fill_(0xCD)
+        pool.fill_(0xEE)
+        g.replay()
+        torch.cuda.synchronize()
+        assert ws.read_result()["status"] == bs.OK
+        assert (stream.cpu().numpy() == want2).all(), "graph replay: stream differs from the oracle's"
+        assert (pool.cpu().numpy()[:need] == oracle.deserialize(want2)["pool"][:need]).all()
