@@ -1147,7 +1147,8 @@ def main():
     ap.add_argument("--tune", type=lambda v: int(v, 0), default=0,
                     help="TMA variant experiment bits: 1 = L2 evict_first on bulk loads, 2 = on bulk stores, 8 = round 1's static "
                          "round-robin deal of the tiles, 0x10 = tiles from the counter whatever the size, 0x100..0xf00 = at most that "
-                         "many tiles loading beside the one being stored, 0x1000 = block table fetched two iterations ahead")
+                         "many tiles loading beside the one being stored, 0x1000 = block table fetched two iterations ahead, "
+                         "0x20 = unpack asks the next stream tile into L2")
     ap.add_argument("--ab", type=int, default=0, metavar="ROUNDS",
                     help="also time the pack / unpack kernels alone under the settings of AB_SETTINGS, ROUNDS interleaved passes "
                          "(detail.ab; the A/B tables of profiles/)")

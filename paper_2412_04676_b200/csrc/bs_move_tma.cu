@@ -734,6 +734,11 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
                     } else {
                         mbar_arrive_expect_tx(bar, (uint32_t)(thi - tlo));
                         bulk_g2s_x(sbase + (uint32_t)(tlo - tbase), stream_at(p, hb, hb + tlo), (uint32_t)(thi - tlo), bar, hints);
+                        if ((p.tune & 0x20u) && tq(it + 1) != kNoTile) {  // experiment: the next tile of the stream into L2 now
+                            const uint64_t nb = tile_base(it + 1);
+                            const uint64_t nlo = nb > plo ? nb : plo, nhi = nb + tile_bytes < phi ? nb + tile_bytes : phi;
+                            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(stream_at(p, hb, hb + nlo)), "r"((uint32_t)(nhi - nlo)) : "memory");
+                        }
                     }
                 }
             } else if (a8) {
