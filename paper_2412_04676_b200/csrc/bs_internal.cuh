@@ -72,7 +72,7 @@ struct __align__(256) WsHead {
     uint32_t pad0[13];
     // ---- the v1 pass's own synchronisation words (bs_scan_phase.cuh), one 128-byte line each: the CTAs of a fused kernel
     // that poll `ready` must not slow the atomics of those still working down ----
-    ScanState ready;         // line 1: {payload_bytes << 8 | (status & 0xff), epoch tag} once tables and fields are final
+    ScanState ready;         // line 1: unused since round 2 (fused kernels poll ep_done and finalise for themselves)
     uint64_t pad1[14];
     uint64_t ep_ticket;      // line 2: work items handed out.  [63:24] a fixed "idle" tag, [23:0] count: the last CTA out of
     uint64_t pad2[15];       //         a launch puts the three counters back to {tag, 0}, so the next launch pays ONE atomic

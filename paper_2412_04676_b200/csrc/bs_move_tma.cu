@@ -525,7 +525,7 @@ constexpr uint64_t kDynamicBytes = 128ull << 20;  // ranges of this size and mor
 // FUSED: called behind the size / offset pass inside one kernel (fused_tma_kernel); `hv` is that pass's outcome.
 template <bool UNPACK, bool FUSED>
 __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::HeadView& hv, const uint32_t opt_stages,
-                                              const uint32_t opt_warps, unsigned char* smem, uint64_t* s_bar)
+                                              const uint32_t opt_warps, unsigned char* smem, uint64_t* s_bar, int* cta_status)
 {
     const WsHead* head = p.ws.head;
     if (hv.status != 0) {  // deferred error: nothing is written (the engine has a stale header blanked, see kFlagPoisonOnError)
@@ -588,7 +588,9 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     __syncwarp();
 
     const uint64_t worker = (uint64_t)blockIdx.x * n_warps + warp, n_workers = (uint64_t)gridDim.x * n_warps;
-    int* const status = const_cast<int*>(&head->status);
+    // where an error met while moving goes: the workspace's status word — in a fused kernel the CTA's own word (the head may
+    // still be on its way there from the pass's finalising CTA; the kernel's end posts it, see scan::leave)
+    int* const status = FUSED ? cta_status : const_cast<int*>(&head->status);
     Hints hints;
     hints.pol = policy_evict_first();
     hints.ld = (p.tune & 1u) != 0;
@@ -856,13 +858,13 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) move_tma_kernel(const
     scan::HeadView hv;
     hv.status = head->status; hv.T = head->n_tensors; hv.B = head->n_blocks; hv.dtype = head->dtype;
     hv.hb = head->header_bytes; hv.P = head->payload_bytes; hv.ng = head->n_granules;
-    move_tma_body<UNPACK, false>(p, hv, opt_stages, opt_warps, smem, s_bar);
+    move_tma_body<UNPACK, false>(p, hv, opt_stages, opt_warps, smem, s_bar, nullptr);
 }
 
 // ONE launch per bs_serialize / bs_deserialize call: the size / offset pass (bs_scan_phase.cuh) run by the
 // first kScanThreads threads of every CTA — its shared state lives at the start of the dynamic shared memory the rings use
 // afterwards — then the data movement above.  A set of one work item (<= 1024 blocks and tensors) runs the pass
-// replicated: no CTA waits for another; larger sets claim items from the ticket and wait for WsHead.ready.
+// replicated: no CTA waits for another; larger sets claim items from the ticket and wait for the completion count.
 template <bool UNPACK>
 __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) fused_tma_kernel(const ScanParams sp, const MoveParams p,
                                                                       const uint32_t opt_stages, const uint32_t opt_warps)
@@ -870,11 +872,13 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) fused_tma_kernel(cons
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t s_bar[kMaxWarps * kMaxStages];
     __shared__ scan::HeadView s_hv;
+    __shared__ int s_move_err;
+    if (threadIdx.x == 0) s_move_err = 0;
     BS_TL(0)
     scan::Shared& sm = *reinterpret_cast<scan::Shared*>(smem);
     const scan::Shape s = scan::shape_of<UNPACK>(sp);
     const bool replicated = s.n_items == 1;
-    if (threadIdx.x < kScanThreads) scan::run<UNPACK>(sp, s, sp.tag, sm, replicated);
+    if (threadIdx.x < kScanThreads) scan::run<UNPACK>(sp, s, sp.tag, sm, replicated, /*defer_exit=*/true);
     BS_TL(1)
     scan::HeadView hv;
     if (replicated) {
@@ -882,11 +886,21 @@ __global__ void __launch_bounds__((kMaxWarps + 1) * 32, 1) fused_tma_kernel(cons
         hv = sm.out;
         __syncthreads();  // the rings reuse the pass's shared memory
     } else {
-        hv = scan::wait_ready<UNPACK>(sp.ws.head, s, sp.tag, &s_hv);
+        hv = scan::wait_done<UNPACK>(sp, s, sp.tag, sm, &s_hv);  // (ends with a barrier: the rings may reuse the pass's shared memory)
+        // this CTA has seen the completion count: it is done with the pass's counters (the last CTA to say so resets them —
+        // by then every CTA has seen it)
+        if (threadIdx.x == 0) scan::leave(sp, sp.tag);
     }
     BS_TL(2)
-    move_tma_body<UNPACK, true>(p, hv, opt_stages, opt_warps, smem, s_bar);
+    move_tma_body<UNPACK, true>(p, hv, opt_stages, opt_warps, smem, s_bar, &s_move_err);
     BS_TL(3)
+    // An error met while moving (an mbarrier that never completed: seconds after the pass's finalising CTA wrote head and
+    // result) becomes the status of the call: the warp that met it sees its own word here, no barrier needed
+    if ((threadIdx.x & 31) == 0 && *(volatile int*)&s_move_err != 0) {
+        volatile WsHead* vh = sp.ws.head;
+        vh->status = s_move_err;
+        if (sp.result != nullptr) sp.result->status = s_move_err;
+    }
 }
 
 // The kernels may use the whole 227 KiB of dynamic shared memory: opt in once per kernel and device.  The flags are atomic

@@ -13,8 +13,8 @@
 //   - reports header / payload / total bytes and the deferred status in bs_result.
 //
 // Work is cut into ITEMS (item i = scan tile i of 1024 blocks + slice i of 1024 tensor records) that CTAs claim in
-// order from one ticket; the CTA that completes the last item finalises (totals, capacity checks, sentinel, result) and
-// publishes WsHead.ready.  An item only ever waits (look-back) for items claimed before it, which are being executed
+// order from one ticket; the CTA that completes the last item finalises (totals, capacity checks, sentinel, result).
+// An item only ever waits (look-back) for items claimed before it, which are being executed
 // by resident CTAs: forward progress needs no co-residency of the grid.
 //
 // No word the pass synchronises on needs clearing beforehand — the workspace may be uninitialised memory:
@@ -504,10 +504,28 @@ __device__ __forceinline__ void finalize(const ScanParams& p, const Shape& s, in
     }
 }
 
+// One thread per CTA, when the CTA is done with the launch's counters.  Every CTA has its last (out of range) ticket by the
+// time the last one is here: that one puts the counters back for the next launch.  A fused kernel calls this when the CTA
+// has SEEN the completion count (wait_done): the last CTA to say so resets ep_done, and by then nobody polls it any more.
+__device__ __forceinline__ void leave(const ScanParams& p, uint64_t tag)
+{
+    (void)tag;
+    WsHead* head = p.ws.head;
+    if (tagged_inc(&head->ep_exit, kIdleTag) == gridDim.x - 1) {
+        volatile uint64_t* c = &head->ep_ticket;
+        *c = kIdleTag;
+        c = &head->ep_done;
+        *c = kIdleTag;
+        c = &head->ep_exit;
+        *c = kIdleTag;
+        __threadfence();
+    }
+}
+
 // The pass, run by threads 0 .. kScanThreads-1 of every CTA of the grid.  Returns with those threads synchronised.
 // replicated (fused kernels only; s.n_items == 1): sm.out holds the outcome on return, nothing to wait for.
 template <bool DESER>
-__device__ __forceinline__ void run(const ScanParams& p, const Shape& s, uint64_t tag, Shared& sm, bool replicated)
+__device__ __forceinline__ void run(const ScanParams& p, const Shape& s, uint64_t tag, Shared& sm, bool replicated, bool defer_exit = false)
 {
     const uint32_t tid = threadIdx.x;
     WsHead* head = p.ws.head;
@@ -543,43 +561,31 @@ __device__ __forceinline__ void run(const ScanParams& p, const Shape& s, uint64_
                 __threadfence();
                 finalize<DESER, false>(p, s, read_err(head, tag), sm, true);
                 __threadfence();
-                st_state(&head->ready, (sm.out.P << 8) | (uint64_t)(uint8_t)(int8_t)sm.out.status, tag);
             }
         }
     }
-    // every CTA has its last (out of range) ticket by the time the last one is here: put the counters back for the next launch
-    if (tid == 0 && tagged_inc(&head->ep_exit, kIdleTag) == gridDim.x - 1) {
-        volatile uint64_t* c = &head->ep_ticket;
-        *c = kIdleTag;
-        c = &head->ep_done;
-        *c = kIdleTag;
-        c = &head->ep_exit;
-        *c = kIdleTag;
-        __threadfence();
-    }
+    if (!defer_exit && tid == 0) leave(p, tag);
 }
 
-// fused kernels, after run(): wait until the pass is complete (one thread per CTA polls).  Everything the data movement
-// needs comes out of the ONE polled word and the shape every CTA derived for itself: no second round trip to the head.
+// fused kernels, after run(): wait until every item of the pass is complete (one thread per CTA polls the completion
+// count, which a fused kernel leaves standing until its end), then work the outcome out HERE, from the shape every CTA
+// derived for itself, the totals the last tile's owner left and the epoch's error word — the CTA that completed the last
+// item writes the workspace head and the caller's result meanwhile, and nobody waits for it (round 2: ~2.5 us per call).
 template <bool DESER>
-__device__ __forceinline__ HeadView wait_ready(const WsHead* head, const Shape& s, uint64_t tag, HeadView* s_out)
+__device__ __forceinline__ HeadView wait_done(const ScanParams& p, const Shape& s, uint64_t tag, Shared& sm, HeadView* s_out)
 {
     if (threadIdx.x == 0) {
-        uint64_t w = 0, wt = 0;
+        const WsHead* head = p.ws.head;
         uint32_t ns = 32;
         for (;;) {
-            ld_state(&head->ready, &w, &wt);
-            if (wt == tag) break;
+            const uint64_t w = ld_acquire_u64(&head->ep_done);
+            if ((w & ~kCountMask) == kIdleTag && (w & kCountMask) >= s.n_items) break;
             __nanosleep(ns);
             if (ns < 256) ns *= 2;
         }
-        HeadView hv;
-        hv.status = (int32_t)(int8_t)(uint8_t)(w & 0xffu);
-        hv.T = (uint32_t)s.T; hv.B = (uint32_t)s.B; hv.dtype = s.dtype | (s.align == 8u ? BS_ALIGN8 : 0u) | (s.legs == 4u ? BS_RANK4 : 0u); hv.hb = s.hb;
-        hv.P = DESER ? s.P_hdr : (w >> 8);
-        if (s.code != 0) hv.P = 0;
-        hv.ng = (hv.P + kGranule - 1) / kGranule;
-        *s_out = hv;
+        finalize<DESER, false>(p, s, read_err(head, tag), sm, false);  // also writes the two sentinels (everybody: same values)
+        *s_out = sm.out;
+        __threadfence();
     }
     __syncthreads();
     return *s_out;
