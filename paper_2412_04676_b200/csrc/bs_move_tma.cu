@@ -206,6 +206,7 @@ constexpr uint32_t kBlkSlots = kBlkAheadMax + 1, kTfSlots = 2 * kBlkAheadMax + 1
 constexpr uint32_t kMetaBlk = 34;
 constexpr uint32_t kTqSlots = 16;            // tile numbers of a warp's iterations i, slot i & 15 (claimed ahead, kept until stored)
 constexpr uint32_t kNoTile = 0xFFFFFFFFu;
+static_assert((kMaxStages - 2) + 2 * kBlkAheadMax + 1 <= kTqSlots, "a claimed tile stays queued from its claim (2 * ahead iterations early) to its store (lag late)");
 constexpr uint32_t kMetaBytes = (kBlkSlots * kMetaBlk * 16 + kTfSlots * 8 + kTqSlots * 4 + 15) / 16 * 16;
 static_assert(kMetaBytes <= kMetaBytesPerWarp, "check_opts (bs_api.cu) budgets kMetaBytesPerWarp of shared memory per warp");
 

@@ -117,8 +117,10 @@ def test_P6_unpack_independent_of_decomposition(opts):
     assert (pool.cpu().numpy()[:need] == ref["pool"][:need]).all()
 
 
+@pytest.mark.parametrize("opts", [None, dict(variant=bs.VARIANT_TMA, tune=0x10), dict(variant=bs.VARIANT_TMA, tile_bytes=20480, stages=4, warps=2, tune=0x10)],
+                         ids=["default", "counter", "counter-20K"])
 @pytest.mark.parametrize("chunk", [16, 4096, 65536, 100000 * 16, 1 << 22])
-def test_P6_concat_of_ranges_is_the_stream(chunk):
+def test_P6_concat_of_ranges_is_the_stream(chunk, opts):
     bset = W.make_config("2")
     up = Uploaded(bset)
     want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
@@ -133,7 +135,7 @@ def test_P6_concat_of_ranges_is_the_stream(chunk):
     first = True
     for lo, hi in zip(cuts[:-1], cuts[1:]):
         seg = torch.full((hi - lo + 32,), 0x77, dtype=torch.uint8, device=DEV)
-        bs.serialize_range(up.dset.desc, seg.data_ptr(), lo, hi, first, ws.ptr, ws.nbytes, ws.result_ptr, None,
+        bs.serialize_range(up.dset.desc, seg.data_ptr(), lo, hi, first, ws.ptr, ws.nbytes, ws.result_ptr, opts,
                            bs.current_stream())
         first = False
         assert (seg[hi - lo:] == 0x77).all(), "range call wrote beyond its segment"
