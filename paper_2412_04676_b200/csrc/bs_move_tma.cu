@@ -15,9 +15,10 @@
 //            the stream must not be written past the end of a destination block).
 //
 // Each warp runs its own ring of `stages` tiles in dynamic shared memory (software pipeline: tile i is loaded while
-// tile i-(stages-2) is stored), `warps` rings per CTA, one persistent CTA per SM; tiles are dealt round-robin over
-// all warps of the grid.  Blocks whose address is only 8-byte aligned take a correct slower path of
-// 8-byte cp.async / 8-byte stores.  The stream produced is byte-identical to the LDG variant's (tests: P6).
+// tile i-(stages-2) is stored), `warps` rings per CTA, one persistent CTA per SM; the warps of the grid claim tiles
+// from one counter in the workspace head (round 2, "tile hand-out" below; small ranges: dealt round-robin).  Blocks
+// whose address is only 8-byte aligned take a correct slower path of 8-byte cp.async / 8-byte stores.
+// The stream produced is byte-identical to the LDG variant's (tests: P6).
 //
 // Roofline: pure data movement — 1 byte read + 1 byte written per stream byte, HBM-bound; ~2 instructions per
 // block segment and per tile instead of ~70 per 512 bytes in the LDG variant.
