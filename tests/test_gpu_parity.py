@@ -378,7 +378,9 @@ def test_the_workspace_needs_no_clearing(junk):
                 assert (pool.cpu().numpy() == oracle.deserialize(want)["pool"][:need]).all()
 
 
-def test_fused_calls_on_two_streams_at_once():
+@pytest.mark.parametrize("opts", [dict(variant=bs.VARIANT_TMA, fuse=2), dict(variant=bs.VARIANT_TMA, fuse=2, tune=0x10),
+                                  dict(variant=bs.VARIANT_TMA, fuse=1, tune=0x10)], ids=["fused", "fused-counter", "two-launches-counter"])
+def test_fused_calls_on_two_streams_at_once(opts):
     """bs.h: calls are re-entrant.  Two streams each run fused serialize + deserialize calls back to back on their own
     workspaces; the kernels are persistent (one CTA per SM each) and may be co-resident only in part — items are claimed
     from a ticket, so a resident CTA never waits for one that is not (bs_scan_phase.cuh).  Results: the oracle's."""
@@ -395,7 +397,6 @@ def test_fused_calls_on_two_streams_at_once():
                           dst=bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB),
                           pool=torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)))
     torch.cuda.synchronize()
-    opts = dict(variant=bs.VARIANT_TMA, fuse=2)
     for it in range(20):
         for s, ln in zip(streams, lanes):
             bs.serialize(up.dset.desc, ln["out"].data_ptr(), total, ln["ws"].ptr, ln["ws"].nbytes, ln["ws"].result_ptr, opts,
