@@ -74,6 +74,28 @@ def test_argument_errors_need_no_device():
     assert e.value.code == bs.ERR_CAPACITY
 
 
+def test_launch_shapes_are_checked_without_a_device():
+    """bs_opts: a TMA tile is any multiple of 1 KiB from 4 KiB to 64 KiB (round 2), an LDG tile a multiple of 16 KiB; rings
+    must fit the shared memory.  A shape the kernels cannot run is BS_ERR_ARG before anything touches the device."""
+    d = bs.make_desc(1, 1, 16, 16, 16, 16)
+    bad = [dict(variant=bs.VARIANT_TMA, tile_bytes=6000, stages=3, warps=1), dict(variant=bs.VARIANT_TMA, tile_bytes=2048, stages=3, warps=1),
+           dict(variant=bs.VARIANT_TMA, tile_bytes=66560, stages=3, warps=1), dict(variant=bs.VARIANT_LDG, tile_bytes=8192),
+           dict(variant=bs.VARIANT_LDG, tile_bytes=20480), dict(variant=bs.VARIANT_TMA, tile_bytes=20480, stages=6, warps=2),
+           dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=2, warps=1), dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=9, warps=1),
+           dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=17), dict(variant=7)]
+    for o in bad:
+        with pytest.raises(bs.BsError) as e:
+            bs.serialize(d, 256, 1024, 256, 1 << 20, 0, o)
+        assert e.value.code == bs.ERR_ARG, o
+    import torch
+    if not torch.cuda.is_available():   # a good shape gets as far as the device: there is none here
+        for o in (dict(variant=bs.VARIANT_TMA, tile_bytes=20480, stages=5, warps=2), dict(variant=bs.VARIANT_TMA, tile_bytes=5120, stages=8, warps=4),
+                  dict(variant=bs.VARIANT_TMA, tile_bytes=65536, stages=3, warps=1, pace=6500, tune=0x1018), dict(variant=bs.VARIANT_LDG, tile_bytes=49152)):
+            with pytest.raises(bs.BsError) as e:
+                bs.serialize(d, 256, 1024, 256, 1 << 20, 0, o)
+            assert e.value.code == bs.ERR_CUDA, o
+
+
 def test_no_cpu_fallback_without_a_device():
     import torch
     if torch.cuda.is_available():
