@@ -713,6 +713,7 @@ def run_mine(args):
 
     # ---- config 5: exposed IO of an offload overlapped with a stand-in contraction (rank 0 only) ----
     if rank == 0 and not args.no_config5 and not v2:
+        c5 = None
         try:
             c5 = config5(args, dev, opts)
             detail["config5"] = c5
@@ -728,6 +729,21 @@ def run_mine(args):
                     e2e["sweep_speedup_queue_over_sync_io"] = c5["sweep_fig3"]["speedup_queue_over_sync"]
         except Exception as ex:  # the headline numbers stand on their own
             detail["config5"] = {"error": repr(ex)}
+        # the same protocol at the total BASELINE.json states for config 3 ("10-20 GB": workload 3L, 11 GB, 42 chunks of 256 MiB)
+        if e2e is not None and not args.no_at_scale and args.workload != "3L":
+            try:
+                del c5
+                torch.cuda.empty_cache()
+                cl = config5(args, dev, opts, name="3L", full=False)
+                hs, hl = cl["headline"], cl["prefetch"]["headline"]
+                e2e["at_scale_3L"] = {"stream_bytes": cl["stream_bytes"], "exposed_io_frac_save": hs["exposed_io_frac"],
+                                      "exposed_io_frac_load": hl["exposed_io_frac"], "exposed_io_r_actual": [hs["r_actual"], hl["r_actual"]],
+                                      "sustained_pcie_GBs_save": hs["sustained_pcie_GBs"], "sustained_pcie_GBs_load": hl["sustained_pcie_GBs"],
+                                      "offload_alone_GBs": round(cl["stream_bytes"] / cl["T_io_ms"] / 1e6, 2),
+                                      "prefetch_alone_GBs": round(cl["stream_bytes"] / cl["prefetch"]["T_io_ms"] / 1e6, 2)}
+                del cl
+            except Exception as ex:
+                e2e["at_scale_3L"] = {"error": repr(ex)}
 
     # ---- cpu baseline: the oracle on a bounded sample (rank 0, N = 1 only) ----
     cpu = None
@@ -922,18 +938,19 @@ def at_scale(bs, torch, W, fill_pool_device, dev, opts, peaks, name="4L", steps=
             "value_GBs": round(2 * total / (ser_ms + des_ms) / 1e6, 1)}
 
 
-def config5(args, dev, opts):
-    """SURVEY §8(d) config-5 protocol on config 3: T_c (stand-in alone), T_io (offload alone), T_both (together)."""
+def config5(args, dev, opts, name="3", full=True):
+    """SURVEY §8(d) config-5 protocol on config 3 (or 3L, the total BASELINE.json states for it): T_c (stand-in alone), T_io
+    (offload alone), T_both (together).  full=False: the headline ratio r = 1.25 only, both directions, no sweeps."""
     import torch
 
     import paper_2412_04676_b200 as bs
     import workloads as W
     from workloads.device import StandInContraction, fill_pool_device
 
-    bset = W.make_config("3")
+    bset = W.make_config(name)
     pool, addr = fill_pool_device(bset, dev)
     dset = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, addr, dev)
-    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, bset.data_bytes + 16 * bset.n_blocks + (64 << 20), dev)
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, bset.data_bytes + 16 * bset.n_blocks + (64 << 20) + bs.header_bytes(bset.n_tensors, bset.n_blocks), dev)
     cs = bs.current_stream()
     hb, total = bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs)
     host = torch.empty(total, dtype=torch.uint8, pin_memory=True)
@@ -972,9 +989,9 @@ def config5(args, dev, opts):
     t_io()
     io_ms = min(t_io()[0] for _ in range(3))
     one = min(t_c(1) for _ in range(2))
-    res = {"workload": "config 3 (BASELINE.json configs[2]) offloaded through bs_offload_async", "stream_bytes": int(total),
+    res = {"workload": f"config {name} (BASELINE.json configs[2]) offloaded through bs_offload_async", "stream_bytes": int(total),
            "T_io_ms": round(io_ms, 3), "standin_ms_per_rep": round(one, 3), "sweep": []}
-    for r in (1.25, 0.5, 1.0, 1.5, 2.0):
+    for r in ((1.25, 0.5, 1.0, 1.5, 2.0) if full else (1.25,)):
         reps = max(1, int(round(r * io_ms / one)))
         tc = min(t_c(reps) for _ in range(2))
         both = [t_both(reps) for _ in range(3)]
@@ -1018,7 +1035,7 @@ def config5(args, dev, opts):
     p_io()
     pio_ms = min(p_io()[0] for _ in range(3))
     pre = {"T_io_ms": round(pio_ms, 3), "sweep": []}
-    for r in (1.25, 0.5, 1.0, 2.0):
+    for r in ((1.25, 0.5, 1.0, 2.0) if full else (1.25,)):
         reps = max(1, int(round(r * pio_ms / one)))
         tc = min(t_c(reps) for _ in range(2))
         both = [p_both(reps) for _ in range(3)]
@@ -1030,6 +1047,8 @@ def config5(args, dev, opts):
     pre["headline"] = pre["sweep"][0]
     res["prefetch"] = pre
     eng.destroy()
+    if not full:
+        return res
 
     # ---- a sweep, PAPER Fig 3: every DMRG step loads the environment block of the next step, computes, and saves the
     # block it renormalized.  Synchronous IO (Fig 3(a): compute halts for every save and load) against the queue

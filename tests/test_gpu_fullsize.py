@@ -101,10 +101,16 @@ def test_full_size_serialize_deserialize(cfg):
     assert torch.equal(again, stream[:total]), "serialize(deserialize(S)) != S"
 
 
-def test_full_size_offload_prefetch_config3():
-    """config 5's data path at full size: 256 MiB double-buffered chunks.  The host bytes (concat(chunks), D15) and the
+@pytest.mark.parametrize("cfg", ["3", "3L"])
+def test_full_size_offload_prefetch_config3(cfg):
+    """config 5's data path at full size — config 3 as its recipe counts (2.2 GB, 9 chunks) and at the total BASELINE.json
+    states for it (3L: 11 GB, 42 chunks): 256 MiB double-buffered chunks.  The host bytes (concat(chunks), D15) and the
     prefetched pool, every byte, against the ORACLE's stream and pool image — not against bs_serialize."""
-    bset = W.make_config("3")
+    bset = W.make_config(cfg)
+    _room_for(cfg, bset)
+    import psutil
+    if int(bset.pool_bytes) + int(bset.data_bytes) + (8 << 30) > psutil.virtual_memory().available:
+        pytest.skip(f"config {cfg}: no host RAM for the pinned stream beside the oracle's copy of the source pool")
     up = Uploaded(bset, fill="device")
     hp = HostPool(bset, up.pool)
     rd = DeviceReader()
