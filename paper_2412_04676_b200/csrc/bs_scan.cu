@@ -13,7 +13,7 @@ namespace bs {
 namespace {
 
 template <bool DESER>
-__global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
+__global__ void __launch_bounds__(kScanThreads, 4) scan_kernel(const ScanParams p)
 {
     __shared__ scan::Shared sm;
     const scan::Shape s = scan::shape_of<DESER>(p);

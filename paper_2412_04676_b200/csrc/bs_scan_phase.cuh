@@ -50,7 +50,8 @@ struct HeadView {
 };
 
 struct __align__(16) Shared {
-    uint64_t warp_sum[kScanThreads / 32];
+    uint64_t warp_sum[kScanItems * (kScanThreads / 32)];   // [row][warp]: sums in block order
+    uint64_t warp_excl[kScanItems * (kScanThreads / 32)];  // their exclusive prefix inside the tile
     uint64_t tile_prefix, tile_total;
     uint64_t tot_payload, tot_pool;  // replicated mode: the totals stay in the CTA
     uint32_t item, big_n, last;
@@ -272,10 +273,9 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
     uint64_t dsta[kScanItems];     // DESER scatter: destination address
     uint32_t oddf[kScanItems];
     int err = 0;
-    uint64_t tsum = 0;
 #pragma unroll
     for (uint32_t k = 0; k < kScanItems; ++k) {
-        const uint64_t i = tile * kScanTile + (uint64_t)tid * kScanItems + k;
+        const uint64_t i = tile * kScanTile + (uint64_t)k * kScanThreads + tid;  // row k of the tile: consecutive lanes, consecutive blocks
         const bool valid = i < B;
         uint32_t d0 = 1, d1 = 1, d2 = 0, d3 = 1;
         uint64_t a = 0, offset = 0;
@@ -350,18 +350,25 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
             val[k] = valid ? st : 0;
             if (valid && (a & 7)) err = BS_ERR_ARG;  // D16
         }
-        tsum += val[k];
     }
     cta_err(sm, err);
 
-    // block-wide exclusive scan of tsum, chained to the earlier tiles
-    const uint64_t incl = warp_incl_scan(tsum, lane);
-    if (lane == 31) sm.warp_sum[warp] = incl;
+    // block-wide exclusive scan in block order — row 0 of all threads, then row 1, ... (a thread's blocks lie kScanThreads
+    // apart so that a warp's loads and table stores touch consecutive addresses) — chained to the earlier tiles
+    static_assert(kScanItems * (kScanThreads / 32) == 32, "one warp scans the (row, warp) sums");
+    uint64_t incl[kScanItems];
+#pragma unroll
+    for (uint32_t k = 0; k < kScanItems; ++k) {
+        incl[k] = warp_incl_scan(val[k], lane);
+        if (lane == 31) sm.warp_sum[k * (kScanThreads / 32) + warp] = incl[k];
+    }
     if (tid == 0) sm.big_n = 0;
     bar();
     if (warp == 0) {
-        const uint64_t ws = (lane < kScanThreads / 32) ? sm.warp_sum[lane] : 0;
-        const uint64_t agg = warp_sum(ws);
+        const uint64_t ws = sm.warp_sum[lane];                 // lane = row * 8 + warp: block order
+        const uint64_t ws_incl = warp_incl_scan(ws, lane);
+        const uint64_t agg = __shfl_sync(0xffffffffu, ws_incl, 31);
+        sm.warp_excl[lane] = ws_incl - ws;
         uint64_t excl = 0;
         if (!REPL) {
             if (tile == 0) {
@@ -388,13 +395,12 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
         if (lane == 0) { sm.tile_prefix = excl; sm.tile_total = agg; }
     }
     bar();
-    uint64_t run = sm.tile_prefix + (incl - tsum);
-    for (uint32_t w = 0; w < warp; ++w) run += sm.warp_sum[w];
 
     // blk[] table and tile_first[] boundaries
 #pragma unroll
     for (uint32_t k = 0; k < kScanItems; ++k) {
-        const uint64_t i = tile * kScanTile + (uint64_t)tid * kScanItems + k;
+        const uint64_t i = tile * kScanTile + (uint64_t)k * kScanThreads + tid;
+        const uint64_t run = sm.tile_prefix + sm.warp_excl[k * (kScanThreads / 32) + warp] + (incl[k] - val[k]);
         if (i < B) {
             uint64_t off, address;
             if (DESER) {
@@ -424,7 +430,6 @@ __device__ __forceinline__ void block_tile(const ScanParams& p, const Shape& s, 
                 }
             }
         }
-        run += val[k];
     }
     bar();
     // large blocks: one warp per block fills its boundaries; huge ones (> 2048 granules) take all the scan threads

@@ -41,6 +41,9 @@ def _room_for(cfg, bset):
     """3L / 4L run whenever the box can hold them: source pool + stream + deserialized pool in HBM, the source pool once more
     in host RAM for the oracle."""
     need_dev = int(bset.pool_bytes) + 2 * (bset.data_bytes + 64 * bset.n_blocks + (64 << 20)) + (2 << 30)
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()   # what earlier tests freed sits in torch's cache, not in the driver's free list
     free_dev, _ = torch.cuda.mem_get_info()
     if need_dev > free_dev:
         pytest.skip(f"config {cfg} needs {need_dev / 1e9:.0f} GB of HBM, {free_dev / 1e9:.0f} GB are free")
