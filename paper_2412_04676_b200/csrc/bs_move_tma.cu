@@ -968,7 +968,7 @@ cudaError_t launch_fused_t(const ScanParams& sp, const MoveParams& p, const bs_o
     cudaError_t e = resolve_shape<UNPACK>(p, o, &sh);
     if (e != cudaSuccess) return e;
     q.tile_bytes = sh.tile_bytes;
-    if (sh.smem < sizeof(scan::Shared)) return cudaErrorInvalidValue;  // cannot happen: a ring is >= 3 x 16 KiB
+    if (sh.smem < sizeof(scan::Shared)) sh.smem = sizeof(scan::Shared);  // small tiles: the pass's state needs more than the rings
     static std::atomic<uint64_t> allowed{0};
     if ((e = allow_max_smem(fused_tma_kernel<UNPACK>, &allowed)) != cudaSuccess) return e;
     if ((e = prepare_scan_state(sp.ws, stream)) != cudaSuccess) return e;

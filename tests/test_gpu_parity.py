@@ -31,6 +31,7 @@ VARIANTS = [dict(variant=bs.VARIANT_LDG, tile_bytes=16384), dict(variant=bs.VARI
             # tiles that do not end on a 16 KiB granule of the work partition (the TMA variant takes any multiple of 1 KiB)
             dict(variant=bs.VARIANT_TMA, tile_bytes=40960, stages=3, warps=1), dict(variant=bs.VARIANT_TMA, tile_bytes=24576, stages=4, warps=2),
             dict(variant=bs.VARIANT_TMA, tile_bytes=20480, stages=3, warps=3, fuse=2), dict(variant=bs.VARIANT_TMA, tile_bytes=5120, stages=5, warps=2),
+            dict(variant=bs.VARIANT_TMA, tile_bytes=4096, stages=3, warps=1, fuse=2), dict(variant=bs.VARIANT_TMA, tile_bytes=4096, stages=3, warps=1, fuse=1),
             # paced launches (bs_opts.reserved[2]): a fixed target rate with the large-set shape, and pacing switched off
             dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=4, warps=1, pace=6500), dict(variant=bs.VARIANT_TMA, pace=1),
             dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=2, pace=200, fuse=2),
