@@ -58,6 +58,21 @@ def upload(rng, tensors, qn, dim, dtype):
     return pool, dset, blocks
 
 
+def wide_opts(rng):
+    """A random TMA launch shape the library accepts (bs.h bs_opts; check_opts in bs_api.cu)."""
+    while True:
+        tile = int(rng.integers(4, 65)) * 1024
+        stages = int(rng.integers(3, 9))
+        warps = int(rng.integers(1, 6))
+        if warps * (stages * tile + 2048) <= 224 * 1024:
+            break
+    tune = int(rng.choice([0, 8, 0x10, 0x1000, 0x1010, 0x1008, 0x20, 0x30]))
+    if rng.random() < 0.3:
+        tune |= int(rng.integers(1, 4)) << 8            # fewer tiles loading beside the one being stored
+    return dict(variant=bs.VARIANT_TMA, tile_bytes=tile, stages=stages, warps=warps, tune=tune, fuse=int(rng.integers(0, 3)),
+                pace=int(rng.choice([0, 0, 300, 6500, 20000])))
+
+
 @pytest.mark.parametrize("seed", range(24))
 def test_random_sets_round_trip_bit_exact(seed):
     rng = np.random.default_rng(1000 + seed)
@@ -115,6 +130,27 @@ def test_random_sets_round_trip_bit_exact(seed):
                       ws.result_ptr, opts, cs)
     assert ws.read_result()["status"] == bs.OK
     assert (opool.cpu().numpy()[:need] == ref["pool"][:need]).all(), f"seed {seed}: blocks differ after the package round trip"
+    # the same set through launch shapes of the whole space round 2 opened: tiles of any multiple of 1 KiB, 3-8 stages, the
+    # tile counter forced or forbidden, the table fetched further ahead, a pace, one launch or two (own generator: the
+    # draws above stay what they were)
+    rng_o = np.random.default_rng(7000 + seed)
+    for _ in range(3):
+        wide = wide_opts(rng_o)
+        out.fill_(0xCD)
+        bs.serialize(dset.desc, out.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, wide, cs)
+        assert ws.read_result()["status"] == bs.OK, wide
+        got = out.cpu().numpy()
+        assert (got[:total] == want).all() and (got[total:] == 0xCD).all(), f"seed {seed}: stream differs with {wide}"
+        chunk = int(rng_o.integers(1, 40)) * 16 * int(rng_o.choice([64, 4096]))
+        rng_out.fill_(0xCD)
+        for lo in range(0, total, chunk):
+            bs.serialize_range(dset.desc, rng_out.data_ptr() + lo, lo, min(lo + chunk, total), lo == 0, ws.ptr, ws.nbytes,
+                               ws.result_ptr, wide, cs)
+        assert (rng_out.cpu().numpy() == want).all(), f"seed {seed}: concat of ranges differs (chunk {chunk}) with {wide}"
+        opool.fill_(0xEE)
+        bs.deserialize(out.data_ptr(), total, o.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, ws.result_ptr, wide, cs)
+        assert ws.read_result()["status"] == bs.OK, wide
+        assert (opool.cpu().numpy()[:need] == ref["pool"][:need]).all(), f"seed {seed}: blocks differ with {wide}"
 
 
 def random_layered(rng):
