@@ -542,9 +542,11 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     const bool a8 = (hv.dtype & BS_ALIGN8) != 0;  // an unpadded stream: segments may sit 8 bytes off the 16-byte grid
     uint32_t tile_bytes = p.tile_bytes, n_warps = opt_warps & 0xffffu, n_stages = opt_stages;
     // The preset (bit 31 of opt_warps: bs_opts left the shape open) is settled here, where the payload size is known
+    bool large = false;
     if ((opt_warps >> 31) && P >= kLargePayload && p.pkg.cap % preset_large(UNPACK).tile_bytes == 0) {
         const Preset ps = preset_large(UNPACK);
         tile_bytes = ps.tile_bytes; n_stages = ps.stages; n_warps = ps.warps;
+        large = true;
     }
     // pacing (experiments; bs_opts.reserved[2] >= 100): that many GB/s of HBM traffic for the whole launch
     const uint32_t rate = p.pace >= 100u ? p.pace : 0u;
@@ -599,7 +601,10 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     hints.st = (p.tune & 2u) != 0;
     int64_t lag = n_stages - 2;  // tile i is stored while tiles i+1 .. i+lag are loading
     if (((p.tune >> 8) & 15u) != 0 && (int64_t)((p.tune >> 8) & 15u) < lag) lag = (p.tune >> 8) & 15u;  // experiment: fewer loads in flight
-    const int64_t ahead = ((p.tune & 0x1000u) || rate) ? 2 : 1;  // iterations between the fetch of a tile's table entries and their use
+    // iterations between the fetch of a tile's table entries and their use.  The one-warp pack of a large set fetches two
+    // ahead: with small blocks (config 3, 3L: ~10 per tile) its iterations are long enough for the one exposed round trip
+    // to show (+0.9 %; unpack: -0.3 %, it keeps one)
+    const int64_t ahead = ((p.tune & 0x1000u) || rate || (!UNPACK && large)) ? 2 : 1;
 
     // ---- which tiles (see "tile hand-out"): iteration i of this warp works on tile tq(i) of the range, kNoTile = none left.
     // Claims are made `reach` iterations ahead: the answer of the atomic is written into the queue one iteration after it
