@@ -176,7 +176,9 @@ uint64_t bs_header_bytes(uint64_t n_tensors, uint64_t n_blocks);
 uint64_t bs_header_bytes_rank4(uint64_t n_tensors, uint64_t n_blocks);
 
 /* Bytes of device workspace a call needs for a set of up to n_blocks blocks whose stream is at most
- * stream_capacity bytes: the offset table ("pointer structure") and scan state. */
+ * stream_capacity bytes: the offset table ("pointer structure"), scan state and the calls' work counters.
+ * 256-byte aligned; it may be uninitialised memory (every word the kernels synchronise on carries a tag) and is reusable
+ * from call to call, but it serves ONE call at a time: calls that may run concurrently (two streams) need a workspace each. */
 uint64_t bs_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint64_t stream_capacity);
 
 /* Parse the 64-byte fixed header (HOST memory).  BS_ERR_CORRUPT if it is not a v1 or v3 header. */
