@@ -207,6 +207,33 @@ int bs_serialize_range(const bs_set_desc *set, void *d_dst, uint64_t lo, uint64_
                        void *d_workspace, uint64_t workspace_bytes, bs_result *d_result,
                        const bs_opts *opts, cudaStream_t stream);
 
+/* bs_serialize without a workspace argument and without any allocation: for callers that cannot get device memory at the
+ * moment they must save a set.  That is the normal state of the solver this library serves — it hands whatever HBM is
+ * left to its own block pool, and the memory peaks of PAPER L132-136 are the very reason data is pushed out, so a
+ * cudaMalloc then fails or is forbidden (a plug-in may not allocate behind the host program's pool) — and of any caller
+ * that cannot afford the device-wide synchronisation a cudaMalloc / cudaFree brings while side streams are busy.
+ *   - The workspace is a fixed array of bs_noalloc_scratch_bytes() = 1.5 MiB of device memory inside the library, held
+ *     on every GPU the library is used on from the moment its code is loaded there until the process exits.  The call
+ *     itself calls no cudaMalloc, cudaFree or other allocating routine; set, d_stream and d_result are still the
+ *     caller's, exactly as for bs_serialize, and the stream written is byte for byte bs_serialize's.
+ *   - Limits: set->n_blocks <= BS_NOALLOC_MAX_BLOCKS and capacity <= BS_NOALLOC_MAX_STREAM_BYTES (pass the smaller of
+ *     your buffer size and the limit).  Beyond either the call returns BS_ERR_CAPACITY at once and enqueues nothing;
+ *     a stream that turns out larger than `capacity` is the usual deferred BS_ERR_CAPACITY in d_result.
+ *   - The FIRST call on each device looks the array's device address up (cudaGetSymbolAddress with that device current;
+ *     BS_ERR_CUDA if the runtime refuses, BS_ERR_UNSUPPORTED for a device ordinal >= 64).  Make that first call during
+ *     set-up, before any stream capture is begun; later calls only read the cached address.
+ *   - Every call on a device uses the SAME array and finds in it whatever the previous call left.  Nothing in it has to
+ *     start at zero (each word the kernels synchronise on carries a per-call tag), so calls one after the other on one
+ *     stream, or ordered by events, need no clearing in between.  Calls that can overlap on the GPU (two streams, no
+ *     event between them) race on it and produce garbage with status BS_OK: give such callers a workspace each
+ *     (bs_serialize).  The array is also what bs_serialize_range would need to follow up on this call: it is not
+ *     exposed, so there is no range form. */
+#define BS_NOALLOC_MAX_BLOCKS 65536u
+#define BS_NOALLOC_MAX_STREAM_BYTES (1ull << 30)
+uint64_t bs_noalloc_scratch_bytes(void); /* host-only: the size of the built-in array */
+int bs_serialize_noalloc(const bs_set_desc *set, void *d_stream, uint64_t capacity, bs_result *d_result,
+                         const bs_opts *opts, cudaStream_t stream);
+
 /* ---- deserialize ---------------------------------------------------------------- */
 
 /* Validate the header of d_stream[0..nbytes) (every check of DESIGN.md "deserialize"), rebuild the

@@ -11,7 +11,8 @@ from ._binding import (  # noqa: F401
     BsError, Engine, LayeredDesc, Opts, Queue, Result, SetDesc, Ticket,
     layered_deserialize, layered_header_bytes, layered_serialize, layered_serialize_range, layered_serialized_size,
     layered_stream_info, layered_workspace_bytes, make_layered_desc,
-    deserialize, deserialize_range, header_bytes, header_bytes_rank4, last_cuda_error, lib, make_desc, serialize, serialize_range, serialized_size,
+    deserialize, deserialize_range, header_bytes, header_bytes_rank4, last_cuda_error, lib, make_desc, serialize, serialize_noalloc, serialize_range, serialized_size,
+    NOALLOC_MAX_BLOCKS, NOALLOC_MAX_STREAM_BYTES, noalloc_scratch_bytes,
     stream_info, strerror, version, workspace_bytes,
     PKG_HEADER, PKG_NO_BLOCK, layered_package_emit, layered_package_unpack, layered_package_workspace_bytes, package_count, package_emit, package_range, package_unpack, package_workspace_bytes,
 )

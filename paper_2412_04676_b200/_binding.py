@@ -135,6 +135,9 @@ def lib():
     L.bs_serialized_size.argtypes = [C.POINTER(SetDesc), vp, u64, pu64, pu64, vp]
     L.bs_serialize.argtypes = [C.POINTER(SetDesc), vp, u64, vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_serialize_range.argtypes = [C.POINTER(SetDesc), vp, u64, u64, i32, vp, u64, vp, C.POINTER(Opts), vp]
+    L.bs_noalloc_scratch_bytes.restype = u64
+    L.bs_noalloc_scratch_bytes.argtypes = []
+    L.bs_serialize_noalloc.argtypes = [C.POINTER(SetDesc), vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_deserialize.argtypes = [vp, u64, C.POINTER(SetDesc), vp, u64, u32, vp, u64, vp, C.POINTER(Opts), vp]
     L.bs_deserialize_range.argtypes = [vp, u64, u64, vp, C.POINTER(SetDesc), u32, vp, u64, C.POINTER(Opts), vp]
     L.bs_engine_create.argtypes = [C.POINTER(vp), C.POINTER(EngineCfg)]
@@ -252,6 +255,20 @@ def serialize(desc: SetDesc, stream_ptr: int, capacity: int, ws_ptr: int, ws_byt
               opts=None, stream: int = 0) -> int:
     return _check(lib().bs_serialize(C.byref(desc), stream_ptr, capacity, ws_ptr, ws_bytes, result_ptr, _opts(opts), stream),
                   "bs_serialize")
+
+
+NOALLOC_MAX_BLOCKS = 65536
+NOALLOC_MAX_STREAM_BYTES = 1 << 30
+
+
+def noalloc_scratch_bytes() -> int:
+    return int(lib().bs_noalloc_scratch_bytes())
+
+
+def serialize_noalloc(desc: SetDesc, stream_ptr: int, capacity: int, result_ptr: int, opts=None, stream: int = 0) -> int:
+    """bs_serialize on the library's built-in workspace: for callers that cannot allocate device memory (bs.h)."""
+    return _check(lib().bs_serialize_noalloc(C.byref(desc), stream_ptr, capacity, result_ptr, _opts(opts), stream),
+                  "bs_serialize_noalloc")
 
 
 def serialize_range(desc: SetDesc, dst_ptr: int, lo: int, hi: int, run_scan: bool, ws_ptr: int, ws_bytes: int,

@@ -10,7 +10,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIBDIR = os.path.join(HERE, "lib")
 SO = os.path.join(LIBDIR, "libbsstream.so")
-SOURCES = ["bs_api.cu", "bs_scan.cu", "bs_move.cu", "bs_move_tma.cu", "bs_layered.cu", "bs_pkg.cu", "bs_engine.cu", "bs_queue.cu"]
+SOURCES = ["bs_api.cu", "bs_noalloc.cu", "bs_scan.cu", "bs_move.cu", "bs_move_tma.cu", "bs_layered.cu", "bs_pkg.cu", "bs_engine.cu", "bs_queue.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr",
               "-cudart", "static"]
