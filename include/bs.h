@@ -56,7 +56,8 @@ extern "C" {
 typedef struct CUstream_st *cudaStream_t;
 #endif
 
-#define BS_VERSION 0x00010000u /* library 1.0, wire format v1 */
+#define BS_VERSION 0x00010200u /* library 1.2 (1.1 = round 2: bs_stream_info_t grew by align / max_rank, bs_layered_stream_info_t by
+                                  dtype, bs_workspace_bytes grew: rebuild callers against this header); wire formats v1, v2, v3 */
 
 enum {
     BS_OK = 0,
@@ -64,7 +65,7 @@ enum {
     BS_ERR_ARG = -1,         /* NULL / misaligned pointer, bad descriptor partition, size overflow */
     BS_ERR_CAPACITY = -2,    /* stream / pool / workspace / descriptor arrays too small */
     BS_ERR_CORRUPT = -3,     /* header validation failed; nothing was written */
-    BS_ERR_UNSUPPORTED = -4, /* rank not in {2,3}, unknown dtype, n_qn != 2 */
+    BS_ERR_UNSUPPORTED = -4, /* rank not in {2,3} ({2,3,4} in a BS_RANK4 set), unknown dtype, n_qn != 2 */
     BS_ERR_CUDA = -5,        /* a CUDA runtime call failed; see bs_last_cuda_error() */
     BS_ERR_IO = -6           /* the storage tier of a bs_queue: open / read / write of a file failed (errno is the C library's) */
 };
@@ -91,7 +92,8 @@ enum { BS_F64 = 0 /* e = 8 */, BS_F32 = 1 /* e = 4 */, BS_C64 = 2 /* e = 8 */, B
  *   block_rec   : i32 qn[4][2]; u32 dim[4]; u32 tensor; u32 reserved = 0; u64 offset      (64 bytes)
  *   header_bytes = align128(64 + 32*T + 64*B) = bs_header_bytes_rank4(T, B);  payload and pool layout as v1.
  * For deserialize / prefetch outputs the flag says how the caller shaped `out`'s arrays: a v3 stream needs it, a v1 stream must
- * not have it (BS_ERR_ARG otherwise).  Not combined with BS_ALIGN8 or layered sets (BS_ERR_UNSUPPORTED). */
+ * not have it (BS_ERR_ARG otherwise).  qn and dim of such a set must be 16-byte aligned (BS_ERR_ARG at once otherwise: their
+ * rows move as 16-byte words).  Not combined with BS_ALIGN8 or layered sets (BS_ERR_UNSUPPORTED). */
 #define BS_RANK4 0x200u
 #define BS_DTYPE_MASK 0xffu
 
@@ -121,8 +123,8 @@ typedef struct bs_set_desc {
     uint32_t dtype;         /* BS_F64, BS_F32, BS_C64 or BS_C128, optionally | BS_ALIGN8 or | BS_RANK4; for outputs: 0 or
                                BS_RANK4 (the shape of qn / dim), the stream's type comes back in bs_result */
     bs_tensor_rec *tensors; /* [T]        */
-    int32_t *qn;            /* [B][3][2]  labels per leg; unused legs 0            (BS_RANK4: [B][4][2]) */
-    uint32_t *dim;          /* [B][3]     extents; unused legs 1                   (BS_RANK4: [B][4])    */
+    int32_t *qn;            /* [B][3][2]  labels per leg; unused legs 0; 8-byte aligned   (BS_RANK4: [B][4][2], 16-byte aligned) */
+    uint32_t *dim;          /* [B][3]     extents; unused legs 1; 4-byte aligned          (BS_RANK4: [B][4], 16-byte aligned)    */
     uint64_t *addr;         /* [B]        device address of each dense, contiguous, row-major (last index
                                           fastest) block; must be 8-byte aligned, 16-byte aligned for the
                                           vector fast path */
@@ -195,7 +197,7 @@ int bs_serialized_size(const bs_set_desc *set, void *d_workspace, uint64_t works
  * Asynchronous.  d_result (DEVICE, 64 bytes) receives total/header/payload bytes and the status:
  * BS_ERR_CAPACITY if total > capacity (total_bytes = required size), BS_ERR_ARG for a descriptor that
  * does not partition its blocks, a block address not 8-byte aligned or a size overflow,
- * BS_ERR_UNSUPPORTED for rank not in {2,3}.  Every byte of [0,total) is written, including padding. */
+ * BS_ERR_UNSUPPORTED for rank not in {2,3} (BS_RANK4 sets: {2,3,4}).  Every byte of [0,total) is written, including padding. */
 int bs_serialize(const bs_set_desc *set, void *d_stream, uint64_t capacity, void *d_workspace,
                  uint64_t workspace_bytes, bs_result *d_result, const bs_opts *opts, cudaStream_t stream);
 

@@ -41,8 +41,10 @@ int check_set(const bs_set_desc* s)
         (s->dtype & (BS_ALIGN8 | BS_RANK4)) == (BS_ALIGN8 | BS_RANK4))
         return BS_ERR_UNSUPPORTED;
     if (s->n_tensors && (s->tensors == nullptr || !aligned(s->tensors, 16))) return BS_ERR_ARG;
-    if (s->n_blocks && (s->qn == nullptr || !aligned(s->qn, 8))) return BS_ERR_ARG;
-    if (s->n_blocks && (s->dim == nullptr || !aligned(s->dim, 4))) return BS_ERR_ARG;
+    // a BS_RANK4 set's qn / dim rows are 32 / 16 bytes and the kernels move them as 16-byte words (bs_move_common.cuh)
+    const uintptr_t qa = (s->dtype & BS_RANK4) ? 16 : 8, da = (s->dtype & BS_RANK4) ? 16 : 4;
+    if (s->n_blocks && (s->qn == nullptr || !aligned(s->qn, qa))) return BS_ERR_ARG;
+    if (s->n_blocks && (s->dim == nullptr || !aligned(s->dim, da))) return BS_ERR_ARG;
     if (s->n_blocks && (s->addr == nullptr || !aligned(s->addr, 8))) return BS_ERR_ARG;
     return BS_OK;
 }

@@ -35,7 +35,7 @@ def test_struct_layouts_match_the_header():
 
 
 def test_host_only_entry_points():
-    assert bs.version() == 0x00010000
+    assert bs.version() == 0x00010200
     assert bs.header_bytes(1, 2) == 256 and bs.header_bytes(0, 0) == 128
     assert bs.header_bytes(2000, 446140) == (64 + 32 * 2000 + 48 * 446140 + 127) // 128 * 128
     assert bs.workspace_bytes(1, 7, 1 << 20) % 256 == 0
@@ -71,6 +71,28 @@ def test_argument_errors_need_no_device():
     d = bs.make_desc(1, 1, 16, 16, 16, 16)
     with pytest.raises(bs.BsError) as e:
         bs.serialize(d, 256, 1024, 256, 64, 0)     # workspace too small
+    assert e.value.code == bs.ERR_CAPACITY
+
+
+def test_rank4_sets_need_16_byte_aligned_label_and_extent_arrays():
+    """A BS_RANK4 set's qn / dim rows are 32 / 16 bytes and move as 16-byte words: arrays 8 (or 4) off that grid — a sub-view
+    of a larger allocation — are BS_ERR_ARG up front, not a misaligned-address fault in the kernel.  Plain sets keep 8 / 4."""
+    for qn, dim, ok in ((32, 32, True), (40, 32, False), (32, 40, False), (32, 36, False)):
+        d = bs.make_desc(1, 1, 16, qn, dim, 16, dtype=bs.F64 | bs.RANK4)
+        if ok:      # passes the descriptor check; the (too small) workspace is what is refused next
+            with pytest.raises(bs.BsError) as e:
+                bs.serialize(d, 256, 1024, 256, 64, 0)
+            assert e.value.code == bs.ERR_CAPACITY
+            continue
+        for call in (lambda: bs.serialize(d, 256, 1024, 256, 1 << 20, 0),
+                     lambda: bs.deserialize(256, 1024, d, 256, 1 << 20, bs.LAYOUT_POOL, 256, 1 << 20, 0),
+                     lambda: bs.serialize_noalloc(d, 256, 1024, 256)):
+            with pytest.raises(bs.BsError) as e:
+                call()
+            assert e.value.code == bs.ERR_ARG
+    d = bs.make_desc(1, 1, 16, 40, 36, 16)         # three legs: 8- and 4-byte alignment is enough
+    with pytest.raises(bs.BsError) as e:
+        bs.serialize(d, 256, 1024, 256, 64, 0)
     assert e.value.code == bs.ERR_CAPACITY
 
 
