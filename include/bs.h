@@ -180,7 +180,9 @@ uint64_t bs_header_bytes_rank4(uint64_t n_tensors, uint64_t n_blocks);
 /* Bytes of device workspace a call needs for a set of up to n_blocks blocks whose stream is at most
  * stream_capacity bytes: the offset table ("pointer structure"), scan state and the calls' work counters.
  * 256-byte aligned; it may be uninitialised memory (every word the kernels synchronise on carries a tag) and is reusable
- * from call to call, but it serves ONE call at a time: calls that may run concurrently (two streams) need a workspace each. */
+ * from call to call, but it serves ONE pass at a time: calls that run the size / offset or parse pass (bs_serialized_size,
+ * bs_serialize, bs_deserialize, a range call with run_scan) and may run concurrently (two streams) need a workspace each.
+ * Range calls behind a completed pass only read it and may overlap one another (see bs_deserialize_range). */
 uint64_t bs_workspace_bytes(uint32_t n_tensors, uint32_t n_blocks, uint64_t stream_capacity);
 
 /* Parse the 64-byte fixed header (HOST memory).  BS_ERR_CORRUPT if it is not a v1 or v3 header. */
@@ -252,7 +254,10 @@ int bs_deserialize(const void *d_stream, uint64_t nbytes, bs_set_desc *out, void
  * parse / validate pass must have run on the same workspace with the same `out` and destination (a bs_deserialize call;
  * the tables it leaves are what this call uses) and its status is honoured: nothing is written unless it was BS_OK.
  * d_header: stream byte 0 .. header_bytes to rebuild the descriptor arrays from as well, or NULL (payload only).
- * The union over a partition of [header_bytes, total) rebuilds every block. */
+ * The union over a partition of [header_bytes, total) rebuilds every block.  BS_VARIANT_LDG on the tables of an unpadded
+ * (BS_ALIGN8) stream writes nothing and leaves BS_ERR_UNSUPPORTED as the workspace's status, which later range calls honour.
+ * Both range forms only READ the workspace: once the pass has completed, the ranges of one stream may be issued on several
+ * CUDA streams at once on the same workspace (order them behind the pass with an event). */
 int bs_deserialize_range(const void *d_src, uint64_t lo, uint64_t hi, const void *d_header, bs_set_desc *out, uint32_t flags,
                          void *d_workspace, uint64_t workspace_bytes, const bs_opts *opts, cudaStream_t stream);
 

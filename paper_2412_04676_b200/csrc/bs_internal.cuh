@@ -79,8 +79,8 @@ struct __align__(256) WsHead {
     uint64_t ep_done;        // line 3: work items completed; the CTA that completes the last one finalises
     uint64_t ep_exit;        //         CTAs that have left the item loop; the last one resets the counters
     uint64_t ep_err;         //         first error of the call: [63:24] epoch tag, [7:0] = -code
-    uint64_t mv_ticket;      //         data movement (bs_move_tma.cu): tiles handed out, [63:32] tag, [31:0] count
-    uint64_t mv_exit;        //         data warps that have left a movement launch; the last one puts both back
+    uint64_t unused_r2[2];   //         (round 2 kept the movement's tile counter here; it now lives in the library's own
+                             //         device memory, one pair per launch: bs_move_tma.cu "tile hand-out")
     uint64_t pad3[11];
 };
 static_assert(sizeof(WsHead) == 512, "WsHead is four 128-byte lines");
@@ -189,6 +189,7 @@ struct MoveParams {
     uint32_t tune;                // bs_opts.reserved[0]: experiment switches of the TMA variant
     uint32_t pace;                // bs_opts.reserved[2]: >= 100: pace the launch at that many GB/s of HBM traffic (experiments)
     uint32_t rank4;               // != 0: qn / dim have four legs per block (BS_RANK4; wire format v3)
+    uint32_t mv_slot;             // which tile-counter pair of the library's ring this launch uses (filled in by the launchers)
     LayeredView lay;              // lay.on != 0: qn / dim are the structure block table, header is wire format v2
     PkgMap pkg;                   // pkg.cap != 0: the stream side is a set of package slots
 };

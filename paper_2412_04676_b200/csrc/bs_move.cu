@@ -49,6 +49,13 @@ __global__ void __launch_bounds__(kThreads) move_kernel(const MoveParams p)
         if (!UNPACK) poison_on_error(p);
         return;
     }
+    if (head->dtype & BS_ALIGN8) {
+        // tables of an unpadded stream (a range call behind a pass that ran for the TMA variant): this variant moves 16-byte
+        // units and would scatter blocks that sit 8 off that grid wrongly.  Nothing is written; the workspace says why.
+        // (Every CTA has read status == 0 above or returns here all the same: the store cannot change another CTA's path.)
+        if (blockIdx.x == 0 && threadIdx.x == 0) const_cast<WsHead*>(head)->status = BS_ERR_UNSUPPORTED;
+        return;
+    }
     const uint32_t T = head->n_tensors, B = head->n_blocks;
     const uint64_t hb = head->header_bytes, P = head->payload_bytes, total = hb + P;
     const uint64_t ng = head->n_granules;

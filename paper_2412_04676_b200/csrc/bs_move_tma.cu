@@ -494,7 +494,20 @@ struct Preset {
 // out by ONE counter in the workspace head: a warp claims its next tile two iterations before it needs the tile's block
 // table, an SM that is served faster simply takes more tiles, all SMs finish together, and an over-subscribed launch runs
 // at the capacity of the memory system instead of falling off it.  The counter needs no clearing: it carries a tag like
-// the pass's counters, the last warp out of a launch puts it back, a stale word (a fresh workspace) is claimed by CAS.
+// the pass's counters, the last warp out of a launch puts it back, a stale word (never used, or left by a killed launch) is
+// claimed by CAS.
+// Round 3: the counter is no longer a word of the caller's workspace.  bs_serialize_range / bs_deserialize_range run on the
+// workspace the pass left its tables in, and issuing the ranges of one stream on two CUDA streams is the natural use: with
+// one counter in the head two such launches drew tile numbers from the same word — tiles skipped, status BS_OK.  Each
+// launch now gets its own {ticket, exit} pair from a ring in the library's device memory, indexed by a host-issued launch
+// number (MoveParams.mv_slot), and the movement kernels only READ the workspace again, as in round 1.  Two launches share
+// a pair only if kMvSlots counter-dealt launches (each >= 128 MiB of movement) are issued while one of them is still running.
+constexpr uint32_t kMvSlots = 1024;
+struct __align__(16) MvCtr {
+    uint64_t ticket;  // tiles handed out: [63:32] tag, [31:0] count
+    uint64_t exit;    // data warps that have left the launch; the last one puts both back
+};
+__device__ MvCtr g_mv_ctr[kMvSlots];
 constexpr uint64_t kMvTag = 0x4D76C1A5ull << 32;  // [63:32] tag of the two move counters between and during launches, [31:0] count
 // take `n` numbers from tagged counter `w`: returns the first
 __device__ __forceinline__ uint32_t mv_take(uint64_t* w, uint32_t n)
@@ -612,12 +625,12 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     // A range of less than kDynamicBytes keeps round 1's static round-robin deal: nothing there is worth the two extra round
     // trips of the counter (config 1: 3 us of 8).  tune bit 3 forces the static deal, bit 4 the counter (tests, A/B runs).
     const bool dynamic = (p.tune & 8u) == 0 && ((p.tune & 16u) != 0 || np * tile_bytes >= kDynamicBytes);
-    WsHead* const whead = const_cast<WsHead*>(head);
+    MvCtr* const ctr = &g_mv_ctr[p.mv_slot & (kMvSlots - 1)];
     uint32_t* const m_tq = reinterpret_cast<uint32_t*>(meta_ptr + kBlkSlots * kMetaBlk * 16 + kTfSlots * 8);
     const int64_t reach = 2 * ahead;
     {
         uint32_t first = 0;
-        if (dynamic && lane == 0) first = mv_take(&whead->mv_ticket, (uint32_t)reach);
+        if (dynamic && lane == 0) first = mv_take(&ctr->ticket, (uint32_t)reach);
         first = __shfl_sync(0xffffffffu, first, 0);
         if (lane < kTqSlots) {
             const uint64_t v = dynamic ? (uint64_t)first + lane : worker + (uint64_t)lane * n_workers;
@@ -628,7 +641,7 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
     // lane 0: the tile number of iteration i, raw (>= np: none left).  Dynamic: an atomic whose answer nobody waits for
     // until the next iteration queues it
     auto next_claim = [&](int64_t i) -> uint64_t {
-        return dynamic ? (uint64_t)mv_take(&whead->mv_ticket, 1u) : worker + (uint64_t)i * n_workers;
+        return dynamic ? (uint64_t)mv_take(&ctr->ticket, 1u) : worker + (uint64_t)i * n_workers;
     };
     bool claiming = m_tq[(reach - 1) & (kTqSlots - 1)] != kNoTile;  // nothing more to ask for once a claim came back empty
     uint64_t pending = np;                                           // lane 0: the claim of iteration it + reach
@@ -842,10 +855,10 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
         // the last warp out puts the counters back for the next launch.  Every warp has its last (empty) claim in hand by
         // then: `pending` is stored first, so an atomic of this warp cannot still be on its way when the counter is reset
         m_tq[0] = (uint32_t)pending;
-        if (mv_take(&whead->mv_exit, 1u) == (uint32_t)n_workers - 1u) {
-            volatile uint64_t* c = &whead->mv_ticket;
+        if (mv_take(&ctr->exit, 1u) == (uint32_t)n_workers - 1u) {
+            volatile uint64_t* c = &ctr->ticket;
             *c = kMvTag;
-            c = &whead->mv_exit;
+            c = &ctr->exit;
             *c = kMvTag;
             __threadfence();
         }
@@ -926,6 +939,13 @@ cudaError_t allow_max_smem(K kernel, std::atomic<uint64_t>* done)
     return cudaSuccess;
 }
 
+// the tile counter pair of a launch ("tile hand-out"): launches take the pairs of the ring in turn
+uint32_t next_mv_slot()
+{
+    static std::atomic<uint32_t> seq{0};
+    return seq.fetch_add(1, std::memory_order_relaxed) & (kMvSlots - 1);
+}
+
 struct Shape3 {
     uint32_t tile_bytes, stages, warps, auto_shape;
     size_t smem;
@@ -956,6 +976,7 @@ cudaError_t launch_tma_t(const MoveParams& p, const bs_opts& o, int sm_count, cu
     cudaError_t e = resolve_shape<UNPACK>(p, o, &sh);
     if (e != cudaSuccess) return e;
     q.tile_bytes = sh.tile_bytes;
+    q.mv_slot = next_mv_slot();
     static std::atomic<uint64_t> allowed{0};
     if ((e = allow_max_smem(move_tma_kernel<UNPACK>, &allowed)) != cudaSuccess) return e;
     move_tma_kernel<UNPACK><<<(unsigned)sm_count, (sh.warps + 1) * 32, sh.smem, stream>>>(q, sh.stages, sh.warps | sh.auto_shape);  // + the header warp
@@ -973,6 +994,7 @@ cudaError_t launch_fused_t(const ScanParams& sp, const MoveParams& p, const bs_o
     cudaError_t e = resolve_shape<UNPACK>(p, o, &sh);
     if (e != cudaSuccess) return e;
     q.tile_bytes = sh.tile_bytes;
+    q.mv_slot = next_mv_slot();
     if (sh.smem < sizeof(scan::Shared)) sh.smem = sizeof(scan::Shared);  // small tiles: the pass's state needs more than the rings
     static std::atomic<uint64_t> allowed{0};
     if ((e = allow_max_smem(fused_tma_kernel<UNPACK>, &allowed)) != cudaSuccess) return e;

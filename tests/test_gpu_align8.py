@@ -229,6 +229,18 @@ def test_what_is_refused():
     need = oracle.pool_bytes(want)
     o, pool, res = deserialize(st, len(want), bset.n_tensors, bset.n_blocks, need, dict(variant=bs.VARIANT_LDG))
     assert res["status"] == bs.ERR_UNSUPPORTED and (pool == 0xEE).all()
+    # a range call with the LDG variant on tables a TMA-variant pass parsed from an unpadded stream: nothing is written
+    # (it used to scatter 16-byte units with status OK), and the workspace refuses every later range call too
+    o2 = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+    pool2 = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    bs.deserialize(st.data_ptr(), len(want), o2.desc, pool2.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, ws.result_ptr, None,
+                   bs.current_stream())
+    assert ws.read_result()["status"] == bs.OK and (pool2.cpu().numpy() == oracle.deserialize(want)["pool"][:need]).all()
+    pool2.fill_(0xEE)
+    for variant in (dict(variant=bs.VARIANT_LDG, tile_bytes=16384), None):
+        bs.deserialize_range(st.data_ptr(), 0, len(want), 0, o2.desc, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, variant, bs.current_stream())
+        torch.cuda.synchronize()
+        assert (pool2 == 0xEE).all()
     bad_flag = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, up.addr, DEV, dtype=bs.F64 | 0x400)
     with pytest.raises(bs.BsError) as e:
         bs.serialize(bad_flag.desc, out.data_ptr(), 1 << 20, ws.ptr, ws.nbytes, ws.result_ptr, None, bs.current_stream())

@@ -411,6 +411,60 @@ def test_fused_calls_on_two_streams_at_once(opts):
         assert (ln["pool"].cpu().numpy() == ref_pool).all()
 
 
+@pytest.mark.parametrize("opts", [dict(variant=bs.VARIANT_TMA, tune=0x10), dict(variant=bs.VARIANT_TMA, tile_bytes=49152, stages=3, warps=1, tune=0x1010),
+                                  dict(variant=bs.VARIANT_TMA)], ids=_vid)
+def test_ranges_of_one_stream_on_two_cuda_streams_share_the_workspace(opts):
+    """The segment calls run on the workspace the pass left its tables in, so the halves of one stream issued on two CUDA
+    streams use the SAME workspace.  The movement only reads it (round 3: the tile counter of a launch is a pair of the
+    library's own ring, not a word of the head — with one shared counter two launches drew tile numbers from the same word
+    and skipped tiles with status BS_OK).  Both directions, tiles from the counter: the oracle's bytes every round."""
+    bset = W.make_config("2")
+    up = Uploaded(bset)
+    want, _, _ = oracle_stream(bset, up.host_pool, up.host_offs)
+    total, need = len(want), oracle.pool_bytes(want)
+    ref_pool = oracle.deserialize(want)["pool"][:need]
+    hb = oracle.header_bytes(bset.n_tensors, bset.n_blocks)
+    mid = (hb + (total - hb) // 2) // 16 * 16
+    cuts = [(0, mid), (mid, total)]
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, total, DEV)
+    main = torch.cuda.current_stream()
+    side = [torch.cuda.Stream(), torch.cuda.Stream()]
+    dst = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB)
+    for it in range(12):
+        out = torch.full((total,), 0xCD, dtype=torch.uint8, device=DEV)
+        pool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+        # the pass on the main stream, then the two halves side by side
+        bs.serialize_range(up.dset.desc, out.data_ptr(), 0, 0, True, ws.ptr, ws.nbytes, ws.result_ptr, opts, main.cuda_stream)
+        for s, (lo, hi) in zip(side, cuts):
+            s.wait_stream(main)
+            bs.serialize_range(up.dset.desc, out.data_ptr() + lo, lo, hi, False, ws.ptr, ws.nbytes, ws.result_ptr, opts, s.cuda_stream)
+        for s in side:
+            main.wait_stream(s)
+        assert ws.read_result()["status"] == bs.OK
+        bad = np.nonzero(out.cpu().numpy() != want)[0]
+        assert bad.size == 0, f"round {it}: first wrong stream byte {bad[0]} of {total}"
+        # the mirror image: bs_deserialize leaves the parsed tables (and fills the pool once); the pool is poisoned again and
+        # the two halves are scattered side by side, the first one rebuilding the descriptor arrays as well
+        bs.deserialize(out.data_ptr(), total, dst.desc, pool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, ws.result_ptr,
+                       opts, main.cuda_stream)
+        pool.fill_(0xEE)
+        for t in (dst.tensors, dst.qn, dst.dim):
+            t.fill_(0xAB)
+        for s, (lo, hi) in zip(side, cuts):
+            s.wait_stream(main)
+            bs.deserialize_range(out.data_ptr() + lo, lo, hi, out.data_ptr() if lo == 0 else 0, dst.desc, bs.LAYOUT_POOL, ws.ptr,
+                                 ws.nbytes, opts, s.cuda_stream)
+        for s in side:
+            main.wait_stream(s)
+        torch.cuda.synchronize()
+        assert ws.read_result()["status"] == bs.OK
+        bad = np.nonzero(pool.cpu().numpy() != ref_pool)[0]
+        assert bad.size == 0, f"round {it}: first wrong pool byte {bad[0]} of {need}"
+        assert bytes(dst.tensors.cpu().numpy()[:32 * bset.n_tensors]) == bset.tensors.tobytes()
+        assert (dst.qn.cpu().numpy()[:24 * bset.n_blocks].view(np.int32).reshape(-1, 3, 2) == bset.qn).all()
+        assert (dst.dim.cpu().numpy()[:12 * bset.n_blocks].view(np.uint32).reshape(-1, 3) == bset.dim).all()
+
+
 def test_deserialize_capacity_errors():
     bset = W.make_set("cap", 42, D=40, S=9, M=2, N0=3, n_ops=13, n_site=1, dims="multinomial")
     want, _, _ = oracle_stream(bset)
