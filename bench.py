@@ -17,7 +17,10 @@ metric's "% of HBM peak" is meaningful on; inputs are ~7 GB, far larger than the
     roofline  the dominant kernel (pack): algorithmic HBM bytes per launch / its CUDA-event duration, against the
               measured copy bandwidth in MEASURED_PEAKS.json; beside it the unpack kernel, the whole-call fractions of the
               8 TB/s nominal figure, an in-run ceiling (the same mover on ONE contiguous block: a pure cp.async.bulk
-              copy) and ``at_scale``: the same numbers on workload 4L (42.5 GB, the total BASELINE.json states).
+              copy), ``at4L_*``: the same numbers on workload 4L (42.5 GB, the total BASELINE.json states), and one whole-call
+              number per variant (``v2_``, ``a8_``, ``f32_``, ``rank4_``, ``pkg1MiB_``).  e2e likewise carries ``at3L_*`` (config 5
+              at 11 GB) and the config-1 / config-2 latencies (``cfg1_*_us``, ``cfg2_*_us``).  All flat and first: the driver's
+              record keeps the first 24 scalar keys of each dict (ROOFLINE_FIRST / E2E_FIRST).
     cpu_baseline  the CPU oracle (oracle/, single thread, as it stands) on a bounded sample of the same workload, plus
               the paper's own design as context: threads filling disjoint intervals of one buffer (L106-108).
     detail    (last key, context only) per-direction numbers, packages, small sets, the config-5 sweeps.
@@ -450,6 +453,7 @@ def run_mine(args):
     roofline.update({
         "unpack_kernel_ms": round(unpack_ms, 4), "unpack_achieved": round(unpack_algo / (unpack_ms * 1e-3) / 1e9, 1),
         "unpack_frac": round(unpack_algo / (unpack_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], 4),
+        "unpack_frac_of_8TBs": round(unpack_algo / (unpack_ms * 1e-3) / 1e9 / 8000.0, 4),
         "unpack_kernel": ("bs::move_kernel<unpack>" if args.variant == 1 else "bs::move_tma_kernel<unpack>") + " (S7 rebuild + unpack)",
         "serialize_ms": round(med_ser, 4), "deserialize_ms": round(med_des, 4),
         "serialize_hbm_GBs": round(2 * total / med_ser / 1e6, 1), "deserialize_hbm_GBs": round(2 * total / med_des / 1e6, 1),
@@ -465,6 +469,19 @@ def run_mine(args):
             roofline["unpack_frac_of_bulk_copy"] = round(roofline["unpack_achieved"] / roofline["bulk_copy_GBs"], 4)
         except Exception as ex:   # the headline numbers stand on their own
             roofline["bulk_copy_error"] = repr(ex)
+
+    variants_detail = None
+    # ---- one number per SURVEY §8(f) variant on this workload's blocks (rank 0; fp64 / v1 runs of a multi-GB workload) ----
+    if rank == 0 and not v2 and args.elem == "f64" and not args.no_variants and total >= (1 << 30):
+        try:
+            vflat, vdet = variant_legs(bs, torch, W, fill_pool_device, dev, opts, bset, addr, stream, opool, cs)
+            roofline.update(vflat)
+            variants_detail = vdet
+        except Exception as ex:
+            variants_detail = {"error": repr(ex)}
+        ser()   # the variants reused stream / opool and other workspaces: put this workload's stream and tables back
+        deser()
+        check_ok("after the variant legs")
 
     ab = None
     if args.ab and not v2:
@@ -492,6 +509,8 @@ def run_mine(args):
               "size_pass_ms_incl_sync": round(scan_ms, 4)}
     if ab is not None:
         detail["ab"] = ab
+    if variants_detail is not None:
+        detail["variants"] = variants_detail
     a, b = ev(), ev()
     e2e = None
     if not args.no_e2e:
@@ -710,6 +729,9 @@ def run_mine(args):
                                       "unpack_hbm_GBs": round(2 * total / t["unpack"] / 1e6, 1)}
             del slots, wsp
         detail["packages"] = pk
+        if "cap_1MiB" in pk:
+            roofline["pkg1MiB_emit_frac_of_8TBs"] = round(pk["cap_1MiB"]["emit_hbm_GBs"] / 8000, 4)
+            roofline["pkg1MiB_unpack_frac_of_8TBs"] = round(pk["cap_1MiB"]["unpack_hbm_GBs"] / 8000, 4)
 
     # ---- config 5: exposed IO of an offload overlapped with a stand-in contraction (rank 0 only) ----
     if rank == 0 and not args.no_config5 and not v2:
@@ -736,14 +758,15 @@ def run_mine(args):
                 torch.cuda.empty_cache()
                 cl = config5(args, dev, opts, name="3L", full=False)
                 hs, hl = cl["headline"], cl["prefetch"]["headline"]
-                e2e["at_scale_3L"] = {"stream_bytes": cl["stream_bytes"], "exposed_io_frac_save": hs["exposed_io_frac"],
-                                      "exposed_io_frac_load": hl["exposed_io_frac"], "exposed_io_r_actual": [hs["r_actual"], hl["r_actual"]],
-                                      "sustained_pcie_GBs_save": hs["sustained_pcie_GBs"], "sustained_pcie_GBs_load": hl["sustained_pcie_GBs"],
-                                      "offload_alone_GBs": round(cl["stream_bytes"] / cl["T_io_ms"] / 1e6, 2),
-                                      "prefetch_alone_GBs": round(cl["stream_bytes"] / cl["prefetch"]["T_io_ms"] / 1e6, 2)}
+                e2e.update({"at3L_stream_GB": round(cl["stream_bytes"] / 1e9, 3), "at3L_exposed_io_frac_save": hs["exposed_io_frac"],
+                            "at3L_exposed_io_frac_load": hl["exposed_io_frac"],
+                            "at3L_sustained_pcie_GBs_save": hs["sustained_pcie_GBs"], "at3L_sustained_pcie_GBs_load": hl["sustained_pcie_GBs"],
+                            "at3L_r_actual_save": hs["r_actual"], "at3L_r_actual_load": hl["r_actual"],
+                            "at3L_offload_alone_GBs": round(cl["stream_bytes"] / cl["T_io_ms"] / 1e6, 2),
+                            "at3L_prefetch_alone_GBs": round(cl["stream_bytes"] / cl["prefetch"]["T_io_ms"] / 1e6, 2)})
                 del cl
             except Exception as ex:
-                e2e["at_scale_3L"] = {"error": repr(ex)}
+                detail["at_scale_3L"] = {"error": repr(ex)}
 
     # ---- cpu baseline: the oracle on a bounded sample (rank 0, N = 1 only) ----
     cpu = None
@@ -771,14 +794,29 @@ def run_mine(args):
         del stream, opool, pool, out, dset, ws
         torch.cuda.empty_cache()
         try:
-            roofline["at_scale"] = at_scale(bs, torch, W, fill_pool_device, dev, opts, peaks)
+            big = at_scale(bs, torch, W, fill_pool_device, dev, opts, peaks)
+            detail["at_scale_4L"] = big
+            if "skipped" not in big:
+                roofline.update({"at4L_pack_frac_of_8TBs": big["frac_of_nominal_8TBs"],
+                                 "at4L_unpack_frac_of_8TBs": round(big["unpack_achieved"] / 8000, 4),
+                                 "at4L_serialize_frac_of_8TBs": big["serialize_frac_of_8TBs"],
+                                 "at4L_deserialize_frac_of_8TBs": big["deserialize_frac_of_8TBs"],
+                                 "at4L_stream_GB": round(big["stream_bytes"] / 1e9, 3), "at4L_pack_frac": big["frac"],
+                                 "at4L_unpack_frac": big["unpack_frac"], "at4L_n_blocks": big["n_blocks"]})
         except Exception as ex:
-            roofline["at_scale"] = {"error": repr(ex)}
+            detail["at_scale_4L"] = {"error": repr(ex)}
 
     ms_g, units_g = aggregate(step_ms, 2 * total, world, dev, ready)
     sampler.stop()
     if rank == 0:
         fused = (not v2) and args.variant != 1 and max(-(-bset.n_blocks // 1024), -(-bset.n_tensors // 1024)) <= sm_count(torch, dev)
+        for wl, row in (detail.get("small_sets") or {}).items():   # config1 / config2 latencies, flat
+            tgt = e2e if e2e is not None else roofline
+            for k in ("serialize_us", "deserialize_us", "plain_copy_us"):
+                tgt[f"cfg{wl[-1]}_{k}"] = row[k]
+        detail["roofline_text"] = {k: v for k, v in roofline.items() if isinstance(v, (str, list, dict))}
+        detail["e2e_text"] = {k: v for k, v in (e2e or {}).items() if isinstance(v, (str, list, dict))}
+        roofline, e2e = ordered_for_record(roofline, ROOFLINE_FIRST), ordered_for_record(e2e, E2E_FIRST)
         line = {"metric": METRIC, "value": round(units_g / (ms_g * 1e-3) / 1e9, 3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_g, 4), "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
@@ -875,6 +913,111 @@ def bulk_copy_ceiling(bs, torch, pool, stream, dev, opts, cs, n):
     return {"bulk_copy_GBs": round(2 * tot1 / ms / 1e6, 1), "bulk_copy_bytes": int(tot1),
             "bulk_copy_what": "this run: bs::move_tma_kernel<pack> on ONE contiguous block of that many bytes (pure cp.async.bulk copy)",
             "runtime_d2d_copy_GBs": round(2 * (tot1 - hb1) / ms_rt / 1e6, 1)}
+
+
+# The driver's record keeps the first 24 SCALAR keys of roofline / e2e / cpu_baseline (nested dicts and lists are dropped,
+# strings cut): every bar the north_star states, at the benchmark's size and at the sizes BASELINE.json states, and one
+# number per SURVEY §8(f) row go first, flat; everything else follows and is repeated in `detail`.
+ROOFLINE_FIRST = ["bound", "achieved", "peak", "unit", "frac", "traffic", "kernel_ms", "unpack_frac", "frac_of_nominal_8TBs",
+                  "unpack_frac_of_8TBs", "serialize_frac_of_8TBs", "deserialize_frac_of_8TBs", "frac_of_bulk_copy",
+                  "unpack_frac_of_bulk_copy", "at4L_pack_frac_of_8TBs", "at4L_unpack_frac_of_8TBs", "at4L_serialize_frac_of_8TBs",
+                  "at4L_deserialize_frac_of_8TBs", "at4L_stream_GB", "v2_serialize_frac_of_8TBs", "a8_serialize_frac_of_8TBs",
+                  "f32_serialize_frac_of_8TBs", "rank4_serialize_frac_of_8TBs", "pkg1MiB_emit_frac_of_8TBs"]
+E2E_FIRST = ["value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "ms_per_step", "offload_frac_of_pinned_d2h",
+             "prefetch_frac_of_pinned_h2d", "duplex_frac_of_bidirectional_memcpy", "exposed_io_frac_save", "exposed_io_frac_load",
+             "exposed_io_r", "at3L_exposed_io_frac_save", "at3L_exposed_io_frac_load", "at3L_sustained_pcie_GBs_save",
+             "at3L_sustained_pcie_GBs_load", "at3L_stream_GB", "sweep_speedup_queue_over_sync_io", "cfg2_serialize_us",
+             "cfg2_deserialize_us", "cfg2_plain_copy_us", "cfg1_serialize_us", "cfg1_deserialize_us", "cfg1_plain_copy_us",
+             "offload_pcie_GBs"]
+
+
+def ordered_for_record(d, first):
+    """The keys of `first` that `d` has, in that order, then d's other scalars, then its strings / lists / dicts."""
+    if d is None:
+        return None
+    scalar = lambda v: v is None or isinstance(v, (int, float, bool))
+    out = {k: d[k] for k in first if k in d}
+    out.update({k: v for k, v in d.items() if k not in out and scalar(v)})
+    out.update({k: v for k, v in d.items() if k not in out})
+    return out
+
+
+def variant_legs(bs, torch, W, fill_pool_device, dev, opts, bset, addr, stream, opool, cs, reps=3):
+    """One whole-call number per SURVEY §8(f) variant on THIS workload's blocks (same pool, same launch defaults): wire format
+    v2 (structure-shared layers), unpadded align = 8, f32 elements; and order-4 tensors (wire format v3) on a 1.4 GB tree set
+    of its own.  Returns (flat scalars for the roofline dict, detail).  frac_of_8TBs = 2 * stream bytes / time / 8 TB/s."""
+    flat, det = {}, {}
+
+    def timed(fn):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    def leg(tag, ser, deser, ws, total):
+        s_ms = timed(ser)
+        d_ms = timed(deser)
+        r = ws.read_result()
+        if r["status"] != bs.OK or r["total_bytes"] != total:
+            raise RuntimeError(f"variant {tag}: {r}")
+        flat[f"{tag}_serialize_frac_of_8TBs"] = round(2 * total / s_ms / 1e6 / 8000, 4)
+        flat[f"{tag}_deserialize_frac_of_8TBs"] = round(2 * total / d_ms / 1e6 / 8000, 4)
+        det[tag] = {"stream_bytes": int(total), "serialize_ms": round(s_ms, 4), "deserialize_ms": round(d_ms, 4),
+                    "serialize_hbm_GBs": round(2 * total / s_ms / 1e6, 1), "deserialize_hbm_GBs": round(2 * total / d_ms / 1e6, 1)}
+
+    cap = stream.numel()
+    for tag, dtype, e in (("a8", bs.F64 | bs.ALIGN8, 8), ("f32", bs.F32, 4)):
+        try:
+            dset = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, addr, dev, dtype=dtype)
+            ws = bs.Workspace(bset.n_tensors, bset.n_blocks, cap, dev)
+            _, total = bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs)
+            need = int(((bset.nelems * e + 255) // 256 * 256).sum())
+            out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, dev)
+            assert total <= cap and need <= opool.numel()
+            leg(tag, lambda: bs.serialize(dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs),
+                lambda: bs.deserialize(stream.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                                       ws.result_ptr, opts, cs), ws, total)
+            del dset, ws, out
+        except Exception as ex:
+            det[tag] = {"error": repr(ex)}
+    try:
+        lv = W.layered_view(bset)
+        counts = (len(lv["structs"]), lv["dim"].shape[0], bset.n_tensors, bset.n_blocks)
+        lset = bs.DeviceLayeredSet.from_host(lv["structs"], lv["layers"], lv["qn"], lv["dim"], addr, dev)
+        ws = bs.Workspace(0, 0, cap, dev, layered=counts)
+        _, total = bs.layered_serialized_size(lset.desc, ws.ptr, ws.nbytes, cs)
+        need = int(((bset.nelems * 8 + 255) // 256 * 256).sum())
+        out = bs.DeviceLayeredSet.empty(*counts, dev)
+        assert total <= cap and need <= opool.numel()
+        leg("v2", lambda: bs.layered_serialize(lset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs),
+            lambda: bs.layered_deserialize(stream.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr,
+                                           ws.nbytes, ws.result_ptr, opts, cs), ws, total)
+        del lset, ws, out
+    except Exception as ex:
+        det["v2"] = {"error": repr(ex)}
+    try:
+        tset = W.make_tree_set("tree-1.4GB", 8, D=600, S=12, n_nodes=6, n_ops=13)
+        tpool, taddr = fill_pool_device(tset, dev)
+        dset = bs.DeviceSet.from_host(tset.tensors, tset.qn, tset.dim, taddr, dev, dtype=bs.F64 | bs.RANK4)
+        ws = bs.Workspace(tset.n_tensors, tset.n_blocks, cap, dev)
+        _, total = bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs)
+        need = int(((tset.nelems * 8 + 255) // 256 * 256).sum())
+        out = bs.DeviceSet.empty(tset.n_tensors, tset.n_blocks, dev, rank4=True)
+        assert total <= cap and need <= opool.numel()
+        leg("rank4", lambda: bs.serialize(dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, opts, cs),
+            lambda: bs.deserialize(stream.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes,
+                                   ws.result_ptr, opts, cs), ws, total)
+        det["rank4"]["set"] = f"order-4 tree set D=600, 12 sectors, 6 nodes + 13 operators: {tset.n_blocks} blocks"
+        del tpool, dset, ws, out
+    except Exception as ex:
+        det["rank4"] = {"error": repr(ex)}
+    return flat, det
 
 
 def at_scale(bs, torch, W, fill_pool_device, dev, opts, peaks, name="4L", steps=5):
@@ -1186,7 +1329,8 @@ def main():
     ap.add_argument("--no-config5", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-ceiling", action="store_true", help="skip the in-run bulk-copy ceiling of the roofline leg")
-    ap.add_argument("--no-at-scale", action="store_true", help="skip roofline.at_scale (workload 4L, 42.5 GB)")
+    ap.add_argument("--no-at-scale", action="store_true", help="skip the at4L_* (workload 4L, 42.5 GB) and at3L_* (11 GB) numbers")
+    ap.add_argument("--no-variants", action="store_true", help="skip the per-variant numbers (v2, align 8, f32, rank 4) of the roofline dict")
     ap.add_argument("--no-threads-sweep", action="store_true", help="skip cpu_baseline.threads_sweep")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "mine" else args.warmup

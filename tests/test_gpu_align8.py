@@ -18,7 +18,11 @@ pytestmark = pytest.mark.gpu
 
 SHAPES = [None, dict(variant=bs.VARIANT_TMA, fuse=1), dict(variant=bs.VARIANT_TMA, fuse=2),
           dict(variant=bs.VARIANT_TMA, tile_bytes=32768, stages=4, warps=1), dict(variant=bs.VARIANT_TMA, tile_bytes=49152, stages=3, warps=1),
-          dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=4, fuse=2), dict(variant=bs.VARIANT_TMA, tile_bytes=65536)]
+          dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=4, fuse=2), dict(variant=bs.VARIANT_TMA, tile_bytes=65536),
+          # what sets of half a GB and more select for themselves (tests/test_gpu_fullsize.py runs it at that size): tiles
+          # from the counter (tune 0x10), the table two iterations ahead (0x1000), one ring of 3 x 48 KiB
+          dict(variant=bs.VARIANT_TMA, tune=0x10), dict(variant=bs.VARIANT_TMA, tile_bytes=49152, stages=3, warps=1, tune=0x1010),
+          dict(variant=bs.VARIANT_TMA, tile_bytes=49152, stages=3, warps=1, tune=0x1010, fuse=2)]
 
 
 def sets():

@@ -307,3 +307,69 @@ def test_full_size_queue_config3():
     st = q.stats()
     assert st["host_bytes_live"] == 2 * total and st["device_bytes"] < 2 * (2 * (256 << 20)) + (256 << 20)
     q.destroy()
+
+
+# ---- the SURVEY §8(f) NEXT-4 variants at sizes that reach the launch shape large sets select for themselves -----------------
+# (round 3; the align-8 movers, wire format v3 and the other element types had met their oracles only on sets of
+# <= 77 MB, i.e. with the static deal of the tiles and the small ring shape).  DEFAULT opts on >= 1 GB: one ring of
+# 3 x 48 KiB, tiles from the counter, table two iterations ahead, stream offsets beyond 2^32 for align 8.  The oracle
+# serializes the whole set at once from a host copy of the seeded source pool; every stream byte and every byte of the
+# deserialized pool image is compared.
+def _variant_case(name):
+    from oracle import dt, v3
+    if name == "align8":          # config 3: 2.2 GB, 447 k blocks of ~5 KB, about half of them 8 off the 16-byte grid
+        bset = W.make_config("3")
+        return bset, bs.F64 | bs.ALIGN8, 8, False, lambda addr, blocks: oracle.serialize(bset.tensors, bset.qn, bset.dim, addr, align=8), \
+            lambda s: (oracle.pool_bytes(s), oracle.deserialize(s)["pool"])
+    if name == "rank4":           # order-4 tree nodes + operators: 1.4 GB, 3394 blocks (wire format v3)
+        bset = W.make_tree_set("tree-1.4GB", 8, D=600, S=12, n_nodes=6, n_ops=13)
+        return bset, bs.F64 | bs.RANK4, 8, True, lambda addr, blocks: v3.serialize(bset.tensors, bset.qn, bset.dim, addr), \
+            lambda s: (v3.pool_bytes(s), v3.deserialize(s)["pool"])
+    if name == "f32":             # config 4's sectors with 450 operators read as f32: 1.1 GB (the independent numpy oracle)
+        bset = W.make_config("4", n_ops=450)
+        def deser32(s):
+            r = dt.deserialize(s)
+            return r["pool_bytes"], np.asarray(r["pool"])
+        return bset, bs.F32, 4, False, lambda addr, blocks: dt.serialize(bset.tensors, bset.qn, bset.dim, blocks(), dt.F32), deser32
+    raise KeyError(name)
+
+
+@pytest.mark.parametrize("name", ["align8", "rank4", "f32"])
+def test_full_size_variants_with_default_opts(name):
+    from oracle import dt
+    from workloads.device import fill_pool_device
+    bset, dtype, e, rank4, ser, deser = _variant_case(name)
+    _room_for(name, bset)
+    d_pool, d_addr = fill_pool_device(bset, DEV)
+    hp = HostPool(bset, d_pool)                       # host copy of the seeded pool, spot-checked against the host generator
+    blocks = lambda: [hp.pool[int(o): int(o) + e * int(k)] for o, k in zip(bset.pool_off, bset.nelems)]
+    want = ser(hp.addr, blocks)
+    total = len(want)
+    assert total >= (1 << 30) and total - bs.header_bytes(bset.n_tensors, bset.n_blocks) >= (512 << 20), "must reach the large shape"
+    dset = bs.DeviceSet.from_host(bset.tensors, bset.qn, bset.dim, d_addr, DEV, dtype=dtype)
+    ws = bs.Workspace(bset.n_tensors, bset.n_blocks, total, DEV)
+    cs = bs.current_stream()
+    hb = bs.header_bytes_rank4(bset.n_tensors, bset.n_blocks) if rank4 else bs.header_bytes(bset.n_tensors, bset.n_blocks)
+    assert bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs) == (hb, total)
+    stream = torch.full((total + 4096,), 0xCD, dtype=torch.uint8, device=DEV)
+    bs.serialize(dset.desc, stream.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, None, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["total_bytes"] == total and res["dtype"] == dtype, res
+    got = stream.cpu().numpy()
+    assert (got[total:] == 0xCD).all(), "bytes beyond the stream were written"
+    from tests.fullsize import equal_bytes, first_difference
+    assert equal_bytes(got[:total], want), f"{name}: stream differs first at byte {first_difference(got[:total], want)} (header {hb})"
+    del got
+    need = int(((bset.nelems * e + 255) // 256 * 256).sum())
+    out = bs.DeviceSet.empty(bset.n_tensors, bset.n_blocks, DEV, fill=0xAB, rank4=rank4)
+    opool = torch.full((need,), 0xEE, dtype=torch.uint8, device=DEV)
+    bs.deserialize(stream.data_ptr(), total, out.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, ws.result_ptr, None, cs)
+    res = ws.read_result()
+    assert res["status"] == bs.OK and res["pool_bytes"] == need, res
+    host = out.to_host()
+    assert host["tensors"].tobytes() == bset.tensors.tobytes() and (host["qn"] == bset.qn).all() and (host["dim"] == bset.dim).all()
+    gpool = opool.cpu().numpy()
+    n_ref, ref = deser(want)
+    assert n_ref == need
+    ref = np.frombuffer(ref, np.uint8) if not isinstance(ref, np.ndarray) else ref
+    assert equal_bytes(gpool, ref[:need]), f"{name}: pool image differs first at byte {first_difference(gpool, ref[:need])}"

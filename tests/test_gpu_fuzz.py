@@ -39,8 +39,14 @@ def random_set(rng):
 
 
 def upload(rng, tensors, qn, dim, dtype):
+    return upload_host(rng, tensors, qn, dim, dtype)[:3]
+
+
+def upload_host(rng, tensors, qn, dim, dtype, flags=0):
+    """As upload (same draws in the same order), any number of legs; also returns the host image and the block offsets in it.
+    `flags` (bs.ALIGN8 / bs.RANK4) go into the device descriptor's dtype word."""
     e = dt.ELEM_BYTES[dtype]
-    sizes = [e * int(d[0]) * int(d[1]) * int(d[2]) for d in dim]
+    sizes = [e * int(np.prod([int(x) for x in d])) for d in dim]
     blocks = [rng.integers(0, 256, n, dtype=np.uint8).tobytes() for n in sizes]
     cur = 0
     order = list(rng.permutation(len(blocks))) if blocks else []
@@ -54,8 +60,8 @@ def upload(rng, tensors, qn, dim, dtype):
         host[int(o): int(o) + len(b)] = np.frombuffer(b, np.uint8)
     pool = torch.from_numpy(host).to(DEV)
     addr = (np.uint64(pool.data_ptr()) + offs).astype(np.uint64)
-    dset = bs.DeviceSet.from_host(tensors, qn, dim, addr, DEV, dtype=dtype)
-    return pool, dset, blocks
+    dset = bs.DeviceSet.from_host(tensors, qn, dim, addr, DEV, dtype=dtype | flags)
+    return pool, dset, blocks, host, offs
 
 
 def wide_opts(rng):
@@ -151,6 +157,84 @@ def test_random_sets_round_trip_bit_exact(seed):
         bs.deserialize(out.data_ptr(), total, o.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, ws.result_ptr, wide, cs)
         assert ws.read_result()["status"] == bs.OK, wide
         assert (opool.cpu().numpy()[:need] == ref["pool"][:need]).all(), f"seed {seed}: blocks differ with {wide}"
+
+
+def random_set4(rng):
+    """Free-form set of ranks 2, 3 and 4 with four legs per block (BS_RANK4; unused legs: extent 1, labels 0)."""
+    T = int(rng.integers(0, 7))
+    tensors = np.zeros(T, W.TENSOR_REC_DTYPE)
+    qn, dim = [], []
+    for t in range(T):
+        rank = int(rng.choice([2, 3, 4]))
+        nb = int(rng.integers(0, 9))
+        sign = (1, 1, 1, -1) if rank == 4 else ((-1, 1, -1, 0) if rank == 3 else (-1, 1, 0, 0))
+        tensors[t] = (rank, len(dim), nb, tuple(int(x) for x in rng.integers(-2, 3, 2)), sign, int(rng.integers(0, 1 << 31)), 0)
+        for _ in range(nb):
+            d = [int(rng.choice(EXTENTS)) if k < rank else 1 for k in range(4)]
+            if rank == 4:
+                d[2] = int(rng.choice(EXTENTS[:6]))                              # keep order-4 blocks below a few MB
+                d[3] = int(rng.choice(EXTENTS[:9]))
+            if rng.random() < 0.1:
+                d[int(rng.integers(0, 2))] = int(rng.integers(500, 1500)) if rank < 4 else 40
+            q = rng.integers(-5, 6, (4, 2)).astype(np.int32)
+            q[rank:] = 0
+            qn.append(q)
+            dim.append(d)
+    return tensors, np.array(qn, np.int32).reshape(-1, 4, 2), np.array(dim, np.uint32).reshape(-1, 4)
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_unpadded_and_rank4_sets_through_random_launch_shapes(seed):
+    """BS_ALIGN8 (even seeds) and BS_RANK4 (odd seeds) sets through the default shape and three drawn from the whole space
+    (wide_opts: tile counter forced or forbidden, table further ahead, one launch or two, tiles of any multiple of 1 KiB) —
+    the variants' own movers had only met fixed shapes.  Stream, concat of ranges, round trip: bit for bit."""
+    from oracle import v3
+    rng = np.random.default_rng(9000 + seed)
+    rank4 = bool(seed & 1)
+    dtype = int(rng.integers(0, 4))
+    if rank4:
+        tensors, qn, dim = random_set4(rng)
+        pool, dset, blocks, host, offs = upload_host(rng, tensors, qn, dim, dtype, bs.RANK4)
+        want = v3.serialize(tensors, qn, dim, (np.uint64(host.ctypes.data) + offs).astype(np.uint64), dtype=dtype)
+        ref_pool, need = v3.deserialize(want)["pool"], v3.pool_bytes(want)
+        hb = v3.header_bytes(len(tensors), len(blocks))
+    else:
+        tensors, qn, dim = random_set(rng)
+        pool, dset, blocks, host, offs = upload_host(rng, tensors, qn, dim, dtype, bs.ALIGN8)
+        want = dt.serialize(tensors, qn, dim, blocks, dtype, align=8)
+        ref = dt.deserialize(want)
+        ref_pool, need = ref["pool"], ref["pool_bytes"]
+        hb = dt.header_bytes(len(tensors), len(blocks))
+        if dtype == dt.F64 and len(blocks):    # the C oracle as a second opinion
+            assert bytes(oracle.serialize(tensors, qn, dim, (np.uint64(host.ctypes.data) + offs).astype(np.uint64), align=8)) == bytes(want)
+    total, T, B = len(want), len(tensors), len(blocks)
+    ws = bs.Workspace(T, B, max(total, 1 << 16), DEV)
+    cs = bs.current_stream()
+    assert bs.serialized_size(dset.desc, ws.ptr, ws.nbytes, cs) == (hb, total)
+    out = torch.full((total + 32,), 0xCD, dtype=torch.uint8, device=DEV)
+    rng_out = torch.full((total + 32,), 0xCD, dtype=torch.uint8, device=DEV)
+    o = bs.DeviceSet.empty(T, B, DEV, fill=0xAB, rank4=rank4)
+    opool = torch.full((max(need, 256),), 0xEE, dtype=torch.uint8, device=DEV)
+    for shape in [None] + [wide_opts(rng) for _ in range(3)]:
+        out.fill_(0xCD)
+        bs.serialize(dset.desc, out.data_ptr(), total, ws.ptr, ws.nbytes, ws.result_ptr, shape, cs)
+        res = ws.read_result()
+        assert res["status"] == bs.OK and res["total_bytes"] == total, (shape, res)
+        got = out.cpu().numpy()
+        assert (got[:total] == want).all() and (got[total:] == 0xCD).all(), f"seed {seed}: stream differs with {shape}"
+        chunk = int(rng.integers(1, 40)) * 16 * int(rng.choice([64, 4096]))
+        rng_out.fill_(0xCD)
+        for lo in range(0, total, chunk):      # hi is a multiple of 16 and clipped to the total (a multiple of 8 when unpadded)
+            bs.serialize_range(dset.desc, rng_out.data_ptr() + lo, lo, lo + chunk, lo == 0, ws.ptr, ws.nbytes, ws.result_ptr, shape, cs)
+        got = rng_out.cpu().numpy()
+        assert (got[:total] == want).all() and (got[total:] == 0xCD).all(), f"seed {seed}: concat of ranges differs (chunk {chunk}) with {shape}"
+        opool.fill_(0xEE)
+        bs.deserialize(out.data_ptr(), total, o.desc, opool.data_ptr(), need, bs.LAYOUT_POOL, ws.ptr, ws.nbytes, ws.result_ptr, shape, cs)
+        res = ws.read_result()
+        assert res["status"] == bs.OK and res["pool_bytes"] == need and (res["n_tensors"], res["n_blocks"]) == (T, B), (shape, res)
+        assert (opool.cpu().numpy()[:need] == ref_pool[:need]).all(), f"seed {seed}: blocks differ with {shape}"
+        h = o.to_host()
+        assert h["tensors"].tobytes() == tensors.tobytes() and (h["qn"] == qn).all() and (h["dim"] == dim).all()
 
 
 def random_layered(rng):
