@@ -50,7 +50,8 @@ UNIT = "GB/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
 
-ELEM = {"f64": (0, 8), "f32": (1, 4), "c64": (2, 8), "c128": (3, 16)}   # bs.h dtype, element bytes
+ELEM = {"f64": (0, 8), "f32": (1, 4), "c64": (2, 8), "c128": (3, 16),   # bs.h dtype, element bytes
+        "f64a8": (0x100, 8)}   # fp64 as an UNPADDED stream (BS_ALIGN8): kernels only, as the other element types
 
 
 def log(*a):
@@ -306,7 +307,9 @@ def workload_config(name, bset, total, fmt="v1"):
 
 
 def with_elem(c, elem):
-    if elem != "f64":
+    if elem == "f64a8":
+        c["element_type"] = "f64, unpadded stream (BS_ALIGN8: the header's align word = 8)"
+    elif elem != "f64":
         c["element_type"] = f"{elem}: every block read as {ELEM[elem][1]}-byte elements (the first e*n bytes of its fp64 storage)"
     return c
 
