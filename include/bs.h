@@ -159,13 +159,25 @@ typedef struct bs_opts {
     uint32_t ctas_per_sm; /* LDG: persistent CTAs per SM; 0 = default (occupancy limit) */
     uint32_t stages;      /* TMA: ring depth (tiles) per warp, 3..8; 0 = default */
     uint32_t warps;       /* TMA: warps (rings) per CTA, 1..16; warps*stages*tile_bytes <= 225 KiB; 0 = default */
-    uint32_t reserved[3]; /* 0.  [0]: experiment switches of the TMA variant (bits; see bs_move_tma.cu); [1]: bs_serialize /
-                             bs_deserialize as one fused launch (size / offset pass + movement in one kernel): 0 = by size
-                             (sets of up to ~150 k blocks), 1 = never, 2 = always; [2]: pacing of the TMA variant (experiments: a warp
-                             starts the loads of its next tile no earlier than its share of a target traffic rate allows):
-                             0 = none, >= 100 = that many GB/s of HBM traffic for the whole launch */
+    uint32_t tune;        /* TMA: how tiles are handed out and how far ahead a tile's block table is fetched — OR of BS_TUNE_* below;
+                             0 = by size.  The static deal and the forced counter are what the decomposition tests (P6) and
+                             bench.py --ab compare; the remaining bits are measurement switches of DESIGN.md §20 (each measured and
+                             left off by default).  Bits outside BS_TUNE_KNOWN_BITS: BS_ERR_ARG. */
+    uint32_t fuse;        /* bs_serialize / bs_deserialize as ONE launch (size / offset pass + movement in one kernel): 0 = by size
+                             (sets of up to ~150 k blocks), 1 = never, 2 = always; > 2: BS_ERR_ARG */
+    uint32_t pace;        /* TMA, measurements only: a warp starts the loads of its next tile no earlier than its share of a target
+                             traffic rate allows; 0 (and anything < 100) = none, >= 100 = that many GB/s of HBM traffic for the launch */
 } bs_opts;
 enum { BS_VARIANT_DEFAULT = 0, BS_VARIANT_LDG = 1, BS_VARIANT_TMA = 2 };
+/* bs_opts.tune (until round 2 these rode in a field called `reserved`; same offsets, so the struct layout is unchanged) */
+#define BS_TUNE_EVICT_FIRST_LD 0x1u    /* L2 evict_first hint on bulk loads (measured: no gain) */
+#define BS_TUNE_EVICT_FIRST_ST 0x2u    /* ... on bulk stores */
+#define BS_TUNE_DEAL_STATIC    0x8u    /* tiles dealt round-robin (round 1) whatever the size */
+#define BS_TUNE_DEAL_COUNTER   0x10u   /* tiles from the launch's counter whatever the size (default: ranges of >= 128 MiB) */
+#define BS_TUNE_L2_PREFETCH    0x20u   /* unpack asks the next stream tile into L2 (measured: inside the spread) */
+#define BS_TUNE_MAX_LOADS_MASK 0xf00u  /* at most ((tune >> 8) & 15) tiles loading beside the one being stored; 0 = ring depth - 2 */
+#define BS_TUNE_TABLE_AHEAD_2  0x1000u /* block table fetched two iterations ahead (default: pack of sets >= 512 MiB) */
+#define BS_TUNE_KNOWN_BITS     0x1f3bu
 
 /* ---- host-only helpers ------------------------------------------------------------------------ */
 uint32_t bs_version(void);

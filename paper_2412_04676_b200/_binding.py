@@ -68,7 +68,7 @@ class StreamInfo(C.Structure):
 
 class Opts(C.Structure):
     _fields_ = [("variant", C.c_uint32), ("tile_bytes", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("stages", C.c_uint32),
-                ("warps", C.c_uint32), ("reserved", C.c_uint32 * 3)]
+                ("warps", C.c_uint32), ("tune", C.c_uint32), ("fuse", C.c_uint32), ("pace", C.c_uint32)]
 
 
 def make_opts(opts) -> "Opts":
@@ -76,11 +76,8 @@ def make_opts(opts) -> "Opts":
     if isinstance(opts, Opts):
         return opts
     o = Opts()
-    for k in ("variant", "tile_bytes", "ctas_per_sm", "stages", "warps"):
+    for k in ("variant", "tile_bytes", "ctas_per_sm", "stages", "warps", "tune", "fuse", "pace"):
         setattr(o, k, int((opts or {}).get(k, 0) or 0))
-    o.reserved[0] = int((opts or {}).get("tune", 0) or 0)
-    o.reserved[1] = int((opts or {}).get("fuse", 0) or 0)
-    o.reserved[2] = int((opts or {}).get("pace", 0) or 0)
     return o
 
 

@@ -53,6 +53,8 @@ int check_opts(const bs_opts& o)
 {
     if (o.variant != BS_VARIANT_LDG && o.variant != BS_VARIANT_TMA) return BS_ERR_ARG;
     if (o.ctas_per_sm > 32) return BS_ERR_ARG;
+    // the named switches (bs.h): garbage in them is refused, not interpreted
+    if (o.fuse > 2u || (o.tune & ~BS_TUNE_KNOWN_BITS) != 0) return BS_ERR_ARG;
     if (o.variant == BS_VARIANT_TMA && o.tile_bytes == 0 && o.stages == 0 && o.warps == 0) return BS_OK;  // presets
     // the LDG variant works on whole granules; a TMA tile is any multiple of 1 KiB (the block range of a tile is looked up
     // by the granules it touches)
@@ -107,8 +109,8 @@ static MoveParams pack_params(const bs_set_desc* set, const WsLayout& L, void* d
     mp.lo = lo;
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
-    mp.tune = o.reserved[0];
-    mp.pace = o.reserved[2];
+    mp.tune = o.tune;
+    mp.pace = o.pace;
     mp.flags = flags;
     mp.rank4 = set->dtype & BS_RANK4;
     return mp;
@@ -122,13 +124,13 @@ int run_pack_range(const bs_set_desc* set, const WsLayout& L, void* d_dst, uint6
     return BS_OK;
 }
 
-// One launch or two?  bs_opts.reserved[1]: 0 = by size, 1 = always separate launches, 2 = always one fused launch.  By size:
+// One launch or two?  bs_opts.fuse: 0 = by size, 1 = always separate launches, 2 = always one fused launch.  By size:
 // the fused kernel runs the pass on one CTA per SM, so sets of more work items than that leave the pass to its own,
 // wider launch (whose ~5 us are then < 1 % of the call).
 static bool use_fused(const bs_opts& o, uint64_t T, uint64_t B, int sms)
 {
-    if (o.variant != BS_VARIANT_TMA || o.reserved[1] == 1u) return false;
-    if (o.reserved[1] == 2u) return true;
+    if (o.variant != BS_VARIANT_TMA || o.fuse == 1u) return false;
+    if (o.fuse == 2u) return true;
     const uint64_t nt = (B + kScanTile - 1) / kScanTile, ntt = (T + kScanTile - 1) / kScanTile;
     return (nt > ntt ? nt : ntt) <= (uint64_t)sms;
 }
@@ -179,8 +181,8 @@ static MoveParams unpack_params(const bs_set_desc* out, const WsLayout& L, const
     mp.lo = lo;
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
-    mp.tune = o.reserved[0];
-    mp.pace = o.reserved[2];
+    mp.tune = o.tune;
+    mp.pace = o.pace;
     mp.flags = flags;
     mp.rank4 = out->dtype & BS_RANK4;
     return mp;
@@ -214,8 +216,8 @@ int run_pack_packages_range(const bs_set_desc* set, const WsLayout& L, const Pkg
     mp.lo = lo;
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
-    mp.tune = o.reserved[0];
-    mp.pace = o.reserved[2];
+    mp.tune = o.tune;
+    mp.pace = o.pace;
     mp.pkg = pm;
     mp.rank4 = set->dtype & BS_RANK4;
     cudaError_t e = launch_move(false, mp, o, sms, stream);
@@ -245,8 +247,8 @@ int run_unpack_packages_range(const bs_set_desc* out, const WsLayout& L, const P
     mp.lo = lo;
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
-    mp.tune = o.reserved[0];
-    mp.pace = o.reserved[2];
+    mp.tune = o.tune;
+    mp.pace = o.pace;
     mp.flags = flags;
     mp.pkg = pm;
     mp.rank4 = out->dtype & BS_RANK4;

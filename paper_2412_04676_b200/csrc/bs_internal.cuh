@@ -186,8 +186,8 @@ struct MoveParams {
     uint64_t lo, hi;
     uint32_t tile_bytes;
     uint32_t flags;
-    uint32_t tune;                // bs_opts.reserved[0]: experiment switches of the TMA variant
-    uint32_t pace;                // bs_opts.reserved[2]: >= 100: pace the launch at that many GB/s of HBM traffic (experiments)
+    uint32_t tune;                // bs_opts.tune: launch-shape switches of the TMA variant (bs.h BS_TUNE_*)
+    uint32_t pace;                // bs_opts.pace: >= 100: pace the launch at that many GB/s of HBM traffic (experiments)
     uint32_t rank4;               // != 0: qn / dim have four legs per block (BS_RANK4; wire format v3)
     uint32_t mv_slot;             // which tile-counter pair of the library's ring this launch uses (filled in by the launchers)
     LayeredView lay;              // lay.on != 0: qn / dim are the structure block table, header is wire format v2

@@ -803,8 +803,8 @@ int run_layered_pack_range(const bs_layered_desc* set, void* d_ws, uint64_t ws_b
     mp.lo = lo;
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
-    mp.tune = o.reserved[0];
-    mp.pace = o.reserved[2];
+    mp.tune = o.tune;
+    mp.pace = o.pace;
     mp.flags = flags;
     if (pm) mp.pkg = *pm;
     cudaError_t e = launch_move(false, mp, o, sms, stream);
@@ -828,8 +828,8 @@ int run_layered_unpack_range(const bs_layered_desc* out, void* d_ws, uint64_t ws
     mp.lo = lo;
     mp.hi = hi;
     mp.tile_bytes = o.tile_bytes;
-    mp.tune = o.reserved[0];
-    mp.pace = o.reserved[2];
+    mp.tune = o.tune;
+    mp.pace = o.pace;
     mp.flags = flags;
     if (pm) mp.pkg = *pm;
     cudaError_t e = launch_move(true, mp, o, sms, stream);

@@ -561,7 +561,7 @@ __device__ __forceinline__ void move_tma_body(const MoveParams& p, const scan::H
         tile_bytes = ps.tile_bytes; n_stages = ps.stages; n_warps = ps.warps;
         large = true;
     }
-    // pacing (experiments; bs_opts.reserved[2] >= 100): that many GB/s of HBM traffic for the whole launch
+    // pacing (experiments; bs_opts.pace >= 100): that many GB/s of HBM traffic for the whole launch
     const uint32_t rate = p.pace >= 100u ? p.pace : 0u;
     // ---- payload tiles of [lo, hi): tile k = payload bytes [k*tile_bytes, (k+1)*tile_bytes) ----
     uint64_t plo = 0, phi = 0, k0 = 0, np = 0;

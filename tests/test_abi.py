@@ -104,7 +104,10 @@ def test_launch_shapes_are_checked_without_a_device():
            dict(variant=bs.VARIANT_TMA, tile_bytes=66560, stages=3, warps=1), dict(variant=bs.VARIANT_LDG, tile_bytes=8192),
            dict(variant=bs.VARIANT_LDG, tile_bytes=20480), dict(variant=bs.VARIANT_TMA, tile_bytes=20480, stages=6, warps=2),
            dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=2, warps=1), dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=9, warps=1),
-           dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=17), dict(variant=7)]
+           dict(variant=bs.VARIANT_TMA, tile_bytes=16384, stages=3, warps=17), dict(variant=7),
+           # the named switches (round 3; they used to ride in bs_opts.reserved[], where garbage could not be refused)
+           dict(variant=bs.VARIANT_TMA, fuse=3), dict(variant=bs.VARIANT_TMA, tune=0x4), dict(variant=bs.VARIANT_TMA, tune=0x80000010),
+           dict(variant=bs.VARIANT_LDG, tile_bytes=16384, tune=0x2000)]
     for o in bad:
         with pytest.raises(bs.BsError) as e:
             bs.serialize(d, 256, 1024, 256, 1 << 20, 0, o)
